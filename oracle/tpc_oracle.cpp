@@ -1,0 +1,613 @@
+/*
+ * tpc_oracle.cpp -- CPU ORACLE for the TPC sector-tracker hot path.  TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may load this.
+ * It shares no code, header, table or helper with the CUDA path (paper_1712_09416_b200/csrc) and neither
+ * includes the other.  Plain, slow, scalar: every neighbour / candidate search is a linear scan of the row.
+ *
+ * What the path is: "our TPC tracker ... bases on a Cellular Automaton and on the Kalman filter"
+ * (abstract; section 2).  PAPER.md gives no equation for it; the step list is
+ * BASELINE.json:5 (north_star): neighbour finding between adjacent pad rows, neighbour cleaning, start-hit
+ * selection, Kalman-filter tracklet construction with state (y, z, sin phi, tg lambda, q/pT) in sector-local
+ * coordinates, tracklet selection resolving shared hits.  Every detail below is the reading O1..O7 of
+ * SURVEY.md 8(c).2, restated with its formulas in DESIGN.md "The method, step by step"; this is an
+ * algorithm (a heuristic plus an extended-Kalman iteration), so the oracle follows it step by step.
+ *
+ * Precision: template<real>.  real = double is the reference arithmetic (pins, margins).  real = float is
+ * the strict-float32 mode: BASELINE.json:5 fixes float32 for the fit, and wherever floating point decides an
+ * integer (a link, a gate, an arg min) both sides must decide in the same precision; in that mode every
+ * expression is evaluated exactly as parenthesised here, IEEE round-to-nearest, no contraction
+ * (compile with -ffp-contract=off), only + - * / sqrt.
+ *
+ * Pins (tests/test_oracle_*.py, -m "not gpu"): O2 against an independent brute-force triplet search and the
+ * mirror symmetry; O3/O4 invariants; transport against the closed-form helix and its Jacobian against central
+ * differences; fit against the textbook straight-line least squares (Bz -> 0), against noise-free helices,
+ * pulls / chi2 per ndf / Gluckstern curvature resolution with noise; O6 ownership invariants and a brute-force
+ * owner; end-to-end efficiency on generated events.
+ * PARITY UNPINNED: the exact link / track values on the BASELINE.json configs have no outside reference
+ * (the paper prints none); they are pinned only through the properties above.
+ */
+#include <algorithm>
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <limits>
+#include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+extern "C" {
+/* The oracle's own parameter block (same fields as the boundary's tpc_params, declared independently). */
+typedef struct {
+    int32_t link_step;          /* Delta: neighbour rows r +- Delta (1 or 2) */
+    float nf_slope_y, nf_slope_z; /* T_y, T_z: window half width = T*|dx| + w0 */
+    float nf_w0;                /* cm */
+    float nf_dmax;              /* D_max cm^2 */
+    float sin_max;              /* s_max: transport fails beyond */
+    float var_s, var_t, var_q;  /* prior variances V_s, V_t, V_q */
+    float chi2_link, chi2_ext;  /* 2-dof gates */
+    float win_nsigma, win_min, win_max; /* search window n_w, w_min, w_max */
+    int32_t max_gap;            /* rows without a hit before a pass ends */
+    float edge_margin;          /* cm beyond the wedge before a pass ends */
+    int32_t min_tracklet_hits, min_track_hits;
+} oracle_params;
+
+typedef struct {
+    int32_t n_sectors, n_rows;
+    const float* row_x;         /* [n_rows] */
+    float tan_half_angle;
+    float sigma_y, sigma_z;
+    float bz;
+} oracle_geometry;
+}
+
+namespace {
+
+constexpr double kLight = 0.00299792458; /* cm^-1 GeV T^-1 */
+constexpr double kTiny = 1e-30;
+
+/* smallest relative margin of all float decisions taken for one unit (a hit in O2, a tracklet in O5) */
+struct Margin {
+    double m = std::numeric_limits<double>::infinity();
+    void rel(double a, double b) {
+        double d = std::fabs(a - b) / std::max(std::max(std::fabs(a), std::fabs(b)), kTiny);
+        if (d < m) m = d;
+    }
+};
+template <class R> inline bool le(R a, R b, Margin& mg) { mg.rel((double)a, (double)b); return a <= b; }
+template <class R> inline bool gt(R a, R b, Margin& mg) { mg.rel((double)a, (double)b); return a > b; }
+
+template <class R> struct Fit {
+    R y, z, s, t, q;   /* state at x: y, z, sin phi, dz/dS = tg lambda, q/pT */
+    R C[5][5];         /* symmetric covariance */
+    R chi2;
+    int n;             /* hits in the fit */
+};
+
+struct Tracklet {
+    int32_t first_row = -1, last_row = -1, n_hits = 0;
+    double par[5] = {0, 0, 0, 0, 0};
+    double cov[5] = {0, 0, 0, 0, 0}; /* diagonal of the covariance at x_ref */
+    double chi2 = 0;
+    double margin = std::numeric_limits<double>::infinity();
+    std::vector<int32_t> table; /* [n_rows] event-local hit index or -1 */
+};
+
+struct Result {
+    int32_t n_clusters = 0, n_sectors = 0, n_rows = 0;
+    std::vector<int32_t> link_up, link_dn, clink_up, clink_dn; /* [N] event-local index of the neighbour */
+    std::vector<double> nf_margin;                              /* [N] */
+    std::vector<int32_t> seed_offset;                           /* [n_sectors+1] */
+    std::vector<int32_t> start_hit;                             /* [S] canonical order */
+    std::vector<Tracklet> tracklets;                            /* [S] */
+    /* tracks */
+    std::vector<int32_t> trk_sector, trk_first_hit, trk_n_hits, trk_ndf, trk_seed, trk_first_row;
+    std::vector<double> trk_x, trk_y, trk_z, trk_sinphi, trk_tgl, trk_qpt, trk_chi2, trk_margin;
+    std::vector<int32_t> hit_idx;
+};
+
+template <class R> struct Sector {
+    const oracle_params& P;
+    const oracle_geometry& G;
+    const float *gy, *gz;  /* event arrays */
+    const int32_t* grow;
+    int n_rows;
+    R kB;                  /* kappa = kB * q */
+    std::vector<R> X;      /* row_x as real */
+    std::vector<std::vector<int32_t>> rows; /* O1: hits of each row, ascending original index */
+
+    Sector(const oracle_params& p, const oracle_geometry& g, const float* y, const float* z, const int32_t* row)
+        : P(p), G(g), gy(y), gz(z), grow(row), n_rows(g.n_rows) {
+        kB = R(-1) * (R(kLight) * R(g.bz)); /* kB = -K*Bz */
+        X.resize(n_rows);
+        for (int r = 0; r < n_rows; r++) X[r] = R(g.row_x[r]);
+        rows.resize(n_rows);
+    }
+
+    /* ---- O1 bucket ---- */
+    void bucket(int32_t begin, int32_t end) {
+        for (int32_t h = begin; h < end; h++) rows[grow[h]].push_back(h);
+    }
+
+    /* ---- O2 neighbour finder: best (up, down) pair by straight-line deviation ---- */
+    void neighbours(Result& res) {
+        const int D = P.link_step;
+        const R Ty = R(P.nf_slope_y), Tz = R(P.nf_slope_z), w0 = R(P.nf_w0), Dmax = R(P.nf_dmax);
+        std::vector<int32_t> U, Dn;
+        for (int r = 0; r < n_rows; r++) {
+            if (r - D < 0 || r + D >= n_rows) continue;
+            const R x0 = X[r], x1 = X[r + D], x2 = X[r - D];
+            const R wyu = Ty * std::fabs(x1 - x0) + w0, wzu = Tz * std::fabs(x1 - x0) + w0;
+            const R wyd = Ty * std::fabs(x2 - x0) + w0, wzd = Tz * std::fabs(x2 - x0) + w0;
+            const R a = (x0 - x2) / (x1 - x2);
+            for (int32_t h : rows[r]) {
+                Margin mg;
+                const R y0 = R(gy[h]), z0 = R(gz[h]);
+                U.clear(); Dn.clear();
+                for (int32_t u : rows[r + D]) {
+                    bool iy = le(std::fabs(R(gy[u]) - y0), wyu, mg);
+                    bool iz = le(std::fabs(R(gz[u]) - z0), wzu, mg);
+                    if (iy && iz) U.push_back(u);
+                }
+                for (int32_t d : rows[r - D]) {
+                    bool iy = le(std::fabs(R(gy[d]) - y0), wyd, mg);
+                    bool iz = le(std::fabs(R(gz[d]) - z0), wzd, mg);
+                    if (iy && iz) Dn.push_back(d);
+                }
+                int32_t bu = -1, bd = -1;
+                R best = 0, second = 0;
+                bool have = false, have2 = false;
+                for (int32_t u : U)          /* ascending u, then ascending d: strict < keeps the lowest pair */
+                    for (int32_t d : Dn) {
+                        const R yd = R(gy[d]), zd = R(gz[d]);
+                        const R yh = yd + a * (R(gy[u]) - yd);
+                        const R zh = zd + a * (R(gz[u]) - zd);
+                        const R dy = y0 - yh, dz = z0 - zh;
+                        const R dev = dy * dy + dz * dz;
+                        if (!have || dev < best) {
+                            if (have) { second = best; have2 = true; }
+                            best = dev; bu = u; bd = d; have = true;
+                        } else if (!have2 || dev < second) { second = dev; have2 = true; }
+                    }
+                if (have2) mg.rel((double)best, (double)second);
+                if (have && le(best, Dmax, mg)) { res.link_up[h] = bu; res.link_dn[h] = bd; }
+                res.nf_margin[h] = mg.m;
+            }
+        }
+    }
+
+    /* ---- O3 cleaner: keep reciprocal links only (one simultaneous pass) ---- */
+    void clean(Result& res, int32_t begin, int32_t end) {
+        for (int32_t h = begin; h < end; h++) {
+            const int32_t u = res.link_up[h], d = res.link_dn[h];
+            res.clink_up[h] = (u >= 0 && res.link_dn[u] == h) ? u : -1;
+            res.clink_dn[h] = (d >= 0 && res.link_up[d] == h) ? d : -1;
+        }
+    }
+
+    /* ---- O4 start hits, ordered by (row, original index) ---- */
+    void start_hits(const Result& res, std::vector<int32_t>& out) {
+        for (int r = 0; r < n_rows; r++)
+            for (int32_t h : rows[r])
+                if (res.clink_up[h] >= 0 && res.clink_dn[h] < 0) out.push_back(h);
+    }
+
+    /* ---- O5 helpers ---- */
+    void prior(Fit<R>& f) const {
+        for (int i = 0; i < 5; i++) for (int j = 0; j < 5; j++) f.C[i][j] = R(0);
+        f.C[0][0] = R(G.sigma_y) * R(G.sigma_y);
+        f.C[1][1] = R(G.sigma_z) * R(G.sigma_z);
+        f.C[2][2] = R(P.var_s); f.C[3][3] = R(P.var_t); f.C[4][4] = R(P.var_q);
+        f.chi2 = R(0);
+    }
+
+    /* move the fit from x to x1 along the helix; false (fit untouched) if |sin phi| exceeds s_max at either end
+       (an update can push sin phi itself past the limit, and sqrt(1 - s^2) must stay real) */
+    bool transport(Fit<R>& f, R x, R x1, Margin& mg) const {
+        const R dx = x1 - x;
+        const R kap = kB * f.q;
+        const R s = f.s, s1 = s + kap * dx;
+        if (gt(std::fabs(s), R(P.sin_max), mg)) return false;
+        if (gt(std::fabs(s1), R(P.sin_max), mg)) return false;
+        const R c0 = std::sqrt(R(1) - s * s), c1 = std::sqrt(R(1) - s1 * s1);
+        const R icc = R(1) / (c0 + c1), ic0 = R(1) / c0, ic1 = R(1) / c1;
+        const R dy = dx * ((s + s1) * icc);
+        const R dl2 = dx * dx + dy * dy;
+        const R dl = (dx < R(0)) ? -std::sqrt(dl2) : std::sqrt(dl2); /* signed chord */
+        const R idl = R(1) / dl;
+        const R u = kap * dl, u2 = u * u;
+        const R c24 = R(1) / R(24), c640 = R(3) / R(640), c12 = R(1) / R(12);
+        const R dS = dl * (R(1) + u2 * (c24 + u2 * c640)); /* arc from chord, series of (2/k) asin(k dl/2) */
+        const R ccd = R(1) + (c0 * c1 + s * s1);
+        /* Jacobian, rows (y z s t q); identity elsewhere */
+        const R Fys = dx * ccd * icc * ic0 * ic1;
+        const R Fyq = kB * (dx * dx) * ccd * ic1 * icc * icc;
+        const R Fzs = f.t * dy * ic0 * ic1;
+        const R Fzt = dS;
+        const R Fzq = f.t * ((dy * idl) * Fyq + (kB * kap) * (dl * dl2) * c12);
+        const R Fsq = kB * dx;
+        R F[5][5];
+        for (int i = 0; i < 5; i++) for (int j = 0; j < 5; j++) F[i][j] = (i == j) ? R(1) : R(0);
+        F[0][2] = Fys; F[0][4] = Fyq; F[1][2] = Fzs; F[1][3] = Fzt; F[1][4] = Fzq; F[2][4] = Fsq;
+        f.y = f.y + dy; f.z = f.z + f.t * dS; f.s = s1;
+        /* C <- F C F^T : M = F C (k ascending), then lower triangle of M F^T (l ascending), mirrored */
+        R M[5][5];
+        for (int i = 0; i < 5; i++)
+            for (int l = 0; l < 5; l++) {
+                R acc = R(0);
+                for (int k = 0; k < 5; k++) acc = acc + F[i][k] * f.C[k][l];
+                M[i][l] = acc;
+            }
+        for (int i = 0; i < 5; i++)
+            for (int j = 0; j <= i; j++) {
+                R acc = R(0);
+                for (int l = 0; l < 5; l++) acc = acc + M[i][l] * F[j][l];
+                f.C[i][j] = acc; f.C[j][i] = acc;
+            }
+        return true;
+    }
+
+    /* gate value of a measurement against the predicted state (both variances from the pre-update C) */
+    R gate(const Fit<R>& f, R my, R mz) const {
+        const R ry = my - f.y, rz = mz - f.z;
+        const R wy = R(1) / (f.C[0][0] + R(G.sigma_y) * R(G.sigma_y));
+        const R wz = R(1) / (f.C[1][1] + R(G.sigma_z) * R(G.sigma_z));
+        return (ry * ry) * wy + (rz * rz) * wz;
+    }
+
+    /* one scalar Kalman update with measurement m of state component k (0 = y, 1 = z) */
+    void update1(Fit<R>& f, int k, R m, R var) const {
+        R* x[5] = {&f.y, &f.z, &f.s, &f.t, &f.q};
+        const R r = m - *x[k];
+        const R w = R(1) / (f.C[k][k] + var);
+        R ck[5], K[5];
+        for (int j = 0; j < 5; j++) { ck[j] = f.C[j][k]; K[j] = ck[j] * w; }
+        for (int j = 0; j < 5; j++) *x[j] = *x[j] + K[j] * r;
+        for (int i = 0; i < 5; i++)
+            for (int j = 0; j <= i; j++) {
+                const R v = f.C[i][j] - K[i] * ck[j];
+                f.C[i][j] = v; f.C[j][i] = v;
+            }
+        f.chi2 = f.chi2 + (r * r) * w;
+    }
+    void update(Fit<R>& f, int32_t h) const {
+        update1(f, 0, R(gy[h]), R(G.sigma_y) * R(G.sigma_y));
+        update1(f, 1, R(gz[h]), R(G.sigma_z) * R(G.sigma_z));
+        f.n++;
+    }
+
+    /* best hit of a row inside the window of the predicted state; -1 if none passes chi2_ext */
+    int32_t search(const Fit<R>& f, int row, Margin& mg) const {
+        const R sy2 = R(G.sigma_y) * R(G.sigma_y), sz2 = R(G.sigma_z) * R(G.sigma_z);
+        const R wy = std::min(std::max(R(P.win_nsigma) * std::sqrt(f.C[0][0] + sy2), R(P.win_min)), R(P.win_max));
+        const R wz = std::min(std::max(R(P.win_nsigma) * std::sqrt(f.C[1][1] + sz2), R(P.win_min)), R(P.win_max));
+        int32_t best = -1;
+        R gb = 0, g2 = 0;
+        bool have2 = false;
+        for (int32_t c : rows[row]) {
+            bool iy = le(std::fabs(R(gy[c]) - f.y), wy, mg);
+            bool iz = le(std::fabs(R(gz[c]) - f.z), wz, mg);
+            if (!(iy && iz)) continue;
+            const R g = gate(f, R(gy[c]), R(gz[c]));
+            if (best < 0 || g < gb) {
+                if (best >= 0) { g2 = gb; have2 = true; }
+                gb = g; best = c;
+            } else if (!have2 || g < g2) { g2 = g; have2 = true; }
+        }
+        if (best < 0) return -1;
+        if (have2) mg.rel((double)gb, (double)g2);
+        return le(gb, R(P.chi2_ext), mg) ? best : -1;
+    }
+
+    /* ---- O5 tracklet constructor for the start hit h0 ---- */
+    void construct(const Result& res, int32_t h0, Tracklet& T) const {
+        Margin mg;
+        std::vector<int32_t>& tab = T.table;
+        tab.assign(n_rows, -1);
+        const int r0 = grow[h0];
+        const int32_t h1 = res.clink_up[h0];
+        Fit<R> f, snap;
+        {   /* initial state from the first link */
+            const R dx = X[grow[h1]] - X[r0];
+            const R dy = R(gy[h1]) - R(gy[h0]), dz = R(gz[h1]) - R(gz[h0]);
+            const R dl = std::sqrt(dx * dx + dy * dy);
+            f.y = R(gy[h0]); f.z = R(gz[h0]); f.s = dy / dl; f.t = dz / dl; f.q = R(0);
+            prior(f); f.n = 1;
+        }
+        tab[r0] = h0;
+        snap = f;
+        int top = r0;
+        /* up pass */
+        {
+            bool follow = true;
+            int32_t cur = h1;
+            int miss = 0;
+            R xc = X[r0];
+            for (int row = r0 + 1; row < n_rows; row++) {
+                if (!transport(f, xc, X[row], mg)) break;
+                xc = X[row];
+                if (follow) {
+                    if (row < grow[cur]) continue;
+                    if (le(gate(f, R(gy[cur]), R(gz[cur])), R(P.chi2_link), mg)) {
+                        update(f, cur); tab[row] = cur; snap = f; top = row;
+                        cur = res.clink_up[cur];
+                        if (cur < 0) follow = false;
+                        continue;
+                    }
+                    follow = false; /* fall through: search this same row */
+                }
+                if (gt(std::fabs(f.y), X[row] * R(G.tan_half_angle) + R(P.edge_margin), mg)) break;
+                const int32_t c = search(f, row, mg);
+                if (c >= 0) { update(f, c); tab[row] = c; snap = f; top = row; miss = 0; }
+                else if (++miss > P.max_gap) break;
+            }
+        }
+        /* down pass: fresh fit from the top recorded hit, direction and curvature from the up pass */
+        int first = top;
+        {
+            const int32_t ht = tab[top];
+            f.y = R(gy[ht]); f.z = R(gz[ht]); f.s = snap.s; f.t = snap.t; f.q = snap.q;
+            prior(f); f.n = 1;
+            snap = f;
+            int miss = 0;
+            R xc = X[top];
+            int row = top - 1;
+            for (; row >= 0; row--) {
+                if (!transport(f, xc, X[row], mg)) break;
+                xc = X[row];
+                const int32_t hr = tab[row];
+                if (hr >= 0) {
+                    if (le(gate(f, R(gy[hr]), R(gz[hr])), R(P.chi2_link), mg)) { update(f, hr); snap = f; first = row; }
+                    else tab[row] = -1;
+                    continue;
+                }
+                const bool below = row < r0;
+                if (below && gt(std::fabs(f.y), X[row] * R(G.tan_half_angle) + R(P.edge_margin), mg)) break;
+                const int32_t c = search(f, row, mg);
+                if (c >= 0) { update(f, c); tab[row] = c; snap = f; first = row; miss = 0; }
+                else if (below && ++miss > P.max_gap) break;
+            }
+            for (; row >= 0; row--) tab[row] = -1; /* rows the pass never reached keep nothing */
+        }
+        T.first_row = first; T.last_row = top; T.n_hits = snap.n;
+        T.par[0] = (double)snap.y; T.par[1] = (double)snap.z; T.par[2] = (double)snap.s;
+        T.par[3] = (double)snap.t; T.par[4] = (double)snap.q;
+        for (int i = 0; i < 5; i++) T.cov[i] = (double)snap.C[i][i];
+        T.chi2 = (double)snap.chi2;
+        T.margin = mg.m;
+    }
+};
+
+template <class R>
+Result* run(const oracle_geometry& G, const oracle_params& P, int32_t n, const int32_t* sector_offset, const float* y,
+            const float* z, const int32_t* row, int n_threads, int stop_after) {
+    Result* res = new Result;
+    res->n_clusters = n; res->n_sectors = G.n_sectors; res->n_rows = G.n_rows;
+    res->link_up.assign(n, -1); res->link_dn.assign(n, -1);
+    res->clink_up.assign(n, -1); res->clink_dn.assign(n, -1);
+    res->nf_margin.assign(n, std::numeric_limits<double>::infinity());
+    const int ns = G.n_sectors;
+    std::vector<std::vector<int32_t>> seeds(ns);
+    std::vector<std::vector<Tracklet>> tls(ns);
+    /* per-sector output tracks */
+    struct Out { std::vector<int32_t> seed, nh, first_row; std::vector<std::vector<int32_t>> hits; };
+    std::vector<Out> outs(ns);
+#ifdef _OPENMP
+    if (n_threads > 0) omp_set_num_threads(n_threads);
+#endif
+#pragma omp parallel for schedule(dynamic, 1)
+    for (int s = 0; s < ns; s++) {
+        Sector<R> S(P, G, y, z, row);
+        const int32_t b = sector_offset[s], e = sector_offset[s + 1];
+        S.bucket(b, e);
+        S.neighbours(*res);
+        if (stop_after == 2) continue;
+        S.clean(*res, b, e);
+        S.start_hits(*res, seeds[s]);
+        if (stop_after == 4) continue;
+        tls[s].resize(seeds[s].size());
+        for (size_t i = 0; i < seeds[s].size(); i++) S.construct(*res, seeds[s][i], tls[s][i]);
+        if (stop_after == 5) continue;
+        /* ---- O6 selector ---- */
+        /* owner(hit) = tracklet with most hits, ties -> lowest canonical id, among tracklets with
+           n_hits >= min_tracklet_hits whose table contains the hit */
+        std::vector<int32_t> owner(e - b, -1);
+        for (size_t i = 0; i < tls[s].size(); i++) {
+            const Tracklet& T = tls[s][i];
+            if (T.n_hits < P.min_tracklet_hits) continue;
+            for (int r = 0; r < G.n_rows; r++) {
+                const int32_t h = T.table[r];
+                if (h < 0) continue;
+                int32_t& o = owner[h - b];
+                if (o < 0 || T.n_hits > tls[s][o].n_hits) o = (int32_t)i; /* ascending i: ties keep the lower id */
+            }
+        }
+        for (size_t i = 0; i < tls[s].size(); i++) {
+            const Tracklet& T = tls[s][i];
+            if (T.n_hits < P.min_tracklet_hits) continue;
+            std::vector<int32_t> hits;
+            for (int r = 0; r < G.n_rows; r++) {
+                const int32_t h = T.table[r];
+                if (h >= 0 && owner[h - b] == (int32_t)i) hits.push_back(h);
+            }
+            if ((int)hits.size() < P.min_track_hits) continue;
+            outs[s].seed.push_back((int32_t)i);
+            outs[s].nh.push_back((int32_t)hits.size());
+            outs[s].first_row.push_back(T.first_row);
+            outs[s].hits.push_back(std::move(hits));
+        }
+    }
+    /* ---- O7 output in canonical order (sector, start row, start-hit index) ---- */
+    res->seed_offset.assign(ns + 1, 0);
+    for (int s = 0; s < ns; s++) res->seed_offset[s + 1] = res->seed_offset[s] + (int32_t)seeds[s].size();
+    for (int s = 0; s < ns; s++) {
+        for (int32_t h : seeds[s]) res->start_hit.push_back(h);
+        for (auto& T : tls[s]) res->tracklets.push_back(std::move(T));
+    }
+    for (int s = 0; s < ns; s++) {
+        for (size_t k = 0; k < outs[s].seed.size(); k++) {
+            const int32_t gid = res->seed_offset[s] + outs[s].seed[k];
+            const Tracklet& T = res->tracklets[gid];
+            res->trk_sector.push_back(s);
+            res->trk_seed.push_back(gid);
+            res->trk_first_hit.push_back((int32_t)res->hit_idx.size());
+            res->trk_n_hits.push_back(outs[s].nh[k]);
+            res->trk_ndf.push_back(2 * T.n_hits - 5);
+            res->trk_first_row.push_back(T.first_row);
+            res->trk_x.push_back((double)G.row_x[T.first_row]);
+            res->trk_y.push_back(T.par[0]); res->trk_z.push_back(T.par[1]); res->trk_sinphi.push_back(T.par[2]);
+            res->trk_tgl.push_back(T.par[3]); res->trk_qpt.push_back(T.par[4]);
+            res->trk_chi2.push_back(T.chi2); res->trk_margin.push_back(T.margin);
+            for (int32_t h : outs[s].hits[k]) res->hit_idx.push_back(h);
+        }
+    }
+    return res;
+}
+
+template <class T> void copy_out(const std::vector<T>& v, void* dst) {
+    if (!v.empty()) std::memcpy(dst, v.data(), sizeof(T) * v.size());
+}
+
+} /* namespace */
+
+extern "C" {
+
+void oracle_default_params(oracle_params* p) {
+    /* defaults of SURVEY.md 8(c).3 (validated by tests/test_oracle_e2e.py) */
+    p->link_step = 1;
+    p->nf_slope_y = 1.5f; p->nf_slope_z = 2.0f; p->nf_w0 = 0.3f; p->nf_dmax = 0.25f;
+    p->sin_max = 0.95f;
+    p->var_s = 0.25f; p->var_t = 1.0f; p->var_q = 100.0f;
+    p->chi2_link = 25.0f; p->chi2_ext = 16.0f;
+    p->win_nsigma = 4.0f; p->win_min = 0.3f; p->win_max = 3.0f;
+    p->max_gap = 5; p->edge_margin = 1.0f;
+    p->min_tracklet_hits = 10; p->min_track_hits = 10;
+}
+
+/* precision: 0 = double, 1 = strict float32.  stop_after: 0 = everything, 2 = after O2, 4 = after O4,
+ * 5 = after O5.  Returns an opaque result (oracle_free). */
+void* oracle_track_event(const oracle_geometry* G, const oracle_params* P, int32_t precision, int32_t n_clusters,
+                         const int32_t* sector_offset, const float* y, const float* z, const int32_t* row,
+                         int32_t n_threads, int32_t stop_after) {
+    if (!G || !P || !sector_offset || G->n_rows <= 0 || G->n_sectors <= 0) return nullptr;
+    if (P->link_step < 1 || P->link_step > 2) return nullptr;
+    for (int32_t i = 0; i < n_clusters; i++)
+        if (row[i] < 0 || row[i] >= G->n_rows) return nullptr;
+    if (precision == 1) return run<float>(*G, *P, n_clusters, sector_offset, y, z, row, n_threads, stop_after);
+    return run<double>(*G, *P, n_clusters, sector_offset, y, z, row, n_threads, stop_after);
+}
+
+void oracle_free(void* r) { delete static_cast<Result*>(r); }
+
+/* sizes: [n_clusters, n_seeds, n_tracks, n_track_hits, n_rows] */
+void oracle_sizes(const void* rv, int64_t* out) {
+    const Result* r = static_cast<const Result*>(rv);
+    out[0] = r->n_clusters; out[1] = (int64_t)r->start_hit.size(); out[2] = (int64_t)r->trk_sector.size();
+    out[3] = (int64_t)r->hit_idx.size(); out[4] = r->n_rows;
+}
+
+enum {
+    F_LINK_UP = 0, F_LINK_DN, F_CLINK_UP, F_CLINK_DN, F_NF_MARGIN, F_SEED_OFFSET, F_START_HIT,
+    F_TL_FIRST_ROW, F_TL_LAST_ROW, F_TL_N_HITS, F_TL_PAR, F_TL_CHI2, F_TL_MARGIN, F_TL_TABLE,
+    F_TRK_SECTOR, F_TRK_FIRST_HIT, F_TRK_N_HITS, F_TRK_NDF, F_TRK_SEED, F_TRK_FIRST_ROW,
+    F_TRK_X, F_TRK_Y, F_TRK_Z, F_TRK_SINPHI, F_TRK_TGL, F_TRK_QPT, F_TRK_CHI2, F_TRK_MARGIN, F_HIT_IDX, F_TL_COV
+};
+
+/* copy one result field into caller memory (int32 or float64, shapes in oracle/__init__.py) */
+int32_t oracle_copy(const void* rv, int32_t field, void* dst) {
+    const Result* r = static_cast<const Result*>(rv);
+    const size_t S = r->tracklets.size();
+    switch (field) {
+        case F_LINK_UP: copy_out(r->link_up, dst); break;
+        case F_LINK_DN: copy_out(r->link_dn, dst); break;
+        case F_CLINK_UP: copy_out(r->clink_up, dst); break;
+        case F_CLINK_DN: copy_out(r->clink_dn, dst); break;
+        case F_NF_MARGIN: copy_out(r->nf_margin, dst); break;
+        case F_SEED_OFFSET: copy_out(r->seed_offset, dst); break;
+        case F_START_HIT: copy_out(r->start_hit, dst); break;
+        case F_TL_FIRST_ROW: for (size_t i = 0; i < S; i++) ((int32_t*)dst)[i] = r->tracklets[i].first_row; break;
+        case F_TL_LAST_ROW: for (size_t i = 0; i < S; i++) ((int32_t*)dst)[i] = r->tracklets[i].last_row; break;
+        case F_TL_N_HITS: for (size_t i = 0; i < S; i++) ((int32_t*)dst)[i] = r->tracklets[i].n_hits; break;
+        case F_TL_PAR: for (size_t i = 0; i < S; i++) std::memcpy((double*)dst + 5 * i, r->tracklets[i].par, 40); break;
+        case F_TL_COV: for (size_t i = 0; i < S; i++) std::memcpy((double*)dst + 5 * i, r->tracklets[i].cov, 40); break;
+        case F_TL_CHI2: for (size_t i = 0; i < S; i++) ((double*)dst)[i] = r->tracklets[i].chi2; break;
+        case F_TL_MARGIN: for (size_t i = 0; i < S; i++) ((double*)dst)[i] = r->tracklets[i].margin; break;
+        case F_TL_TABLE:
+            for (size_t i = 0; i < S; i++)
+                if (!r->tracklets[i].table.empty())
+                    std::memcpy((int32_t*)dst + (size_t)r->n_rows * i, r->tracklets[i].table.data(), 4 * (size_t)r->n_rows);
+            break;
+        case F_TRK_SECTOR: copy_out(r->trk_sector, dst); break;
+        case F_TRK_FIRST_HIT: copy_out(r->trk_first_hit, dst); break;
+        case F_TRK_N_HITS: copy_out(r->trk_n_hits, dst); break;
+        case F_TRK_NDF: copy_out(r->trk_ndf, dst); break;
+        case F_TRK_SEED: copy_out(r->trk_seed, dst); break;
+        case F_TRK_FIRST_ROW: copy_out(r->trk_first_row, dst); break;
+        case F_TRK_X: copy_out(r->trk_x, dst); break;
+        case F_TRK_Y: copy_out(r->trk_y, dst); break;
+        case F_TRK_Z: copy_out(r->trk_z, dst); break;
+        case F_TRK_SINPHI: copy_out(r->trk_sinphi, dst); break;
+        case F_TRK_TGL: copy_out(r->trk_tgl, dst); break;
+        case F_TRK_QPT: copy_out(r->trk_qpt, dst); break;
+        case F_TRK_CHI2: copy_out(r->trk_chi2, dst); break;
+        case F_TRK_MARGIN: copy_out(r->trk_margin, dst); break;
+        case F_HIT_IDX: copy_out(r->hit_idx, dst); break;
+        default: return -1;
+    }
+    return 0;
+}
+
+/* ---- single-step entry points for the pins (double and float) ---- */
+/* state: [y z s t q], cov: 25 row-major.  Returns 0 ok, 1 transport failed. */
+int32_t oracle_transport(const oracle_geometry* G, const oracle_params* P, int32_t precision, double x, double x1,
+                         double* state, double* cov) {
+    oracle_geometry g = *G;
+    float rx[1] = {0.f};
+    g.n_rows = 1; g.row_x = rx;
+    Margin mg;
+    if (precision == 1) {
+        Sector<float> S(*P, g, nullptr, nullptr, nullptr);
+        Fit<float> f;
+        f.y = (float)state[0]; f.z = (float)state[1]; f.s = (float)state[2]; f.t = (float)state[3]; f.q = (float)state[4];
+        for (int i = 0; i < 5; i++) for (int j = 0; j < 5; j++) f.C[i][j] = (float)cov[5 * i + j];
+        if (!S.transport(f, (float)x, (float)x1, mg)) return 1;
+        state[0] = f.y; state[1] = f.z; state[2] = f.s; state[3] = f.t; state[4] = f.q;
+        for (int i = 0; i < 5; i++) for (int j = 0; j < 5; j++) cov[5 * i + j] = f.C[i][j];
+    } else {
+        Sector<double> S(*P, g, nullptr, nullptr, nullptr);
+        Fit<double> f;
+        f.y = state[0]; f.z = state[1]; f.s = state[2]; f.t = state[3]; f.q = state[4];
+        for (int i = 0; i < 5; i++) for (int j = 0; j < 5; j++) f.C[i][j] = cov[5 * i + j];
+        if (!S.transport(f, x, x1, mg)) return 1;
+        state[0] = f.y; state[1] = f.z; state[2] = f.s; state[3] = f.t; state[4] = f.q;
+        for (int i = 0; i < 5; i++) for (int j = 0; j < 5; j++) cov[5 * i + j] = f.C[i][j];
+    }
+    return 0;
+}
+
+/* one measurement update (y then z) in double; chi2 in/out */
+void oracle_update(const oracle_geometry* G, const oracle_params* P, double my, double mz, double* state, double* cov,
+                   double* chi2) {
+    oracle_geometry g = *G;
+    float rx[1] = {0.f};
+    g.n_rows = 1; g.row_x = rx;
+    Sector<double> S(*P, g, nullptr, nullptr, nullptr);
+    Fit<double> f;
+    f.y = state[0]; f.z = state[1]; f.s = state[2]; f.t = state[3]; f.q = state[4]; f.chi2 = *chi2; f.n = 0;
+    for (int i = 0; i < 5; i++) for (int j = 0; j < 5; j++) f.C[i][j] = cov[5 * i + j];
+    S.update1(f, 0, my, (double)G->sigma_y * (double)G->sigma_y);
+    S.update1(f, 1, mz, (double)G->sigma_z * (double)G->sigma_z);
+    state[0] = f.y; state[1] = f.z; state[2] = f.s; state[3] = f.t; state[4] = f.q; *chi2 = f.chi2;
+    for (int i = 0; i < 5; i++) for (int j = 0; j < 5; j++) cov[5 * i + j] = f.C[i][j];
+}
+
+int32_t oracle_max_threads(void) {
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+} /* extern "C" */
