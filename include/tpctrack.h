@@ -1,0 +1,167 @@
+/*
+ * tpctrack.h -- C ABI of libtpctrack.so: the data-parallel hot path of the ALICE HLT TPC sector tracker
+ * (arxiv 1712.09416) on one NVIDIA B200 (sm_100a).
+ *
+ * What it computes.  "our TPC tracker ... bases on a Cellular Automaton and on the Kalman filter"
+ * (abstract; section 2).  The paper names no further step; the step list is the
+ * contract of BASELINE.json:5: per-row cluster sort + uniform (y,z) grid; Cellular-Automaton neighbour finding
+ * between adjacent pad rows (best up/down pair by straight-line deviation); mutual-link cleaning; start-hit
+ * selection; Kalman-filter tracklet construction (float32 helix fit, state y, z, sin phi, tg lambda, q/pT in
+ * sector-local coordinates); tracklet selection resolving shared hits.  The entry points are the ones that
+ * sentence lists: tpc_tracker_create(geometry, Bz), tpc_track_event(clusters as SoA x,y,z,row -> tracks with hit
+ * lists and helix parameters), tpc_tracker_destroy; plus the batch form for "several events concurrently".
+ * The exact arithmetic of every step is written out in DESIGN.md ("The method, step by step").
+ *
+ * Every step runs in hand-written CUDA kernels; there is no CPU fallback.  Plain C types only.
+ * A tracker is not thread-safe: one per host thread.  No exception crosses this boundary.
+ */
+#ifndef TPCTRACK_H
+#define TPCTRACK_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* ---- status codes (0 = ok, negative = error) ---- */
+#define TPC_OK 0
+#define TPC_ERR_ARG (-1)       /* NULL pointer, bad size, row outside [0,n_rows), non-monotonic sector_offset */
+#define TPC_ERR_GEOMETRY (-2)  /* row_x not strictly increasing, n_rows not in [3,255], n_sectors < 1 */
+#define TPC_ERR_CAPACITY (-3)  /* more than TPC_MAX_ROW_HITS clusters in one (sector,row), or a pool limit */
+#define TPC_ERR_CUDA (-4)      /* a CUDA call failed; tpc_last_error() has the text */
+
+#define TPC_MAX_ROWS 255
+#define TPC_MAX_ROW_HITS 2048  /* clusters per (sector, pad row) */
+
+/* Geometry of the detector (copied at create; host pointers).  Units: cm, Tesla, GeV/c.
+ * Sector-local frame: x along the sector axis (a cluster of pad row r sits at x = row_x[r] exactly), y across,
+ * z along the drift (signed: C-side sectors have z < 0).  BASELINE.json:7: 159 rows, 20 degree wedges. */
+typedef struct {
+    int32_t n_sectors;         /* 36 (or 1): the number of independent sector tasks per event */
+    int32_t n_rows;            /* pad rows per sector, 3..TPC_MAX_ROWS */
+    const float* row_x;        /* [n_rows] host, strictly increasing */
+    float tan_half_angle;      /* tan(10 deg): the wedge is |y| <= row_x * tan_half_angle */
+    float z_abs_max;           /* 250 cm, informational */
+    float sigma_y, sigma_z;    /* cluster errors used by the fit, cm */
+    const float* sector_alpha; /* [n_sectors] host or NULL; echoed only, tracking is sector-local */
+} tpc_geometry;
+
+/* Algorithm parameters (defaults from tpc_default_params). */
+typedef struct {
+    int32_t link_step;          /* Delta: neighbour rows r +- Delta, 1 or 2 */
+    float nf_slope_y, nf_slope_z; /* neighbour window half width = slope * |dx| + nf_w0 */
+    float nf_w0;                /* cm */
+    float nf_dmax;              /* largest accepted straight-line deviation, cm^2 */
+    float sin_max;              /* the helix transport fails beyond |sin phi| = sin_max */
+    float var_s, var_t, var_q;  /* prior variances of sin phi, tg lambda, q/pT */
+    float chi2_link, chi2_ext;  /* 2-dof gates: following a link / attaching a searched hit */
+    float win_nsigma, win_min, win_max; /* search window = clamp(n * sqrt(C + sigma^2), min, max) cm */
+    int32_t max_gap;            /* consecutive rows without a hit before a pass ends */
+    float edge_margin;          /* cm beyond the wedge edge before a pass ends */
+    int32_t min_tracklet_hits;  /* tracklets with fewer hits do not take part in the selection */
+    int32_t min_track_hits;     /* tracks keeping fewer owned hits are dropped */
+} tpc_params;
+
+/* One event's clusters: SoA, grouped by sector, ANY order inside a sector.
+ * mem_space 0: x, y, z, row are host pointers; the call copies them to the device (pinned memory makes the
+ *              copy asynchronous) and the outputs come back in library-owned pinned host memory.
+ * mem_space 1: x, y, z, row are device pointers (must stay valid and unchanged until the call returns); the
+ *              outputs are library-owned device memory.
+ * sector_offset is ALWAYS a host pointer.  x is redundant with row_x[row]: the library reads row and ignores x
+ * (x may be NULL). */
+typedef struct {
+    int32_t n_clusters;
+    const int32_t* sector_offset; /* [n_sectors+1] host, non-decreasing, [0] = 0, [n_sectors] = n_clusters */
+    const float* x;
+    const float* y;
+    const float* z;
+    const int32_t* row;           /* [n_clusters] in [0, n_rows) */
+    int32_t mem_space;
+} tpc_event_in;
+
+/* One event's tracks.  All arrays are library-owned (host or device as the input's mem_space) and valid until
+ * the next tpc_track_event(s) call on this tracker or its destruction.  Tracks come in canonical order
+ * (sector, pad row of the start hit, caller's index of the start hit).  A hit is in at most one track.
+ * Parameters are given at x = trk_x (the pad row of the track's innermost fitted hit). */
+typedef struct {
+    int32_t n_tracks;
+    int32_t n_track_hits;
+    const int32_t* trk_sector;    /* [n_tracks] */
+    const int32_t* trk_first_hit; /* [n_tracks] offset into hit_idx */
+    const int32_t* trk_n_hits;    /* [n_tracks] hits this track owns */
+    const int32_t* trk_ndf;       /* [n_tracks] 2 * (hits in the fit) - 5 */
+    const float* trk_x;           /* [n_tracks] cm */
+    const float* trk_y;
+    const float* trk_z;
+    const float* trk_sinphi;
+    const float* trk_tgl;
+    const float* trk_qpt;         /* 1/(GeV/c), signed */
+    const float* trk_chi2;
+    const int32_t* hit_idx;       /* [n_track_hits] indices into the caller's cluster arrays, row-ascending */
+} tpc_event_out;
+
+/* Counters of the last call (whole batch); used for the algorithmic-byte count of DESIGN.md. */
+typedef struct {
+    int64_t n_events, n_clusters;
+    int64_t n_links;         /* hits with a cleaned up-link */
+    int64_t n_seeds;         /* start hits = tracklets constructed */
+    int64_t n_row_visits;    /* Kalman transport steps taken by the constructor */
+    int64_t n_tracklet_hits; /* hits in tracklets entering the selection */
+    int64_t n_tracks, n_track_hits;
+    int64_t n_kernel_launches; /* kernels this library launched during the call */
+    int64_t n_retries;       /* internal re-runs after growing a pool */
+} tpc_counters;
+
+typedef struct tpc_tracker tpc_tracker;
+
+/* Fill *p with the defaults. */
+void tpc_default_params(tpc_params* p);
+
+/* Create a tracker for the given geometry and solenoid field Bz (Tesla, signed).  Default parameters; work
+ * space grows on demand.  Returns NULL on failure (tpc_last_error()). */
+tpc_tracker* tpc_tracker_create(const tpc_geometry* geometry, float bz_tesla);
+
+/* As above with explicit parameters (NULL = defaults) and pre-sized work space: the tracker allocates once
+ * for batches of up to max_events events holding up to max_clusters clusters in total (0 = grow on demand). */
+tpc_tracker* tpc_tracker_create_ex(const tpc_geometry* geometry, float bz_tesla, const tpc_params* params,
+                                   int32_t max_events, int64_t max_clusters);
+
+/* Run all kernels on this CUDA stream (a cudaStream_t; NULL = the tracker's own stream). */
+int tpc_tracker_set_stream(tpc_tracker* t, void* cuda_stream);
+
+/* Track one event.  Synchronous: returns when the outputs are complete.  Zero clusters, empty sectors and
+ * empty rows are legal (0 tracks).  Returns a status code. */
+int tpc_track_event(tpc_tracker* t, const tpc_event_in* in, tpc_event_out* out);
+
+/* Track n independent events in one pass: all n * n_sectors sector tasks go through every kernel together.
+ * in/out are host arrays of n structs; all inputs must share one mem_space. */
+int tpc_track_events(tpc_tracker* t, int32_t n, const tpc_event_in* in, tpc_event_out* out);
+
+void tpc_tracker_destroy(tpc_tracker* t);
+
+const char* tpc_status_string(int status);
+const char* tpc_last_error(void); /* thread-local text of the last failure */
+
+int tpc_get_counters(const tpc_tracker* t, tpc_counters* c);
+
+/* ---- intermediates of the last call, for stage-by-stage parity tests (not part of the hot path) ----
+ * All hit indices are the caller's indices within event `event`; -1 = none.  buf is a HOST buffer of `bytes`
+ * bytes; the call fails with TPC_ERR_ARG if it is too small.  Sizes: tpc_debug_size(). */
+#define TPC_DBG_LINK_UP 0    /* int32 [n_clusters(event)]  neighbour before cleaning */
+#define TPC_DBG_LINK_DN 1
+#define TPC_DBG_CLINK_UP 2   /* int32 [n_clusters(event)]  after cleaning */
+#define TPC_DBG_CLINK_DN 3
+#define TPC_DBG_START_HIT 4  /* int32 [n_seeds(event)]     canonical order */
+#define TPC_DBG_TL_ROWS 5    /* int32 [n_seeds(event)][3]  first_row, last_row, n_hits */
+#define TPC_DBG_TL_PAR 6     /* float [n_seeds(event)][6]  y, z, sin phi, tg lambda, q/pT, chi2 */
+#define TPC_DBG_TL_TABLE 7   /* int32 [n_seeds(event)][n_rows] row -> hit */
+#define TPC_DBG_SORTED 8     /* int32 [n_clusters(event)]  caller's index of each cluster in (sector,row,cell) order */
+int64_t tpc_debug_size(const tpc_tracker* t, int32_t what, int32_t event); /* bytes, or negative status */
+int tpc_debug_get(tpc_tracker* t, int32_t what, int32_t event, void* buf, size_t bytes);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TPCTRACK_H */

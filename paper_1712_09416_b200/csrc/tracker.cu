@@ -1,0 +1,545 @@
+// tracker.cu -- host side of libtpctrack.so: the C ABI of include/tpctrack.h, work-space management and the
+// launch sequence K1..K6 for a batch of events (all n_events * n_sectors sector tasks in every launch).
+#include <algorithm>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "ca_kernels.cuh"
+#include "kf_kernels.cuh"
+
+namespace {
+
+thread_local std::string g_err;
+
+void set_err(const char* fmt, ...) {
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    g_err = buf;
+}
+
+#define CK(call)                                                                       \
+    do {                                                                               \
+        cudaError_t e_ = (call);                                                       \
+        if (e_ != cudaSuccess) {                                                       \
+            set_err("%s failed: %s (%s:%d)", #call, cudaGetErrorString(e_), __FILE__, __LINE__); \
+            return TPC_ERR_CUDA;                                                       \
+        }                                                                              \
+    } while (0)
+
+// a device (or pinned host) array that only ever grows
+template <class T> struct Buf {
+    T* p = nullptr;
+    size_t cap = 0;
+    bool host = false;
+    int reserve(size_t n) {
+        if (n <= cap) return TPC_OK;
+        release();
+        const size_t want = n + n / 8 + 64;
+        cudaError_t e = host ? cudaMallocHost((void**)&p, want * sizeof(T)) : cudaMalloc((void**)&p, want * sizeof(T));
+        if (e != cudaSuccess) {
+            p = nullptr; cap = 0;
+            set_err("allocation of %zu bytes failed: %s", want * sizeof(T), cudaGetErrorString(e));
+            return TPC_ERR_CUDA;
+        }
+        cap = want;
+        return TPC_OK;
+    }
+    void release() {
+        if (p) { if (host) cudaFreeHost(p); else cudaFree(p); }
+        p = nullptr; cap = 0;
+    }
+};
+
+}  // namespace
+
+using namespace tpc;
+
+struct tpc_tracker {
+    Const c;
+    std::vector<float> sector_alpha;
+    cudaStream_t own_stream = nullptr, stream = nullptr;
+    int sm_count = 148;
+    // batch state
+    View v;
+    int n_events = 0;
+    int64_t N = 0;
+    std::vector<int32_t> ev_n, ev_off;       // clusters per event, offset in the batch
+    int mem_space = 1;
+    tpc_counters counters;
+    bool have_result = false;
+    // device pools
+    Buf<float> in_y, in_z, ty, tz, sy, sz, tl_par, o_f[7];
+    Buf<int32_t> in_row, sec_off, bin_count, bin_start, tidx, sorig, link_up, link_dn, clink_up, clink_dn, seed_count,
+        seed_start, seeds, seed_bin, tl_table, tl_rows, tl_nown, tl_keep, trk_scan, hit_scan, ev_off_d, scratch,
+        o_i[4], o_hit;
+    Buf<uint16_t> slot, cells;
+    Buf<float4> grid_f;
+    Buf<int2> grid_n;
+    Buf<uint32_t> owner;
+    Buf<EventSrc> ev_src;
+    Buf<unsigned long long> cnt;
+    // pinned host mirrors
+    Buf<EventSrc> h_ev_src;
+    Buf<int32_t> h_sec_off, h_ev_off, h_o_i[4], h_o_hit;
+    Buf<unsigned long long> h_cnt;
+    Buf<float> h_o_f[7];
+    int64_t S_cap = 0;
+
+    tpc_tracker() {
+        h_ev_src.host = h_sec_off.host = h_ev_off.host = h_cnt.host = h_o_hit.host = true;
+        for (auto& b : h_o_i) b.host = true;
+        for (auto& b : h_o_f) b.host = true;
+        memset(&v, 0, sizeof v);
+        memset(&counters, 0, sizeof counters);
+    }
+    void free_all() {
+        in_y.release(); in_z.release(); ty.release(); tz.release(); sy.release(); sz.release(); tl_par.release();
+        for (auto& b : o_f) b.release();
+        in_row.release(); sec_off.release(); bin_count.release(); bin_start.release(); tidx.release(); sorig.release();
+        link_up.release(); link_dn.release(); clink_up.release(); clink_dn.release(); seed_count.release();
+        seed_start.release(); seeds.release(); seed_bin.release(); tl_table.release(); tl_rows.release();
+        tl_nown.release(); tl_keep.release(); trk_scan.release(); hit_scan.release(); ev_off_d.release();
+        scratch.release(); o_hit.release();
+        for (auto& b : o_i) b.release();
+        slot.release(); cells.release(); grid_f.release(); grid_n.release(); owner.release(); ev_src.release();
+        cnt.release(); h_ev_src.release(); h_sec_off.release(); h_ev_off.release(); h_o_hit.release(); h_cnt.release();
+        for (auto& b : h_o_i) b.release();
+        for (auto& b : h_o_f) b.release();
+    }
+};
+
+namespace {
+
+int reserve_batch(tpc_tracker* t, int n_events, int64_t N, int64_t S_cap) {
+    const int64_t nb = (int64_t)n_events * t->c.n_sectors * t->c.n_rows;
+    const size_t n = (size_t)std::max<int64_t>(N, 1);
+    int rc = TPC_OK;
+#define RS(b, k) if ((rc = t->b.reserve(k)) != TPC_OK) return rc
+    RS(sec_off, (size_t)n_events * (t->c.n_sectors + 1)); RS(h_sec_off, (size_t)n_events * (t->c.n_sectors + 1));
+    RS(ev_src, n_events); RS(h_ev_src, n_events);
+    RS(bin_count, nb + 1); RS(bin_start, nb + 1); RS(seed_count, nb + 1); RS(seed_start, nb + 1);
+    RS(slot, n); RS(ty, n); RS(tz, n); RS(tidx, n); RS(sy, n); RS(sz, n); RS(sorig, n);
+    RS(grid_f, nb); RS(grid_n, nb); RS(cells, n + (size_t)nb * kCellPad + 64);
+    RS(link_up, n); RS(link_dn, n); RS(clink_up, n); RS(clink_dn, n); RS(owner, n);
+    RS(seeds, S_cap); RS(seed_bin, S_cap); RS(tl_rows, S_cap); RS(tl_par, 6 * (size_t)S_cap);
+    RS(tl_table, ((size_t)S_cap / kChunk + 1) * t->c.n_rows * kChunk);
+    RS(tl_nown, S_cap + 1); RS(tl_keep, S_cap + 1); RS(trk_scan, S_cap + 2); RS(hit_scan, S_cap + 2);
+    RS(ev_off_d, 2 * ((size_t)n_events + 1)); RS(h_ev_off, 2 * ((size_t)n_events + 1));
+    RS(scratch, (size_t)std::max<int64_t>(nb, S_cap) / kScanTile + 8);
+    RS(cnt, CNT_N); RS(h_cnt, CNT_N);
+    for (int k = 0; k < 4; k++) RS(o_i[k], S_cap);
+    for (int k = 0; k < 7; k++) RS(o_f[k], S_cap);
+    RS(o_hit, n);
+#undef RS
+    t->S_cap = S_cap;
+    return TPC_OK;
+}
+
+int64_t default_seed_cap(int64_t N) { return std::max<int64_t>(N / 8 + 4096, 4096); }
+
+int validate(const tpc_tracker* t, int n, const tpc_event_in* in) {
+    if (!t || !in || n < 1) { set_err("null tracker / events or n < 1"); return TPC_ERR_ARG; }
+    const int ns = t->c.n_sectors;
+    for (int e = 0; e < n; e++) {
+        const tpc_event_in& ev = in[e];
+        if (ev.n_clusters < 0 || !ev.sector_offset) { set_err("event %d: bad n_clusters / sector_offset", e); return TPC_ERR_ARG; }
+        if (ev.mem_space != in[0].mem_space || (ev.mem_space != 0 && ev.mem_space != 1)) {
+            set_err("event %d: mem_space must be 0 or 1 and the same for the whole batch", e);
+            return TPC_ERR_ARG;
+        }
+        if (ev.n_clusters > 0 && (!ev.y || !ev.z || !ev.row)) { set_err("event %d: null cluster arrays", e); return TPC_ERR_ARG; }
+        if (ev.sector_offset[0] != 0 || ev.sector_offset[ns] != ev.n_clusters) {
+            set_err("event %d: sector_offset must run from 0 to n_clusters", e);
+            return TPC_ERR_ARG;
+        }
+        for (int s = 0; s < ns; s++)
+            if (ev.sector_offset[s + 1] < ev.sector_offset[s]) { set_err("event %d: sector_offset decreases", e); return TPC_ERR_ARG; }
+    }
+    return TPC_OK;
+}
+
+// launch K1..K6 for the staged batch; counts launches
+int launch_all(tpc_tracker* t, int64_t* launches) {
+    const View& v = t->v;
+    const Const& c = t->c;
+    cudaStream_t st = t->stream;
+    const int ns = c.n_sectors, nr = c.n_rows;
+    const int nb = v.n_bins;
+    int64_t L = 0;
+    CK(cudaMemsetAsync(v.bin_count, 0, sizeof(int32_t) * (nb + 1), st));
+    CK(cudaMemsetAsync(v.cnt, 0, sizeof(unsigned long long) * CNT_N, st));
+    if (v.N > 0) CK(cudaMemsetAsync(v.owner, 0, sizeof(uint32_t) * (size_t)v.N, st));
+    int maxn = 0;
+    for (int e = 0; e < t->n_events; e++) maxn = std::max(maxn, t->ev_n[e]);
+    if (maxn > 0) {
+        dim3 g((maxn + 255) / 256, t->n_events);
+        k_count<<<g, 256, 0, st>>>(v, ns, nr); L++;
+    }
+    L += scan_exclusive(v.bin_count, v.bin_start, nb, t->scratch.p, st);
+    if (maxn > 0) {
+        dim3 g((maxn + 255) / 256, t->n_events);
+        k_scatter<<<g, 256, 0, st>>>(v, ns, nr); L++;
+    }
+    k_sort_row<<<nb, kSortThreads, 0, st>>>(v); L++;
+    k_neighbours<<<nb, kNfThreads, 0, st>>>(v, c); L++;
+    k_clean<<<nb, kCleanThreads, 0, st>>>(v); L++;
+    L += scan_exclusive(v.seed_count, v.seed_start, nb, t->scratch.p, st);
+    k_seeds<<<nb, kSeedThreads, 0, st>>>(v); L++;
+    {
+        const int blocks = (int)std::min<int64_t>((t->S_cap + kKfThreads - 1) / kKfThreads, (int64_t)t->sm_count * 16);
+        k_construct<<<std::max(blocks, 1), kKfThreads, 0, st>>>(v, c); L++;
+    }
+    const int chunks = (int)((t->S_cap + kChunk - 1) / kChunk);
+    const int sel_blocks = std::max(1, (chunks * 32 + kSelThreads - 1) / kSelThreads);
+    k_claim<<<sel_blocks, kSelThreads, 0, st>>>(v, c); L++;
+    k_count_owned<<<sel_blocks, kSelThreads, 0, st>>>(v, c); L++;
+    // scans run over the whole seed capacity; entries beyond the seed count are zeroed first
+    L += scan_exclusive(v.tl_keep, v.trk_scan, (int)t->S_cap, t->scratch.p, st);
+    L += scan_exclusive(v.tl_nown, v.hit_scan, (int)t->S_cap, t->scratch.p, st);
+    k_event_offsets<<<(t->n_events + 1 + 63) / 64, 64, 0, st>>>(v, ns * nr); L++;
+    k_write_tracks<<<sel_blocks, kSelThreads, 0, st>>>(v, c); L++;
+    CK(cudaGetLastError());
+    *launches += L;
+    return TPC_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+void tpc_default_params(tpc_params* p) {
+    if (!p) return;
+    p->link_step = 1;
+    p->nf_slope_y = 1.5f; p->nf_slope_z = 2.0f; p->nf_w0 = 0.3f; p->nf_dmax = 0.25f;
+    p->sin_max = 0.95f;
+    p->var_s = 0.25f; p->var_t = 1.0f; p->var_q = 100.0f;
+    p->chi2_link = 25.0f; p->chi2_ext = 16.0f;
+    p->win_nsigma = 4.0f; p->win_min = 0.3f; p->win_max = 3.0f;
+    p->max_gap = 5; p->edge_margin = 1.0f;
+    p->min_tracklet_hits = 10; p->min_track_hits = 10;
+}
+
+const char* tpc_status_string(int s) {
+    switch (s) {
+        case TPC_OK: return "ok";
+        case TPC_ERR_ARG: return "bad argument";
+        case TPC_ERR_GEOMETRY: return "bad geometry";
+        case TPC_ERR_CAPACITY: return "capacity exceeded";
+        case TPC_ERR_CUDA: return "CUDA error";
+        default: return "unknown status";
+    }
+}
+
+const char* tpc_last_error(void) { return g_err.c_str(); }
+
+tpc_tracker* tpc_tracker_create_ex(const tpc_geometry* g, float bz, const tpc_params* params, int32_t max_events,
+                                   int64_t max_clusters) {
+    if (!g || !g->row_x) { set_err("null geometry"); return nullptr; }
+    if (g->n_rows < 3 || g->n_rows > TPC_MAX_ROWS || g->n_sectors < 1 || g->n_sectors > 64) {
+        set_err("geometry: n_rows must be in [3,%d], n_sectors in [1,64]", TPC_MAX_ROWS);
+        return nullptr;
+    }
+    for (int r = 1; r < g->n_rows; r++)
+        if (!(g->row_x[r] > g->row_x[r - 1])) { set_err("geometry: row_x must be strictly increasing"); return nullptr; }
+    if (!(g->sigma_y > 0.f) || !(g->sigma_z > 0.f) || !(g->tan_half_angle > 0.f)) {
+        set_err("geometry: sigma_y, sigma_z, tan_half_angle must be positive");
+        return nullptr;
+    }
+    tpc_params p;
+    if (params) p = *params; else tpc_default_params(&p);
+    if (p.link_step < 1 || p.link_step > 2 || p.min_tracklet_hits < 1 || p.min_track_hits < 1 || p.max_gap < 0) {
+        set_err("params: link_step must be 1 or 2, minimum hit counts >= 1, max_gap >= 0");
+        return nullptr;
+    }
+    int dev = 0, ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
+        set_err("no CUDA device: libtpctrack has no CPU fallback");
+        cudaGetLastError();
+        return nullptr;
+    }
+    cudaGetDevice(&dev);
+    tpc_tracker* t = new tpc_tracker;
+    memset(&t->c, 0, sizeof t->c);
+    for (int r = 0; r < g->n_rows; r++) t->c.row_x[r] = g->row_x[r];
+    t->c.n_sectors = g->n_sectors; t->c.n_rows = g->n_rows;
+    t->c.tan_half_angle = g->tan_half_angle;
+    t->c.sigma_y2 = g->sigma_y * g->sigma_y; t->c.sigma_z2 = g->sigma_z * g->sigma_z;
+    t->c.kB = -1.f * (0.00299792458f * bz);  // curvature = kB * q/pT, DESIGN.md "Conventions"
+    t->c.p = p;
+    if (g->sector_alpha) t->sector_alpha.assign(g->sector_alpha, g->sector_alpha + g->n_sectors);
+    cudaDeviceGetAttribute(&t->sm_count, cudaDevAttrMultiProcessorCount, dev);
+    if (cudaStreamCreateWithFlags(&t->own_stream, cudaStreamNonBlocking) != cudaSuccess) {
+        set_err("cudaStreamCreate failed");
+        delete t;
+        return nullptr;
+    }
+    t->stream = t->own_stream;
+    if (max_events > 0 && max_clusters > 0) {
+        if (reserve_batch(t, max_events, max_clusters, default_seed_cap(max_clusters)) != TPC_OK) {
+            t->free_all(); cudaStreamDestroy(t->own_stream); delete t;
+            return nullptr;
+        }
+    }
+    return t;
+}
+
+tpc_tracker* tpc_tracker_create(const tpc_geometry* g, float bz) { return tpc_tracker_create_ex(g, bz, nullptr, 0, 0); }
+
+void tpc_tracker_destroy(tpc_tracker* t) {
+    if (!t) return;
+    cudaStreamSynchronize(t->stream);
+    t->free_all();
+    if (t->own_stream) cudaStreamDestroy(t->own_stream);
+    delete t;
+}
+
+int tpc_tracker_set_stream(tpc_tracker* t, void* s) {
+    if (!t) return TPC_ERR_ARG;
+    t->stream = s ? (cudaStream_t)s : t->own_stream;
+    return TPC_OK;
+}
+
+int tpc_track_events(tpc_tracker* t, int32_t n, const tpc_event_in* in, tpc_event_out* out) {
+    int rc = validate(t, n, in);
+    if (rc != TPC_OK) return rc;
+    if (!out) { set_err("null output array"); return TPC_ERR_ARG; }
+    t->have_result = false;
+    const int ns = t->c.n_sectors, nr = t->c.n_rows;
+    int64_t N = 0;
+    t->ev_n.assign(n, 0); t->ev_off.assign(n + 1, 0);
+    for (int e = 0; e < n; e++) { t->ev_n[e] = in[e].n_clusters; t->ev_off[e] = (int32_t)N; N += in[e].n_clusters; }
+    t->ev_off[n] = (int32_t)N;
+    if (N > 0x7fff0000ll) { set_err("batch holds more than 2^31 clusters"); return TPC_ERR_CAPACITY; }
+    const bool host_in = in[0].mem_space == 0;
+    int64_t S_cap = std::max<int64_t>(t->S_cap, default_seed_cap(N));
+    memset(&t->counters, 0, sizeof t->counters);
+    cudaStream_t st = t->stream;
+
+    bool done = false;
+    for (int attempt = 0; attempt < 3; attempt++) {
+        if ((rc = reserve_batch(t, n, N, S_cap)) != TPC_OK) return rc;
+        if (host_in) {
+            const size_t nn = (size_t)std::max<int64_t>(N, 1);
+            if ((rc = t->in_y.reserve(nn)) != TPC_OK || (rc = t->in_z.reserve(nn)) != TPC_OK ||
+                (rc = t->in_row.reserve(nn)) != TPC_OK)
+                return rc;
+        }
+        // stage the event table and sector offsets
+        for (int e = 0; e < n; e++) {
+            EventSrc& s = t->h_ev_src.p[e];
+            s.n = in[e].n_clusters; s.off = t->ev_off[e];
+            if (host_in) {
+                s.y = t->in_y.p + s.off; s.z = t->in_z.p + s.off; s.row = t->in_row.p + s.off;
+                if (attempt == 0 && s.n > 0) {
+                    CK(cudaMemcpyAsync(t->in_y.p + s.off, in[e].y, sizeof(float) * s.n, cudaMemcpyHostToDevice, st));
+                    CK(cudaMemcpyAsync(t->in_z.p + s.off, in[e].z, sizeof(float) * s.n, cudaMemcpyHostToDevice, st));
+                    CK(cudaMemcpyAsync(t->in_row.p + s.off, in[e].row, sizeof(int32_t) * s.n, cudaMemcpyHostToDevice, st));
+                }
+            } else {
+                s.y = in[e].y; s.z = in[e].z; s.row = in[e].row;
+            }
+            memcpy(t->h_sec_off.p + (size_t)e * (ns + 1), in[e].sector_offset, sizeof(int32_t) * (ns + 1));
+        }
+        CK(cudaMemcpyAsync(t->ev_src.p, t->h_ev_src.p, sizeof(EventSrc) * n, cudaMemcpyHostToDevice, st));
+        CK(cudaMemcpyAsync(t->sec_off.p, t->h_sec_off.p, sizeof(int32_t) * (size_t)n * (ns + 1), cudaMemcpyHostToDevice, st));
+
+        View& v = t->v;
+        v.n_events = n; v.n_tasks = n * ns; v.n_bins = n * ns * nr; v.N = (int32_t)N;
+        v.ev = t->ev_src.p; v.sec_off = t->sec_off.p;
+        v.bin_count = t->bin_count.p; v.bin_start = t->bin_start.p; v.slot = t->slot.p;
+        v.ty = t->ty.p; v.tz = t->tz.p; v.tidx = t->tidx.p; v.sy = t->sy.p; v.sz = t->sz.p; v.sorig = t->sorig.p;
+        v.grid_f = t->grid_f.p; v.grid_n = t->grid_n.p; v.cells = t->cells.p;
+        v.link_up = t->link_up.p; v.link_dn = t->link_dn.p; v.clink_up = t->clink_up.p; v.clink_dn = t->clink_dn.p;
+        v.seed_count = t->seed_count.p; v.seed_start = t->seed_start.p; v.seeds = t->seeds.p; v.seed_bin = t->seed_bin.p;
+        v.S_cap = (int32_t)t->S_cap;
+        v.tl_table = t->tl_table.p; v.tl_rows = t->tl_rows.p; v.tl_par = t->tl_par.p;
+        v.owner = t->owner.p; v.tl_nown = t->tl_nown.p; v.tl_keep = t->tl_keep.p;
+        v.trk_scan = t->trk_scan.p; v.hit_scan = t->hit_scan.p; v.ev_off = t->ev_off_d.p;
+        v.o_sector = t->o_i[0].p; v.o_first_hit = t->o_i[1].p; v.o_n_hits = t->o_i[2].p; v.o_ndf = t->o_i[3].p;
+        v.o_hit_idx = t->o_hit.p;
+        v.o_x = t->o_f[0].p; v.o_y = t->o_f[1].p; v.o_z = t->o_f[2].p; v.o_sinphi = t->o_f[3].p;
+        v.o_tgl = t->o_f[4].p; v.o_qpt = t->o_f[5].p; v.o_chi2 = t->o_f[6].p;
+        v.cnt = t->cnt.p;
+        t->n_events = n; t->N = N; t->mem_space = in[0].mem_space;
+
+        // keep / nown must read as 0 beyond the seed count
+        CK(cudaMemsetAsync(v.tl_keep, 0, sizeof(int32_t) * (size_t)(t->S_cap + 1), st));
+        CK(cudaMemsetAsync(v.tl_nown, 0, sizeof(int32_t) * (size_t)(t->S_cap + 1), st));
+        if ((rc = launch_all(t, &t->counters.n_kernel_launches)) != TPC_OK) return rc;
+        CK(cudaMemcpyAsync(t->h_cnt.p, v.cnt, sizeof(unsigned long long) * CNT_N, cudaMemcpyDeviceToHost, st));
+        CK(cudaMemcpyAsync(t->h_ev_off.p, v.ev_off, sizeof(int32_t) * 2 * (n + 1), cudaMemcpyDeviceToHost, st));
+        int32_t n_seeds = 0;
+        CK(cudaMemcpyAsync(&n_seeds, v.seed_start + v.n_bins, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+        const unsigned err = (unsigned)(t->h_cnt.p[CNT_ERR] & 0xffffffffu);
+        if (err & kErrBadRow) { set_err("a cluster has row outside [0,%d)", nr); return TPC_ERR_ARG; }
+        if (err & kErrRowCapacity) {
+            set_err("more than %d clusters in one (sector,row)", TPC_MAX_ROW_HITS);
+            return TPC_ERR_CAPACITY;
+        }
+        if ((err & kErrSeedCapacity) || n_seeds > t->S_cap) {  // grow the tracklet pools and run again
+            S_cap = (int64_t)n_seeds + n_seeds / 8 + 1024;
+            t->counters.n_retries++;
+            continue;
+        }
+        t->counters.n_events = n; t->counters.n_clusters = N;
+        t->counters.n_links = (int64_t)t->h_cnt.p[CNT_LINKS];
+        t->counters.n_seeds = n_seeds;
+        t->counters.n_row_visits = (int64_t)t->h_cnt.p[CNT_ROW_VISITS];
+        t->counters.n_tracklet_hits = (int64_t)t->h_cnt.p[CNT_TL_HITS];
+        t->counters.n_tracks = (int64_t)t->h_cnt.p[CNT_TRACKS];
+        t->counters.n_track_hits = (int64_t)t->h_cnt.p[CNT_TRACK_HITS];
+        done = true;
+        break;
+    }
+    if (!done) {
+        set_err("tracklet pool could not be grown");
+        return TPC_ERR_CAPACITY;
+    }
+    // outputs
+    const int64_t T = t->counters.n_tracks, H = t->counters.n_track_hits;
+    const View& v = t->v;
+    const int32_t* toff = t->h_ev_off.p;
+    const int32_t* hoff = t->h_ev_off.p + (n + 1);
+    const int32_t* oi[4] = {v.o_sector, v.o_first_hit, v.o_n_hits, v.o_ndf};
+    const float* of[7] = {v.o_x, v.o_y, v.o_z, v.o_sinphi, v.o_tgl, v.o_qpt, v.o_chi2};
+    const int32_t* ohit = v.o_hit_idx;
+    if (host_in) {
+        for (int k = 0; k < 4; k++) {
+            if ((rc = t->h_o_i[k].reserve((size_t)std::max<int64_t>(T, 1))) != TPC_OK) return rc;
+            if (T) CK(cudaMemcpyAsync(t->h_o_i[k].p, oi[k], sizeof(int32_t) * T, cudaMemcpyDeviceToHost, st));
+            oi[k] = t->h_o_i[k].p;
+        }
+        for (int k = 0; k < 7; k++) {
+            if ((rc = t->h_o_f[k].reserve((size_t)std::max<int64_t>(T, 1))) != TPC_OK) return rc;
+            if (T) CK(cudaMemcpyAsync(t->h_o_f[k].p, of[k], sizeof(float) * T, cudaMemcpyDeviceToHost, st));
+            of[k] = t->h_o_f[k].p;
+        }
+        if ((rc = t->h_o_hit.reserve((size_t)std::max<int64_t>(H, 1))) != TPC_OK) return rc;
+        if (H) CK(cudaMemcpyAsync(t->h_o_hit.p, ohit, sizeof(int32_t) * H, cudaMemcpyDeviceToHost, st));
+        ohit = t->h_o_hit.p;
+        CK(cudaStreamSynchronize(st));
+    }
+    for (int e = 0; e < n; e++) {
+        tpc_event_out& o = out[e];
+        const int32_t a = toff[e], b = toff[e + 1];
+        o.n_tracks = b - a; o.n_track_hits = hoff[e + 1] - hoff[e];
+        o.trk_sector = oi[0] + a; o.trk_first_hit = oi[1] + a; o.trk_n_hits = oi[2] + a; o.trk_ndf = oi[3] + a;
+        o.trk_x = of[0] + a; o.trk_y = of[1] + a; o.trk_z = of[2] + a; o.trk_sinphi = of[3] + a; o.trk_tgl = of[4] + a;
+        o.trk_qpt = of[5] + a; o.trk_chi2 = of[6] + a;
+        o.hit_idx = ohit + hoff[e];
+    }
+    t->have_result = true;
+    return TPC_OK;
+}
+
+int tpc_track_event(tpc_tracker* t, const tpc_event_in* in, tpc_event_out* out) { return tpc_track_events(t, 1, in, out); }
+
+int tpc_get_counters(const tpc_tracker* t, tpc_counters* c) {
+    if (!t || !c) return TPC_ERR_ARG;
+    *c = t->counters;
+    return TPC_OK;
+}
+
+// ---- intermediates (host-side conversion to the caller's indices; not on the hot path) ----
+static int dbg_ranges(const tpc_tracker* t, int event, int* g0, int* g1, int* s0, int* s1) {
+    if (!t || !t->have_result || event < 0 || event >= t->n_events) { set_err("no result / bad event"); return TPC_ERR_ARG; }
+    const int bpe = t->c.n_sectors * t->c.n_rows;
+    int32_t r[2], q[2];
+    cudaStreamSynchronize(t->stream);
+    if (cudaMemcpy(&r[0], t->v.bin_start + (size_t)event * bpe, 4, cudaMemcpyDeviceToHost) != cudaSuccess ||
+        cudaMemcpy(&r[1], t->v.bin_start + (size_t)(event + 1) * bpe, 4, cudaMemcpyDeviceToHost) != cudaSuccess ||
+        cudaMemcpy(&q[0], t->v.seed_start + (size_t)event * bpe, 4, cudaMemcpyDeviceToHost) != cudaSuccess ||
+        cudaMemcpy(&q[1], t->v.seed_start + (size_t)(event + 1) * bpe, 4, cudaMemcpyDeviceToHost) != cudaSuccess) {
+        set_err("cudaMemcpy failed in debug access");
+        return TPC_ERR_CUDA;
+    }
+    *g0 = r[0]; *g1 = r[1]; *s0 = q[0]; *s1 = q[1];
+    return TPC_OK;
+}
+
+int64_t tpc_debug_size(const tpc_tracker* t, int32_t what, int32_t event) {
+    int g0, g1, s0, s1;
+    int rc = dbg_ranges(t, event, &g0, &g1, &s0, &s1);
+    if (rc != TPC_OK) return rc;
+    const int64_t n = g1 - g0, s = s1 - s0;
+    switch (what) {
+        case TPC_DBG_LINK_UP: case TPC_DBG_LINK_DN: case TPC_DBG_CLINK_UP: case TPC_DBG_CLINK_DN: case TPC_DBG_SORTED:
+            return 4 * n;
+        case TPC_DBG_START_HIT: return 4 * s;
+        case TPC_DBG_TL_ROWS: return 12 * s;
+        case TPC_DBG_TL_PAR: return 24 * s;
+        case TPC_DBG_TL_TABLE: return 4 * s * t->c.n_rows;
+        default: set_err("unknown debug item"); return TPC_ERR_ARG;
+    }
+}
+
+int tpc_debug_get(tpc_tracker* t, int32_t what, int32_t event, void* buf, size_t bytes) {
+    int g0, g1, s0, s1;
+    int rc = dbg_ranges(t, event, &g0, &g1, &s0, &s1);
+    if (rc != TPC_OK) return rc;
+    const int64_t need = tpc_debug_size(t, what, event);
+    if (need < 0) return (int)need;
+    if (!buf || bytes < (size_t)need) { set_err("debug buffer too small: need %lld bytes", (long long)need); return TPC_ERR_ARG; }
+    const int n = g1 - g0, s = s1 - s0, nr = t->c.n_rows;
+    std::vector<int32_t> sorig(std::max(n, 1));
+    if (n) CK(cudaMemcpy(sorig.data(), t->v.sorig + g0, 4 * (size_t)n, cudaMemcpyDeviceToHost));
+    auto to_orig = [&](int32_t g) { return g < 0 ? -1 : sorig[g - g0]; };
+    int32_t* ob = (int32_t*)buf;
+    switch (what) {
+        case TPC_DBG_SORTED: memcpy(buf, sorig.data(), 4 * (size_t)n); return TPC_OK;
+        case TPC_DBG_LINK_UP: case TPC_DBG_LINK_DN: case TPC_DBG_CLINK_UP: case TPC_DBG_CLINK_DN: {
+            const int32_t* src = what == TPC_DBG_LINK_UP ? t->v.link_up : what == TPC_DBG_LINK_DN ? t->v.link_dn
+                                 : what == TPC_DBG_CLINK_UP ? t->v.clink_up : t->v.clink_dn;
+            std::vector<int32_t> l(std::max(n, 1));
+            if (n) CK(cudaMemcpy(l.data(), src + g0, 4 * (size_t)n, cudaMemcpyDeviceToHost));
+            for (int k = 0; k < n; k++) ob[sorig[k]] = to_orig(l[k]);
+            return TPC_OK;
+        }
+        case TPC_DBG_START_HIT: {
+            std::vector<int32_t> l(std::max(s, 1));
+            if (s) CK(cudaMemcpy(l.data(), t->v.seeds + s0, 4 * (size_t)s, cudaMemcpyDeviceToHost));
+            for (int k = 0; k < s; k++) ob[k] = to_orig(l[k]);
+            return TPC_OK;
+        }
+        case TPC_DBG_TL_ROWS: {
+            std::vector<int32_t> l(std::max(s, 1));
+            if (s) CK(cudaMemcpy(l.data(), t->v.tl_rows + s0, 4 * (size_t)s, cudaMemcpyDeviceToHost));
+            for (int k = 0; k < s; k++) { ob[3 * k] = l[k] & 0xff; ob[3 * k + 1] = (l[k] >> 8) & 0xff; ob[3 * k + 2] = l[k] >> 16; }
+            return TPC_OK;
+        }
+        case TPC_DBG_TL_PAR: {
+            std::vector<float> l(std::max(s, 1));
+            float* of = (float*)buf;
+            for (int j = 0; j < 6; j++) {
+                if (s) CK(cudaMemcpy(l.data(), t->v.tl_par + (size_t)j * t->S_cap + s0, 4 * (size_t)s, cudaMemcpyDeviceToHost));
+                for (int k = 0; k < s; k++) of[6 * k + j] = l[k];
+            }
+            return TPC_OK;
+        }
+        case TPC_DBG_TL_TABLE: {
+            if (!s) return TPC_OK;
+            std::vector<int32_t> rows(s), tab;
+            CK(cudaMemcpy(rows.data(), t->v.tl_rows + s0, 4 * (size_t)s, cudaMemcpyDeviceToHost));
+            const int c0 = s0 / kChunk, c1 = (s1 - 1) / kChunk;
+            tab.resize((size_t)(c1 - c0 + 1) * nr * kChunk);
+            CK(cudaMemcpy(tab.data(), t->v.tl_table + (size_t)c0 * nr * kChunk, 4 * tab.size(), cudaMemcpyDeviceToHost));
+            for (int k = 0; k < s; k++) {
+                const int i = s0 + k;
+                const int first = rows[k] & 0xff, last = (rows[k] >> 8) & 0xff;
+                const int32_t* tp = tab.data() + (size_t)(i / kChunk - c0) * nr * kChunk + (i % kChunk);
+                for (int r = 0; r < nr; r++) ob[(size_t)k * nr + r] = (r >= first && r <= last) ? to_orig(tp[r * kChunk]) : -1;
+            }
+            return TPC_OK;
+        }
+        default: set_err("unknown debug item"); return TPC_ERR_ARG;
+    }
+}
+
+}  // extern "C"

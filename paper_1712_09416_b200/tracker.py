@@ -1,0 +1,245 @@
+"""Thin ctypes binding of ``csrc/libtpctrack.so`` (the C ABI of ``include/tpctrack.h``).
+
+Argument marshalling only: every step of the path runs in the library's CUDA kernels.  The functions carry the
+names of the C entry points.  There is no CPU fallback: importing this module fails loudly when the library is
+missing, and ``tpc_tracker_create`` fails when no CUDA device is present.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from pathlib import Path
+
+import numpy as np
+
+LIB_PATH = Path(__file__).resolve().parent / "csrc" / "libtpctrack.so"
+
+TPC_OK, TPC_ERR_ARG, TPC_ERR_GEOMETRY, TPC_ERR_CAPACITY, TPC_ERR_CUDA = 0, -1, -2, -3, -4
+DBG = {"link_up": 0, "link_dn": 1, "clink_up": 2, "clink_dn": 3, "start_hit": 4, "tl_rows": 5, "tl_par": 6,
+       "tl_table": 7, "sorted": 8}
+
+
+class tpc_geometry(C.Structure):
+    _fields_ = [("n_sectors", C.c_int32), ("n_rows", C.c_int32), ("row_x", C.POINTER(C.c_float)),
+                ("tan_half_angle", C.c_float), ("z_abs_max", C.c_float), ("sigma_y", C.c_float),
+                ("sigma_z", C.c_float), ("sector_alpha", C.POINTER(C.c_float))]
+
+
+class tpc_params(C.Structure):
+    _fields_ = [("link_step", C.c_int32), ("nf_slope_y", C.c_float), ("nf_slope_z", C.c_float), ("nf_w0", C.c_float),
+                ("nf_dmax", C.c_float), ("sin_max", C.c_float), ("var_s", C.c_float), ("var_t", C.c_float),
+                ("var_q", C.c_float), ("chi2_link", C.c_float), ("chi2_ext", C.c_float), ("win_nsigma", C.c_float),
+                ("win_min", C.c_float), ("win_max", C.c_float), ("max_gap", C.c_int32), ("edge_margin", C.c_float),
+                ("min_tracklet_hits", C.c_int32), ("min_track_hits", C.c_int32)]
+
+    def as_dict(self):
+        return {n: getattr(self, n) for n, _ in self._fields_}
+
+
+class tpc_event_in(C.Structure):
+    _fields_ = [("n_clusters", C.c_int32), ("sector_offset", C.c_void_p), ("x", C.c_void_p), ("y", C.c_void_p),
+                ("z", C.c_void_p), ("row", C.c_void_p), ("mem_space", C.c_int32)]
+
+
+_OUT_I = ("trk_sector", "trk_first_hit", "trk_n_hits", "trk_ndf")
+_OUT_F = ("trk_x", "trk_y", "trk_z", "trk_sinphi", "trk_tgl", "trk_qpt", "trk_chi2")
+
+
+class tpc_event_out(C.Structure):
+    _fields_ = ([("n_tracks", C.c_int32), ("n_track_hits", C.c_int32)] + [(n, C.c_void_p) for n in _OUT_I]
+                + [(n, C.c_void_p) for n in _OUT_F] + [("hit_idx", C.c_void_p)])
+
+
+class tpc_counters(C.Structure):
+    _fields_ = [(n, C.c_int64) for n in ("n_events", "n_clusters", "n_links", "n_seeds", "n_row_visits",
+                                         "n_tracklet_hits", "n_tracks", "n_track_hits", "n_kernel_launches",
+                                         "n_retries")]
+
+    def as_dict(self):
+        return {n: int(getattr(self, n)) for n, _ in self._fields_}
+
+
+class TpcError(RuntimeError):
+    def __init__(self, status, text):
+        super().__init__("tpctrack status %d (%s): %s" % (status, tpc_status_string(status), text))
+        self.status = status
+
+
+def _load():
+    if not LIB_PATH.exists():
+        raise ImportError("%s is missing: build it with `python -c 'import __graft_entry__ as g; g.build()'` "
+                          "(nvcc, sm_100a).  There is no CPU fallback." % LIB_PATH)
+    lib = C.CDLL(str(LIB_PATH))
+    lib.tpc_default_params.argtypes = [C.POINTER(tpc_params)]
+    lib.tpc_tracker_create.restype = C.c_void_p
+    lib.tpc_tracker_create.argtypes = [C.POINTER(tpc_geometry), C.c_float]
+    lib.tpc_tracker_create_ex.restype = C.c_void_p
+    lib.tpc_tracker_create_ex.argtypes = [C.POINTER(tpc_geometry), C.c_float, C.POINTER(tpc_params), C.c_int32, C.c_int64]
+    lib.tpc_tracker_set_stream.argtypes = [C.c_void_p, C.c_void_p]
+    lib.tpc_track_event.argtypes = [C.c_void_p, C.POINTER(tpc_event_in), C.POINTER(tpc_event_out)]
+    lib.tpc_track_events.argtypes = [C.c_void_p, C.c_int32, C.POINTER(tpc_event_in), C.POINTER(tpc_event_out)]
+    lib.tpc_tracker_destroy.argtypes = [C.c_void_p]
+    lib.tpc_tracker_destroy.restype = None
+    lib.tpc_status_string.restype = C.c_char_p
+    lib.tpc_status_string.argtypes = [C.c_int]
+    lib.tpc_last_error.restype = C.c_char_p
+    lib.tpc_get_counters.argtypes = [C.c_void_p, C.POINTER(tpc_counters)]
+    lib.tpc_debug_size.restype = C.c_int64
+    lib.tpc_debug_size.argtypes = [C.c_void_p, C.c_int32, C.c_int32]
+    lib.tpc_debug_get.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_size_t]
+    return lib
+
+
+lib = _load()
+
+EXPORTS = ("tpc_default_params", "tpc_tracker_create", "tpc_tracker_create_ex", "tpc_tracker_set_stream",
+           "tpc_track_event", "tpc_track_events", "tpc_tracker_destroy", "tpc_status_string", "tpc_last_error",
+           "tpc_get_counters", "tpc_debug_size", "tpc_debug_get")
+
+
+def tpc_status_string(status: int) -> str:
+    return lib.tpc_status_string(status).decode()
+
+
+def tpc_last_error() -> str:
+    return lib.tpc_last_error().decode()
+
+
+def tpc_default_params() -> tpc_params:
+    p = tpc_params()
+    lib.tpc_default_params(C.byref(p))
+    return p
+
+
+def _check(status):
+    if status != TPC_OK:
+        raise TpcError(status, tpc_last_error())
+
+
+class Tracker:
+    """Owns one ``tpc_tracker*``.  ``row_x``: float32 pad-row radii (host)."""
+
+    def __init__(self, n_sectors, row_x, tan_half_angle, sigma_y, sigma_z, bz, params: tpc_params | None = None,
+                 z_abs_max=250.0, max_events=0, max_clusters=0):
+        self._rx = np.ascontiguousarray(row_x, dtype=np.float32)
+        g = tpc_geometry(n_sectors, self._rx.shape[0], self._rx.ctypes.data_as(C.POINTER(C.c_float)), tan_half_angle,
+                         z_abs_max, sigma_y, sigma_z, None)
+        self.n_sectors, self.n_rows = n_sectors, int(self._rx.shape[0])
+        self._h = lib.tpc_tracker_create_ex(C.byref(g), bz, C.byref(params) if params is not None else None,
+                                            max_events, max_clusters)
+        if not self._h:
+            raise TpcError(TPC_ERR_CUDA, tpc_last_error())
+        self._keep = None
+
+    def close(self):
+        if getattr(self, "_h", None):
+            lib.tpc_tracker_destroy(self._h)
+            self._h = None
+
+    __del__ = close
+
+    def set_stream(self, cuda_stream_ptr: int | None):
+        _check(lib.tpc_tracker_set_stream(self._h, C.c_void_p(cuda_stream_ptr or 0)))
+
+    # ---- marshalling ----
+    @staticmethod
+    def _ptr(a):
+        if a is None:
+            return None, 0
+        if isinstance(a, np.ndarray):
+            return a.ctypes.data, 0
+        return a.data_ptr(), 1        # torch tensor
+
+    def _marshal(self, events):
+        n = len(events)
+        ins = (tpc_event_in * n)()
+        keep = []
+        for i, ev in enumerate(events):
+            so = np.ascontiguousarray(ev["sector_offset"], dtype=np.int32)
+            keep.append(so)
+            spaces = set()
+            ptrs = {}
+            for k in ("y", "z", "row"):
+                a = ev[k]
+                if isinstance(a, np.ndarray):
+                    want = np.int32 if k == "row" else np.float32
+                    if a.dtype != want or not a.flags.c_contiguous:
+                        a = np.ascontiguousarray(a, dtype=want)
+                    keep.append(a)
+                else:
+                    assert a.is_cuda and a.is_contiguous(), "device inputs must be contiguous CUDA tensors"
+                    keep.append(a)
+                p, sp = self._ptr(a)
+                ptrs[k] = p
+                spaces.add(sp)
+            assert len(spaces) == 1, "y, z, row must live in one memory space"
+            ncl = int(so[-1])
+            ins[i] = tpc_event_in(ncl, so.ctypes.data, None, ptrs["y"], ptrs["z"], ptrs["row"], spaces.pop())
+        return ins, keep
+
+    def tpc_track_events(self, events):
+        """events: list of dicts with sector_offset (host int32), y, z (float32), row (int32): all numpy (host)
+        or all torch CUDA tensors (device).  Returns a list of raw ``tpc_event_out`` structs (pointers are
+        library-owned; host or device like the input) -- see ``to_numpy``."""
+        n = len(events)
+        ins, keep = self._marshal(events)
+        outs = (tpc_event_out * n)()
+        self._keep = keep
+        _check(lib.tpc_track_events(self._h, n, ins, outs))
+        self._mem_space = ins[0].mem_space if n else 0
+        return list(outs)
+
+    def tpc_track_event(self, event):
+        return self.tpc_track_events([event])[0]
+
+    def tpc_get_counters(self) -> dict:
+        c = tpc_counters()
+        _check(lib.tpc_get_counters(self._h, C.byref(c)))
+        return c.as_dict()
+
+    def tpc_debug_get(self, what: str, event: int = 0) -> np.ndarray:
+        w = DBG[what]
+        nbytes = lib.tpc_debug_size(self._h, w, event)
+        if nbytes < 0:
+            raise TpcError(int(nbytes), tpc_last_error())
+        dt = np.float32 if what == "tl_par" else np.int32
+        a = np.zeros(nbytes // 4, dt)
+        _check(lib.tpc_debug_get(self._h, w, event, a.ctypes.data, a.nbytes))
+        if what == "tl_rows":
+            a = a.reshape(-1, 3)
+        elif what == "tl_par":
+            a = a.reshape(-1, 6)
+        elif what == "tl_table":
+            a = a.reshape(-1, self.n_rows)
+        return a
+
+    @staticmethod
+    def as_tensor(ptr, n, dt):
+        """Zero-copy torch view of a library-owned device array."""
+        import torch
+
+        class _Dev:
+            pass
+        d = _Dev()
+        d.__cuda_array_interface__ = {"shape": (n,), "typestr": "<i4" if dt == np.int32 else "<f4",
+                                      "data": (int(ptr), False), "version": 2}
+        return torch.as_tensor(d, device="cuda")
+
+    def to_numpy(self, out: tpc_event_out) -> dict:
+        """Copy one event's outputs into numpy arrays."""
+        T, H = out.n_tracks, out.n_track_hits
+        res = {"n_tracks": T, "n_track_hits": H}
+
+        def fetch(ptr, n, dt):
+            if n == 0 or not ptr:
+                return np.zeros(0, dt)
+            if self._mem_space == 0:
+                return np.ctypeslib.as_array(C.cast(ptr, C.POINTER(C.c_int32 if dt == np.int32 else C.c_float)),
+                                             shape=(n,)).copy()
+            return self.as_tensor(ptr, n, dt).cpu().numpy()
+
+        for k in _OUT_I:
+            res[k] = fetch(getattr(out, k), T, np.int32)
+        for k in _OUT_F:
+            res[k] = fetch(getattr(out, k), T, np.float32)
+        res["hit_idx"] = fetch(out.hit_idx, H, np.int32)
+        return res
