@@ -146,6 +146,13 @@ const char* tpc_last_error(void); /* thread-local text of the last failure */
 
 int tpc_get_counters(const tpc_tracker* t, tpc_counters* c);
 
+/* Per-stage device times of the last call, measured with CUDA events on the tracker's stream (off by default:
+ * the events cost a few microseconds).  Stages: 0 = K1 bucket + grid sort, 1 = K2 neighbour finder,
+ * 2 = K3 cleaner + K4 start hits, 3 = K5 tracklet constructor (one kernel), 4 = K6 selector + output. */
+#define TPC_N_STAGES 5
+int tpc_tracker_set_profiling(tpc_tracker* t, int32_t on);
+int tpc_get_stage_ms(const tpc_tracker* t, float* ms /* [TPC_N_STAGES] */);
+
 /* ---- intermediates of the last call, for stage-by-stage parity tests (not part of the hot path) ----
  * All hit indices are the caller's indices within event `event`; -1 = none.  buf is a HOST buffer of `bytes`
  * bytes; the call fails with TPC_ERR_ARG if it is too small.  Sizes: tpc_debug_size(). */

@@ -90,6 +90,9 @@ struct tpc_tracker {
     Buf<unsigned long long> h_cnt;
     Buf<float> h_o_f[7];
     int64_t S_cap = 0;
+    bool profiling = false;
+    cudaEvent_t evt[TPC_N_STAGES + 1] = {};
+    float stage_ms[TPC_N_STAGES] = {};
 
     tpc_tracker() {
         h_ev_src.host = h_sec_off.host = h_ev_off.host = h_cnt.host = h_o_hit.host = true;
@@ -175,6 +178,8 @@ int launch_all(tpc_tracker* t, int64_t* launches) {
     CK(cudaMemsetAsync(v.bin_count, 0, sizeof(int32_t) * (nb + 1), st));
     CK(cudaMemsetAsync(v.cnt, 0, sizeof(unsigned long long) * CNT_N, st));
     if (v.N > 0) CK(cudaMemsetAsync(v.owner, 0, sizeof(uint32_t) * (size_t)v.N, st));
+    auto mark = [&](int k) { if (t->profiling) cudaEventRecord(t->evt[k], st); };
+    mark(0);
     int maxn = 0;
     for (int e = 0; e < t->n_events; e++) maxn = std::max(maxn, t->ev_n[e]);
     if (maxn > 0) {
@@ -187,14 +192,18 @@ int launch_all(tpc_tracker* t, int64_t* launches) {
         k_scatter<<<g, 256, 0, st>>>(v, ns, nr); L++;
     }
     k_sort_row<<<nb, kSortThreads, 0, st>>>(v); L++;
+    mark(1);
     k_neighbours<<<nb, kNfThreads, 0, st>>>(v, c); L++;
+    mark(2);
     k_clean<<<nb, kCleanThreads, 0, st>>>(v); L++;
     L += scan_exclusive(v.seed_count, v.seed_start, nb, t->scratch.p, st);
     k_seeds<<<nb, kSeedThreads, 0, st>>>(v); L++;
+    mark(3);
     {
         const int blocks = (int)std::min<int64_t>((t->S_cap + kKfThreads - 1) / kKfThreads, (int64_t)t->sm_count * 16);
         k_construct<<<std::max(blocks, 1), kKfThreads, 0, st>>>(v, c); L++;
     }
+    mark(4);
     const int chunks = (int)((t->S_cap + kChunk - 1) / kChunk);
     const int sel_blocks = std::max(1, (chunks * 32 + kSelThreads - 1) / kSelThreads);
     k_claim<<<sel_blocks, kSelThreads, 0, st>>>(v, c); L++;
@@ -204,6 +213,7 @@ int launch_all(tpc_tracker* t, int64_t* launches) {
     L += scan_exclusive(v.tl_nown, v.hit_scan, (int)t->S_cap, t->scratch.p, st);
     k_event_offsets<<<(t->n_events + 1 + 63) / 64, 64, 0, st>>>(v, ns * nr); L++;
     k_write_tracks<<<sel_blocks, kSelThreads, 0, st>>>(v, c); L++;
+    mark(5);
     CK(cudaGetLastError());
     *launches += L;
     return TPC_OK;
@@ -296,6 +306,7 @@ void tpc_tracker_destroy(tpc_tracker* t) {
     cudaStreamSynchronize(t->stream);
     t->free_all();
     if (t->own_stream) cudaStreamDestroy(t->own_stream);
+    for (auto& e : t->evt) if (e) cudaEventDestroy(e);
     delete t;
 }
 
@@ -377,6 +388,8 @@ int tpc_track_events(tpc_tracker* t, int32_t n, const tpc_event_in* in, tpc_even
         int32_t n_seeds = 0;
         CK(cudaMemcpyAsync(&n_seeds, v.seed_start + v.n_bins, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
         CK(cudaStreamSynchronize(st));
+        if (t->profiling)
+            for (int k = 0; k < TPC_N_STAGES; k++) cudaEventElapsedTime(&t->stage_ms[k], t->evt[k], t->evt[k + 1]);
         const unsigned err = (unsigned)(t->h_cnt.p[CNT_ERR] & 0xffffffffu);
         if (err & kErrBadRow) { set_err("a cluster has row outside [0,%d)", nr); return TPC_ERR_ARG; }
         if (err & kErrRowCapacity) {
@@ -440,6 +453,21 @@ int tpc_track_events(tpc_tracker* t, int32_t n, const tpc_event_in* in, tpc_even
 }
 
 int tpc_track_event(tpc_tracker* t, const tpc_event_in* in, tpc_event_out* out) { return tpc_track_events(t, 1, in, out); }
+
+int tpc_tracker_set_profiling(tpc_tracker* t, int32_t on) {
+    if (!t) return TPC_ERR_ARG;
+    if (on)
+        for (auto& e : t->evt)
+            if (!e) CK(cudaEventCreate(&e));
+    t->profiling = on != 0;
+    return TPC_OK;
+}
+
+int tpc_get_stage_ms(const tpc_tracker* t, float* ms) {
+    if (!t || !ms) return TPC_ERR_ARG;
+    for (int k = 0; k < TPC_N_STAGES; k++) ms[k] = t->profiling ? t->stage_ms[k] : 0.f;
+    return TPC_OK;
+}
 
 int tpc_get_counters(const tpc_tracker* t, tpc_counters* c) {
     if (!t || !c) return TPC_ERR_ARG;

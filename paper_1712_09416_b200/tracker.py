@@ -83,6 +83,8 @@ def _load():
     lib.tpc_status_string.argtypes = [C.c_int]
     lib.tpc_last_error.restype = C.c_char_p
     lib.tpc_get_counters.argtypes = [C.c_void_p, C.POINTER(tpc_counters)]
+    lib.tpc_tracker_set_profiling.argtypes = [C.c_void_p, C.c_int32]
+    lib.tpc_get_stage_ms.argtypes = [C.c_void_p, C.POINTER(C.c_float)]
     lib.tpc_debug_size.restype = C.c_int64
     lib.tpc_debug_size.argtypes = [C.c_void_p, C.c_int32, C.c_int32]
     lib.tpc_debug_get.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_size_t]
@@ -93,7 +95,7 @@ lib = _load()
 
 EXPORTS = ("tpc_default_params", "tpc_tracker_create", "tpc_tracker_create_ex", "tpc_tracker_set_stream",
            "tpc_track_event", "tpc_track_events", "tpc_tracker_destroy", "tpc_status_string", "tpc_last_error",
-           "tpc_get_counters", "tpc_debug_size", "tpc_debug_get")
+           "tpc_get_counters", "tpc_tracker_set_profiling", "tpc_get_stage_ms", "tpc_debug_size", "tpc_debug_get")
 
 
 def tpc_status_string(status: int) -> str:
@@ -195,6 +197,14 @@ class Tracker:
         c = tpc_counters()
         _check(lib.tpc_get_counters(self._h, C.byref(c)))
         return c.as_dict()
+
+    def tpc_tracker_set_profiling(self, on: bool):
+        _check(lib.tpc_tracker_set_profiling(self._h, int(on)))
+
+    def tpc_get_stage_ms(self):
+        ms = (C.c_float * 5)()
+        _check(lib.tpc_get_stage_ms(self._h, ms))
+        return [float(v) for v in ms]
 
     def tpc_debug_get(self, what: str, event: int = 0) -> np.ndarray:
         w = DBG[what]
