@@ -103,6 +103,22 @@ def stage_bytes(c):
     }
 
 
+def max_over_ranks(ms, world, device="cuda"):
+    """Elapsed time of the job = the slowest rank's (all_reduce MAX; identity for one rank)."""
+    if world <= 1:
+        return float(ms)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([ms], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(events_per_rank, steps, ms, world):
+    """Whole-job events/s: every rank tracked its own events_per_rank x steps events in ms milliseconds."""
+    return world * events_per_rank * steps / (ms * 1e-3)
+
+
 def run_reference(args, rank, world):
     """The CPU oracle (unmodified, strict-float32 mode, all host threads) -- one event per step."""
     if rank != 0:
@@ -210,11 +226,7 @@ def main():
                 stages += np.array(trk.tpc_get_stage_ms())
         e1.record(stream)
         barrier()
-        ms = e0.elapsed_time(e1)
-        if world > 1:
-            t = torch.tensor([ms], device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms = float(t.item())
+        ms = max_over_ranks(e0.elapsed_time(e1), world)
         return ms, stages / max(steps, 1), outs, launches
 
     for _ in range(args.warmup):
@@ -233,7 +245,7 @@ def main():
             trk.tpc_track_events(host_in)
         ms_e, _, outs_e, _ = timed(host_in, args.steps, False)
         assert sum(o.n_tracks for o in outs_e) == n_tracks
-        e2e = {"value": world * len(evs) * args.steps / (ms_e * 1e-3), "unit": UNIT,
+        e2e = {"value": aggregate_value(len(evs), args.steps, ms_e, world), "unit": UNIT,
                "h2d_bytes_per_step": int(12 * n_total + sum(4 * (ev.n_sectors + 1) for ev in evs)),
                "d2h_bytes_per_step": int(44 * n_tracks + 4 * n_hits), "ms_per_step": ms_e / args.steps}
 
@@ -267,7 +279,7 @@ def main():
             cpu = {"value": nb / dt, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle",
                    "sample": "first %d events of the batch (%d clusters), strict-float32 mode, OpenMP over sectors"
                              % (nb, sum(ev.n_clusters for ev in evs[:nb]))}
-        value = world * len(evs) * args.steps / (ms * 1e-3)
+        value = aggregate_value(len(evs), args.steps, ms, world)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
