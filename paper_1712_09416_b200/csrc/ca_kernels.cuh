@@ -55,30 +55,32 @@ __global__ void __launch_bounds__(256) k_scatter(const View v, int ns, int nr) {
     const int sl = v.slot[src.off + i];
     if (sl >= TPC_MAX_ROW_HITS) return;
     const int pos = v.bin_start[bin] + sl;
-    v.ty[pos] = src.y[i];
-    v.tz[pos] = src.z[i];
+    v.thit[pos] = make_float2(src.y[i], src.z[i]);
     v.tidx[pos] = i;
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// K1c: one CTA per bin: bounding box -> grid dims -> sort the bin by (cell, caller's index) -> cell table.
-// The grid only accelerates the window searches; windows are defined on coordinates, so its shape never
-// changes a result.
+// K1c: one CTA per bin: bounding box -> grid dims -> counting sort of the bin by grid cell -> cell table.
+// The grid only accelerates the window searches; windows are defined on coordinates and every tie is broken
+// on the caller's index, so neither the grid's shape nor the order inside a cell changes a result.
 // ---------------------------------------------------------------------------------------------------------
-constexpr int kSortThreads = 256;
+constexpr int kSortThreads = 128;
 
 __global__ void __launch_bounds__(kSortThreads) k_sort_row(const View v) {
-    __shared__ unsigned long long key[TPC_MAX_ROW_HITS];
+    __shared__ int cnt[TPC_MAX_ROW_HITS + kCellPad + 1];  // hits per cell, then first hit of each cell
+    __shared__ uint16_t ck[TPC_MAX_ROW_HITS];             // cell of hit k
+    __shared__ uint16_t rk[TPC_MAX_ROW_HITS];             // arrival rank of hit k inside its cell
     __shared__ float red[4][kSortThreads / 32];
     __shared__ float box[4];
+    __shared__ int scan_total;
     const int bin = blockIdx.x;
     const int b0 = v.bin_start[bin];
     const int n = min(v.bin_start[bin + 1] - b0, TPC_MAX_ROW_HITS);
     uint16_t* cs = v.cells + (size_t)b0 + (size_t)bin * kCellPad;
     if (n == 0) {
         if (threadIdx.x == 0) {
-            v.grid_f[bin] = make_float4(0.f, 0.f, 0.f, 0.f);
-            v.grid_n[bin] = make_int2(1, 1);
+            BinDesc d; d.y0 = 0.f; d.z0 = 0.f; d.idy = 0.f; d.idz = 0.f; d.base = b0; d.n = 0; d.ny = 1; d.nz = 1;
+            v.desc[bin] = d;
             cs[0] = 0; cs[1] = 0;
         }
         return;
@@ -86,13 +88,13 @@ __global__ void __launch_bounds__(kSortThreads) k_sort_row(const View v) {
     // bounding box
     float ymin = 3.0e38f, ymax = -3.0e38f, zmin = 3.0e38f, zmax = -3.0e38f;
     for (int k = threadIdx.x; k < n; k += kSortThreads) {
-        const float y = v.ty[b0 + k], z = v.tz[b0 + k];
-        ymin = fminf(ymin, y); ymax = fmaxf(ymax, y); zmin = fminf(zmin, z); zmax = fmaxf(zmax, z);
+        const float2 h = v.thit[b0 + k];
+        ymin = fminf(ymin, h.x); ymax = fmaxf(ymax, h.x); zmin = fminf(zmin, h.y); zmax = fmaxf(zmax, h.y);
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
-        ymin = fminf(ymin, __shfl_xor_sync(0xffffffffu, ymin, o)); ymax = fmaxf(ymax, __shfl_xor_sync(0xffffffffu, ymax, o));
-        zmin = fminf(zmin, __shfl_xor_sync(0xffffffffu, zmin, o)); zmax = fmaxf(zmax, __shfl_xor_sync(0xffffffffu, zmax, o));
+        ymin = fminf(ymin, __shfl_xor_sync(kFull, ymin, o)); ymax = fmaxf(ymax, __shfl_xor_sync(kFull, ymax, o));
+        zmin = fminf(zmin, __shfl_xor_sync(kFull, zmin, o)); zmax = fmaxf(zmax, __shfl_xor_sync(kFull, zmax, o));
     }
     if (lane_id() == 0) {
         const int w = threadIdx.x >> 5;
@@ -118,113 +120,146 @@ __global__ void __launch_bounds__(kSortThreads) k_sort_row(const View v) {
     if (nz > cap) nz = cap;
     if (ny * nz > cap) ny = max(1, cap / nz);
     const float idy = (float)ny / (ylen * 1.0001f), idz = (float)nz / (zlen * 1.0001f);
-    // keys: cell << 48 | caller's index << 16 | arrival slot
-    int P = 1;
-    while (P < n) P <<= 1;
-    for (int k = threadIdx.x; k < P; k += kSortThreads) {
-        unsigned long long kk = ~0ull;
-        if (k < n) {
-            const float y = v.ty[b0 + k], z = v.tz[b0 + k];
-            const int iy = max(0, min((int)((y - ymin) * idy), ny - 1));
-            const int iz = max(0, min((int)((z - zmin) * idz), nz - 1));
-            const unsigned long long cell = (unsigned long long)(iz * ny + iy);
-            kk = (cell << 48) | ((unsigned long long)(unsigned)v.tidx[b0 + k] << 16) | (unsigned long long)k;
-        }
-        key[k] = kk;
+    const int ncell = ny * nz;
+    for (int q = threadIdx.x; q <= ncell; q += kSortThreads) cnt[q] = 0;
+    __syncthreads();
+    for (int k = threadIdx.x; k < n; k += kSortThreads) {
+        const float2 h = v.thit[b0 + k];
+        const int cell = grid_cell(h.y, zmin, idz, nz) * ny + grid_cell(h.x, ymin, idy, ny);
+        ck[k] = (uint16_t)cell;
+        rk[k] = (uint16_t)atomicAdd(&cnt[cell], 1);
     }
     __syncthreads();
-    // bitonic sort
-    for (int size = 2; size <= P; size <<= 1) {
-        for (int stride = size >> 1; stride > 0; stride >>= 1) {
-            for (int t = threadIdx.x; t < (P >> 1); t += kSortThreads) {
-                const int lo = 2 * t - (t & (stride - 1));
-                const int hi = lo + stride;
-                const bool up = ((lo & size) == 0);
-                const unsigned long long a = key[lo], b = key[hi];
-                if ((a > b) == up) { key[lo] = b; key[hi] = a; }
-            }
-            __syncthreads();
-        }
+    // exclusive scan of cnt[0..ncell): each thread owns a contiguous chunk
+    {
+        const int per = (ncell + kSortThreads - 1) / kSortThreads;
+        const int q0 = threadIdx.x * per, q1 = min(q0 + per, ncell);
+        int s = 0;
+        for (int q = q0; q < q1; q++) s += cnt[q];
+        int ex = block_excl_scan<kSortThreads>(s, &scan_total);
+        for (int q = q0; q < q1; q++) { const int t = cnt[q]; cnt[q] = ex; ex += t; }
     }
-    // write sorted hits and the cell table
-    const int ncell = ny * nz;
+    __syncthreads();
+    for (int q = threadIdx.x; q <= ncell; q += kSortThreads) cs[q] = (uint16_t)(q < ncell ? cnt[q] : n);
     for (int k = threadIdx.x; k < n; k += kSortThreads) {
-        const unsigned long long kk = key[k];
-        const int sl = (int)(kk & 0xffffull);
-        v.sy[b0 + k] = v.ty[b0 + sl];
-        v.sz[b0 + k] = v.tz[b0 + sl];
-        v.sorig[b0 + k] = (int32_t)((kk >> 16) & 0xffffffffull);
-        const int c = (int)(kk >> 48);
-        const int cprev = k == 0 ? -1 : (int)(key[k - 1] >> 48);
-        for (int q = cprev + 1; q <= c; q++) cs[q] = (uint16_t)k;
-        if (k == n - 1)
-            for (int q = c + 1; q <= ncell; q++) cs[q] = (uint16_t)n;
+        const int pos = b0 + cnt[ck[k]] + rk[k];
+        v.shit[pos] = v.thit[b0 + k];
+        v.sorig[pos] = v.tidx[b0 + k];
     }
     if (threadIdx.x == 0) {
-        v.grid_f[bin] = make_float4(ymin, zmin, idy, idz);
-        v.grid_n[bin] = make_int2(ny, nz);
+        BinDesc d; d.y0 = ymin; d.z0 = zmin; d.idy = idy; d.idz = idz; d.base = b0; d.n = n; d.ny = ny; d.nz = nz;
+        v.desc[bin] = d;
     }
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// K2 neighbour finder.  One CTA per bin (task,row); a thread takes hits of the row.
+// K2 neighbour finder.  One CTA per bin (task,row); the two neighbour rows (hits + cell tables)
+// are staged in shared memory; a thread takes hits of the row.
 // For hit h of row r: among up-candidates u (row r+D) and down-candidates d (row r-D) inside the windows,
 // minimise D = (y0 - yhat)^2 + (z0 - zhat)^2 with (yhat, zhat) the point of the line d->u at x0;
 // ties -> lowest caller's index of u, then of d.
 // ---------------------------------------------------------------------------------------------------------
 constexpr int kNfThreads = 128;
+constexpr int kNfCap = 1024;   // hits of a neighbour row held in shared memory; larger rows are read in place
+constexpr int kNfList = 8;     // down-candidates remembered per hit; more -> nested walk
 
 __global__ void __launch_bounds__(kNfThreads) k_neighbours(const View v, const __grid_constant__ Const c) {
+    __shared__ float2 s_hu[kNfCap], s_hd[kNfCap];
+    __shared__ uint16_t s_cu[kNfCap + kCellPad + 1], s_cd[kNfCap + kCellPad + 1];
+    __shared__ uint16_t s_dl[kNfList][kNfThreads];
     const int bin = blockIdx.x;
     const int nr = c.n_rows, D = c.p.link_step;
     const int r = bin % nr;
-    const int b0 = v.bin_start[bin], n = v.bin_start[bin + 1] - b0;
+    const int4 own = load_desc_n(v, bin);
+    const int b0 = own.x, n = own.y;
     if (n == 0) return;
-    if (r - D < 0 || r + D >= nr) {
+    bool none = (r - D < 0 || r + D >= nr);
+    int4 du = make_int4(0, 0, 1, 1), dd = du;
+    if (!none) {
+        du = load_desc_n(v, bin + D); dd = load_desc_n(v, bin - D);
+        none = du.y == 0 || dd.y == 0;
+    }
+    if (none) {
         for (int k = threadIdx.x; k < n; k += kNfThreads) { v.link_up[b0 + k] = -1; v.link_dn[b0 + k] = -1; }
         return;
     }
+    const float4 gfu = load_desc_f(v, bin + D), gfd = load_desc_f(v, bin - D);
+    const float2* hu = v.shit + du.x; const float2* hd = v.shit + dd.x;
+    const uint16_t* cu = cell_table(v, bin + D, du.x); const uint16_t* cd = cell_table(v, bin - D, dd.x);
+    if (du.y <= kNfCap) {
+        for (int k = threadIdx.x; k < du.y; k += kNfThreads) s_hu[k] = hu[k];
+        for (int k = threadIdx.x; k <= du.z * du.w; k += kNfThreads) s_cu[k] = cu[k];
+        hu = s_hu; cu = s_cu;
+    }
+    if (dd.y <= kNfCap) {
+        for (int k = threadIdx.x; k < dd.y; k += kNfThreads) s_hd[k] = hd[k];
+        for (int k = threadIdx.x; k <= dd.z * dd.w; k += kNfThreads) s_cd[k] = cd[k];
+        hd = s_hd; cd = s_cd;
+    }
+    __syncthreads();
     const float x0 = c.row_x[r], x1 = c.row_x[r + D], x2 = c.row_x[r - D];
     const float wyu = c.p.nf_slope_y * fabsf(x1 - x0) + c.p.nf_w0, wzu = c.p.nf_slope_z * fabsf(x1 - x0) + c.p.nf_w0;
     const float wyd = c.p.nf_slope_y * fabsf(x2 - x0) + c.p.nf_w0, wzd = c.p.nf_slope_z * fabsf(x2 - x0) + c.p.nf_w0;
     const float a = (x0 - x2) / (x1 - x2);
-    const RowGrid gu = load_grid(v, bin + D), gd = load_grid(v, bin - D);
-    const bool none = (v.bin_start[bin + D + 1] - gu.base == 0) || (v.bin_start[bin - D + 1] - gd.base == 0);
+    const int nyu = du.z, nyd = dd.z;
     for (int k = threadIdx.x; k < n; k += kNfThreads) {
         const int h = b0 + k;
-        int bu = -1, bd = -1, bou = 0, bod = 0;
+        const float2 h0 = v.shit[h];
+        const float y0 = h0.x, z0 = h0.y;
+        int bu = -1, bd = -1;   // row-local indices of the best pair
         float best = 0.f;
-        if (!none) {
-            const float y0 = v.sy[h], z0 = v.sz[h];
-            GridIter iu;
-            iu.start(gu, y0, z0, wyu, wzu);
-            int u;
-            while (iu.next(u)) {
-                const float yu = v.sy[u], zu = v.sz[u];
-                if (!(fabsf(yu - y0) <= wyu && fabsf(zu - z0) <= wzu)) continue;
-                const int ou = v.sorig[u];
-                GridIter id;
-                id.start(gd, y0, z0, wyd, wzd);
-                int d;
-                while (id.next(d)) {
-                    const float yd = v.sy[d], zd = v.sz[d];
-                    if (!(fabsf(yd - y0) <= wyd && fabsf(zd - z0) <= wzd)) continue;
-                    const float yh = yd + a * (yu - yd);
-                    const float zh = zd + a * (zu - zd);
-                    const float dy = y0 - yh, dz = z0 - zh;
-                    const float dev = dy * dy + dz * dz;
-                    bool take = bu < 0 || dev < best;
-                    if (!take && dev == best) {
-                        const int od = v.sorig[d];
-                        take = ou < bou || (ou == bou && od < bod);
-                    }
-                    if (take) { best = dev; bu = u; bd = d; bou = ou; bod = v.sorig[d]; }
+        auto eval = [&](int u, const float2& pu, int d, const float2& pd) {
+            const float yh = pd.x + a * (pu.x - pd.x);
+            const float zh = pd.y + a * (pu.y - pd.y);
+            const float dy = y0 - yh, dz = z0 - zh;
+            const float dev = dy * dy + dz * dz;
+            bool take = bu < 0 || dev < best;
+            if (!take && dev == best) {  // exact tie: lowest caller's index of u, then of d
+                const int ou = v.sorig[du.x + u], obu = v.sorig[du.x + bu];
+                take = ou < obu || (ou == obu && v.sorig[dd.x + d] < v.sorig[dd.x + bd]);
+            }
+            if (take) { best = dev; bu = u; bd = d; }
+        };
+        // down-candidates inside the window, remembered
+        const CellWin wd = cell_window(gfd, nyd, dd.w, y0, z0, wyd, wzd);
+        int nd = 0;
+        for (int iz = wd.iz0; iz <= wd.iz1; iz++) {
+            int p = cd[iz * nyd + wd.iy0];
+            const int pe = cd[iz * nyd + wd.iy1 + 1];
+            for (; p < pe; p++) {
+                const float2 pd = hd[p];
+                if (fabsf(pd.x - y0) <= wyd && fabsf(pd.y - z0) <= wzd) {
+                    if (nd < kNfList) s_dl[nd][threadIdx.x] = (uint16_t)p;
+                    nd++;
                 }
             }
-            if (!(bu >= 0 && best <= c.p.nf_dmax)) { bu = -1; bd = -1; }
         }
-        v.link_up[h] = bu;
-        v.link_dn[h] = bd;
+        if (nd > 0) {
+            const CellWin wu = cell_window(gfu, nyu, du.w, y0, z0, wyu, wzu);
+            for (int iz = wu.iz0; iz <= wu.iz1; iz++) {
+                int p = cu[iz * nyu + wu.iy0];
+                const int pe = cu[iz * nyu + wu.iy1 + 1];
+                for (; p < pe; p++) {
+                    const float2 pu = hu[p];
+                    if (!(fabsf(pu.x - y0) <= wyu && fabsf(pu.y - z0) <= wzu)) continue;
+                    if (nd <= kNfList) {
+                        for (int j = 0; j < nd; j++) { const int d = s_dl[j][threadIdx.x]; eval(p, pu, d, hd[d]); }
+                    } else {
+                        for (int jz = wd.iz0; jz <= wd.iz1; jz++) {
+                            int q = cd[jz * nyd + wd.iy0];
+                            const int qe = cd[jz * nyd + wd.iy1 + 1];
+                            for (; q < qe; q++) {
+                                const float2 pd = hd[q];
+                                if (fabsf(pd.x - y0) <= wyd && fabsf(pd.y - z0) <= wzd) eval(p, pu, q, pd);
+                            }
+                        }
+                    }
+                }
+            }
+        }
+        const bool ok = bu >= 0 && best <= c.p.nf_dmax;
+        v.link_up[h] = ok ? du.x + bu : -1;
+        v.link_dn[h] = ok ? dd.x + bd : -1;
     }
 }
 
@@ -252,7 +287,7 @@ __global__ void __launch_bounds__(kCleanThreads) k_clean(const View v) {
         nl += (cu >= 0);
     }
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) { ns += __shfl_xor_sync(0xffffffffu, ns, o); nl += __shfl_xor_sync(0xffffffffu, nl, o); }
+    for (int o = 16; o > 0; o >>= 1) { ns += __shfl_xor_sync(kFull, ns, o); nl += __shfl_xor_sync(kFull, nl, o); }
     if (lane_id() == 0 && (ns | nl)) { atomicAdd(&nstart, ns); atomicAdd(&nlink, nl); }
     __syncthreads();
     if (threadIdx.x == 0) {
@@ -281,10 +316,10 @@ __global__ void __launch_bounds__(kSeedThreads) k_seeds(const View v) {
         const int k = k0 + threadIdx.x;
         bool st = false;
         if (k < n) st = v.clink_up[b0 + k] >= 0 && v.clink_dn[b0 + k] < 0;
-        const unsigned m = __ballot_sync(0xffffffffu, st);
+        const unsigned m = __ballot_sync(kFull, st);
         int basep = 0;
         if (lane_id() == 0 && m) basep = atomicAdd(&fill, __popc(m));
-        basep = __shfl_sync(0xffffffffu, basep, 0);
+        basep = __shfl_sync(kFull, basep, 0);
         if (st) {
             const int p = basep + __popc(m & ((1u << lane_id()) - 1u));
             list_h[p] = b0 + k;

@@ -10,13 +10,14 @@ namespace tpc {
 
 constexpr int kCellPad = 32;          // cell table of a bin holds up to n_hits + kCellPad entries
 constexpr float kGridPad = 1.0e-3f;   // cm added to every grid query so that rounding never hides a candidate
-constexpr int kChunk = 32;            // tracklets per table chunk: table[chunk][row][lane]
+constexpr uint16_t kNoHit = 0xffffu;  // empty entry of a tracklet's row -> hit table (hits are row-local, < 2048)
+constexpr unsigned kFull = 0xffffffffu;
 
 // error bits raised by kernels
 constexpr unsigned kErrBadRow = 1u, kErrRowCapacity = 2u, kErrSeedCapacity = 4u;
 
 // device counters (unsigned long long each)
-enum { CNT_ERR = 0, CNT_LINKS, CNT_ROW_VISITS, CNT_TL_HITS, CNT_TRACKS, CNT_TRACK_HITS, CNT_N };
+enum { CNT_ERR = 0, CNT_LINKS, CNT_ROW_VISITS, CNT_TL_HITS, CNT_TRACKS, CNT_TRACK_HITS, CNT_CURSOR, CNT_N };
 
 // One event's input arrays (device pointers) and its place in the batch-global cluster numbering.
 struct EventSrc {
@@ -35,6 +36,13 @@ struct Const {
     tpc_params p;
 };
 
+// One (task,row) bin after K1: where its hits are and the uniform (y,z) grid laid over them.  32 bytes = one
+// sector; the second half alone (base, n, ny, nz) serves the paths that only need the hit range.
+struct __align__(16) BinDesc {
+    float y0, z0, idy, idz;   // cell = (int)((y - y0) * idy), (int)((z - z0) * idz), clamped
+    int32_t base, n, ny, nz;  // first sorted hit (batch-global), hits, grid dims
+};
+
 // Everything a kernel may touch, for one batch.
 struct View {
     int32_t n_events, n_tasks, n_bins, N;
@@ -44,11 +52,10 @@ struct View {
     int32_t* bin_count;      // [n_bins+1]
     int32_t* bin_start;      // [n_bins+1] exclusive scan of bin_count
     uint16_t* slot;          // [N] position of a cluster inside its bin, arrival order (batch-global cluster order)
-    float* ty; float* tz; int32_t* tidx; // [N] bucketed, unsorted
-    float* sy; float* sz; int32_t* sorig; // [N] sorted by (task,row,cell,index); sorig = caller's index in its event
-    float4* grid_f;          // [n_bins] y0, z0, 1/dy, 1/dz
-    int2* grid_n;            // [n_bins] ny, nz
-    uint16_t* cells;         // [N + n_bins*kCellPad] first hit of each cell, relative to bin_start
+    float2* thit; int32_t* tidx;   // [N] bucketed, unsorted: (y,z), caller's index
+    float2* shit; int32_t* sorig;  // [N] sorted by (task,row,cell): (y,z), caller's index in its event
+    BinDesc* desc;           // [n_bins]
+    uint16_t* cells;         // [N + n_bins*kCellPad] first hit of each cell, relative to the bin's base
     // K2-K4
     int32_t *link_up, *link_dn, *clink_up, *clink_dn; // [N] batch-global sorted index or -1
     int32_t* seed_count;     // [n_bins+1]
@@ -57,7 +64,8 @@ struct View {
     int32_t* seed_bin;       // [S_cap]
     int32_t S_cap;
     // K5
-    int32_t* tl_table;       // [S_cap/32][n_rows][32] sorted index or -1
+    uint16_t* tl_tab;        // [S_cap][tab_stride] row -> row-local hit or kNoHit; valid for first_row..last_row
+    int32_t tab_stride;
     int32_t* tl_rows;        // [S_cap] first_row | last_row << 8 | n_hits << 16
     float* tl_par;           // [6][S_cap] y z s t q chi2
     // K6
@@ -74,52 +82,31 @@ struct View {
 };
 
 __device__ __forceinline__ int lane_id() { return threadIdx.x & 31; }
+__device__ __forceinline__ unsigned lanemask_lt() { return (1u << lane_id()) - 1u; }
 
-// Row grid of one bin.
-struct RowGrid {
-    float y0, z0, idy, idz;
-    int ny, nz;
-    int base;              // bin_start
-    const uint16_t* cs;    // cell table of this bin
-    __device__ __forceinline__ int cy(float y) const {
-        int i = (int)((y - y0) * idy);
-        return max(0, min(i, ny - 1));
-    }
-    __device__ __forceinline__ int cz(float z) const {
-        int i = (int)((z - z0) * idz);
-        return max(0, min(i, nz - 1));
-    }
-};
-
-__device__ __forceinline__ RowGrid load_grid(const View& v, int bin) {
-    RowGrid g;
-    const float4 f = __ldg(&v.grid_f[bin]);
-    const int2 n = __ldg(&v.grid_n[bin]);
-    g.y0 = f.x; g.z0 = f.y; g.idy = f.z; g.idz = f.w; g.ny = n.x; g.nz = n.y;
-    g.base = __ldg(&v.bin_start[bin]);
-    g.cs = v.cells + (size_t)g.base + (size_t)bin * kCellPad;
-    return g;
+__device__ __forceinline__ int4 load_desc_n(const View& v, int bin) {   // base, n, ny, nz
+    return __ldg(reinterpret_cast<const int4*>(&v.desc[bin]) + 1);
+}
+__device__ __forceinline__ float4 load_desc_f(const View& v, int bin) { // y0, z0, idy, idz
+    return __ldg(reinterpret_cast<const float4*>(&v.desc[bin]));
+}
+__device__ __forceinline__ const uint16_t* cell_table(const View& v, int bin, int base) {
+    return v.cells + (size_t)base + (size_t)bin * kCellPad;
 }
 
-// Walks the hits of all cells overlapping [y-wy, y+wy] x [z-wz, z+wz] (padded); exact tests are the caller's.
-struct GridIter {
-    const uint16_t* cs;
-    int base, ny, iy0, iy1, iz, iz1, p, pend;
-    __device__ __forceinline__ void start(const RowGrid& g, float y, float z, float wy, float wz) {
-        cs = g.cs; base = g.base; ny = g.ny;
-        iy0 = g.cy(y - wy - kGridPad); iy1 = g.cy(y + wy + kGridPad);
-        iz = g.cz(z - wz - kGridPad) - 1; iz1 = g.cz(z + wz + kGridPad);
-        p = 0; pend = 0;
-    }
-    __device__ __forceinline__ bool next(int& h) {
-        while (p >= pend) {
-            if (++iz > iz1) return false;
-            p = base + cs[iz * ny + iy0];
-            pend = base + cs[iz * ny + iy1 + 1];
-        }
-        h = p++;
-        return true;
-    }
-};
+__device__ __forceinline__ int grid_cell(float v, float v0, float iv, int n) {
+    const int i = (int)((v - v0) * iv);
+    return max(0, min(i, n - 1));
+}
+
+// Cell window of [y-wy, y+wy] x [z-wz, z+wz] (padded) in the grid (gf, ny, nz): columns iy0..iy1, rows iz0..iz1.
+// A grid row's candidates are the contiguous hits cs[iz*ny+iy0] .. cs[iz*ny+iy1+1]; exact tests are the caller's.
+struct CellWin { int iy0, iy1, iz0, iz1; };
+__device__ __forceinline__ CellWin cell_window(const float4& gf, int ny, int nz, float y, float z, float wy, float wz) {
+    CellWin w;
+    w.iy0 = grid_cell(y - wy - kGridPad, gf.x, gf.z, ny); w.iy1 = grid_cell(y + wy + kGridPad, gf.x, gf.z, ny);
+    w.iz0 = grid_cell(z - wz - kGridPad, gf.y, gf.w, nz); w.iz1 = grid_cell(z + wz + kGridPad, gf.y, gf.w, nz);
+    return w;
+}
 
 }  // namespace tpc

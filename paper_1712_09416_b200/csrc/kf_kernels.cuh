@@ -119,224 +119,262 @@ __device__ __forceinline__ void fit_update(Fit& f, float my, float mz, const Con
     f.n++;
 }
 
-// best hit of bin (task,row) inside the window of the predicted state, or -1
-__device__ __forceinline__ int fit_search(const Fit& f, const View& v, int bin, const Const& c) {
-    if (v.bin_start[bin + 1] == v.bin_start[bin]) return -1;
+// best hit of bin (task,row) inside the window of the predicted state, or -1;
+// (*ay, *az) = its coordinates.  dn = second half of the bin's descriptor (base, n, ny, nz).
+__device__ __forceinline__ int fit_search(const Fit& f, const View& v, int bin, const int4& dn, const Const& c,
+                                          float* ay, float* az) {
+    if (dn.y == 0) return -1;
     const float wy = fminf(fmaxf(c.p.win_nsigma * sqrtf(f.c00 + c.sigma_y2), c.p.win_min), c.p.win_max);
     const float wz = fminf(fmaxf(c.p.win_nsigma * sqrtf(f.c11 + c.sigma_z2), c.p.win_min), c.p.win_max);
-    const RowGrid g = load_grid(v, bin);
-    GridIter it;
-    it.start(g, f.y, f.z, wy, wz);
-    int best = -1, bo = 0, h;
-    float gb = 0.f;
-    while (it.next(h)) {
-        const float y = v.sy[h], z = v.sz[h];
-        if (!(fabsf(y - f.y) <= wy && fabsf(z - f.z) <= wz)) continue;
-        const float gv = fit_gate(f, y, z, c);
-        bool take = best < 0 || gv < gb;
-        int o = 0;
-        if (!take && gv == gb) { o = v.sorig[h]; take = o < bo; }
-        else if (take) o = v.sorig[h];
-        if (take) { gb = gv; best = h; bo = o; }
+    const float iwy = 1.f / (f.c00 + c.sigma_y2), iwz = 1.f / (f.c11 + c.sigma_z2);
+    const float4 gf = load_desc_f(v, bin);
+    const CellWin w = cell_window(gf, dn.z, dn.w, f.y, f.z, wy, wz);
+    const uint16_t* cs = cell_table(v, bin, dn.x);
+    const float2* hits = v.shit + dn.x;
+    int best = -1;
+    float gb = 0.f, by = 0.f, bz = 0.f;
+    for (int iz = w.iz0; iz <= w.iz1; iz++) {
+        int p = __ldg(&cs[iz * dn.z + w.iy0]);
+        const int pe = __ldg(&cs[iz * dn.z + w.iy1 + 1]);
+        for (; p < pe; p++) {
+            const float2 h = __ldg(&hits[p]);
+            if (!(fabsf(h.x - f.y) <= wy && fabsf(h.y - f.z) <= wz)) continue;
+            const float ry = h.x - f.y, rz = h.y - f.z;
+            const float gv = (ry * ry) * iwy + (rz * rz) * iwz;   // = fit_gate(f, h.x, h.y, c)
+            bool take = best < 0 || gv < gb;
+            if (!take && gv == gb) take = v.sorig[dn.x + p] < v.sorig[dn.x + best];  // exact tie: lowest caller's index
+            if (take) { gb = gv; best = p; by = h.x; bz = h.y; }
+        }
     }
-    if (best < 0) return -1;
-    return (gb <= c.p.chi2_ext) ? best : -1;
+    if (best < 0 || !(gb <= c.p.chi2_ext)) return -1;
+    *ay = by; *az = bz;
+    return dn.x + best;
 }
 
-__device__ __forceinline__ int32_t* table_ptr(const View& v, int i, int nr) {
-    return v.tl_table + (size_t)(i / kChunk) * nr * kChunk + (i % kChunk);
+// selection key of tracklet i: more hits first, then the lower canonical id within the sector task
+__device__ __forceinline__ uint32_t tl_key(const View& v, int i, int nh, int task_bin0) {
+    const int id_in_task = i - v.seed_start[task_bin0];
+    return ((uint32_t)nh << 24) | (uint32_t)(0xffffff - id_in_task);
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// K5: one thread per start hit (grid-stride).  Up pass along the cleaned links, then extension by search;
-// down pass = fresh fit from the top hit through everything recorded, searching the empty rows.
+// K5 tracklet constructor.  Persistent CTAs; every lane runs one tracklet as a small state machine that
+// advances ONE pad row per loop trip (transport -> candidate -> update), so that the 32 lanes of a warp stay
+// on the same code whatever their tracklets' lengths; a lane whose tracklet is finished takes the next start
+// hit from a device counter at once.  The row -> hit table of the tracklet under construction lives in shared
+// memory ([thread][row], row-local 16-bit hit numbers); when a tracklet ends, its warp writes the rows
+// first..last of the table to HBM with coalesced stores and claims the hits for the selector (K6a: atomicMax of
+// the tracklet's key on owner[hit]).
+//   phase 1: up pass, following the cleaned links      phase 2: up pass, extending by search
+//   phase 3: down pass = fresh fit from the top hit through everything recorded, searching the empty rows
 // ---------------------------------------------------------------------------------------------------------
 constexpr int kKfThreads = 128;
+constexpr int kKfBlocksPerSM = 5;
 
-__global__ void __launch_bounds__(kKfThreads) k_construct(const View v, const __grid_constant__ Const c) {
+__host__ __device__ inline int kf_tab_pitch(int n_rows) {   // entries per thread; pitch/2 odd -> no bank conflicts
+    int p = (n_rows + 1) & ~1;                               // between lanes working on the same row
+    if (((p >> 1) & 1) == 0) p += 2;
+    return p;
+}
+
+__global__ void __launch_bounds__(kKfThreads, kKfBlocksPerSM) k_construct(const View v, const __grid_constant__ Const c) {
+    extern __shared__ uint16_t s_tab[];   // [kKfThreads][pitch]
     const int S = min(v.seed_start[v.n_bins], v.S_cap);
-    const int nr = c.n_rows;
-    unsigned long long visits = 0;
-    for (int i = blockIdx.x * kKfThreads + threadIdx.x; i < S; i += gridDim.x * kKfThreads) {
-        int32_t* tab = table_ptr(v, i, nr);  // tab[row * kChunk]
-        const int h0 = v.seeds[i];
-        const int bin0 = v.seed_bin[i];
-        const int r0 = bin0 % nr;
-        const int tb = bin0 - r0;  // first bin of this task
-        const int h1 = v.clink_up[h0];
-        Fit f;
-        {
-            const int D = c.p.link_step;
-            const float dx = c.row_x[r0 + D] - c.row_x[r0];
-            const float y0 = v.sy[h0], z0 = v.sz[h0];
-            const float dy = v.sy[h1] - y0, dz = v.sz[h1] - z0;
-            const float dl = sqrtf(dx * dx + dy * dy);
-            f.y = y0; f.z = z0; f.s = dy / dl; f.t = dz / dl; f.q = 0.f;
-            fit_prior(f, c); f.n = 1;
+    const int nr = c.n_rows, D = c.p.link_step;
+    const int pitch = kf_tab_pitch(nr);
+    const int lane = lane_id();
+    uint16_t* const mytab = s_tab + threadIdx.x * pitch;
+    uint16_t* const warptab = s_tab + (threadIdx.x & ~31) * pitch;
+    unsigned long long* const cursor = &v.cnt[CNT_CURSOR];
+
+    Fit f;
+    float p0 = 0.f, p1 = 0.f, p2 = 0.f, p3 = 0.f, p4 = 0.f, p5 = 0.f;  // up: top hit (y,z), s,t,q there; down: result
+    float cy = 0.f, cz = 0.f;    // coordinates of the hit the up pass follows next
+    int ph = 0;                  // 0 idle, 1 up/follow, 2 up/extend, 3 down
+    int i = -1, row = 0, r0 = 0, top = 0, first = 0, nh = 0, tb = 0, cur = -1, rcur = 0, miss = 0;
+    f.n = 0;
+    unsigned visits = 0, claimed = 0;
+    bool more = true;
+
+    for (;;) {
+        // ---- idle lanes take the next start hits ----
+        const unsigned idle = __ballot_sync(kFull, ph == 0);
+        if (idle && more) {
+            int b = 0;
+            if (lane == 0) b = (int)atomicAdd(cursor, (unsigned long long)__popc(idle));
+            b = __shfl_sync(kFull, b, 0);
+            if (b >= S) more = false;
+            const int cand = b + __popc(idle & lanemask_lt());
+            if (ph == 0 && cand < S) {
+                i = cand;
+                const int h0 = v.seeds[i];
+                const int bin0 = v.seed_bin[i];
+                r0 = bin0 % nr; tb = bin0 - r0;
+                const int h1 = v.clink_up[h0];
+                const float2 a0 = v.shit[h0], a1 = v.shit[h1];
+                const int base0 = load_desc_n(v, bin0).x;
+                const float dx = c.row_x[r0 + D] - c.row_x[r0];
+                const float dy = a1.x - a0.x, dz = a1.y - a0.y;
+                const float dl = sqrtf(dx * dx + dy * dy);
+                f.y = a0.x; f.z = a0.y; f.s = dy / dl; f.t = dz / dl; f.q = 0.f;
+                fit_prior(f, c); f.n = 1;
+                mytab[r0] = (uint16_t)(h0 - base0);
+                p0 = a0.x; p1 = a0.y; p2 = f.s; p3 = f.t; p4 = f.q;
+                top = r0; row = r0; cur = h1; rcur = r0 + D; cy = a1.x; cz = a1.y; miss = 0;
+                ph = 1;
+            }
         }
-        tab[r0 * kChunk] = h0;
-        float ss = f.s, st = f.t, sq = f.q;  // direction / curvature at the last accepted update
-        int top = r0;
-        // ---- up pass ----
-        {
-            bool follow = true;
-            int cur = h1, rcur = r0 + c.p.link_step, miss = 0;
-            float xc = c.row_x[r0];
-            for (int row = r0 + 1; row < nr; row++) {
-                if (!fit_transport(f, xc, c.row_x[row], c)) break;
+        if (__all_sync(kFull, ph == 0)) break;
+
+        // ---- one pad row ----
+        bool finished = false;
+        if (ph != 0) {
+            const bool up = ph != 3;
+            const int prev = row;
+            row += up ? 1 : -1;
+            bool end = up ? (row >= nr) : (row < 0);
+            int4 dn = make_int4(0, 0, 1, 1);
+            int nxt = -1, known = -1;
+            float ky = 0.f, kz = 0.f;
+            if (!end) {
+                // loads that do not depend on the fit are issued before the transport
+                dn = load_desc_n(v, tb + row);
+                if (ph == 1) {
+                    if (row == rcur) { known = cur; ky = cy; kz = cz; nxt = v.clink_up[cur]; }
+                } else if (ph == 3 && row >= r0) {
+                    const uint16_t e = mytab[row];
+                    if (e != kNoHit) { known = dn.x + e; const float2 hk = v.shit[known]; ky = hk.x; kz = hk.y; }
+                }
+                end = !fit_transport(f, c.row_x[prev], c.row_x[row], c);
+            }
+            if (!end) {
                 visits++;
-                xc = c.row_x[row];
                 int acc = -1;
-                bool stop = false;
-                if (follow && row < rcur) {
-                    // in-between row of a step-2 link: nothing to do
+                float ay = 0.f, az = 0.f;
+                bool search = false, counted = false;   // counted: the edge test and the gap count apply
+                if (ph == 1) {
+                    if (row == rcur) {
+                        if (fit_gate(f, ky, kz, c) <= c.p.chi2_link) {
+                            acc = known; ay = ky; az = kz;
+                            cur = nxt; rcur += D;
+                            if (cur < 0) ph = 2;
+                            else { const float2 hn = v.shit[cur]; cy = hn.x; cz = hn.y; }
+                        } else { ph = 2; search = true; counted = true; }
+                    }   // else: in-between row of a step-2 link
+                } else if (ph == 2) {
+                    search = true; counted = true;
                 } else {
-                    if (follow) {
-                        const float my = v.sy[cur], mz = v.sz[cur];
-                        if (fit_gate(f, my, mz, c) <= c.p.chi2_link) {
-                            acc = cur;
-                            cur = v.clink_up[cur];
-                            rcur += c.p.link_step;
-                            if (cur < 0) follow = false;
-                        } else {
-                            follow = false;
-                        }
-                    }
-                    if (acc < 0) {  // extend by search (also the row where following just failed)
-                        if (fabsf(f.y) > c.row_x[row] * c.tan_half_angle + c.p.edge_margin) stop = true;
-                        else {
-                            acc = fit_search(f, v, tb + row, c);
-                            if (acc >= 0) miss = 0;
-                            else if (++miss > c.p.max_gap) stop = true;
-                        }
+                    if (row >= r0) {
+                        if (known >= 0) { if (fit_gate(f, ky, kz, c) <= c.p.chi2_link) { acc = known; ay = ky; az = kz; } }
+                        else search = true;
+                    } else { search = true; counted = true; }
+                }
+                if (search) {
+                    if (counted && fabsf(f.y) > c.row_x[row] * c.tan_half_angle + c.p.edge_margin) end = true;
+                    else {
+                        acc = fit_search(f, v, tb + row, dn, c, &ay, &az);
+                        if (acc >= 0) miss = 0;
+                        else if (counted && ++miss > c.p.max_gap) end = true;
                     }
                 }
-                if (stop) break;
-                tab[row * kChunk] = acc;
-                if (acc >= 0) {
-                    fit_update(f, v.sy[acc], v.sz[acc], c);
-                    ss = f.s; st = f.t; sq = f.q; top = row;
+                if (!end) {
+                    mytab[row] = acc >= 0 ? (uint16_t)(acc - dn.x) : kNoHit;
+                    if (acc >= 0) {
+                        fit_update(f, ay, az, c);
+                        if (up) { p0 = ay; p1 = az; p2 = f.s; p3 = f.t; p4 = f.q; top = row; }
+                        else { p0 = f.y; p1 = f.z; p2 = f.s; p3 = f.t; p4 = f.q; p5 = f.chi2; first = row; nh = f.n; }
+                    }
+                }
+            }
+            if (end) {
+                if (up) {   // start the down pass at the top hit
+                    f.y = p0; f.z = p1; f.s = p2; f.t = p3; f.q = p4;
+                    fit_prior(f, c); f.n = 1;
+                    p5 = 0.f;
+                    row = top; first = top; nh = 1; miss = 0;
+                    ph = 3;
+                } else {
+                    finished = true;
                 }
             }
         }
-        // ---- down pass ----
-        int first = top, nh = 1;
-        float py, pz, ps, pt, pq, pchi2;
-        {
-            const int ht = tab[top * kChunk];
-            f.y = v.sy[ht]; f.z = v.sz[ht]; f.s = ss; f.t = st; f.q = sq;
-            fit_prior(f, c); f.n = 1;
-            py = f.y; pz = f.z; ps = f.s; pt = f.t; pq = f.q; pchi2 = f.chi2;
-            int miss = 0;
-            float xc = c.row_x[top];
-            int row = top - 1;
-            for (; row >= 0; row--) {
-                if (!fit_transport(f, xc, c.row_x[row], c)) break;
-                visits++;
-                xc = c.row_x[row];
-                const bool below = row < r0;
-                int acc = -1;
-                bool searched = false;
-                if (!below) {
-                    const int hr = tab[row * kChunk];
-                    if (hr >= 0) {
-                        if (fit_gate(f, v.sy[hr], v.sz[hr], c) <= c.p.chi2_link) acc = hr;
-                    } else searched = true;
-                } else searched = true;
-                if (searched) {
-                    if (below && fabsf(f.y) > c.row_x[row] * c.tan_half_angle + c.p.edge_margin) break;
-                    acc = fit_search(f, v, tb + row, c);
-                    if (acc >= 0) miss = 0;
-                    else if (below && ++miss > c.p.max_gap) break;
-                }
-                tab[row * kChunk] = acc;
-                if (acc >= 0) {
-                    fit_update(f, v.sy[acc], v.sz[acc], c);
-                    py = f.y; pz = f.z; ps = f.s; pt = f.t; pq = f.q; pchi2 = f.chi2;
-                    first = row; nh = f.n;
+
+        // ---- finished tracklets: parameters, table rows first..top to HBM, claim of the hits (K6a) ----
+        unsigned fin = __ballot_sync(kFull, finished);
+        if (fin) {
+            uint32_t key = 0;
+            if (finished) {
+                v.tl_rows[i] = first | (top << 8) | (nh << 16);
+                const int sc = v.S_cap;
+                v.tl_par[i] = p0; v.tl_par[sc + i] = p1; v.tl_par[2 * sc + i] = p2; v.tl_par[3 * sc + i] = p3;
+                v.tl_par[4 * sc + i] = p4; v.tl_par[5 * sc + i] = p5;
+                if (nh >= c.p.min_tracklet_hits) key = tl_key(v, i, nh, tb);
+                ph = 0;
+            }
+            __syncwarp();
+            while (fin) {
+                const int L = __ffs(fin) - 1;
+                fin &= fin - 1;
+                const int li = __shfl_sync(kFull, i, L), lfirst = __shfl_sync(kFull, first, L);
+                const int ltop = __shfl_sync(kFull, top, L), ltb = __shfl_sync(kFull, tb, L);
+                const uint32_t lkey = __shfl_sync(kFull, key, L);
+                const uint16_t* col = warptab + L * pitch;
+                uint16_t* gt = v.tl_tab + (size_t)li * v.tab_stride;
+                for (int r = lfirst + lane; r <= ltop; r += 32) {
+                    const uint16_t e = col[r];
+                    gt[r] = e;
+                    if (e != kNoHit && lkey) {
+                        atomicMax(&v.owner[load_desc_n(v, ltb + r).x + e], lkey);
+                        claimed++;
+                    }
                 }
             }
-            // rows the pass never reached keep nothing (only rows >= r0 can hold stale up-pass entries)
-            for (; row >= r0; row--) tab[row * kChunk] = -1;
+            __syncwarp();
         }
-        v.tl_rows[i] = first | (top << 8) | (nh << 16);
-        const int sc = v.S_cap;
-        v.tl_par[i] = py; v.tl_par[sc + i] = pz; v.tl_par[2 * sc + i] = ps; v.tl_par[3 * sc + i] = pt;
-        v.tl_par[4 * sc + i] = pq; v.tl_par[5 * sc + i] = pchi2;
     }
+    unsigned long long vs = visits, cl = claimed;
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) visits += __shfl_xor_sync(0xffffffffu, visits, o);
-    if (lane_id() == 0 && visits) atomicAdd(&v.cnt[CNT_ROW_VISITS], visits);
+    for (int o = 16; o > 0; o >>= 1) { vs += __shfl_xor_sync(kFull, vs, o); cl += __shfl_xor_sync(kFull, cl, o); }
+    if (lane == 0) {
+        if (vs) atomicAdd(&v.cnt[CNT_ROW_VISITS], vs);
+        if (cl) atomicAdd(&v.cnt[CNT_TL_HITS], cl);
+    }
 }
 
 // ---------------------------------------------------------------------------------------------------------
 // K6 selector.  key = n_hits << 24 | (2^24 - 1 - id within the task): larger = more hits, then lower
-// canonical id.  owner[hit] = max key over tracklets (n_hits >= min_tracklet_hits) holding the hit.
-// One warp per table chunk: lane = tracklet, loop over rows -> coalesced table reads.
+// canonical id.  owner[hit] = max key over tracklets (n_hits >= min_tracklet_hits) holding the hit (claimed by
+// K5 as each tracklet ends).  One warp per tracklet, lanes over its rows: coalesced table reads.
 // ---------------------------------------------------------------------------------------------------------
-__device__ __forceinline__ uint32_t tl_key(const View& v, int i, int nh, int nr) {
-    const int bin = v.seed_bin[i];
-    const int id_in_task = i - v.seed_start[bin - bin % nr];
-    return ((uint32_t)nh << 24) | (uint32_t)(0xffffff - id_in_task);
-}
-
 constexpr int kSelThreads = 128;
 
-__global__ void __launch_bounds__(kSelThreads) k_claim(const View v, const __grid_constant__ Const c) {
-    const int S = min(v.seed_start[v.n_bins], v.S_cap);
-    const int nr = c.n_rows;
-    const int chunk = (blockIdx.x * kSelThreads + threadIdx.x) / 32;
-    const int i = chunk * kChunk + lane_id();
-    if (chunk * kChunk >= S) return;
-    int first = nr, last = -1, nh = 0;
-    uint32_t key = 0;
-    if (i < S) {
-        const int pk = v.tl_rows[i];
-        nh = pk >> 16;
-        if (nh >= c.p.min_tracklet_hits) { first = pk & 0xff; last = (pk >> 8) & 0xff; key = tl_key(v, i, nh, nr); }
-    }
-    int lo = first, hi = last;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) { lo = min(lo, __shfl_xor_sync(0xffffffffu, lo, o)); hi = max(hi, __shfl_xor_sync(0xffffffffu, hi, o)); }
-    const int32_t* tab = v.tl_table + (size_t)chunk * nr * kChunk + lane_id();
-    int cnt = 0;
-    for (int row = lo; row <= hi; row++) {
-        if (row < first || row > last) continue;
-        const int h = tab[row * kChunk];
-        if (h >= 0) { atomicMax(&v.owner[h], key); cnt++; }
-    }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) cnt += __shfl_xor_sync(0xffffffffu, cnt, o);
-    if (lane_id() == 0 && cnt) atomicAdd(&v.cnt[CNT_TL_HITS], (unsigned long long)cnt);
-}
-
+// K6b: hits each tracklet owns; a track is kept when it owns at least min_track_hits
 __global__ void __launch_bounds__(kSelThreads) k_count_owned(const View v, const __grid_constant__ Const c) {
     const int S = min(v.seed_start[v.n_bins], v.S_cap);
     const int nr = c.n_rows;
-    const int chunk = (blockIdx.x * kSelThreads + threadIdx.x) / 32;
-    const int i = chunk * kChunk + lane_id();
-    if (chunk * kChunk >= S) return;
-    int first = nr, last = -1, nh = 0;
-    uint32_t key = 0;
-    if (i < S) {
-        const int pk = v.tl_rows[i];
-        nh = pk >> 16;
-        if (nh >= c.p.min_tracklet_hits) { first = pk & 0xff; last = (pk >> 8) & 0xff; key = tl_key(v, i, nh, nr); }
-    }
-    int lo = first, hi = last;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) { lo = min(lo, __shfl_xor_sync(0xffffffffu, lo, o)); hi = max(hi, __shfl_xor_sync(0xffffffffu, hi, o)); }
-    const int32_t* tab = v.tl_table + (size_t)chunk * nr * kChunk + lane_id();
+    const int lane = lane_id();
+    for (int i = (blockIdx.x * kSelThreads + threadIdx.x) >> 5; i < S; i += (gridDim.x * kSelThreads) >> 5) {
+    const int pk = v.tl_rows[i];
+    const int nh = pk >> 16;
     int own = 0;
-    for (int row = lo; row <= hi; row++) {
-        if (row < first || row > last) continue;
-        const int h = tab[row * kChunk];
-        if (h >= 0 && v.owner[h] == key) own++;
+    if (nh >= c.p.min_tracklet_hits) {
+        const int first = pk & 0xff, last = (pk >> 8) & 0xff;
+        const int bin = v.seed_bin[i];
+        const int tb = bin - bin % nr;
+        const uint32_t key = tl_key(v, i, nh, tb);
+        const uint16_t* gt = v.tl_tab + (size_t)i * v.tab_stride;
+        for (int r = first + lane; r <= last; r += 32) {
+            const uint16_t e = gt[r];
+            if (e != kNoHit && v.owner[load_desc_n(v, tb + r).x + e] == key) own++;
+        }
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) own += __shfl_xor_sync(kFull, own, o);
     }
-    if (i < S) {
+    if (lane == 0) {
         const int keep = own >= c.p.min_track_hits;
         v.tl_keep[i] = keep;
         v.tl_nown[i] = keep ? own : 0;
+    }
     }
 }
 
@@ -351,20 +389,21 @@ __global__ void k_event_offsets(const View v, int bins_per_event) {
     if (e == v.n_events) { v.cnt[CNT_TRACKS] = (unsigned long long)v.trk_scan[s]; v.cnt[CNT_TRACK_HITS] = (unsigned long long)v.hit_scan[s]; }
 }
 
+// K6c: output tracks in canonical order; hit lists row-ascending (ballot + prefix popcount keeps the order)
 __global__ void __launch_bounds__(kSelThreads) k_write_tracks(const View v, const __grid_constant__ Const c) {
     const int S = min(v.seed_start[v.n_bins], v.S_cap);
     const int nr = c.n_rows;
-    const int chunk = (blockIdx.x * kSelThreads + threadIdx.x) / 32;
-    const int i = chunk * kChunk + lane_id();
-    if (chunk * kChunk >= S) return;
-    int first = nr, last = -1, nh = 0, ho = 0;
-    uint32_t key = 0;
-    if (i < S && v.tl_keep[i]) {
-        const int pk = v.tl_rows[i];
-        nh = pk >> 16; first = pk & 0xff; last = (pk >> 8) & 0xff; key = tl_key(v, i, nh, nr);
+    const int lane = lane_id();
+    for (int i = (blockIdx.x * kSelThreads + threadIdx.x) >> 5; i < S; i += (gridDim.x * kSelThreads) >> 5) {
+    if (!v.tl_keep[i]) continue;
+    const int pk = v.tl_rows[i];
+    const int nh = pk >> 16, first = pk & 0xff, last = (pk >> 8) & 0xff;
+    const int bin = v.seed_bin[i];
+    const int tb = bin - bin % nr;
+    const uint32_t key = tl_key(v, i, nh, tb);
+    int ho = v.hit_scan[i];
+    if (lane == 0) {
         const int ti = v.trk_scan[i];
-        ho = v.hit_scan[i];
-        const int bin = v.seed_bin[i];
         const int task = bin / nr;
         const int e = task / c.n_sectors;
         const int sc = v.S_cap;
@@ -376,14 +415,18 @@ __global__ void __launch_bounds__(kSelThreads) k_write_tracks(const View v, cons
         v.o_y[ti] = v.tl_par[i]; v.o_z[ti] = v.tl_par[sc + i]; v.o_sinphi[ti] = v.tl_par[2 * sc + i];
         v.o_tgl[ti] = v.tl_par[3 * sc + i]; v.o_qpt[ti] = v.tl_par[4 * sc + i]; v.o_chi2[ti] = v.tl_par[5 * sc + i];
     }
-    int lo = first, hi = last;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) { lo = min(lo, __shfl_xor_sync(0xffffffffu, lo, o)); hi = max(hi, __shfl_xor_sync(0xffffffffu, hi, o)); }
-    const int32_t* tab = v.tl_table + (size_t)chunk * nr * kChunk + lane_id();
-    for (int row = lo; row <= hi; row++) {
-        if (row < first || row > last) continue;
-        const int h = tab[row * kChunk];
-        if (h >= 0 && v.owner[h] == key) v.o_hit_idx[ho++] = v.sorig[h];
+    const uint16_t* gt = v.tl_tab + (size_t)i * v.tab_stride;
+    for (int r0 = first; r0 <= last; r0 += 32) {
+        const int r = r0 + lane;
+        int h = -1;
+        if (r <= last) {
+            const uint16_t e = gt[r];
+            if (e != kNoHit) { h = load_desc_n(v, tb + r).x + e; if (v.owner[h] != key) h = -1; }
+        }
+        const unsigned m = __ballot_sync(kFull, h >= 0);
+        if (h >= 0) v.o_hit_idx[ho + __popc(m & lanemask_lt())] = v.sorig[h];
+        ho += __popc(m);
+    }
     }
 }
 

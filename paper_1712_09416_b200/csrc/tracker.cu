@@ -65,6 +65,7 @@ struct tpc_tracker {
     std::vector<float> sector_alpha;
     cudaStream_t own_stream = nullptr, stream = nullptr;
     int sm_count = 148;
+    int kf_blocks = 148, kf_smem = 0;   // persistent constructor grid, bytes of its row -> hit tables
     // batch state
     View v;
     int n_events = 0;
@@ -74,13 +75,13 @@ struct tpc_tracker {
     tpc_counters counters;
     bool have_result = false;
     // device pools
-    Buf<float> in_y, in_z, ty, tz, sy, sz, tl_par, o_f[7];
+    Buf<float> in_y, in_z, tl_par, o_f[7];
+    Buf<float2> thit, shit;
     Buf<int32_t> in_row, sec_off, bin_count, bin_start, tidx, sorig, link_up, link_dn, clink_up, clink_dn, seed_count,
-        seed_start, seeds, seed_bin, tl_table, tl_rows, tl_nown, tl_keep, trk_scan, hit_scan, ev_off_d, scratch,
+        seed_start, seeds, seed_bin, tl_rows, tl_nown, tl_keep, trk_scan, hit_scan, ev_off_d, scratch,
         o_i[4], o_hit;
-    Buf<uint16_t> slot, cells;
-    Buf<float4> grid_f;
-    Buf<int2> grid_n;
+    Buf<uint16_t> slot, cells, tl_tab;
+    Buf<BinDesc> desc;
     Buf<uint32_t> owner;
     Buf<EventSrc> ev_src;
     Buf<unsigned long long> cnt;
@@ -102,15 +103,15 @@ struct tpc_tracker {
         memset(&counters, 0, sizeof counters);
     }
     void free_all() {
-        in_y.release(); in_z.release(); ty.release(); tz.release(); sy.release(); sz.release(); tl_par.release();
+        in_y.release(); in_z.release(); thit.release(); shit.release(); tl_par.release();
         for (auto& b : o_f) b.release();
         in_row.release(); sec_off.release(); bin_count.release(); bin_start.release(); tidx.release(); sorig.release();
         link_up.release(); link_dn.release(); clink_up.release(); clink_dn.release(); seed_count.release();
-        seed_start.release(); seeds.release(); seed_bin.release(); tl_table.release(); tl_rows.release();
+        seed_start.release(); seeds.release(); seed_bin.release(); tl_tab.release(); tl_rows.release();
         tl_nown.release(); tl_keep.release(); trk_scan.release(); hit_scan.release(); ev_off_d.release();
         scratch.release(); o_hit.release();
         for (auto& b : o_i) b.release();
-        slot.release(); cells.release(); grid_f.release(); grid_n.release(); owner.release(); ev_src.release();
+        slot.release(); cells.release(); desc.release(); owner.release(); ev_src.release();
         cnt.release(); h_ev_src.release(); h_sec_off.release(); h_ev_off.release(); h_o_hit.release(); h_cnt.release();
         for (auto& b : h_o_i) b.release();
         for (auto& b : h_o_f) b.release();
@@ -118,6 +119,8 @@ struct tpc_tracker {
 };
 
 namespace {
+
+int tab_stride(int n_rows) { return (n_rows + 31) & ~31; }
 
 int reserve_batch(tpc_tracker* t, int n_events, int64_t N, int64_t S_cap) {
     const int64_t nb = (int64_t)n_events * t->c.n_sectors * t->c.n_rows;
@@ -127,11 +130,11 @@ int reserve_batch(tpc_tracker* t, int n_events, int64_t N, int64_t S_cap) {
     RS(sec_off, (size_t)n_events * (t->c.n_sectors + 1)); RS(h_sec_off, (size_t)n_events * (t->c.n_sectors + 1));
     RS(ev_src, n_events); RS(h_ev_src, n_events);
     RS(bin_count, nb + 1); RS(bin_start, nb + 1); RS(seed_count, nb + 1); RS(seed_start, nb + 1);
-    RS(slot, n); RS(ty, n); RS(tz, n); RS(tidx, n); RS(sy, n); RS(sz, n); RS(sorig, n);
-    RS(grid_f, nb); RS(grid_n, nb); RS(cells, n + (size_t)nb * kCellPad + 64);
+    RS(slot, n); RS(thit, n); RS(tidx, n); RS(shit, n); RS(sorig, n);
+    RS(desc, nb); RS(cells, n + (size_t)nb * kCellPad + 64);
     RS(link_up, n); RS(link_dn, n); RS(clink_up, n); RS(clink_dn, n); RS(owner, n);
     RS(seeds, S_cap); RS(seed_bin, S_cap); RS(tl_rows, S_cap); RS(tl_par, 6 * (size_t)S_cap);
-    RS(tl_table, ((size_t)S_cap / kChunk + 1) * t->c.n_rows * kChunk);
+    RS(tl_tab, (size_t)S_cap * tab_stride(t->c.n_rows));
     RS(tl_nown, S_cap + 1); RS(tl_keep, S_cap + 1); RS(trk_scan, S_cap + 2); RS(hit_scan, S_cap + 2);
     RS(ev_off_d, 2 * ((size_t)n_events + 1)); RS(h_ev_off, 2 * ((size_t)n_events + 1));
     RS(scratch, (size_t)std::max<int64_t>(nb, S_cap) / kScanTile + 8);
@@ -199,14 +202,9 @@ int launch_all(tpc_tracker* t, int64_t* launches) {
     L += scan_exclusive(v.seed_count, v.seed_start, nb, t->scratch.p, st);
     k_seeds<<<nb, kSeedThreads, 0, st>>>(v); L++;
     mark(3);
-    {
-        const int blocks = (int)std::min<int64_t>((t->S_cap + kKfThreads - 1) / kKfThreads, (int64_t)t->sm_count * 16);
-        k_construct<<<std::max(blocks, 1), kKfThreads, 0, st>>>(v, c); L++;
-    }
+    k_construct<<<t->kf_blocks, kKfThreads, t->kf_smem, st>>>(v, c); L++;   // also claims the hits (K6a)
     mark(4);
-    const int chunks = (int)((t->S_cap + kChunk - 1) / kChunk);
-    const int sel_blocks = std::max(1, (chunks * 32 + kSelThreads - 1) / kSelThreads);
-    k_claim<<<sel_blocks, kSelThreads, 0, st>>>(v, c); L++;
+    const int sel_blocks = t->sm_count * 16;
     k_count_owned<<<sel_blocks, kSelThreads, 0, st>>>(v, c); L++;
     // scans run over the whole seed capacity; entries beyond the seed count are zeroed first
     L += scan_exclusive(v.tl_keep, v.trk_scan, (int)t->S_cap, t->scratch.p, st);
@@ -290,6 +288,18 @@ tpc_tracker* tpc_tracker_create_ex(const tpc_geometry* g, float bz, const tpc_pa
         return nullptr;
     }
     t->stream = t->own_stream;
+    {   // constructor: one CTA's row -> hit tables in dynamic shared memory, as many CTAs as fit
+        t->kf_smem = kKfThreads * kf_tab_pitch(g->n_rows) * (int)sizeof(uint16_t);
+        int per_sm = 0;
+        if (cudaFuncSetAttribute(k_construct, cudaFuncAttributeMaxDynamicSharedMemorySize, t->kf_smem) != cudaSuccess ||
+            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_construct, kKfThreads, t->kf_smem) != cudaSuccess ||
+            per_sm < 1) {
+            set_err("k_construct cannot be configured: %s", cudaGetErrorString(cudaGetLastError()));
+            cudaStreamDestroy(t->own_stream); delete t;
+            return nullptr;
+        }
+        t->kf_blocks = t->sm_count * per_sm;
+    }
     if (max_events > 0 && max_clusters > 0) {
         if (reserve_batch(t, max_events, max_clusters, default_seed_cap(max_clusters)) != TPC_OK) {
             t->free_all(); cudaStreamDestroy(t->own_stream); delete t;
@@ -364,12 +374,12 @@ int tpc_track_events(tpc_tracker* t, int32_t n, const tpc_event_in* in, tpc_even
         v.n_events = n; v.n_tasks = n * ns; v.n_bins = n * ns * nr; v.N = (int32_t)N;
         v.ev = t->ev_src.p; v.sec_off = t->sec_off.p;
         v.bin_count = t->bin_count.p; v.bin_start = t->bin_start.p; v.slot = t->slot.p;
-        v.ty = t->ty.p; v.tz = t->tz.p; v.tidx = t->tidx.p; v.sy = t->sy.p; v.sz = t->sz.p; v.sorig = t->sorig.p;
-        v.grid_f = t->grid_f.p; v.grid_n = t->grid_n.p; v.cells = t->cells.p;
+        v.thit = t->thit.p; v.tidx = t->tidx.p; v.shit = t->shit.p; v.sorig = t->sorig.p;
+        v.desc = t->desc.p; v.cells = t->cells.p;
         v.link_up = t->link_up.p; v.link_dn = t->link_dn.p; v.clink_up = t->clink_up.p; v.clink_dn = t->clink_dn.p;
         v.seed_count = t->seed_count.p; v.seed_start = t->seed_start.p; v.seeds = t->seeds.p; v.seed_bin = t->seed_bin.p;
         v.S_cap = (int32_t)t->S_cap;
-        v.tl_table = t->tl_table.p; v.tl_rows = t->tl_rows.p; v.tl_par = t->tl_par.p;
+        v.tl_tab = t->tl_tab.p; v.tab_stride = tab_stride(nr); v.tl_rows = t->tl_rows.p; v.tl_par = t->tl_par.p;
         v.owner = t->owner.p; v.tl_nown = t->tl_nown.p; v.tl_keep = t->tl_keep.p;
         v.trk_scan = t->trk_scan.p; v.hit_scan = t->hit_scan.p; v.ev_off = t->ev_off_d.p;
         v.o_sector = t->o_i[0].p; v.o_first_hit = t->o_i[1].p; v.o_n_hits = t->o_i[2].p; v.o_ndf = t->o_i[3].p;
@@ -553,16 +563,21 @@ int tpc_debug_get(tpc_tracker* t, int32_t what, int32_t event, void* buf, size_t
         }
         case TPC_DBG_TL_TABLE: {
             if (!s) return TPC_OK;
-            std::vector<int32_t> rows(s), tab;
+            const int stride = t->v.tab_stride;
+            std::vector<int32_t> rows(s), sbin(s);
+            std::vector<uint16_t> tab((size_t)s * stride);
+            const int bpe = t->c.n_sectors * nr;
+            std::vector<BinDesc> desc(bpe);
             CK(cudaMemcpy(rows.data(), t->v.tl_rows + s0, 4 * (size_t)s, cudaMemcpyDeviceToHost));
-            const int c0 = s0 / kChunk, c1 = (s1 - 1) / kChunk;
-            tab.resize((size_t)(c1 - c0 + 1) * nr * kChunk);
-            CK(cudaMemcpy(tab.data(), t->v.tl_table + (size_t)c0 * nr * kChunk, 4 * tab.size(), cudaMemcpyDeviceToHost));
+            CK(cudaMemcpy(sbin.data(), t->v.seed_bin + s0, 4 * (size_t)s, cudaMemcpyDeviceToHost));
+            CK(cudaMemcpy(tab.data(), t->v.tl_tab + (size_t)s0 * stride, 2 * tab.size(), cudaMemcpyDeviceToHost));
+            CK(cudaMemcpy(desc.data(), t->v.desc + (size_t)event * bpe, sizeof(BinDesc) * (size_t)bpe, cudaMemcpyDeviceToHost));
             for (int k = 0; k < s; k++) {
-                const int i = s0 + k;
                 const int first = rows[k] & 0xff, last = (rows[k] >> 8) & 0xff;
-                const int32_t* tp = tab.data() + (size_t)(i / kChunk - c0) * nr * kChunk + (i % kChunk);
-                for (int r = 0; r < nr; r++) ob[(size_t)k * nr + r] = (r >= first && r <= last) ? to_orig(tp[r * kChunk]) : -1;
+                const int tb = sbin[k] - sbin[k] % nr - event * bpe;   // first bin of the tracklet's task, event-local
+                const uint16_t* tp = tab.data() + (size_t)k * stride;
+                for (int r = 0; r < nr; r++)
+                    ob[(size_t)k * nr + r] = (r >= first && r <= last && tp[r] != kNoHit) ? to_orig(desc[tb + r].base + tp[r]) : -1;
             }
             return TPC_OK;
         }
