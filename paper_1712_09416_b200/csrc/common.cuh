@@ -17,7 +17,9 @@ constexpr unsigned kFull = 0xffffffffu;
 constexpr unsigned kErrBadRow = 1u, kErrRowCapacity = 2u, kErrSeedCapacity = 4u;
 
 // device counters (unsigned long long each)
-enum { CNT_ERR = 0, CNT_LINKS, CNT_ROW_VISITS, CNT_TL_HITS, CNT_TRACKS, CNT_TRACK_HITS, CNT_CURSOR, CNT_N };
+// CNT_CURSOR.. : one cursor per SM (K5 hands out the start hits SM by SM)
+constexpr int kMaxSM = 256;
+enum { CNT_ERR = 0, CNT_LINKS, CNT_ROW_VISITS, CNT_TL_HITS, CNT_TRACKS, CNT_TRACK_HITS, CNT_CURSOR, CNT_N = CNT_CURSOR + kMaxSM };
 
 // One event's input arrays (device pointers) and its place in the batch-global cluster numbering.
 struct EventSrc {

@@ -86,11 +86,11 @@ __device__ __forceinline__ float fit_gate(const Fit& f, float my, float mz, cons
     return (ry * ry) * wy + (rz * rz) * wz;
 }
 
-// two scalar updates, y then z
-__device__ __forceinline__ void fit_update(Fit& f, float my, float mz, const Const& c) {
+// two scalar updates, y then z; iwy = 1 / (C_yy + sigma_y^2) of the predicted state
+__device__ __forceinline__ void fit_update(Fit& f, float my, float mz, float iwy, const Const& c) {
     {
         const float r = my - f.y;
-        const float w = 1.f / (f.c00 + c.sigma_y2);
+        const float w = iwy;
         const float k0 = f.c00, k1 = f.c10, k2 = f.c20, k3 = f.c30, k4 = f.c40;
         const float g0 = k0 * w, g1 = k1 * w, g2 = k2 * w, g3 = k3 * w, g4 = k4 * w;
         f.y = f.y + g0 * r; f.z = f.z + g1 * r; f.s = f.s + g2 * r; f.t = f.t + g3 * r; f.q = f.q + g4 * r;
@@ -119,38 +119,6 @@ __device__ __forceinline__ void fit_update(Fit& f, float my, float mz, const Con
     f.n++;
 }
 
-// best hit of bin (task,row) inside the window of the predicted state, or -1;
-// (*ay, *az) = its coordinates.  dn = second half of the bin's descriptor (base, n, ny, nz).
-__device__ __forceinline__ int fit_search(const Fit& f, const View& v, int bin, const int4& dn, const Const& c,
-                                          float* ay, float* az) {
-    if (dn.y == 0) return -1;
-    const float wy = fminf(fmaxf(c.p.win_nsigma * sqrtf(f.c00 + c.sigma_y2), c.p.win_min), c.p.win_max);
-    const float wz = fminf(fmaxf(c.p.win_nsigma * sqrtf(f.c11 + c.sigma_z2), c.p.win_min), c.p.win_max);
-    const float iwy = 1.f / (f.c00 + c.sigma_y2), iwz = 1.f / (f.c11 + c.sigma_z2);
-    const float4 gf = load_desc_f(v, bin);
-    const CellWin w = cell_window(gf, dn.z, dn.w, f.y, f.z, wy, wz);
-    const uint16_t* cs = cell_table(v, bin, dn.x);
-    const float2* hits = v.shit + dn.x;
-    int best = -1;
-    float gb = 0.f, by = 0.f, bz = 0.f;
-    for (int iz = w.iz0; iz <= w.iz1; iz++) {
-        int p = __ldg(&cs[iz * dn.z + w.iy0]);
-        const int pe = __ldg(&cs[iz * dn.z + w.iy1 + 1]);
-        for (; p < pe; p++) {
-            const float2 h = __ldg(&hits[p]);
-            if (!(fabsf(h.x - f.y) <= wy && fabsf(h.y - f.z) <= wz)) continue;
-            const float ry = h.x - f.y, rz = h.y - f.z;
-            const float gv = (ry * ry) * iwy + (rz * rz) * iwz;   // = fit_gate(f, h.x, h.y, c)
-            bool take = best < 0 || gv < gb;
-            if (!take && gv == gb) take = v.sorig[dn.x + p] < v.sorig[dn.x + best];  // exact tie: lowest caller's index
-            if (take) { gb = gv; best = p; by = h.x; bz = h.y; }
-        }
-    }
-    if (best < 0 || !(gb <= c.p.chi2_ext)) return -1;
-    *ay = by; *az = bz;
-    return dn.x + best;
-}
-
 // selection key of tracklet i: more hits first, then the lower canonical id within the sector task
 __device__ __forceinline__ uint32_t tl_key(const View& v, int i, int nh, int task_bin0) {
     const int id_in_task = i - v.seed_start[task_bin0];
@@ -161,51 +129,74 @@ __device__ __forceinline__ uint32_t tl_key(const View& v, int i, int nh, int tas
 // K5 tracklet constructor.  Persistent CTAs; every lane runs one tracklet as a small state machine that
 // advances ONE pad row per loop trip (transport -> candidate -> update), so that the 32 lanes of a warp stay
 // on the same code whatever their tracklets' lengths; a lane whose tracklet is finished takes the next start
-// hit from a device counter at once.  The row -> hit table of the tracklet under construction lives in shared
-// memory ([thread][row], row-local 16-bit hit numbers); when a tracklet ends, its warp writes the rows
-// first..last of the table to HBM with coalesced stores and claims the hits for the selector (K6a: atomicMax of
-// the tracklet's key on owner[hit]).
+// hit from a device counter at once.
 //   phase 1: up pass, following the cleaned links      phase 2: up pass, extending by search
 //   phase 3: down pass = fresh fit from the top hit through everything recorded, searching the empty rows
+// Window searches are shared out over the warp: every lane that needs one posts its
+// query (predicted y, z, window, weights, cell window) in shared memory; the queries are cut into work items
+// of one grid row each (the candidates of a grid row are contiguous in memory) and the 32 lanes take one item
+// each; the owner lane then merges its items' results.  The best hit = min gate value, exact ties -> lowest
+// caller's index, whatever the order of evaluation.
+// The row -> hit table of a tracklet ([tracklet][row], row-local 16-bit hit numbers) is written as the passes
+// go; when a tracklet ends, its warp claims the hits of rows first..last for the selector (K6a: atomicMax of the
+// tracklet's key on owner[hit]).
 // ---------------------------------------------------------------------------------------------------------
 constexpr int kKfThreads = 128;
 constexpr int kKfBlocksPerSM = 5;
+constexpr int kKfUnroll = 4;       // candidates of a grid row loaded at once
+constexpr int kKfMaxItems = 256;   // >= 32 lanes x grid rows a window can span (window <= 2 * 3 cm + pad, cells >= 1.2 cm)
 
-__host__ __device__ inline int kf_tab_pitch(int n_rows) {   // entries per thread; pitch/2 odd -> no bank conflicts
-    int p = (n_rows + 1) & ~1;                               // between lanes working on the same row
-    if (((p >> 1) & 1) == 0) p += 2;
-    return p;
-}
+struct SearchQuery {
+    float y, z, wy, wz, iwy, iwz;  // predicted position, window half widths, 1 / (C + sigma^2)
+    int32_t base, bin;             // first sorted hit of the bin, the bin
+    uint32_t win;                  // ny | iy0 << 8 | iy1 << 16 | iz0 << 24
+};
 
 __global__ void __launch_bounds__(kKfThreads, kKfBlocksPerSM) k_construct(const View v, const __grid_constant__ Const c) {
-    extern __shared__ uint16_t s_tab[];   // [kKfThreads][pitch]
+    __shared__ SearchQuery s_q[kKfThreads];
+    __shared__ float4 s_res[kKfThreads];                       // result of the item a lane took: gate, y, z, hit
+    __shared__ uint16_t s_item[kKfThreads / 32][kKfMaxItems];  // owner lane | grid row within the window << 8
     const int S = min(v.seed_start[v.n_bins], v.S_cap);
     const int nr = c.n_rows, D = c.p.link_step;
-    const int pitch = kf_tab_pitch(nr);
     const int lane = lane_id();
-    uint16_t* const mytab = s_tab + threadIdx.x * pitch;
-    uint16_t* const warptab = s_tab + (threadIdx.x & ~31) * pitch;
-    unsigned long long* const cursor = &v.cnt[CNT_CURSOR];
+    const int wbase = threadIdx.x & ~31;
+    uint16_t* const items = s_item[threadIdx.x >> 5];
+    unsigned long long* const cursor = &v.cnt[CNT_CURSOR];   // [n_sm] start hits taken from each SM's share
+    unsigned sm, n_sm_u;
+    asm("mov.u32 %0, %%smid;" : "=r"(sm));
+    asm("mov.u32 %0, %%nsmid;" : "=r"(n_sm_u));
+    const int n_sm = (int)n_sm_u;
+    int victim = 0;   // SMs whose share this warp has found exhausted, starting with its own
 
     Fit f;
     float p0 = 0.f, p1 = 0.f, p2 = 0.f, p3 = 0.f, p4 = 0.f, p5 = 0.f;  // up: top hit (y,z), s,t,q there; down: result
     float cy = 0.f, cz = 0.f;    // coordinates of the hit the up pass follows next
     int ph = 0;                  // 0 idle, 1 up/follow, 2 up/extend, 3 down
-    int i = -1, row = 0, r0 = 0, top = 0, first = 0, nh = 0, tb = 0, cur = -1, rcur = 0, miss = 0;
+    int i = 0, row = 0, r0 = 0, top = 0, first = 0, nh = 0, tb = 0, cur = -1, rcur = 0, miss = 0;
+    uint16_t enext = kNoHit;     // down pass: table entry of the row below, loaded one trip ahead
     f.n = 0;
     unsigned visits = 0, claimed = 0;
     bool more = true;
 
     for (;;) {
-        // ---- idle lanes take the next start hits ----
+        // ---- idle lanes take the next start hits: first from this SM's share of the list, then from the others' ----
         const unsigned idle = __ballot_sync(kFull, ph == 0);
         if (idle && more) {
-            int b = 0;
-            if (lane == 0) b = (int)atomicAdd(cursor, (unsigned long long)__popc(idle));
-            b = __shfl_sync(kFull, b, 0);
-            if (b >= S) more = false;
+            int b = 0, e = 0;
+            if (lane == 0) {
+                const int want = __popc(idle);
+                while (victim < n_sm) {
+                    const int s = (sm + victim) % n_sm;
+                    const int lo = (int)((long long)S * s / n_sm), hi = (int)((long long)S * (s + 1) / n_sm);
+                    const int got = lo + (int)atomicAdd(&cursor[s], (unsigned long long)want);
+                    if (got < hi) { b = got; e = hi; break; }
+                    victim++;
+                }
+            }
+            b = __shfl_sync(kFull, b, 0); e = __shfl_sync(kFull, e, 0); victim = __shfl_sync(kFull, victim, 0);
+            if (victim >= n_sm) more = false;
             const int cand = b + __popc(idle & lanemask_lt());
-            if (ph == 0 && cand < S) {
+            if (ph == 0 && cand < e) {
                 i = cand;
                 const int h0 = v.seeds[i];
                 const int bin0 = v.seed_bin[i];
@@ -218,7 +209,7 @@ __global__ void __launch_bounds__(kKfThreads, kKfBlocksPerSM) k_construct(const 
                 const float dl = sqrtf(dx * dx + dy * dy);
                 f.y = a0.x; f.z = a0.y; f.s = dy / dl; f.t = dz / dl; f.q = 0.f;
                 fit_prior(f, c); f.n = 1;
-                mytab[r0] = (uint16_t)(h0 - base0);
+                v.tl_tab[(size_t)i * v.tab_stride + r0] = (uint16_t)(h0 - base0);
                 p0 = a0.x; p1 = a0.y; p2 = f.s; p3 = f.t; p4 = f.q;
                 top = r0; row = r0; cur = h1; rcur = r0 + D; cy = a1.x; cz = a1.y; miss = 0;
                 ph = 1;
@@ -226,80 +217,155 @@ __global__ void __launch_bounds__(kKfThreads, kKfBlocksPerSM) k_construct(const 
         }
         if (__all_sync(kFull, ph == 0)) break;
 
-        // ---- one pad row ----
-        bool finished = false;
-        if (ph != 0) {
-            const bool up = ph != 3;
+        // ---- one pad row, part 1: transport and the candidate that is already known ----
+        const bool active = ph != 0;
+        const bool up = ph != 3;
+        uint16_t* const gt = v.tl_tab + (size_t)i * v.tab_stride;
+        bool end = false, search = false, counted = false;   // counted: the edge test and the gap count apply
+        int acc = -1;
+        float ay = 0.f, az = 0.f, iwy = 0.f, iwz = 0.f;
+        int4 dn = make_int4(0, 0, 1, 1);
+        if (active) {
             const int prev = row;
             row += up ? 1 : -1;
-            bool end = up ? (row >= nr) : (row < 0);
-            int4 dn = make_int4(0, 0, 1, 1);
-            int nxt = -1, known = -1;
-            float ky = 0.f, kz = 0.f;
+            end = up ? (row >= nr) : (row < 0);
             if (!end) {
                 // loads that do not depend on the fit are issued before the transport
                 dn = load_desc_n(v, tb + row);
+                int nxt = -1, known = -1;
+                float ky = 0.f, kz = 0.f;
                 if (ph == 1) {
                     if (row == rcur) { known = cur; ky = cy; kz = cz; nxt = v.clink_up[cur]; }
                 } else if (ph == 3 && row >= r0) {
-                    const uint16_t e = mytab[row];
+                    const uint16_t e = enext;
+                    if (row > r0) enext = gt[row - 1];
                     if (e != kNoHit) { known = dn.x + e; const float2 hk = v.shit[known]; ky = hk.x; kz = hk.y; }
                 }
                 end = !fit_transport(f, c.row_x[prev], c.row_x[row], c);
-            }
-            if (!end) {
-                visits++;
-                int acc = -1;
-                float ay = 0.f, az = 0.f;
-                bool search = false, counted = false;   // counted: the edge test and the gap count apply
-                if (ph == 1) {
-                    if (row == rcur) {
-                        if (fit_gate(f, ky, kz, c) <= c.p.chi2_link) {
-                            acc = known; ay = ky; az = kz;
-                            cur = nxt; rcur += D;
-                            if (cur < 0) ph = 2;
-                            else { const float2 hn = v.shit[cur]; cy = hn.x; cz = hn.y; }
-                        } else { ph = 2; search = true; counted = true; }
-                    }   // else: in-between row of a step-2 link
-                } else if (ph == 2) {
-                    search = true; counted = true;
-                } else {
-                    if (row >= r0) {
-                        if (known >= 0) { if (fit_gate(f, ky, kz, c) <= c.p.chi2_link) { acc = known; ay = ky; az = kz; } }
-                        else search = true;
-                    } else { search = true; counted = true; }
-                }
-                if (search) {
-                    if (counted && fabsf(f.y) > c.row_x[row] * c.tan_half_angle + c.p.edge_margin) end = true;
-                    else {
-                        acc = fit_search(f, v, tb + row, dn, c, &ay, &az);
-                        if (acc >= 0) miss = 0;
-                        else if (counted && ++miss > c.p.max_gap) end = true;
-                    }
-                }
                 if (!end) {
-                    mytab[row] = acc >= 0 ? (uint16_t)(acc - dn.x) : kNoHit;
-                    if (acc >= 0) {
-                        fit_update(f, ay, az, c);
-                        if (up) { p0 = ay; p1 = az; p2 = f.s; p3 = f.t; p4 = f.q; top = row; }
-                        else { p0 = f.y; p1 = f.z; p2 = f.s; p3 = f.t; p4 = f.q; p5 = f.chi2; first = row; nh = f.n; }
+                    visits++;
+                    iwy = 1.f / (f.c00 + c.sigma_y2); iwz = 1.f / (f.c11 + c.sigma_z2);
+                    bool gate_ok = false;
+                    if (known >= 0) {   // the gate value of (ky, kz) on the predicted state
+                        const float ry = ky - f.y, rz = kz - f.z;
+                        gate_ok = (ry * ry) * iwy + (rz * rz) * iwz <= c.p.chi2_link;
+                        if (gate_ok) { acc = known; ay = ky; az = kz; }
                     }
-                }
-            }
-            if (end) {
-                if (up) {   // start the down pass at the top hit
-                    f.y = p0; f.z = p1; f.s = p2; f.t = p3; f.q = p4;
-                    fit_prior(f, c); f.n = 1;
-                    p5 = 0.f;
-                    row = top; first = top; nh = 1; miss = 0;
-                    ph = 3;
-                } else {
-                    finished = true;
+                    if (ph == 1) {
+                        if (row == rcur) {
+                            if (gate_ok) {
+                                cur = nxt; rcur += D;
+                                if (cur < 0) ph = 2;
+                                else { const float2 hn = v.shit[cur]; cy = hn.x; cz = hn.y; }
+                            } else { ph = 2; search = true; counted = true; }
+                        }   // else: in-between row of a step-2 link
+                    } else if (ph == 2) {
+                        search = true; counted = true;
+                    } else {
+                        search = row < r0 || known < 0;
+                        counted = row < r0;
+                    }
+                    if (search && counted && fabsf(f.y) > c.row_x[row] * c.tan_half_angle + c.p.edge_margin) {
+                        end = true; search = false;
+                    }
                 }
             }
         }
 
-        // ---- finished tracklets: parameters, table rows first..top to HBM, claim of the hits (K6a) ----
+        // ---- part 2: the window searches of this trip, shared out over the warp ----
+        int n_iz = 0;
+        if (search && dn.y > 0) {
+            SearchQuery q;
+            q.y = f.y; q.z = f.z;
+            q.wy = fminf(fmaxf(c.p.win_nsigma * sqrtf(f.c00 + c.sigma_y2), c.p.win_min), c.p.win_max);
+            q.wz = fminf(fmaxf(c.p.win_nsigma * sqrtf(f.c11 + c.sigma_z2), c.p.win_min), c.p.win_max);
+            q.iwy = iwy; q.iwz = iwz;
+            const float4 gf = load_desc_f(v, tb + row);
+            const CellWin w = cell_window(gf, dn.z, dn.w, q.y, q.z, q.wy, q.wz);
+            q.base = dn.x; q.bin = tb + row;
+            q.win = (uint32_t)dn.z | ((uint32_t)w.iy0 << 8) | ((uint32_t)w.iy1 << 16) | ((uint32_t)w.iz0 << 24);
+            s_q[threadIdx.x] = q;
+            n_iz = w.iz1 - w.iz0 + 1;
+        }
+        const int incl = warp_incl_scan(n_iz);
+        const int n_items = __shfl_sync(kFull, incl, 31);
+        if (n_items > 0) {
+            const int off = incl - n_iz;
+            for (int j = 0; j < n_iz; j++) items[off + j] = (uint16_t)(lane | (j << 8));
+            __syncwarp();
+            float bg = 0.f;
+            int bp = -1;
+            for (int t0 = 0; t0 < n_items; t0 += 32) {
+                float4 res = make_float4(0.f, 0.f, 0.f, __int_as_float(-1));
+                if (t0 + lane < n_items) {
+                    const int it = items[t0 + lane];
+                    const SearchQuery q = s_q[wbase + (it & 0xff)];
+                    const int ny = q.win & 0xff, iy0 = (q.win >> 8) & 0xff, iy1 = (q.win >> 16) & 0xff;
+                    const int iz = (int)(q.win >> 24) + (it >> 8);
+                    const uint16_t* cs = cell_table(v, q.bin, q.base);
+                    const float2* hits = v.shit + q.base;
+                    int p = __ldg(&cs[iz * ny + iy0]);
+                    const int pe = __ldg(&cs[iz * ny + iy1 + 1]);
+                    int rp = -1;
+                    for (; p < pe; p += kKfUnroll) {   // the candidates of a grid row are contiguous: loads go out together
+                        float2 h[kKfUnroll];
+#pragma unroll
+                        for (int k = 0; k < kKfUnroll; k++) h[k] = __ldg(&hits[min(p + k, pe - 1)]);
+#pragma unroll
+                        for (int k = 0; k < kKfUnroll; k++) {
+                            const float ry = h[k].x - q.y, rz = h[k].y - q.z;
+                            if (p + k < pe && fabsf(ry) <= q.wy && fabsf(rz) <= q.wz) {
+                                const float gv = (ry * ry) * q.iwy + (rz * rz) * q.iwz;   // the gate value of h[k]
+                                bool take = rp < 0 || gv < res.x;
+                                if (!take && gv == res.x) take = v.sorig[q.base + p + k] < v.sorig[q.base + rp];
+                                if (take) { res.x = gv; res.y = h[k].x; res.z = h[k].y; rp = p + k; }
+                            }
+                        }
+                    }
+                    res.w = __int_as_float(rp);
+                }
+                s_res[threadIdx.x] = res;
+                __syncwarp();
+                for (int t = max(off, t0); t < min(off + n_iz, t0 + 32); t++) {   // the owner merges its items
+                    const float4 r = s_res[wbase + t - t0];
+                    const int rp = __float_as_int(r.w);
+                    if (rp < 0) continue;
+                    bool take = bp < 0 || r.x < bg;
+                    if (!take && r.x == bg) take = v.sorig[dn.x + rp] < v.sorig[dn.x + bp];
+                    if (take) { bg = r.x; bp = rp; ay = r.y; az = r.z; }
+                }
+                __syncwarp();
+            }
+            if (bp >= 0 && bg <= c.p.chi2_ext) acc = dn.x + bp;
+        }
+
+        // ---- part 3: bookkeeping, update, end of a pass ----
+        bool finished = false;
+        if (active) {
+            if (search) {
+                if (acc >= 0) miss = 0;
+                else if (counted && ++miss > c.p.max_gap) end = true;
+            }
+            if (!end) {
+                gt[row] = acc >= 0 ? (uint16_t)(acc - dn.x) : kNoHit;
+                if (acc >= 0) {
+                    fit_update(f, ay, az, iwy, c);
+                    p0 = up ? ay : f.y; p1 = up ? az : f.z; p2 = f.s; p3 = f.t; p4 = f.q; p5 = f.chi2;
+                    top = up ? row : top; first = row; nh = f.n;
+                }
+            } else if (up) {   // start the down pass at the top hit
+                f.y = p0; f.z = p1; f.s = p2; f.t = p3; f.q = p4;
+                fit_prior(f, c); f.n = 1;
+                p5 = 0.f;
+                row = top; first = top; nh = 1; miss = 0;
+                enext = top > r0 ? gt[top - 1] : kNoHit;
+                ph = 3;
+            } else {
+                finished = true;
+            }
+        }
+
+        // ---- finished tracklets: parameters, claim of the hits of rows first..top (K6a) ----
         unsigned fin = __ballot_sync(kFull, finished);
         if (fin) {
             uint32_t key = 0;
@@ -311,6 +377,7 @@ __global__ void __launch_bounds__(kKfThreads, kKfBlocksPerSM) k_construct(const 
                 if (nh >= c.p.min_tracklet_hits) key = tl_key(v, i, nh, tb);
                 ph = 0;
             }
+            fin = __ballot_sync(kFull, key != 0);
             __syncwarp();
             while (fin) {
                 const int L = __ffs(fin) - 1;
@@ -318,18 +385,15 @@ __global__ void __launch_bounds__(kKfThreads, kKfBlocksPerSM) k_construct(const 
                 const int li = __shfl_sync(kFull, i, L), lfirst = __shfl_sync(kFull, first, L);
                 const int ltop = __shfl_sync(kFull, top, L), ltb = __shfl_sync(kFull, tb, L);
                 const uint32_t lkey = __shfl_sync(kFull, key, L);
-                const uint16_t* col = warptab + L * pitch;
-                uint16_t* gt = v.tl_tab + (size_t)li * v.tab_stride;
+                const uint16_t* lt = v.tl_tab + (size_t)li * v.tab_stride;
                 for (int r = lfirst + lane; r <= ltop; r += 32) {
-                    const uint16_t e = col[r];
-                    gt[r] = e;
-                    if (e != kNoHit && lkey) {
+                    const uint16_t e = lt[r];
+                    if (e != kNoHit) {
                         atomicMax(&v.owner[load_desc_n(v, ltb + r).x + e], lkey);
                         claimed++;
                     }
                 }
             }
-            __syncwarp();
         }
     }
     unsigned long long vs = visits, cl = claimed;

@@ -65,7 +65,7 @@ struct tpc_tracker {
     std::vector<float> sector_alpha;
     cudaStream_t own_stream = nullptr, stream = nullptr;
     int sm_count = 148;
-    int kf_blocks = 148, kf_smem = 0;   // persistent constructor grid, bytes of its row -> hit tables
+    int kf_blocks = 148;   // persistent constructor grid
     // batch state
     View v;
     int n_events = 0;
@@ -202,7 +202,7 @@ int launch_all(tpc_tracker* t, int64_t* launches) {
     L += scan_exclusive(v.seed_count, v.seed_start, nb, t->scratch.p, st);
     k_seeds<<<nb, kSeedThreads, 0, st>>>(v); L++;
     mark(3);
-    k_construct<<<t->kf_blocks, kKfThreads, t->kf_smem, st>>>(v, c); L++;   // also claims the hits (K6a)
+    k_construct<<<t->kf_blocks, kKfThreads, 0, st>>>(v, c); L++;   // also claims the hits (K6a)
     mark(4);
     const int sel_blocks = t->sm_count * 16;
     k_count_owned<<<sel_blocks, kSelThreads, 0, st>>>(v, c); L++;
@@ -288,12 +288,9 @@ tpc_tracker* tpc_tracker_create_ex(const tpc_geometry* g, float bz, const tpc_pa
         return nullptr;
     }
     t->stream = t->own_stream;
-    {   // constructor: one CTA's row -> hit tables in dynamic shared memory, as many CTAs as fit
-        t->kf_smem = kKfThreads * kf_tab_pitch(g->n_rows) * (int)sizeof(uint16_t);
+    {   // persistent constructor grid: as many CTAs as are resident at once
         int per_sm = 0;
-        if (cudaFuncSetAttribute(k_construct, cudaFuncAttributeMaxDynamicSharedMemorySize, t->kf_smem) != cudaSuccess ||
-            cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_construct, kKfThreads, t->kf_smem) != cudaSuccess ||
-            per_sm < 1) {
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_construct, kKfThreads, 0) != cudaSuccess || per_sm < 1) {
             set_err("k_construct cannot be configured: %s", cudaGetErrorString(cudaGetLastError()));
             cudaStreamDestroy(t->own_stream); delete t;
             return nullptr;
@@ -393,7 +390,7 @@ int tpc_track_events(tpc_tracker* t, int32_t n, const tpc_event_in* in, tpc_even
         CK(cudaMemsetAsync(v.tl_keep, 0, sizeof(int32_t) * (size_t)(t->S_cap + 1), st));
         CK(cudaMemsetAsync(v.tl_nown, 0, sizeof(int32_t) * (size_t)(t->S_cap + 1), st));
         if ((rc = launch_all(t, &t->counters.n_kernel_launches)) != TPC_OK) return rc;
-        CK(cudaMemcpyAsync(t->h_cnt.p, v.cnt, sizeof(unsigned long long) * CNT_N, cudaMemcpyDeviceToHost, st));
+        CK(cudaMemcpyAsync(t->h_cnt.p, v.cnt, sizeof(unsigned long long) * CNT_CURSOR, cudaMemcpyDeviceToHost, st));
         CK(cudaMemcpyAsync(t->h_ev_off.p, v.ev_off, sizeof(int32_t) * 2 * (n + 1), cudaMemcpyDeviceToHost, st));
         int32_t n_seeds = 0;
         CK(cudaMemcpyAsync(&n_seeds, v.seed_start + v.n_bins, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
