@@ -131,6 +131,12 @@ tpc_tracker* tpc_tracker_create_ex(const tpc_geometry* geometry, float bz_tesla,
 /* Run all kernels on this CUDA stream (a cudaStream_t; NULL = the tracker's own stream). */
 int tpc_tracker_set_stream(tpc_tracker* t, void* cuda_stream);
 
+/* Host-input batches (mem_space 0) are cut into groups of events that run on separate streams, so that the copies
+ * of one group overlap the kernels of another ("several events ... processed concurrently on one GPU via streams",
+ * BASELINE.json:5).  n = events per group; 0 (default) = automatic (up to four groups of at least ~2 M clusters).
+ * Results do not depend on the grouping.  Device-input batches always run as one group. */
+int tpc_tracker_set_group_events(tpc_tracker* t, int32_t n);
+
 /* Track one event.  Synchronous: returns when the outputs are complete.  Zero clusters, empty sectors and
  * empty rows are legal (0 tracks).  Returns a status code. */
 int tpc_track_event(tpc_tracker* t, const tpc_event_in* in, tpc_event_out* out);
@@ -155,7 +161,9 @@ int tpc_get_stage_ms(const tpc_tracker* t, float* ms /* [TPC_N_STAGES] */);
 
 /* ---- intermediates of the last call, for stage-by-stage parity tests (not part of the hot path) ----
  * All hit indices are the caller's indices within event `event`; -1 = none.  buf is a HOST buffer of `bytes`
- * bytes; the call fails with TPC_ERR_ARG if it is too small.  Sizes: tpc_debug_size(). */
+ * bytes; the call fails with TPC_ERR_ARG if it is too small.  Sizes: tpc_debug_size().  After a host-input batch
+ * that ran as more than three groups only the events of the last three groups still have their intermediates
+ * (TPC_ERR_ARG for the others). */
 #define TPC_DBG_LINK_UP 0    /* int32 [n_clusters(event)]  neighbour before cleaning */
 #define TPC_DBG_LINK_DN 1
 #define TPC_DBG_CLINK_UP 2   /* int32 [n_clusters(event)]  after cleaning */

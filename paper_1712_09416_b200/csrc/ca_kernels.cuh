@@ -67,7 +67,7 @@ __global__ void __launch_bounds__(256) k_scatter(const View v, int ns, int nr) {
 constexpr int kSortThreads = 128;
 
 __global__ void __launch_bounds__(kSortThreads) k_sort_row(const View v) {
-    __shared__ int cnt[TPC_MAX_ROW_HITS + kCellPad + 1];  // hits per cell, then first hit of each cell
+    __shared__ int cnt[kMaxCells + 1];                    // hits per cell, then first hit of each cell
     __shared__ uint16_t ck[TPC_MAX_ROW_HITS];             // cell of hit k
     __shared__ uint16_t rk[TPC_MAX_ROW_HITS];             // arrival rank of hit k inside its cell
     __shared__ float red[4][kSortThreads / 32];
@@ -76,7 +76,7 @@ __global__ void __launch_bounds__(kSortThreads) k_sort_row(const View v) {
     const int bin = blockIdx.x;
     const int b0 = v.bin_start[bin];
     const int n = min(v.bin_start[bin + 1] - b0, TPC_MAX_ROW_HITS);
-    uint16_t* cs = v.cells + (size_t)b0 + (size_t)bin * kCellPad;
+    uint16_t* cs = v.cells + (size_t)kCellsPerHit * b0 + (size_t)bin * kCellPad;
     if (n == 0) {
         if (threadIdx.x == 0) {
             BinDesc d; d.y0 = 0.f; d.z0 = 0.f; d.idy = 0.f; d.idz = 0.f; d.base = b0; d.n = 0; d.ny = 1; d.nz = 1;
@@ -110,13 +110,15 @@ __global__ void __launch_bounds__(kSortThreads) k_sort_row(const View v) {
     }
     __syncthreads();
     ymin = box[0]; ymax = box[1]; zmin = box[2]; zmax = box[3];
-    // grid dims: about one cell per hit, cells ~0.6 : 1/0.6 in (y : z), never finer than 0.7 x 1.2 cm
+    // grid dims: cells of about one hit's area, ~0.6 : 1/0.6 in (y : z), then kCellsPerHit times finer in y (the
+    // hits of the cells iy0..iy1 of one grid row are contiguous, so fine y cells cost no extra range), never finer
+    // than 0.35 x 1.2 cm
     const float ylen = fmaxf(ymax - ymin, 1.0e-3f), zlen = fmaxf(zmax - zmin, 1.0e-3f);
     const float area = ylen * zlen / (float)n;
-    const float dy = fmaxf(sqrtf(area * 0.6f), 0.7f), dz = fmaxf(sqrtf(area / 0.6f), 1.2f);
+    const float dy = fmaxf(sqrtf(area * 0.6f) / (float)kCellsPerHit, 0.35f), dz = fmaxf(sqrtf(area / 0.6f), 1.2f);
     int nz = max(1, min((int)(zlen / dz) + 1, 255));
     int ny = max(1, min((int)(ylen / dy) + 1, 255));
-    const int cap = n + kCellPad - 1;  // ny*nz + 1 entries must fit
+    const int cap = min(kCellsPerHit * n + kCellPad - 1, kMaxCells);  // ny*nz + 1 entries must fit
     if (nz > cap) nz = cap;
     if (ny * nz > cap) ny = max(1, cap / nz);
     const float idy = (float)ny / (ylen * 1.0001f), idz = (float)nz / (zlen * 1.0001f);
@@ -165,7 +167,8 @@ constexpr int kNfList = 8;     // down-candidates remembered per hit; more -> ne
 
 __global__ void __launch_bounds__(kNfThreads) k_neighbours(const View v, const __grid_constant__ Const c) {
     __shared__ float2 s_hu[kNfCap], s_hd[kNfCap];
-    __shared__ uint16_t s_cu[kNfCap + kCellPad + 1], s_cd[kNfCap + kCellPad + 1];
+    constexpr int kNfCells = kCellsPerHit * kNfCap + kCellPad;   // cell-table entries held in shared memory
+    __shared__ uint16_t s_cu[kNfCells], s_cd[kNfCells];
     __shared__ uint16_t s_dl[kNfList][kNfThreads];
     const int bin = blockIdx.x;
     const int nr = c.n_rows, D = c.p.link_step;
@@ -186,12 +189,12 @@ __global__ void __launch_bounds__(kNfThreads) k_neighbours(const View v, const _
     const float4 gfu = load_desc_f(v, bin + D), gfd = load_desc_f(v, bin - D);
     const float2* hu = v.shit + du.x; const float2* hd = v.shit + dd.x;
     const uint16_t* cu = cell_table(v, bin + D, du.x); const uint16_t* cd = cell_table(v, bin - D, dd.x);
-    if (du.y <= kNfCap) {
+    if (du.y <= kNfCap && du.z * du.w < kNfCells) {
         for (int k = threadIdx.x; k < du.y; k += kNfThreads) s_hu[k] = hu[k];
         for (int k = threadIdx.x; k <= du.z * du.w; k += kNfThreads) s_cu[k] = cu[k];
         hu = s_hu; cu = s_cu;
     }
-    if (dd.y <= kNfCap) {
+    if (dd.y <= kNfCap && dd.z * dd.w < kNfCells) {
         for (int k = threadIdx.x; k < dd.y; k += kNfThreads) s_hd[k] = hd[k];
         for (int k = threadIdx.x; k <= dd.z * dd.w; k += kNfThreads) s_cd[k] = cd[k];
         hd = s_hd; cd = s_cd;

@@ -8,7 +8,12 @@
 
 namespace tpc {
 
-constexpr int kCellPad = 32;          // cell table of a bin holds up to n_hits + kCellPad entries
+#ifndef TPC_CELLS_PER_HIT
+#define TPC_CELLS_PER_HIT 1
+#endif
+constexpr int kCellsPerHit = TPC_CELLS_PER_HIT;       // grid cells per hit of a bin (the cells are this much finer in y than in z)
+constexpr int kCellPad = 32;          // cell table of a bin holds up to kCellsPerHit * n_hits + kCellPad entries
+constexpr int kMaxCells = kCellsPerHit == 1 ? TPC_MAX_ROW_HITS + kCellPad - 1 : 4096;  // and never more than kMaxCells + 1
 constexpr float kGridPad = 1.0e-3f;   // cm added to every grid query so that rounding never hides a candidate
 constexpr uint16_t kNoHit = 0xffffu;  // empty entry of a tracklet's row -> hit table (hits are row-local, < 2048)
 constexpr unsigned kFull = 0xffffffffu;
@@ -57,7 +62,7 @@ struct View {
     float2* thit; int32_t* tidx;   // [N] bucketed, unsorted: (y,z), caller's index
     float2* shit; int32_t* sorig;  // [N] sorted by (task,row,cell): (y,z), caller's index in its event
     BinDesc* desc;           // [n_bins]
-    uint16_t* cells;         // [N + n_bins*kCellPad] first hit of each cell, relative to the bin's base
+    uint16_t* cells;         // [kCellsPerHit*N + n_bins*kCellPad] first hit of each cell, relative to the bin's base
     // K2-K4
     int32_t *link_up, *link_dn, *clink_up, *clink_dn; // [N] batch-global sorted index or -1
     int32_t* seed_count;     // [n_bins+1]
@@ -93,7 +98,7 @@ __device__ __forceinline__ float4 load_desc_f(const View& v, int bin) { // y0, z
     return __ldg(reinterpret_cast<const float4*>(&v.desc[bin]));
 }
 __device__ __forceinline__ const uint16_t* cell_table(const View& v, int bin, int base) {
-    return v.cells + (size_t)base + (size_t)bin * kCellPad;
+    return v.cells + (size_t)kCellsPerHit * base + (size_t)bin * kCellPad;
 }
 
 __device__ __forceinline__ int grid_cell(float v, float v0, float iv, int n) {

@@ -142,8 +142,14 @@ __device__ __forceinline__ uint32_t tl_key(const View& v, int i, int nh, int tas
 // tracklet's key on owner[hit]).
 // ---------------------------------------------------------------------------------------------------------
 constexpr int kKfThreads = 128;
-constexpr int kKfBlocksPerSM = 5;
-constexpr int kKfUnroll = 4;       // candidates of a grid row loaded at once
+#ifndef TPC_KF_BLOCKS
+#define TPC_KF_BLOCKS 5
+#endif
+#ifndef TPC_KF_UNROLL
+#define TPC_KF_UNROLL 4
+#endif
+constexpr int kKfBlocksPerSM = TPC_KF_BLOCKS;
+constexpr int kKfUnroll = TPC_KF_UNROLL;       // candidates of a grid row loaded at once
 constexpr int kKfMaxItems = 256;   // >= 32 lanes x grid rows a window can span (window <= 2 * 3 cm + pad, cells >= 1.2 cm)
 
 struct SearchQuery {
@@ -339,8 +345,8 @@ __global__ void __launch_bounds__(kKfThreads, kKfBlocksPerSM) k_construct(const 
             if (bp >= 0 && bg <= c.p.chi2_ext) acc = dn.x + bp;
         }
 
-        // ---- part 3: bookkeeping, update, end of a pass ----
-        bool finished = false;
+        // ---- part 3: bookkeeping, update, end of a pass (the warp is brought together before each piece) ----
+        bool finished = false, upd = false;
         if (active) {
             if (search) {
                 if (acc >= 0) miss = 0;
@@ -348,12 +354,18 @@ __global__ void __launch_bounds__(kKfThreads, kKfBlocksPerSM) k_construct(const 
             }
             if (!end) {
                 gt[row] = acc >= 0 ? (uint16_t)(acc - dn.x) : kNoHit;
-                if (acc >= 0) {
-                    fit_update(f, ay, az, iwy, c);
-                    p0 = up ? ay : f.y; p1 = up ? az : f.z; p2 = f.s; p3 = f.t; p4 = f.q; p5 = f.chi2;
-                    top = up ? row : top; first = row; nh = f.n;
-                }
-            } else if (up) {   // start the down pass at the top hit
+                upd = acc >= 0;
+            }
+        }
+        __syncwarp();
+        if (upd) {
+            fit_update(f, ay, az, iwy, c);
+            p0 = up ? ay : f.y; p1 = up ? az : f.z; p2 = f.s; p3 = f.t; p4 = f.q; p5 = f.chi2;
+            top = up ? row : top; first = row; nh = f.n;
+        }
+        __syncwarp();
+        if (active && end) {
+            if (up) {   // start the down pass at the top hit
                 f.y = p0; f.z = p1; f.s = p2; f.t = p3; f.q = p4;
                 fit_prior(f, c); f.n = 1;
                 p5 = 0.f;

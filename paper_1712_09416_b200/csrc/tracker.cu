@@ -3,6 +3,7 @@
 #include <algorithm>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <string>
 #include <vector>
@@ -60,20 +61,16 @@ template <class T> struct Buf {
 
 using namespace tpc;
 
-struct tpc_tracker {
-    Const c;
-    std::vector<float> sector_alpha;
-    cudaStream_t own_stream = nullptr, stream = nullptr;
-    int sm_count = 148;
-    int kf_blocks = 148;   // persistent constructor grid
-    // batch state
+// Work space and state of one group of events in flight: every kernel launch covers all its sector tasks.
+struct Batch {
+    cudaStream_t stream = nullptr;           // the stream this group runs on
     View v;
-    int n_events = 0;
-    int64_t N = 0;
-    std::vector<int32_t> ev_n, ev_off;       // clusters per event, offset in the batch
-    int mem_space = 1;
-    tpc_counters counters;
-    bool have_result = false;
+    int n_events = 0, first_event = 0;
+    int64_t N = 0, S_cap = 0;
+    bool host_in = false;
+    const tpc_event_in* in = nullptr;
+    std::vector<int32_t> ev_n, ev_off;       // clusters per event, offset in the group
+    tpc_counters counters;                   // of the group's last run
     // device pools
     Buf<float> in_y, in_z, tl_par, o_f[7];
     Buf<float2> thit, shit;
@@ -87,18 +84,13 @@ struct tpc_tracker {
     Buf<unsigned long long> cnt;
     // pinned host mirrors
     Buf<EventSrc> h_ev_src;
-    Buf<int32_t> h_sec_off, h_ev_off, h_o_i[4], h_o_hit;
+    Buf<int32_t> h_sec_off, h_ev_off, h_nseeds;
     Buf<unsigned long long> h_cnt;
-    Buf<float> h_o_f[7];
-    int64_t S_cap = 0;
-    bool profiling = false;
     cudaEvent_t evt[TPC_N_STAGES + 1] = {};
     float stage_ms[TPC_N_STAGES] = {};
 
-    tpc_tracker() {
-        h_ev_src.host = h_sec_off.host = h_ev_off.host = h_cnt.host = h_o_hit.host = true;
-        for (auto& b : h_o_i) b.host = true;
-        for (auto& b : h_o_f) b.host = true;
+    Batch() {
+        h_ev_src.host = h_sec_off.host = h_ev_off.host = h_cnt.host = h_nseeds.host = true;
         memset(&v, 0, sizeof v);
         memset(&counters, 0, sizeof counters);
     }
@@ -112,7 +104,43 @@ struct tpc_tracker {
         scratch.release(); o_hit.release();
         for (auto& b : o_i) b.release();
         slot.release(); cells.release(); desc.release(); owner.release(); ev_src.release();
-        cnt.release(); h_ev_src.release(); h_sec_off.release(); h_ev_off.release(); h_o_hit.release(); h_cnt.release();
+        cnt.release(); h_ev_src.release(); h_sec_off.release(); h_ev_off.release(); h_cnt.release(); h_nseeds.release();
+        for (auto& e : evt) if (e) { cudaEventDestroy(e); e = nullptr; }
+    }
+};
+
+struct tpc_tracker {
+    Const c;
+    std::vector<float> sector_alpha;
+    cudaStream_t user_stream = nullptr;      // tpc_tracker_set_stream: used by slot 0 when the call is one group
+    std::vector<cudaStream_t> own_streams;   // one per slot
+    int sm_count = 148;
+    int kf_blocks = 148;                     // persistent constructor grid
+    int group_events = 0;                    // host-input batches: events per group (0 = automatic)
+    std::vector<Batch*> slots;               // groups in flight; slots[0] always exists
+    // the last call
+    tpc_counters counters;
+    bool have_result = false;
+    int n_events = 0;
+    std::vector<int> ev_slot, ev_local;      // where the intermediates of each event are (-1: overwritten since)
+    Buf<int32_t> h_o_i[4], h_o_hit;          // host-input calls: the outputs of all groups, pinned
+    Buf<float> h_o_f[7];
+    bool profiling = false;
+    float stage_ms[TPC_N_STAGES] = {};
+
+    tpc_tracker() {
+        h_o_hit.host = true;
+        for (auto& b : h_o_i) b.host = true;
+        for (auto& b : h_o_f) b.host = true;
+        memset(&counters, 0, sizeof counters);
+    }
+    void sync_all() { for (auto s : own_streams) cudaStreamSynchronize(s); if (user_stream) cudaStreamSynchronize(user_stream); }
+    void free_all() {
+        for (auto* b : slots) { b->free_all(); delete b; }
+        slots.clear();
+        for (auto s : own_streams) cudaStreamDestroy(s);
+        own_streams.clear();
+        h_o_hit.release();
         for (auto& b : h_o_i) b.release();
         for (auto& b : h_o_f) b.release();
     }
@@ -122,23 +150,23 @@ namespace {
 
 int tab_stride(int n_rows) { return (n_rows + 31) & ~31; }
 
-int reserve_batch(tpc_tracker* t, int n_events, int64_t N, int64_t S_cap) {
-    const int64_t nb = (int64_t)n_events * t->c.n_sectors * t->c.n_rows;
+int reserve_batch(const tpc_tracker* tr, Batch* t, int n_events, int64_t N, int64_t S_cap) {
+    const int64_t nb = (int64_t)n_events * tr->c.n_sectors * tr->c.n_rows;
     const size_t n = (size_t)std::max<int64_t>(N, 1);
     int rc = TPC_OK;
 #define RS(b, k) if ((rc = t->b.reserve(k)) != TPC_OK) return rc
-    RS(sec_off, (size_t)n_events * (t->c.n_sectors + 1)); RS(h_sec_off, (size_t)n_events * (t->c.n_sectors + 1));
+    RS(sec_off, (size_t)n_events * (tr->c.n_sectors + 1)); RS(h_sec_off, (size_t)n_events * (tr->c.n_sectors + 1));
     RS(ev_src, n_events); RS(h_ev_src, n_events);
     RS(bin_count, nb + 1); RS(bin_start, nb + 1); RS(seed_count, nb + 1); RS(seed_start, nb + 1);
     RS(slot, n); RS(thit, n); RS(tidx, n); RS(shit, n); RS(sorig, n);
-    RS(desc, nb); RS(cells, n + (size_t)nb * kCellPad + 64);
+    RS(desc, nb); RS(cells, (size_t)kCellsPerHit * n + (size_t)nb * kCellPad + 64);
     RS(link_up, n); RS(link_dn, n); RS(clink_up, n); RS(clink_dn, n); RS(owner, n);
     RS(seeds, S_cap); RS(seed_bin, S_cap); RS(tl_rows, S_cap); RS(tl_par, 6 * (size_t)S_cap);
-    RS(tl_tab, (size_t)S_cap * tab_stride(t->c.n_rows));
+    RS(tl_tab, (size_t)S_cap * tab_stride(tr->c.n_rows));
     RS(tl_nown, S_cap + 1); RS(tl_keep, S_cap + 1); RS(trk_scan, S_cap + 2); RS(hit_scan, S_cap + 2);
     RS(ev_off_d, 2 * ((size_t)n_events + 1)); RS(h_ev_off, 2 * ((size_t)n_events + 1));
     RS(scratch, (size_t)std::max<int64_t>(nb, S_cap) / kScanTile + 8);
-    RS(cnt, CNT_N); RS(h_cnt, CNT_N);
+    RS(cnt, CNT_N); RS(h_cnt, CNT_N); RS(h_nseeds, 1);
     for (int k = 0; k < 4; k++) RS(o_i[k], S_cap);
     for (int k = 0; k < 7; k++) RS(o_f[k], S_cap);
     RS(o_hit, n);
@@ -170,10 +198,10 @@ int validate(const tpc_tracker* t, int n, const tpc_event_in* in) {
     return TPC_OK;
 }
 
-// launch K1..K6 for the staged batch; counts launches
-int launch_all(tpc_tracker* t, int64_t* launches) {
+// launch K1..K6 for the staged group; counts launches
+int launch_all(const tpc_tracker* tr, Batch* t) {
     const View& v = t->v;
-    const Const& c = t->c;
+    const Const& c = tr->c;
     cudaStream_t st = t->stream;
     const int ns = c.n_sectors, nr = c.n_rows;
     const int nb = v.n_bins;
@@ -181,7 +209,7 @@ int launch_all(tpc_tracker* t, int64_t* launches) {
     CK(cudaMemsetAsync(v.bin_count, 0, sizeof(int32_t) * (nb + 1), st));
     CK(cudaMemsetAsync(v.cnt, 0, sizeof(unsigned long long) * CNT_N, st));
     if (v.N > 0) CK(cudaMemsetAsync(v.owner, 0, sizeof(uint32_t) * (size_t)v.N, st));
-    auto mark = [&](int k) { if (t->profiling) cudaEventRecord(t->evt[k], st); };
+    auto mark = [&](int k) { if (tr->profiling) cudaEventRecord(t->evt[k], st); };
     mark(0);
     int maxn = 0;
     for (int e = 0; e < t->n_events; e++) maxn = std::max(maxn, t->ev_n[e]);
@@ -202,9 +230,9 @@ int launch_all(tpc_tracker* t, int64_t* launches) {
     L += scan_exclusive(v.seed_count, v.seed_start, nb, t->scratch.p, st);
     k_seeds<<<nb, kSeedThreads, 0, st>>>(v); L++;
     mark(3);
-    k_construct<<<t->kf_blocks, kKfThreads, 0, st>>>(v, c); L++;   // also claims the hits (K6a)
+    k_construct<<<tr->kf_blocks, kKfThreads, 0, st>>>(v, c); L++;   // also claims the hits (K6a)
     mark(4);
-    const int sel_blocks = t->sm_count * 16;
+    const int sel_blocks = tr->sm_count * 16;
     k_count_owned<<<sel_blocks, kSelThreads, 0, st>>>(v, c); L++;
     // scans run over the whole seed capacity; entries beyond the seed count are zeroed first
     L += scan_exclusive(v.tl_keep, v.trk_scan, (int)t->S_cap, t->scratch.p, st);
@@ -213,8 +241,142 @@ int launch_all(tpc_tracker* t, int64_t* launches) {
     k_write_tracks<<<sel_blocks, kSelThreads, 0, st>>>(v, c); L++;
     mark(5);
     CK(cudaGetLastError());
-    *launches += L;
+    t->counters.n_kernel_launches += L;
     return TPC_OK;
+}
+
+// Enqueue one group of events on its slot's stream: input copies (host inputs), K1..K6, the counters' way back.
+// Nothing here waits for the device.
+int batch_begin(const tpc_tracker* tr, Batch* t, int first_event, int n, const tpc_event_in* in, int64_t S_cap, bool copy_inputs) {
+    const int ns = tr->c.n_sectors, nr = tr->c.n_rows;
+    int rc;
+    int64_t N = 0;
+    t->ev_n.assign(n, 0); t->ev_off.assign(n + 1, 0);
+    for (int e = 0; e < n; e++) { t->ev_n[e] = in[e].n_clusters; t->ev_off[e] = (int32_t)N; N += in[e].n_clusters; }
+    t->ev_off[n] = (int32_t)N;
+    if (N > 0x7fff0000ll) { set_err("a group of events holds more than 2^31 clusters"); return TPC_ERR_CAPACITY; }
+    t->host_in = in[0].mem_space == 0;
+    t->in = in; t->first_event = first_event;
+    cudaStream_t st = t->stream;
+    S_cap = std::max<int64_t>(std::max<int64_t>(t->S_cap, S_cap), default_seed_cap(N));
+    if ((rc = reserve_batch(tr, t, n, N, S_cap)) != TPC_OK) return rc;
+    if (t->host_in) {
+        const size_t nn = (size_t)std::max<int64_t>(N, 1);
+        if ((rc = t->in_y.reserve(nn)) != TPC_OK || (rc = t->in_z.reserve(nn)) != TPC_OK || (rc = t->in_row.reserve(nn)) != TPC_OK)
+            return rc;
+    }
+    // the event table and the sector offsets
+    for (int e = 0; e < n; e++) {
+        EventSrc& s = t->h_ev_src.p[e];
+        s.n = in[e].n_clusters; s.off = t->ev_off[e];
+        if (t->host_in) {
+            s.y = t->in_y.p + s.off; s.z = t->in_z.p + s.off; s.row = t->in_row.p + s.off;
+            if (copy_inputs && s.n > 0) {
+                CK(cudaMemcpyAsync(t->in_y.p + s.off, in[e].y, sizeof(float) * s.n, cudaMemcpyHostToDevice, st));
+                CK(cudaMemcpyAsync(t->in_z.p + s.off, in[e].z, sizeof(float) * s.n, cudaMemcpyHostToDevice, st));
+                CK(cudaMemcpyAsync(t->in_row.p + s.off, in[e].row, sizeof(int32_t) * s.n, cudaMemcpyHostToDevice, st));
+            }
+        } else {
+            s.y = in[e].y; s.z = in[e].z; s.row = in[e].row;
+        }
+        memcpy(t->h_sec_off.p + (size_t)e * (ns + 1), in[e].sector_offset, sizeof(int32_t) * (ns + 1));
+    }
+    CK(cudaMemcpyAsync(t->ev_src.p, t->h_ev_src.p, sizeof(EventSrc) * n, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(t->sec_off.p, t->h_sec_off.p, sizeof(int32_t) * (size_t)n * (ns + 1), cudaMemcpyHostToDevice, st));
+
+    View& v = t->v;
+    v.n_events = n; v.n_tasks = n * ns; v.n_bins = n * ns * nr; v.N = (int32_t)N;
+    v.ev = t->ev_src.p; v.sec_off = t->sec_off.p;
+    v.bin_count = t->bin_count.p; v.bin_start = t->bin_start.p; v.slot = t->slot.p;
+    v.thit = t->thit.p; v.tidx = t->tidx.p; v.shit = t->shit.p; v.sorig = t->sorig.p;
+    v.desc = t->desc.p; v.cells = t->cells.p;
+    v.link_up = t->link_up.p; v.link_dn = t->link_dn.p; v.clink_up = t->clink_up.p; v.clink_dn = t->clink_dn.p;
+    v.seed_count = t->seed_count.p; v.seed_start = t->seed_start.p; v.seeds = t->seeds.p; v.seed_bin = t->seed_bin.p;
+    v.S_cap = (int32_t)t->S_cap;
+    v.tl_tab = t->tl_tab.p; v.tab_stride = tab_stride(nr); v.tl_rows = t->tl_rows.p; v.tl_par = t->tl_par.p;
+    v.owner = t->owner.p; v.tl_nown = t->tl_nown.p; v.tl_keep = t->tl_keep.p;
+    v.trk_scan = t->trk_scan.p; v.hit_scan = t->hit_scan.p; v.ev_off = t->ev_off_d.p;
+    v.o_sector = t->o_i[0].p; v.o_first_hit = t->o_i[1].p; v.o_n_hits = t->o_i[2].p; v.o_ndf = t->o_i[3].p;
+    v.o_hit_idx = t->o_hit.p;
+    v.o_x = t->o_f[0].p; v.o_y = t->o_f[1].p; v.o_z = t->o_f[2].p; v.o_sinphi = t->o_f[3].p;
+    v.o_tgl = t->o_f[4].p; v.o_qpt = t->o_f[5].p; v.o_chi2 = t->o_f[6].p;
+    v.cnt = t->cnt.p;
+    t->n_events = n; t->N = N;
+    if (tr->profiling)
+        for (auto& e : t->evt)
+            if (!e) CK(cudaEventCreate(&e));
+
+    // keep / nown must read as 0 beyond the seed count
+    CK(cudaMemsetAsync(v.tl_keep, 0, sizeof(int32_t) * (size_t)(t->S_cap + 1), st));
+    CK(cudaMemsetAsync(v.tl_nown, 0, sizeof(int32_t) * (size_t)(t->S_cap + 1), st));
+    if ((rc = launch_all(tr, t)) != TPC_OK) return rc;
+    CK(cudaMemcpyAsync(t->h_cnt.p, v.cnt, sizeof(unsigned long long) * CNT_CURSOR, cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(t->h_ev_off.p, v.ev_off, sizeof(int32_t) * 2 * (n + 1), cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(t->h_nseeds.p, v.seed_start + v.n_bins, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+    return TPC_OK;
+}
+
+// Wait for the group, check what the kernels reported, grow the tracklet pools and run again if they overflowed.
+int batch_finish(const tpc_tracker* tr, Batch* t) {
+    const int nr = tr->c.n_rows;
+    for (int attempt = 0;; attempt++) {
+        CK(cudaStreamSynchronize(t->stream));
+        if (tr->profiling)
+            for (int k = 0; k < TPC_N_STAGES; k++) cudaEventElapsedTime(&t->stage_ms[k], t->evt[k], t->evt[k + 1]);
+        const unsigned err = (unsigned)(t->h_cnt.p[CNT_ERR] & 0xffffffffu);
+        const int32_t n_seeds = t->h_nseeds.p[0];
+        if (err & kErrBadRow) { set_err("a cluster has row outside [0,%d)", nr); return TPC_ERR_ARG; }
+        if (err & kErrRowCapacity) {
+            set_err("more than %d clusters in one (sector,row)", TPC_MAX_ROW_HITS);
+            return TPC_ERR_CAPACITY;
+        }
+        if ((err & kErrSeedCapacity) || n_seeds > t->S_cap) {
+            if (attempt >= 2) { set_err("tracklet pool could not be grown"); return TPC_ERR_CAPACITY; }
+            t->counters.n_retries++;
+            int rc = batch_begin(tr, t, t->first_event, t->n_events, t->in, (int64_t)n_seeds + n_seeds / 8 + 1024, false);
+            if (rc != TPC_OK) return rc;
+            continue;
+        }
+        t->counters.n_events = t->n_events; t->counters.n_clusters = t->N;
+        t->counters.n_links = (int64_t)t->h_cnt.p[CNT_LINKS];
+        t->counters.n_seeds = n_seeds;
+        t->counters.n_row_visits = (int64_t)t->h_cnt.p[CNT_ROW_VISITS];
+        t->counters.n_tracklet_hits = (int64_t)t->h_cnt.p[CNT_TL_HITS];
+        t->counters.n_tracks = (int64_t)t->h_cnt.p[CNT_TRACKS];
+        t->counters.n_track_hits = (int64_t)t->h_cnt.p[CNT_TRACK_HITS];
+        return TPC_OK;
+    }
+}
+
+Batch* get_slot(tpc_tracker* t, int k) {
+    while ((int)t->slots.size() <= k) {
+        cudaStream_t s = nullptr;
+        if (cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking) != cudaSuccess) { set_err("cudaStreamCreate failed"); return nullptr; }
+        t->own_streams.push_back(s);
+        Batch* b = new Batch;
+        b->stream = s;
+        t->slots.push_back(b);
+    }
+    return t->slots[k];
+}
+
+// pinned output array of a host-input call: grow, keeping what earlier groups have written
+template <class T> int grow_keep(tpc_tracker* t, Buf<T>& b, size_t need, size_t keep, size_t hint) {
+    if (need <= b.cap) return TPC_OK;
+    t->sync_all();   // copies into the old array may be in flight
+    Buf<T> nb; nb.host = true;
+    int rc = nb.reserve(std::max(need, hint));
+    if (rc != TPC_OK) return rc;
+    if (keep) memcpy(nb.p, b.p, keep * sizeof(T));
+    b.release();
+    b = nb;
+    return TPC_OK;
+}
+
+void add_counters(tpc_counters& a, const tpc_counters& b) {
+    a.n_events += b.n_events; a.n_clusters += b.n_clusters; a.n_links += b.n_links; a.n_seeds += b.n_seeds;
+    a.n_row_visits += b.n_row_visits; a.n_tracklet_hits += b.n_tracklet_hits; a.n_tracks += b.n_tracks;
+    a.n_track_hits += b.n_track_hits; a.n_kernel_launches += b.n_kernel_launches; a.n_retries += b.n_retries;
 }
 
 }  // namespace
@@ -282,24 +444,22 @@ tpc_tracker* tpc_tracker_create_ex(const tpc_geometry* g, float bz, const tpc_pa
     t->c.p = p;
     if (g->sector_alpha) t->sector_alpha.assign(g->sector_alpha, g->sector_alpha + g->n_sectors);
     cudaDeviceGetAttribute(&t->sm_count, cudaDevAttrMultiProcessorCount, dev);
-    if (cudaStreamCreateWithFlags(&t->own_stream, cudaStreamNonBlocking) != cudaSuccess) {
-        set_err("cudaStreamCreate failed");
-        delete t;
-        return nullptr;
-    }
-    t->stream = t->own_stream;
+    if (t->sm_count > kMaxSM) { set_err("more than %d SMs", kMaxSM); delete t; return nullptr; }
     {   // persistent constructor grid: as many CTAs as are resident at once
         int per_sm = 0;
         if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_construct, kKfThreads, 0) != cudaSuccess || per_sm < 1) {
             set_err("k_construct cannot be configured: %s", cudaGetErrorString(cudaGetLastError()));
-            cudaStreamDestroy(t->own_stream); delete t;
+            delete t;
             return nullptr;
         }
         t->kf_blocks = t->sm_count * per_sm;
     }
+    if (const char* ge = getenv("TPCTRACK_GROUP_EVENTS")) t->group_events = atoi(ge);
+    Batch* b0 = get_slot(t, 0);
+    if (!b0) { t->free_all(); delete t; return nullptr; }
     if (max_events > 0 && max_clusters > 0) {
-        if (reserve_batch(t, max_events, max_clusters, default_seed_cap(max_clusters)) != TPC_OK) {
-            t->free_all(); cudaStreamDestroy(t->own_stream); delete t;
+        if (reserve_batch(t, b0, max_events, max_clusters, default_seed_cap(max_clusters)) != TPC_OK) {
+            t->free_all(); delete t;
             return nullptr;
         }
     }
@@ -310,16 +470,20 @@ tpc_tracker* tpc_tracker_create(const tpc_geometry* g, float bz) { return tpc_tr
 
 void tpc_tracker_destroy(tpc_tracker* t) {
     if (!t) return;
-    cudaStreamSynchronize(t->stream);
+    t->sync_all();
     t->free_all();
-    if (t->own_stream) cudaStreamDestroy(t->own_stream);
-    for (auto& e : t->evt) if (e) cudaEventDestroy(e);
     delete t;
 }
 
 int tpc_tracker_set_stream(tpc_tracker* t, void* s) {
     if (!t) return TPC_ERR_ARG;
-    t->stream = s ? (cudaStream_t)s : t->own_stream;
+    t->user_stream = (cudaStream_t)s;
+    return TPC_OK;
+}
+
+int tpc_tracker_set_group_events(tpc_tracker* t, int32_t n) {
+    if (!t || n < 0) return TPC_ERR_ARG;
+    t->group_events = n;
     return TPC_OK;
 }
 
@@ -328,132 +492,103 @@ int tpc_track_events(tpc_tracker* t, int32_t n, const tpc_event_in* in, tpc_even
     if (rc != TPC_OK) return rc;
     if (!out) { set_err("null output array"); return TPC_ERR_ARG; }
     t->have_result = false;
-    const int ns = t->c.n_sectors, nr = t->c.n_rows;
-    int64_t N = 0;
-    t->ev_n.assign(n, 0); t->ev_off.assign(n + 1, 0);
-    for (int e = 0; e < n; e++) { t->ev_n[e] = in[e].n_clusters; t->ev_off[e] = (int32_t)N; N += in[e].n_clusters; }
-    t->ev_off[n] = (int32_t)N;
-    if (N > 0x7fff0000ll) { set_err("batch holds more than 2^31 clusters"); return TPC_ERR_CAPACITY; }
-    const bool host_in = in[0].mem_space == 0;
-    int64_t S_cap = std::max<int64_t>(t->S_cap, default_seed_cap(N));
     memset(&t->counters, 0, sizeof t->counters);
-    cudaStream_t st = t->stream;
+    for (float& m : t->stage_ms) m = 0.f;
+    const bool host_in = in[0].mem_space == 0;
+    int64_t N = 0;
+    for (int e = 0; e < n; e++) N += in[e].n_clusters;
 
-    bool done = false;
-    for (int attempt = 0; attempt < 3; attempt++) {
-        if ((rc = reserve_batch(t, n, N, S_cap)) != TPC_OK) return rc;
-        if (host_in) {
-            const size_t nn = (size_t)std::max<int64_t>(N, 1);
-            if ((rc = t->in_y.reserve(nn)) != TPC_OK || (rc = t->in_z.reserve(nn)) != TPC_OK ||
-                (rc = t->in_row.reserve(nn)) != TPC_OK)
-                return rc;
+    // Groups of events.  Device inputs: one group (every launch covers the whole batch).  Host inputs: a few groups
+    // on their own streams, so that the copies of one group overlap the kernels of another.
+    int per_group = n;
+    if (host_in && n > 1) {
+        if (t->group_events > 0) per_group = std::min<int>(t->group_events, n);
+        else {
+            const int want = (int)std::min<int64_t>(4, std::max<int64_t>(1, N / 2000000));   // >= ~2 M clusters per group
+            per_group = (n + want - 1) / want;
         }
-        // stage the event table and sector offsets
-        for (int e = 0; e < n; e++) {
-            EventSrc& s = t->h_ev_src.p[e];
-            s.n = in[e].n_clusters; s.off = t->ev_off[e];
-            if (host_in) {
-                s.y = t->in_y.p + s.off; s.z = t->in_z.p + s.off; s.row = t->in_row.p + s.off;
-                if (attempt == 0 && s.n > 0) {
-                    CK(cudaMemcpyAsync(t->in_y.p + s.off, in[e].y, sizeof(float) * s.n, cudaMemcpyHostToDevice, st));
-                    CK(cudaMemcpyAsync(t->in_z.p + s.off, in[e].z, sizeof(float) * s.n, cudaMemcpyHostToDevice, st));
-                    CK(cudaMemcpyAsync(t->in_row.p + s.off, in[e].row, sizeof(int32_t) * s.n, cudaMemcpyHostToDevice, st));
-                }
-            } else {
-                s.y = in[e].y; s.z = in[e].z; s.row = in[e].row;
+    }
+    const int n_groups = (n + per_group - 1) / per_group;
+    const int n_slots = std::min(n_groups, 3);
+    for (int k = 0; k < n_slots; k++)
+        if (!get_slot(t, k)) return TPC_ERR_CUDA;
+    for (int k = 0; k < n_slots; k++) {
+        t->slots[k]->stream = (n_groups == 1 && t->user_stream) ? t->user_stream : t->own_streams[k];
+        memset(&t->slots[k]->counters, 0, sizeof(tpc_counters));
+    }
+    t->ev_slot.assign(n, -1); t->ev_local.assign(n, 0);
+    t->n_events = n;
+
+    int64_t T_cum = 0, H_cum = 0;
+    std::vector<int64_t> trk_off(n + 1, 0), hit_off(n + 1, 0);   // per event, in the call's output arrays
+    std::vector<const Batch*> ev_batch(n, nullptr);
+    int g_issue = 0, g_done = 0;
+    while (g_done < n_groups) {
+        while (g_issue < n_groups && g_issue - g_done < n_slots) {
+            Batch* b = t->slots[g_issue % n_slots];
+            const int e0 = g_issue * per_group, ne = std::min(per_group, n - e0);
+            memset(&b->counters, 0, sizeof(tpc_counters));
+            if ((rc = batch_begin(t, b, e0, ne, in + e0, 0, true)) != TPC_OK) { t->sync_all(); return rc; }
+            g_issue++;
+        }
+        Batch* b = t->slots[g_done % n_slots];
+        if ((rc = batch_finish(t, b)) != TPC_OK) { t->sync_all(); return rc; }
+        add_counters(t->counters, b->counters);
+        if (t->profiling) for (int k = 0; k < TPC_N_STAGES; k++) t->stage_ms[k] += b->stage_ms[k];
+        const int64_t T = b->counters.n_tracks, H = b->counters.n_track_hits;
+        const int e0 = b->first_event, ne = b->n_events;
+        const int32_t* toff = b->h_ev_off.p;
+        const int32_t* hoff = b->h_ev_off.p + (ne + 1);
+        for (int e = 0; e < ne; e++) {
+            trk_off[e0 + e] = T_cum + toff[e]; hit_off[e0 + e] = H_cum + hoff[e];
+            out[e0 + e].n_tracks = toff[e + 1] - toff[e];
+            out[e0 + e].n_track_hits = hoff[e + 1] - hoff[e];
+        }
+        for (int e = 0; e < n; e++) if (t->ev_slot[e] == g_done % n_slots) t->ev_slot[e] = -1;   // overwritten
+        for (int e = 0; e < ne; e++) { t->ev_slot[e0 + e] = g_done % n_slots; t->ev_local[e0 + e] = e; }
+        if (host_in) {   // the group's tracks go behind those of the groups before it
+            const size_t left = (size_t)(n_groups - g_done - 1);
+            const View& v = b->v;
+            const int32_t* oi[4] = {v.o_sector, v.o_first_hit, v.o_n_hits, v.o_ndf};
+            const float* of[7] = {v.o_x, v.o_y, v.o_z, v.o_sinphi, v.o_tgl, v.o_qpt, v.o_chi2};
+            const size_t needT = (size_t)std::max<int64_t>(T_cum + T, 1), hintT = needT + needT / 8 + left * (size_t)(T + T / 4);
+            const size_t needH = (size_t)std::max<int64_t>(H_cum + H, 1), hintH = needH + needH / 8 + left * (size_t)(H + H / 4);
+            for (int k = 0; k < 4; k++) {
+                if ((rc = grow_keep(t, t->h_o_i[k], needT, (size_t)T_cum, hintT)) != TPC_OK) return rc;
+                if (T) CK(cudaMemcpyAsync(t->h_o_i[k].p + T_cum, oi[k], sizeof(int32_t) * T, cudaMemcpyDeviceToHost, b->stream));
             }
-            memcpy(t->h_sec_off.p + (size_t)e * (ns + 1), in[e].sector_offset, sizeof(int32_t) * (ns + 1));
+            for (int k = 0; k < 7; k++) {
+                if ((rc = grow_keep(t, t->h_o_f[k], needT, (size_t)T_cum, hintT)) != TPC_OK) return rc;
+                if (T) CK(cudaMemcpyAsync(t->h_o_f[k].p + T_cum, of[k], sizeof(float) * T, cudaMemcpyDeviceToHost, b->stream));
+            }
+            if ((rc = grow_keep(t, t->h_o_hit, needH, (size_t)H_cum, hintH)) != TPC_OK) return rc;
+            if (H) CK(cudaMemcpyAsync(t->h_o_hit.p + H_cum, v.o_hit_idx, sizeof(int32_t) * H, cudaMemcpyDeviceToHost, b->stream));
+        } else {
+            for (int e = 0; e < ne; e++) ev_batch[e0 + e] = b;
         }
-        CK(cudaMemcpyAsync(t->ev_src.p, t->h_ev_src.p, sizeof(EventSrc) * n, cudaMemcpyHostToDevice, st));
-        CK(cudaMemcpyAsync(t->sec_off.p, t->h_sec_off.p, sizeof(int32_t) * (size_t)n * (ns + 1), cudaMemcpyHostToDevice, st));
-
-        View& v = t->v;
-        v.n_events = n; v.n_tasks = n * ns; v.n_bins = n * ns * nr; v.N = (int32_t)N;
-        v.ev = t->ev_src.p; v.sec_off = t->sec_off.p;
-        v.bin_count = t->bin_count.p; v.bin_start = t->bin_start.p; v.slot = t->slot.p;
-        v.thit = t->thit.p; v.tidx = t->tidx.p; v.shit = t->shit.p; v.sorig = t->sorig.p;
-        v.desc = t->desc.p; v.cells = t->cells.p;
-        v.link_up = t->link_up.p; v.link_dn = t->link_dn.p; v.clink_up = t->clink_up.p; v.clink_dn = t->clink_dn.p;
-        v.seed_count = t->seed_count.p; v.seed_start = t->seed_start.p; v.seeds = t->seeds.p; v.seed_bin = t->seed_bin.p;
-        v.S_cap = (int32_t)t->S_cap;
-        v.tl_tab = t->tl_tab.p; v.tab_stride = tab_stride(nr); v.tl_rows = t->tl_rows.p; v.tl_par = t->tl_par.p;
-        v.owner = t->owner.p; v.tl_nown = t->tl_nown.p; v.tl_keep = t->tl_keep.p;
-        v.trk_scan = t->trk_scan.p; v.hit_scan = t->hit_scan.p; v.ev_off = t->ev_off_d.p;
-        v.o_sector = t->o_i[0].p; v.o_first_hit = t->o_i[1].p; v.o_n_hits = t->o_i[2].p; v.o_ndf = t->o_i[3].p;
-        v.o_hit_idx = t->o_hit.p;
-        v.o_x = t->o_f[0].p; v.o_y = t->o_f[1].p; v.o_z = t->o_f[2].p; v.o_sinphi = t->o_f[3].p;
-        v.o_tgl = t->o_f[4].p; v.o_qpt = t->o_f[5].p; v.o_chi2 = t->o_f[6].p;
-        v.cnt = t->cnt.p;
-        t->n_events = n; t->N = N; t->mem_space = in[0].mem_space;
-
-        // keep / nown must read as 0 beyond the seed count
-        CK(cudaMemsetAsync(v.tl_keep, 0, sizeof(int32_t) * (size_t)(t->S_cap + 1), st));
-        CK(cudaMemsetAsync(v.tl_nown, 0, sizeof(int32_t) * (size_t)(t->S_cap + 1), st));
-        if ((rc = launch_all(t, &t->counters.n_kernel_launches)) != TPC_OK) return rc;
-        CK(cudaMemcpyAsync(t->h_cnt.p, v.cnt, sizeof(unsigned long long) * CNT_CURSOR, cudaMemcpyDeviceToHost, st));
-        CK(cudaMemcpyAsync(t->h_ev_off.p, v.ev_off, sizeof(int32_t) * 2 * (n + 1), cudaMemcpyDeviceToHost, st));
-        int32_t n_seeds = 0;
-        CK(cudaMemcpyAsync(&n_seeds, v.seed_start + v.n_bins, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
-        CK(cudaStreamSynchronize(st));
-        if (t->profiling)
-            for (int k = 0; k < TPC_N_STAGES; k++) cudaEventElapsedTime(&t->stage_ms[k], t->evt[k], t->evt[k + 1]);
-        const unsigned err = (unsigned)(t->h_cnt.p[CNT_ERR] & 0xffffffffu);
-        if (err & kErrBadRow) { set_err("a cluster has row outside [0,%d)", nr); return TPC_ERR_ARG; }
-        if (err & kErrRowCapacity) {
-            set_err("more than %d clusters in one (sector,row)", TPC_MAX_ROW_HITS);
-            return TPC_ERR_CAPACITY;
-        }
-        if ((err & kErrSeedCapacity) || n_seeds > t->S_cap) {  // grow the tracklet pools and run again
-            S_cap = (int64_t)n_seeds + n_seeds / 8 + 1024;
-            t->counters.n_retries++;
-            continue;
-        }
-        t->counters.n_events = n; t->counters.n_clusters = N;
-        t->counters.n_links = (int64_t)t->h_cnt.p[CNT_LINKS];
-        t->counters.n_seeds = n_seeds;
-        t->counters.n_row_visits = (int64_t)t->h_cnt.p[CNT_ROW_VISITS];
-        t->counters.n_tracklet_hits = (int64_t)t->h_cnt.p[CNT_TL_HITS];
-        t->counters.n_tracks = (int64_t)t->h_cnt.p[CNT_TRACKS];
-        t->counters.n_track_hits = (int64_t)t->h_cnt.p[CNT_TRACK_HITS];
-        done = true;
-        break;
+        T_cum += T; H_cum += H;
+        g_done++;
     }
-    if (!done) {
-        set_err("tracklet pool could not be grown");
-        return TPC_ERR_CAPACITY;
-    }
-    // outputs
-    const int64_t T = t->counters.n_tracks, H = t->counters.n_track_hits;
-    const View& v = t->v;
-    const int32_t* toff = t->h_ev_off.p;
-    const int32_t* hoff = t->h_ev_off.p + (n + 1);
-    const int32_t* oi[4] = {v.o_sector, v.o_first_hit, v.o_n_hits, v.o_ndf};
-    const float* of[7] = {v.o_x, v.o_y, v.o_z, v.o_sinphi, v.o_tgl, v.o_qpt, v.o_chi2};
-    const int32_t* ohit = v.o_hit_idx;
-    if (host_in) {
-        for (int k = 0; k < 4; k++) {
-            if ((rc = t->h_o_i[k].reserve((size_t)std::max<int64_t>(T, 1))) != TPC_OK) return rc;
-            if (T) CK(cudaMemcpyAsync(t->h_o_i[k].p, oi[k], sizeof(int32_t) * T, cudaMemcpyDeviceToHost, st));
-            oi[k] = t->h_o_i[k].p;
-        }
-        for (int k = 0; k < 7; k++) {
-            if ((rc = t->h_o_f[k].reserve((size_t)std::max<int64_t>(T, 1))) != TPC_OK) return rc;
-            if (T) CK(cudaMemcpyAsync(t->h_o_f[k].p, of[k], sizeof(float) * T, cudaMemcpyDeviceToHost, st));
-            of[k] = t->h_o_f[k].p;
-        }
-        if ((rc = t->h_o_hit.reserve((size_t)std::max<int64_t>(H, 1))) != TPC_OK) return rc;
-        if (H) CK(cudaMemcpyAsync(t->h_o_hit.p, ohit, sizeof(int32_t) * H, cudaMemcpyDeviceToHost, st));
-        ohit = t->h_o_hit.p;
-        CK(cudaStreamSynchronize(st));
-    }
+    if (host_in)
+        for (int k = 0; k < n_slots; k++) CK(cudaStreamSynchronize(t->slots[k]->stream));
     for (int e = 0; e < n; e++) {
         tpc_event_out& o = out[e];
-        const int32_t a = toff[e], b = toff[e + 1];
-        o.n_tracks = b - a; o.n_track_hits = hoff[e + 1] - hoff[e];
+        const int32_t* oi[4]; const float* of[7]; const int32_t* ohit;
+        int64_t a = trk_off[e], h = hit_off[e];
+        if (host_in) {
+            for (int k = 0; k < 4; k++) oi[k] = t->h_o_i[k].p;
+            for (int k = 0; k < 7; k++) of[k] = t->h_o_f[k].p;
+            ohit = t->h_o_hit.p;
+        } else {
+            const View& v = ev_batch[e]->v;
+            oi[0] = v.o_sector; oi[1] = v.o_first_hit; oi[2] = v.o_n_hits; oi[3] = v.o_ndf;
+            of[0] = v.o_x; of[1] = v.o_y; of[2] = v.o_z; of[3] = v.o_sinphi; of[4] = v.o_tgl; of[5] = v.o_qpt; of[6] = v.o_chi2;
+            ohit = v.o_hit_idx;
+        }
         o.trk_sector = oi[0] + a; o.trk_first_hit = oi[1] + a; o.trk_n_hits = oi[2] + a; o.trk_ndf = oi[3] + a;
         o.trk_x = of[0] + a; o.trk_y = of[1] + a; o.trk_z = of[2] + a; o.trk_sinphi = of[3] + a; o.trk_tgl = of[4] + a;
         o.trk_qpt = of[5] + a; o.trk_chi2 = of[6] + a;
-        o.hit_idx = ohit + hoff[e];
+        o.hit_idx = ohit + h;
     }
     t->have_result = true;
     return TPC_OK;
@@ -463,9 +598,6 @@ int tpc_track_event(tpc_tracker* t, const tpc_event_in* in, tpc_event_out* out) 
 
 int tpc_tracker_set_profiling(tpc_tracker* t, int32_t on) {
     if (!t) return TPC_ERR_ARG;
-    if (on)
-        for (auto& e : t->evt)
-            if (!e) CK(cudaEventCreate(&e));
     t->profiling = on != 0;
     return TPC_OK;
 }
@@ -483,9 +615,13 @@ int tpc_get_counters(const tpc_tracker* t, tpc_counters* c) {
 }
 
 // ---- intermediates (host-side conversion to the caller's indices; not on the hot path) ----
-static int dbg_ranges(const tpc_tracker* t, int event, int* g0, int* g1, int* s0, int* s1) {
-    if (!t || !t->have_result || event < 0 || event >= t->n_events) { set_err("no result / bad event"); return TPC_ERR_ARG; }
-    const int bpe = t->c.n_sectors * t->c.n_rows;
+static int dbg_ranges(const tpc_tracker* tr, int& event, const Batch** bp, int* g0, int* g1, int* s0, int* s1) {
+    if (!tr || !tr->have_result || event < 0 || event >= tr->n_events) { set_err("no result / bad event"); return TPC_ERR_ARG; }
+    if (tr->ev_slot[event] < 0) { set_err("the intermediates of event %d have been overwritten by a later group", event); return TPC_ERR_ARG; }
+    const Batch* t = tr->slots[tr->ev_slot[event]];
+    event = tr->ev_local[event];
+    *bp = t;
+    const int bpe = tr->c.n_sectors * tr->c.n_rows;
     int32_t r[2], q[2];
     cudaStreamSynchronize(t->stream);
     if (cudaMemcpy(&r[0], t->v.bin_start + (size_t)event * bpe, 4, cudaMemcpyDeviceToHost) != cudaSuccess ||
@@ -499,9 +635,10 @@ static int dbg_ranges(const tpc_tracker* t, int event, int* g0, int* g1, int* s0
     return TPC_OK;
 }
 
-int64_t tpc_debug_size(const tpc_tracker* t, int32_t what, int32_t event) {
+int64_t tpc_debug_size(const tpc_tracker* tr, int32_t what, int32_t event) {
     int g0, g1, s0, s1;
-    int rc = dbg_ranges(t, event, &g0, &g1, &s0, &s1);
+    const Batch* t = nullptr;
+    int rc = dbg_ranges(tr, event, &t, &g0, &g1, &s0, &s1);
     if (rc != TPC_OK) return rc;
     const int64_t n = g1 - g0, s = s1 - s0;
     switch (what) {
@@ -510,19 +647,20 @@ int64_t tpc_debug_size(const tpc_tracker* t, int32_t what, int32_t event) {
         case TPC_DBG_START_HIT: return 4 * s;
         case TPC_DBG_TL_ROWS: return 12 * s;
         case TPC_DBG_TL_PAR: return 24 * s;
-        case TPC_DBG_TL_TABLE: return 4 * s * t->c.n_rows;
+        case TPC_DBG_TL_TABLE: return 4 * s * tr->c.n_rows;
         default: set_err("unknown debug item"); return TPC_ERR_ARG;
     }
 }
 
-int tpc_debug_get(tpc_tracker* t, int32_t what, int32_t event, void* buf, size_t bytes) {
+int tpc_debug_get(tpc_tracker* tr, int32_t what, int32_t event, void* buf, size_t bytes) {
     int g0, g1, s0, s1;
-    int rc = dbg_ranges(t, event, &g0, &g1, &s0, &s1);
+    const int64_t need = tpc_debug_size(tr, what, event);
+    const Batch* t = nullptr;
+    int rc = dbg_ranges(tr, event, &t, &g0, &g1, &s0, &s1);
     if (rc != TPC_OK) return rc;
-    const int64_t need = tpc_debug_size(t, what, event);
     if (need < 0) return (int)need;
     if (!buf || bytes < (size_t)need) { set_err("debug buffer too small: need %lld bytes", (long long)need); return TPC_ERR_ARG; }
-    const int n = g1 - g0, s = s1 - s0, nr = t->c.n_rows;
+    const int n = g1 - g0, s = s1 - s0, nr = tr->c.n_rows;
     std::vector<int32_t> sorig(std::max(n, 1));
     if (n) CK(cudaMemcpy(sorig.data(), t->v.sorig + g0, 4 * (size_t)n, cudaMemcpyDeviceToHost));
     auto to_orig = [&](int32_t g) { return g < 0 ? -1 : sorig[g - g0]; };
@@ -563,7 +701,7 @@ int tpc_debug_get(tpc_tracker* t, int32_t what, int32_t event, void* buf, size_t
             const int stride = t->v.tab_stride;
             std::vector<int32_t> rows(s), sbin(s);
             std::vector<uint16_t> tab((size_t)s * stride);
-            const int bpe = t->c.n_sectors * nr;
+            const int bpe = tr->c.n_sectors * nr;
             std::vector<BinDesc> desc(bpe);
             CK(cudaMemcpy(rows.data(), t->v.tl_rows + s0, 4 * (size_t)s, cudaMemcpyDeviceToHost));
             CK(cudaMemcpy(sbin.data(), t->v.seed_bin + s0, 4 * (size_t)s, cudaMemcpyDeviceToHost));

@@ -11,7 +11,9 @@ from pathlib import Path
 
 import numpy as np
 
-LIB_PATH = Path(__file__).resolve().parent / "csrc" / "libtpctrack.so"
+import os
+
+LIB_PATH = Path(os.environ.get("TPCTRACK_LIB") or Path(__file__).resolve().parent / "csrc" / "libtpctrack.so")
 
 TPC_OK, TPC_ERR_ARG, TPC_ERR_GEOMETRY, TPC_ERR_CAPACITY, TPC_ERR_CUDA = 0, -1, -2, -3, -4
 DBG = {"link_up": 0, "link_dn": 1, "clink_up": 2, "clink_dn": 3, "start_hit": 4, "tl_rows": 5, "tl_par": 6,
@@ -75,6 +77,7 @@ def _load():
     lib.tpc_tracker_create_ex.restype = C.c_void_p
     lib.tpc_tracker_create_ex.argtypes = [C.POINTER(tpc_geometry), C.c_float, C.POINTER(tpc_params), C.c_int32, C.c_int64]
     lib.tpc_tracker_set_stream.argtypes = [C.c_void_p, C.c_void_p]
+    lib.tpc_tracker_set_group_events.argtypes = [C.c_void_p, C.c_int32]
     lib.tpc_track_event.argtypes = [C.c_void_p, C.POINTER(tpc_event_in), C.POINTER(tpc_event_out)]
     lib.tpc_track_events.argtypes = [C.c_void_p, C.c_int32, C.POINTER(tpc_event_in), C.POINTER(tpc_event_out)]
     lib.tpc_tracker_destroy.argtypes = [C.c_void_p]
@@ -94,6 +97,7 @@ def _load():
 lib = _load()
 
 EXPORTS = ("tpc_default_params", "tpc_tracker_create", "tpc_tracker_create_ex", "tpc_tracker_set_stream",
+           "tpc_tracker_set_group_events",
            "tpc_track_event", "tpc_track_events", "tpc_tracker_destroy", "tpc_status_string", "tpc_last_error",
            "tpc_get_counters", "tpc_tracker_set_profiling", "tpc_get_stage_ms", "tpc_debug_size", "tpc_debug_get")
 
@@ -141,6 +145,9 @@ class Tracker:
 
     def set_stream(self, cuda_stream_ptr: int | None):
         _check(lib.tpc_tracker_set_stream(self._h, C.c_void_p(cuda_stream_ptr or 0)))
+
+    def tpc_tracker_set_group_events(self, n: int):
+        _check(lib.tpc_tracker_set_group_events(self._h, int(n)))
 
     # ---- marshalling ----
     @staticmethod

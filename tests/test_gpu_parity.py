@@ -122,6 +122,35 @@ def test_parity_batch_of_events_matches_single_events(trk_mod, gen_mod, oracle_m
     trk.close()
 
 
+@pytest.mark.parametrize("per_group", [1, 2, 0])
+def test_host_batches_run_as_overlapping_groups(trk_mod, gen_mod, oracle_mod, per_group):
+    """Host-input batches are cut into groups of events on separate streams (copies of one group overlap the
+    kernels of another); 7 events in groups of 1 also cycle the three slots.  Results must not depend on it."""
+    evs = [gen_mod.generate("pp", e) for e in range(4)] + [gen_mod.generate("semicentral", 0)] + \
+          [gen_mod.generate("pp", e) for e in range(4, 6)]
+    trk = make_tracker(trk_mod, gen_mod, evs[0])
+    trk.tpc_tracker_set_group_events(per_group)
+    outs = trk.tpc_track_events([ev_dict(ev, False) for ev in evs])
+    res = [trk.to_numpy(o) for o in outs]
+    c = trk.tpc_get_counters()
+    assert c["n_events"] == len(evs) and c["n_clusters"] == sum(ev.n_clusters for ev in evs)
+    assert c["n_tracks"] == sum(r["n_tracks"] for r in res)
+    for e, ev in enumerate(evs):
+        ref = oracle_mod.track_event(make_geometry(oracle_mod, gen_mod, ev), ev.sector_offset, ev.y, ev.z, ev.row,
+                                     precision="float")
+        assert res[e]["n_tracks"] == ref.n_tracks
+        for k in ("trk_sector", "trk_first_hit", "trk_n_hits", "trk_ndf", "hit_idx"):
+            assert np.array_equal(res[e][k], ref[k]), (e, k)
+        for k in ("trk_y", "trk_z", "trk_sinphi", "trk_tgl", "trk_qpt", "trk_chi2"):
+            err = np.abs(res[e][k] - ref[k]) / np.maximum(1.0, np.abs(ref[k]))
+            assert err.max(initial=0.0) <= TOL, (e, k, err.max())
+    if per_group == 1:   # events of the last three groups keep their intermediates, earlier ones do not
+        assert np.array_equal(trk.tpc_debug_get("start_hit", 6), ref.start_hit)
+        with pytest.raises(trk_mod.TpcError):
+            trk.tpc_debug_get("start_hit", 0)
+    trk.close()
+
+
 @pytest.mark.parametrize("step", [1, 2])
 def test_parity_link_step_and_dense_rows(trk_mod, gen_mod, oracle_mod, step):
     p = oracle_mod.default_params()
