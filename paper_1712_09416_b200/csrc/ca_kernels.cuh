@@ -20,22 +20,62 @@ __device__ __forceinline__ int sector_of(const int32_t* so, int ns, int i) {
     return lo;
 }
 
+constexpr int kCountPer = 8;                    // clusters per thread
+constexpr int kCountChunk = 256 * kCountPer;    // clusters per CTA
+constexpr int kCountBins = 2048;                // (sector,row) bins of a chunk counted in shared memory
+
 __global__ void __launch_bounds__(256) k_count(const View v, int ns, int nr) {
     __shared__ int32_t so[64 + 1];
+    __shared__ int32_t hist[kCountBins];   // clusters of this chunk per bin, then the chunk's first slot in the bin
     const int e = blockIdx.y;
     const EventSrc src = v.ev[e];
-    if (blockIdx.x * 256 >= src.n) return;
+    const int i0 = blockIdx.x * kCountChunk;
+    if (i0 >= src.n) return;
+    const int i1 = min(i0 + kCountChunk, src.n);
     for (int k = threadIdx.x; k <= ns; k += 256) so[k] = v.sec_off[e * (ns + 1) + k];
     __syncthreads();
-    const int i = blockIdx.x * 256 + threadIdx.x;
-    if (i >= src.n) return;
-    const int r = src.row[i];
-    if (r < 0 || r >= nr) { atomicOr((unsigned int*)&v.cnt[CNT_ERR], kErrBadRow); return; }
-    const int s = sector_of(so, ns, i);
-    const int bin = (e * ns + s) * nr + r;
-    const int sl = atomicAdd(&v.bin_count[bin], 1);
-    if (sl >= TPC_MAX_ROW_HITS) atomicOr((unsigned int*)&v.cnt[CNT_ERR], kErrRowCapacity);
-    v.slot[src.off + i] = (uint16_t)min(sl, 65535);
+    // a chunk of consecutive clusters spans few sectors: its bins are counted in shared memory and every bin
+    // is then reserved with ONE global atomic per chunk
+    const int s_lo = sector_of(so, ns, i0), s_hi = sector_of(so, ns, i1 - 1);
+    const int nb = (s_hi - s_lo + 1) * nr;
+    const int bin0 = (e * ns + s_lo) * nr;
+    const bool local = nb <= kCountBins;
+    if (local) for (int b = threadIdx.x; b < nb; b += 256) hist[b] = 0;
+    __syncthreads();
+    uint32_t pk[kCountPer];   // bin within the chunk << 12 | arrival rank within the chunk
+#pragma unroll
+    for (int k = 0; k < kCountPer; k++) {
+        const int i = i0 + k * 256 + threadIdx.x;
+        pk[k] = 0xffffffffu;
+        if (i < i1) {
+            const int r = src.row[i];
+            if (r < 0 || r >= nr) { atomicOr((unsigned int*)&v.cnt[CNT_ERR], kErrBadRow); continue; }
+            int s = s_lo;
+            while (i >= so[s + 1]) s++;
+            const int bl = (s - s_lo) * nr + r;
+            if (local) pk[k] = ((uint32_t)bl << 12) | (uint32_t)atomicAdd(&hist[bl], 1);
+            else {
+                const int sl = atomicAdd(&v.bin_count[bin0 + bl], 1);
+                if (sl >= TPC_MAX_ROW_HITS) atomicOr((unsigned int*)&v.cnt[CNT_ERR], kErrRowCapacity);
+                v.slot[src.off + i] = (uint16_t)min(sl, 65535);
+            }
+        }
+    }
+    if (!local) return;
+    __syncthreads();
+    for (int b = threadIdx.x; b < nb; b += 256) {
+        const int cnt = hist[b];
+        if (cnt) hist[b] = atomicAdd(&v.bin_count[bin0 + b], cnt);
+    }
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < kCountPer; k++) {
+        if (pk[k] == 0xffffffffu) continue;
+        const int i = i0 + k * 256 + threadIdx.x;
+        const int sl = hist[pk[k] >> 12] + (int)(pk[k] & 0xfffu);
+        if (sl >= TPC_MAX_ROW_HITS) atomicOr((unsigned int*)&v.cnt[CNT_ERR], kErrRowCapacity);
+        v.slot[src.off + i] = (uint16_t)min(sl, 65535);
+    }
 }
 
 // K1b: move (y, z, index) into the bin, arrival order.

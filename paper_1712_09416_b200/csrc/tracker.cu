@@ -214,7 +214,7 @@ int launch_all(const tpc_tracker* tr, Batch* t) {
     int maxn = 0;
     for (int e = 0; e < t->n_events; e++) maxn = std::max(maxn, t->ev_n[e]);
     if (maxn > 0) {
-        dim3 g((maxn + 255) / 256, t->n_events);
+        dim3 g((maxn + kCountChunk - 1) / kCountChunk, t->n_events);
         k_count<<<g, 256, 0, st>>>(v, ns, nr); L++;
     }
     L += scan_exclusive(v.bin_count, v.bin_start, nb, t->scratch.p, st);
