@@ -32,7 +32,8 @@ __device__ __forceinline__ bool fit_transport(Fit& f, float x, float x1, const C
     const float icc = 1.f / (c0 + c1), ic0 = 1.f / c0, ic1 = 1.f / c1;
     const float dy = dx * ((s + s1) * icc);
     const float dl2 = dx * dx + dy * dy;
-    const float dl = (dx < 0.f) ? -sqrtf(dl2) : sqrtf(dl2);
+    const float adl = sqrtf(dl2);
+    const float dl = (dx < 0.f) ? -adl : adl;
     const float idl = 1.f / dl;
     const float u = kap * dl, u2 = u * u;
     const float c24 = 1.f / 24.f, c640 = 3.f / 640.f, c12 = 1.f / 12.f;
@@ -132,41 +133,28 @@ __device__ __forceinline__ uint32_t tl_key(const View& v, int i, int nh, int tas
 // hit from a device counter at once.
 //   phase 1: up pass, following the cleaned links      phase 2: up pass, extending by search
 //   phase 3: down pass = fresh fit from the top hit through everything recorded, searching the empty rows
-// Window searches are shared out over the warp: every lane that needs one posts its
-// query (predicted y, z, window, weights, cell window) in shared memory; the queries are cut into work items
-// of one grid row each (the candidates of a grid row are contiguous in memory) and the 32 lanes take one item
-// each; the owner lane then merges its items' results.  The best hit = min gate value, exact ties -> lowest
-// caller's index, whatever the order of evaluation.
+// Window search: the candidates of one grid row of the window are contiguous in memory and
+// are loaded kKfUnroll at a time; the best hit = min gate value, exact ties -> lowest caller's index, whatever the
+// order of evaluation.  The warp is brought together (__syncwarp) before the transport, the search and the update,
+// so that each runs once per trip for all lanes that need it.
 // The row -> hit table of a tracklet ([tracklet][row], row-local 16-bit hit numbers) is written as the passes
 // go; when a tracklet ends, its warp claims the hits of rows first..last for the selector (K6a: atomicMax of the
 // tracklet's key on owner[hit]).
 // ---------------------------------------------------------------------------------------------------------
 constexpr int kKfThreads = 128;
 #ifndef TPC_KF_BLOCKS
-#define TPC_KF_BLOCKS 5
+#define TPC_KF_BLOCKS 6
 #endif
 #ifndef TPC_KF_UNROLL
-#define TPC_KF_UNROLL 4
+#define TPC_KF_UNROLL 2
 #endif
 constexpr int kKfBlocksPerSM = TPC_KF_BLOCKS;
 constexpr int kKfUnroll = TPC_KF_UNROLL;       // candidates of a grid row loaded at once
-constexpr int kKfMaxItems = 256;   // >= 32 lanes x grid rows a window can span (window <= 2 * 3 cm + pad, cells >= 1.2 cm)
-
-struct SearchQuery {
-    float y, z, wy, wz, iwy, iwz;  // predicted position, window half widths, 1 / (C + sigma^2)
-    int32_t base, bin;             // first sorted hit of the bin, the bin
-    uint32_t win;                  // ny | iy0 << 8 | iy1 << 16 | iz0 << 24
-};
 
 __global__ void __launch_bounds__(kKfThreads, kKfBlocksPerSM) k_construct(const View v, const __grid_constant__ Const c) {
-    __shared__ SearchQuery s_q[kKfThreads];
-    __shared__ float4 s_res[kKfThreads];                       // result of the item a lane took: gate, y, z, hit
-    __shared__ uint16_t s_item[kKfThreads / 32][kKfMaxItems];  // owner lane | grid row within the window << 8
     const int S = min(v.seed_start[v.n_bins], v.S_cap);
     const int nr = c.n_rows, D = c.p.link_step;
     const int lane = lane_id();
-    const int wbase = threadIdx.x & ~31;
-    uint16_t* const items = s_item[threadIdx.x >> 5];
     unsigned long long* const cursor = &v.cnt[CNT_CURSOR];   // [n_sm] start hits taken from each SM's share
     unsigned sm, n_sm_u;
     asm("mov.u32 %0, %%smid;" : "=r"(sm));
@@ -278,72 +266,39 @@ __global__ void __launch_bounds__(kKfThreads, kKfBlocksPerSM) k_construct(const 
             }
         }
 
-        // ---- part 2: the window searches of this trip, shared out over the warp ----
-        int n_iz = 0;
+        // ---- part 2: the window searches of this trip ----
+        __syncwarp();
         if (search && dn.y > 0) {
-            SearchQuery q;
-            q.y = f.y; q.z = f.z;
-            q.wy = fminf(fmaxf(c.p.win_nsigma * sqrtf(f.c00 + c.sigma_y2), c.p.win_min), c.p.win_max);
-            q.wz = fminf(fmaxf(c.p.win_nsigma * sqrtf(f.c11 + c.sigma_z2), c.p.win_min), c.p.win_max);
-            q.iwy = iwy; q.iwz = iwz;
+            const float wy = fminf(fmaxf(c.p.win_nsigma * sqrtf(f.c00 + c.sigma_y2), c.p.win_min), c.p.win_max);
+            const float wz = fminf(fmaxf(c.p.win_nsigma * sqrtf(f.c11 + c.sigma_z2), c.p.win_min), c.p.win_max);
             const float4 gf = load_desc_f(v, tb + row);
-            const CellWin w = cell_window(gf, dn.z, dn.w, q.y, q.z, q.wy, q.wz);
-            q.base = dn.x; q.bin = tb + row;
-            q.win = (uint32_t)dn.z | ((uint32_t)w.iy0 << 8) | ((uint32_t)w.iy1 << 16) | ((uint32_t)w.iz0 << 24);
-            s_q[threadIdx.x] = q;
-            n_iz = w.iz1 - w.iz0 + 1;
-        }
-        const int incl = warp_incl_scan(n_iz);
-        const int n_items = __shfl_sync(kFull, incl, 31);
-        if (n_items > 0) {
-            const int off = incl - n_iz;
-            for (int j = 0; j < n_iz; j++) items[off + j] = (uint16_t)(lane | (j << 8));
-            __syncwarp();
+            const CellWin w = cell_window(gf, dn.z, dn.w, f.y, f.z, wy, wz);
+            const uint16_t* cs = cell_table(v, tb + row, dn.x);
+            const float2* hits = v.shit + dn.x;
             float bg = 0.f;
             int bp = -1;
-            for (int t0 = 0; t0 < n_items; t0 += 32) {
-                float4 res = make_float4(0.f, 0.f, 0.f, __int_as_float(-1));
-                if (t0 + lane < n_items) {
-                    const int it = items[t0 + lane];
-                    const SearchQuery q = s_q[wbase + (it & 0xff)];
-                    const int ny = q.win & 0xff, iy0 = (q.win >> 8) & 0xff, iy1 = (q.win >> 16) & 0xff;
-                    const int iz = (int)(q.win >> 24) + (it >> 8);
-                    const uint16_t* cs = cell_table(v, q.bin, q.base);
-                    const float2* hits = v.shit + q.base;
-                    int p = __ldg(&cs[iz * ny + iy0]);
-                    const int pe = __ldg(&cs[iz * ny + iy1 + 1]);
-                    int rp = -1;
-                    for (; p < pe; p += kKfUnroll) {   // the candidates of a grid row are contiguous: loads go out together
-                        float2 h[kKfUnroll];
+            for (int iz = w.iz0; iz <= w.iz1; iz++) {
+                int p = __ldg(&cs[iz * dn.z + w.iy0]);
+                const int pe = __ldg(&cs[iz * dn.z + w.iy1 + 1]);
+                for (; p < pe; p += kKfUnroll) {   // the candidates of a grid row are contiguous: loads go out together
+                    float2 h[kKfUnroll];
 #pragma unroll
-                        for (int k = 0; k < kKfUnroll; k++) h[k] = __ldg(&hits[min(p + k, pe - 1)]);
+                    for (int k = 0; k < kKfUnroll; k++) h[k] = __ldg(&hits[min(p + k, pe - 1)]);
 #pragma unroll
-                        for (int k = 0; k < kKfUnroll; k++) {
-                            const float ry = h[k].x - q.y, rz = h[k].y - q.z;
-                            if (p + k < pe && fabsf(ry) <= q.wy && fabsf(rz) <= q.wz) {
-                                const float gv = (ry * ry) * q.iwy + (rz * rz) * q.iwz;   // the gate value of h[k]
-                                bool take = rp < 0 || gv < res.x;
-                                if (!take && gv == res.x) take = v.sorig[q.base + p + k] < v.sorig[q.base + rp];
-                                if (take) { res.x = gv; res.y = h[k].x; res.z = h[k].y; rp = p + k; }
-                            }
+                    for (int k = 0; k < kKfUnroll; k++) {
+                        const float ry = h[k].x - f.y, rz = h[k].y - f.z;
+                        if (p + k < pe && fabsf(ry) <= wy && fabsf(rz) <= wz) {
+                            const float gv = (ry * ry) * iwy + (rz * rz) * iwz;   // the gate value of h[k]
+                            bool take = bp < 0 || gv < bg;
+                            if (!take && gv == bg) take = v.sorig[dn.x + p + k] < v.sorig[dn.x + bp];
+                            if (take) { bg = gv; bp = p + k; ay = h[k].x; az = h[k].y; }
                         }
                     }
-                    res.w = __int_as_float(rp);
                 }
-                s_res[threadIdx.x] = res;
-                __syncwarp();
-                for (int t = max(off, t0); t < min(off + n_iz, t0 + 32); t++) {   // the owner merges its items
-                    const float4 r = s_res[wbase + t - t0];
-                    const int rp = __float_as_int(r.w);
-                    if (rp < 0) continue;
-                    bool take = bp < 0 || r.x < bg;
-                    if (!take && r.x == bg) take = v.sorig[dn.x + rp] < v.sorig[dn.x + bp];
-                    if (take) { bg = r.x; bp = rp; ay = r.y; az = r.z; }
-                }
-                __syncwarp();
             }
             if (bp >= 0 && bg <= c.p.chi2_ext) acc = dn.x + bp;
         }
+        __syncwarp();
 
         // ---- part 3: bookkeeping, update, end of a pass (the warp is brought together before each piece) ----
         bool finished = false, upd = false;
