@@ -22,9 +22,8 @@ constexpr unsigned kFull = 0xffffffffu;
 constexpr unsigned kErrBadRow = 1u, kErrRowCapacity = 2u, kErrSeedCapacity = 4u;
 
 // device counters (unsigned long long each)
-// CNT_CURSOR.. : one cursor per SM (K5 hands out the start hits SM by SM)
 constexpr int kMaxSM = 256;
-enum { CNT_ERR = 0, CNT_LINKS, CNT_ROW_VISITS, CNT_TL_HITS, CNT_TRACKS, CNT_TRACK_HITS, CNT_CURSOR, CNT_N = CNT_CURSOR + kMaxSM };
+enum { CNT_ERR = 0, CNT_LINKS, CNT_ROW_VISITS, CNT_TL_HITS, CNT_TRACKS, CNT_TRACK_HITS, CNT_N };
 
 // One event's input arrays (device pointers) and its place in the batch-global cluster numbering.
 struct EventSrc {
@@ -86,6 +85,7 @@ struct View {
     int32_t *o_sector, *o_first_hit, *o_n_hits, *o_ndf, *o_hit_idx;
     float *o_x, *o_y, *o_z, *o_sinphi, *o_tgl, *o_qpt, *o_chi2;
     unsigned long long* cnt; // [CNT_N]
+    unsigned long long* kf_cursor;  // [n_events * kMaxSM] K5: start hits handed out per (event, SM) share
 };
 
 __device__ __forceinline__ int lane_id() { return threadIdx.x & 31; }

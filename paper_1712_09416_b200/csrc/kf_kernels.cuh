@@ -145,6 +145,9 @@ constexpr int kKfThreads = 128;
 #ifndef TPC_KF_BLOCKS
 #define TPC_KF_BLOCKS 6
 #endif
+#ifndef TPC_KF_SCHED
+#define TPC_KF_SCHED 1
+#endif
 #ifndef TPC_KF_UNROLL
 #define TPC_KF_UNROLL 2
 #endif
@@ -155,8 +158,8 @@ __global__ void __launch_bounds__(kKfThreads, kKfBlocksPerSM) k_construct(const 
     const int S = min(v.seed_start[v.n_bins], v.S_cap);
     const int nr = c.n_rows, D = c.p.link_step;
     const int lane = lane_id();
-    unsigned long long* const cursor = &v.cnt[CNT_CURSOR];   // [n_sm] start hits taken from each SM's share
-    unsigned sm, n_sm_u;
+    unsigned long long* const cursor = v.kf_cursor;   // start hits taken from each share of the list
+    unsigned sm = 0, n_sm_u;
     asm("mov.u32 %0, %%smid;" : "=r"(sm));
     asm("mov.u32 %0, %%nsmid;" : "=r"(n_sm_u));
     const int n_sm = (int)n_sm_u;
@@ -179,6 +182,24 @@ __global__ void __launch_bounds__(kKfThreads, kKfBlocksPerSM) k_construct(const 
             int b = 0, e = 0;
             if (lane == 0) {
                 const int want = __popc(idle);
+#if TPC_KF_SCHED == 1
+                // one cursor for the whole list: all SMs work in the same narrow window of start hits
+                const int got = (int)atomicAdd(&cursor[0], (unsigned long long)want);
+                if (got < S) { b = got; e = S; } else victim = n_sm;
+#elif TPC_KF_SCHED == 2
+                // event by event: an SM takes its own share of every event first (the SMs then stay in the same
+                // one or two events, whose hits fit the L2), and only then the other SMs' shares
+                const int ne = v.n_events, bpe = c.n_sectors * nr;
+                while (victim < n_sm * ne) {
+                    const int vs = victim / ne, ev = victim - vs * ne;
+                    const int s = (sm + vs) % n_sm;
+                    const int e_lo = min(v.seed_start[ev * bpe], S), e_n = min(v.seed_start[(ev + 1) * bpe], S) - e_lo;
+                    const int lo = e_lo + (int)((long long)e_n * s / n_sm), hi = e_lo + (int)((long long)e_n * (s + 1) / n_sm);
+                    const int got = lo + (int)atomicAdd(&cursor[ev * n_sm + s], (unsigned long long)want);
+                    if (got < hi) { b = got; e = hi; break; }
+                    victim++;
+                }
+#else
                 while (victim < n_sm) {
                     const int s = (sm + victim) % n_sm;
                     const int lo = (int)((long long)S * s / n_sm), hi = (int)((long long)S * (s + 1) / n_sm);
@@ -186,9 +207,10 @@ __global__ void __launch_bounds__(kKfThreads, kKfBlocksPerSM) k_construct(const 
                     if (got < hi) { b = got; e = hi; break; }
                     victim++;
                 }
+#endif
             }
             b = __shfl_sync(kFull, b, 0); e = __shfl_sync(kFull, e, 0); victim = __shfl_sync(kFull, victim, 0);
-            if (victim >= n_sm) more = false;
+            if (victim >= n_sm * (TPC_KF_SCHED == 2 ? v.n_events : 1)) more = false;
             const int cand = b + __popc(idle & lanemask_lt());
             if (ph == 0 && cand < e) {
                 i = cand;

@@ -81,7 +81,7 @@ struct Batch {
     Buf<BinDesc> desc;
     Buf<uint32_t> owner;
     Buf<EventSrc> ev_src;
-    Buf<unsigned long long> cnt;
+    Buf<unsigned long long> cnt, kf_cursor;
     // pinned host mirrors
     Buf<EventSrc> h_ev_src;
     Buf<int32_t> h_sec_off, h_ev_off, h_nseeds;
@@ -104,7 +104,7 @@ struct Batch {
         scratch.release(); o_hit.release();
         for (auto& b : o_i) b.release();
         slot.release(); cells.release(); desc.release(); owner.release(); ev_src.release();
-        cnt.release(); h_ev_src.release(); h_sec_off.release(); h_ev_off.release(); h_cnt.release(); h_nseeds.release();
+        cnt.release(); kf_cursor.release(); h_ev_src.release(); h_sec_off.release(); h_ev_off.release(); h_cnt.release(); h_nseeds.release();
         for (auto& e : evt) if (e) { cudaEventDestroy(e); e = nullptr; }
     }
 };
@@ -166,7 +166,7 @@ int reserve_batch(const tpc_tracker* tr, Batch* t, int n_events, int64_t N, int6
     RS(tl_nown, S_cap + 1); RS(tl_keep, S_cap + 1); RS(trk_scan, S_cap + 2); RS(hit_scan, S_cap + 2);
     RS(ev_off_d, 2 * ((size_t)n_events + 1)); RS(h_ev_off, 2 * ((size_t)n_events + 1));
     RS(scratch, (size_t)std::max<int64_t>(nb, S_cap) / kScanTile + 8);
-    RS(cnt, CNT_N); RS(h_cnt, CNT_N); RS(h_nseeds, 1);
+    RS(cnt, CNT_N); RS(h_cnt, CNT_N); RS(kf_cursor, (size_t)n_events * kMaxSM); RS(h_nseeds, 1);
     for (int k = 0; k < 4; k++) RS(o_i[k], S_cap);
     for (int k = 0; k < 7; k++) RS(o_f[k], S_cap);
     RS(o_hit, n);
@@ -208,6 +208,7 @@ int launch_all(const tpc_tracker* tr, Batch* t) {
     int64_t L = 0;
     CK(cudaMemsetAsync(v.bin_count, 0, sizeof(int32_t) * (nb + 1), st));
     CK(cudaMemsetAsync(v.cnt, 0, sizeof(unsigned long long) * CNT_N, st));
+    CK(cudaMemsetAsync(v.kf_cursor, 0, sizeof(unsigned long long) * (size_t)v.n_events * kMaxSM, st));
     if (v.N > 0) CK(cudaMemsetAsync(v.owner, 0, sizeof(uint32_t) * (size_t)v.N, st));
     auto mark = [&](int k) { if (tr->profiling) cudaEventRecord(t->evt[k], st); };
     mark(0);
@@ -300,7 +301,7 @@ int batch_begin(const tpc_tracker* tr, Batch* t, int first_event, int n, const t
     v.o_hit_idx = t->o_hit.p;
     v.o_x = t->o_f[0].p; v.o_y = t->o_f[1].p; v.o_z = t->o_f[2].p; v.o_sinphi = t->o_f[3].p;
     v.o_tgl = t->o_f[4].p; v.o_qpt = t->o_f[5].p; v.o_chi2 = t->o_f[6].p;
-    v.cnt = t->cnt.p;
+    v.cnt = t->cnt.p; v.kf_cursor = t->kf_cursor.p;
     t->n_events = n; t->N = N;
     if (tr->profiling)
         for (auto& e : t->evt)
@@ -310,7 +311,7 @@ int batch_begin(const tpc_tracker* tr, Batch* t, int first_event, int n, const t
     CK(cudaMemsetAsync(v.tl_keep, 0, sizeof(int32_t) * (size_t)(t->S_cap + 1), st));
     CK(cudaMemsetAsync(v.tl_nown, 0, sizeof(int32_t) * (size_t)(t->S_cap + 1), st));
     if ((rc = launch_all(tr, t)) != TPC_OK) return rc;
-    CK(cudaMemcpyAsync(t->h_cnt.p, v.cnt, sizeof(unsigned long long) * CNT_CURSOR, cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(t->h_cnt.p, v.cnt, sizeof(unsigned long long) * CNT_N, cudaMemcpyDeviceToHost, st));
     CK(cudaMemcpyAsync(t->h_ev_off.p, v.ev_off, sizeof(int32_t) * 2 * (n + 1), cudaMemcpyDeviceToHost, st));
     CK(cudaMemcpyAsync(t->h_nseeds.p, v.seed_start + v.n_bins, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
     return TPC_OK;
