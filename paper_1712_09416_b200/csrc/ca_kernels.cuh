@@ -374,8 +374,14 @@ __global__ void __launch_bounds__(kSeedThreads) k_seeds(const View v) {
         const int o = list_o[i];
         int rank = 0;
         for (int j = 0; j < ns; j++) rank += (list_o[j] < o);
-        if (s0 + rank < v.S_cap) { v.seeds[s0 + rank] = list_h[i]; v.seed_bin[s0 + rank] = bin; }
-        else atomicOr((unsigned int*)&v.cnt[CNT_ERR], kErrSeedCapacity);
+        if (s0 + rank < v.S_cap) {
+            const int h0 = list_h[i], h1 = v.clink_up[h0];
+            v.seeds[s0 + rank] = h0; v.seed_bin[s0 + rank] = bin;
+            const float2 a0 = v.shit[h0], a1 = v.shit[h1];
+            float4* rec = reinterpret_cast<float4*>(v.seed_rec) + 2 * (size_t)(s0 + rank);
+            rec[0] = make_float4(a0.x, a0.y, a1.x, a1.y);
+            rec[1] = make_float4(__int_as_float(h0), __int_as_float(h1), 0.f, 0.f);
+        } else atomicOr((unsigned int*)&v.cnt[CNT_ERR], kErrSeedCapacity);
     }
 }
 

@@ -19,7 +19,7 @@ constexpr uint16_t kNoHit = 0xffffu;  // empty entry of a tracklet's row -> hit 
 constexpr unsigned kFull = 0xffffffffu;
 
 // error bits raised by kernels
-constexpr unsigned kErrBadRow = 1u, kErrRowCapacity = 2u, kErrSeedCapacity = 4u;
+constexpr unsigned kErrBadRow = 1u, kErrRowCapacity = 2u, kErrSeedCapacity = 4u, kErrHang = 8u;
 
 // device counters (unsigned long long each)
 constexpr int kMaxSM = 256;
@@ -50,6 +50,9 @@ struct __align__(16) BinDesc {
 };
 
 // Everything a kernel may touch, for one batch.
+struct SeedRec;
+struct UpRec;
+
 struct View {
     int32_t n_events, n_tasks, n_bins, N;
     const EventSrc* ev;      // [n_events]
@@ -74,6 +77,11 @@ struct View {
     int32_t tab_stride;
     int32_t* tl_rows;        // [S_cap] first_row | last_row << 8 | n_hits << 16
     float* tl_par;           // [6][S_cap] y z s t q chi2
+    SeedRec* seed_rec;       // [S_cap] start hit and its up-link: coordinates and sorted indices (K4 -> K5 up sweep)
+    UpRec* tl_up;            // [S_cap] what the up pass hands to the down pass, by tracklet
+    UpRec* dn_rec;           // [S_cap] the same records ordered by (task, top row)
+    int32_t *dn_count, *dn_start, *dn_fill;   // [n_bins+1] tracklets per (task, top row)
+    int32_t kf_K;            // CTAs sharing the start hits of one sector task
     // K6
     uint32_t* owner;         // [N] best key among tracklets holding the hit
     int32_t* tl_nown;        // [S_cap+1] hits owned (0 when the track is dropped)

@@ -145,6 +145,9 @@ constexpr int kKfThreads = 128;
 #ifndef TPC_KF_BLOCKS
 #define TPC_KF_BLOCKS 6
 #endif
+#ifndef TPC_KF_SWEEP
+#define TPC_KF_SWEEP 1
+#endif
 #ifndef TPC_KF_SCHED
 #define TPC_KF_SCHED 1
 #endif

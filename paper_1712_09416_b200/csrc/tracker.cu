@@ -10,6 +10,7 @@
 
 #include "ca_kernels.cuh"
 #include "kf_kernels.cuh"
+#include "kf_sweep.cuh"
 
 namespace {
 
@@ -79,6 +80,9 @@ struct Batch {
         o_i[4], o_hit;
     Buf<uint16_t> slot, cells, tl_tab;
     Buf<BinDesc> desc;
+    Buf<SeedRec> seed_rec;
+    Buf<UpRec> tl_up, dn_rec;
+    Buf<int32_t> dn_count, dn_start, dn_fill;
     Buf<uint32_t> owner;
     Buf<EventSrc> ev_src;
     Buf<unsigned long long> cnt, kf_cursor;
@@ -104,6 +108,7 @@ struct Batch {
         scratch.release(); o_hit.release();
         for (auto& b : o_i) b.release();
         slot.release(); cells.release(); desc.release(); owner.release(); ev_src.release();
+        seed_rec.release(); tl_up.release(); dn_rec.release(); dn_count.release(); dn_start.release(); dn_fill.release();
         cnt.release(); kf_cursor.release(); h_ev_src.release(); h_sec_off.release(); h_ev_off.release(); h_cnt.release(); h_nseeds.release();
         for (auto& e : evt) if (e) { cudaEventDestroy(e); e = nullptr; }
     }
@@ -116,6 +121,8 @@ struct tpc_tracker {
     std::vector<cudaStream_t> own_streams;   // one per slot
     int sm_count = 148;
     int kf_blocks = 148;                     // persistent constructor grid
+    int sw_blocks = 148;                     // resident CTAs of the sweep constructor
+    int sweepers = 0;                        // CTAs per sector task (0 = automatic)
     int group_events = 0;                    // host-input batches: events per group (0 = automatic)
     std::vector<Batch*> slots;               // groups in flight; slots[0] always exists
     // the last call
@@ -163,6 +170,7 @@ int reserve_batch(const tpc_tracker* tr, Batch* t, int n_events, int64_t N, int6
     RS(link_up, n); RS(link_dn, n); RS(clink_up, n); RS(clink_dn, n); RS(owner, n);
     RS(seeds, S_cap); RS(seed_bin, S_cap); RS(tl_rows, S_cap); RS(tl_par, 6 * (size_t)S_cap);
     RS(tl_tab, (size_t)S_cap * tab_stride(tr->c.n_rows));
+    RS(seed_rec, S_cap); RS(tl_up, S_cap); RS(dn_rec, S_cap); RS(dn_count, nb + 1); RS(dn_start, nb + 1); RS(dn_fill, nb + 1);
     RS(tl_nown, S_cap + 1); RS(tl_keep, S_cap + 1); RS(trk_scan, S_cap + 2); RS(hit_scan, S_cap + 2);
     RS(ev_off_d, 2 * ((size_t)n_events + 1)); RS(h_ev_off, 2 * ((size_t)n_events + 1));
     RS(scratch, (size_t)std::max<int64_t>(nb, S_cap) / kScanTile + 8);
@@ -231,8 +239,22 @@ int launch_all(const tpc_tracker* tr, Batch* t) {
     L += scan_exclusive(v.seed_count, v.seed_start, nb, t->scratch.p, st);
     k_seeds<<<nb, kSeedThreads, 0, st>>>(v); L++;
     mark(3);
+#if TPC_KF_SWEEP
+    {
+        CK(cudaMemsetAsync(v.dn_count, 0, sizeof(int32_t) * (nb + 1), st));
+        CK(cudaMemsetAsync(v.dn_fill, 0, sizeof(int32_t) * (nb + 1), st));
+        const int grid = std::max(1, std::min(tr->sw_blocks, v.n_tasks * v.kf_K));
+        k_sweep<true><<<grid, kSwThreads, 0, st>>>(v, c); L++;
+        L += scan_exclusive(v.dn_count, v.dn_start, nb, t->scratch.p, st);
+        k_dn_scatter<<<(int)((t->S_cap + 255) / 256), 256, 0, st>>>(v, nr); L++;
+        k_sweep<false><<<grid, kSwThreads, 0, st>>>(v, c); L++;
+    }
+    mark(4);
+    k_claim<<<tr->sm_count * 16, 128, 0, st>>>(v, c); L++;
+#else
     k_construct<<<tr->kf_blocks, kKfThreads, 0, st>>>(v, c); L++;   // also claims the hits (K6a)
     mark(4);
+#endif
     const int sel_blocks = tr->sm_count * 16;
     k_count_owned<<<sel_blocks, kSelThreads, 0, st>>>(v, c); L++;
     // scans run over the whole seed capacity; entries beyond the seed count are zeroed first
@@ -302,6 +324,9 @@ int batch_begin(const tpc_tracker* tr, Batch* t, int first_event, int n, const t
     v.o_x = t->o_f[0].p; v.o_y = t->o_f[1].p; v.o_z = t->o_f[2].p; v.o_sinphi = t->o_f[3].p;
     v.o_tgl = t->o_f[4].p; v.o_qpt = t->o_f[5].p; v.o_chi2 = t->o_f[6].p;
     v.cnt = t->cnt.p; v.kf_cursor = t->kf_cursor.p;
+    v.seed_rec = t->seed_rec.p; v.tl_up = t->tl_up.p; v.dn_rec = t->dn_rec.p;
+    v.dn_count = t->dn_count.p; v.dn_start = t->dn_start.p; v.dn_fill = t->dn_fill.p;
+    v.kf_K = tr->sweepers > 0 ? tr->sweepers : std::max(1, (tr->sw_blocks + v.n_tasks / 2) / std::max(v.n_tasks, 1));
     t->n_events = n; t->N = N;
     if (tr->profiling)
         for (auto& e : t->evt)
@@ -327,6 +352,7 @@ int batch_finish(const tpc_tracker* tr, Batch* t) {
         const unsigned err = (unsigned)(t->h_cnt.p[CNT_ERR] & 0xffffffffu);
         const int32_t n_seeds = t->h_nseeds.p[0];
         if (err & kErrBadRow) { set_err("a cluster has row outside [0,%d)", nr); return TPC_ERR_ARG; }
+        if (err & kErrHang) { set_err("the constructor lost a shared-memory pipeline signal"); return TPC_ERR_CUDA; }
         if (err & kErrRowCapacity) {
             set_err("more than %d clusters in one (sector,row)", TPC_MAX_ROW_HITS);
             return TPC_ERR_CAPACITY;
@@ -454,6 +480,13 @@ tpc_tracker* tpc_tracker_create_ex(const tpc_geometry* g, float bz, const tpc_pa
             return nullptr;
         }
         t->kf_blocks = t->sm_count * per_sm;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_sweep<true>, kSwThreads, 0) != cudaSuccess || per_sm < 1) {
+            set_err("k_sweep cannot be configured: %s", cudaGetErrorString(cudaGetLastError()));
+            delete t;
+            return nullptr;
+        }
+        t->sw_blocks = t->sm_count * per_sm;
+        if (const char* se = getenv("TPCTRACK_SWEEPERS")) t->sweepers = atoi(se);
     }
     if (const char* ge = getenv("TPCTRACK_GROUP_EVENTS")) t->group_events = atoi(ge);
     Batch* b0 = get_slot(t, 0);
