@@ -19,7 +19,7 @@ constexpr uint16_t kNoHit = 0xffffu;  // empty entry of a tracklet's row -> hit 
 constexpr unsigned kFull = 0xffffffffu;
 
 // error bits raised by kernels
-constexpr unsigned kErrBadRow = 1u, kErrRowCapacity = 2u, kErrSeedCapacity = 4u, kErrHang = 8u;
+constexpr unsigned kErrBadRow = 1u, kErrRowCapacity = 2u, kErrSeedCapacity = 4u, kErrHang = 8u, kErrSelCapacity = 16u;
 
 // device counters (unsigned long long each)
 constexpr int kMaxSM = 256;
@@ -86,6 +86,8 @@ struct View {
     uint32_t* owner;         // [N] best key among tracklets holding the hit
     int32_t* tl_nown;        // [S_cap+1] hits owned (0 when the track is dropped)
     int32_t* tl_keep;        // [S_cap+1] 1 when the track is kept
+    int32_t* tl_cnt;         // [sel_C][S_cap] hits owned in each chunk of the task's pad rows
+    int32_t sel_C;           // chunks per sector task in the selector
     int32_t* trk_scan;       // [S_cap+1]
     int32_t* hit_scan;       // [S_cap+1]
     int32_t* ev_off;         // [2][n_events+1] track / hit offsets of each event

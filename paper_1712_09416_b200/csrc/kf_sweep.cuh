@@ -77,14 +77,32 @@ __device__ __forceinline__ bool mbar_try_wait(unsigned long long* b, uint32_t pa
                  : "=r"(ok) : "r"(smem_u32(b)), "r"(parity) : "memory");
     return ok != 0;
 }
+#ifndef TPC_SW_WAITMODE
+#define TPC_SW_WAITMODE 1
+#endif
+// try_wait that lets the hardware suspend the warp for up to `ns` before it answers
+__device__ __forceinline__ bool mbar_try_wait_hint(unsigned long long* b, uint32_t parity, uint32_t ns) {
+    uint32_t ok;
+    asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n selp.u32 %0, 1, 0, p;\n}"
+                 : "=r"(ok) : "r"(smem_u32(b)), "r"(parity), "r"(ns) : "memory");
+    return ok != 0;
+}
 template <int SLEEP_NS>
 __device__ __forceinline__ bool mbar_wait(unsigned long long* b, uint32_t parity, volatile int32_t* abort) {
     if (mbar_try_wait(b, parity)) return true;
+#if TPC_SW_WAITMODE == 1
+    // suspended waits: a waiting warp issues nothing until the phase completes or the hint runs out
+    for (unsigned n = 0; n < (1u << 17); n++) {
+        if (mbar_try_wait_hint(b, parity, 20000u)) return true;
+        if ((n & 63u) == 63u && *abort) return false;
+    }
+#else
     for (unsigned n = 0; n < kSwSpinMax; n++) {   // back off: a spinning warp takes issue slots from the working ones
         __nanosleep(SLEEP_NS);
         if (mbar_try_wait(b, parity)) return true;
         if ((n & 255u) == 255u && *abort) return false;
     }
+#endif
     *abort = 1;
     return false;
 }
@@ -397,32 +415,6 @@ __global__ void __launch_bounds__(256) k_dn_scatter(const View v, int nr) {
     const int pos = v.dn_start[bin] + atomicAdd(&v.dn_fill[bin], 1);
     float4* dst = reinterpret_cast<float4*>(&v.dn_rec[pos]);
     dst[0] = a; dst[1] = b;
-}
-
-// K6a: every tracklet that enters the selection claims its hits: owner[hit] = max key
-__global__ void __launch_bounds__(128) k_claim(const View v, const __grid_constant__ Const c) {
-    const int S = min(v.seed_start[v.n_bins], v.S_cap);
-    const int nr = c.n_rows;
-    const int lane = lane_id();
-    unsigned claimed = 0;
-    for (int i = (blockIdx.x * 128 + threadIdx.x) >> 5; i < S; i += (gridDim.x * 128) >> 5) {
-        const int pk = v.tl_rows[i];
-        const int nh = pk >> 16;
-        if (nh < c.p.min_tracklet_hits) continue;
-        const int first = pk & 0xff, last = (pk >> 8) & 0xff;
-        const int bin = v.seed_bin[i];
-        const int tb = bin - bin % nr;
-        const uint32_t key = tl_key(v, i, nh, tb);
-        const uint16_t* gt = v.tl_tab + (size_t)i * v.tab_stride;
-        for (int r = first + lane; r <= last; r += 32) {
-            const uint16_t e = gt[r];
-            if (e != kNoHit) { atomicMax(&v.owner[load_desc_n(v, tb + r).x + e], key); claimed++; }
-        }
-    }
-    unsigned long long cl = claimed;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) cl += __shfl_xor_sync(kFull, cl, o);
-    if (lane == 0 && cl) atomicAdd(&v.cnt[CNT_TL_HITS], cl);
 }
 
 }  // namespace tpc

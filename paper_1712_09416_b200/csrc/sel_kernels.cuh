@@ -1,0 +1,168 @@
+// sel_kernels.cuh -- K6 tracklet selector with the hit-ownership words of a sector task held in shared memory.
+//
+// owner[hit] = max key over the tracklets (n_hits >= min_tracklet_hits) holding the hit, key = n_hits << 24 |
+// (2^24 - 1 - id within the task): more hits first, then the lower canonical id.  All tracklets
+// that can hold a hit of sector task T belong to T, so the claims of a task touch only the task's own hits: a CTA
+// takes one task -- or, when the task's hits do not fit the shared memory, one of C runs of consecutive pad rows
+// of it ("chunk", balanced by hits) -- keeps the owner words of those hits in shared memory, and walks the
+// task's tracklets twice: atomicMax of the keys, then the count of the hits each tracklet owns.  The random
+// 4-byte gathers and atomics of the selection never leave the SM; global memory sees the row -> hit tables
+// (read coalesced, one warp per tracklet) and one coalesced copy of the owner words.
+#pragma once
+#include "common.cuh"
+#include "kf_kernels.cuh"
+
+namespace tpc {
+
+constexpr int kSelCtaThreads = 512;
+constexpr int kSelCap = 26000;          // owner words of a chunk (104 KB: two CTAs per SM)
+
+// rows [r_lo, r_hi) of chunk c of task `tb / nr`: the rows whose first hit falls into the c-th of C equal
+// shares of the task's hits.  s_base[r - r_lo] = first hit of row r (batch-global), one entry more than rows.
+__device__ __forceinline__ void sel_chunk(const View& v, int tb, int nr, int c, int C, int& r_lo, int& r_hi) {
+    const int b0 = v.bin_start[tb];
+    const long long nt = v.bin_start[tb + nr] - b0;
+    const int lo_hit = b0 + (int)(nt * c / C), hi_hit = b0 + (int)(nt * (c + 1) / C);
+    // first row whose first hit is >= x (rows are in hit order; empty rows share their successor's first hit)
+    auto first_row_at = [&](int x) {
+        int lo = 0, hi = nr;
+        while (lo < hi) {
+            const int mid = (lo + hi) >> 1;
+            if (v.bin_start[tb + mid] >= x) hi = mid; else lo = mid + 1;
+        }
+        return lo;
+    };
+    r_lo = c == 0 ? 0 : first_row_at(lo_hit);
+    r_hi = c == C - 1 ? nr : first_row_at(hi_hit);
+}
+
+// K6a + K6b: claims and owned-hit counts of one (task, chunk); the owner words go back to global memory for K6c
+__global__ void __launch_bounds__(kSelCtaThreads, 2) k_select_claim(const View v, const __grid_constant__ Const c) {
+    extern __shared__ uint32_t s_owner[];
+    __shared__ int32_t s_base[TPC_MAX_ROWS + 2];
+    __shared__ unsigned long long s_claimed;
+    const int C = v.sel_C, nr = c.n_rows;
+    const int task = blockIdx.x / C, ch = blockIdx.x - task * C, tb = task * nr;
+    const int lane = lane_id(), warp = threadIdx.x >> 5, n_warps = kSelCtaThreads / 32;
+    int r_lo, r_hi;
+    sel_chunk(v, tb, nr, ch, C, r_lo, r_hi);
+    for (int r = r_lo + threadIdx.x; r <= r_hi; r += kSelCtaThreads) s_base[r - r_lo] = v.bin_start[tb + r];
+    if (threadIdx.x == 0) s_claimed = 0ull;
+    __syncthreads();
+    const int h_lo = s_base[0], n_h = s_base[r_hi - r_lo] - h_lo;
+    if (n_h > kSelCap) {   // the host sizes C so that this cannot happen
+        if (threadIdx.x == 0) atomicOr((unsigned int*)&v.cnt[CNT_ERR], kErrSelCapacity);
+        return;
+    }
+    for (int k = threadIdx.x; k < n_h; k += kSelCtaThreads) s_owner[k] = 0u;
+    __syncthreads();
+    const int S = min(v.seed_start[v.n_bins], v.S_cap);
+    const int i0 = min(v.seed_start[tb], S), i1 = min(v.seed_start[tb + nr], S);
+    // The task's row -> hit tables are one contiguous block; a thread takes 8 consecutive rows of one tracklet
+    // (one 16-byte load), so the block streams through with every load independent of the others.
+    const int g_lo = r_lo >> 3, G = ((r_hi - 1) >> 3) - g_lo + 1;
+    const int n_units = (i1 - i0) * G;
+    unsigned claimed = 0;
+    for (int pass = 0; pass < 2; pass++) {
+        for (int u = threadIdx.x; u < n_units; u += kSelCtaThreads) {
+            const int j = u / G, g = g_lo + (u - j * G);
+            const int i = i0 + j;
+            const int pk = v.tl_rows[i];
+            const int nh = pk >> 16;
+            if (nh < c.p.min_tracklet_hits) continue;
+            const int a = max(pk & 0xff, r_lo), b = min((pk >> 8) & 0xff, r_hi - 1);
+            const int r8 = g << 3;
+            if (r8 > b || r8 + 7 < a) continue;
+            const uint32_t key = ((uint32_t)nh << 24) | (uint32_t)(0xffffff - j);
+            const uint4 q = *reinterpret_cast<const uint4*>(v.tl_tab + (size_t)i * v.tab_stride + r8);
+            const uint32_t w[4] = {q.x, q.y, q.z, q.w};
+            int own = 0;
+#pragma unroll
+            for (int k = 0; k < 8; k++) {
+                const uint32_t e = (w[k >> 1] >> ((k & 1) * 16)) & 0xffffu;
+                const int r = r8 + k;
+                if (e != kNoHit && r >= a && r <= b) {
+                    uint32_t* o = &s_owner[s_base[r - r_lo] - h_lo + (int)e];
+                    if (pass == 0) { atomicMax(o, key); claimed++; }
+                    else own += (*o == key);
+                }
+            }
+            if (pass == 1 && own) atomicAdd(&v.tl_cnt[(size_t)ch * v.S_cap + i], own);
+        }
+        __syncthreads();
+    }
+    for (int k = threadIdx.x; k < n_h; k += kSelCtaThreads) v.owner[h_lo + k] = s_owner[k];
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) claimed += __shfl_xor_sync(kFull, claimed, o);
+    if (lane == 0 && claimed) atomicAdd(&s_claimed, (unsigned long long)claimed);
+    __syncthreads();
+    if (threadIdx.x == 0 && s_claimed) atomicAdd(&v.cnt[CNT_TL_HITS], s_claimed);
+}
+
+// a track is kept when its tracklet owns at least min_track_hits hits; entries beyond the start-hit count read 0
+__global__ void __launch_bounds__(256) k_select_keep(const View v, int min_track_hits) {
+    const int i = blockIdx.x * 256 + threadIdx.x;
+    if (i > v.S_cap) return;
+    const int S = min(v.seed_start[v.n_bins], v.S_cap);
+    int own = 0;
+    if (i < S)
+        for (int ch = 0; ch < v.sel_C; ch++) own += v.tl_cnt[(size_t)ch * v.S_cap + i];
+    const int keep = own >= min_track_hits;
+    v.tl_keep[i] = keep;
+    v.tl_nown[i] = keep ? own : 0;
+}
+
+// K6c: output tracks in canonical order; hit lists row-ascending.  The chunks of a task write the pieces of a
+// hit list side by side: a chunk's piece starts behind the hits the lower chunks own.
+__global__ void __launch_bounds__(kSelCtaThreads, 2) k_select_write(const View v, const __grid_constant__ Const c) {
+    extern __shared__ uint32_t s_owner[];
+    __shared__ int32_t s_base[TPC_MAX_ROWS + 2];
+    const int C = v.sel_C, nr = c.n_rows;
+    const int task = blockIdx.x / C, ch = blockIdx.x - task * C, tb = task * nr;
+    const int lane = lane_id(), warp = threadIdx.x >> 5, n_warps = kSelCtaThreads / 32;
+    int r_lo, r_hi;
+    sel_chunk(v, tb, nr, ch, C, r_lo, r_hi);
+    for (int r = r_lo + threadIdx.x; r <= r_hi; r += kSelCtaThreads) s_base[r - r_lo] = v.bin_start[tb + r];
+    __syncthreads();
+    const int h_lo = s_base[0], n_h = s_base[r_hi - r_lo] - h_lo;
+    if (n_h > kSelCap) return;
+    for (int k = threadIdx.x; k < n_h; k += kSelCtaThreads) s_owner[k] = v.owner[h_lo + k];
+    __syncthreads();
+    const int S = min(v.seed_start[v.n_bins], v.S_cap);
+    const int i0 = min(v.seed_start[tb], S), i1 = min(v.seed_start[tb + nr], S);
+    const int e = task / c.n_sectors;
+    for (int i = i0 + warp; i < i1; i += n_warps) {
+        if (!v.tl_keep[i]) continue;
+        const int pk = v.tl_rows[i];
+        const int nh = pk >> 16, first = pk & 0xff, last = (pk >> 8) & 0xff;
+        const uint32_t key = ((uint32_t)nh << 24) | (uint32_t)(0xffffff - (i - i0));
+        int ho = v.hit_scan[i];
+        if (ch == 0 && lane == 0) {
+            const int ti = v.trk_scan[i];
+            const int sc = v.S_cap;
+            v.o_sector[ti] = task - e * c.n_sectors;
+            v.o_first_hit[ti] = ho - v.ev_off[v.n_events + 1 + e];
+            v.o_n_hits[ti] = v.tl_nown[i];
+            v.o_ndf[ti] = 2 * nh - 5;
+            v.o_x[ti] = c.row_x[first];
+            v.o_y[ti] = v.tl_par[i]; v.o_z[ti] = v.tl_par[sc + i]; v.o_sinphi[ti] = v.tl_par[2 * sc + i];
+            v.o_tgl[ti] = v.tl_par[3 * sc + i]; v.o_qpt[ti] = v.tl_par[4 * sc + i]; v.o_chi2[ti] = v.tl_par[5 * sc + i];
+        }
+        for (int k = 0; k < ch; k++) ho += v.tl_cnt[(size_t)k * v.S_cap + i];
+        const int a = max(first, r_lo), b = min(last, r_hi - 1);
+        const uint16_t* gt = v.tl_tab + (size_t)i * v.tab_stride;
+        for (int ra = a; ra <= b; ra += 32) {
+            const int r = ra + lane;
+            int h = -1;
+            if (r <= b) {
+                const uint16_t en = gt[r];
+                if (en != kNoHit) { h = s_base[r - r_lo] + en; if (s_owner[h - h_lo] != key) h = -1; }
+            }
+            const unsigned m = __ballot_sync(kFull, h >= 0);
+            if (h >= 0) v.o_hit_idx[ho + __popc(m & lanemask_lt())] = v.sorig[h];
+            ho += __popc(m);
+        }
+    }
+}
+
+}  // namespace tpc

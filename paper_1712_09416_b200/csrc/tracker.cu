@@ -11,6 +11,7 @@
 #include "ca_kernels.cuh"
 #include "kf_kernels.cuh"
 #include "kf_sweep.cuh"
+#include "sel_kernels.cuh"
 
 namespace {
 
@@ -82,7 +83,8 @@ struct Batch {
     Buf<BinDesc> desc;
     Buf<SeedRec> seed_rec;
     Buf<UpRec> tl_up, dn_rec;
-    Buf<int32_t> dn_count, dn_start, dn_fill;
+    Buf<int32_t> dn_count, dn_start, dn_fill, tl_cnt;
+    int sel_C = 1;                           // selector chunks per sector task
     Buf<uint32_t> owner;
     Buf<EventSrc> ev_src;
     Buf<unsigned long long> cnt, kf_cursor;
@@ -108,7 +110,7 @@ struct Batch {
         scratch.release(); o_hit.release();
         for (auto& b : o_i) b.release();
         slot.release(); cells.release(); desc.release(); owner.release(); ev_src.release();
-        seed_rec.release(); tl_up.release(); dn_rec.release(); dn_count.release(); dn_start.release(); dn_fill.release();
+        seed_rec.release(); tl_up.release(); dn_rec.release(); dn_count.release(); dn_start.release(); dn_fill.release(); tl_cnt.release();
         cnt.release(); kf_cursor.release(); h_ev_src.release(); h_sec_off.release(); h_ev_off.release(); h_cnt.release(); h_nseeds.release();
         for (auto& e : evt) if (e) { cudaEventDestroy(e); e = nullptr; }
     }
@@ -120,7 +122,6 @@ struct tpc_tracker {
     cudaStream_t user_stream = nullptr;      // tpc_tracker_set_stream: used by slot 0 when the call is one group
     std::vector<cudaStream_t> own_streams;   // one per slot
     int sm_count = 148;
-    int kf_blocks = 148;                     // persistent constructor grid
     int sw_blocks = 148;                     // resident CTAs of the sweep constructor
     int sweepers = 0;                        // CTAs per sector task (0 = automatic)
     int group_events = 0;                    // host-input batches: events per group (0 = automatic)
@@ -171,7 +172,7 @@ int reserve_batch(const tpc_tracker* tr, Batch* t, int n_events, int64_t N, int6
     RS(seeds, S_cap); RS(seed_bin, S_cap); RS(tl_rows, S_cap); RS(tl_par, 6 * (size_t)S_cap);
     RS(tl_tab, (size_t)S_cap * tab_stride(tr->c.n_rows));
     RS(seed_rec, S_cap); RS(tl_up, S_cap); RS(dn_rec, S_cap); RS(dn_count, nb + 1); RS(dn_start, nb + 1); RS(dn_fill, nb + 1);
-    RS(tl_nown, S_cap + 1); RS(tl_keep, S_cap + 1); RS(trk_scan, S_cap + 2); RS(hit_scan, S_cap + 2);
+    RS(tl_nown, S_cap + 1); RS(tl_keep, S_cap + 1); RS(tl_cnt, (size_t)t->sel_C * S_cap); RS(trk_scan, S_cap + 2); RS(hit_scan, S_cap + 2);
     RS(ev_off_d, 2 * ((size_t)n_events + 1)); RS(h_ev_off, 2 * ((size_t)n_events + 1));
     RS(scratch, (size_t)std::max<int64_t>(nb, S_cap) / kScanTile + 8);
     RS(cnt, CNT_N); RS(h_cnt, CNT_N); RS(kf_cursor, (size_t)n_events * kMaxSM); RS(h_nseeds, 1);
@@ -217,7 +218,6 @@ int launch_all(const tpc_tracker* tr, Batch* t) {
     CK(cudaMemsetAsync(v.bin_count, 0, sizeof(int32_t) * (nb + 1), st));
     CK(cudaMemsetAsync(v.cnt, 0, sizeof(unsigned long long) * CNT_N, st));
     CK(cudaMemsetAsync(v.kf_cursor, 0, sizeof(unsigned long long) * (size_t)v.n_events * kMaxSM, st));
-    if (v.N > 0) CK(cudaMemsetAsync(v.owner, 0, sizeof(uint32_t) * (size_t)v.N, st));
     auto mark = [&](int k) { if (tr->profiling) cudaEventRecord(t->evt[k], st); };
     mark(0);
     int maxn = 0;
@@ -239,7 +239,6 @@ int launch_all(const tpc_tracker* tr, Batch* t) {
     L += scan_exclusive(v.seed_count, v.seed_start, nb, t->scratch.p, st);
     k_seeds<<<nb, kSeedThreads, 0, st>>>(v); L++;
     mark(3);
-#if TPC_KF_SWEEP
     {
         CK(cudaMemsetAsync(v.dn_count, 0, sizeof(int32_t) * (nb + 1), st));
         CK(cudaMemsetAsync(v.dn_fill, 0, sizeof(int32_t) * (nb + 1), st));
@@ -250,18 +249,15 @@ int launch_all(const tpc_tracker* tr, Batch* t) {
         k_sweep<false><<<grid, kSwThreads, 0, st>>>(v, c); L++;
     }
     mark(4);
-    k_claim<<<tr->sm_count * 16, 128, 0, st>>>(v, c); L++;
-#else
-    k_construct<<<tr->kf_blocks, kKfThreads, 0, st>>>(v, c); L++;   // also claims the hits (K6a)
-    mark(4);
-#endif
-    const int sel_blocks = tr->sm_count * 16;
-    k_count_owned<<<sel_blocks, kSelThreads, 0, st>>>(v, c); L++;
-    // scans run over the whole seed capacity; entries beyond the seed count are zeroed first
+    // K6: claims + owned counts per (task, chunk) in shared memory, keep flags, scans, output
+    const int sel_grid = v.n_tasks * v.sel_C;
+    CK(cudaMemsetAsync(v.tl_cnt, 0, sizeof(int32_t) * (size_t)v.sel_C * t->S_cap, st));
+    k_select_claim<<<sel_grid, kSelCtaThreads, kSelCap * sizeof(uint32_t), st>>>(v, c); L++;
+    k_select_keep<<<(int)((t->S_cap + 1 + 255) / 256), 256, 0, st>>>(v, c.p.min_track_hits); L++;
     L += scan_exclusive(v.tl_keep, v.trk_scan, (int)t->S_cap, t->scratch.p, st);
     L += scan_exclusive(v.tl_nown, v.hit_scan, (int)t->S_cap, t->scratch.p, st);
     k_event_offsets<<<(t->n_events + 1 + 63) / 64, 64, 0, st>>>(v, ns * nr); L++;
-    k_write_tracks<<<sel_blocks, kSelThreads, 0, st>>>(v, c); L++;
+    k_select_write<<<sel_grid, kSelCtaThreads, kSelCap * sizeof(uint32_t), st>>>(v, c); L++;
     mark(5);
     CK(cudaGetLastError());
     t->counters.n_kernel_launches += L;
@@ -282,6 +278,17 @@ int batch_begin(const tpc_tracker* tr, Batch* t, int first_event, int n, const t
     t->in = in; t->first_event = first_event;
     cudaStream_t st = t->stream;
     S_cap = std::max<int64_t>(std::max<int64_t>(t->S_cap, S_cap), default_seed_cap(N));
+    {   // selector: chunks per sector task so that a chunk's owner words fit the shared memory (a chunk holds at
+        // most its share of the task's hits plus one pad row)
+        int64_t max_task = 0;
+        for (int e = 0; e < n; e++)
+            for (int s = 0; s < ns; s++)
+                max_task = std::max<int64_t>(max_task, in[e].sector_offset[s + 1] - in[e].sector_offset[s]);
+        const int64_t room = kSelCap - TPC_MAX_ROW_HITS - 1;
+        const int C = (int)std::max<int64_t>(1, (max_task + room - 1) / room);
+        if (C > t->sel_C) { t->tl_cnt.release(); }
+        t->sel_C = std::max(t->sel_C, C);
+    }
     if ((rc = reserve_batch(tr, t, n, N, S_cap)) != TPC_OK) return rc;
     if (t->host_in) {
         const size_t nn = (size_t)std::max<int64_t>(N, 1);
@@ -317,7 +324,7 @@ int batch_begin(const tpc_tracker* tr, Batch* t, int first_event, int n, const t
     v.seed_count = t->seed_count.p; v.seed_start = t->seed_start.p; v.seeds = t->seeds.p; v.seed_bin = t->seed_bin.p;
     v.S_cap = (int32_t)t->S_cap;
     v.tl_tab = t->tl_tab.p; v.tab_stride = tab_stride(nr); v.tl_rows = t->tl_rows.p; v.tl_par = t->tl_par.p;
-    v.owner = t->owner.p; v.tl_nown = t->tl_nown.p; v.tl_keep = t->tl_keep.p;
+    v.owner = t->owner.p; v.tl_nown = t->tl_nown.p; v.tl_keep = t->tl_keep.p; v.tl_cnt = t->tl_cnt.p; v.sel_C = t->sel_C;
     v.trk_scan = t->trk_scan.p; v.hit_scan = t->hit_scan.p; v.ev_off = t->ev_off_d.p;
     v.o_sector = t->o_i[0].p; v.o_first_hit = t->o_i[1].p; v.o_n_hits = t->o_i[2].p; v.o_ndf = t->o_i[3].p;
     v.o_hit_idx = t->o_hit.p;
@@ -332,9 +339,6 @@ int batch_begin(const tpc_tracker* tr, Batch* t, int first_event, int n, const t
         for (auto& e : t->evt)
             if (!e) CK(cudaEventCreate(&e));
 
-    // keep / nown must read as 0 beyond the seed count
-    CK(cudaMemsetAsync(v.tl_keep, 0, sizeof(int32_t) * (size_t)(t->S_cap + 1), st));
-    CK(cudaMemsetAsync(v.tl_nown, 0, sizeof(int32_t) * (size_t)(t->S_cap + 1), st));
     if ((rc = launch_all(tr, t)) != TPC_OK) return rc;
     CK(cudaMemcpyAsync(t->h_cnt.p, v.cnt, sizeof(unsigned long long) * CNT_N, cudaMemcpyDeviceToHost, st));
     CK(cudaMemcpyAsync(t->h_ev_off.p, v.ev_off, sizeof(int32_t) * 2 * (n + 1), cudaMemcpyDeviceToHost, st));
@@ -353,6 +357,7 @@ int batch_finish(const tpc_tracker* tr, Batch* t) {
         const int32_t n_seeds = t->h_nseeds.p[0];
         if (err & kErrBadRow) { set_err("a cluster has row outside [0,%d)", nr); return TPC_ERR_ARG; }
         if (err & kErrHang) { set_err("the constructor lost a shared-memory pipeline signal"); return TPC_ERR_CUDA; }
+        if (err & kErrSelCapacity) { set_err("selector: a chunk of pad rows exceeds the shared-memory owner table"); return TPC_ERR_CAPACITY; }
         if (err & kErrRowCapacity) {
             set_err("more than %d clusters in one (sector,row)", TPC_MAX_ROW_HITS);
             return TPC_ERR_CAPACITY;
@@ -474,18 +479,18 @@ tpc_tracker* tpc_tracker_create_ex(const tpc_geometry* g, float bz, const tpc_pa
     if (t->sm_count > kMaxSM) { set_err("more than %d SMs", kMaxSM); delete t; return nullptr; }
     {   // persistent constructor grid: as many CTAs as are resident at once
         int per_sm = 0;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_construct, kKfThreads, 0) != cudaSuccess || per_sm < 1) {
-            set_err("k_construct cannot be configured: %s", cudaGetErrorString(cudaGetLastError()));
-            delete t;
-            return nullptr;
-        }
-        t->kf_blocks = t->sm_count * per_sm;
         if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_sweep<true>, kSwThreads, 0) != cudaSuccess || per_sm < 1) {
             set_err("k_sweep cannot be configured: %s", cudaGetErrorString(cudaGetLastError()));
             delete t;
             return nullptr;
         }
         t->sw_blocks = t->sm_count * per_sm;
+        if (cudaFuncSetAttribute(k_select_claim, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kSelCap * sizeof(uint32_t))) != cudaSuccess ||
+            cudaFuncSetAttribute(k_select_write, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kSelCap * sizeof(uint32_t))) != cudaSuccess) {
+            set_err("the selector's shared memory cannot be configured: %s", cudaGetErrorString(cudaGetLastError()));
+            delete t;
+            return nullptr;
+        }
         if (const char* se = getenv("TPCTRACK_SWEEPERS")) t->sweepers = atoi(se);
     }
     if (const char* ge = getenv("TPCTRACK_GROUP_EVENTS")) t->group_events = atoi(ge);
@@ -535,6 +540,7 @@ int tpc_track_events(tpc_tracker* t, int32_t n, const tpc_event_in* in, tpc_even
     // Groups of events.  Device inputs: one group (every launch covers the whole batch).  Host inputs: a few groups
     // on their own streams, so that the copies of one group overlap the kernels of another.
     int per_group = n;
+    if (!host_in && n > 1 && t->group_events > 0) per_group = std::max(std::min<int>(t->group_events, n), (n + 3) / 4);
     if (host_in && n > 1) {
         if (t->group_events > 0) per_group = std::min<int>(t->group_events, n);
         else {
@@ -543,7 +549,7 @@ int tpc_track_events(tpc_tracker* t, int32_t n, const tpc_event_in* in, tpc_even
         }
     }
     const int n_groups = (n + per_group - 1) / per_group;
-    const int n_slots = std::min(n_groups, 3);
+    const int n_slots = host_in ? std::min(n_groups, 3) : n_groups;   // device inputs: outputs stay in the slots
     for (int k = 0; k < n_slots; k++)
         if (!get_slot(t, k)) return TPC_ERR_CUDA;
     for (int k = 0; k < n_slots; k++) {
