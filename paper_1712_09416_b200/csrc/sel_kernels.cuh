@@ -16,6 +16,7 @@ namespace tpc {
 
 constexpr int kSelCtaThreads = 512;
 constexpr int kSelCap = 26000;          // owner words of a chunk (104 KB: two CTAs per SM)
+constexpr int kSelTile = 2048;          // tracklets whose kept members are listed at a time
 
 // rows [r_lo, r_hi) of chunk c of task `tb / nr`: the rows whose first hit falls into the c-th of C equal
 // shares of the task's hits.  s_base[r - r_lo] = first hit of row r (batch-global), one entry more than rows.
@@ -117,6 +118,8 @@ __global__ void __launch_bounds__(256) k_select_keep(const View v, int min_track
 __global__ void __launch_bounds__(kSelCtaThreads, 2) k_select_write(const View v, const __grid_constant__ Const c) {
     extern __shared__ uint32_t s_owner[];
     __shared__ int32_t s_base[TPC_MAX_ROWS + 2];
+    __shared__ int32_t s_list[kSelTile];
+    __shared__ int32_t s_n;
     const int C = v.sel_C, nr = c.n_rows;
     const int task = blockIdx.x / C, ch = blockIdx.x - task * C, tb = task * nr;
     const int lane = lane_id(), warp = threadIdx.x >> 5, n_warps = kSelCtaThreads / 32;
@@ -131,36 +134,76 @@ __global__ void __launch_bounds__(kSelCtaThreads, 2) k_select_write(const View v
     const int S = min(v.seed_start[v.n_bins], v.S_cap);
     const int i0 = min(v.seed_start[tb], S), i1 = min(v.seed_start[tb + nr], S);
     const int e = task / c.n_sectors;
-    for (int i = i0 + warp; i < i1; i += n_warps) {
-        if (!v.tl_keep[i]) continue;
-        const int pk = v.tl_rows[i];
-        const int nh = pk >> 16, first = pk & 0xff, last = (pk >> 8) & 0xff;
-        const uint32_t key = ((uint32_t)nh << 24) | (uint32_t)(0xffffff - (i - i0));
-        int ho = v.hit_scan[i];
-        if (ch == 0 && lane == 0) {
-            const int ti = v.trk_scan[i];
-            const int sc = v.S_cap;
-            v.o_sector[ti] = task - e * c.n_sectors;
-            v.o_first_hit[ti] = ho - v.ev_off[v.n_events + 1 + e];
-            v.o_n_hits[ti] = v.tl_nown[i];
-            v.o_ndf[ti] = 2 * nh - 5;
-            v.o_x[ti] = c.row_x[first];
-            v.o_y[ti] = v.tl_par[i]; v.o_z[ti] = v.tl_par[sc + i]; v.o_sinphi[ti] = v.tl_par[2 * sc + i];
-            v.o_tgl[ti] = v.tl_par[3 * sc + i]; v.o_qpt[ti] = v.tl_par[4 * sc + i]; v.o_chi2[ti] = v.tl_par[5 * sc + i];
+    // A lane takes 8 consecutive rows of one kept tracklet (one 16-byte load); the G row groups of a tracklet sit
+    // in G neighbouring lanes, so a warp works on 32 / G tracklets at once and a segmented scan over the groups'
+    // owned-hit counts gives every group its place in the track's hit list.
+    const int g_lo = r_lo >> 3, G = ((r_hi - 1) >> 3) - g_lo + 1;   // G <= 32
+    const int T = 32 / G;
+    const int tl = lane / G, gi = lane - tl * G, g = g_lo + gi;
+    for (int tile = i0; tile < i1; tile += kSelTile) {
+        __syncthreads();
+        if (threadIdx.x == 0) s_n = 0;
+        __syncthreads();
+        for (int k = threadIdx.x; k < kSelTile; k += kSelCtaThreads) {   // the kept tracklets of the tile
+            const int i = tile + k;
+            const bool keep = i < i1 && v.tl_keep[i] != 0;
+            const unsigned m = __ballot_sync(kFull, keep);
+            int base = 0;
+            if (lane == 0 && m) base = atomicAdd(&s_n, __popc(m));
+            base = __shfl_sync(kFull, base, 0);
+            if (keep) s_list[base + __popc(m & lanemask_lt())] = i;
         }
-        for (int k = 0; k < ch; k++) ho += v.tl_cnt[(size_t)k * v.S_cap + i];
-        const int a = max(first, r_lo), b = min(last, r_hi - 1);
-        const uint16_t* gt = v.tl_tab + (size_t)i * v.tab_stride;
-        for (int ra = a; ra <= b; ra += 32) {
-            const int r = ra + lane;
-            int h = -1;
-            if (r <= b) {
-                const uint16_t en = gt[r];
-                if (en != kNoHit) { h = s_base[r - r_lo] + en; if (s_owner[h - h_lo] != key) h = -1; }
+        __syncthreads();
+        const int n_kept = s_n;
+        for (int t0 = warp * T; t0 < n_kept; t0 += n_warps * T) {
+            const bool on = tl < T && t0 + tl < n_kept;
+            int own = 0, ho = 0, a = 0, b = -1, r8 = g << 3;
+            uint32_t key = 0;
+            uint32_t w[4] = {0u, 0u, 0u, 0u};
+            if (on) {
+                const int i = s_list[t0 + tl];
+                const int pk = v.tl_rows[i];
+                const int nh = pk >> 16, first = pk & 0xff, last = (pk >> 8) & 0xff;
+                key = ((uint32_t)nh << 24) | (uint32_t)(0xffffff - (i - i0));
+                ho = v.hit_scan[i];
+                if (ch == 0 && gi == 0) {
+                    const int ti = v.trk_scan[i];
+                    const int sc = v.S_cap;
+                    v.o_sector[ti] = task - e * c.n_sectors;
+                    v.o_first_hit[ti] = ho - v.ev_off[v.n_events + 1 + e];
+                    v.o_n_hits[ti] = v.tl_nown[i];
+                    v.o_ndf[ti] = 2 * nh - 5;
+                    v.o_x[ti] = c.row_x[first];
+                    v.o_y[ti] = v.tl_par[i]; v.o_z[ti] = v.tl_par[sc + i]; v.o_sinphi[ti] = v.tl_par[2 * sc + i];
+                    v.o_tgl[ti] = v.tl_par[3 * sc + i]; v.o_qpt[ti] = v.tl_par[4 * sc + i]; v.o_chi2[ti] = v.tl_par[5 * sc + i];
+                }
+                for (int k = 0; k < ch; k++) ho += v.tl_cnt[(size_t)k * v.S_cap + i];
+                a = max(first, r_lo); b = min(last, r_hi - 1);
+                if (r8 <= b && r8 + 7 >= a) {
+                    const uint4 q = *reinterpret_cast<const uint4*>(v.tl_tab + (size_t)i * v.tab_stride + r8);
+                    w[0] = q.x; w[1] = q.y; w[2] = q.z; w[3] = q.w;
+                } else b = -1;
             }
-            const unsigned m = __ballot_sync(kFull, h >= 0);
-            if (h >= 0) v.o_hit_idx[ho + __popc(m & lanemask_lt())] = v.sorig[h];
-            ho += __popc(m);
+            int hits[8];
+#pragma unroll
+            for (int k = 0; k < 8; k++) {
+                const uint32_t en = (w[k >> 1] >> ((k & 1) * 16)) & 0xffffu;
+                const int r = r8 + k;
+                int h = -1;
+                if (r >= a && r <= b && en != kNoHit) {
+                    h = s_base[r - r_lo] + (int)en;
+                    if (s_owner[h - h_lo] != key) h = -1;
+                }
+                hits[k] = h;
+                own += h >= 0;
+            }
+            int incl = own;   // scan over the G lanes of the tracklet
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) { const int x = __shfl_up_sync(kFull, incl, o); if (gi >= o) incl += x; }
+            int pos = ho + incl - own;
+#pragma unroll
+            for (int k = 0; k < 8; k++)
+                if (hits[k] >= 0) v.o_hit_idx[pos++] = v.sorig[hits[k]];
         }
     }
 }
