@@ -112,6 +112,7 @@ typedef struct {
     int64_t n_tracks, n_track_hits;
     int64_t n_kernel_launches; /* kernels this library launched during the call */
     int64_t n_retries;       /* internal re-runs after growing a pool */
+    int64_t n_updates;       /* Kalman updates (accepted measurements, both passes) */
 } tpc_counters;
 
 typedef struct tpc_tracker tpc_tracker;

@@ -23,7 +23,7 @@ constexpr unsigned kErrBadRow = 1u, kErrRowCapacity = 2u, kErrSeedCapacity = 4u,
 
 // device counters (unsigned long long each)
 constexpr int kMaxSM = 256;
-enum { CNT_ERR = 0, CNT_LINKS, CNT_ROW_VISITS, CNT_TL_HITS, CNT_TRACKS, CNT_TRACK_HITS, CNT_N };
+enum { CNT_ERR = 0, CNT_LINKS, CNT_ROW_VISITS, CNT_TL_HITS, CNT_TRACKS, CNT_TRACK_HITS, CNT_UPDATES, CNT_N };
 
 // One event's input arrays (device pointers) and its place in the batch-global cluster numbering.
 struct EventSrc {

@@ -247,7 +247,7 @@ __global__ void __launch_bounds__(kSwThreads, kSwBlocksPerSM) k_sweep(const View
     int i = 0, r0 = 0, top = 0, first = 0, nh = 0, cur = -1, rcur = 0, miss = 0;
     uint16_t enext = kNoHit;     // down pass: table entry of the row below, loaded one step ahead
     f.n = 0; f.chi2 = 0.f;
-    unsigned visits = 0;
+    unsigned visits = 0, updates = 0;
     uint32_t it = 0;
 
     for (;;) {
@@ -374,6 +374,7 @@ __global__ void __launch_bounds__(kSwThreads, kSwBlocksPerSM) k_sweep(const View
         __syncwarp();
         if (upd) {
             fit_update(f, ay, az, iwy, c);
+            updates++;
             if (UP) { p0 = ay; p1 = az; p2 = f.s; p3 = f.t; p4 = f.q; top = row; }
             else { p0 = f.y; p1 = f.z; p2 = f.s; p3 = f.t; p4 = f.q; p5 = f.chi2; first = row; nh = f.n; }
         }
@@ -397,10 +398,10 @@ __global__ void __launch_bounds__(kSwThreads, kSwBlocksPerSM) k_sweep(const View
         if (lane == 0) mbar_arrive(&sm.empty[s]);
         it++;
     }
-    unsigned long long vs = visits;
+    unsigned long long vs = visits, us = updates;
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) vs += __shfl_xor_sync(kFull, vs, o);
-    if (lane == 0 && vs) atomicAdd(&v.cnt[CNT_ROW_VISITS], vs);
+    for (int o = 16; o > 0; o >>= 1) { vs += __shfl_xor_sync(kFull, vs, o); us += __shfl_xor_sync(kFull, us, o); }
+    if (lane == 0 && vs) { atomicAdd(&v.cnt[CNT_ROW_VISITS], vs); atomicAdd(&v.cnt[CNT_UPDATES], us); }
 }
 
 // parked tracklets -> lists by (task, top row) for the down sweep

@@ -376,6 +376,7 @@ int batch_finish(const tpc_tracker* tr, Batch* t) {
         t->counters.n_tracklet_hits = (int64_t)t->h_cnt.p[CNT_TL_HITS];
         t->counters.n_tracks = (int64_t)t->h_cnt.p[CNT_TRACKS];
         t->counters.n_track_hits = (int64_t)t->h_cnt.p[CNT_TRACK_HITS];
+        t->counters.n_updates = (int64_t)t->h_cnt.p[CNT_UPDATES];
         return TPC_OK;
     }
 }
@@ -408,7 +409,7 @@ template <class T> int grow_keep(tpc_tracker* t, Buf<T>& b, size_t need, size_t 
 void add_counters(tpc_counters& a, const tpc_counters& b) {
     a.n_events += b.n_events; a.n_clusters += b.n_clusters; a.n_links += b.n_links; a.n_seeds += b.n_seeds;
     a.n_row_visits += b.n_row_visits; a.n_tracklet_hits += b.n_tracklet_hits; a.n_tracks += b.n_tracks;
-    a.n_track_hits += b.n_track_hits; a.n_kernel_launches += b.n_kernel_launches; a.n_retries += b.n_retries;
+    a.n_track_hits += b.n_track_hits; a.n_kernel_launches += b.n_kernel_launches; a.n_retries += b.n_retries; a.n_updates += b.n_updates;
 }
 
 }  // namespace

@@ -54,7 +54,7 @@ class tpc_event_out(C.Structure):
 class tpc_counters(C.Structure):
     _fields_ = [(n, C.c_int64) for n in ("n_events", "n_clusters", "n_links", "n_seeds", "n_row_visits",
                                          "n_tracklet_hits", "n_tracks", "n_track_hits", "n_kernel_launches",
-                                         "n_retries")]
+                                         "n_retries", "n_updates")]
 
     def as_dict(self):
         return {n: int(getattr(self, n)) for n, _ in self._fields_}
