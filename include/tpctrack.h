@@ -135,7 +135,8 @@ int tpc_tracker_set_stream(tpc_tracker* t, void* cuda_stream);
 /* Host-input batches (mem_space 0) are cut into groups of events that run on separate streams, so that the copies
  * of one group overlap the kernels of another ("several events ... processed concurrently on one GPU via streams",
  * BASELINE.json:5).  n = events per group; 0 (default) = automatic (up to four groups of at least ~2 M clusters).
- * Results do not depend on the grouping.  Device-input batches always run as one group. */
+ * Results do not depend on the grouping.  Device-input batches run as one group unless n > 0 is set, in which
+ * case they are cut into at most four groups whose kernels may overlap on the device. */
 int tpc_tracker_set_group_events(tpc_tracker* t, int32_t n);
 
 /* Track one event.  Synchronous: returns when the outputs are complete.  Zero clusters, empty sectors and

@@ -122,15 +122,16 @@ def test_parity_batch_of_events_matches_single_events(trk_mod, gen_mod, oracle_m
     trk.close()
 
 
-@pytest.mark.parametrize("per_group", [1, 2, 0])
-def test_host_batches_run_as_overlapping_groups(trk_mod, gen_mod, oracle_mod, per_group):
+@pytest.mark.parametrize("per_group,device", [(1, False), (2, False), (0, False), (2, True)])
+def test_host_batches_run_as_overlapping_groups(trk_mod, gen_mod, oracle_mod, per_group, device):
     """Host-input batches are cut into groups of events on separate streams (copies of one group overlap the
-    kernels of another); 7 events in groups of 1 also cycle the three slots.  Results must not depend on it."""
+    kernels of another); 7 events in groups of 1 also cycle the three slots; device-input batches are grouped on
+    request.  Results must not depend on it."""
     evs = [gen_mod.generate("pp", e) for e in range(4)] + [gen_mod.generate("semicentral", 0)] + \
           [gen_mod.generate("pp", e) for e in range(4, 6)]
     trk = make_tracker(trk_mod, gen_mod, evs[0])
     trk.tpc_tracker_set_group_events(per_group)
-    outs = trk.tpc_track_events([ev_dict(ev, False) for ev in evs])
+    outs = trk.tpc_track_events([ev_dict(ev, device) for ev in evs])
     res = [trk.to_numpy(o) for o in outs]
     c = trk.tpc_get_counters()
     assert c["n_events"] == len(evs) and c["n_clusters"] == sum(ev.n_clusters for ev in evs)
