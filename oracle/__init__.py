@@ -39,6 +39,7 @@ class Params(C.Structure):
         ("win_nsigma", C.c_float), ("win_min", C.c_float), ("win_max", C.c_float),
         ("max_gap", C.c_int32), ("edge_margin", C.c_float),
         ("min_tracklet_hits", C.c_int32), ("min_track_hits", C.c_int32),
+        ("refit", C.c_int32),
     ]
 
     def as_dict(self):

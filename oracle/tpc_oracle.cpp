@@ -23,7 +23,9 @@
  * mirror symmetry; O3/O4 invariants; transport against the closed-form helix and its Jacobian against central
  * differences; fit against the textbook straight-line least squares (Bz -> 0), against noise-free helices,
  * pulls / chi2 per ndf / Gluckstern curvature resolution with noise; O6 ownership invariants and a brute-force
- * owner; end-to-end efficiency on generated events.
+ * owner; end-to-end efficiency on generated events; O8 (refit of the selected tracks) against the
+ * generated helix, the least-squares line, a test-side composition of the pinned transport / update steps,
+ * chi2 per ndf and Gluckstern (tests/test_oracle_refit.py).
  * PARITY UNPINNED: the exact link / track values on the BASELINE.json configs have no outside reference
  * (the paper prints none); they are pinned only through the properties above.
  */
@@ -51,6 +53,7 @@ typedef struct {
     int32_t max_gap;            /* rows without a hit before a pass ends */
     float edge_margin;          /* cm beyond the wedge before a pass ends */
     int32_t min_tracklet_hits, min_track_hits;
+    int32_t refit;              /* O8: 1 = track parameters from a refit over the final hit list */
 } oracle_params;
 
 typedef struct {
@@ -377,6 +380,57 @@ template <class R> struct Sector {
         T.chi2 = (double)snap.chi2;
         T.margin = mg.m;
     }
+
+    /* ---- O8 refit of a selected track over its final hit list ----
+       hits: the track's hits, row-ascending (at most one per row).  No search and no gate: every hit of the list
+       is a measurement.  Up pass from the lowest hit (direction from the first two hits, q = 0, prior covariance),
+       transporting to every consecutive row; down pass = fresh fit at the top hit reached with (s, t, q) of the
+       up pass.  A failed transport ends a pass.  Result = state after the last update of the down pass
+       (x_ref = row of that hit), chi2 and hit count of the down pass.  Lists of fewer than 2 hits are left alone. */
+    bool refit(const std::vector<int32_t>& hits, double par[5], double& chi2, int& n_fit, int& ref_row) const {
+        const int m = (int)hits.size();
+        if (m < 2) return false;
+        Margin mg;
+        Fit<R> f, snap;
+        const int32_t h0 = hits[0], h1 = hits[1];
+        const int r0 = grow[h0];
+        {
+            const R dx = X[grow[h1]] - X[r0];
+            const R dy = R(gy[h1]) - R(gy[h0]), dz = R(gz[h1]) - R(gz[h0]);
+            const R dl = std::sqrt(dx * dx + dy * dy);
+            f.y = R(gy[h0]); f.z = R(gz[h0]); f.s = dy / dl; f.t = dz / dl; f.q = R(0);
+            prior(f); f.n = 1;
+        }
+        snap = f;
+        int k_top = 0;                       /* position in the list of the last hit the up pass used */
+        {
+            R xc = X[r0];
+            int k = 1;
+            for (int row = r0 + 1; row <= grow[hits[m - 1]]; row++) {
+                if (!transport(f, xc, X[row], mg)) break;
+                xc = X[row];
+                if (row == grow[hits[k]]) { update(f, hits[k]); snap = f; k_top = k; k++; }
+            }
+        }
+        {
+            const int32_t ht = hits[k_top];
+            f.y = R(gy[ht]); f.z = R(gz[ht]); f.s = snap.s; f.t = snap.t; f.q = snap.q;
+            prior(f); f.n = 1;
+            snap = f;
+            ref_row = grow[ht];
+            R xc = X[grow[ht]];
+            int k = k_top - 1;
+            for (int row = grow[ht] - 1; row >= r0; row--) {
+                if (!transport(f, xc, X[row], mg)) break;
+                xc = X[row];
+                if (row == grow[hits[k]]) { update(f, hits[k]); snap = f; ref_row = row; k--; }
+            }
+        }
+        par[0] = (double)snap.y; par[1] = (double)snap.z; par[2] = (double)snap.s; par[3] = (double)snap.t;
+        par[4] = (double)snap.q;
+        chi2 = (double)snap.chi2; n_fit = snap.n;
+        return true;
+    }
 };
 
 template <class R>
@@ -391,7 +445,8 @@ Result* run(const oracle_geometry& G, const oracle_params& P, int32_t n, const i
     std::vector<std::vector<int32_t>> seeds(ns);
     std::vector<std::vector<Tracklet>> tls(ns);
     /* per-sector output tracks */
-    struct Out { std::vector<int32_t> seed, nh, first_row; std::vector<std::vector<int32_t>> hits; };
+    struct Refit { bool ok = false; double par[5] = {0, 0, 0, 0, 0}, chi2 = 0; int n_fit = 0, ref_row = 0; };
+    struct Out { std::vector<int32_t> seed, nh, first_row; std::vector<std::vector<int32_t>> hits; std::vector<Refit> refit; };
     std::vector<Out> outs(ns);
 #ifdef _OPENMP
     if (n_threads > 0) omp_set_num_threads(n_threads);
@@ -435,6 +490,9 @@ Result* run(const oracle_geometry& G, const oracle_params& P, int32_t n, const i
             outs[s].seed.push_back((int32_t)i);
             outs[s].nh.push_back((int32_t)hits.size());
             outs[s].first_row.push_back(T.first_row);
+            Refit rf;   /* ---- O8 ---- */
+            if (P.refit) rf.ok = S.refit(hits, rf.par, rf.chi2, rf.n_fit, rf.ref_row);
+            outs[s].refit.push_back(rf);
             outs[s].hits.push_back(std::move(hits));
         }
     }
@@ -459,6 +517,14 @@ Result* run(const oracle_geometry& G, const oracle_params& P, int32_t n, const i
             res->trk_y.push_back(T.par[0]); res->trk_z.push_back(T.par[1]); res->trk_sinphi.push_back(T.par[2]);
             res->trk_tgl.push_back(T.par[3]); res->trk_qpt.push_back(T.par[4]);
             res->trk_chi2.push_back(T.chi2); res->trk_margin.push_back(T.margin);
+            const Refit& rf = outs[s].refit[k];
+            if (rf.ok) {   /* O8: parameters, chi2, ndf and reference row of the refit replace the tracklet's */
+                res->trk_ndf.back() = 2 * rf.n_fit - 5;
+                res->trk_first_row.back() = rf.ref_row;
+                res->trk_x.back() = (double)G.row_x[rf.ref_row];
+                res->trk_y.back() = rf.par[0]; res->trk_z.back() = rf.par[1]; res->trk_sinphi.back() = rf.par[2];
+                res->trk_tgl.back() = rf.par[3]; res->trk_qpt.back() = rf.par[4]; res->trk_chi2.back() = rf.chi2;
+            }
             for (int32_t h : outs[s].hits[k]) res->hit_idx.push_back(h);
         }
     }
@@ -483,6 +549,7 @@ void oracle_default_params(oracle_params* p) {
     p->win_nsigma = 4.0f; p->win_min = 0.3f; p->win_max = 3.0f;
     p->max_gap = 5; p->edge_margin = 1.0f;
     p->min_tracklet_hits = 10; p->min_track_hits = 10;
+    p->refit = 0;
 }
 
 /* precision: 0 = double, 1 = strict float32.  stop_after: 0 = everything, 2 = after O2, 4 = after O4,
