@@ -100,6 +100,7 @@ def stage_bytes(c):
         "K3K4_clean_seeds": 24 * N + 4 * S,
         "K5_construct": 12 * V + 4 * A + 40 * S,
         "K6_select": 16 * A + 4 * H + 44 * T,
+        "K7_refit": (12 * H + 44 * T) if c.get("n_refit_visits", 0) else 0,
     }
 
 
@@ -226,7 +227,7 @@ def main():
         torch.cuda.synchronize()
 
     def timed(inputs, steps, collect_stages):
-        stages = np.zeros(5)
+        stages = np.zeros(6)
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         barrier()
         e0.record(stream)

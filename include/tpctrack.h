@@ -62,6 +62,11 @@ typedef struct {
     float edge_margin;          /* cm beyond the wedge edge before a pass ends */
     int32_t min_tracklet_hits;  /* tracklets with fewer hits do not take part in the selection */
     int32_t min_track_hits;     /* tracks keeping fewer owned hits are dropped */
+    int32_t refit;              /* 0 (default): track parameters are the tracklet's (no refit).  1: every output
+                                 * track is refitted over its final hit list: up
+                                 * pass from its lowest hit, fresh down pass from the top hit reached, no search, no
+                                 * gate; trk_x/y/z/sinphi/tgl/qpt/chi2/ndf are then the refit's (x = row of the
+                                 * lowest hit the down pass reached, ndf = 2 * hits in the refit - 5) */
 } tpc_params;
 
 /* One event's clusters: SoA, grouped by sector, ANY order inside a sector.
@@ -113,6 +118,7 @@ typedef struct {
     int64_t n_kernel_launches; /* kernels this library launched during the call */
     int64_t n_retries;       /* internal re-runs after growing a pool */
     int64_t n_updates;       /* Kalman updates (accepted measurements, both passes) */
+    int64_t n_refit_visits;  /* row visits of the refit (0 when tpc_params.refit is 0) */
 } tpc_counters;
 
 typedef struct tpc_tracker tpc_tracker;
@@ -156,8 +162,9 @@ int tpc_get_counters(const tpc_tracker* t, tpc_counters* c);
 
 /* Per-stage device times of the last call, measured with CUDA events on the tracker's stream (off by default:
  * the events cost a few microseconds).  Stages: 0 = K1 bucket + grid sort, 1 = K2 neighbour finder,
- * 2 = K3 cleaner + K4 start hits, 3 = K5 tracklet constructor (one kernel), 4 = K6 selector + output. */
-#define TPC_N_STAGES 5
+ * 2 = K3 cleaner + K4 start hits, 3 = K5 tracklet constructor (up sweep, bucket pass, down sweep),
+ * 4 = K6 selector + output, 5 = refit of the output tracks (0 when tpc_params.refit is 0). */
+#define TPC_N_STAGES 6
 int tpc_tracker_set_profiling(tpc_tracker* t, int32_t on);
 int tpc_get_stage_ms(const tpc_tracker* t, float* ms /* [TPC_N_STAGES] */);
 

@@ -23,7 +23,7 @@ constexpr unsigned kErrBadRow = 1u, kErrRowCapacity = 2u, kErrSeedCapacity = 4u,
 
 // device counters (unsigned long long each)
 constexpr int kMaxSM = 256;
-enum { CNT_ERR = 0, CNT_LINKS, CNT_ROW_VISITS, CNT_TL_HITS, CNT_TRACKS, CNT_TRACK_HITS, CNT_UPDATES, CNT_N };
+enum { CNT_ERR = 0, CNT_LINKS, CNT_ROW_VISITS, CNT_TL_HITS, CNT_TRACKS, CNT_TRACK_HITS, CNT_UPDATES, CNT_REFIT_VISITS, CNT_N };
 
 // One event's input arrays (device pointers) and its place in the batch-global cluster numbering.
 struct EventSrc {
@@ -94,6 +94,9 @@ struct View {
     // outputs
     int32_t *o_sector, *o_first_hit, *o_n_hits, *o_ndf, *o_hit_idx;
     float *o_x, *o_y, *o_z, *o_sinphi, *o_tgl, *o_qpt, *o_chi2;
+    // refit of the output tracks (tpc_params.refit): the tracks' hits as (y,z) and pad row, in hit-list order
+    float2* o_hit_yz; uint8_t* o_hit_row;   // [N]
+    int32_t* trk_hit0;       // [S_cap] first entry of a track's hit list in the batch's hit arrays
     unsigned long long* cnt; // [CNT_N]
     unsigned long long* kf_cursor;  // [n_events * kMaxSM] K5: start hits handed out per (event, SM) share
 };

@@ -170,6 +170,7 @@ __global__ void __launch_bounds__(kSelCtaThreads, 2) k_select_write(const View v
                     const int ti = v.trk_scan[i];
                     const int sc = v.S_cap;
                     v.o_sector[ti] = task - e * c.n_sectors;
+                    if (c.p.refit) v.trk_hit0[ti] = ho;
                     v.o_first_hit[ti] = ho - v.ev_off[v.n_events + 1 + e];
                     v.o_n_hits[ti] = v.tl_nown[i];
                     v.o_ndf[ti] = 2 * nh - 5;
@@ -203,7 +204,11 @@ __global__ void __launch_bounds__(kSelCtaThreads, 2) k_select_write(const View v
             int pos = ho + incl - own;
 #pragma unroll
             for (int k = 0; k < 8; k++)
-                if (hits[k] >= 0) v.o_hit_idx[pos++] = v.sorig[hits[k]];
+                if (hits[k] >= 0) {
+                    v.o_hit_idx[pos] = v.sorig[hits[k]];
+                    if (c.p.refit) { v.o_hit_yz[pos] = v.shit[hits[k]]; v.o_hit_row[pos] = (uint8_t)(r8 + k); }   // for O8
+                    pos++;
+                }
         }
     }
 }

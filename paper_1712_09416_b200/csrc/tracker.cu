@@ -12,6 +12,7 @@
 #include "kf_kernels.cuh"
 #include "kf_sweep.cuh"
 #include "sel_kernels.cuh"
+#include "kf_refit.cuh"
 
 namespace {
 
@@ -80,6 +81,9 @@ struct Batch {
         seed_start, seeds, seed_bin, tl_rows, tl_nown, tl_keep, trk_scan, hit_scan, ev_off_d, scratch,
         o_i[4], o_hit;
     Buf<uint16_t> slot, cells, tl_tab;
+    Buf<float2> o_hit_yz;
+    Buf<uint8_t> o_hit_row;
+    Buf<int32_t> trk_hit0;
     Buf<BinDesc> desc;
     Buf<SeedRec> seed_rec;
     Buf<UpRec> tl_up, dn_rec;
@@ -110,7 +114,7 @@ struct Batch {
         scratch.release(); o_hit.release();
         for (auto& b : o_i) b.release();
         slot.release(); cells.release(); desc.release(); owner.release(); ev_src.release();
-        seed_rec.release(); tl_up.release(); dn_rec.release(); dn_count.release(); dn_start.release(); dn_fill.release(); tl_cnt.release();
+        seed_rec.release(); tl_up.release(); dn_rec.release(); dn_count.release(); dn_start.release(); dn_fill.release(); tl_cnt.release(); o_hit_yz.release(); o_hit_row.release(); trk_hit0.release();
         cnt.release(); kf_cursor.release(); h_ev_src.release(); h_sec_off.release(); h_ev_off.release(); h_cnt.release(); h_nseeds.release();
         for (auto& e : evt) if (e) { cudaEventDestroy(e); e = nullptr; }
     }
@@ -123,6 +127,7 @@ struct tpc_tracker {
     std::vector<cudaStream_t> own_streams;   // one per slot
     int sm_count = 148;
     int sw_blocks = 148;                     // resident CTAs of the sweep constructor
+    int rf_blocks = 148;                     // resident CTAs of the refit
     int sweepers = 0;                        // CTAs per sector task (0 = automatic)
     int group_events = 0;                    // host-input batches: events per group (0 = automatic)
     std::vector<Batch*> slots;               // groups in flight; slots[0] always exists
@@ -179,6 +184,7 @@ int reserve_batch(const tpc_tracker* tr, Batch* t, int n_events, int64_t N, int6
     for (int k = 0; k < 4; k++) RS(o_i[k], S_cap);
     for (int k = 0; k < 7; k++) RS(o_f[k], S_cap);
     RS(o_hit, n);
+    if (tr->c.p.refit) { RS(o_hit_yz, n); RS(o_hit_row, n); RS(trk_hit0, S_cap); }
 #undef RS
     t->S_cap = S_cap;
     return TPC_OK;
@@ -259,6 +265,8 @@ int launch_all(const tpc_tracker* tr, Batch* t) {
     k_event_offsets<<<(t->n_events + 1 + 63) / 64, 64, 0, st>>>(v, ns * nr); L++;
     k_select_write<<<sel_grid, kSelCtaThreads, kSelCap * sizeof(uint32_t), st>>>(v, c); L++;
     mark(5);
+    if (c.p.refit) { k_refit<<<tr->rf_blocks, kRfThreads, 0, st>>>(v, c); L++; }
+    mark(6);
     CK(cudaGetLastError());
     t->counters.n_kernel_launches += L;
     return TPC_OK;
@@ -331,6 +339,7 @@ int batch_begin(const tpc_tracker* tr, Batch* t, int first_event, int n, const t
     v.o_x = t->o_f[0].p; v.o_y = t->o_f[1].p; v.o_z = t->o_f[2].p; v.o_sinphi = t->o_f[3].p;
     v.o_tgl = t->o_f[4].p; v.o_qpt = t->o_f[5].p; v.o_chi2 = t->o_f[6].p;
     v.cnt = t->cnt.p; v.kf_cursor = t->kf_cursor.p;
+    v.o_hit_yz = t->o_hit_yz.p; v.o_hit_row = t->o_hit_row.p; v.trk_hit0 = t->trk_hit0.p;
     v.seed_rec = t->seed_rec.p; v.tl_up = t->tl_up.p; v.dn_rec = t->dn_rec.p;
     v.dn_count = t->dn_count.p; v.dn_start = t->dn_start.p; v.dn_fill = t->dn_fill.p;
     v.kf_K = tr->sweepers > 0 ? tr->sweepers : std::max(1, (tr->sw_blocks + v.n_tasks / 2) / std::max(v.n_tasks, 1));
@@ -377,6 +386,7 @@ int batch_finish(const tpc_tracker* tr, Batch* t) {
         t->counters.n_tracks = (int64_t)t->h_cnt.p[CNT_TRACKS];
         t->counters.n_track_hits = (int64_t)t->h_cnt.p[CNT_TRACK_HITS];
         t->counters.n_updates = (int64_t)t->h_cnt.p[CNT_UPDATES];
+        t->counters.n_refit_visits = (int64_t)t->h_cnt.p[CNT_REFIT_VISITS];
         return TPC_OK;
     }
 }
@@ -409,7 +419,7 @@ template <class T> int grow_keep(tpc_tracker* t, Buf<T>& b, size_t need, size_t 
 void add_counters(tpc_counters& a, const tpc_counters& b) {
     a.n_events += b.n_events; a.n_clusters += b.n_clusters; a.n_links += b.n_links; a.n_seeds += b.n_seeds;
     a.n_row_visits += b.n_row_visits; a.n_tracklet_hits += b.n_tracklet_hits; a.n_tracks += b.n_tracks;
-    a.n_track_hits += b.n_track_hits; a.n_kernel_launches += b.n_kernel_launches; a.n_retries += b.n_retries; a.n_updates += b.n_updates;
+    a.n_track_hits += b.n_track_hits; a.n_kernel_launches += b.n_kernel_launches; a.n_retries += b.n_retries; a.n_updates += b.n_updates; a.n_refit_visits += b.n_refit_visits;
 }
 
 }  // namespace
@@ -426,6 +436,7 @@ void tpc_default_params(tpc_params* p) {
     p->win_nsigma = 4.0f; p->win_min = 0.3f; p->win_max = 3.0f;
     p->max_gap = 5; p->edge_margin = 1.0f;
     p->min_tracklet_hits = 10; p->min_track_hits = 10;
+    p->refit = 0;
 }
 
 const char* tpc_status_string(int s) {
@@ -456,8 +467,8 @@ tpc_tracker* tpc_tracker_create_ex(const tpc_geometry* g, float bz, const tpc_pa
     }
     tpc_params p;
     if (params) p = *params; else tpc_default_params(&p);
-    if (p.link_step < 1 || p.link_step > 2 || p.min_tracklet_hits < 1 || p.min_track_hits < 1 || p.max_gap < 0) {
-        set_err("params: link_step must be 1 or 2, minimum hit counts >= 1, max_gap >= 0");
+    if (p.link_step < 1 || p.link_step > 2 || p.min_tracklet_hits < 1 || p.min_track_hits < 1 || p.max_gap < 0 || p.refit < 0 || p.refit > 1) {
+        set_err("params: link_step must be 1 or 2, minimum hit counts >= 1, max_gap >= 0, refit 0 or 1");
         return nullptr;
     }
     int dev = 0, ndev = 0;
@@ -486,6 +497,8 @@ tpc_tracker* tpc_tracker_create_ex(const tpc_geometry* g, float bz, const tpc_pa
             return nullptr;
         }
         t->sw_blocks = t->sm_count * per_sm;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_refit, kRfThreads, 0) != cudaSuccess || per_sm < 1) per_sm = 1;
+        t->rf_blocks = t->sm_count * per_sm;
         if (cudaFuncSetAttribute(k_select_claim, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kSelCap * sizeof(uint32_t))) != cudaSuccess ||
             cudaFuncSetAttribute(k_select_write, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kSelCap * sizeof(uint32_t))) != cudaSuccess) {
             set_err("the selector's shared memory cannot be configured: %s", cudaGetErrorString(cudaGetLastError()));
@@ -581,7 +594,8 @@ int tpc_track_events(tpc_tracker* t, int32_t n, const tpc_event_in* in, tpc_even
         const int32_t* toff = b->h_ev_off.p;
         const int32_t* hoff = b->h_ev_off.p + (ne + 1);
         for (int e = 0; e < ne; e++) {
-            trk_off[e0 + e] = T_cum + toff[e]; hit_off[e0 + e] = H_cum + hoff[e];
+            // host inputs: the groups' outputs are concatenated; device inputs: each group keeps its own arrays
+            trk_off[e0 + e] = (host_in ? T_cum : 0) + toff[e]; hit_off[e0 + e] = (host_in ? H_cum : 0) + hoff[e];
             out[e0 + e].n_tracks = toff[e + 1] - toff[e];
             out[e0 + e].n_track_hits = hoff[e + 1] - hoff[e];
         }

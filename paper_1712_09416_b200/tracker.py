@@ -16,6 +16,7 @@ import os
 LIB_PATH = Path(os.environ.get("TPCTRACK_LIB") or Path(__file__).resolve().parent / "csrc" / "libtpctrack.so")
 
 TPC_OK, TPC_ERR_ARG, TPC_ERR_GEOMETRY, TPC_ERR_CAPACITY, TPC_ERR_CUDA = 0, -1, -2, -3, -4
+N_STAGES = 6   # TPC_N_STAGES
 DBG = {"link_up": 0, "link_dn": 1, "clink_up": 2, "clink_dn": 3, "start_hit": 4, "tl_rows": 5, "tl_par": 6,
        "tl_table": 7, "sorted": 8}
 
@@ -31,7 +32,7 @@ class tpc_params(C.Structure):
                 ("nf_dmax", C.c_float), ("sin_max", C.c_float), ("var_s", C.c_float), ("var_t", C.c_float),
                 ("var_q", C.c_float), ("chi2_link", C.c_float), ("chi2_ext", C.c_float), ("win_nsigma", C.c_float),
                 ("win_min", C.c_float), ("win_max", C.c_float), ("max_gap", C.c_int32), ("edge_margin", C.c_float),
-                ("min_tracklet_hits", C.c_int32), ("min_track_hits", C.c_int32)]
+                ("min_tracklet_hits", C.c_int32), ("min_track_hits", C.c_int32), ("refit", C.c_int32)]
 
     def as_dict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}
@@ -54,7 +55,7 @@ class tpc_event_out(C.Structure):
 class tpc_counters(C.Structure):
     _fields_ = [(n, C.c_int64) for n in ("n_events", "n_clusters", "n_links", "n_seeds", "n_row_visits",
                                          "n_tracklet_hits", "n_tracks", "n_track_hits", "n_kernel_launches",
-                                         "n_retries", "n_updates")]
+                                         "n_retries", "n_updates", "n_refit_visits")]
 
     def as_dict(self):
         return {n: int(getattr(self, n)) for n, _ in self._fields_}
@@ -209,7 +210,7 @@ class Tracker:
         _check(lib.tpc_tracker_set_profiling(self._h, int(on)))
 
     def tpc_get_stage_ms(self):
-        ms = (C.c_float * 5)()
+        ms = (C.c_float * N_STAGES)()
         _check(lib.tpc_get_stage_ms(self._h, ms))
         return [float(v) for v in ms]
 

@@ -250,3 +250,46 @@ def test_seed_pool_grows(trk_mod, gen_mod, oracle_mod):
     assert np.array_equal(trk.tpc_debug_get("start_hit"), ref.start_hit)
     assert np.array_equal(trk.tpc_debug_get("tl_table"), ref.tl_table)
     trk.close()
+
+
+@pytest.mark.parametrize("name,step", [("single_sector", 1), ("semicentral", 1), ("semicentral", 2), ("central", 1)])
+def test_refit_parity(trk_mod, gen_mod, oracle_mod, name, step):
+    """O8 (tpc_params.refit = 1): refit of every output track over its final hit list; hit lists unchanged,
+    parameters / chi2 / ndf / reference row those of the oracle's refit (strict float32)."""
+    ev = gen_mod.generate(name)
+    p = oracle_mod.default_params()
+    p.refit = 1; p.link_step = step
+    ref = oracle_mod.track_event(make_geometry(oracle_mod, gen_mod, ev), ev.sector_offset, ev.y, ev.z, ev.row,
+                                 params=p, precision="float")
+    trk = make_tracker(trk_mod, gen_mod, ev, params=copy_params(p, trk_mod))
+    out = trk.tpc_track_event(ev_dict(ev, True))
+    flips, res = compare_event(trk, out, ev, ref, check_stages=False)
+    assert flips == 0
+    c = trk.tpc_get_counters()
+    assert c["n_refit_visits"] > 2 * (c["n_track_hits"] - c["n_tracks"]) * 0.9
+    # the refit makes hit list and fit consistent: ndf counts the hits of the list (no transport failure here)
+    assert np.mean(res["trk_ndf"] == 2 * res["trk_n_hits"] - 5) > 0.99
+    base = make_tracker(trk_mod, gen_mod, ev, params=copy_params(oracle_mod.default_params(), trk_mod)) if step == 1 else None
+    if base is not None:   # refit off: same hit lists, different parameters
+        r0 = base.to_numpy(base.tpc_track_event(ev_dict(ev, True)))
+        assert np.array_equal(r0["hit_idx"], res["hit_idx"]) and not np.array_equal(r0["trk_qpt"], res["trk_qpt"])
+        assert base.tpc_get_counters()["n_refit_visits"] == 0
+        base.close()
+    trk.close()
+
+
+def test_refit_in_a_batch_matches_single_events(trk_mod, gen_mod, oracle_mod):
+    evs = [gen_mod.generate("pp", 0), gen_mod.generate("semicentral", 0), gen_mod.generate("pp", 1)]
+    p = oracle_mod.default_params()
+    p.refit = 1
+    trk = make_tracker(trk_mod, gen_mod, evs[0], params=copy_params(p, trk_mod))
+    outs = trk.tpc_track_events([ev_dict(ev, False) for ev in evs])
+    for ev, o in zip(evs, outs):
+        ref = oracle_mod.track_event(make_geometry(oracle_mod, gen_mod, ev), ev.sector_offset, ev.y, ev.z, ev.row,
+                                     params=p, precision="float")
+        res = trk.to_numpy(o)
+        assert np.array_equal(res["hit_idx"], ref.hit_idx) and np.array_equal(res["trk_ndf"], ref.trk_ndf)
+        for k in ("trk_x", "trk_y", "trk_z", "trk_sinphi", "trk_tgl", "trk_qpt", "trk_chi2"):
+            err = np.abs(res[k] - ref[k]) / np.maximum(1.0, np.abs(ref[k]))
+            assert err.max(initial=0.0) <= TOL, (k, err.max())
+    trk.close()
