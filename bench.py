@@ -181,6 +181,7 @@ def main():
     ap.add_argument("--workload", default="central", choices=["central", "semicentral", "pp"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--refit", action="store_true", help="also refit the output tracks (O8, SURVEY.md 8(f).1; not part of the headline path)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
 
@@ -204,8 +205,12 @@ def main():
     evs = make_events(args.workload, args.events)
     n_total = sum(ev.n_clusters for ev in evs)
     rx = gen.row_x().astype(np.float32)
+    params = None
+    if args.refit:
+        params = tracker.tpc_default_params()
+        params.refit = 1
     trk = tracker.Tracker(evs[0].n_sectors, rx, gen.TAN_HALF_ANGLE, evs[0].sigma, evs[0].sigma, evs[0].bz,
-                          max_events=len(evs), max_clusters=n_total)
+                          params=params, max_events=len(evs), max_clusters=n_total)
     stream = torch.cuda.Stream()
     trk.set_stream(stream.cuda_stream)
     trk.tpc_tracker_set_profiling(True)
