@@ -178,7 +178,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--events", type=int, default=16, help="events per batch (one step)")
-    ap.add_argument("--workload", default="central", choices=["central", "semicentral", "pp"])
+    ap.add_argument("--workload", default="central", choices=["central", "semicentral", "pp", "single_sector"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--refit", action="store_true", help="also refit the output tracks (O8, SURVEY.md 8(f).1; not part of the headline path)")
@@ -315,8 +315,8 @@ def main():
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f32", "data": "synthetic",
-            "config": {"workload": "%d x %s Pb-Pb-like events per step (BASELINE.json config 5 = 16 x config 4)"
-                                   % (len(evs), args.workload),
+            "config": {"workload": ("%d x central Pb-Pb-like events per step (BASELINE.json config 5 = 16 x config 4)" % len(evs))
+                                   if args.workload == "central" else "%d x %s event(s) per step" % (len(evs), args.workload),
                        "events_per_step": len(evs), "clusters_per_step": int(n_total),
                        "tracks_per_step": int(n_tracks), "parallelism": "replicas only" if world > 1 else "1 GPU",
                        "l2": "inputs (%.0f MB per step) larger than L2 (126 MB); no flush" % (12 * n_total / 1e6)},
