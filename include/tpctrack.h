@@ -67,6 +67,12 @@ typedef struct {
                                  * pass from its lowest hit, fresh down pass from the top hit reached, no search, no
                                  * gate; trk_x/y/z/sinphi/tgl/qpt/chi2/ndf are then the refit's (x = row of the
                                  * lowest hit the down pass reached, ndf = 2 * hits in the refit - 5) */
+    int32_t merge;              /* 1: link the track segments of one particle across sector borders (O9, SURVEY.md
+                                 * 8(f).2; needs refit = 1): trk_next / trk_prev.  Sectors: n_sectors / 2 per side,
+                                 * sector s = side * (n_sectors / 2) + k at azimuth (k + 1/2) * 4 pi / n_sectors */
+    float merge_dy, merge_dz;   /* cm: tolerated |dy|, |dz| between the extrapolated and the found segment */
+    float merge_ds, merge_dt;   /* tolerated |d sin phi|, |d tg lambda| */
+    int32_t merge_max_gap;      /* pad rows that may be missing between the two segments */
 } tpc_params;
 
 /* One event's clusters: SoA, grouped by sector, ANY order inside a sector.

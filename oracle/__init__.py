@@ -40,6 +40,8 @@ class Params(C.Structure):
         ("max_gap", C.c_int32), ("edge_margin", C.c_float),
         ("min_tracklet_hits", C.c_int32), ("min_track_hits", C.c_int32),
         ("refit", C.c_int32),
+        ("merge", C.c_int32), ("merge_dy", C.c_float), ("merge_dz", C.c_float), ("merge_ds", C.c_float),
+        ("merge_dt", C.c_float), ("merge_max_gap", C.c_int32),
     ]
 
     def as_dict(self):
@@ -54,9 +56,9 @@ class _Geometry(C.Structure):
 _FIELDS = ["link_up", "link_dn", "clink_up", "clink_dn", "nf_margin", "seed_offset", "start_hit",
            "tl_first_row", "tl_last_row", "tl_n_hits", "tl_par", "tl_chi2", "tl_margin", "tl_table",
            "trk_sector", "trk_first_hit", "trk_n_hits", "trk_ndf", "trk_seed", "trk_first_row",
-           "trk_x", "trk_y", "trk_z", "trk_sinphi", "trk_tgl", "trk_qpt", "trk_chi2", "trk_margin", "hit_idx", "tl_cov"]
+           "trk_x", "trk_y", "trk_z", "trk_sinphi", "trk_tgl", "trk_qpt", "trk_chi2", "trk_margin", "hit_idx", "tl_cov", "trk_row_out", "trk_out", "trk_next", "trk_prev"]
 _F64 = {"nf_margin", "tl_par", "tl_cov", "tl_chi2", "tl_margin", "trk_x", "trk_y", "trk_z", "trk_sinphi", "trk_tgl",
-        "trk_qpt", "trk_chi2", "trk_margin"}
+        "trk_qpt", "trk_chi2", "trk_margin", "trk_out"}
 
 _lib = None
 
@@ -138,7 +140,7 @@ def track_event(geom: Geometry, sector_offset, y, z, row, params: Params | None 
         shapes = {"link_up": (N,), "link_dn": (N,), "clink_up": (N,), "clink_dn": (N,), "nf_margin": (N,),
                   "seed_offset": (geom.n_sectors + 1,), "start_hit": (S,), "tl_first_row": (S,), "tl_last_row": (S,),
                   "tl_n_hits": (S,), "tl_par": (S, 5), "tl_cov": (S, 5), "tl_chi2": (S,), "tl_margin": (S,), "tl_table": (S, NR),
-                  "hit_idx": (H,)}
+                  "hit_idx": (H,), "trk_out": (T, 6)}
         out = Result(n_clusters=N, n_seeds=S, n_tracks=T, n_track_hits=H)
         for i, name in enumerate(_FIELDS):
             shape = shapes.get(name, (T,))

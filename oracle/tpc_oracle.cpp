@@ -54,6 +54,10 @@ typedef struct {
     float edge_margin;          /* cm beyond the wedge before a pass ends */
     int32_t min_tracklet_hits, min_track_hits;
     int32_t refit;              /* O8: 1 = track parameters from a refit over the final hit list */
+    int32_t merge;              /* O9: 1 = link track segments across sector borders (needs refit) */
+    float merge_dy, merge_dz;   /* cm: tolerated |dy|, |dz| between the extrapolated and the found segment */
+    float merge_ds, merge_dt;   /* tolerated |d sin phi|, |d tg lambda| */
+    int32_t merge_max_gap;      /* pad rows that may be missing between the two segments */
 } oracle_params;
 
 typedef struct {
@@ -108,6 +112,9 @@ struct Result {
     std::vector<int32_t> trk_sector, trk_first_hit, trk_n_hits, trk_ndf, trk_seed, trk_first_row;
     std::vector<double> trk_x, trk_y, trk_z, trk_sinphi, trk_tgl, trk_qpt, trk_chi2, trk_margin;
     std::vector<int32_t> hit_idx;
+    /* O8 outer state (up pass of the refit, at its top hit) and O9 links */
+    std::vector<int32_t> trk_row_out, trk_next, trk_prev;
+    std::vector<double> trk_out; /* [T][6] x y z sin phi tg lambda q/pT */
 };
 
 template <class R> struct Sector {
@@ -387,7 +394,8 @@ template <class R> struct Sector {
        transporting to every consecutive row; down pass = fresh fit at the top hit reached with (s, t, q) of the
        up pass.  A failed transport ends a pass.  Result = state after the last update of the down pass
        (x_ref = row of that hit), chi2 and hit count of the down pass.  Lists of fewer than 2 hits are left alone. */
-    bool refit(const std::vector<int32_t>& hits, double par[5], double& chi2, int& n_fit, int& ref_row) const {
+    bool refit(const std::vector<int32_t>& hits, double par[5], double& chi2, int& n_fit, int& ref_row, double out[5],
+               int& out_row) const {
         const int m = (int)hits.size();
         if (m < 2) return false;
         Margin mg;
@@ -412,6 +420,9 @@ template <class R> struct Sector {
                 if (row == grow[hits[k]]) { update(f, hits[k]); snap = f; k_top = k; k++; }
             }
         }
+        /* outer state: the up pass right after its last update (all hits below are in it) */
+        out[0] = (double)snap.y; out[1] = (double)snap.z; out[2] = (double)snap.s; out[3] = (double)snap.t;
+        out[4] = (double)snap.q; out_row = grow[hits[k_top]];
         {
             const int32_t ht = hits[k_top];
             f.y = R(gy[ht]); f.z = R(gz[ht]); f.s = snap.s; f.t = snap.t; f.q = snap.q;
@@ -433,6 +444,83 @@ template <class R> struct Sector {
     }
 };
 
+
+/* ---- O9 cross-sector merge ("merged together" PAPER.md:53) ----
+ * Sectors: half = n_sectors / 2 per side, sector s = side * half + k, centre azimuth (k + 1/2) * 2 pi / half.
+ * Segment A (sector s_A, outer state of its refit at pad row r_A) may continue in segment B of a sector next to it on
+ * the same side whose first fitted row r_B obeys 1 <= r_B - r_A <= 1 + max_gap.  A's outer state is turned into
+ * B's frame (angle alpha_A - alpha_B), moved along its helix to x = row_x[r_B] (state only, the O5 transport
+ * formulas) and compared with B's parameters there:
+ *   |dy| <= merge_dy, |dz| <= merge_dz, |d sin phi| <= merge_ds, |d tg lambda| <= merge_dt,
+ *   D = (dy/merge_dy)^2 + (dz/merge_dz)^2 + (ds/merge_ds)^2 + (dt/merge_dt)^2.
+ * next(A) = arg min_B D, prev(B) = arg min_A D (ties -> lowest track index); a link is kept when mutual. */
+template <class R>
+void merge_segments(const oracle_geometry& G, const oracle_params& P, Result& res) {
+    const int T = (int)res.trk_sector.size();
+    res.trk_next.assign(T, -1); res.trk_prev.assign(T, -1);
+    if (G.n_sectors < 4 || (G.n_sectors & 1)) return;
+    const int half = G.n_sectors / 2;
+    const double step = 2.0 * 3.14159265358979323846 / (double)half;
+    const R cd = R(std::cos(step)), sd = R(std::sin(step));   /* rounded once to R */
+    const R kB = R(-1) * (R(kLight) * R(G.bz));
+    const R smax = R(P.sin_max);
+    const R ty = R(P.merge_dy), tz = R(P.merge_dz), ts = R(P.merge_ds), tt = R(P.merge_dt);
+    std::vector<R> bestn(T, R(0)), bestp(T, R(0));
+    auto pair_score = [&](int a, int b, R& D) -> bool {
+        if (res.trk_row_out[a] < 0 || res.trk_row_out[b] < 0) return false;   /* no refit (fewer than 2 hits) */
+        const int sa = res.trk_sector[a], sb = res.trk_sector[b];
+        if (sa / half != sb / half) return false;
+        const int dk = ((sb % half) - (sa % half) + half) % half;
+        if (dk != 1 && dk != half - 1) return false;
+        const int gap = res.trk_first_row[b] - res.trk_row_out[a];
+        if (gap < 1 || gap > 1 + P.merge_max_gap) return false;
+        const double* o = &res.trk_out[6 * (size_t)a];
+        const R xa = R(o[0]), ya = R(o[1]), za = R(o[2]), s0 = R(o[3]), t0 = R(o[4]), q0 = R(o[5]);
+        /* turn by alpha_A - alpha_B: -step when B is the next sector, +step when it is the one before */
+        const R sn = (dk == 1) ? R(0) - sd : sd;
+        if (std::fabs(s0) > smax) return false;
+        const R c0a = std::sqrt(R(1) - s0 * s0);
+        const R x1 = xa * cd - ya * sn;
+        const R y1 = xa * sn + ya * cd;
+        const R s1 = s0 * cd + c0a * sn;
+        /* along the helix to B's reference row */
+        const R xb = R(res.trk_x[b]);
+        const R dx = xb - x1;
+        const R kap = kB * q0;
+        const R s2 = s1 + kap * dx;
+        if (std::fabs(s1) > smax || std::fabs(s2) > smax) return false;
+        const R c1 = std::sqrt(R(1) - s1 * s1), c2 = std::sqrt(R(1) - s2 * s2);
+        const R dy = dx * ((s1 + s2) * (R(1) / (c1 + c2)));
+        const R dl2 = dx * dx + dy * dy;
+        const R adl = std::sqrt(dl2);
+        const R dl = (dx < R(0)) ? R(0) - adl : adl;
+        const R u = kap * dl, u2 = u * u;
+        const R dS = dl * (R(1) + u2 * (R(1) / R(24) + u2 * (R(3) / R(640))));
+        const R y2 = y1 + dy, z2 = za + t0 * dS;
+        const R ey = y2 - R(res.trk_y[b]), ez = z2 - R(res.trk_z[b]);
+        const R es = s2 - R(res.trk_sinphi[b]), et = t0 - R(res.trk_tgl[b]);
+        if (!(std::fabs(ey) <= ty && std::fabs(ez) <= tz && std::fabs(es) <= ts && std::fabs(et) <= tt)) return false;
+        const R ny = ey * (R(1) / ty), nz = ez * (R(1) / tz), ns = es * (R(1) / ts), nt = et * (R(1) / tt);
+        D = ((ny * ny + nz * nz) + ns * ns) + nt * nt;
+        return true;
+    };
+    std::vector<int32_t> nx(T, -1), pv(T, -1);
+    for (int a = 0; a < T; a++)
+        for (int b = 0; b < T; b++) {
+            R D;
+            if (a == b || !pair_score(a, b, D)) continue;
+            if (nx[a] < 0 || D < bestn[a]) { nx[a] = b; bestn[a] = D; }   /* ascending b: ties keep the lower index */
+        }
+    for (int b = 0; b < T; b++)
+        for (int a = 0; a < T; a++) {
+            R D;
+            if (a == b || !pair_score(a, b, D)) continue;
+            if (pv[b] < 0 || D < bestp[b]) { pv[b] = a; bestp[b] = D; }
+        }
+    for (int a = 0; a < T; a++)
+        if (nx[a] >= 0 && pv[nx[a]] == a) { res.trk_next[a] = nx[a]; res.trk_prev[nx[a]] = a; }
+}
+
 template <class R>
 Result* run(const oracle_geometry& G, const oracle_params& P, int32_t n, const int32_t* sector_offset, const float* y,
             const float* z, const int32_t* row, int n_threads, int stop_after) {
@@ -445,7 +533,7 @@ Result* run(const oracle_geometry& G, const oracle_params& P, int32_t n, const i
     std::vector<std::vector<int32_t>> seeds(ns);
     std::vector<std::vector<Tracklet>> tls(ns);
     /* per-sector output tracks */
-    struct Refit { bool ok = false; double par[5] = {0, 0, 0, 0, 0}, chi2 = 0; int n_fit = 0, ref_row = 0; };
+    struct Refit { bool ok = false; double par[5] = {0, 0, 0, 0, 0}, chi2 = 0, out[5] = {0, 0, 0, 0, 0}; int n_fit = 0, ref_row = 0, out_row = -1; };
     struct Out { std::vector<int32_t> seed, nh, first_row; std::vector<std::vector<int32_t>> hits; std::vector<Refit> refit; };
     std::vector<Out> outs(ns);
 #ifdef _OPENMP
@@ -491,7 +579,7 @@ Result* run(const oracle_geometry& G, const oracle_params& P, int32_t n, const i
             outs[s].nh.push_back((int32_t)hits.size());
             outs[s].first_row.push_back(T.first_row);
             Refit rf;   /* ---- O8 ---- */
-            if (P.refit) rf.ok = S.refit(hits, rf.par, rf.chi2, rf.n_fit, rf.ref_row);
+            if (P.refit) rf.ok = S.refit(hits, rf.par, rf.chi2, rf.n_fit, rf.ref_row, rf.out, rf.out_row);
             outs[s].refit.push_back(rf);
             outs[s].hits.push_back(std::move(hits));
         }
@@ -525,9 +613,14 @@ Result* run(const oracle_geometry& G, const oracle_params& P, int32_t n, const i
                 res->trk_y.back() = rf.par[0]; res->trk_z.back() = rf.par[1]; res->trk_sinphi.back() = rf.par[2];
                 res->trk_tgl.back() = rf.par[3]; res->trk_qpt.back() = rf.par[4]; res->trk_chi2.back() = rf.chi2;
             }
+            res->trk_row_out.push_back(rf.ok ? rf.out_row : -1);
+            res->trk_out.push_back(rf.ok ? (double)G.row_x[rf.out_row] : 0.0);
+            for (int j = 0; j < 5; j++) res->trk_out.push_back(rf.ok ? rf.out[j] : 0.0);
             for (int32_t h : outs[s].hits[k]) res->hit_idx.push_back(h);
         }
     }
+    if (P.merge && P.refit && stop_after == 0) merge_segments<R>(G, P, *res);
+    else { res->trk_next.assign(res->trk_sector.size(), -1); res->trk_prev.assign(res->trk_sector.size(), -1); }
     return res;
 }
 
@@ -550,6 +643,7 @@ void oracle_default_params(oracle_params* p) {
     p->max_gap = 5; p->edge_margin = 1.0f;
     p->min_tracklet_hits = 10; p->min_track_hits = 10;
     p->refit = 0;
+    p->merge = 0; p->merge_dy = 1.0f; p->merge_dz = 1.0f; p->merge_ds = 0.05f; p->merge_dt = 0.05f; p->merge_max_gap = 6;
 }
 
 /* precision: 0 = double, 1 = strict float32.  stop_after: 0 = everything, 2 = after O2, 4 = after O4,
@@ -578,7 +672,7 @@ enum {
     F_LINK_UP = 0, F_LINK_DN, F_CLINK_UP, F_CLINK_DN, F_NF_MARGIN, F_SEED_OFFSET, F_START_HIT,
     F_TL_FIRST_ROW, F_TL_LAST_ROW, F_TL_N_HITS, F_TL_PAR, F_TL_CHI2, F_TL_MARGIN, F_TL_TABLE,
     F_TRK_SECTOR, F_TRK_FIRST_HIT, F_TRK_N_HITS, F_TRK_NDF, F_TRK_SEED, F_TRK_FIRST_ROW,
-    F_TRK_X, F_TRK_Y, F_TRK_Z, F_TRK_SINPHI, F_TRK_TGL, F_TRK_QPT, F_TRK_CHI2, F_TRK_MARGIN, F_HIT_IDX, F_TL_COV
+    F_TRK_X, F_TRK_Y, F_TRK_Z, F_TRK_SINPHI, F_TRK_TGL, F_TRK_QPT, F_TRK_CHI2, F_TRK_MARGIN, F_HIT_IDX, F_TL_COV, F_TRK_ROW_OUT, F_TRK_OUT, F_TRK_NEXT, F_TRK_PREV
 };
 
 /* copy one result field into caller memory (int32 or float64, shapes in oracle/__init__.py) */
@@ -620,6 +714,10 @@ int32_t oracle_copy(const void* rv, int32_t field, void* dst) {
         case F_TRK_CHI2: copy_out(r->trk_chi2, dst); break;
         case F_TRK_MARGIN: copy_out(r->trk_margin, dst); break;
         case F_HIT_IDX: copy_out(r->hit_idx, dst); break;
+        case F_TRK_ROW_OUT: copy_out(r->trk_row_out, dst); break;
+        case F_TRK_OUT: copy_out(r->trk_out, dst); break;
+        case F_TRK_NEXT: copy_out(r->trk_next, dst); break;
+        case F_TRK_PREV: copy_out(r->trk_prev, dst); break;
         default: return -1;
     }
     return 0;

@@ -437,6 +437,7 @@ void tpc_default_params(tpc_params* p) {
     p->max_gap = 5; p->edge_margin = 1.0f;
     p->min_tracklet_hits = 10; p->min_track_hits = 10;
     p->refit = 0;
+    p->merge = 0; p->merge_dy = 1.0f; p->merge_dz = 1.0f; p->merge_ds = 0.05f; p->merge_dt = 0.05f; p->merge_max_gap = 6;
 }
 
 const char* tpc_status_string(int s) {
@@ -467,8 +468,9 @@ tpc_tracker* tpc_tracker_create_ex(const tpc_geometry* g, float bz, const tpc_pa
     }
     tpc_params p;
     if (params) p = *params; else tpc_default_params(&p);
-    if (p.link_step < 1 || p.link_step > 2 || p.min_tracklet_hits < 1 || p.min_track_hits < 1 || p.max_gap < 0 || p.refit < 0 || p.refit > 1) {
-        set_err("params: link_step must be 1 or 2, minimum hit counts >= 1, max_gap >= 0, refit 0 or 1");
+    if (p.link_step < 1 || p.link_step > 2 || p.min_tracklet_hits < 1 || p.min_track_hits < 1 || p.max_gap < 0 || p.refit < 0 || p.refit > 1 || p.merge < 0 || p.merge > 1 ||
+        (p.merge && !p.refit) || p.merge_max_gap < 0 || !(p.merge_dy > 0.f) || !(p.merge_dz > 0.f) || !(p.merge_ds > 0.f) || !(p.merge_dt > 0.f)) {
+        set_err("params: link_step must be 1 or 2, minimum hit counts >= 1, max_gap >= 0, refit 0 or 1, merge 0 or 1 (needs refit) with positive tolerances");
         return nullptr;
     }
     int dev = 0, ndev = 0;

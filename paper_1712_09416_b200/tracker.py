@@ -32,7 +32,9 @@ class tpc_params(C.Structure):
                 ("nf_dmax", C.c_float), ("sin_max", C.c_float), ("var_s", C.c_float), ("var_t", C.c_float),
                 ("var_q", C.c_float), ("chi2_link", C.c_float), ("chi2_ext", C.c_float), ("win_nsigma", C.c_float),
                 ("win_min", C.c_float), ("win_max", C.c_float), ("max_gap", C.c_int32), ("edge_margin", C.c_float),
-                ("min_tracklet_hits", C.c_int32), ("min_track_hits", C.c_int32), ("refit", C.c_int32)]
+                ("min_tracklet_hits", C.c_int32), ("min_track_hits", C.c_int32), ("refit", C.c_int32),
+                ("merge", C.c_int32), ("merge_dy", C.c_float), ("merge_dz", C.c_float), ("merge_ds", C.c_float),
+                ("merge_dt", C.c_float), ("merge_max_gap", C.c_int32)]
 
     def as_dict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}
