@@ -111,6 +111,18 @@ typedef struct {
     const float* trk_qpt;         /* 1/(GeV/c), signed */
     const float* trk_chi2;
     const int32_t* hit_idx;       /* [n_track_hits] indices into the caller's cluster arrays, row-ascending */
+    /* tpc_params.refit = 1 (NULL otherwise): the refit's OUTER state, i.e. its up pass right after the update with
+     * the track's top hit, at x = trk_out_x (all hits of the track are in it; it is what extrapolates outwards) */
+    const float* trk_out_x;       /* [n_tracks] cm */
+    const float* trk_out_y;
+    const float* trk_out_z;
+    const float* trk_out_sinphi;
+    const float* trk_out_tgl;
+    const float* trk_out_qpt;
+    /* tpc_params.merge = 1 (NULL otherwise): the segment that continues this one in a neighbouring sector /
+     * the segment this one continues; index into this event's tracks or -1.  Links are mutual and one-to-one. */
+    const int32_t* trk_next;      /* [n_tracks] */
+    const int32_t* trk_prev;      /* [n_tracks] */
 } tpc_event_out;
 
 /* Counters of the last call (whole batch); used for the algorithmic-byte count of DESIGN.md. */

@@ -39,6 +39,7 @@ struct Const {
     float row_x[TPC_MAX_ROWS + 1];
     int32_t n_sectors, n_rows;
     float tan_half_angle, sigma_y2, sigma_z2, kB;
+    float merge_cd, merge_sd;   // cos, sin of the angle between neighbouring sectors (O9)
     tpc_params p;
 };
 
@@ -97,6 +98,10 @@ struct View {
     // refit of the output tracks (tpc_params.refit): the tracks' hits as (y,z) and pad row, in hit-list order
     float2* o_hit_yz; uint8_t* o_hit_row;   // [N]
     int32_t* trk_hit0;       // [S_cap] first entry of a track's hit list in the batch's hit arrays
+    int32_t* trk_rows;       // [S_cap] refit: reference row | outer row << 8, or -1 (no refit)
+    int32_t* trk_task;       // [S_cap] sector task of a track (O9)
+    float *o_xo, *o_yo, *o_zo, *o_so, *o_to, *o_qo;   // [S_cap] outer state of the refit (up pass at its top hit)
+    int32_t *o_next, *o_prev;   // [S_cap] O9 links, event-local track index or -1
     unsigned long long* cnt; // [CNT_N]
     unsigned long long* kf_cursor;  // [n_events * kMaxSM] K5: start hits handed out per (event, SM) share
 };

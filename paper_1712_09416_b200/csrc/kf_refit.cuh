@@ -25,6 +25,7 @@ __global__ void __launch_bounds__(kRfThreads, kRfBlocksPerSM) k_refit(const View
     f.n = 0; f.chi2 = 0.f;
     float s_s = 0.f, s_t = 0.f, s_q = 0.f;          // sin phi, tg lambda, q/pT right after the last update (up pass)
     float ty = 0.f, tz = 0.f;                        // the hit of that update
+    float uy = 0.f, uz = 0.f;                        // y, z of the up pass right after that update
     float p0 = 0.f, p1 = 0.f, p2 = 0.f, p3 = 0.f, p4 = 0.f, p5 = 0.f;   // down pass: state after its last update
     float ny = 0.f, nz = 0.f;                        // the track's next hit, read one trip ahead
     int nrow = -1;
@@ -39,6 +40,7 @@ __global__ void __launch_bounds__(kRfThreads, kRfBlocksPerSM) k_refit(const View
             b = __shfl_sync(kFull, b, 0);
             if (b >= T) more = false;
             const int cand = b + __popc(idle & lanemask_lt());
+            if (ph == 0 && cand < T && v.o_n_hits[cand] < 2) v.trk_rows[cand] = -1;
             if (ph == 0 && cand < T && v.o_n_hits[cand] >= 2) {
                 ti = cand; h0 = v.trk_hit0[ti]; m = v.o_n_hits[ti];
                 const float2 a0 = v.o_hit_yz[h0], a1 = v.o_hit_yz[h0 + 1];
@@ -49,7 +51,7 @@ __global__ void __launch_bounds__(kRfThreads, kRfBlocksPerSM) k_refit(const View
                 const float dl = sqrtf(dx * dx + dy * dy);
                 f.y = a0.x; f.z = a0.y; f.s = dy / dl; f.t = dz / dl; f.q = 0.f;
                 fit_prior(f, c); f.n = 1;
-                s_s = f.s; s_t = f.t; s_q = f.q; ty = a0.x; tz = a0.y;
+                s_s = f.s; s_t = f.t; s_q = f.q; ty = a0.x; tz = a0.y; uy = a0.x; uz = a0.y;
                 row = rfirst; rtop = rfirst; ktop = 0; k = 1; ny = a1.x; nz = a1.y; nrow = r1;
                 ph = 1;
             }
@@ -68,14 +70,15 @@ __global__ void __launch_bounds__(kRfThreads, kRfBlocksPerSM) k_refit(const View
         if (upd) {
             const float iwy = 1.f / (f.c00 + c.sigma_y2);
             fit_update(f, ny, nz, iwy, c);
-            if (up) { s_s = f.s; s_t = f.t; s_q = f.q; ty = ny; tz = nz; rtop = row; ktop = k; k++; }
+            if (up) { s_s = f.s; s_t = f.t; s_q = f.q; ty = ny; tz = nz; uy = f.y; uz = f.z; rtop = row; ktop = k; k++; }
             else { p0 = f.y; p1 = f.z; p2 = f.s; p3 = f.t; p4 = f.q; p5 = f.chi2; rref = row; nfit = f.n; k--; }
             nrow = -1;
             if (k >= 0 && k < m) { const float2 hn = v.o_hit_yz[h0 + k]; ny = hn.x; nz = hn.y; nrow = v.o_hit_row[h0 + k]; }
         }
         __syncwarp();
         if (ph != 0 && end) {
-            if (up) {   // fresh fit at the top hit reached
+            if (up) {   // outer state for O9, then a fresh fit at the top hit reached
+                v.o_xo[ti] = c.row_x[rtop]; v.o_yo[ti] = uy; v.o_zo[ti] = uz; v.o_so[ti] = s_s; v.o_to[ti] = s_t; v.o_qo[ti] = s_q;
                 f.y = ty; f.z = tz; f.s = s_s; f.t = s_t; f.q = s_q;
                 fit_prior(f, c); f.n = 1;
                 p0 = ty; p1 = tz; p2 = s_s; p3 = s_t; p4 = s_q; p5 = 0.f; rref = rtop; nfit = 1;
@@ -87,6 +90,7 @@ __global__ void __launch_bounds__(kRfThreads, kRfBlocksPerSM) k_refit(const View
                 v.o_x[ti] = c.row_x[rref];
                 v.o_y[ti] = p0; v.o_z[ti] = p1; v.o_sinphi[ti] = p2; v.o_tgl[ti] = p3; v.o_qpt[ti] = p4; v.o_chi2[ti] = p5;
                 v.o_ndf[ti] = 2 * nfit - 5;
+                v.trk_rows[ti] = rref | (rtop << 8);
                 ph = 0;
             }
         }

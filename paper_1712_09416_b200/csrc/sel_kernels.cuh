@@ -170,7 +170,7 @@ __global__ void __launch_bounds__(kSelCtaThreads, 2) k_select_write(const View v
                     const int ti = v.trk_scan[i];
                     const int sc = v.S_cap;
                     v.o_sector[ti] = task - e * c.n_sectors;
-                    if (c.p.refit) v.trk_hit0[ti] = ho;
+                    if (c.p.refit) { v.trk_hit0[ti] = ho; v.trk_task[ti] = task; }
                     v.o_first_hit[ti] = ho - v.ev_off[v.n_events + 1 + e];
                     v.o_n_hits[ti] = v.tl_nown[i];
                     v.o_ndf[ti] = 2 * nh - 5;

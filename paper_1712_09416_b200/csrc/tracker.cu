@@ -1,6 +1,7 @@
 // tracker.cu -- host side of libtpctrack.so: the C ABI of include/tpctrack.h, work-space management and the
 // launch sequence K1..K6 for a batch of events (all n_events * n_sectors sector tasks in every launch).
 #include <algorithm>
+#include <cmath>
 #include <cstdarg>
 #include <cstdio>
 #include <cstdlib>
@@ -13,8 +14,11 @@
 #include "kf_sweep.cuh"
 #include "sel_kernels.cuh"
 #include "kf_refit.cuh"
+#include "merge_kernels.cuh"
 
 namespace {
+
+constexpr int kOutI = 6, kOutF = 13;   // int32 / float arrays per track: 4 + next, prev; 7 + the outer state
 
 thread_local std::string g_err;
 
@@ -75,11 +79,11 @@ struct Batch {
     std::vector<int32_t> ev_n, ev_off;       // clusters per event, offset in the group
     tpc_counters counters;                   // of the group's last run
     // device pools
-    Buf<float> in_y, in_z, tl_par, o_f[7];
+    Buf<float> in_y, in_z, tl_par, o_f[kOutF];
     Buf<float2> thit, shit;
     Buf<int32_t> in_row, sec_off, bin_count, bin_start, tidx, sorig, link_up, link_dn, clink_up, clink_dn, seed_count,
         seed_start, seeds, seed_bin, tl_rows, tl_nown, tl_keep, trk_scan, hit_scan, ev_off_d, scratch,
-        o_i[4], o_hit;
+        o_i[kOutI], o_hit, trk_rows, trk_task, mg_next, mg_prev;
     Buf<uint16_t> slot, cells, tl_tab;
     Buf<float2> o_hit_yz;
     Buf<uint8_t> o_hit_row;
@@ -114,7 +118,7 @@ struct Batch {
         scratch.release(); o_hit.release();
         for (auto& b : o_i) b.release();
         slot.release(); cells.release(); desc.release(); owner.release(); ev_src.release();
-        seed_rec.release(); tl_up.release(); dn_rec.release(); dn_count.release(); dn_start.release(); dn_fill.release(); tl_cnt.release(); o_hit_yz.release(); o_hit_row.release(); trk_hit0.release();
+        seed_rec.release(); tl_up.release(); dn_rec.release(); dn_count.release(); dn_start.release(); dn_fill.release(); tl_cnt.release(); o_hit_yz.release(); o_hit_row.release(); trk_hit0.release(); trk_rows.release(); trk_task.release(); mg_next.release(); mg_prev.release();
         cnt.release(); kf_cursor.release(); h_ev_src.release(); h_sec_off.release(); h_ev_off.release(); h_cnt.release(); h_nseeds.release();
         for (auto& e : evt) if (e) { cudaEventDestroy(e); e = nullptr; }
     }
@@ -136,8 +140,8 @@ struct tpc_tracker {
     bool have_result = false;
     int n_events = 0;
     std::vector<int> ev_slot, ev_local;      // where the intermediates of each event are (-1: overwritten since)
-    Buf<int32_t> h_o_i[4], h_o_hit;          // host-input calls: the outputs of all groups, pinned
-    Buf<float> h_o_f[7];
+    Buf<int32_t> h_o_i[kOutI], h_o_hit;          // host-input calls: the outputs of all groups, pinned
+    Buf<float> h_o_f[kOutF];
     bool profiling = false;
     float stage_ms[TPC_N_STAGES] = {};
 
@@ -181,8 +185,10 @@ int reserve_batch(const tpc_tracker* tr, Batch* t, int n_events, int64_t N, int6
     RS(ev_off_d, 2 * ((size_t)n_events + 1)); RS(h_ev_off, 2 * ((size_t)n_events + 1));
     RS(scratch, (size_t)std::max<int64_t>(nb, S_cap) / kScanTile + 8);
     RS(cnt, CNT_N); RS(h_cnt, CNT_N); RS(kf_cursor, (size_t)n_events * kMaxSM); RS(h_nseeds, 1);
-    for (int k = 0; k < 4; k++) RS(o_i[k], S_cap);
-    for (int k = 0; k < 7; k++) RS(o_f[k], S_cap);
+    for (int k = 0; k < kOutI; k++) RS(o_i[k], S_cap);
+    for (int k = 0; k < kOutF; k++) RS(o_f[k], S_cap);
+    if (tr->c.p.refit) { RS(trk_rows, S_cap); RS(trk_task, S_cap); }
+    if (tr->c.p.merge) { RS(mg_next, S_cap); RS(mg_prev, S_cap); }
     RS(o_hit, n);
     if (tr->c.p.refit) { RS(o_hit_yz, n); RS(o_hit_row, n); RS(trk_hit0, S_cap); }
 #undef RS
@@ -266,6 +272,12 @@ int launch_all(const tpc_tracker* tr, Batch* t) {
     k_select_write<<<sel_grid, kSelCtaThreads, kSelCap * sizeof(uint32_t), st>>>(v, c); L++;
     mark(5);
     if (c.p.refit) { k_refit<<<tr->rf_blocks, kRfThreads, 0, st>>>(v, c); L++; }
+    if (c.p.merge) {   // the track count is on the device: grids cover the start-hit capacity
+        const int g = (int)((t->S_cap + 127) / 128);
+        k_merge_best<true><<<g, 128, 0, st>>>(v, c, t->mg_next.p); L++;
+        k_merge_best<false><<<g, 128, 0, st>>>(v, c, t->mg_prev.p); L++;
+        k_merge_mutual<<<g, 128, 0, st>>>(v, c, t->mg_next.p, t->mg_prev.p); L++;
+    }
     mark(6);
     CK(cudaGetLastError());
     t->counters.n_kernel_launches += L;
@@ -338,6 +350,8 @@ int batch_begin(const tpc_tracker* tr, Batch* t, int first_event, int n, const t
     v.o_hit_idx = t->o_hit.p;
     v.o_x = t->o_f[0].p; v.o_y = t->o_f[1].p; v.o_z = t->o_f[2].p; v.o_sinphi = t->o_f[3].p;
     v.o_tgl = t->o_f[4].p; v.o_qpt = t->o_f[5].p; v.o_chi2 = t->o_f[6].p;
+    v.o_xo = t->o_f[7].p; v.o_yo = t->o_f[8].p; v.o_zo = t->o_f[9].p; v.o_so = t->o_f[10].p; v.o_to = t->o_f[11].p; v.o_qo = t->o_f[12].p;
+    v.o_next = t->o_i[4].p; v.o_prev = t->o_i[5].p; v.trk_rows = t->trk_rows.p; v.trk_task = t->trk_task.p;
     v.cnt = t->cnt.p; v.kf_cursor = t->kf_cursor.p;
     v.o_hit_yz = t->o_hit_yz.p; v.o_hit_row = t->o_hit_row.p; v.trk_hit0 = t->trk_hit0.p;
     v.seed_rec = t->seed_rec.p; v.tl_up = t->tl_up.p; v.dn_rec = t->dn_rec.p;
@@ -488,6 +502,10 @@ tpc_tracker* tpc_tracker_create_ex(const tpc_geometry* g, float bz, const tpc_pa
     t->c.sigma_y2 = g->sigma_y * g->sigma_y; t->c.sigma_z2 = g->sigma_z * g->sigma_z;
     t->c.kB = -1.f * (0.00299792458f * bz);  // curvature = kB * q/pT, DESIGN.md "Conventions"
     t->c.p = p;
+    {   // O9: angle between neighbouring sectors, rounded once to float
+        const double step = 2.0 * 3.14159265358979323846 / (double)std::max(g->n_sectors / 2, 1);
+        t->c.merge_cd = (float)cos(step); t->c.merge_sd = (float)sin(step);
+    }
     if (g->sector_alpha) t->sector_alpha.assign(g->sector_alpha, g->sector_alpha + g->n_sectors);
     cudaDeviceGetAttribute(&t->sm_count, cudaDevAttrMultiProcessorCount, dev);
     if (t->sm_count > kMaxSM) { set_err("more than %d SMs", kMaxSM); delete t; return nullptr; }
@@ -576,6 +594,7 @@ int tpc_track_events(tpc_tracker* t, int32_t n, const tpc_event_in* in, tpc_even
     t->n_events = n;
 
     int64_t T_cum = 0, H_cum = 0;
+    const int nI = t->c.p.merge ? kOutI : 4, nF = t->c.p.refit ? kOutF : 7;   // arrays that hold something
     std::vector<int64_t> trk_off(n + 1, 0), hit_off(n + 1, 0);   // per event, in the call's output arrays
     std::vector<const Batch*> ev_batch(n, nullptr);
     int g_issue = 0, g_done = 0;
@@ -606,17 +625,15 @@ int tpc_track_events(tpc_tracker* t, int32_t n, const tpc_event_in* in, tpc_even
         if (host_in) {   // the group's tracks go behind those of the groups before it
             const size_t left = (size_t)(n_groups - g_done - 1);
             const View& v = b->v;
-            const int32_t* oi[4] = {v.o_sector, v.o_first_hit, v.o_n_hits, v.o_ndf};
-            const float* of[7] = {v.o_x, v.o_y, v.o_z, v.o_sinphi, v.o_tgl, v.o_qpt, v.o_chi2};
             const size_t needT = (size_t)std::max<int64_t>(T_cum + T, 1), hintT = needT + needT / 8 + left * (size_t)(T + T / 4);
             const size_t needH = (size_t)std::max<int64_t>(H_cum + H, 1), hintH = needH + needH / 8 + left * (size_t)(H + H / 4);
-            for (int k = 0; k < 4; k++) {
+            for (int k = 0; k < nI; k++) {
                 if ((rc = grow_keep(t, t->h_o_i[k], needT, (size_t)T_cum, hintT)) != TPC_OK) return rc;
-                if (T) CK(cudaMemcpyAsync(t->h_o_i[k].p + T_cum, oi[k], sizeof(int32_t) * T, cudaMemcpyDeviceToHost, b->stream));
+                if (T) CK(cudaMemcpyAsync(t->h_o_i[k].p + T_cum, b->o_i[k].p, sizeof(int32_t) * T, cudaMemcpyDeviceToHost, b->stream));
             }
-            for (int k = 0; k < 7; k++) {
+            for (int k = 0; k < nF; k++) {
                 if ((rc = grow_keep(t, t->h_o_f[k], needT, (size_t)T_cum, hintT)) != TPC_OK) return rc;
-                if (T) CK(cudaMemcpyAsync(t->h_o_f[k].p + T_cum, of[k], sizeof(float) * T, cudaMemcpyDeviceToHost, b->stream));
+                if (T) CK(cudaMemcpyAsync(t->h_o_f[k].p + T_cum, b->o_f[k].p, sizeof(float) * T, cudaMemcpyDeviceToHost, b->stream));
             }
             if ((rc = grow_keep(t, t->h_o_hit, needH, (size_t)H_cum, hintH)) != TPC_OK) return rc;
             if (H) CK(cudaMemcpyAsync(t->h_o_hit.p + H_cum, v.o_hit_idx, sizeof(int32_t) * H, cudaMemcpyDeviceToHost, b->stream));
@@ -630,21 +647,26 @@ int tpc_track_events(tpc_tracker* t, int32_t n, const tpc_event_in* in, tpc_even
         for (int k = 0; k < n_slots; k++) CK(cudaStreamSynchronize(t->slots[k]->stream));
     for (int e = 0; e < n; e++) {
         tpc_event_out& o = out[e];
-        const int32_t* oi[4]; const float* of[7]; const int32_t* ohit;
+        const int32_t* oi[kOutI]; const float* of[kOutF]; const int32_t* ohit;
         int64_t a = trk_off[e], h = hit_off[e];
         if (host_in) {
-            for (int k = 0; k < 4; k++) oi[k] = t->h_o_i[k].p;
-            for (int k = 0; k < 7; k++) of[k] = t->h_o_f[k].p;
+            for (int k = 0; k < kOutI; k++) oi[k] = t->h_o_i[k].p;
+            for (int k = 0; k < kOutF; k++) of[k] = t->h_o_f[k].p;
             ohit = t->h_o_hit.p;
         } else {
-            const View& v = ev_batch[e]->v;
-            oi[0] = v.o_sector; oi[1] = v.o_first_hit; oi[2] = v.o_n_hits; oi[3] = v.o_ndf;
-            of[0] = v.o_x; of[1] = v.o_y; of[2] = v.o_z; of[3] = v.o_sinphi; of[4] = v.o_tgl; of[5] = v.o_qpt; of[6] = v.o_chi2;
-            ohit = v.o_hit_idx;
+            const Batch* b = ev_batch[e];
+            for (int k = 0; k < kOutI; k++) oi[k] = b->o_i[k].p;
+            for (int k = 0; k < kOutF; k++) of[k] = b->o_f[k].p;
+            ohit = b->v.o_hit_idx;
         }
         o.trk_sector = oi[0] + a; o.trk_first_hit = oi[1] + a; o.trk_n_hits = oi[2] + a; o.trk_ndf = oi[3] + a;
         o.trk_x = of[0] + a; o.trk_y = of[1] + a; o.trk_z = of[2] + a; o.trk_sinphi = of[3] + a; o.trk_tgl = of[4] + a;
         o.trk_qpt = of[5] + a; o.trk_chi2 = of[6] + a;
+        const bool rf = t->c.p.refit != 0, mg = t->c.p.merge != 0;
+        o.trk_out_x = rf ? of[7] + a : nullptr; o.trk_out_y = rf ? of[8] + a : nullptr; o.trk_out_z = rf ? of[9] + a : nullptr;
+        o.trk_out_sinphi = rf ? of[10] + a : nullptr; o.trk_out_tgl = rf ? of[11] + a : nullptr;
+        o.trk_out_qpt = rf ? of[12] + a : nullptr;
+        o.trk_next = mg ? oi[4] + a : nullptr; o.trk_prev = mg ? oi[5] + a : nullptr;
         o.hit_idx = ohit + h;
     }
     t->have_result = true;

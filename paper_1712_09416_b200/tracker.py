@@ -47,11 +47,14 @@ class tpc_event_in(C.Structure):
 
 _OUT_I = ("trk_sector", "trk_first_hit", "trk_n_hits", "trk_ndf")
 _OUT_F = ("trk_x", "trk_y", "trk_z", "trk_sinphi", "trk_tgl", "trk_qpt", "trk_chi2")
+_OUT_F2 = ("trk_out_x", "trk_out_y", "trk_out_z", "trk_out_sinphi", "trk_out_tgl", "trk_out_qpt")   # refit = 1
+_OUT_I2 = ("trk_next", "trk_prev")                                                                   # merge = 1
 
 
 class tpc_event_out(C.Structure):
     _fields_ = ([("n_tracks", C.c_int32), ("n_track_hits", C.c_int32)] + [(n, C.c_void_p) for n in _OUT_I]
-                + [(n, C.c_void_p) for n in _OUT_F] + [("hit_idx", C.c_void_p)])
+                + [(n, C.c_void_p) for n in _OUT_F] + [("hit_idx", C.c_void_p)]
+                + [(n, C.c_void_p) for n in _OUT_F2] + [(n, C.c_void_p) for n in _OUT_I2])
 
 
 class tpc_counters(C.Structure):
@@ -262,4 +265,10 @@ class Tracker:
         for k in _OUT_F:
             res[k] = fetch(getattr(out, k), T, np.float32)
         res["hit_idx"] = fetch(out.hit_idx, H, np.int32)
+        for k in _OUT_F2:          # present with refit = 1
+            if getattr(out, k):
+                res[k] = fetch(getattr(out, k), T, np.float32)
+        for k in _OUT_I2:          # present with merge = 1
+            if getattr(out, k):
+                res[k] = fetch(getattr(out, k), T, np.int32)
         return res

@@ -293,3 +293,55 @@ def test_refit_in_a_batch_matches_single_events(trk_mod, gen_mod, oracle_mod):
             err = np.abs(res[k] - ref[k]) / np.maximum(1.0, np.abs(ref[k]))
             assert err.max(initial=0.0) <= TOL, (k, err.max())
     trk.close()
+
+
+@pytest.mark.parametrize("name,device", [("pp", True), ("semicentral", True), ("semicentral", False), ("central", True)])
+def test_merge_parity(trk_mod, gen_mod, oracle_mod, name, device):
+    """O9 (tpc_params.merge = 1): links between the segments of one particle across sector borders, and the refit's
+    outer states they are made from, against the oracle (strict float32)."""
+    ev = gen_mod.generate(name)
+    p = oracle_mod.default_params()
+    p.refit = 1; p.merge = 1
+    ref = oracle_mod.track_event(make_geometry(oracle_mod, gen_mod, ev), ev.sector_offset, ev.y, ev.z, ev.row,
+                                 params=p, precision="float")
+    trk = make_tracker(trk_mod, gen_mod, ev, params=copy_params(p, trk_mod))
+    out = trk.tpc_track_event(ev_dict(ev, device))
+    flips, res = compare_event(trk, out, ev, ref, check_stages=False)
+    assert flips == 0
+    outer = np.stack([res[k] for k in ("trk_out_x", "trk_out_y", "trk_out_z", "trk_out_sinphi", "trk_out_tgl",
+                                       "trk_out_qpt")], axis=1)
+    err = np.abs(outer - ref.trk_out) / np.maximum(1.0, np.abs(ref.trk_out))
+    assert err.max(initial=0.0) <= TOL, err.max()
+    assert np.array_equal(res["trk_next"], ref.trk_next) and np.array_equal(res["trk_prev"], ref.trk_prev)
+    assert (res["trk_next"] >= 0).sum() >= (40 if name == "pp" else 1000)
+    trk.close()
+
+
+def test_merge_in_a_batch_and_argument_checks(trk_mod, gen_mod, oracle_mod):
+    evs = [gen_mod.generate("pp", 0), gen_mod.generate("semicentral", 0), gen_mod.generate("pp", 1)]
+    p = oracle_mod.default_params()
+    p.refit = 1; p.merge = 1
+    trk = make_tracker(trk_mod, gen_mod, evs[0], params=copy_params(p, trk_mod))
+    for device in (True, False):
+        outs = trk.tpc_track_events([ev_dict(ev, device) for ev in evs])
+        for ev, o in zip(evs, outs):
+            ref = oracle_mod.track_event(make_geometry(oracle_mod, gen_mod, ev), ev.sector_offset, ev.y, ev.z, ev.row,
+                                         params=p, precision="float")
+            res = trk.to_numpy(o)
+            assert np.array_equal(res["trk_next"], ref.trk_next) and np.array_equal(res["trk_prev"], ref.trk_prev)
+    trk.close()
+    # without refit / merge the extra outputs are absent; merge without refit is refused
+    t0 = make_tracker(trk_mod, gen_mod, evs[0])
+    r0 = t0.to_numpy(t0.tpc_track_event(ev_dict(evs[0], True)))
+    assert "trk_next" not in r0 and "trk_out_x" not in r0
+    t0.close()
+    q = copy_params(oracle_mod.default_params(), trk_mod)
+    q.merge = 1
+    with pytest.raises(trk_mod.TpcError):
+        make_tracker(trk_mod, gen_mod, evs[0], params=q)
+    # a single-sector geometry has no neighbours: no links
+    ev1 = gen_mod.generate("single_sector")
+    t1 = make_tracker(trk_mod, gen_mod, ev1, params=copy_params(p, trk_mod))
+    r1 = t1.to_numpy(t1.tpc_track_event(ev_dict(ev1, True)))
+    assert np.all(r1["trk_next"] == -1) and np.all(r1["trk_prev"] == -1)
+    t1.close()
