@@ -182,6 +182,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--link-step", type=int, default=1, choices=[1, 2], help="neighbour rows r +- step (SURVEY.md 8(f).4)")
+    ap.add_argument("--merge", action="store_true", help="also link segments across sector borders (O9, SURVEY.md 8(f).2; implies --refit)")
     ap.add_argument("--refit", action="store_true", help="also refit the output tracks (O8, SURVEY.md 8(f).1; not part of the headline path)")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
@@ -207,9 +208,11 @@ def main():
     n_total = sum(ev.n_clusters for ev in evs)
     rx = gen.row_x().astype(np.float32)
     params = None
+    args.refit = args.refit or args.merge
     if args.refit or args.link_step != 1:
         params = tracker.tpc_default_params()
         params.refit = int(args.refit)
+        params.merge = int(args.merge)
         params.link_step = args.link_step
     trk = tracker.Tracker(evs[0].n_sectors, rx, gen.TAN_HALF_ANGLE, evs[0].sigma, evs[0].sigma, evs[0].bz,
                           params=params, max_events=len(evs), max_clusters=n_total)

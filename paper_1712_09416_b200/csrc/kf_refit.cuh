@@ -91,6 +91,7 @@ __global__ void __launch_bounds__(kRfThreads, kRfBlocksPerSM) k_refit(const View
                 v.o_y[ti] = p0; v.o_z[ti] = p1; v.o_sinphi[ti] = p2; v.o_tgl[ti] = p3; v.o_qpt[ti] = p4; v.o_chi2[ti] = p5;
                 v.o_ndf[ti] = 2 * nfit - 5;
                 v.trk_rows[ti] = rref | (rtop << 8);
+                if (c.p.merge) atomicAdd(&v.dn_count[v.trk_task[ti] * c.n_rows + rref], 1);   // O9: lists by (task, first row)
                 ph = 0;
             }
         }

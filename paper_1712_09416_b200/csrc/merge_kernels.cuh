@@ -5,8 +5,8 @@
 // same side whose first fitted row r_B obeys 1 <= r_B - r_A <= 1 + max_gap.  A's outer state is turned into B's
 // frame, moved along its helix to x = row_x[r_B] (state only, the transport formulas of DESIGN.md "O5") and
 // compared with B's parameters there.  next(A) = arg min_B D, prev(B) = arg min_A D, ties -> lowest track index;
-// a link is kept when mutual.  One thread per track; the tracks of a sector task are contiguous (canonical order),
-// so the threads of a warp walk the same candidate ranges and their loads are broadcasts.
+// a link is kept when mutual.  The refitted tracks are listed by (sector task, first fitted row) -- counted by K7,
+// scanned, scattered -- so that a segment meets only the few candidates in the 1 + max_gap rows above its outer row.
 #pragma once
 #include "common.cuh"
 
@@ -48,57 +48,71 @@ __device__ __forceinline__ bool merge_score(const View& v, const Const& c, int a
     return true;
 }
 
-// first track of sector task `task` (tracks are ordered by task)
-__device__ __forceinline__ int task_track0(const View& v, int task, int nr, int S) {
-    return v.trk_scan[min(v.seed_start[task * nr], S)];
-}
+constexpr unsigned long long kNoLink = ~0ull;
 
-// NEXT: thread a looks for its best continuation b;  !NEXT: thread b looks for its best predecessor a
-template <bool NEXT>
-__global__ void __launch_bounds__(128) k_merge_best(const View v, const __grid_constant__ Const c, int32_t* best) {
-    const int T = (int)v.cnt[CNT_TRACKS];
-    const int me = blockIdx.x * 128 + threadIdx.x;
-    if (me >= T) return;
-    int res = -1;
-    const int rows_me = v.trk_rows[me];
-    const int ns = c.n_sectors, nr = c.n_rows, half = ns >> 1;
-    if (rows_me >= 0 && ns >= 4 && !(ns & 1)) {
-        const int S = min(v.seed_start[v.n_bins], v.S_cap);
-        const int task = v.trk_task[me];
-        const int ev = task / ns, s = task - ev * ns, side = s / half, k = s - side * half;
-        const int k_lo = (k + half - 1) % half, k_hi = (k + 1) % half;   // the sectors before / after mine
-        // candidate ranges in ascending track order (a strict < then keeps the lowest index on ties)
-        int kk[2] = {min(k_lo, k_hi), max(k_lo, k_hi)};
-        float bd = 0.f;
-        for (int j = 0; j < 2; j++) {
-            if (j == 1 && kk[1] == kk[0]) break;   // half == 2: one neighbour only
-            const int other = ev * ns + side * half + kk[j];
-            // the other sector is "next" of mine when it follows mine in azimuth
-            const bool other_is_next = kk[j] == k_hi, other_is_prev = kk[j] == k_lo;
-            const int t0 = task_track0(v, other, nr, S), t1 = task_track0(v, other + 1, nr, S);
-            for (int o = t0; o < t1; o++) {
-                const int rows_o = v.trk_rows[o];
-                if (rows_o < 0) continue;
-                float D;
-                const bool ok = NEXT ? merge_score(v, c, me, o, rows_me, rows_o, other_is_next, D)
-                                     : merge_score(v, c, o, me, rows_o, rows_me, other_is_prev, D);
-                if (ok && (res < 0 || D < bd)) { res = o; bd = D; }
-            }
-        }
-    }
-    best[me] = res;
-}
-
-// keep the mutual links; indices become event-local
-__global__ void __launch_bounds__(128) k_merge_mutual(const View v, const __grid_constant__ Const c, const int32_t* nx, const int32_t* pv) {
+// tracks with a refit -> lists by (task, first fitted row); dn_count was filled by k_refit, dn_start is its scan
+__global__ void __launch_bounds__(128) k_merge_scatter(const View v, int nr, int32_t* list, unsigned long long* pvkey) {
     const int T = (int)v.cnt[CNT_TRACKS];
     const int a = blockIdx.x * 128 + threadIdx.x;
     if (a >= T) return;
-    const int e = v.trk_task[a] / c.n_sectors;
-    const int e0 = v.ev_off[e];
-    const int b = nx[a], p = pv[a];
-    v.o_next[a] = (b >= 0 && pv[b] == a) ? b - e0 : -1;
-    v.o_prev[a] = (p >= 0 && nx[p] == a) ? p - e0 : -1;
+    pvkey[a] = kNoLink;
+    const int rows = v.trk_rows[a];
+    if (rows < 0) return;
+    const int bin = v.trk_task[a] * nr + (rows & 0xff);
+    list[v.dn_start[bin] + atomicAdd(&v.dn_fill[bin], 1)] = a;
+}
+
+// One thread per segment a: the candidates b are the segments of the two neighbouring sectors whose first fitted
+// row lies 1 .. 1 + max_gap rows above a's outer row (taken from the (task, row) lists).  Every candidate pair is
+// scored once: it competes for next(a) in a register and for prev(b) with an atomicMin.  Keys are
+// (bits of D) << 32 | track index: D >= +0, so the order of the keys is the order of (D, index) -- the lowest index
+// wins a tie, as the reference's ascending loops do.
+__global__ void __launch_bounds__(128) k_merge_pairs(const View v, const __grid_constant__ Const c, const int32_t* list,
+                                                     unsigned long long* nxkey, unsigned long long* pvkey) {
+    const int T = (int)v.cnt[CNT_TRACKS];
+    const int a = blockIdx.x * 128 + threadIdx.x;
+    if (a >= T) return;
+    unsigned long long best = kNoLink;
+    const int rows_a = v.trk_rows[a];
+    const int ns = c.n_sectors, nr = c.n_rows, half = ns >> 1;
+    if (rows_a >= 0 && ns >= 4 && !(ns & 1)) {
+        const int task = v.trk_task[a];
+        const int ev = task / ns, s = task - ev * ns, side = s / half, k = s - side * half;
+        const int k_lo = (k + half - 1) % half, k_hi = (k + 1) % half;   // the sectors before / after a's
+        const int r_out = (rows_a >> 8) & 0xff;
+        const int r0 = r_out + 1, r1 = min(r_out + 1 + c.p.merge_max_gap, nr - 1);
+        for (int j = 0; j < 2; j++) {
+            if (j == 1 && k_hi == k_lo) break;   // two sectors per side: one neighbour
+            const int kb = j == 0 ? k_hi : k_lo;
+            const int other = ev * ns + side * half + kb;
+            if (r0 > r1) break;
+            const int p0 = v.dn_start[other * nr + r0], p1 = v.dn_start[other * nr + r1 + 1];
+            for (int p = p0; p < p1; p++) {
+                const int b = list[p];
+                float D;
+                if (!merge_score(v, c, a, b, rows_a, v.trk_rows[b], kb == k_hi, D)) continue;
+                const unsigned long long d = (unsigned long long)__float_as_uint(D) << 32;
+                best = min(best, d | (unsigned)b);
+                atomicMin(&pvkey[b], d | (unsigned)a);
+            }
+        }
+    }
+    nxkey[a] = best;
+}
+
+// keep the mutual links; indices become event-local
+__global__ void __launch_bounds__(128) k_merge_mutual(const View v, const __grid_constant__ Const c, const unsigned long long* nxkey,
+                                                      const unsigned long long* pvkey) {
+    const int T = (int)v.cnt[CNT_TRACKS];
+    const int a = blockIdx.x * 128 + threadIdx.x;
+    if (a >= T) return;
+    const int e0 = v.ev_off[v.trk_task[a] / c.n_sectors];
+    const unsigned long long kn = nxkey[a], kp = pvkey[a];
+    const int b = kn == kNoLink ? -1 : (int)(kn & 0xffffffffu), p = kp == kNoLink ? -1 : (int)(kp & 0xffffffffu);
+    const bool fwd = b >= 0 && pvkey[b] != kNoLink && (int)(pvkey[b] & 0xffffffffu) == a;
+    const bool bwd = p >= 0 && nxkey[p] != kNoLink && (int)(nxkey[p] & 0xffffffffu) == a;
+    v.o_next[a] = fwd ? b - e0 : -1;
+    v.o_prev[a] = bwd ? p - e0 : -1;
 }
 
 }  // namespace tpc

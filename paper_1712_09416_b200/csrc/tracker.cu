@@ -83,7 +83,8 @@ struct Batch {
     Buf<float2> thit, shit;
     Buf<int32_t> in_row, sec_off, bin_count, bin_start, tidx, sorig, link_up, link_dn, clink_up, clink_dn, seed_count,
         seed_start, seeds, seed_bin, tl_rows, tl_nown, tl_keep, trk_scan, hit_scan, ev_off_d, scratch,
-        o_i[kOutI], o_hit, trk_rows, trk_task, mg_next, mg_prev;
+        o_i[kOutI], o_hit, trk_rows, trk_task, mg_list;
+    Buf<unsigned long long> mg_next, mg_prev;
     Buf<uint16_t> slot, cells, tl_tab;
     Buf<float2> o_hit_yz;
     Buf<uint8_t> o_hit_row;
@@ -118,7 +119,7 @@ struct Batch {
         scratch.release(); o_hit.release();
         for (auto& b : o_i) b.release();
         slot.release(); cells.release(); desc.release(); owner.release(); ev_src.release();
-        seed_rec.release(); tl_up.release(); dn_rec.release(); dn_count.release(); dn_start.release(); dn_fill.release(); tl_cnt.release(); o_hit_yz.release(); o_hit_row.release(); trk_hit0.release(); trk_rows.release(); trk_task.release(); mg_next.release(); mg_prev.release();
+        seed_rec.release(); tl_up.release(); dn_rec.release(); dn_count.release(); dn_start.release(); dn_fill.release(); tl_cnt.release(); o_hit_yz.release(); o_hit_row.release(); trk_hit0.release(); trk_rows.release(); trk_task.release(); mg_next.release(); mg_prev.release(); mg_list.release();
         cnt.release(); kf_cursor.release(); h_ev_src.release(); h_sec_off.release(); h_ev_off.release(); h_cnt.release(); h_nseeds.release();
         for (auto& e : evt) if (e) { cudaEventDestroy(e); e = nullptr; }
     }
@@ -188,7 +189,7 @@ int reserve_batch(const tpc_tracker* tr, Batch* t, int n_events, int64_t N, int6
     for (int k = 0; k < kOutI; k++) RS(o_i[k], S_cap);
     for (int k = 0; k < kOutF; k++) RS(o_f[k], S_cap);
     if (tr->c.p.refit) { RS(trk_rows, S_cap); RS(trk_task, S_cap); }
-    if (tr->c.p.merge) { RS(mg_next, S_cap); RS(mg_prev, S_cap); }
+    if (tr->c.p.merge) { RS(mg_next, S_cap); RS(mg_prev, S_cap); RS(mg_list, S_cap); }
     RS(o_hit, n);
     if (tr->c.p.refit) { RS(o_hit_yz, n); RS(o_hit_row, n); RS(trk_hit0, S_cap); }
 #undef RS
@@ -271,11 +272,16 @@ int launch_all(const tpc_tracker* tr, Batch* t) {
     k_event_offsets<<<(t->n_events + 1 + 63) / 64, 64, 0, st>>>(v, ns * nr); L++;
     k_select_write<<<sel_grid, kSelCtaThreads, kSelCap * sizeof(uint32_t), st>>>(v, c); L++;
     mark(5);
+    if (c.p.merge) {   // the (task, row) counters of the down sweep are free again: K7 counts the refitted tracks there
+        CK(cudaMemsetAsync(v.dn_count, 0, sizeof(int32_t) * (nb + 1), st));
+        CK(cudaMemsetAsync(v.dn_fill, 0, sizeof(int32_t) * (nb + 1), st));
+    }
     if (c.p.refit) { k_refit<<<tr->rf_blocks, kRfThreads, 0, st>>>(v, c); L++; }
     if (c.p.merge) {   // the track count is on the device: grids cover the start-hit capacity
         const int g = (int)((t->S_cap + 127) / 128);
-        k_merge_best<true><<<g, 128, 0, st>>>(v, c, t->mg_next.p); L++;
-        k_merge_best<false><<<g, 128, 0, st>>>(v, c, t->mg_prev.p); L++;
+        L += scan_exclusive(v.dn_count, v.dn_start, nb, t->scratch.p, st);
+        k_merge_scatter<<<g, 128, 0, st>>>(v, nr, t->mg_list.p, t->mg_prev.p); L++;
+        k_merge_pairs<<<g, 128, 0, st>>>(v, c, t->mg_list.p, t->mg_next.p, t->mg_prev.p); L++;
         k_merge_mutual<<<g, 128, 0, st>>>(v, c, t->mg_next.p, t->mg_prev.p); L++;
     }
     mark(6);
