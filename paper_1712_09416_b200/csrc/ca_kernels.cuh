@@ -202,10 +202,16 @@ __global__ void __launch_bounds__(kSortThreads) k_sort_row(const View v) {
 // ties -> lowest caller's index of u, then of d.
 // ---------------------------------------------------------------------------------------------------------
 constexpr int kNfThreads = 128;
-constexpr int kNfCap = 1024;   // hits of a neighbour row held in shared memory; larger rows are read in place
+#ifndef TPC_NF_CAP
+#define TPC_NF_CAP 640
+#endif
+#ifndef TPC_NF_BLOCKS
+#define TPC_NF_BLOCKS 12
+#endif
+constexpr int kNfCap = TPC_NF_CAP;   // hits of a neighbour row held in shared memory; larger rows are read in place
 constexpr int kNfList = 8;     // down-candidates remembered per hit; more -> nested walk
 
-__global__ void __launch_bounds__(kNfThreads) k_neighbours(const View v, const __grid_constant__ Const c) {
+__global__ void __launch_bounds__(kNfThreads, TPC_NF_BLOCKS) k_neighbours(const View v, const __grid_constant__ Const c) {
     __shared__ float2 s_hu[kNfCap], s_hd[kNfCap];
     constexpr int kNfCells = kCellsPerHit * kNfCap + kCellPad;   // cell-table entries held in shared memory
     __shared__ uint16_t s_cu[kNfCells], s_cd[kNfCells];
