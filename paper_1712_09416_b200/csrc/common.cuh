@@ -9,7 +9,7 @@
 namespace tpc {
 
 #ifndef TPC_CELLS_PER_HIT
-#define TPC_CELLS_PER_HIT 2
+#define TPC_CELLS_PER_HIT 3
 #endif
 constexpr int kCellsPerHit = TPC_CELLS_PER_HIT;       // grid cells per hit of a bin (the cells are this much finer in y than in z)
 constexpr int kCellPad = 32;          // cell table of a bin holds up to kCellsPerHit * n_hits + kCellPad entries

@@ -32,7 +32,7 @@ namespace tpc {
 #define TPC_SW_CSLEEP 100
 #endif
 #ifndef TPC_SW_SLOTS
-#define TPC_SW_SLOTS 4
+#define TPC_SW_SLOTS 2
 #endif
 constexpr int kSwWarps = TPC_SW_WARPS;                 // consumer warps of a CTA (one more warp produces)
 constexpr int kSwThreads = (kSwWarps + 1) * 32;
