@@ -197,6 +197,20 @@ int reserve_batch(const tpc_tracker* tr, Batch* t, int n_events, int64_t N, int6
     return TPC_OK;
 }
 
+// CTAs that share the start hits of one sector task in K5.  A unit of work (task, share) costs about
+// (1/K + 0.075) of a whole task -- every share sweeps all pad rows -- and the units run in waves of `slots`
+// resident CTAs; K minimises waves x unit cost (measured on 1..24 central events).
+int sweepers_per_task(int n_tasks, int slots) {
+    int best = 1;
+    double best_cost = 1e30;
+    for (int K = 1; K <= 32; K++) {
+        const int64_t units = (int64_t)std::max(n_tasks, 1) * K;
+        const double cost = (double)((units + slots - 1) / slots) * (1.0 / K + 0.075);
+        if (cost < best_cost - 1e-12) { best_cost = cost; best = K; }
+    }
+    return best;
+}
+
 int64_t default_seed_cap(int64_t N) { return std::max<int64_t>(N / 8 + 4096, 4096); }
 
 int validate(const tpc_tracker* t, int n, const tpc_event_in* in) {
@@ -362,7 +376,7 @@ int batch_begin(const tpc_tracker* tr, Batch* t, int first_event, int n, const t
     v.o_hit_yz = t->o_hit_yz.p; v.o_hit_row = t->o_hit_row.p; v.trk_hit0 = t->trk_hit0.p;
     v.seed_rec = t->seed_rec.p; v.tl_up = t->tl_up.p; v.dn_rec = t->dn_rec.p;
     v.dn_count = t->dn_count.p; v.dn_start = t->dn_start.p; v.dn_fill = t->dn_fill.p;
-    v.kf_K = tr->sweepers > 0 ? tr->sweepers : std::max(1, (tr->sw_blocks + v.n_tasks / 2) / std::max(v.n_tasks, 1));
+    v.kf_K = tr->sweepers > 0 ? tr->sweepers : sweepers_per_task(v.n_tasks, tr->sw_blocks);
     t->n_events = n; t->N = N;
     if (tr->profiling)
         for (auto& e : t->evt)
