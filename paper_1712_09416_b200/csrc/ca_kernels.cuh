@@ -104,7 +104,10 @@ __global__ void __launch_bounds__(256) k_scatter(const View v, int ns, int nr) {
 // The grid only accelerates the window searches; windows are defined on coordinates and every tie is broken
 // on the caller's index, so neither the grid's shape nor the order inside a cell changes a result.
 // ---------------------------------------------------------------------------------------------------------
-constexpr int kSortThreads = 128;
+#ifndef TPC_SORT_THREADS
+#define TPC_SORT_THREADS 128
+#endif
+constexpr int kSortThreads = TPC_SORT_THREADS;
 
 __global__ void __launch_bounds__(kSortThreads) k_sort_row(const View v) {
     __shared__ int cnt[kMaxCells + 1];                    // hits per cell, then first hit of each cell
