@@ -345,3 +345,28 @@ def test_merge_in_a_batch_and_argument_checks(trk_mod, gen_mod, oracle_mod):
     r1 = t1.to_numpy(t1.tpc_track_event(ev_dict(ev1, True)))
     assert np.all(r1["trk_next"] == -1) and np.all(r1["trk_prev"] == -1)
     t1.close()
+
+
+def test_parity_config5_in_the_bench_configuration(trk_mod, gen_mod, oracle_mod):
+    """BASELINE.json config 5 at full size (16 central events, 29.7 M clusters) launched as bench.py launches it
+    (one call, device-resident inputs, work space reserved at create): three sampled events compared with the oracle
+    output by output, and counts that hold for the whole batch."""
+    import bench
+    evs = bench.make_events("central", 16)
+    n_total = sum(ev.n_clusters for ev in evs)
+    trk = trk_mod.Tracker(evs[0].n_sectors, gen_mod.row_x().astype(np.float32), gen_mod.TAN_HALF_ANGLE, evs[0].sigma,
+                          evs[0].sigma, evs[0].bz, max_events=len(evs), max_clusters=n_total)
+    outs = trk.tpc_track_events([ev_dict(ev, True) for ev in evs])
+    c = trk.tpc_get_counters()
+    assert c["n_events"] == 16 and c["n_clusters"] == n_total and c["n_retries"] == 0
+    assert c["n_tracks"] == sum(o.n_tracks for o in outs) and c["n_track_hits"] == sum(o.n_track_hits for o in outs)
+    for e in (0, 7, 15):
+        ev = evs[e]
+        ref = oracle_mod.track_event(make_geometry(oracle_mod, gen_mod, ev), ev.sector_offset, ev.y, ev.z, ev.row,
+                                     precision="float")
+        flips, res = compare_event(trk, outs[e], ev, ref, event=e)
+        assert flips == 0
+    for o in outs:   # every event: a hit is in at most one track
+        h = trk.to_numpy(o)["hit_idx"]
+        assert np.unique(h).size == h.size
+    trk.close()
