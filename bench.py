@@ -160,7 +160,9 @@ def run_reference(args, rank, world):
         "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
         "vs_baseline": None, "dtype": "f32", "data": "synthetic",
-        "config": {"workload": "1 central Pb-Pb-like event per step (BASELINE.json config 4 recipe), CPU oracle"},
+        "config": {"workload": "%d x central Pb-Pb-like events per step (BASELINE.json config 5 = 16 x config 4)" % args.events
+                               if args.workload == "central" else "%d x %s event(s) per step" % (args.events, args.workload),
+                   "sample": "each step of this arm is ONE event of that batch (bounded sample), CPU oracle"},
         "clusters_per_s": ncl / dt,
         "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle",
                          "sample": "%d steps x 1 event (~%d clusters each), strict-float32 mode, OpenMP over sectors"
