@@ -22,7 +22,7 @@ constexpr unsigned kFull = 0xffffffffu;
 constexpr unsigned kErrBadRow = 1u, kErrRowCapacity = 2u, kErrSeedCapacity = 4u, kErrHang = 8u, kErrSelCapacity = 16u;
 
 // device counters (unsigned long long each)
-constexpr int kMaxSM = 256;
+constexpr int kNCursors = 4;           // work cursors: up sweep, down sweep, refit
 enum { CNT_ERR = 0, CNT_LINKS, CNT_ROW_VISITS, CNT_TL_HITS, CNT_TRACKS, CNT_TRACK_HITS, CNT_UPDATES, CNT_REFIT_VISITS, CNT_N };
 
 // One event's input arrays (device pointers) and its place in the batch-global cluster numbering.
@@ -103,7 +103,7 @@ struct View {
     float *o_xo, *o_yo, *o_zo, *o_so, *o_to, *o_qo;   // [S_cap] outer state of the refit (up pass at its top hit)
     int32_t *o_next, *o_prev;   // [S_cap] O9 links, event-local track index or -1
     unsigned long long* cnt; // [CNT_N]
-    unsigned long long* kf_cursor;  // [n_events * kMaxSM] K5: start hits handed out per (event, SM) share
+    unsigned long long* kf_cursor;  // [kNCursors] units of work handed out: [0] up sweep, [1] down sweep, [2] refit
 };
 
 __device__ __forceinline__ int lane_id() { return threadIdx.x & 31; }

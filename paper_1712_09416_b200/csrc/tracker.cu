@@ -185,7 +185,7 @@ int reserve_batch(const tpc_tracker* tr, Batch* t, int n_events, int64_t N, int6
     RS(tl_nown, S_cap + 1); RS(tl_keep, S_cap + 1); RS(tl_cnt, (size_t)t->sel_C * S_cap); RS(trk_scan, S_cap + 2); RS(hit_scan, S_cap + 2);
     RS(ev_off_d, 2 * ((size_t)n_events + 1)); RS(h_ev_off, 2 * ((size_t)n_events + 1));
     RS(scratch, (size_t)std::max<int64_t>(nb, S_cap) / kScanTile + 8);
-    RS(cnt, CNT_N); RS(h_cnt, CNT_N); RS(kf_cursor, (size_t)n_events * kMaxSM); RS(h_nseeds, 1);
+    RS(cnt, CNT_N); RS(h_cnt, CNT_N); RS(kf_cursor, kNCursors); RS(h_nseeds, 1);
     for (int k = 0; k < kOutI; k++) RS(o_i[k], S_cap);
     for (int k = 0; k < kOutF; k++) RS(o_f[k], S_cap);
     if (tr->c.p.refit) { RS(trk_rows, S_cap); RS(trk_task, S_cap); }
@@ -244,7 +244,7 @@ int launch_all(const tpc_tracker* tr, Batch* t) {
     int64_t L = 0;
     CK(cudaMemsetAsync(v.bin_count, 0, sizeof(int32_t) * (nb + 1), st));
     CK(cudaMemsetAsync(v.cnt, 0, sizeof(unsigned long long) * CNT_N, st));
-    CK(cudaMemsetAsync(v.kf_cursor, 0, sizeof(unsigned long long) * (size_t)v.n_events * kMaxSM, st));
+    CK(cudaMemsetAsync(v.kf_cursor, 0, sizeof(unsigned long long) * kNCursors, st));
     auto mark = [&](int k) { if (tr->profiling) cudaEventRecord(t->evt[k], st); };
     mark(0);
     int maxn = 0;
@@ -528,7 +528,6 @@ tpc_tracker* tpc_tracker_create_ex(const tpc_geometry* g, float bz, const tpc_pa
     }
     if (g->sector_alpha) t->sector_alpha.assign(g->sector_alpha, g->sector_alpha + g->n_sectors);
     cudaDeviceGetAttribute(&t->sm_count, cudaDevAttrMultiProcessorCount, dev);
-    if (t->sm_count > kMaxSM) { set_err("more than %d SMs", kMaxSM); delete t; return nullptr; }
     {   // persistent constructor grid: as many CTAs as are resident at once
         int per_sm = 0;
         if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_sweep<true>, kSwThreads, 0) != cudaSuccess || per_sm < 1) {
