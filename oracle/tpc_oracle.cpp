@@ -113,7 +113,7 @@ struct Result {
     std::vector<double> trk_x, trk_y, trk_z, trk_sinphi, trk_tgl, trk_qpt, trk_chi2, trk_margin;
     std::vector<int32_t> hit_idx;
     /* O8 outer state (up pass of the refit, at its top hit) and O9 links */
-    std::vector<int32_t> trk_row_out, trk_next, trk_prev;
+    std::vector<int32_t> trk_row_out, trk_next, trk_prev, trk_global; /* global: first segment of the chain */
     std::vector<double> trk_out; /* [T][6] x y z sin phi tg lambda q/pT */
 };
 
@@ -458,6 +458,8 @@ template <class R>
 void merge_segments(const oracle_geometry& G, const oracle_params& P, Result& res) {
     const int T = (int)res.trk_sector.size();
     res.trk_next.assign(T, -1); res.trk_prev.assign(T, -1);
+    res.trk_global.resize(T);
+    for (int a = 0; a < T; a++) res.trk_global[a] = a;
     if (G.n_sectors < 4 || (G.n_sectors & 1)) return;
     const int half = G.n_sectors / 2;
     const double step = 2.0 * 3.14159265358979323846 / (double)half;
@@ -519,6 +521,13 @@ void merge_segments(const oracle_geometry& G, const oracle_params& P, Result& re
         }
     for (int a = 0; a < T; a++)
         if (nx[a] >= 0 && pv[nx[a]] == a) { res.trk_next[a] = nx[a]; res.trk_prev[nx[a]] = a; }
+    /* global track = chain of linked segments, named by its first segment (links join a sector to the next one
+       outwards in row, so a chain cannot close on itself) */
+    for (int a = 0; a < T; a++) {
+        int h = a;
+        while (res.trk_prev[h] >= 0) h = res.trk_prev[h];
+        res.trk_global[a] = h;
+    }
 }
 
 template <class R>
@@ -620,7 +629,11 @@ Result* run(const oracle_geometry& G, const oracle_params& P, int32_t n, const i
         }
     }
     if (P.merge && P.refit && stop_after == 0) merge_segments<R>(G, P, *res);
-    else { res->trk_next.assign(res->trk_sector.size(), -1); res->trk_prev.assign(res->trk_sector.size(), -1); }
+    else {
+        const size_t T = res->trk_sector.size();
+        res->trk_next.assign(T, -1); res->trk_prev.assign(T, -1); res->trk_global.resize(T);
+        for (size_t a = 0; a < T; a++) res->trk_global[a] = (int32_t)a;
+    }
     return res;
 }
 
@@ -672,7 +685,7 @@ enum {
     F_LINK_UP = 0, F_LINK_DN, F_CLINK_UP, F_CLINK_DN, F_NF_MARGIN, F_SEED_OFFSET, F_START_HIT,
     F_TL_FIRST_ROW, F_TL_LAST_ROW, F_TL_N_HITS, F_TL_PAR, F_TL_CHI2, F_TL_MARGIN, F_TL_TABLE,
     F_TRK_SECTOR, F_TRK_FIRST_HIT, F_TRK_N_HITS, F_TRK_NDF, F_TRK_SEED, F_TRK_FIRST_ROW,
-    F_TRK_X, F_TRK_Y, F_TRK_Z, F_TRK_SINPHI, F_TRK_TGL, F_TRK_QPT, F_TRK_CHI2, F_TRK_MARGIN, F_HIT_IDX, F_TL_COV, F_TRK_ROW_OUT, F_TRK_OUT, F_TRK_NEXT, F_TRK_PREV
+    F_TRK_X, F_TRK_Y, F_TRK_Z, F_TRK_SINPHI, F_TRK_TGL, F_TRK_QPT, F_TRK_CHI2, F_TRK_MARGIN, F_HIT_IDX, F_TL_COV, F_TRK_ROW_OUT, F_TRK_OUT, F_TRK_NEXT, F_TRK_PREV, F_TRK_GLOBAL
 };
 
 /* copy one result field into caller memory (int32 or float64, shapes in oracle/__init__.py) */
@@ -718,6 +731,7 @@ int32_t oracle_copy(const void* rv, int32_t field, void* dst) {
         case F_TRK_OUT: copy_out(r->trk_out, dst); break;
         case F_TRK_NEXT: copy_out(r->trk_next, dst); break;
         case F_TRK_PREV: copy_out(r->trk_prev, dst); break;
+        case F_TRK_GLOBAL: copy_out(r->trk_global, dst); break;
         default: return -1;
     }
     return 0;

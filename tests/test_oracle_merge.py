@@ -120,3 +120,25 @@ def test_merge_links_agree_with_exact_helix_geometry(oracle_mod, gen_mod):
         assert abs(s2 - r.trk_sinphi[b]) <= p.merge_ds * (1 + 1e-6) and abs(to - r.trk_tgl[b]) <= p.merge_dt * (1 + 1e-6)
         n += 1
     assert n > 1000
+
+
+def test_global_tracks_are_the_chains_of_links(oracle_mod, gen_mod):
+    """trk_global names every segment's chain by its first segment: heads have no predecessor, a link never joins
+    two chains, chains grow outwards, and (truth) the segments of a chain belong to one particle."""
+    ev, p, r = _run(oracle_mod, gen_mod, "semicentral")
+    g, nx, pv = r.trk_global, r.trk_next, r.trk_prev
+    T = r.n_tracks
+    assert np.all(pv[g] == -1) and np.all(g[g] == g)
+    assert np.array_equal(g[pv >= 0], g[pv[pv >= 0]])            # a segment and its predecessor: same chain
+    assert np.all(g[pv < 0] == np.nonzero(pv < 0)[0])            # heads name themselves
+    a = np.nonzero(nx >= 0)[0]
+    assert np.all(r.trk_first_row[nx[a]] > r.trk_row_out[a])     # outwards
+    sizes = np.bincount(g, minlength=T)
+    assert sizes.max() >= 2 and sizes.max() <= ev.n_sectors // 2
+    lab, pur = _labels(ev, r)
+    multi = np.nonzero(sizes >= 2)[0]
+    same = [np.unique(lab[g == h]).size == 1 for h in multi[:400]]
+    assert np.mean(same) > 0.995
+    # merge off: every track is its own global track
+    ev2, p2, r2 = _run(oracle_mod, gen_mod, "pp", merge=0)
+    assert np.array_equal(r2.trk_global, np.arange(r2.n_tracks))
