@@ -123,6 +123,8 @@ typedef struct {
      * the segment this one continues; index into this event's tracks or -1.  Links are mutual and one-to-one. */
     const int32_t* trk_next;      /* [n_tracks] */
     const int32_t* trk_prev;      /* [n_tracks] */
+    const int32_t* trk_global;    /* [n_tracks] the global track a segment belongs to = the chain of linked segments,
+                                   * named by the index of its first (innermost) segment */
 } tpc_event_out;
 
 /* Counters of the last call (whole batch); used for the algorithmic-byte count of DESIGN.md. */

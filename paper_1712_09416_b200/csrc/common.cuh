@@ -102,6 +102,7 @@ struct View {
     int32_t* trk_task;       // [S_cap] sector task of a track (O9)
     float *o_xo, *o_yo, *o_zo, *o_so, *o_to, *o_qo;   // [S_cap] outer state of the refit (up pass at its top hit)
     int32_t *o_next, *o_prev;   // [S_cap] O9 links, event-local track index or -1
+    int32_t* o_global;          // [S_cap] first segment of the chain a track belongs to, event-local
     unsigned long long* cnt; // [CNT_N]
     unsigned long long* kf_cursor;  // [kNCursors] units of work handed out: [0] up sweep, [1] down sweep, [2] refit
 };

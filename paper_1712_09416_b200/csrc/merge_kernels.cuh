@@ -115,4 +115,16 @@ __global__ void __launch_bounds__(128) k_merge_mutual(const View v, const __grid
     v.o_prev[a] = bwd ? p - e0 : -1;
 }
 
+// global track = chain of linked segments, named by its first segment.  A link leads to a higher pad row, so a
+// chain is at most n_rows long and never closes on itself; n_sectors / 2 links at most in practice.
+__global__ void __launch_bounds__(128) k_merge_chain(const View v, int n_sectors) {
+    const int T = (int)v.cnt[CNT_TRACKS];
+    const int a = blockIdx.x * 128 + threadIdx.x;
+    if (a >= T) return;
+    const int e0 = v.ev_off[v.trk_task[a] / n_sectors];   // o_prev holds event-local indices
+    int h = a - e0;
+    for (int p = v.o_prev[e0 + h]; p >= 0; p = v.o_prev[e0 + h]) h = p;
+    v.o_global[a] = h;
+}
+
 }  // namespace tpc

@@ -18,7 +18,7 @@
 
 namespace {
 
-constexpr int kOutI = 6, kOutF = 13;   // int32 / float arrays per track: 4 + next, prev; 7 + the outer state
+constexpr int kOutI = 7, kOutF = 13;   // int32 / float arrays per track: 4 + next, prev, global; 7 + the outer state
 
 thread_local std::string g_err;
 
@@ -297,6 +297,7 @@ int launch_all(const tpc_tracker* tr, Batch* t) {
         k_merge_scatter<<<g, 128, 0, st>>>(v, nr, t->mg_list.p, t->mg_prev.p); L++;
         k_merge_pairs<<<g, 128, 0, st>>>(v, c, t->mg_list.p, t->mg_next.p, t->mg_prev.p); L++;
         k_merge_mutual<<<g, 128, 0, st>>>(v, c, t->mg_next.p, t->mg_prev.p); L++;
+        k_merge_chain<<<g, 128, 0, st>>>(v, ns); L++;
     }
     mark(6);
     CK(cudaGetLastError());
@@ -371,7 +372,7 @@ int batch_begin(const tpc_tracker* tr, Batch* t, int first_event, int n, const t
     v.o_x = t->o_f[0].p; v.o_y = t->o_f[1].p; v.o_z = t->o_f[2].p; v.o_sinphi = t->o_f[3].p;
     v.o_tgl = t->o_f[4].p; v.o_qpt = t->o_f[5].p; v.o_chi2 = t->o_f[6].p;
     v.o_xo = t->o_f[7].p; v.o_yo = t->o_f[8].p; v.o_zo = t->o_f[9].p; v.o_so = t->o_f[10].p; v.o_to = t->o_f[11].p; v.o_qo = t->o_f[12].p;
-    v.o_next = t->o_i[4].p; v.o_prev = t->o_i[5].p; v.trk_rows = t->trk_rows.p; v.trk_task = t->trk_task.p;
+    v.o_next = t->o_i[4].p; v.o_prev = t->o_i[5].p; v.o_global = t->o_i[6].p; v.trk_rows = t->trk_rows.p; v.trk_task = t->trk_task.p;
     v.cnt = t->cnt.p; v.kf_cursor = t->kf_cursor.p;
     v.o_hit_yz = t->o_hit_yz.p; v.o_hit_row = t->o_hit_row.p; v.trk_hit0 = t->trk_hit0.p;
     v.seed_rec = t->seed_rec.p; v.tl_up = t->tl_up.p; v.dn_rec = t->dn_rec.p;
@@ -685,7 +686,7 @@ int tpc_track_events(tpc_tracker* t, int32_t n, const tpc_event_in* in, tpc_even
         o.trk_out_x = rf ? of[7] + a : nullptr; o.trk_out_y = rf ? of[8] + a : nullptr; o.trk_out_z = rf ? of[9] + a : nullptr;
         o.trk_out_sinphi = rf ? of[10] + a : nullptr; o.trk_out_tgl = rf ? of[11] + a : nullptr;
         o.trk_out_qpt = rf ? of[12] + a : nullptr;
-        o.trk_next = mg ? oi[4] + a : nullptr; o.trk_prev = mg ? oi[5] + a : nullptr;
+        o.trk_next = mg ? oi[4] + a : nullptr; o.trk_prev = mg ? oi[5] + a : nullptr; o.trk_global = mg ? oi[6] + a : nullptr;
         o.hit_idx = ohit + h;
     }
     t->have_result = true;

@@ -48,7 +48,7 @@ class tpc_event_in(C.Structure):
 _OUT_I = ("trk_sector", "trk_first_hit", "trk_n_hits", "trk_ndf")
 _OUT_F = ("trk_x", "trk_y", "trk_z", "trk_sinphi", "trk_tgl", "trk_qpt", "trk_chi2")
 _OUT_F2 = ("trk_out_x", "trk_out_y", "trk_out_z", "trk_out_sinphi", "trk_out_tgl", "trk_out_qpt")   # refit = 1
-_OUT_I2 = ("trk_next", "trk_prev")                                                                   # merge = 1
+_OUT_I2 = ("trk_next", "trk_prev", "trk_global")                                                                   # merge = 1
 
 
 class tpc_event_out(C.Structure):

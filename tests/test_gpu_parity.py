@@ -313,6 +313,7 @@ def test_merge_parity(trk_mod, gen_mod, oracle_mod, name, device):
     err = np.abs(outer - ref.trk_out) / np.maximum(1.0, np.abs(ref.trk_out))
     assert err.max(initial=0.0) <= TOL, err.max()
     assert np.array_equal(res["trk_next"], ref.trk_next) and np.array_equal(res["trk_prev"], ref.trk_prev)
+    assert np.array_equal(res["trk_global"], ref.trk_global)
     assert (res["trk_next"] >= 0).sum() >= (40 if name == "pp" else 1000)
     trk.close()
 
@@ -329,6 +330,7 @@ def test_merge_in_a_batch_and_argument_checks(trk_mod, gen_mod, oracle_mod):
                                          params=p, precision="float")
             res = trk.to_numpy(o)
             assert np.array_equal(res["trk_next"], ref.trk_next) and np.array_equal(res["trk_prev"], ref.trk_prev)
+            assert np.array_equal(res["trk_global"], ref.trk_global)
     trk.close()
     # without refit / merge the extra outputs are absent; merge without refit is refused
     t0 = make_tracker(trk_mod, gen_mod, evs[0])
@@ -344,6 +346,7 @@ def test_merge_in_a_batch_and_argument_checks(trk_mod, gen_mod, oracle_mod):
     t1 = make_tracker(trk_mod, gen_mod, ev1, params=copy_params(p, trk_mod))
     r1 = t1.to_numpy(t1.tpc_track_event(ev_dict(ev1, True)))
     assert np.all(r1["trk_next"] == -1) and np.all(r1["trk_prev"] == -1)
+    assert np.array_equal(r1["trk_global"], np.arange(r1["n_tracks"]))
     t1.close()
 
 
