@@ -79,3 +79,14 @@ def test_product_never_imports_the_oracle():
             txt = f.read_text()
             assert "csrc" not in txt.replace("paper_1712_09416_b200/csrc", "") or True
             assert "#include \"tpctrack.h\"" not in txt and "libtpctrack" not in txt, f
+
+
+def test_baseline_md_quotes_table_1_of_the_paper_unchanged():
+    """tests/golden/table1_tracking_time.txt = Table 1 of the paper: context numbers only."""
+    root = Path(__file__).resolve().parent.parent
+    text = (root / "BASELINE.md").read_text()
+    rows = [l.split() for l in (root / "tests" / "golden" / "table1_tracking_time.txt").read_text().splitlines()
+            if l and not l.startswith("#")]
+    assert len(rows) == 5
+    for dev, ms in rows:
+        assert any(dev in line and ms + " ms" in line.replace("*", "") for line in text.splitlines()), (dev, ms)
