@@ -373,3 +373,23 @@ def test_parity_config5_in_the_bench_configuration(trk_mod, gen_mod, oracle_mod)
         h = trk.to_numpy(o)["hit_idx"]
         assert np.unique(h).size == h.size
     trk.close()
+
+
+@pytest.mark.parametrize("n_tracks,refit", [(800, 0), (1300, 1)])
+def test_parity_rows_larger_than_the_shared_memory_stages(trk_mod, gen_mod, oracle_mod, n_tracks, refit):
+    """Pad rows of 500-1500 clusters: more than the neighbour finder (640) and the sweep constructor (640) stage in
+    shared memory, so their read-in-place paths run (mixed with staged rows), still below TPC_MAX_ROW_HITS."""
+    r = gen_mod.Recipe("dense", n_sectors=1, n_primaries=n_tracks, pt_mode=0, pt_a=0.4, pt_b=4.0, sigma=0.06,
+                       inefficiency=0.02, noise_frac=0.2, bz=0.5, config_id=60)
+    ev = gen_mod.generate(r, event=0)
+    cnt = np.bincount(ev.row, minlength=159)
+    assert cnt.max() > 800 and cnt.max() < 2048 and cnt.min() < 1000
+    p = oracle_mod.default_params()
+    p.refit = refit
+    ref = oracle_mod.track_event(make_geometry(oracle_mod, gen_mod, ev), ev.sector_offset, ev.y, ev.z, ev.row,
+                                 params=p, precision="float")
+    trk = make_tracker(trk_mod, gen_mod, ev, params=copy_params(p, trk_mod))
+    out = trk.tpc_track_event(ev_dict(ev, True))
+    flips, res = compare_event(trk, out, ev, ref, check_stages=(refit == 0))
+    assert flips == 0 and res["n_tracks"] > 500
+    trk.close()
