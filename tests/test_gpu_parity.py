@@ -393,3 +393,31 @@ def test_parity_rows_larger_than_the_shared_memory_stages(trk_mod, gen_mod, orac
     flips, res = compare_event(trk, out, ev, ref, check_stages=(refit == 0))
     assert flips == 0 and res["n_tracks"] > 500
     trk.close()
+
+
+@pytest.mark.parametrize("n_rows", [37, 64])
+def test_parity_other_row_counts(trk_mod, gen_mod, oracle_mod, n_rows):
+    """Geometry is an input: a TPC of 37 or 64 pad rows (not multiples of 8 / 32), refit and merge on."""
+    ev = gen_mod.generate("semicentral")
+    keep = ev.row < n_rows
+    so = np.concatenate([[0], np.cumsum([keep[ev.sector_offset[s]:ev.sector_offset[s + 1]].sum()
+                                         for s in range(ev.n_sectors)])]).astype(np.int32)
+    y, z, row = ev.y[keep].copy(), ev.z[keep].copy(), ev.row[keep].copy()
+    rx = gen_mod.row_x().astype(np.float32)[:n_rows].copy()
+    p = oracle_mod.default_params()
+    p.refit = 1; p.merge = 1
+    g = oracle_mod.Geometry(ev.n_sectors, rx, gen_mod.TAN_HALF_ANGLE, ev.sigma, ev.sigma, ev.bz)
+    ref = oracle_mod.track_event(g, so, y, z, row, params=p, precision="float")
+    trk = trk_mod.Tracker(ev.n_sectors, rx, gen_mod.TAN_HALF_ANGLE, ev.sigma, ev.sigma, ev.bz, params=copy_params(p, trk_mod))
+    import torch
+    out = trk.tpc_track_event(dict(sector_offset=so, y=torch.from_numpy(y).cuda(), z=torch.from_numpy(z).cuda(),
+                                   row=torch.from_numpy(row).cuda()))
+    res = trk.to_numpy(out)
+    assert ref.n_tracks > 500 and res["n_tracks"] == ref.n_tracks
+    for k in ("trk_sector", "trk_first_hit", "trk_n_hits", "trk_ndf", "hit_idx", "trk_next", "trk_prev", "trk_global"):
+        assert np.array_equal(res[k], ref[k]), k
+    for k in ("trk_x", "trk_y", "trk_z", "trk_sinphi", "trk_tgl", "trk_qpt", "trk_chi2"):
+        err = np.abs(res[k] - ref[k]) / np.maximum(1.0, np.abs(ref[k]))
+        assert err.max(initial=0.0) <= TOL, (k, err.max())
+    assert np.array_equal(trk.tpc_debug_get("start_hit", 0), ref.start_hit)
+    trk.close()
