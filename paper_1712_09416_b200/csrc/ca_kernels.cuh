@@ -327,20 +327,31 @@ __global__ void __launch_bounds__(kCleanThreads) k_clean(const View v) {
     const int b0 = v.bin_start[bin], n = v.bin_start[bin + 1] - b0;
     if (threadIdx.x == 0) { nstart = 0; nlink = 0; }
     __syncthreads();
-    int ns = 0, nl = 0;
-    for (int k = threadIdx.x; k < n; k += kCleanThreads) {
-        const int h = b0 + k;
-        const int u = v.link_up[h], d = v.link_dn[h];
-        const int cu = (u >= 0 && v.link_dn[u] == h) ? u : -1;
-        const int cd = (d >= 0 && v.link_up[d] == h) ? d : -1;
-        v.clink_up[h] = cu;
-        v.clink_dn[h] = cd;
-        ns += (cu >= 0 && cd < 0);
-        nl += (cu >= 0);
+    int nl = 0;
+    for (int k0 = 0; k0 < n; k0 += kCleanThreads) {
+        const int k = k0 + threadIdx.x;
+        bool st = false;
+        if (k < n) {
+            const int h = b0 + k;
+            const int u = v.link_up[h], d = v.link_dn[h];
+            const int cu = (u >= 0 && v.link_dn[u] == h) ? u : -1;
+            const int cd = (d >= 0 && v.link_up[d] == h) ? d : -1;
+            v.clink_up[h] = cu;
+            v.clink_dn[h] = cd;
+            st = cu >= 0 && cd < 0;
+            nl += (cu >= 0);
+        }
+        // the row's start hits, in any order, into the bin's stretch of the (now free) bucket index array: K4
+        // then reads a short list instead of the row's links
+        const unsigned m = __ballot_sync(kFull, st);
+        int basep = 0;
+        if (lane_id() == 0 && m) basep = atomicAdd(&nstart, __popc(m));
+        basep = __shfl_sync(kFull, basep, 0);
+        if (st) v.tidx[b0 + basep + __popc(m & lanemask_lt())] = b0 + k;
     }
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) { ns += __shfl_xor_sync(kFull, ns, o); nl += __shfl_xor_sync(kFull, nl, o); }
-    if (lane_id() == 0 && (ns | nl)) { atomicAdd(&nstart, ns); atomicAdd(&nlink, nl); }
+    for (int o = 16; o > 0; o >>= 1) nl += __shfl_xor_sync(kFull, nl, o);
+    if (lane_id() == 0 && nl) atomicAdd(&nlink, nl);
     __syncthreads();
     if (threadIdx.x == 0) {
         v.seed_count[bin] = nstart;
@@ -349,34 +360,22 @@ __global__ void __launch_bounds__(kCleanThreads) k_clean(const View v) {
 }
 
 // ---------------------------------------------------------------------------------------------------------
-// K4 start-hit compaction in canonical order (task, row, caller's index): warp ballot + prefix popcount
-// collects the row's start hits, a rank by caller's index orders them.
+// K4 start-hit compaction in canonical order (task, row, caller's index): K3 collected the row's start hits with
+// warp ballots + prefix popcounts; here a rank by caller's index orders them.
 // ---------------------------------------------------------------------------------------------------------
 constexpr int kSeedThreads = 128;
 
 __global__ void __launch_bounds__(kSeedThreads) k_seeds(const View v) {
     __shared__ int list_h[TPC_MAX_ROW_HITS];
     __shared__ int list_o[TPC_MAX_ROW_HITS];
-    __shared__ int fill;
     const int bin = blockIdx.x;
     const int s0 = v.seed_start[bin], ns = v.seed_start[bin + 1] - s0;
     if (ns == 0) return;
-    const int b0 = v.bin_start[bin], n = v.bin_start[bin + 1] - b0;
-    if (threadIdx.x == 0) fill = 0;
-    __syncthreads();
-    for (int k0 = 0; k0 < n; k0 += kSeedThreads) {
-        const int k = k0 + threadIdx.x;
-        bool st = false;
-        if (k < n) st = v.clink_up[b0 + k] >= 0 && v.clink_dn[b0 + k] < 0;
-        const unsigned m = __ballot_sync(kFull, st);
-        int basep = 0;
-        if (lane_id() == 0 && m) basep = atomicAdd(&fill, __popc(m));
-        basep = __shfl_sync(kFull, basep, 0);
-        if (st) {
-            const int p = basep + __popc(m & ((1u << lane_id()) - 1u));
-            list_h[p] = b0 + k;
-            list_o[p] = v.sorig[b0 + k];
-        }
+    const int b0 = v.bin_start[bin];
+    for (int i = threadIdx.x; i < ns; i += kSeedThreads) {   // the list K3 left (any order)
+        const int h = v.tidx[b0 + i];
+        list_h[i] = h;
+        list_o[i] = v.sorig[h];
     }
     __syncthreads();
     for (int i = threadIdx.x; i < ns; i += kSeedThreads) {
