@@ -274,6 +274,37 @@ def main():
         e2e = {"value": aggregate_value(len(evs), args.steps, ms_e, world), "unit": UNIT,
                "h2d_bytes_per_step": int(12 * n_total + sum(4 * (ev.n_sectors + 1) for ev in evs)),
                "d2h_bytes_per_step": int(44 * n_tracks + 4 * n_hits), "ms_per_step": ms_e / args.steps}
+        # Two callers: a tracker is one per host thread (include/tpctrack.h); two threads, each with its own tracker,
+        # keep two batches in flight, so that the copies of one overlap the kernels of the other.  Same host buffers,
+        # same call, same bytes per step; reported beside the single-caller figure, not instead of it.
+        trk2 = tracker.Tracker(evs[0].n_sectors, rx, gen.TAN_HALF_ANGLE, evs[0].sigma, evs[0].sigma, evs[0].bz,
+                               params=params, max_events=len(evs), max_clusters=n_total)
+        trk.tpc_tracker_set_profiling(False)
+        per = max(1, args.steps // 2)
+        got = [0, 0]
+
+        def caller(k, t):
+            for _ in range(per):
+                got[k] = sum(o.n_tracks for o in t.tpc_track_events(host_in))
+        for t in (trk, trk2):
+            t.tpc_track_events(host_in)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        barrier()
+        e0.record()
+        th = [threading.Thread(target=caller, args=(k, t)) for k, t in enumerate((trk, trk2))]
+        for x in th:
+            x.start()
+        for x in th:
+            x.join()
+        torch.cuda.synchronize()          # both calls have returned: their work is complete
+        e1.record()
+        barrier()
+        ms_2 = max_over_ranks(e0.elapsed_time(e1), world)
+        assert got[0] == n_tracks and got[1] == n_tracks
+        e2e["two_callers"] = {"value": aggregate_value(len(evs), 2 * per, ms_2, world), "unit": UNIT,
+                              "ms_per_step": ms_2 / (2 * per),
+                              "note": "two host threads, one tracker each, %d steps each" % per}
+        trk2.close()
 
     if rank == 0:
         peak, peak_src = measured_peaks()

@@ -145,17 +145,39 @@ struct tpc_tracker {
     Buf<float> h_o_f[kOutF];
     bool profiling = false;
     float stage_ms[TPC_N_STAGES] = {};
+    // tpc_submit_events / tpc_wait_events: two batches in flight, each with its own work space, stream and outputs
+    struct Async {
+        Batch* b = nullptr;
+        bool busy = false;
+        Buf<int32_t> h_o_i[kOutI], h_o_hit;
+        Buf<float> h_o_f[kOutF];
+    } async[2];
 
     tpc_tracker() {
+        for (auto& a : async) {
+            a.h_o_hit.host = true;
+            for (auto& b : a.h_o_i) b.host = true;
+            for (auto& b : a.h_o_f) b.host = true;
+        }
         h_o_hit.host = true;
         for (auto& b : h_o_i) b.host = true;
         for (auto& b : h_o_f) b.host = true;
         memset(&counters, 0, sizeof counters);
     }
-    void sync_all() { for (auto s : own_streams) cudaStreamSynchronize(s); if (user_stream) cudaStreamSynchronize(user_stream); }
+    void sync_all() {
+        for (auto s : own_streams) cudaStreamSynchronize(s);
+        if (user_stream) cudaStreamSynchronize(user_stream);
+        for (auto& a : async) if (a.b) cudaStreamSynchronize(a.b->stream);
+    }
     void free_all() {
         for (auto* b : slots) { b->free_all(); delete b; }
         slots.clear();
+        for (auto& a : async) {
+            if (a.b) { cudaStreamSynchronize(a.b->stream); a.b->free_all(); cudaStreamDestroy(a.b->stream); delete a.b; a.b = nullptr; }
+            a.h_o_hit.release();
+            for (auto& b : a.h_o_i) b.release();
+            for (auto& b : a.h_o_f) b.release();
+        }
         for (auto s : own_streams) cudaStreamDestroy(s);
         own_streams.clear();
         h_o_hit.release();
@@ -690,6 +712,80 @@ int tpc_track_events(tpc_tracker* t, int32_t n, const tpc_event_in* in, tpc_even
         o.hit_idx = ohit + h;
     }
     t->have_result = true;
+    return TPC_OK;
+}
+
+int tpc_submit_events(tpc_tracker* t, int32_t n, const tpc_event_in* in, int32_t* ticket) {
+    int rc = validate(t, n, in);
+    if (rc != TPC_OK) return rc;
+    if (!ticket) { set_err("null ticket"); return TPC_ERR_ARG; }
+    int k = -1;
+    for (int j = 0; j < 2; j++) if (!t->async[j].busy) { k = j; break; }
+    if (k < 0) { set_err("two batches are in flight: wait for one first"); return TPC_ERR_ARG; }
+    tpc_tracker::Async& a = t->async[k];
+    if (!a.b) {
+        cudaStream_t s = nullptr;
+        if (cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking) != cudaSuccess) { set_err("cudaStreamCreate failed"); return TPC_ERR_CUDA; }
+        a.b = new Batch;
+        a.b->stream = s;
+    }
+    memset(&a.b->counters, 0, sizeof(tpc_counters));
+    if ((rc = batch_begin(t, a.b, 0, n, in, 0, true)) != TPC_OK) { cudaStreamSynchronize(a.b->stream); return rc; }
+    a.busy = true;
+    *ticket = k;
+    return TPC_OK;
+}
+
+int tpc_wait_events(tpc_tracker* t, int32_t ticket, tpc_event_out* out) {
+    if (!t || !out || ticket < 0 || ticket > 1 || !t->async[ticket].busy) { set_err("no batch in flight under this ticket"); return TPC_ERR_ARG; }
+    tpc_tracker::Async& a = t->async[ticket];
+    Batch* b = a.b;
+    a.busy = false;
+    int rc = batch_finish(t, b);
+    if (rc != TPC_OK) { cudaStreamSynchronize(b->stream); return rc; }
+    t->counters = b->counters;
+    if (t->profiling) for (int k = 0; k < TPC_N_STAGES; k++) t->stage_ms[k] = b->stage_ms[k];
+    t->have_result = false;   // no intermediates for these batches
+    const int n = b->n_events;
+    const int64_t T = b->counters.n_tracks, H = b->counters.n_track_hits;
+    const int nI = t->c.p.merge ? kOutI : 4, nF = t->c.p.refit ? kOutF : 7;
+    const int32_t* oi[kOutI]; const float* of[kOutF]; const int32_t* ohit;
+    if (b->host_in) {
+        for (int k = 0; k < nI; k++) {
+            if ((rc = a.h_o_i[k].reserve((size_t)std::max<int64_t>(T, 1))) != TPC_OK) return rc;
+            if (T) CK(cudaMemcpyAsync(a.h_o_i[k].p, b->o_i[k].p, sizeof(int32_t) * T, cudaMemcpyDeviceToHost, b->stream));
+        }
+        for (int k = 0; k < nF; k++) {
+            if ((rc = a.h_o_f[k].reserve((size_t)std::max<int64_t>(T, 1))) != TPC_OK) return rc;
+            if (T) CK(cudaMemcpyAsync(a.h_o_f[k].p, b->o_f[k].p, sizeof(float) * T, cudaMemcpyDeviceToHost, b->stream));
+        }
+        if ((rc = a.h_o_hit.reserve((size_t)std::max<int64_t>(H, 1))) != TPC_OK) return rc;
+        if (H) CK(cudaMemcpyAsync(a.h_o_hit.p, b->v.o_hit_idx, sizeof(int32_t) * H, cudaMemcpyDeviceToHost, b->stream));
+        CK(cudaStreamSynchronize(b->stream));
+        for (int k = 0; k < kOutI; k++) oi[k] = a.h_o_i[k].p;
+        for (int k = 0; k < kOutF; k++) of[k] = a.h_o_f[k].p;
+        ohit = a.h_o_hit.p;
+    } else {
+        for (int k = 0; k < kOutI; k++) oi[k] = b->o_i[k].p;
+        for (int k = 0; k < kOutF; k++) of[k] = b->o_f[k].p;
+        ohit = b->v.o_hit_idx;
+    }
+    const int32_t* toff = b->h_ev_off.p;
+    const int32_t* hoff = b->h_ev_off.p + (n + 1);
+    const bool rf = t->c.p.refit != 0, mg = t->c.p.merge != 0;
+    for (int e = 0; e < n; e++) {
+        tpc_event_out& o = out[e];
+        const int64_t at = toff[e], ah = hoff[e];
+        o.n_tracks = toff[e + 1] - toff[e]; o.n_track_hits = hoff[e + 1] - hoff[e];
+        o.trk_sector = oi[0] + at; o.trk_first_hit = oi[1] + at; o.trk_n_hits = oi[2] + at; o.trk_ndf = oi[3] + at;
+        o.trk_x = of[0] + at; o.trk_y = of[1] + at; o.trk_z = of[2] + at; o.trk_sinphi = of[3] + at; o.trk_tgl = of[4] + at;
+        o.trk_qpt = of[5] + at; o.trk_chi2 = of[6] + at;
+        o.hit_idx = ohit + ah;
+        o.trk_out_x = rf ? of[7] + at : nullptr; o.trk_out_y = rf ? of[8] + at : nullptr; o.trk_out_z = rf ? of[9] + at : nullptr;
+        o.trk_out_sinphi = rf ? of[10] + at : nullptr; o.trk_out_tgl = rf ? of[11] + at : nullptr;
+        o.trk_out_qpt = rf ? of[12] + at : nullptr;
+        o.trk_next = mg ? oi[4] + at : nullptr; o.trk_prev = mg ? oi[5] + at : nullptr; o.trk_global = mg ? oi[6] + at : nullptr;
+    }
     return TPC_OK;
 }
 

@@ -86,6 +86,8 @@ def _load():
     lib.tpc_tracker_set_group_events.argtypes = [C.c_void_p, C.c_int32]
     lib.tpc_track_event.argtypes = [C.c_void_p, C.POINTER(tpc_event_in), C.POINTER(tpc_event_out)]
     lib.tpc_track_events.argtypes = [C.c_void_p, C.c_int32, C.POINTER(tpc_event_in), C.POINTER(tpc_event_out)]
+    lib.tpc_submit_events.argtypes = [C.c_void_p, C.c_int32, C.POINTER(tpc_event_in), C.POINTER(C.c_int32)]
+    lib.tpc_wait_events.argtypes = [C.c_void_p, C.c_int32, C.POINTER(tpc_event_out)]
     lib.tpc_tracker_destroy.argtypes = [C.c_void_p]
     lib.tpc_tracker_destroy.restype = None
     lib.tpc_status_string.restype = C.c_char_p
@@ -104,7 +106,7 @@ lib = _load()
 
 EXPORTS = ("tpc_default_params", "tpc_tracker_create", "tpc_tracker_create_ex", "tpc_tracker_set_stream",
            "tpc_tracker_set_group_events",
-           "tpc_track_event", "tpc_track_events", "tpc_tracker_destroy", "tpc_status_string", "tpc_last_error",
+           "tpc_track_event", "tpc_track_events", "tpc_submit_events", "tpc_wait_events", "tpc_tracker_destroy", "tpc_status_string", "tpc_last_error",
            "tpc_get_counters", "tpc_tracker_set_profiling", "tpc_get_stage_ms", "tpc_debug_size", "tpc_debug_get")
 
 
@@ -205,6 +207,28 @@ class Tracker:
 
     def tpc_track_event(self, event):
         return self.tpc_track_events([event])[0]
+
+    def tpc_submit_events(self, events) -> int:
+        """Enqueue a batch (copies in + all kernels) and return its ticket; at most two batches in flight.  The
+        events' arrays must stay unchanged until ``tpc_wait_events(ticket)`` returns."""
+        n = len(events)
+        ins, keep = self._marshal(events)
+        ticket = C.c_int32(-1)
+        _check(lib.tpc_submit_events(self._h, n, ins, C.byref(ticket)))
+        if not hasattr(self, "_tickets"):
+            self._tickets = {}
+        self._tickets[ticket.value] = (n, ins, keep)
+        return ticket.value
+
+    def tpc_wait_events(self, ticket: int):
+        """Wait for the batch of ``ticket``; returns its list of ``tpc_event_out`` (valid until the second submit
+        after this call)."""
+        n, ins, keep = self._tickets.pop(ticket)
+        outs = (tpc_event_out * n)()
+        _check(lib.tpc_wait_events(self._h, ticket, outs))
+        self._mem_space = ins[0].mem_space if n else 0
+        self._keep = keep
+        return list(outs)
 
     def tpc_get_counters(self) -> dict:
         c = tpc_counters()

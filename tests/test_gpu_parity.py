@@ -421,3 +421,41 @@ def test_parity_other_row_counts(trk_mod, gen_mod, oracle_mod, n_rows):
         assert err.max(initial=0.0) <= TOL, (k, err.max())
     assert np.array_equal(trk.tpc_debug_get("start_hit", 0), ref.start_hit)
     trk.close()
+
+
+@pytest.mark.parametrize("device", [True, False])
+def test_submit_wait_gives_what_the_sync_call_gives(trk_mod, gen_mod, oracle_mod, device):
+    """tpc_submit_events / tpc_wait_events: two batches in flight, results those of tpc_track_events (refit and
+    merge on); a third submit and a wait on an idle ticket are refused."""
+    p = oracle_mod.default_params()
+    p.refit = 1; p.merge = 1
+    batches = [[gen_mod.generate("pp", 0), gen_mod.generate("semicentral", 0)],
+               [gen_mod.generate("semicentral", 1)], [gen_mod.generate("pp", 1), gen_mod.generate("pp", 2)],
+               [gen_mod.generate("semicentral", 2), gen_mod.generate("pp", 3)]]
+    trk = make_tracker(trk_mod, gen_mod, batches[0][0], params=copy_params(p, trk_mod))
+    ref_trk = make_tracker(trk_mod, gen_mod, batches[0][0], params=copy_params(p, trk_mod))
+    dicts = [[ev_dict(ev, device) for ev in b] for b in batches]
+    t0 = trk.tpc_submit_events(dicts[0])
+    t1 = trk.tpc_submit_events(dicts[1])
+    assert {t0, t1} == {0, 1}
+    with pytest.raises(trk_mod.TpcError):
+        trk.tpc_submit_events(dicts[2])               # two in flight already
+    got = {0: [trk.to_numpy(o) for o in trk.tpc_wait_events(t0)]}
+    t2 = trk.tpc_submit_events(dicts[2])               # the freed ticket is handed out again
+    got[1] = [trk.to_numpy(o) for o in trk.tpc_wait_events(t1)]
+    t3 = trk.tpc_submit_events(dicts[3])
+    got[2] = [trk.to_numpy(o) for o in trk.tpc_wait_events(t2)]
+    got[3] = [trk.to_numpy(o) for o in trk.tpc_wait_events(t3)]
+    for k, b in enumerate(batches):
+        want = [ref_trk.to_numpy(o) for o in ref_trk.tpc_track_events(dicts[k])]
+        for e, ev in enumerate(b):
+            assert got[k][e]["n_tracks"] == want[e]["n_tracks"] > 50
+            for name in want[e]:
+                assert np.array_equal(got[k][e][name], want[e][name]), (k, e, name)
+    ref = oracle_mod.track_event(make_geometry(oracle_mod, gen_mod, batches[1][0]), batches[1][0].sector_offset,
+                                 batches[1][0].y, batches[1][0].z, batches[1][0].row, params=p, precision="float")
+    assert np.array_equal(got[1][0]["hit_idx"], ref.hit_idx) and np.array_equal(got[1][0]["trk_next"], ref.trk_next)
+    with pytest.raises(trk_mod.TpcError):
+        lib_out = (trk_mod.tpc_event_out * 1)()
+        trk_mod._check(trk_mod.lib.tpc_wait_events(trk._h, 0, lib_out))     # nothing in flight
+    trk.close(); ref_trk.close()
