@@ -102,6 +102,8 @@ struct Batch {
     Buf<int32_t> h_sec_off, h_ev_off, h_nseeds;
     Buf<unsigned long long> h_cnt;
     cudaEvent_t evt[TPC_N_STAGES + 1] = {};
+    cudaEvent_t kernels_done = nullptr;      // recorded behind the last kernel of a run (submit / wait pipeline)
+    cudaEvent_t wait_for = nullptr;          // the kernels of this run start behind this event (another batch's kernels)
     float stage_ms[TPC_N_STAGES] = {};
 
     Batch() {
@@ -122,6 +124,7 @@ struct Batch {
         seed_rec.release(); tl_up.release(); dn_rec.release(); dn_count.release(); dn_start.release(); dn_fill.release(); tl_cnt.release(); o_hit_yz.release(); o_hit_row.release(); trk_hit0.release(); trk_rows.release(); trk_task.release(); mg_next.release(); mg_prev.release(); mg_list.release();
         cnt.release(); kf_cursor.release(); h_ev_src.release(); h_sec_off.release(); h_ev_off.release(); h_cnt.release(); h_nseeds.release();
         for (auto& e : evt) if (e) { cudaEventDestroy(e); e = nullptr; }
+        if (kernels_done) { cudaEventDestroy(kernels_done); kernels_done = nullptr; }
     }
 };
 
@@ -405,7 +408,10 @@ int batch_begin(const tpc_tracker* tr, Batch* t, int first_event, int n, const t
         for (auto& e : t->evt)
             if (!e) CK(cudaEventCreate(&e));
 
+    // submit / wait pipeline: the input copies above run beside the other batch's kernels, the kernels behind them
+    if (t->wait_for) CK(cudaStreamWaitEvent(st, t->wait_for, 0));
     if ((rc = launch_all(tr, t)) != TPC_OK) return rc;
+    if (t->kernels_done) CK(cudaEventRecord(t->kernels_done, st));
     CK(cudaMemcpyAsync(t->h_cnt.p, v.cnt, sizeof(unsigned long long) * CNT_N, cudaMemcpyDeviceToHost, st));
     CK(cudaMemcpyAsync(t->h_ev_off.p, v.ev_off, sizeof(int32_t) * 2 * (n + 1), cudaMemcpyDeviceToHost, st));
     CK(cudaMemcpyAsync(t->h_nseeds.p, v.seed_start + v.n_bins, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
@@ -728,7 +734,12 @@ int tpc_submit_events(tpc_tracker* t, int32_t n, const tpc_event_in* in, int32_t
         if (cudaStreamCreateWithFlags(&s, cudaStreamNonBlocking) != cudaSuccess) { set_err("cudaStreamCreate failed"); return TPC_ERR_CUDA; }
         a.b = new Batch;
         a.b->stream = s;
+        if (cudaEventCreateWithFlags(&a.b->kernels_done, cudaEventDisableTiming) != cudaSuccess) { set_err("cudaEventCreate failed"); return TPC_ERR_CUDA; }
     }
+    // copy-in | kernels | copy-out pipeline: the kernels of this batch queue behind those of the batch in flight, so
+    // that two batches never share the SMs; only the copies run beside the other batch's kernels
+    tpc_tracker::Async& o = t->async[1 - k];
+    a.b->wait_for = (o.busy && o.b) ? o.b->kernels_done : nullptr;
     memset(&a.b->counters, 0, sizeof(tpc_counters));
     if ((rc = batch_begin(t, a.b, 0, n, in, 0, true)) != TPC_OK) { cudaStreamSynchronize(a.b->stream); return rc; }
     a.busy = true;
