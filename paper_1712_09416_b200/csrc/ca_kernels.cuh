@@ -258,19 +258,20 @@ __global__ void __launch_bounds__(kNfThreads, TPC_NF_BLOCKS) k_neighbours(const 
         const int h = b0 + k;
         const float2 h0 = v.shit[h];
         const float y0 = h0.x, z0 = h0.y;
-        int bu = -1, bd = -1;   // row-local indices of the best pair
-        float best = 0.f;
+        int bpair = -1;         // row-local indices of the best pair, u << 16 | d (both < 2048)
+        float best = __int_as_float(0x7f800000);   // +inf: the first pair always wins
         auto eval = [&](int u, const float2& pu, int d, const float2& pd) {
             const float yh = pd.x + a * (pu.x - pd.x);
             const float zh = pd.y + a * (pu.y - pd.y);
             const float dy = y0 - yh, dz = z0 - zh;
             const float dev = dy * dy + dz * dz;
-            bool take = bu < 0 || dev < best;
-            if (!take && dev == best) {  // exact tie: lowest caller's index of u, then of d
+            bool take = dev < best;
+            if (dev == best && bpair >= 0) {  // exact tie: lowest caller's index of u, then of d
+                const int bu = bpair >> 16, bd = bpair & 0xffff;
                 const int ou = v.sorig[du.x + u], obu = v.sorig[du.x + bu];
                 take = ou < obu || (ou == obu && v.sorig[dd.x + d] < v.sorig[dd.x + bd]);
             }
-            if (take) { best = dev; bu = u; bd = d; }
+            if (take) { best = dev; bpair = (u << 16) | d; }
         };
         // down-candidates inside the window, remembered
         const CellWin wd = cell_window(gfd, nyd, dd.w, y0, z0, wyd, wzd);
@@ -309,9 +310,9 @@ __global__ void __launch_bounds__(kNfThreads, TPC_NF_BLOCKS) k_neighbours(const 
                 }
             }
         }
-        const bool ok = bu >= 0 && best <= c.p.nf_dmax;
-        v.link_up[h] = ok ? du.x + bu : -1;
-        v.link_dn[h] = ok ? dd.x + bd : -1;
+        const bool ok = bpair >= 0 && best <= c.p.nf_dmax;
+        v.link_up[h] = ok ? du.x + (bpair >> 16) : -1;
+        v.link_dn[h] = ok ? dd.x + (bpair & 0xffff) : -1;
     }
 }
 
