@@ -204,7 +204,7 @@ __device__ __forceinline__ int sweep_search(const View& v, const Const& c, const
     const float wz = fminf(fmaxf(c.p.win_nsigma * sqrtf(f.c11 + c.sigma_z2), c.p.win_min), c.p.win_max);
     const CellWin w = cell_window(gf, dn.z, dn.w, f.y, f.z, wy, wz);
     int bp = -1;
-    bg = 0.f;
+    bg = __int_as_float(0x7f800000);   // +inf: the first hit inside the window always wins
     for (int iz = w.iz0; iz <= w.iz1; iz++) {
         int p = cs[iz * dn.z + w.iy0];
         const int pe = cs[iz * dn.z + w.iy1 + 1];
@@ -213,12 +213,13 @@ __device__ __forceinline__ int sweep_search(const View& v, const Const& c, const
             const float ry = h.x - f.y, rz = h.y - f.z;
             if (fabsf(ry) <= wy && fabsf(rz) <= wz) {
                 const float gv = (ry * ry) * iwy + (rz * rz) * iwz;   // the gate value of h
-                bool take = bp < 0 || gv < bg;
-                if (!take && gv == bg) take = v.sorig[dn.x + p] < v.sorig[dn.x + bp];
-                if (take) { bg = gv; bp = p; ay = h.x; az = h.y; }
+                bool take = gv < bg;
+                if (gv == bg && bp >= 0) take = v.sorig[dn.x + p] < v.sorig[dn.x + bp];
+                if (take) { bg = gv; bp = p; }
             }
         }
     }
+    if (bp >= 0) { const float2 h = hits[bp]; ay = h.x; az = h.y; }
     return bp;
 }
 
