@@ -353,9 +353,9 @@ __global__ void __launch_bounds__(kSwThreads, kSwBlocksPerSM) k_sweep(const View
         __syncwarp();
         if (search && dn.y > 0) {
             const float4 gf = make_float4(dsc.y0, dsc.z0, dsc.idy, dsc.idz);
-            float by = 0.f, bz = 0.f, bg = 0.f;
-            const int bp = sweep_search(v, c, f, gf, dn, hits, cs, iwy, iwz, by, bz, bg);
-            if (bp >= 0 && bg <= c.p.chi2_ext) { acc = dn.x + bp; ay = by; az = bz; }
+            float bg = 0.f;   // a lane that searches has accepted nothing yet on this row: (ay, az) are free
+            const int bp = sweep_search(v, c, f, gf, dn, hits, cs, iwy, iwz, ay, az, bg);
+            if (bp >= 0 && bg <= c.p.chi2_ext) acc = dn.x + bp;
         }
         __syncwarp();
 
