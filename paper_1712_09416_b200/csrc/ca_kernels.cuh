@@ -266,7 +266,7 @@ __global__ void __launch_bounds__(kNfThreads, TPC_NF_BLOCKS) k_neighbours(const 
             const float dy = y0 - yh, dz = z0 - zh;
             const float dev = dy * dy + dz * dz;
             bool take = dev < best;
-            if (dev == best && bpair >= 0) {  // exact tie: lowest caller's index of u, then of d
+            if (dev == best) {  // exact tie (dev is finite, so a pair is held): lowest caller's index of u, then of d
                 const int bu = bpair >> 16, bd = bpair & 0xffff;
                 const int ou = v.sorig[du.x + u], obu = v.sorig[du.x + bu];
                 take = ou < obu || (ou == obu && v.sorig[dd.x + d] < v.sorig[dd.x + bd]);

@@ -214,7 +214,7 @@ __device__ __forceinline__ int sweep_search(const View& v, const Const& c, const
             if (fabsf(ry) <= wy && fabsf(rz) <= wz) {
                 const float gv = (ry * ry) * iwy + (rz * rz) * iwz;   // the gate value of h
                 bool take = gv < bg;
-                if (gv == bg && bp >= 0) take = v.sorig[dn.x + p] < v.sorig[dn.x + bp];
+                if (gv == bg) take = v.sorig[dn.x + p] < v.sorig[dn.x + bp];   // exact tie (gv is finite: bp >= 0 here)
                 if (take) { bg = gv; bp = p; }
             }
         }
