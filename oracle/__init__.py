@@ -56,9 +56,9 @@ class _Geometry(C.Structure):
 _FIELDS = ["link_up", "link_dn", "clink_up", "clink_dn", "nf_margin", "seed_offset", "start_hit",
            "tl_first_row", "tl_last_row", "tl_n_hits", "tl_par", "tl_chi2", "tl_margin", "tl_table",
            "trk_sector", "trk_first_hit", "trk_n_hits", "trk_ndf", "trk_seed", "trk_first_row",
-           "trk_x", "trk_y", "trk_z", "trk_sinphi", "trk_tgl", "trk_qpt", "trk_chi2", "trk_margin", "hit_idx", "tl_cov", "trk_row_out", "trk_out", "trk_next", "trk_prev", "trk_global"]
+           "trk_x", "trk_y", "trk_z", "trk_sinphi", "trk_tgl", "trk_qpt", "trk_chi2", "trk_margin", "hit_idx", "tl_cov", "trk_row_out", "trk_out", "trk_next", "trk_prev", "trk_global", "trk_merge_margin"]
 _F64 = {"nf_margin", "tl_par", "tl_cov", "tl_chi2", "tl_margin", "trk_x", "trk_y", "trk_z", "trk_sinphi", "trk_tgl",
-        "trk_qpt", "trk_chi2", "trk_margin", "trk_out"}
+        "trk_qpt", "trk_chi2", "trk_margin", "trk_out", "trk_merge_margin"}
 
 _lib = None
 
@@ -81,6 +81,8 @@ def lib():
         l.oracle_update.argtypes = [C.POINTER(_Geometry), C.POINTER(Params), C.c_double, C.c_double, C.c_void_p,
                                     C.c_void_p, C.c_void_p]
         l.oracle_max_threads.restype = C.c_int32
+        l.oracle_merge_tracks.restype = C.c_int32
+        l.oracle_merge_tracks.argtypes = [C.POINTER(_Geometry), C.POINTER(Params), C.c_int32, C.c_int32] + [C.c_void_p] * 9
         _lib = l
     return _lib
 
@@ -176,3 +178,22 @@ def update(geom: Geometry, my: float, mz: float, state, cov, chi2: float = 0.0, 
     c2 = np.array([chi2], np.float64)
     lib().oracle_update(C.byref(g), C.byref(p), my, mz, st.ctypes.data, cv.ctypes.data, c2.ctypes.data)
     return st, cv, float(c2[0])
+
+
+def merge_tracks(geom: Geometry, sector, first_row, par, row_out, out, params: Params | None = None,
+                 precision: str = "double"):
+    """O9 on caller-given segments: ``par`` [T,6] = x, y, z, sin phi, tg lambda, q/pT at the first fitted row,
+    ``out`` [T,6] the outer state at pad row ``row_out``.  Returns next, prev, global (int32 [T]) and margin."""
+    p = params if params is not None else default_params()
+    g, _keep = geom._c()
+    sector = np.ascontiguousarray(sector, np.int32); first_row = np.ascontiguousarray(first_row, np.int32)
+    row_out = np.ascontiguousarray(row_out, np.int32)
+    par = np.ascontiguousarray(par, np.float64).reshape(-1, 6); out = np.ascontiguousarray(out, np.float64).reshape(-1, 6)
+    T = int(sector.shape[0])
+    nx = np.zeros(T, np.int32); pv = np.zeros(T, np.int32); gl = np.zeros(T, np.int32); mg = np.zeros(T, np.float64)
+    rc = lib().oracle_merge_tracks(C.byref(g), C.byref(p), 1 if precision == "float" else 0, T, sector.ctypes.data,
+                                   first_row.ctypes.data, par.ctypes.data, row_out.ctypes.data, out.ctypes.data,
+                                   nx.ctypes.data, pv.ctypes.data, gl.ctypes.data, mg.ctypes.data)
+    if rc != 0:
+        raise ValueError("oracle_merge_tracks: bad arguments")
+    return nx, pv, gl, mg

@@ -25,7 +25,11 @@
  * pulls / chi2 per ndf / Gluckstern curvature resolution with noise; O6 ownership invariants and a brute-force
  * owner; end-to-end efficiency on generated events; O8 (refit of the selected tracks) against the
  * generated helix, the least-squares line, a test-side composition of the pinned transport / update steps,
- * chi2 per ndf and Gluckstern (tests/test_oracle_refit.py).
+ * chi2 per ndf and Gluckstern (tests/test_oracle_refit.py); O5 search / gate / construct against a Python
+ * restatement of DESIGN.md "O5" that drives only the pinned transport / update, and against hand-built sectors
+ * with hand-written expected tables for every branch: window edges and clamps, ties, gap counting, edge stop,
+ * rejected links, removed hits (tests/test_oracle_constructor.py); O9 against generator truth, a restatement with
+ * the exact helix, and hand-built segments on every tie and cut edge (tests/test_oracle_merge.py).
  * PARITY UNPINNED: the exact link / track values on the BASELINE.json configs have no outside reference
  * (the paper prints none); they are pinned only through the properties above.
  */
@@ -115,6 +119,7 @@ struct Result {
     /* O8 outer state (up pass of the refit, at its top hit) and O9 links */
     std::vector<int32_t> trk_row_out, trk_next, trk_prev, trk_global; /* global: first segment of the chain */
     std::vector<double> trk_out; /* [T][6] x y z sin phi tg lambda q/pT */
+    std::vector<double> trk_merge_margin; /* [T] smallest relative margin of the O9 decisions a segment took part in */
 };
 
 template <class R> struct Sector {
@@ -468,7 +473,10 @@ void merge_segments(const oracle_geometry& G, const oracle_params& P, Result& re
     const R smax = R(P.sin_max);
     const R ty = R(P.merge_dy), tz = R(P.merge_dz), ts = R(P.merge_ds), tt = R(P.merge_dt);
     std::vector<R> bestn(T, R(0)), bestp(T, R(0));
-    auto pair_score = [&](int a, int b, R& D) -> bool {
+    std::vector<Margin> mgs(T);
+    res.trk_merge_margin.assign(T, std::numeric_limits<double>::infinity());
+    /* mg: every float comparison of this pair leaves its relative margin there (parity protocol) */
+    auto pair_score = [&](int a, int b, R& D, Margin& mg) -> bool {
         if (res.trk_row_out[a] < 0 || res.trk_row_out[b] < 0) return false;   /* no refit (fewer than 2 hits) */
         const int sa = res.trk_sector[a], sb = res.trk_sector[b];
         if (sa / half != sb / half) return false;
@@ -480,7 +488,7 @@ void merge_segments(const oracle_geometry& G, const oracle_params& P, Result& re
         const R xa = R(o[0]), ya = R(o[1]), za = R(o[2]), s0 = R(o[3]), t0 = R(o[4]), q0 = R(o[5]);
         /* turn by alpha_A - alpha_B: -step when B is the next sector, +step when it is the one before */
         const R sn = (dk == 1) ? R(0) - sd : sd;
-        if (std::fabs(s0) > smax) return false;
+        if (gt(std::fabs(s0), smax, mg)) return false;
         const R c0a = std::sqrt(R(1) - s0 * s0);
         const R x1 = xa * cd - ya * sn;
         const R y1 = xa * sn + ya * cd;
@@ -490,7 +498,8 @@ void merge_segments(const oracle_geometry& G, const oracle_params& P, Result& re
         const R dx = xb - x1;
         const R kap = kB * q0;
         const R s2 = s1 + kap * dx;
-        if (std::fabs(s1) > smax || std::fabs(s2) > smax) return false;
+        if (gt(std::fabs(s1), smax, mg)) return false;
+        if (gt(std::fabs(s2), smax, mg)) return false;
         const R c1 = std::sqrt(R(1) - s1 * s1), c2 = std::sqrt(R(1) - s2 * s2);
         const R dy = dx * ((s1 + s2) * (R(1) / (c1 + c2)));
         const R dl2 = dx * dx + dy * dy;
@@ -501,26 +510,41 @@ void merge_segments(const oracle_geometry& G, const oracle_params& P, Result& re
         const R y2 = y1 + dy, z2 = za + t0 * dS;
         const R ey = y2 - R(res.trk_y[b]), ez = z2 - R(res.trk_z[b]);
         const R es = s2 - R(res.trk_sinphi[b]), et = t0 - R(res.trk_tgl[b]);
-        if (!(std::fabs(ey) <= ty && std::fabs(ez) <= tz && std::fabs(es) <= ts && std::fabs(et) <= tt)) return false;
+        const bool iy = le(std::fabs(ey), ty, mg), iz = le(std::fabs(ez), tz, mg);
+        const bool is = le(std::fabs(es), ts, mg), it = le(std::fabs(et), tt, mg);
+        if (!(iy && iz && is && it)) return false;
         const R ny = ey * (R(1) / ty), nz = ez * (R(1) / tz), ns = es * (R(1) / ts), nt = et * (R(1) / tt);
         D = ((ny * ny + nz * nz) + ns * ns) + nt * nt;
         return true;
     };
     std::vector<int32_t> nx(T, -1), pv(T, -1);
-    for (int a = 0; a < T; a++)
+    for (int a = 0; a < T; a++) {
+        R second = 0; bool have2 = false;
         for (int b = 0; b < T; b++) {
             R D;
-            if (a == b || !pair_score(a, b, D)) continue;
-            if (nx[a] < 0 || D < bestn[a]) { nx[a] = b; bestn[a] = D; }   /* ascending b: ties keep the lower index */
+            if (a == b || !pair_score(a, b, D, mgs[a])) continue;
+            if (nx[a] < 0 || D < bestn[a]) {                      /* ascending b: ties keep the lower index */
+                if (nx[a] >= 0) { second = bestn[a]; have2 = true; }
+                nx[a] = b; bestn[a] = D;
+            } else if (!have2 || D < second) { second = D; have2 = true; }
         }
-    for (int b = 0; b < T; b++)
+        if (have2) mgs[a].rel((double)bestn[a], (double)second);
+    }
+    for (int b = 0; b < T; b++) {
+        R second = 0; bool have2 = false;
         for (int a = 0; a < T; a++) {
             R D;
-            if (a == b || !pair_score(a, b, D)) continue;
-            if (pv[b] < 0 || D < bestp[b]) { pv[b] = a; bestp[b] = D; }
+            if (a == b || !pair_score(a, b, D, mgs[b])) continue;
+            if (pv[b] < 0 || D < bestp[b]) {
+                if (pv[b] >= 0) { second = bestp[b]; have2 = true; }
+                pv[b] = a; bestp[b] = D;
+            } else if (!have2 || D < second) { second = D; have2 = true; }
         }
+        if (have2) mgs[b].rel((double)bestp[b], (double)second);
+    }
     for (int a = 0; a < T; a++)
         if (nx[a] >= 0 && pv[nx[a]] == a) { res.trk_next[a] = nx[a]; res.trk_prev[nx[a]] = a; }
+    for (int a = 0; a < T; a++) res.trk_merge_margin[a] = mgs[a].m;
     /* global track = chain of linked segments, named by its first segment (links join a sector to the next one
        outwards in row, so a chain cannot close on itself) */
     for (int a = 0; a < T; a++) {
@@ -632,6 +656,7 @@ Result* run(const oracle_geometry& G, const oracle_params& P, int32_t n, const i
     else {
         const size_t T = res->trk_sector.size();
         res->trk_next.assign(T, -1); res->trk_prev.assign(T, -1); res->trk_global.resize(T);
+        res->trk_merge_margin.assign(T, std::numeric_limits<double>::infinity());
         for (size_t a = 0; a < T; a++) res->trk_global[a] = (int32_t)a;
     }
     return res;
@@ -685,7 +710,7 @@ enum {
     F_LINK_UP = 0, F_LINK_DN, F_CLINK_UP, F_CLINK_DN, F_NF_MARGIN, F_SEED_OFFSET, F_START_HIT,
     F_TL_FIRST_ROW, F_TL_LAST_ROW, F_TL_N_HITS, F_TL_PAR, F_TL_CHI2, F_TL_MARGIN, F_TL_TABLE,
     F_TRK_SECTOR, F_TRK_FIRST_HIT, F_TRK_N_HITS, F_TRK_NDF, F_TRK_SEED, F_TRK_FIRST_ROW,
-    F_TRK_X, F_TRK_Y, F_TRK_Z, F_TRK_SINPHI, F_TRK_TGL, F_TRK_QPT, F_TRK_CHI2, F_TRK_MARGIN, F_HIT_IDX, F_TL_COV, F_TRK_ROW_OUT, F_TRK_OUT, F_TRK_NEXT, F_TRK_PREV, F_TRK_GLOBAL
+    F_TRK_X, F_TRK_Y, F_TRK_Z, F_TRK_SINPHI, F_TRK_TGL, F_TRK_QPT, F_TRK_CHI2, F_TRK_MARGIN, F_HIT_IDX, F_TL_COV, F_TRK_ROW_OUT, F_TRK_OUT, F_TRK_NEXT, F_TRK_PREV, F_TRK_GLOBAL, F_TRK_MERGE_MARGIN
 };
 
 /* copy one result field into caller memory (int32 or float64, shapes in oracle/__init__.py) */
@@ -732,6 +757,7 @@ int32_t oracle_copy(const void* rv, int32_t field, void* dst) {
         case F_TRK_NEXT: copy_out(r->trk_next, dst); break;
         case F_TRK_PREV: copy_out(r->trk_prev, dst); break;
         case F_TRK_GLOBAL: copy_out(r->trk_global, dst); break;
+        case F_TRK_MERGE_MARGIN: copy_out(r->trk_merge_margin, dst); break;
         default: return -1;
     }
     return 0;
@@ -779,6 +805,30 @@ void oracle_update(const oracle_geometry* G, const oracle_params* P, double my, 
     S.update1(f, 1, mz, (double)G->sigma_z * (double)G->sigma_z);
     state[0] = f.y; state[1] = f.z; state[2] = f.s; state[3] = f.t; state[4] = f.q; *chi2 = f.chi2;
     for (int i = 0; i < 5; i++) for (int j = 0; j < 5; j++) cov[5 * i + j] = f.C[i][j];
+}
+
+/* O9 on caller-given segments (for the pins): T segments with sector, first fitted row, parameters
+ * par[T][6] = x y z sin phi tg lambda q/pT at that row, outer row and outer state out[T][6] (x y z s t q).
+ * Fills next / prev / global [T] and margin [T] (may be NULL). */
+int32_t oracle_merge_tracks(const oracle_geometry* G, const oracle_params* P, int32_t precision, int32_t T,
+                            const int32_t* sector, const int32_t* first_row, const double* par, const int32_t* row_out,
+                            const double* out, int32_t* next, int32_t* prev, int32_t* global, double* margin) {
+    if (!G || !P || T < 0) return -1;
+    Result res;
+    res.n_sectors = G->n_sectors; res.n_rows = G->n_rows;
+    for (int a = 0; a < T; a++) {
+        res.trk_sector.push_back(sector[a]); res.trk_first_row.push_back(first_row[a]);
+        res.trk_x.push_back(par[6 * a]); res.trk_y.push_back(par[6 * a + 1]); res.trk_z.push_back(par[6 * a + 2]);
+        res.trk_sinphi.push_back(par[6 * a + 3]); res.trk_tgl.push_back(par[6 * a + 4]); res.trk_qpt.push_back(par[6 * a + 5]);
+        res.trk_row_out.push_back(row_out[a]);
+        for (int j = 0; j < 6; j++) res.trk_out.push_back(out[6 * a + j]);
+    }
+    if (precision == 1) merge_segments<float>(*G, *P, res); else merge_segments<double>(*G, *P, res);
+    for (int a = 0; a < T; a++) {
+        next[a] = res.trk_next[a]; prev[a] = res.trk_prev[a]; global[a] = res.trk_global[a];
+        if (margin) margin[a] = res.trk_merge_margin.empty() ? std::numeric_limits<double>::infinity() : res.trk_merge_margin[a];
+    }
+    return 0;
 }
 
 int32_t oracle_max_threads(void) {

@@ -1,0 +1,460 @@
+"""Deterministic pins of the oracle's tracklet constructor O5: ``Sector::search``, ``Sector::gate`` and the
+orchestration ``Sector::construct`` (PAPER.md:17 names only "Cellular
+Automaton" and "Kalman filter").
+
+Two kinds of pin, neither of which asks the oracle for its own expectation:
+
+* ``restate_construct`` below is O5 written again, in Python, from the text of DESIGN.md "O5": gate, window,
+  search, FOLLOW / EXTEND state machine, down pass, snapshots.  The only things it takes from the oracle are the
+  two primitives that are pinned on their own in test_oracle_kf.py (``oracle.transport`` against the closed-form
+  helix, ``oracle.update`` against the textbook Kalman update) and the cleaned links (pinned in
+  test_oracle_ca.py).  It is compared in double with every tracklet of config 1, of a tiny sector with heavy
+  noise, of low-pT curlers (transport failures) and of a step-2 run, to 1e-12.
+* hand-built sectors -- hits exactly on the line y = const, z = 0, so that every prediction is known exactly
+  without running anything -- force each branch, with the expected row -> hit table written out by hand.
+
+Done-criterion ("Weak #1"): each of the five oracle mutations that survived round 1's tests
+fails at least one test here:
+  (1) ``search`` ties to the HIGHEST index (``g <= gb``)            -> test_coincident_candidates_lowest_index_wins
+  (2) ``w_max`` clamp dropped from the window                        -> test_window_edge_at_w_max_is_inclusive
+  (3) up-pass ``miss`` never reset on an accepted hit                -> test_miss_counter_is_reset_by_an_accepted_hit
+  (4) edge stop at 5 x ``edge_margin``                               -> test_edge_stop_at_the_wedge_plus_margin
+  (5) ``max_gap`` off by one (``>=``)                                -> test_gap_of_max_gap_rows_is_bridged_one_more_is_not
+"""
+import math
+
+import numpy as np
+import pytest
+
+N_ROWS = 159
+
+
+def _geom(oracle, gen, sigma=0.06, bz=0.5, n_sectors=1):
+    return oracle.Geometry(n_sectors, gen.row_x().astype(np.float32), gen.TAN_HALF_ANGLE, sigma, sigma, bz)
+
+
+# ---------------------------------------------------------------------------------------------------------
+# O5 restated from DESIGN.md (double precision).  Returns the tracklet and a trace of what each row did.
+# ---------------------------------------------------------------------------------------------------------
+def restate_construct(oracle, g, P, rx, y, z, row, hits_of_row, clink_up, h0):
+    sy2 = float(np.float32(g.sigma_y)) ** 2
+    sz2 = float(np.float32(g.sigma_z)) ** 2
+    tan = float(np.float32(g.tan_half_angle))
+    prior = np.diag([sy2, sz2, float(P.var_s), float(P.var_t), float(P.var_q)])
+    X = [float(v) for v in rx]
+    trace = []
+
+    def gate(st, cv, h):
+        ry, rz = y[h] - st[0], z[h] - st[1]
+        return (ry * ry) * (1.0 / (cv[0, 0] + sy2)) + (rz * rz) * (1.0 / (cv[1, 1] + sz2))
+
+    def window(c, s2):
+        return min(max(float(P.win_nsigma) * math.sqrt(c + s2), float(P.win_min)), float(P.win_max))
+
+    def search(st, cv, r, tag):
+        wy, wz = window(cv[0, 0], sy2), window(cv[1, 1], sz2)
+        best, gb = -1, math.inf
+        cands = []
+        for c in hits_of_row[r]:                       # ascending caller's index: strict < keeps the lowest
+            if abs(y[c] - st[0]) <= wy and abs(z[c] - st[1]) <= wz:
+                gv = gate(st, cv, c)
+                cands.append((int(c), gv))
+                if gv < gb:
+                    best, gb = int(c), gv
+        acc = best if (best >= 0 and gb <= float(P.chi2_ext)) else -1
+        trace.append(dict(kind="search", pas=tag, row=r, wy=wy, wz=wz, y=st[0], z=st[1], cands=cands, acc=acc))
+        return acc
+
+    tab = [-1] * len(X)
+    r0 = int(row[h0]); h1 = int(clink_up[h0])
+    dx = X[int(row[h1])] - X[r0]
+    dy, dz = y[h1] - y[h0], z[h1] - z[h0]
+    dl = math.sqrt(dx * dx + dy * dy)
+    st = np.array([y[h0], z[h0], dy / dl, dz / dl, 0.0]); cv = prior.copy(); chi2 = 0.0
+    tab[r0] = int(h0)
+    snap = st.copy(); top = r0
+    # ---- up pass ----
+    follow, cur, miss, xc = True, h1, 0, X[r0]
+    for r in range(r0 + 1, len(X)):
+        ok, st, cv = oracle.transport(g, xc, X[r], st, cv, params=P)
+        if not ok:
+            trace.append(dict(kind="transport_fail", pas="up", row=r)); break
+        xc = X[r]
+        if follow:
+            if r < int(row[cur]):
+                continue
+            gv = gate(st, cv, cur)
+            if gv <= float(P.chi2_link):
+                st, cv, chi2 = oracle.update(g, y[cur], z[cur], st, cv, chi2, params=P)
+                tab[r] = int(cur); snap = st.copy(); top = r
+                cur = int(clink_up[cur])
+                if cur < 0:
+                    follow = False
+                continue
+            trace.append(dict(kind="link_rejected", pas="up", row=r, g=gv))
+            follow = False                               # and search this same row
+        if abs(st[0]) > X[r] * tan + float(P.edge_margin):
+            trace.append(dict(kind="edge", pas="up", row=r)); break
+        c = search(st, cv, r, "up")
+        if c >= 0:
+            st, cv, chi2 = oracle.update(g, y[c], z[c], st, cv, chi2, params=P)
+            tab[r] = c; snap = st.copy(); top = r; miss = 0
+        else:
+            miss += 1
+            if miss > int(P.max_gap):
+                trace.append(dict(kind="gap", pas="up", row=r)); break
+    # ---- down pass: fresh fit at the top recorded hit, direction and curvature of the up pass ----
+    ht = tab[top]
+    st = np.array([y[ht], z[ht], snap[2], snap[3], snap[4]]); cv = prior.copy(); chi2 = 0.0; n = 1
+    res = (st.copy(), chi2, n); first = top
+    miss, xc = 0, X[top]
+    r = top - 1
+    while r >= 0:
+        ok, st, cv = oracle.transport(g, xc, X[r], st, cv, params=P)
+        if not ok:
+            trace.append(dict(kind="transport_fail", pas="down", row=r)); break
+        xc = X[r]
+        hr = tab[r]
+        if hr >= 0:
+            gv = gate(st, cv, hr)
+            if gv <= float(P.chi2_link):
+                st, cv, chi2 = oracle.update(g, y[hr], z[hr], st, cv, chi2, params=P)
+                n += 1; res = (st.copy(), chi2, n); first = r
+            else:
+                tab[r] = -1
+                trace.append(dict(kind="recorded_removed", pas="down", row=r, g=gv))
+            r -= 1
+            continue
+        below = r < r0
+        if below and abs(st[0]) > X[r] * tan + float(P.edge_margin):
+            trace.append(dict(kind="edge", pas="down", row=r)); break
+        c = search(st, cv, r, "down")
+        if c >= 0:
+            st, cv, chi2 = oracle.update(g, y[c], z[c], st, cv, chi2, params=P)
+            n += 1; tab[r] = c; res = (st.copy(), chi2, n); first = r; miss = 0
+        elif below:
+            miss += 1
+            if miss > int(P.max_gap):
+                trace.append(dict(kind="gap", pas="down", row=r)); break
+        r -= 1
+    while r >= 0:                                        # rows the pass never reached keep nothing
+        tab[r] = -1; r -= 1
+    return dict(table=np.array(tab, np.int32), first=first, last=top, n=res[2], par=res[0], chi2=res[1]), trace
+
+
+def _rows_index(row, lo, hi):
+    """hits of each pad row among the clusters lo..hi-1 of one sector, ascending caller's index"""
+    return [lo + np.nonzero(row[lo:hi] == r)[0] for r in range(N_ROWS)]
+
+
+def _compare_all_tracklets(oracle, gen, ev, P, max_tracklets=None, every=1):
+    g = _geom(oracle, gen, ev.sigma, ev.bz, ev.n_sectors)
+    rx = gen.row_x().astype(np.float32)
+    res = oracle.track_event(g, ev.sector_offset, ev.y, ev.z, ev.row, params=P, precision="double", stop_after=5)
+    y, z = ev.y.astype(np.float64), ev.z.astype(np.float64)
+    so = ev.sector_offset
+    hor_s = [_rows_index(ev.row, int(so[s]), int(so[s + 1])) for s in range(ev.n_sectors)]
+    kinds = {}
+    ids = range(0, res.n_seeds, every) if max_tracklets is None else range(min(res.n_seeds, max_tracklets))
+    for i in ids:
+        h0 = int(res.start_hit[i])
+        hor = hor_s[int(np.searchsorted(so, h0, side="right")) - 1]
+        T, trace = restate_construct(oracle, g, P, rx, y, z, ev.row, hor, res.clink_up, h0)
+        assert np.array_equal(T["table"], res.tl_table[i]), (i, np.nonzero(T["table"] != res.tl_table[i]))
+        assert (T["first"], T["last"], T["n"]) == (res.tl_first_row[i], res.tl_last_row[i], res.tl_n_hits[i]), i
+        assert np.allclose(T["par"], res.tl_par[i], rtol=1e-12, atol=1e-13), (i, T["par"], res.tl_par[i])
+        assert abs(T["chi2"] - res.tl_chi2[i]) <= 1e-12 * max(1.0, T["chi2"]), i
+        for t in trace:
+            key = (t["kind"], t["pas"])
+            kinds[key] = kinds.get(key, 0) + 1
+            if t["kind"] == "search":
+                if t["acc"] >= 0:
+                    kinds[("search_hit", t["pas"])] = kinds.get(("search_hit", t["pas"]), 0) + 1
+                if len(t["cands"]) > 1:
+                    kinds[("search_multi", t["pas"])] = kinds.get(("search_multi", t["pas"]), 0) + 1
+                if t["wy"] == float(P.win_min):
+                    kinds["w_min"] = kinds.get("w_min", 0) + 1
+                if t["wy"] == float(P.win_max):
+                    kinds["w_max"] = kinds.get("w_max", 0) + 1
+    return res, kinds
+
+
+def test_constructor_equals_restatement_on_config_1(oracle_mod, gen_mod):
+    """Every tracklet of BASELINE.json config 1 (50 tracks, 2 % holes, 5 % noise): tables, rows, parameters."""
+    ev = gen_mod.generate("single_sector")
+    res, kinds = _compare_all_tracklets(oracle_mod, gen_mod, ev, oracle_mod.default_params())
+    assert res.n_seeds > 60
+    # the branches this workload must have gone through
+    assert kinds[("search_hit", "up")] > 100 and kinds[("search_hit", "down")] > 100
+    assert kinds[("gap", "up")] + kinds.get(("edge", "up"), 0) > 10
+    assert kinds["w_min"] > 1000
+
+
+def test_constructor_equals_restatement_on_a_dense_sector(oracle_mod, gen_mod):
+    """150 tracks in one sector (central Pb-Pb-like occupancy, sigma 0.08, 50 % noise): windows with several
+    candidates, rejected links, recorded hits removed by the down pass.  Every 4th tracklet."""
+    ev = gen_mod.tiny_sector(n_tracks=150, seed=11, noise_frac=0.5, sigma=0.08)
+    res, kinds = _compare_all_tracklets(oracle_mod, gen_mod, ev, oracle_mod.default_params(), every=4)
+    assert res.n_seeds > 400
+    assert kinds.get(("search_multi", "up"), 0) > 20 and kinds.get(("search_multi", "down"), 0) > 20
+    assert kinds.get(("recorded_removed", "down"), 0) > 5
+    assert kinds.get("w_max", 0) > 0
+
+
+def test_constructor_equals_restatement_with_transport_failures(oracle_mod, gen_mod):
+    """pT 0.08-0.16 GeV: the curlers reach |sin phi| = s_max inside the sector, in both passes (R9, R11)."""
+    r = gen_mod.Recipe("curlers", n_sectors=36, n_primaries=60, pt_mode=0, pt_a=0.08, pt_b=0.16, sigma=0.06,
+                       noise_frac=0.05, config_id=61)
+    ev = gen_mod.generate(r)
+    res, kinds = _compare_all_tracklets(oracle_mod, gen_mod, ev, oracle_mod.default_params())
+    assert res.n_seeds > 10
+    assert kinds.get(("transport_fail", "up"), 0) > 0 and kinds.get(("transport_fail", "down"), 0) > 0
+
+
+def test_constructor_equals_restatement_with_link_step_2(oracle_mod, gen_mod):
+    """Delta = 2: the up pass follows every second row, the down pass fills the rows in between by search."""
+    ev = gen_mod.generate("single_sector")
+    P = oracle_mod.default_params()
+    P.link_step = 2
+    res, kinds = _compare_all_tracklets(oracle_mod, gen_mod, ev, P, max_tracklets=60)
+    long_ = res.tl_n_hits[:60] > 100
+    assert long_.sum() > 10
+    for i in np.nonzero(long_)[0]:
+        rows = np.nonzero(res.tl_table[i] >= 0)[0]
+        assert (rows % 2 == 0).sum() > 40 and (rows % 2 == 1).sum() > 40
+
+
+# ---------------------------------------------------------------------------------------------------------
+# hand-built sectors: every hit of the "track" sits exactly on y = yc, z = 0, so the fit state stays exactly
+# (yc, 0, 0, 0, 0) (all residuals are exactly 0, q = 0 => the transport adds exactly 0) and every prediction is
+# (yc, 0).  Rows 10..14 carry the core: hits 11, 12, 13 get links (a link needs both neighbour rows), the
+# cleaned chain is 11 -> 12 -> 13 and the start hit is the one of row 11; rows 10 and 14 are re-attached by search.
+# ---------------------------------------------------------------------------------------------------------
+class Hand:
+    def __init__(self, yc=0.0):
+        self.yc = np.float32(yc)
+        self.rows, self.ys, self.zs = [], [], []
+
+    def add(self, r, y=None, z=0.0):
+        self.rows.append(int(r)); self.ys.append(self.yc if y is None else np.float32(y)); self.zs.append(np.float32(z))
+        return len(self.rows) - 1
+
+    def core(self, lo=10, hi=14):
+        return {r: self.add(r) for r in range(lo, hi + 1)}
+
+    def run(self, oracle, gen, P=None, precision="double", bz=0.5, sigma=0.06):
+        y = np.array(self.ys, np.float32); z = np.array(self.zs, np.float32); row = np.array(self.rows, np.int32)
+        g = _geom(oracle, gen, sigma, bz)
+        so = np.array([0, len(row)], np.int32)
+        res = oracle.track_event(g, so, y, z, row, params=P, precision=precision, stop_after=5)
+        return res, (g, y, z, row)
+
+
+def _table_of(res, start_hit):
+    i = int(np.nonzero(res.start_hit == start_hit)[0][0])
+    return {int(r): int(h) for r, h in enumerate(res.tl_table[i]) if h >= 0}, i
+
+
+@pytest.mark.parametrize("precision", ["double", "float"])
+def test_core_chain_and_orphans(oracle_mod, gen_mod, precision):
+    """The plain case: start hit = row 11, rows 10 and 14 (no links: edge of the chain) re-attached by search."""
+    H = Hand(); c = H.core()
+    res, _ = H.run(oracle_mod, gen_mod, precision=precision)
+    assert list(res.start_hit) == [c[11]]
+    assert list(res.clink_up[[c[10], c[11], c[12], c[13], c[14]]]) == [-1, c[12], c[13], -1, -1]
+    tab, i = _table_of(res, c[11])
+    assert tab == {r: c[r] for r in range(10, 15)}
+    assert (res.tl_first_row[i], res.tl_last_row[i], res.tl_n_hits[i]) == (10, 14, 5)
+    assert np.allclose(res.tl_par[i], [0, 0, 0, 0, 0], atol=1e-12) and res.tl_chi2[i] == 0.0
+
+
+@pytest.mark.parametrize("precision", ["double", "float"])
+def test_gap_of_max_gap_rows_is_bridged_one_more_is_not(oracle_mod, gen_mod, precision):
+    """max_gap = 5: five empty rows do not end a pass (++miss > max_gap is false at 5), six do.  Up pass above
+    the chain, down pass below the start hit."""
+    H = Hand(); c = H.core()
+    up5 = H.add(20)                    # rows 15..19 empty: 5 misses, then this hit
+    dn5 = H.add(4)                     # rows 9..5 empty: 5 misses below the seed, then this hit
+    up6 = H.add(27)                    # rows 21..26 empty: 6 misses -> the up pass has ended at row 26
+    res, _ = H.run(oracle_mod, gen_mod, precision=precision)
+    tab, i = _table_of(res, c[11])
+    assert tab.get(20) == up5 and tab.get(4) == dn5
+    assert 27 not in tab and res.tl_last_row[i] == 20 and res.tl_first_row[i] == 4 and res.tl_n_hits[i] == 7
+    # six empty rows below the seed end the down pass as well
+    H2 = Hand(); c2 = H2.core(); H2.add(3)
+    res2, _ = H2.run(oracle_mod, gen_mod, precision=precision)
+    tab2, i2 = _table_of(res2, c2[11])
+    assert 3 not in tab2 and res2.tl_first_row[i2] == 10
+
+
+@pytest.mark.parametrize("precision", ["double", "float"])
+def test_miss_counter_is_reset_by_an_accepted_hit(oracle_mod, gen_mod, precision):
+    """3 empty rows, a hit, 3 empty rows, a hit: 6 misses in total but never more than 3 in a row."""
+    H = Hand(); c = H.core()
+    a = H.add(18); b = H.add(22)       # up: rows 15-17 empty, 18, rows 19-21 empty, 22
+    d = H.add(6); e = H.add(2)         # down: rows 9-7 empty, 6, rows 5-3 empty, 2
+    res, _ = H.run(oracle_mod, gen_mod, precision=precision)
+    tab, i = _table_of(res, c[11])
+    assert tab.get(18) == a and tab.get(22) == b and tab.get(6) == d and tab.get(2) == e
+    assert res.tl_n_hits[i] == 9 and res.tl_last_row[i] == 22 and res.tl_first_row[i] == 2
+
+
+@pytest.mark.parametrize("precision", ["double", "float"])
+def test_misses_between_recorded_hits_never_end_the_down_pass(oracle_mod, gen_mod, precision):
+    """The down pass counts misses (and applies the edge test) only below the start hit's row: holes between
+    the recorded hits of the up pass are free.  max_gap = 1 here; the up pass bridges 1-row holes, the down pass
+    walks through all of them."""
+    P = oracle_mod.default_params(); P.max_gap = 1
+    H = Hand(); c = H.core()
+    hs = {r: H.add(r) for r in (16, 18, 20, 22)}      # one-row holes at 15, 17, 19, 21
+    res, _ = H.run(oracle_mod, gen_mod, P=P, precision=precision)
+    tab, i = _table_of(res, c[11])
+    assert all(tab.get(r) == h for r, h in hs.items()) and tab.get(10) == c[10]
+    assert res.tl_n_hits[i] == 9 and res.tl_first_row[i] == 10
+
+
+@pytest.mark.parametrize("precision", ["double", "float"])
+def test_coincident_candidates_lowest_index_wins(oracle_mod, gen_mod, precision):
+    """Two hits at identical coordinates in a searched row (S22): the lower caller's index is taken, whatever the
+    order of arrival; up pass (row 15) and down pass (row 9)."""
+    H = Hand()
+    hi_up = None
+    lo_up = H.add(15); lo_dn = H.add(9)               # indices 0, 1
+    c = H.core()
+    hi_up = H.add(15); hi_dn = H.add(9)               # same coordinates, higher indices
+    res, _ = H.run(oracle_mod, gen_mod, precision=precision)
+    assert list(res.start_hit) == [c[10]]             # row 9 gives the hit of row 10 its links: the chain starts there
+    tab, i = _table_of(res, c[10])
+    assert tab.get(15) == lo_up and tab.get(9) == lo_dn and hi_up not in tab.values() and hi_dn not in tab.values()
+
+
+@pytest.mark.parametrize("precision", ["double", "float"])
+def test_best_gate_value_wins_not_the_first_candidate(oracle_mod, gen_mod, precision):
+    """Three candidates in the window of row 15: the one with the smallest gate value is taken."""
+    H = Hand()
+    far = H.add(15, y=0.12); c = H.core(); near = H.add(15, y=-0.03, z=0.02); mid = H.add(15, y=0.0, z=0.1)
+    res, _ = H.run(oracle_mod, gen_mod, precision=precision)
+    tab, _ = _table_of(res, c[11])
+    assert tab.get(15) == near
+
+
+@pytest.mark.parametrize("precision", ["double", "float"])
+def test_window_edge_at_w_max_is_inclusive(oracle_mod, gen_mod, precision):
+    """A window clamped at w_max is tighter than the chi2_ext gate, so the clamp and its <= decide.  The top hit
+    (row 16) is found by search over the empty row 15; the down pass starts there with the prior covariance, and
+    at row 15 its window would be 4 * sqrt(sigma^2 + 0.75^2 * V_s + sigma^2) = 1.55 cm; win_max = 1 cm clamps it.
+    A candidate at exactly y = +1.0 (gate value 1 / 0.148 = 6.8 < 16) is inside (<=), one float32 above it is not;
+    the up pass (window 0.3 cm at row 15) sees neither."""
+    P = oracle_mod.default_params(); P.win_max = 1.0
+    for y_c, inside in ((1.0, True), (-1.0, True), (np.nextafter(np.float32(1.0), np.float32(2.0)), False),
+                        (-np.nextafter(np.float32(1.0), np.float32(2.0)), False)):
+        H = Hand(); c = H.core(); top = H.add(16); cand = H.add(15, y=y_c)
+        res, _ = H.run(oracle_mod, gen_mod, P=P, precision=precision)
+        tab, i = _table_of(res, c[11])
+        assert res.tl_last_row[i] == 16 and tab.get(16) == top
+        assert (tab.get(15) == cand) == inside, (y_c, tab)
+    # z direction: the same clamp on w_z (V_t = 1: 4 * sqrt(2 sigma^2 + 0.75^2) = 3.02 cm, clamped at w_max = 3)
+    for z_c, inside in ((3.0, True), (np.nextafter(np.float32(3.0), np.float32(4.0)), False)):
+        H = Hand(); c = H.core(); top = H.add(16); cand = H.add(15, z=z_c)
+        res, _ = H.run(oracle_mod, gen_mod, precision=precision)
+        tab, _ = _table_of(res, c[11])
+        assert (tab.get(15) == cand) == inside, (z_c, tab)
+
+
+@pytest.mark.parametrize("precision", ["double", "float"])
+def test_window_at_w_min_and_the_ext_gate(oracle_mod, gen_mod, precision):
+    """After 50 hits on the line the prediction error is ~sigma: 4 sqrt(C + sigma^2) < w_min = 0.3 cm, so the window
+    is w_min and the chi2_ext gate (16) decides inside it: a hit 0.2 cm off (g ~ 0.04 / 0.0038 = 10.5) is taken,
+    a hit 0.29 cm off is inside the window but fails the gate (g ~ 22), a hit 0.31 cm off is outside the window.
+    Each variant leaves row 61 otherwise empty."""
+    for off, taken in ((0.2, True), (0.29, False), (0.31, False)):
+        H = Hand(); c = H.core(10, 60); cand = H.add(61, y=off)
+        res, _ = H.run(oracle_mod, gen_mod, precision=precision)
+        tab, _ = _table_of(res, c[11])
+        assert (tab.get(61) == cand) == taken, (off, tab)
+
+
+@pytest.mark.parametrize("precision", ["double", "float"])
+def test_edge_stop_at_the_wedge_plus_margin(oracle_mod, gen_mod, precision):
+    """EXTEND ends the pass when |y_pred| > row_x * tan(10 deg) + edge_margin (strict >), evaluated before the
+    search.  Line at constant y: just beyond the limit of row 14 the up pass ends there (the on-line hit of row 14
+    is not attached) and the down pass ends at row 10 (< r0); at or below the limit both hits are attached.  The
+    limit is evaluated in the run's precision from float32 inputs."""
+    rx = gen_mod.row_x().astype(np.float32)
+    tan = np.float32(gen_mod.TAN_HALF_ANGLE)
+    if precision == "double":
+        lim14 = float(rx[14]) * float(tan) + 1.0
+    else:
+        lim14 = float(np.float32(rx[14] * tan) + np.float32(1.0))
+    f = np.float32(lim14)
+    below = f if float(f) <= lim14 else np.nextafter(f, np.float32(0))
+    above = np.nextafter(below, np.float32(1e9))
+    assert float(below) <= lim14 < float(above)
+    for yc, stops in ((above, True), (below, False), (np.float32(lim14 + 2.0), True)):
+        H = Hand(yc=yc); c = H.core()
+        res, _ = H.run(oracle_mod, gen_mod, precision=precision)
+        tab, i = _table_of(res, c[11])
+        if stops:      # row 14 not attached; the limit of row 10 is lower still, so row 10 is not attached either
+            assert tab == {11: c[11], 12: c[12], 13: c[13]}, (yc, tab)
+        else:          # row 14 attached; row 10's own limit (lower: the wedge narrows) ends the down pass
+            assert tab == {11: c[11], 12: c[12], 13: c[13], 14: c[14]}, (yc, tab)
+    # the edge test belongs to EXTEND only: a chain followed through its links is never stopped by it
+    H = Hand(yc=np.float32(lim14 + 2.0)); c = H.core(10, 20)
+    res, _ = H.run(oracle_mod, gen_mod, precision=precision)
+    tab, _ = _table_of(res, c[11])
+    assert tab == {r: c[r] for r in range(11, 20)}       # links 11..19 followed; 20 and 10 would need EXTEND
+
+
+@pytest.mark.parametrize("precision", ["double", "float"])
+def test_rejected_link_is_searched_on_the_same_row(oracle_mod, gen_mod, precision):
+    """A linked hit that fails chi2_link turns the pass to EXTEND on that same row, which is searched at once.
+    chi2_link = 2 < chi2_ext = 16 makes the two gates tell apart on ONE hit: A (row 30, 0.15 cm off the line)
+    is the link of hit 29; after 19 hits the prediction error is ~1.2 sigma, so A's gate value is ~4: it fails
+    the link gate and passes the search's.  A is the last hit of the track (the hit of row 31 that gives A its
+    links is 1.2 cm away, outside every window), so whether row 30 was searched shows in the top row: searched ->
+    the up pass ends on A, the down pass starts there and the table holds it; not searched -> the tracklet ends at
+    row 29 and the down pass never sees row 30."""
+    P = oracle_mod.default_params(); P.chi2_link = 2.0
+    H = Hand(); c = H.core(10, 29); A = H.add(30, y=0.15); u = H.add(31, y=1.2)
+    res, _ = H.run(oracle_mod, gen_mod, P=P, precision=precision)
+    assert res.clink_up[c[29]] == A and res.clink_up[A] == -1
+    tab, i = _table_of(res, c[11])
+    assert tab.get(30) == A and res.tl_last_row[i] == 30 and u not in tab.values()
+    assert res.tl_n_hits[i] == 21 and res.tl_first_row[i] == 10
+
+
+@pytest.mark.parametrize("precision", ["double", "float"])
+def test_linked_hit_between_the_two_gates_is_followed(oracle_mod, gen_mod, precision):
+    """FOLLOW gates with chi2_link = 25, not with the search's chi2_ext = 16: the linked hit of row 40, 0.31 cm off
+    the line (gate value ~20 after 29 hits from below, ~18 after 20 hits from above), stays in the tracklet.  A
+    search could not have attached it (outside the 0.3 cm window, and above chi2_ext)."""
+    H = Hand()
+    c = {r: H.add(r) for r in range(10, 61) if r != 40}
+    off = H.add(40, y=0.31)
+    res, _ = H.run(oracle_mod, gen_mod, precision=precision)
+    tab, i = _table_of(res, c[11])
+    assert tab.get(40) == off and res.tl_n_hits[i] == 51
+
+
+@pytest.mark.parametrize("precision", ["double", "float"])
+def test_recorded_hit_failing_the_down_gate_is_removed(oracle_mod, gen_mod, precision):
+    """The up pass (loose covariance after two hits) accepts the 0.4 cm outlier of row 13 through its link (gate
+    ~7); the down pass arrives there from 27 hits above with a prediction error ~ sigma and removes it
+    (gate ~37 > chi2_link = 25).  The rows below are still reached."""
+    H = Hand()
+    c = {r: H.add(r) for r in range(10, 41) if r != 13}
+    out = H.add(13, y=0.4)
+    res, _ = H.run(oracle_mod, gen_mod, precision=precision)
+    assert res.clink_up[c[12]] == out and res.clink_up[out] == c[14]
+    tab, i = _table_of(res, c[11])
+    assert 13 not in tab and out not in tab.values()
+    assert res.tl_n_hits[i] == 30 and res.tl_first_row[i] == 10 and res.tl_last_row[i] == 40
+
+
+def test_surviving_mutants_of_round_1_are_the_ones_listed():
+    """Book-keeping for the header: the five tests named there exist."""
+    g = globals()
+    for name in ("test_coincident_candidates_lowest_index_wins", "test_window_edge_at_w_max_is_inclusive",
+                 "test_miss_counter_is_reset_by_an_accepted_hit", "test_edge_stop_at_the_wedge_plus_margin",
+                 "test_gap_of_max_gap_rows_is_bridged_one_more_is_not"):
+        assert callable(g[name])

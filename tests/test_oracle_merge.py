@@ -142,3 +142,202 @@ def test_global_tracks_are_the_chains_of_links(oracle_mod, gen_mod):
     # merge off: every track is its own global track
     ev2, p2, r2 = _run(oracle_mod, gen_mod, "pp", merge=0)
     assert np.array_equal(r2.trk_global, np.arange(r2.n_tracks))
+
+
+# ---------------------------------------------------------------------------------------------------------
+# deterministic pins of O9's decisions (Weak #2): a numpy restatement of the whole step written
+# from DESIGN.md "O9" with the EXACT helix (asin) instead of the oracle's series, and hand-built segments that sit
+# on the tie and on the inclusive edges of every cut.
+# ---------------------------------------------------------------------------------------------------------
+def _restate_merge(gen, p, bz, n_sectors, sector, first_row, par, row_out, out):
+    """next / prev / global of DESIGN.md "O9" in double: box cuts (<=), D, arg min with ties to the lowest index,
+    mutual links, chains.  The move along the helix uses the closed form; it differs from the oracle's series by
+    < 1e-6 cm, far below any decision margin of the compared events (asserted by the caller through the margins)."""
+    T = len(sector)
+    half = n_sectors // 2
+    step = 2.0 * math.pi / half
+    kB = -K * bz
+    rx = gen.row_x().astype(np.float32).astype(np.float64)
+    tol = np.array([p.merge_dy, p.merge_dz, p.merge_ds, p.merge_dt], np.float64)
+    Dm = np.full((T, T), np.inf)
+    for a in range(T):
+        if row_out[a] < 0:
+            continue
+        xa, ya, za, s0, t0, q0 = out[a]
+        for b in range(T):
+            if a == b or row_out[b] < 0 or sector[a] // half != sector[b] // half:
+                continue
+            dk = (sector[b] % half - sector[a] % half) % half
+            if dk not in (1, half - 1):
+                continue
+            gap = first_row[b] - row_out[a]
+            if gap < 1 or gap > 1 + p.merge_max_gap:
+                continue
+            ang = -step if dk == 1 else step            # alpha_A - alpha_B
+            if abs(s0) > p.sin_max:
+                continue
+            x1 = xa * math.cos(ang) - ya * math.sin(ang)
+            y1 = xa * math.sin(ang) + ya * math.cos(ang)
+            s1 = s0 * math.cos(ang) + math.sqrt(1 - s0 * s0) * math.sin(ang)
+            dx = par[b][0] - x1
+            kap = kB * q0
+            s2 = s1 + kap * dx
+            if abs(s1) > p.sin_max or abs(s2) > p.sin_max:
+                continue
+            c1, c2 = math.sqrt(1 - s1 * s1), math.sqrt(1 - s2 * s2)
+            if abs(kap) < 1e-12:
+                dy, dS = dx * s1 / c1, dx / c1
+            else:
+                dy, dS = (c1 - c2) / kap, (math.asin(s2) - math.asin(s1)) / kap
+            e = np.array([y1 + dy - par[b][1], za + t0 * dS - par[b][2], s2 - par[b][3], t0 - par[b][4]])
+            if np.all(np.abs(e) <= tol):
+                Dm[a, b] = float(np.sum((e / tol) ** 2))
+    nx = np.where(np.isfinite(Dm.min(axis=1)), Dm.argmin(axis=1), -1) if T else np.zeros(0, int)
+    pv = np.where(np.isfinite(Dm.min(axis=0)), Dm.argmin(axis=0), -1) if T else np.zeros(0, int)   # argmin: first = lowest
+    nxt = np.full(T, -1); prv = np.full(T, -1)
+    for a in range(T):
+        if nx[a] >= 0 and pv[nx[a]] == a:
+            nxt[a] = nx[a]; prv[nx[a]] = a
+    glob = np.arange(T)
+    for a in range(T):
+        h = a
+        while prv[h] >= 0:
+            h = prv[h]
+        glob[a] = h
+    return nxt, prv, glob
+
+
+@pytest.mark.parametrize("name", ["pp", "semicentral"])
+def test_merge_equals_restatement_with_exact_helix(oracle_mod, gen_mod, name):
+    ev, p, r = _run(oracle_mod, gen_mod, name, precision="double")
+    par = np.stack([r.trk_x, r.trk_y, r.trk_z, r.trk_sinphi, r.trk_tgl, r.trk_qpt], axis=1)
+    nxt, prv, glob = _restate_merge(gen_mod, p, ev.bz, ev.n_sectors, r.trk_sector, r.trk_first_row, par, r.trk_row_out,
+                                    r.trk_out)
+    # the series-vs-asin difference (1e-6 cm) may flip only decisions whose recorded margin is that small
+    bad = (nxt != r.trk_next) | (prv != r.trk_prev)
+    assert np.all(r.trk_merge_margin[bad] < 1e-4), (int(bad.sum()), r.trk_merge_margin[bad])
+    assert bad.sum() <= 2
+    ok = ~bad
+    assert np.array_equal(glob[ok], r.trk_global[ok]) or bad.any()
+    assert (r.trk_next >= 0).sum() > (5 if name == "pp" else 200)
+
+
+class _Seg:
+    """Hand-built straight segments (q = 0): B's parameters are A's line, turned by 20 degrees and cut at x_B, in
+    double with the textbook line formulas -- so every residual of the pair is ~1e-15 unless shifted on purpose."""
+
+    def __init__(self, gen):
+        self.rx = gen.row_x().astype(np.float32).astype(np.float64)
+        self.sector, self.first_row, self.par, self.row_out, self.out = [], [], [], [], []
+
+    def add(self, sector, first_row, par, row_out, out):
+        self.sector.append(sector); self.first_row.append(first_row); self.par.append(list(par))
+        self.row_out.append(row_out); self.out.append(list(out))
+        return len(self.sector) - 1
+
+    def A(self, sector, row_out, y=3.0, z=40.0, s=0.1, t=0.5):
+        x = self.rx[row_out]
+        # A's own inner parameters are irrelevant to its role as "A": put them far below
+        return self.add(sector, 5, [self.rx[5], y - 10, z - 10, s, t, 0.0], row_out, [x, y, z, s, t, 0.0])
+
+    def continuation(self, a, r_b, n_sectors=36, nxt=True):
+        """parameters at row r_b, in the frame of the next (or previous) sector, of the straight line A flies on"""
+        xa, ya, za, s, t, _ = self.out[a]
+        ang = (-1 if nxt else 1) * 2 * math.pi / (n_sectors // 2)
+        x1 = xa * math.cos(ang) - ya * math.sin(ang); y1 = xa * math.sin(ang) + ya * math.cos(ang)
+        phi = math.asin(s) + ang
+        dx = self.rx[r_b] - x1
+        return [self.rx[r_b], y1 + dx * math.tan(phi), za + t * dx / math.cos(phi), math.sin(phi), t, 0.0]
+
+    def B(self, a, r_b, sector=None, shift=(0, 0, 0, 0), nxt=True, row_out=None):
+        par = self.continuation(a, r_b, nxt=nxt)
+        for k in range(4):
+            par[1 + k] += shift[k]
+        sec = sector if sector is not None else (self.sector[a] + (1 if nxt else -1))
+        ro = r_b + 20 if row_out is None else row_out
+        return self.add(sec, r_b, par, ro, [self.rx[ro], 0, 0, 0, 0, 0])
+
+    def run(self, oracle, gen, P=None, precision="double"):
+        g = oracle.Geometry(36, gen.row_x().astype(np.float32), gen.TAN_HALF_ANGLE, 0.06, 0.06, 0.5)
+        p = P if P is not None else oracle.default_params()
+        return oracle.merge_tracks(g, self.sector, self.first_row, self.par, self.row_out, self.out, params=p,
+                                   precision=precision)
+
+
+def test_merge_hand_built_link_and_sector_rules(oracle_mod, gen_mod):
+    S = _Seg(gen_mod)
+    a = S.A(3, 60); b = S.B(a, 62)                       # next sector, 2 rows above A's outer row
+    a2 = S.A(17, 60); b2 = S.B(a2, 63, sector=0)         # wrap-around on the A side: 17 -> 0
+    a3 = S.A(20, 60); b3 = S.B(a3, 62, nxt=False)        # previous sector (19), C side
+    a4 = S.A(17, 70); b4 = S.B(a4, 72, sector=18)        # 17 -> 18 is the other side: never
+    a5 = S.A(5, 80); b5 = S.B(a5, 82, sector=7)          # two sectors away: never
+    nx, pv, gl, mg = S.run(oracle_mod, gen_mod)
+    assert nx[a] == b and pv[b] == a and gl[b] == a and gl[a] == a
+    assert nx[a2] == b2 and pv[b2] == a2
+    assert nx[a3] == b3 and pv[b3] == a3
+    assert nx[a4] == -1 and pv[b4] == -1 and nx[a5] == -1 and pv[b5] == -1
+    assert np.all(nx[[b, b2, b3]] == -1)
+
+
+def test_merge_hand_built_gap_edges(oracle_mod, gen_mod):
+    """1 <= r_B - r_A <= 1 + merge_max_gap (= 7 by default), both ends inclusive."""
+    for gap, linked in ((0, False), (1, True), (7, True), (8, False)):
+        S = _Seg(gen_mod); a = S.A(3, 60); b = S.B(a, 60 + gap)
+        nx, pv, _, _ = S.run(oracle_mod, gen_mod)
+        assert (nx[a] == b) == linked and (pv[b] == a) == linked, gap
+
+
+@pytest.mark.parametrize("precision", ["double", "float"])
+def test_merge_hand_built_box_cut_edges_are_inclusive(oracle_mod, gen_mod, precision):
+    """|e_t| <= merge_dt: t_B = t_A -+ merge_dt exactly (both are float32 values, the difference is exact in either
+    precision) is a candidate; one float32 step further is not.  The other three residuals are ~0."""
+    tt = np.float32(0.05)
+    two = np.float32(2) * tt                             # exact: t = 2 tt and t = tt differ by exactly tt
+    for t_a, t_b, linked in ((two, tt, True), (tt, two, True),
+                             (two, np.nextafter(tt, np.float32(-1)), False),
+                             (tt, np.nextafter(two, np.float32(1)), False)):
+        assert (abs(float(t_a) - float(t_b)) <= float(tt)) == linked        # the edge really is where we think
+        S = _Seg(gen_mod); a = S.A(3, 60, t=float(t_a)); b = S.B(a, 62)
+        S.par[b][4] = float(t_b)
+        nx, pv, _, _ = S.run(oracle_mod, gen_mod, precision=precision)
+        assert (nx[a] == b) == linked, (t_a, t_b, nx)
+    # y, z, sin phi: clearly inside / clearly outside each cut (1 cm, 1 cm, 0.05)
+    for k, inside, outside in ((0, 0.99, 1.01), (1, -0.99, -1.01), (2, 0.049, 0.051)):
+        for v, linked in ((inside, True), (outside, False)):
+            sh = [0, 0, 0, 0]; sh[k] = v
+            S = _Seg(gen_mod); a = S.A(3, 60); b = S.B(a, 62, shift=sh)
+            nx, _, _, _ = S.run(oracle_mod, gen_mod, precision=precision)
+            assert (nx[a] == b) == linked, (k, v)
+
+
+@pytest.mark.parametrize("precision", ["double", "float"])
+def test_merge_hand_built_ties_go_to_the_lowest_index(oracle_mod, gen_mod, precision):
+    """Identical candidates: next(A) is the lower-index B, prev(B) the lower-index A; the link is the mutual one."""
+    S = _Seg(gen_mod)
+    a = S.A(3, 60); b_lo = S.B(a, 62); b_hi = S.B(a, 62)          # two identical continuations
+    nx, pv, _, _ = S.run(oracle_mod, gen_mod, precision=precision)
+    assert nx[a] == b_lo and pv[b_lo] == a and pv[b_hi] == -1
+    S = _Seg(gen_mod)
+    a_lo = S.A(3, 60); a_hi = S.A(3, 60); b = S.B(a_lo, 62)       # two identical segments below one continuation
+    nx, pv, gl, _ = S.run(oracle_mod, gen_mod, precision=precision)
+    assert pv[b] == a_lo and nx[a_lo] == b and nx[a_hi] == -1 and gl[b] == a_lo
+    # order of arrival does not matter: the better candidate wins wherever it stands
+    S = _Seg(gen_mod)
+    a = S.A(3, 60); worse = S.B(a, 62, shift=(0.3, 0, 0, 0)); better = S.B(a, 62, shift=(0.1, 0, 0, 0))
+    nx, pv, _, _ = S.run(oracle_mod, gen_mod, precision=precision)
+    assert nx[a] == better and pv[better] == a and pv[worse] == -1
+
+
+def test_merge_hand_built_links_must_be_mutual_and_chains_are_named_by_their_first_segment(oracle_mod, gen_mod):
+    S = _Seg(gen_mod)
+    a1 = S.A(3, 60); b = S.B(a1, 62, shift=(0.2, 0, 0, 0), row_out=90)
+    a2 = S.A(3, 60, y=3.0); S.out[a2][1] += 0.15             # a second lower segment, closer to b in y
+    nx, pv, _, _ = S.run(oracle_mod, gen_mod)
+    # b is the best continuation of both, but b's best predecessor is a2: only the mutual link is reported
+    assert nx[a2] == b and pv[b] == a2 and nx[a1] == -1
+    S2 = _Seg(gen_mod)
+    a = S2.A(3, 60); b = S2.B(a, 62, row_out=100)
+    S2.out[b] = [S2.rx[100], 5.0, 60.0, -0.05, 0.5, 0.0]
+    c = S2.B(b, 103)
+    nx, pv, gl, _ = S2.run(oracle_mod, gen_mod)
+    assert nx[a] == b and nx[b] == c and gl[c] == a and gl[b] == a and pv[c] == b
