@@ -62,6 +62,8 @@ typedef struct {
     float merge_dy, merge_dz;   /* cm: tolerated |dy|, |dz| between the extrapolated and the found segment */
     float merge_ds, merge_dt;   /* tolerated |d sin phi|, |d tg lambda| */
     int32_t merge_max_gap;      /* pad rows that may be missing between the two segments */
+    int32_t seed_dedup;         /* O5: 1 = a start hit already recorded by the up pass of an earlier tracklet of its
+                                 * sector is skipped (no tracklet is built from it); reading R23 */
 } oracle_params;
 
 typedef struct {
@@ -97,7 +99,7 @@ template <class R> struct Fit {
 };
 
 struct Tracklet {
-    int32_t first_row = -1, last_row = -1, n_hits = 0;
+    int32_t first_row = -1, last_row = -1, n_hits = 0;   /* n_hits = 0: no tracklet was built (O5 seed de-duplication) */
     double par[5] = {0, 0, 0, 0, 0};
     double cov[5] = {0, 0, 0, 0, 0}; /* diagonal of the covariance at x_ref */
     double chi2 = 0;
@@ -316,7 +318,7 @@ template <class R> struct Sector {
     }
 
     /* ---- O5 tracklet constructor for the start hit h0 ---- */
-    void construct(const Result& res, int32_t h0, Tracklet& T) const {
+    void construct(const Result& res, int32_t h0, Tracklet& T, std::vector<uint8_t>* used = nullptr, int32_t base = 0) const {
         Margin mg;
         std::vector<int32_t>& tab = T.table;
         tab.assign(n_rows, -1);
@@ -358,6 +360,8 @@ template <class R> struct Sector {
                 else if (++miss > P.max_gap) break;
             }
         }
+        if (used)   /* seed de-duplication: the hits this up pass recorded (sector-local index = hit - base) */
+            for (int row = r0; row <= top; row++) if (tab[row] >= 0) (*used)[tab[row] - base] = 1;
         /* down pass: fresh fit from the top recorded hit, direction and curvature from the up pass */
         int first = top;
         {
@@ -583,7 +587,16 @@ Result* run(const oracle_geometry& G, const oracle_params& P, int32_t n, const i
         S.start_hits(*res, seeds[s]);
         if (stop_after == 4) continue;
         tls[s].resize(seeds[s].size());
-        for (size_t i = 0; i < seeds[s].size(); i++) S.construct(*res, seeds[s][i], tls[s][i]);
+        {   /* O5 with seed de-duplication (R23): start hits are taken in canonical order (pad row, caller's
+               index); every hit an up pass records is marked; a start hit that is already marked builds no tracklet
+               (its track is being followed from below).  Marks come from up passes of lower rows only, so the
+               order of the start hits inside a row plays no role. */
+            std::vector<uint8_t> used(P.seed_dedup ? e - b : 0, 0);
+            for (size_t i = 0; i < seeds[s].size(); i++) {
+                if (P.seed_dedup && used[seeds[s][i] - b]) { tls[s][i].table.assign(G.n_rows, -1); continue; }
+                S.construct(*res, seeds[s][i], tls[s][i], P.seed_dedup ? &used : nullptr, b);
+            }
+        }
         if (stop_after == 5) continue;
         /* ---- O6 selector ---- */
         /* owner(hit) = tracklet with most hits, ties -> lowest canonical id, among tracklets with
@@ -682,6 +695,7 @@ void oracle_default_params(oracle_params* p) {
     p->min_tracklet_hits = 10; p->min_track_hits = 10;
     p->refit = 0;
     p->merge = 0; p->merge_dy = 1.0f; p->merge_dz = 1.0f; p->merge_ds = 0.05f; p->merge_dt = 0.05f; p->merge_max_gap = 6;
+    p->seed_dedup = 1;
 }
 
 /* precision: 0 = double, 1 = strict float32.  stop_after: 0 = everything, 2 = after O2, 4 = after O4,

@@ -103,6 +103,7 @@ def restate_construct(oracle, g, P, rx, y, z, row, hits_of_row, clink_up, h0):
             miss += 1
             if miss > int(P.max_gap):
                 trace.append(dict(kind="gap", pas="up", row=r)); break
+    up_hits = [h for h in tab if h >= 0]                 # what the up pass recorded (seed de-duplication, R23)
     # ---- down pass: fresh fit at the top recorded hit, direction and curvature of the up pass ----
     ht = tab[top]
     st = np.array([y[ht], z[ht], snap[2], snap[3], snap[4]]); cv = prior.copy(); chi2 = 0.0; n = 1
@@ -139,7 +140,8 @@ def restate_construct(oracle, g, P, rx, y, z, row, hits_of_row, clink_up, h0):
         r -= 1
     while r >= 0:                                        # rows the pass never reached keep nothing
         tab[r] = -1; r -= 1
-    return dict(table=np.array(tab, np.int32), first=first, last=top, n=res[2], par=res[0], chi2=res[1]), trace
+    return dict(table=np.array(tab, np.int32), first=first, last=top, n=res[2], par=res[0], chi2=res[1],
+                up_hits=up_hits), trace
 
 
 def _rows_index(row, lo, hi):
@@ -155,11 +157,22 @@ def _compare_all_tracklets(oracle, gen, ev, P, max_tracklets=None, every=1):
     so = ev.sector_offset
     hor_s = [_rows_index(ev.row, int(so[s]), int(so[s + 1])) for s in range(ev.n_sectors)]
     kinds = {}
-    ids = range(0, res.n_seeds, every) if max_tracklets is None else range(min(res.n_seeds, max_tracklets))
-    for i in ids:
+    n_ids = res.n_seeds if max_tracklets is None else min(res.n_seeds, max_tracklets)
+    # seed de-duplication (R23), restated: start hits in canonical order; a start hit that an earlier up
+    # pass of its sector recorded builds no tracklet.  (Sectors never share hits, so one set serves all.)
+    used = set()
+    for i in range(n_ids):
         h0 = int(res.start_hit[i])
+        if int(P.seed_dedup) and h0 in used:
+            assert res.tl_n_hits[i] == 0 and np.all(res.tl_table[i] == -1), i
+            kinds["skipped"] = kinds.get("skipped", 0) + 1
+            continue
         hor = hor_s[int(np.searchsorted(so, h0, side="right")) - 1]
         T, trace = restate_construct(oracle, g, P, rx, y, z, ev.row, hor, res.clink_up, h0)
+        used.update(T["up_hits"])
+        if i % every:
+            assert res.tl_n_hits[i] > 0
+            continue
         assert np.array_equal(T["table"], res.tl_table[i]), (i, np.nonzero(T["table"] != res.tl_table[i]))
         assert (T["first"], T["last"], T["n"]) == (res.tl_first_row[i], res.tl_last_row[i], res.tl_n_hits[i]), i
         assert np.allclose(T["par"], res.tl_par[i], rtol=1e-12, atol=1e-13), (i, T["par"], res.tl_par[i])
@@ -179,23 +192,29 @@ def _compare_all_tracklets(oracle, gen, ev, P, max_tracklets=None, every=1):
     return res, kinds
 
 
-def test_constructor_equals_restatement_on_config_1(oracle_mod, gen_mod):
-    """Every tracklet of BASELINE.json config 1 (50 tracks, 2 % holes, 5 % noise): tables, rows, parameters."""
+@pytest.mark.parametrize("dedup", [1, 0])
+def test_constructor_equals_restatement_on_config_1(oracle_mod, gen_mod, dedup):
+    """Every tracklet of BASELINE.json config 1 (50 tracks, 2 % holes, 5 % noise): tables, rows, parameters; with
+    the seed de-duplication (which start hits build a tracklet) and without."""
     ev = gen_mod.generate("single_sector")
-    res, kinds = _compare_all_tracklets(oracle_mod, gen_mod, ev, oracle_mod.default_params())
+    P = oracle_mod.default_params(); P.seed_dedup = dedup
+    res, kinds = _compare_all_tracklets(oracle_mod, gen_mod, ev, P)
     assert res.n_seeds > 60
+    built = int((res.tl_n_hits > 0).sum())
+    assert (built == res.n_seeds) if not dedup else (47 <= built <= 60 and kinds["skipped"] == res.n_seeds - built)
     # the branches this workload must have gone through
-    assert kinds[("search_hit", "up")] > 100 and kinds[("search_hit", "down")] > 100
-    assert kinds[("gap", "up")] + kinds.get(("edge", "up"), 0) > 10
+    assert kinds[("search_hit", "up")] > 100 and kinds[("search_hit", "down")] > 50
+    assert kinds[("gap", "up")] + kinds.get(("edge", "up"), 0) > 3
     assert kinds["w_min"] > 1000
 
 
 def test_constructor_equals_restatement_on_a_dense_sector(oracle_mod, gen_mod):
     """150 tracks in one sector (central Pb-Pb-like occupancy, sigma 0.08, 50 % noise): windows with several
-    candidates, rejected links, recorded hits removed by the down pass.  Every 4th tracklet."""
+    candidates, rejected links, recorded hits removed by the down pass; two thirds of the start hits are skipped
+    by the seed de-duplication."""
     ev = gen_mod.tiny_sector(n_tracks=150, seed=11, noise_frac=0.5, sigma=0.08)
-    res, kinds = _compare_all_tracklets(oracle_mod, gen_mod, ev, oracle_mod.default_params(), every=4)
-    assert res.n_seeds > 400
+    res, kinds = _compare_all_tracklets(oracle_mod, gen_mod, ev, oracle_mod.default_params())
+    assert res.n_seeds > 400 and kinds["skipped"] > 200 and (res.tl_n_hits > 0).sum() < 250
     assert kinds.get(("search_multi", "up"), 0) > 20 and kinds.get(("search_multi", "down"), 0) > 20
     assert kinds.get(("recorded_removed", "down"), 0) > 5
     assert kinds.get("w_max", 0) > 0

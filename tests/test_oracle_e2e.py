@@ -18,13 +18,16 @@ def test_tracklet_tables_are_consistent(event_and_oracle, name):
     assert np.array_equal(has.sum(axis=1), res.tl_n_hits)
     rows = np.arange(NR)[None, :]
     first = np.where(has, rows, NR).min(axis=1); last = np.where(has, rows, -1).max(axis=1)
-    assert np.array_equal(first, res.tl_first_row) and np.array_equal(last, res.tl_last_row)
+    built = res.tl_n_hits > 0       # a start hit skipped by the seed de-duplication (R23) builds nothing
+    assert np.array_equal(first[built], res.tl_first_row[built]) and np.array_equal(last[built], res.tl_last_row[built])
+    assert np.all(res.tl_first_row[~built] == -1) and np.all(res.tl_last_row[~built] == -1)
+    assert 0.15 * S < built.sum() < 0.75 * S
     # a table entry of row r is a hit of row r in the seed's sector
     ti, ri = np.nonzero(has)
     assert np.array_equal(ev.row[tab[ti, ri]], ri)
     seed_sector = np.repeat(np.arange(ev.n_sectors), np.diff(res.seed_offset))
     assert np.array_equal(sector[tab[ti, ri]], seed_sector[ti])
-    assert np.all(res.tl_n_hits >= 1)
+    assert np.all(res.tl_n_hits[built] >= 1)
     assert np.all(np.isfinite(res.tl_par))
     good = res.tl_n_hits >= 10          # a 2-3 hit stub may end on an update that pushes |sin phi| past 1
     assert np.all(np.abs(res.tl_par[good, 2]) < 1.0)
