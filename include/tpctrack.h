@@ -58,7 +58,7 @@ typedef struct {
     float var_s, var_t, var_q;  /* prior variances of sin phi, tg lambda, q/pT */
     float chi2_link, chi2_ext;  /* 2-dof gates: following a link / attaching a searched hit */
     float win_nsigma, win_min, win_max; /* search window = clamp(n * sqrt(C + sigma^2), min, max) cm */
-    int32_t max_gap;            /* consecutive rows without a hit before a pass ends */
+    int32_t max_gap;            /* consecutive rows without a hit before a pass ends, 0..60 */
     float edge_margin;          /* cm beyond the wedge edge before a pass ends */
     int32_t min_tracklet_hits;  /* tracklets with fewer hits do not take part in the selection */
     int32_t min_track_hits;     /* tracks keeping fewer owned hits are dropped */
@@ -73,6 +73,9 @@ typedef struct {
     float merge_dy, merge_dz;   /* cm: tolerated |dy|, |dz| between the extrapolated and the found segment */
     float merge_ds, merge_dt;   /* tolerated |d sin phi|, |d tg lambda| */
     int32_t merge_max_gap;      /* pad rows that may be missing between the two segments */
+    int32_t seed_dedup;         /* 1 (default): a start hit that the up pass of a tracklet built from a lower pad row of
+                                 * its sector has already recorded builds no tracklet (R23).
+                                 * 0: every start hit is fitted (round-1 behaviour, ~3 tracklets per output track) */
 } tpc_params;
 
 /* One event's clusters: SoA, grouped by sector, ANY order inside a sector.
@@ -131,7 +134,7 @@ typedef struct {
 typedef struct {
     int64_t n_events, n_clusters;
     int64_t n_links;         /* hits with a cleaned up-link */
-    int64_t n_seeds;         /* start hits = tracklets constructed */
+    int64_t n_seeds;         /* start hits (with seed_dedup only part of them build a tracklet: n_tracklets) */
     int64_t n_row_visits;    /* Kalman transport steps taken by the constructor */
     int64_t n_tracklet_hits; /* hits in tracklets entering the selection */
     int64_t n_tracks, n_track_hits;
@@ -139,6 +142,7 @@ typedef struct {
     int64_t n_retries;       /* internal re-runs after growing a pool */
     int64_t n_updates;       /* Kalman updates (accepted measurements, both passes) */
     int64_t n_refit_visits;  /* row visits of the refit (0 when tpc_params.refit is 0) */
+    int64_t n_tracklets;     /* tracklets constructed (start hits not skipped by the seed de-duplication) */
 } tpc_counters;
 
 typedef struct tpc_tracker tpc_tracker;

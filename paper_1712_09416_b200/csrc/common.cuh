@@ -19,11 +19,12 @@ constexpr uint16_t kNoHit = 0xffffu;  // empty entry of a tracklet's row -> hit 
 constexpr unsigned kFull = 0xffffffffu;
 
 // error bits raised by kernels
-constexpr unsigned kErrBadRow = 1u, kErrRowCapacity = 2u, kErrSeedCapacity = 4u, kErrHang = 8u, kErrSelCapacity = 16u;
+constexpr unsigned kErrBadRow = 1u, kErrRowCapacity = 2u, kErrSeedCapacity = 4u, kErrHang = 8u, kErrSelCapacity = 16u,
+                   kErrSlotCapacity = 32u;   // K5: more tracklets under way in a sector task than state slots
 
 // device counters (unsigned long long each)
-constexpr int kNCursors = 4;           // work cursors: up sweep, down sweep, refit
-enum { CNT_ERR = 0, CNT_LINKS, CNT_ROW_VISITS, CNT_TL_HITS, CNT_TRACKS, CNT_TRACK_HITS, CNT_UPDATES, CNT_REFIT_VISITS, CNT_N };
+constexpr int kNCursors = 4;           // work cursors: [0] K5 sector tasks, [2] refit
+enum { CNT_ERR = 0, CNT_LINKS, CNT_ROW_VISITS, CNT_TL_HITS, CNT_TRACKS, CNT_TRACK_HITS, CNT_UPDATES, CNT_REFIT_VISITS, CNT_TRACKLETS, CNT_N };
 
 // One event's input arrays (device pointers) and its place in the batch-global cluster numbering.
 struct EventSrc {
@@ -80,9 +81,8 @@ struct View {
     float* tl_par;           // [6][S_cap] y z s t q chi2
     SeedRec* seed_rec;       // [S_cap] start hit and its up-link: coordinates and sorted indices (K4 -> K5 up sweep)
     UpRec* tl_up;            // [S_cap] what the up pass hands to the down pass, by tracklet
-    UpRec* dn_rec;           // [S_cap] the same records ordered by (task, top row)
-    int32_t *dn_count, *dn_start, *dn_fill;   // [n_bins+1] tracklets per (task, top row)
-    int32_t kf_K;            // CTAs sharing the start hits of one sector task
+    UpRec* dn_rec;           // [S_cap] K5 scratch: per task, the list of parked tracklets (id in task | top row << 24)
+    int32_t *dn_count, *dn_start, *dn_fill;   // [n_bins+1] O9: refitted tracks per (task, first fitted row)
     // K6
     uint32_t* owner;         // [N] best key among tracklets holding the hit
     int32_t* tl_nown;        // [S_cap+1] hits owned (0 when the track is dropped)
@@ -104,7 +104,7 @@ struct View {
     int32_t *o_next, *o_prev;   // [S_cap] O9 links, event-local track index or -1
     int32_t* o_global;          // [S_cap] first segment of the chain a track belongs to, event-local
     unsigned long long* cnt; // [CNT_N]
-    unsigned long long* kf_cursor;  // [kNCursors] units of work handed out: [0] up sweep, [1] down sweep, [2] refit
+    unsigned long long* kf_cursor;  // [kNCursors] units of work handed out: [0] K5 sector tasks, [2] refit
 };
 
 __device__ __forceinline__ int lane_id() { return threadIdx.x & 31; }

@@ -1,0 +1,534 @@
+// kf_construct.cuh -- K5 tracklet constructor: one CTA per sector task, pad rows in lock step, tracklet states in
+// shared memory, row data staged by TMA bulk copies.
+//
+// A CTA takes a sector task and sweeps its pad rows twice: upwards for the up passes, then downwards for the down
+// passes.  A producer warp streams the rows -- hits and grid cell table of row r, one
+// cp.async.bulk each, completion on an mbarrier -- through a ring of kCtRing shared-memory slots.  The Kalman
+// state of every tracklet under way (31 words) lives in a shared-memory slot; at each row the 13 consumer warps
+// take the occupied slots 32 at a time, load the states, advance them by that row (transport, linked / recorded hit
+// or window search in the staged row, update) and store them back.  All tracklets of the task are therefore at the
+// same row at the same time, which is what the seed de-duplication needs (R23): an up pass marks every
+// hit it records in a per-row bitmap; after a barrier the start hits of that row are taken in, and those already
+// marked build no tracklet.  A tracklet whose up pass has ended is parked (its top hit and direction, 32 bytes);
+// the down sweep picks it up at its top row.  Nothing depends on which warp or slot a tracklet lands in.
+//
+// The arithmetic is that of kf_kernels.cuh (fit_transport / fit_update), so every decision is the one DESIGN.md
+// "O5" describes.
+#pragma once
+#include "common.cuh"
+#include "kf_kernels.cuh"
+
+namespace tpc {
+
+#ifndef TPC_CT_WARPS
+#define TPC_CT_WARPS 13
+#endif
+#ifndef TPC_CT_RING
+#define TPC_CT_RING 3
+#endif
+constexpr int kCtWarps = TPC_CT_WARPS;                 // consumer warps of a CTA (one more warp produces)
+constexpr int kCtConsumers = kCtWarps * 32;
+constexpr int kCtThreads = (kCtWarps + 1) * 32;
+constexpr int kCtRing = TPC_CT_RING;                   // rows in flight
+constexpr int kCtWords = 31;                           // 4-byte words of a tracklet's state
+// State slots per sector task = tracklets under way at once, in three tiers (the host moves up one tier when a
+// launch reports kErrSlotCapacity and stays there): shared-memory slots + slots in global memory (L2)
+constexpr int kCtTiers = 3;
+constexpr int kCtCapSmem[kCtTiers] = {512, 1472, 1344};   // tier 0: two CTAs per SM; tiers 1, 2: one
+constexpr int kCtCapSpill[kCtTiers] = {0, 0, 4096};
+constexpr int kCtCapMax = 1344 + 4096;
+constexpr int kSwCap = 640;                            // hits of a row staged in shared memory; larger rows are read in place
+constexpr int kSwHitBytes = (kSwCap + 2) * 8;          // + alignment slack of the bulk copy (16-byte granules)
+constexpr int kSwCellEntries = kCellsPerHit * kSwCap + kCellPad + 16;
+constexpr int kSwCellBytes = kSwCellEntries * 2;
+static_assert(kSwHitBytes % 16 == 0 && kSwCellBytes % 16 == 0, "bulk copies are 16-byte granular");
+constexpr int kCtDown = 0x100;                         // cmd flag: the row belongs to the down sweep
+
+struct __align__(16) SeedRec { float y0, z0, y1, z1; int32_t h0, h1, pad0, pad1; };   // start hit, its up-link
+struct __align__(16) UpRec { float y, z, s, t, q; int32_t r0, top, id; };             // what the up pass hands down
+
+struct __align__(128) CtSmem {
+    BinDesc desc[TPC_MAX_ROWS + 1];                    // the task's row descriptors
+    unsigned char hits[kCtRing][kSwHitBytes];
+    unsigned char cells[kCtRing][kSwCellBytes];
+    int32_t lo[TPC_MAX_ROWS + 1];                      // first start hit of each row in the canonical list
+    int32_t cnt[TPC_MAX_ROWS + 1];                     // start hits of the row
+    uint32_t used[2][TPC_MAX_ROW_HITS / 32];           // hits of the row at hand recorded by an up pass (double buffered)
+    uint32_t occ[(kCtCapMax + 31) / 32];               // occupied state slots
+    unsigned long long full[kCtRing], empty[kCtRing], tbar;
+    int32_t cmd[kCtRing];                              // row held by the ring slot (| kCtDown); -1 = no more work
+    int32_t task, abort, n_free, n_hw, n_parked, top_max, i0;
+};
+
+// ---- mbarrier / bulk-copy wrappers (PTX ISA: mbarrier, cp.async.bulk) ----
+__device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
+__device__ __forceinline__ void mbar_init(unsigned long long* b, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(b)), "r"(count));
+}
+__device__ __forceinline__ void mbar_arrive(unsigned long long* b) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(b)) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive_expect_tx(unsigned long long* b, uint32_t bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(b)), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ bool mbar_try_wait(unsigned long long* b, uint32_t parity) {
+    uint32_t ok;
+    asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n selp.u32 %0, 1, 0, p;\n}"
+                 : "=r"(ok) : "r"(smem_u32(b)), "r"(parity) : "memory");
+    return ok != 0;
+}
+// try_wait that lets the hardware suspend the warp for up to `ns` before it answers
+__device__ __forceinline__ bool mbar_try_wait_hint(unsigned long long* b, uint32_t parity, uint32_t ns) {
+    uint32_t ok;
+    asm volatile("{\n .reg .pred p;\n mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n selp.u32 %0, 1, 0, p;\n}"
+                 : "=r"(ok) : "r"(smem_u32(b)), "r"(parity), "r"(ns) : "memory");
+    return ok != 0;
+}
+// bounded wait: a lost signal ends the kernel with kErrHang instead of hanging the device
+__device__ __forceinline__ bool mbar_wait(unsigned long long* b, uint32_t parity, volatile int32_t* abort) {
+    if (mbar_try_wait(b, parity)) return true;
+    for (unsigned n = 0; n < (1u << 17); n++) {   // a waiting warp issues nothing until the phase completes or the hint runs out
+        if (mbar_try_wait_hint(b, parity, 20000u)) return true;
+        if ((n & 63u) == 63u && *abort) return false;
+    }
+    *abort = 1;
+    return false;
+}
+__device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t bytes, unsigned long long* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+// barrier of the consumer warps only (the producer never joins)
+__device__ __forceinline__ void ct_bar() { asm volatile("bar.sync 1, %0;" ::"n"(kCtConsumers) : "memory"); }
+
+__device__ __forceinline__ size_t cell_index(int base, int bin) { return (size_t)kCellsPerHit * base + (size_t)bin * kCellPad; }
+
+// ---------------------------------------------------------------------------------------------------------
+// producer warp: hands the CTA its sector tasks and streams their rows, up then down
+// ---------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void ct_producer(const View& v, const Const& c, CtSmem& sm, uint16_t* freel, int cap) {
+    const int lane = lane_id();
+    const int nr = c.n_rows;
+    volatile int32_t* const abort = &sm.abort;
+    uint32_t it = 0, tphase = 0;
+    bool ok = true;
+    // lane 0: one row into the ring
+    auto issue = [&](int row, int flag, int tb) {
+        const int s = (int)(it % kCtRing);
+        if (!(ok = mbar_wait(&sm.empty[s], ((it / kCtRing) & 1u) ^ 1u, abort))) return;
+        sm.cmd[s] = row | flag;
+        const BinDesc& d = sm.desc[row];
+        if (d.n > 0 && d.n <= kSwCap) {
+            const int offh = d.base & 1;
+            const uint32_t hb = (uint32_t)((offh + d.n + 1) & ~1) * 8u;
+            const size_t g = cell_index(d.base, tb + row);
+            const int offc = (int)(g & 7);
+            const uint32_t cb = ((uint32_t)(offc + d.ny * d.nz + 1) * 2u + 15u) & ~15u;
+            mbar_arrive_expect_tx(&sm.full[s], hb + cb);
+            bulk_g2s(sm.hits[s], v.shit + (d.base - offh), hb, &sm.full[s]);
+            bulk_g2s(sm.cells[s], v.cells + (g - offc), cb, &sm.full[s]);
+        } else {
+            mbar_arrive(&sm.full[s]);
+        }
+        it++;
+    };
+    // lane 0: wait until the consumers are through with everything issued so far
+    auto drain = [&]() {
+        for (uint32_t j = it > (uint32_t)kCtRing ? it - kCtRing : 0; ok && j < it; j++)
+            ok = mbar_wait(&sm.empty[j % kCtRing], (j / kCtRing) & 1u, abort);
+    };
+    auto reset_slots = [&]() {   // the consumers are idle: all state slots are free again, lowest on top
+        for (int k = lane; k < cap; k += 32) freel[k] = (uint16_t)(cap - 1 - k);
+        for (int k = lane; k < (kCtCapMax + 31) / 32; k += 32) sm.occ[k] = 0u;
+        if (lane == 0) { sm.n_free = cap; sm.n_hw = 0; }
+    };
+    while (ok) {
+        int task = 0;
+        if (lane == 0) task = (int)atomicAdd(&v.kf_cursor[0], 1ull);
+        task = __shfl_sync(kFull, task, 0);
+        if (task >= v.n_tasks) break;
+        const int tb = task * nr;
+        // the consumers are idle here (start of the kernel, or the ring drained): the task's tables may be replaced
+        if (lane == 0) {
+            mbar_arrive_expect_tx(&sm.tbar, (uint32_t)nr * 32u);
+            bulk_g2s(sm.desc, v.desc + tb, (uint32_t)nr * 32u, &sm.tbar);
+            sm.task = task; sm.n_parked = 0; sm.top_max = -1; sm.i0 = v.seed_start[tb];
+        }
+        int f = nr;
+        for (int r = lane; r < nr; r += 32) {
+            const int lo = v.seed_start[tb + r], n = v.seed_start[tb + r + 1] - lo;
+            sm.lo[r] = lo; sm.cnt[r] = n;
+            if (n > 0) f = min(f, r);
+        }
+        for (int k = lane; k < 2 * (TPC_MAX_ROW_HITS / 32); k += 32) (&sm.used[0][0])[k] = 0u;
+        reset_slots();
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) f = min(f, __shfl_xor_sync(kFull, f, o));
+        if (lane == 0) ok = mbar_wait(&sm.tbar, tphase, abort);
+        tphase ^= 1u;
+        ok = __shfl_sync(kFull, (int)ok, 0) != 0;
+        __syncwarp();
+        if (!ok || f >= nr) continue;
+        if (lane == 0) {   // up sweep
+            for (int row = f; ok && row < nr; row++) issue(row, 0, tb);
+            drain();
+        }
+        ok = __shfl_sync(kFull, (int)ok, 0) != 0;
+        it = __shfl_sync(kFull, it, 0);
+        __syncwarp();
+        if (!ok) break;
+        reset_slots();
+        __syncwarp();
+        if (lane == 0) {   // down sweep from the highest top row
+            const int tm = *(volatile int32_t*)&sm.top_max;
+            for (int row = tm; ok && row >= 0; row--) issue(row, kCtDown, tb);
+            drain();
+        }
+        ok = __shfl_sync(kFull, (int)ok, 0) != 0;
+        it = __shfl_sync(kFull, it, 0);
+        __syncwarp();
+    }
+    if (lane == 0) {
+        const int s = (int)(it % kCtRing);
+        if (ok) ok = mbar_wait(&sm.empty[s], ((it / kCtRing) & 1u) ^ 1u, abort);
+        sm.cmd[s] = -1;
+        mbar_arrive(&sm.full[s]);
+        if (!ok) atomicOr((unsigned int*)&v.cnt[CNT_ERR], kErrHang);
+    }
+}
+
+// ---------------------------------------------------------------------------------------------------------
+// window search in one row: min gate value, exact ties -> lowest caller's index
+// hits / cs point to the row's hits and cell table (shared memory, or global for an oversized row)
+// ---------------------------------------------------------------------------------------------------------
+__device__ __forceinline__ int sweep_search(const View& v, const Const& c, const Fit& f, const float4& gf, const int4& dn,
+                                            const float2* hits, const uint16_t* cs, float iwy, float iwz, float& ay,
+                                            float& az, float& bg) {
+    const float wy = fminf(fmaxf(c.p.win_nsigma * sqrtf(f.c00 + c.sigma_y2), c.p.win_min), c.p.win_max);
+    const float wz = fminf(fmaxf(c.p.win_nsigma * sqrtf(f.c11 + c.sigma_z2), c.p.win_min), c.p.win_max);
+    const CellWin w = cell_window(gf, dn.z, dn.w, f.y, f.z, wy, wz);
+    int bp = -1;
+    bg = __int_as_float(0x7f800000);   // +inf: the first hit inside the window always wins
+    for (int iz = w.iz0; iz <= w.iz1; iz++) {
+        int p = cs[iz * dn.z + w.iy0];
+        const int pe = cs[iz * dn.z + w.iy1 + 1];
+        for (; p < pe; p++) {
+            const float2 h = hits[p];
+            const float ry = h.x - f.y, rz = h.y - f.z;
+            if (fabsf(ry) <= wy && fabsf(rz) <= wz) {
+                const float gv = (ry * ry) * iwy + (rz * rz) * iwz;   // the gate value of h
+                bool take = gv < bg;
+                if (gv == bg) take = v.sorig[dn.x + p] < v.sorig[dn.x + bp];   // exact tie (gv is finite: bp >= 0 here)
+                if (take) { bg = gv; bp = p; }
+            }
+        }
+    }
+    if (bp >= 0) { const float2 h = hits[bp]; ay = h.x; az = h.y; }
+    return bp;
+}
+
+// ---- a tracklet's state in its shared-memory slot: word k of slot s sits at st[k * cap + s] ----
+struct CtTrk {
+    Fit f;
+    float p0, p1, p2, p3, p4, p5;   // state right after the last accepted update
+    int i;                          // tracklet = canonical start-hit number (batch-global)
+    int cur;                        // up: the linked hit to come; down: table entry of the row below (read one row ahead)
+    int ph, miss, r0, top, aux;     // ph 1 up/follow, 2 up/extend, 3 down; aux: up = row of cur, down = first row
+};
+__device__ __forceinline__ void ct_load(CtTrk& t, const float* S, int cap) {
+    Fit& f = t.f;
+    f.y = S[0]; f.z = S[cap]; f.s = S[2 * cap]; f.t = S[3 * cap]; f.q = S[4 * cap];
+    f.c00 = S[5 * cap]; f.c10 = S[6 * cap]; f.c11 = S[7 * cap]; f.c20 = S[8 * cap]; f.c21 = S[9 * cap];
+    f.c22 = S[10 * cap]; f.c30 = S[11 * cap]; f.c31 = S[12 * cap]; f.c32 = S[13 * cap]; f.c33 = S[14 * cap];
+    f.c40 = S[15 * cap]; f.c41 = S[16 * cap]; f.c42 = S[17 * cap]; f.c43 = S[18 * cap]; f.c44 = S[19 * cap];
+    f.chi2 = S[20 * cap]; f.n = __float_as_int(S[21 * cap]);
+    t.p0 = S[22 * cap]; t.p1 = S[23 * cap]; t.p2 = S[24 * cap]; t.p3 = S[25 * cap]; t.p4 = S[26 * cap]; t.p5 = S[27 * cap];
+    t.i = __float_as_int(S[28 * cap]); t.cur = __float_as_int(S[29 * cap]);
+    const uint32_t pk = __float_as_uint(S[30 * cap]);
+    t.ph = pk & 3u; t.miss = (pk >> 2) & 63u; t.r0 = (pk >> 8) & 255u; t.top = (pk >> 16) & 255u; t.aux = pk >> 24;
+}
+__device__ __forceinline__ void ct_store(const CtTrk& t, float* S, int cap) {
+    const Fit& f = t.f;
+    S[0] = f.y; S[cap] = f.z; S[2 * cap] = f.s; S[3 * cap] = f.t; S[4 * cap] = f.q;
+    S[5 * cap] = f.c00; S[6 * cap] = f.c10; S[7 * cap] = f.c11; S[8 * cap] = f.c20; S[9 * cap] = f.c21;
+    S[10 * cap] = f.c22; S[11 * cap] = f.c30; S[12 * cap] = f.c31; S[13 * cap] = f.c32; S[14 * cap] = f.c33;
+    S[15 * cap] = f.c40; S[16 * cap] = f.c41; S[17 * cap] = f.c42; S[18 * cap] = f.c43; S[19 * cap] = f.c44;
+    S[20 * cap] = f.chi2; S[21 * cap] = __int_as_float(f.n);
+    S[22 * cap] = t.p0; S[23 * cap] = t.p1; S[24 * cap] = t.p2; S[25 * cap] = t.p3; S[26 * cap] = t.p4; S[27 * cap] = t.p5;
+    S[28 * cap] = __int_as_float(t.i); S[29 * cap] = __int_as_float(t.cur);
+    S[30 * cap] = __uint_as_float((uint32_t)t.ph | ((uint32_t)t.miss << 2) | ((uint32_t)t.r0 << 8) | ((uint32_t)t.top << 16) |
+                                  ((uint32_t)t.aux << 24));
+}
+
+// take `need` state slots for the lanes that ask; -1 when the task has more tracklets under way than slots
+__device__ __forceinline__ int ct_pop(const View& v, CtSmem& sm, const uint16_t* freel, bool need, int cap) {
+    const unsigned m = __ballot_sync(kFull, need);
+    if (!m) return -1;
+    int old = 0;
+    if (lane_id() == 0) old = atomicSub(&sm.n_free, __popc(m));
+    old = __shfl_sync(kFull, old, 0);
+    if (!need) return -1;
+    const int idx = old - 1 - __popc(m & lanemask_lt());
+    if (idx < 0 || idx >= cap) { atomicOr((unsigned int*)&v.cnt[CNT_ERR], kErrSlotCapacity); return -1; }
+    const int slot = freel[idx];
+    atomicOr(&sm.occ[slot >> 5], 1u << (slot & 31));
+    atomicMax(&sm.n_hw, slot + 1);
+    return slot;
+}
+__device__ __forceinline__ void ct_push(CtSmem& sm, uint16_t* freel, int slot, int cap) {
+    atomicAnd(&sm.occ[slot >> 5], ~(1u << (slot & 31)));
+    const int idx = atomicAdd(&sm.n_free, 1);
+    if (idx >= 0 && idx < cap) freel[idx] = (uint16_t)slot;
+}
+// slot -> where its state lives: the first cap_s slots in shared memory, the others in this CTA's stretch of
+// global memory (both multiples of 32, so a warp's 32 slots are all of one kind)
+struct CtSlots {
+    float* st; float* gs; int cap_s, cap_g;
+    __device__ __forceinline__ void load(CtTrk& t, int slot) const {
+        if (slot < cap_s) ct_load(t, st + slot, cap_s); else ct_load(t, gs + (slot - cap_s), cap_g);
+    }
+    __device__ __forceinline__ void store(const CtTrk& t, int slot) const {
+        if (slot < cap_s) ct_store(t, st + slot, cap_s); else ct_store(t, gs + (slot - cap_s), cap_g);
+    }
+};
+
+// ---------------------------------------------------------------------------------------------------------
+// K5
+// ---------------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(kCtThreads, 2) k_construct(const View v, const __grid_constant__ Const c, const int cap_s,
+                                                             const int cap_g, float* const spill) {
+    extern __shared__ __align__(128) unsigned char ct_raw[];
+    CtSmem& sm = *reinterpret_cast<CtSmem*>(ct_raw);
+    const int cap = cap_s + cap_g;
+    CtSlots sl;
+    sl.st = reinterpret_cast<float*>(ct_raw + sizeof(CtSmem)); sl.cap_s = cap_s; sl.cap_g = cap_g;
+    sl.gs = spill + (size_t)blockIdx.x * kCtWords * cap_g;
+    uint16_t* const freel = reinterpret_cast<uint16_t*>(sl.st + (size_t)kCtWords * cap_s);   // stack of free slots
+    const int warp = threadIdx.x >> 5, lane = lane_id();
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < kCtRing; s++) { mbar_init(&sm.full[s], 1); mbar_init(&sm.empty[s], kCtWarps); }
+        mbar_init(&sm.tbar, 1);
+        sm.abort = 0;
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    if (warp == kCtWarps) { ct_producer(v, c, sm, freel, cap); return; }
+
+    const int nr = c.n_rows, D = c.p.link_step;
+    const int ctid = threadIdx.x;                       // consumer threads are 0 .. kCtConsumers-1
+    const int S = min(v.seed_start[v.n_bins], v.S_cap);
+    const bool dedup = c.p.seed_dedup != 0;
+    volatile int32_t* const abort = &sm.abort;
+    unsigned visits = 0, updates = 0, built = 0;
+    uint32_t it = 0;
+
+    for (;;) {
+        const int s = (int)(it % kCtRing);
+        if (!mbar_wait(&sm.full[s], (it / kCtRing) & 1u, abort)) break;
+        const int cmd = sm.cmd[s];
+        if (cmd < 0) break;
+        const int row = cmd & 0xff;
+        const bool up = !(cmd & kCtDown);
+        const int tb = sm.task * nr;
+        const BinDesc& dsc = sm.desc[row];
+        const int4 dn = make_int4(dsc.base, dsc.n, dsc.ny, dsc.nz);
+        const bool staged = dn.y <= kSwCap;
+        const size_t cg = cell_index(dn.x, tb + row);
+        const float2* const hits = staged ? reinterpret_cast<const float2*>(sm.hits[s]) + (dn.x & 1) : v.shit + dn.x;
+        const uint16_t* const cs = staged ? reinterpret_cast<const uint16_t*>(sm.cells[s]) + (cg & 7) : v.cells + cg;
+        uint32_t* const plist = reinterpret_cast<uint32_t*>(v.dn_rec) + sm.i0;   // parked tracklets of this task
+
+        if (!up) {
+            // ---- down sweep, intake: the parked tracklets whose top hit is in this row start a fresh fit there ----
+            const int np = sm.n_parked;
+            for (int k0 = 0; k0 < np; k0 += kCtConsumers) {
+                const int k = k0 + ctid;
+                uint32_t w = 0;
+                bool need = false;
+                if (k < np) { w = __ldcg(&plist[k]); need = (int)(w >> 24) == row; }
+                const int slot = ct_pop(v, sm, freel, need, cap);
+                if (slot >= 0) {
+                    const int id = sm.i0 + (int)(w & 0xffffffu);
+                    const float4 a4 = __ldcg(reinterpret_cast<const float4*>(&v.tl_up[id]));
+                    const float4 b4 = __ldcg(reinterpret_cast<const float4*>(&v.tl_up[id]) + 1);
+                    CtTrk t;
+                    t.p0 = a4.x; t.p1 = a4.y; t.p2 = a4.z; t.p3 = a4.w; t.p4 = b4.x; t.p5 = 0.f;
+                    t.r0 = __float_as_int(b4.y); t.top = row; t.i = id;
+                    t.f.y = t.p0; t.f.z = t.p1; t.f.s = t.p2; t.f.t = t.p3; t.f.q = t.p4;
+                    fit_prior(t.f, c); t.f.n = 1;
+                    t.aux = row; t.miss = 0; t.ph = 3;
+                    t.cur = row > t.r0 ? (int)v.tl_tab[(size_t)id * v.tab_stride + row - 1] : (int)kNoHit;
+                    sl.store(t, slot);
+                }
+            }
+            ct_bar();
+        }
+
+        // ---- one pad row for the tracklets under way ----
+        const int n_groups = (*(volatile int32_t*)&sm.n_hw + 31) >> 5;
+        for (int g = warp; g < n_groups; g += kCtWarps) {
+            const uint32_t occ = *(volatile uint32_t*)&sm.occ[g];
+            if (!occ) continue;
+            const int slot = (g << 5) + lane;
+            CtTrk t;
+            bool on = (occ >> lane) & 1u;
+            if (on) sl.load(t, slot);
+            if (on && !up && t.top == row) on = false;          // taken in at this very row: starts below
+            Fit& f = t.f;
+            uint16_t* const gt = v.tl_tab + (size_t)(on ? t.i : 0) * v.tab_stride;
+            bool end = false, search = false, counted = false;
+            int acc = -1;
+            uint16_t eold = kNoHit;
+            float ay = 0.f, az = 0.f, iwy = 0.f, iwz = 0.f;
+            // part 1: transport and the candidate that is already known
+            if (on) {
+                int nxt = -1, known = -1;
+                float ky = 0.f, kz = 0.f;
+                if (up) {
+                    if (t.ph == 1 && row == t.aux) { known = t.cur; nxt = __ldg(&v.clink_up[t.cur]); const float2 hk = hits[t.cur - dn.x]; ky = hk.x; kz = hk.y; }
+                } else if (row >= t.r0) {
+                    eold = (uint16_t)t.cur;
+                    if (row > t.r0) t.cur = gt[row - 1];
+                    if (eold != kNoHit) { known = dn.x + eold; const float2 hk = hits[eold]; ky = hk.x; kz = hk.y; }
+                }
+                end = !fit_transport(f, c.row_x[up ? row - 1 : row + 1], c.row_x[row], c);
+                if (!end) {
+                    visits++;
+                    iwy = 1.f / (f.c00 + c.sigma_y2); iwz = 1.f / (f.c11 + c.sigma_z2);
+                    bool gate_ok = false;
+                    if (known >= 0) {   // the gate value of (ky, kz) on the predicted state
+                        const float ry = ky - f.y, rz = kz - f.z;
+                        gate_ok = (ry * ry) * iwy + (rz * rz) * iwz <= c.p.chi2_link;
+                        if (gate_ok) { acc = known; ay = ky; az = kz; }
+                    }
+                    if (up) {
+                        if (t.ph == 1) {
+                            if (row == t.aux) {
+                                if (gate_ok) { t.cur = nxt; t.aux += D; if (nxt < 0) t.ph = 2; }
+                                else { t.ph = 2; search = true; counted = true; }
+                            }   // else: in-between row of a step-2 link
+                        } else {
+                            search = true; counted = true;
+                        }
+                    } else {
+                        search = row < t.r0 || known < 0;
+                        counted = row < t.r0;
+                    }
+                    if (search && counted && fabsf(f.y) > c.row_x[row] * c.tan_half_angle + c.p.edge_margin) {
+                        end = true; search = false;
+                    }
+                }
+            }
+            // part 2: the window searches of this row
+            __syncwarp();
+            if (search && dn.y > 0) {
+                const float4 gf = make_float4(dsc.y0, dsc.z0, dsc.idy, dsc.idz);
+                float bg = 0.f;   // a lane that searches has accepted nothing yet on this row: (ay, az) are free
+                const int bp = sweep_search(v, c, f, gf, dn, hits, cs, iwy, iwz, ay, az, bg);
+                if (bp >= 0 && bg <= c.p.chi2_ext) acc = dn.x + bp;
+            }
+            __syncwarp();
+            // part 3: bookkeeping, update, end of the pass
+            bool upd = false;
+            if (on) {
+                if (search) {
+                    if (acc >= 0) t.miss = 0;
+                    else if (counted && ++t.miss > c.p.max_gap) end = true;
+                }
+                if (!end) {
+                    const uint16_t enew = acc >= 0 ? (uint16_t)(acc - dn.x) : kNoHit;
+                    if (up || row < t.r0 || enew != eold) gt[row] = enew;
+                    upd = acc >= 0;
+                }
+            }
+            __syncwarp();
+            if (upd) {
+                fit_update(f, ay, az, iwy, c);
+                updates++;
+                if (up) {
+                    t.p0 = ay; t.p1 = az; t.p2 = f.s; t.p3 = f.t; t.p4 = f.q; t.top = row;
+                    const int hl = acc - dn.x;                  // seed de-duplication: this hit is being followed
+                    atomicOr(&sm.used[row & 1][hl >> 5], 1u << (hl & 31));
+                } else {
+                    t.p0 = f.y; t.p1 = f.z; t.p2 = f.s; t.p3 = f.t; t.p4 = f.q; t.p5 = f.chi2; t.aux = row;
+                }
+            }
+            __syncwarp();
+            if (on) {
+                if (end || row == (up ? nr - 1 : 0)) {
+                    if (up) {   // park: a fresh fit will start at the top hit in the down sweep
+                        float4* dst = reinterpret_cast<float4*>(&v.tl_up[t.i]);
+                        dst[0] = make_float4(t.p0, t.p1, t.p2, t.p3);
+                        dst[1] = make_float4(t.p4, __int_as_float(t.r0), __int_as_float(t.top), __int_as_float(t.i));
+                        const int k = atomicAdd(&sm.n_parked, 1);
+                        plist[k] = (uint32_t)(t.i - sm.i0) | ((uint32_t)t.top << 24);
+                        atomicMax(&sm.top_max, t.top);
+                    } else {
+                        v.tl_rows[t.i] = t.aux | (t.top << 8) | (f.n << 16);
+                        const int sc = v.S_cap;
+                        v.tl_par[t.i] = t.p0; v.tl_par[sc + t.i] = t.p1; v.tl_par[2 * sc + t.i] = t.p2; v.tl_par[3 * sc + t.i] = t.p3;
+                        v.tl_par[4 * sc + t.i] = t.p4; v.tl_par[5 * sc + t.i] = t.p5;
+                    }
+                    ct_push(sm, freel, slot, cap);
+                } else {
+                    sl.store(t, slot);
+                }
+            }
+        }
+        ct_bar();
+
+        if (up) {
+            // ---- up sweep, intake: the start hits of this row that no up pass has recorded build a tracklet ----
+            const int n = sm.cnt[row];
+            const uint32_t* const ub = sm.used[row & 1];
+            for (int j0 = 0; j0 < n; j0 += kCtConsumers) {
+                const int j = j0 + ctid;
+                bool need = false;
+                int e = 0, hl = 0;
+                float4 a4 = make_float4(0.f, 0.f, 0.f, 0.f);
+                int2 h01 = make_int2(0, 0);
+                if (j < n) {
+                    e = sm.lo[row] + j;
+                    if (e < S) {
+                        a4 = __ldg(reinterpret_cast<const float4*>(&v.seed_rec[e]));
+                        h01 = __ldg(reinterpret_cast<const int2*>(&v.seed_rec[e]) + 2);
+                        hl = h01.x - dn.x;
+                        if (dedup && ((ub[hl >> 5] >> (hl & 31)) & 1u)) v.tl_rows[e] = 0;   // skipped: n_hits = 0
+                        else need = true;
+                    }
+                }
+                const int slot = ct_pop(v, sm, freel, need, cap);
+                if (need && slot < 0) v.tl_rows[e] = 0;
+                if (slot >= 0) {
+                    built++;
+                    CtTrk t;
+                    Fit& f = t.f;
+                    const float dx = c.row_x[row + D] - c.row_x[row];
+                    const float dy = a4.z - a4.x, dz = a4.w - a4.y;
+                    const float dl = sqrtf(dx * dx + dy * dy);
+                    f.y = a4.x; f.z = a4.y; f.s = dy / dl; f.t = dz / dl; f.q = 0.f;
+                    fit_prior(f, c); f.n = 0;
+                    t.p0 = a4.x; t.p1 = a4.y; t.p2 = f.s; t.p3 = f.t; t.p4 = f.q; t.p5 = 0.f;
+                    t.i = e; t.cur = h01.y; t.ph = 1; t.miss = 0; t.r0 = row; t.top = row; t.aux = row + D;
+                    v.tl_tab[(size_t)e * v.tab_stride + row] = (uint16_t)hl;
+                    sl.store(t, slot);
+                }
+            }
+            for (int k = ctid; k < TPC_MAX_ROW_HITS / 32; k += kCtConsumers) sm.used[(row + 1) & 1][k] = 0u;
+            ct_bar();
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&sm.empty[s]);
+        it++;
+    }
+    unsigned long long vs = visits, us = updates, bs = built;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+        vs += __shfl_xor_sync(kFull, vs, o); us += __shfl_xor_sync(kFull, us, o); bs += __shfl_xor_sync(kFull, bs, o);
+    }
+    if (lane == 0 && (vs | bs)) {
+        atomicAdd(&v.cnt[CNT_ROW_VISITS], vs); atomicAdd(&v.cnt[CNT_UPDATES], us); atomicAdd(&v.cnt[CNT_TRACKLETS], bs);
+    }
+}
+
+}  // namespace tpc

@@ -11,7 +11,7 @@
 
 #include "ca_kernels.cuh"
 #include "kf_kernels.cuh"
-#include "kf_sweep.cuh"
+#include "kf_construct.cuh"
 #include "sel_kernels.cuh"
 #include "kf_refit.cuh"
 #include "merge_kernels.cuh"
@@ -94,6 +94,7 @@ struct Batch {
     Buf<UpRec> tl_up, dn_rec;
     Buf<int32_t> dn_count, dn_start, dn_fill, tl_cnt;
     int sel_C = 1;                           // selector chunks per sector task
+    int ct_tier = 0;                         // K5 slot tier used by this group's last launch
     Buf<uint32_t> owner;
     Buf<EventSrc> ev_src;
     Buf<unsigned long long> cnt, kf_cursor;
@@ -134,9 +135,10 @@ struct tpc_tracker {
     cudaStream_t user_stream = nullptr;      // tpc_tracker_set_stream: used by slot 0 when the call is one group
     std::vector<cudaStream_t> own_streams;   // one per slot
     int sm_count = 148;
-    int sw_blocks = 148;                     // resident CTAs of the sweep constructor
+    int ct_tier = 0;                         // K5: state-slot tier (kf_construct.cuh); moves up on kErrSlotCapacity
+    int ct_blocks[kCtTiers] = {296, 148, 148};   // resident CTAs of the constructor in each tier
+    Buf<float> ct_spill;                     // tier 2: state slots in global memory, per CTA
     int rf_blocks = 148;                     // resident CTAs of the refit
-    int sweepers = 0;                        // CTAs per sector task (0 = automatic)
     int group_events = 0;                    // host-input batches: events per group (0 = automatic)
     std::vector<Batch*> slots;               // groups in flight; slots[0] always exists
     // the last call
@@ -186,6 +188,7 @@ struct tpc_tracker {
         h_o_hit.release();
         for (auto& b : h_o_i) b.release();
         for (auto& b : h_o_f) b.release();
+        ct_spill.release();
     }
 };
 
@@ -222,18 +225,9 @@ int reserve_batch(const tpc_tracker* tr, Batch* t, int n_events, int64_t N, int6
     return TPC_OK;
 }
 
-// CTAs that share the start hits of one sector task in K5.  A unit of work (task, share) costs about
-// (1/K + 0.075) of a whole task -- every share sweeps all pad rows -- and the units run in waves of `slots`
-// resident CTAs; K minimises waves x unit cost (measured on 1..24 central events).
-int sweepers_per_task(int n_tasks, int slots) {
-    int best = 1;
-    double best_cost = 1e30;
-    for (int K = 1; K <= 32; K++) {
-        const int64_t units = (int64_t)std::max(n_tasks, 1) * K;
-        const double cost = (double)((units + slots - 1) / slots) * (1.0 / K + 0.075);
-        if (cost < best_cost - 1e-12) { best_cost = cost; best = K; }
-    }
-    return best;
+size_t ct_smem_bytes(int tier) {   // CtSmem, the shared-memory state slots, the stack of free slots
+    const size_t b = sizeof(CtSmem) + (size_t)kCtWords * 4 * (size_t)kCtCapSmem[tier] + 2 * (size_t)(kCtCapSmem[tier] + kCtCapSpill[tier]);
+    return (b + 127) & ~(size_t)127;
 }
 
 int64_t default_seed_cap(int64_t N) { return std::max<int64_t>(N / 8 + 4096, 4096); }
@@ -291,14 +285,10 @@ int launch_all(const tpc_tracker* tr, Batch* t) {
     L += scan_exclusive(v.seed_count, v.seed_start, nb, t->scratch.p, st);
     k_seeds<<<nb, kSeedThreads, 0, st>>>(v); L++;
     mark(3);
-    {
-        CK(cudaMemsetAsync(v.dn_count, 0, sizeof(int32_t) * (nb + 1), st));
-        CK(cudaMemsetAsync(v.dn_fill, 0, sizeof(int32_t) * (nb + 1), st));
-        const int grid = std::max(1, std::min(tr->sw_blocks, v.n_tasks * v.kf_K));
-        k_sweep<true><<<grid, kSwThreads, 0, st>>>(v, c); L++;
-        L += scan_exclusive(v.dn_count, v.dn_start, nb, t->scratch.p, st);
-        k_dn_scatter<<<(int)((t->S_cap + 255) / 256), 256, 0, st>>>(v, nr); L++;
-        k_sweep<false><<<grid, kSwThreads, 0, st>>>(v, c); L++;
+    {   // K5: one CTA per sector task, up sweep then down sweep (kf_construct.cuh)
+        const int tier = t->ct_tier;
+        const int grid = std::max(1, std::min(tr->ct_blocks[tier], v.n_tasks));
+        k_construct<<<grid, kCtThreads, ct_smem_bytes(tier), st>>>(v, c, kCtCapSmem[tier], kCtCapSpill[tier], tr->ct_spill.p); L++;
     }
     mark(4);
     // K6: claims + owned counts per (task, chunk) in shared memory, keep flags, scans, output
@@ -402,7 +392,11 @@ int batch_begin(const tpc_tracker* tr, Batch* t, int first_event, int n, const t
     v.o_hit_yz = t->o_hit_yz.p; v.o_hit_row = t->o_hit_row.p; v.trk_hit0 = t->trk_hit0.p;
     v.seed_rec = t->seed_rec.p; v.tl_up = t->tl_up.p; v.dn_rec = t->dn_rec.p;
     v.dn_count = t->dn_count.p; v.dn_start = t->dn_start.p; v.dn_fill = t->dn_fill.p;
-    v.kf_K = tr->sweepers > 0 ? tr->sweepers : sweepers_per_task(v.n_tasks, tr->sw_blocks);
+    t->ct_tier = std::max(t->ct_tier, tr->ct_tier);
+    if (kCtCapSpill[t->ct_tier] > 0) {   // slots in global memory for every resident CTA (allocated once, on the way up)
+        tpc_tracker* w = const_cast<tpc_tracker*>(tr);
+        if ((rc = w->ct_spill.reserve((size_t)tr->ct_blocks[t->ct_tier] * kCtWords * kCtCapSpill[t->ct_tier])) != TPC_OK) return rc;
+    }
     t->n_events = n; t->N = N;
     if (tr->profiling)
         for (auto& e : t->evt)
@@ -434,10 +428,16 @@ int batch_finish(const tpc_tracker* tr, Batch* t) {
             set_err("more than %d clusters in one (sector,row)", TPC_MAX_ROW_HITS);
             return TPC_ERR_CAPACITY;
         }
-        if ((err & kErrSeedCapacity) || n_seeds > t->S_cap) {
-            if (attempt >= 2) { set_err("tracklet pool could not be grown"); return TPC_ERR_CAPACITY; }
+        const bool slots = (err & kErrSlotCapacity) != 0;
+        if (slots && t->ct_tier >= kCtTiers - 1) {
+            set_err("more than %d tracklets under way at once in one sector task", kCtCapMax);
+            return TPC_ERR_CAPACITY;
+        }
+        if (slots || (err & kErrSeedCapacity) || n_seeds > t->S_cap) {
+            if (attempt >= 4) { set_err("tracklet pool could not be grown"); return TPC_ERR_CAPACITY; }
             t->counters.n_retries++;
-            int rc = batch_begin(tr, t, t->first_event, t->n_events, t->in, (int64_t)n_seeds + n_seeds / 8 + 1024, false);
+            if (slots) { t->ct_tier++; const_cast<tpc_tracker*>(tr)->ct_tier = t->ct_tier; }   // sticky: the tracker stays in the higher tier
+            int rc = batch_begin(tr, t, t->first_event, t->n_events, t->in, std::max<int64_t>(t->S_cap, (int64_t)n_seeds + n_seeds / 8 + 1024), false);
             if (rc != TPC_OK) return rc;
             continue;
         }
@@ -450,6 +450,7 @@ int batch_finish(const tpc_tracker* tr, Batch* t) {
         t->counters.n_track_hits = (int64_t)t->h_cnt.p[CNT_TRACK_HITS];
         t->counters.n_updates = (int64_t)t->h_cnt.p[CNT_UPDATES];
         t->counters.n_refit_visits = (int64_t)t->h_cnt.p[CNT_REFIT_VISITS];
+        t->counters.n_tracklets = (int64_t)t->h_cnt.p[CNT_TRACKLETS];
         return TPC_OK;
     }
 }
@@ -482,7 +483,7 @@ template <class T> int grow_keep(tpc_tracker* t, Buf<T>& b, size_t need, size_t 
 void add_counters(tpc_counters& a, const tpc_counters& b) {
     a.n_events += b.n_events; a.n_clusters += b.n_clusters; a.n_links += b.n_links; a.n_seeds += b.n_seeds;
     a.n_row_visits += b.n_row_visits; a.n_tracklet_hits += b.n_tracklet_hits; a.n_tracks += b.n_tracks;
-    a.n_track_hits += b.n_track_hits; a.n_kernel_launches += b.n_kernel_launches; a.n_retries += b.n_retries; a.n_updates += b.n_updates; a.n_refit_visits += b.n_refit_visits;
+    a.n_track_hits += b.n_track_hits; a.n_kernel_launches += b.n_kernel_launches; a.n_retries += b.n_retries; a.n_updates += b.n_updates; a.n_refit_visits += b.n_refit_visits; a.n_tracklets += b.n_tracklets;
 }
 
 }  // namespace
@@ -501,6 +502,7 @@ void tpc_default_params(tpc_params* p) {
     p->min_tracklet_hits = 10; p->min_track_hits = 10;
     p->refit = 0;
     p->merge = 0; p->merge_dy = 1.0f; p->merge_dz = 1.0f; p->merge_ds = 0.05f; p->merge_dt = 0.05f; p->merge_max_gap = 6;
+    p->seed_dedup = 1;
 }
 
 const char* tpc_status_string(int s) {
@@ -531,9 +533,10 @@ tpc_tracker* tpc_tracker_create_ex(const tpc_geometry* g, float bz, const tpc_pa
     }
     tpc_params p;
     if (params) p = *params; else tpc_default_params(&p);
-    if (p.link_step < 1 || p.link_step > 2 || p.min_tracklet_hits < 1 || p.min_track_hits < 1 || p.max_gap < 0 || p.refit < 0 || p.refit > 1 || p.merge < 0 || p.merge > 1 ||
+    if (p.link_step < 1 || p.link_step > 2 || p.min_tracklet_hits < 1 || p.min_track_hits < 1 || p.max_gap < 0 || p.max_gap > 60 ||
+        p.seed_dedup < 0 || p.seed_dedup > 1 || p.refit < 0 || p.refit > 1 || p.merge < 0 || p.merge > 1 ||
         (p.merge && !p.refit) || p.merge_max_gap < 0 || !(p.merge_dy > 0.f) || !(p.merge_dz > 0.f) || !(p.merge_ds > 0.f) || !(p.merge_dt > 0.f)) {
-        set_err("params: link_step must be 1 or 2, minimum hit counts >= 1, max_gap >= 0, refit 0 or 1, merge 0 or 1 (needs refit) with positive tolerances");
+        set_err("params: link_step must be 1 or 2, minimum hit counts >= 1, max_gap in [0,60], seed_dedup 0 or 1, refit 0 or 1, merge 0 or 1 (needs refit) with positive tolerances");
         return nullptr;
     }
     int dev = 0, ndev = 0;
@@ -557,14 +560,25 @@ tpc_tracker* tpc_tracker_create_ex(const tpc_geometry* g, float bz, const tpc_pa
     }
     if (g->sector_alpha) t->sector_alpha.assign(g->sector_alpha, g->sector_alpha + g->n_sectors);
     cudaDeviceGetAttribute(&t->sm_count, cudaDevAttrMultiProcessorCount, dev);
-    {   // persistent constructor grid: as many CTAs as are resident at once
+    {   // persistent constructor grid: as many CTAs as are resident at once, for both slot counts
         int per_sm = 0;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_sweep<true>, kSwThreads, 0) != cudaSuccess || per_sm < 1) {
-            set_err("k_sweep cannot be configured: %s", cudaGetErrorString(cudaGetLastError()));
+        size_t most = 0;
+        for (int k = 0; k < kCtTiers; k++) most = std::max(most, ct_smem_bytes(k));
+        if (cudaFuncSetAttribute(k_construct, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)most) != cudaSuccess) {
+            set_err("k_construct: %zu bytes of shared memory cannot be configured: %s", most, cudaGetErrorString(cudaGetLastError()));
             delete t;
             return nullptr;
         }
-        t->sw_blocks = t->sm_count * per_sm;
+        for (int k = 0; k < kCtTiers; k++) {
+            if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_construct, kCtThreads, ct_smem_bytes(k)) != cudaSuccess || per_sm < 1) {
+                set_err("k_construct cannot be configured: %s", cudaGetErrorString(cudaGetLastError()));
+                delete t;
+                return nullptr;
+            }
+            t->ct_blocks[k] = t->sm_count * per_sm;
+        }
+        if (!p.seed_dedup) t->ct_tier = 1;   // ~3x the tracklets under way
+        if (const char* se = getenv("TPCTRACK_CT_TIER")) t->ct_tier = std::max(0, std::min(atoi(se), kCtTiers - 1));
         if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_refit, kRfThreads, 0) != cudaSuccess || per_sm < 1) per_sm = 1;
         t->rf_blocks = t->sm_count * per_sm;
         if (cudaFuncSetAttribute(k_select_claim, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kSelCap * sizeof(uint32_t))) != cudaSuccess ||
@@ -573,7 +587,6 @@ tpc_tracker* tpc_tracker_create_ex(const tpc_geometry* g, float bz, const tpc_pa
             delete t;
             return nullptr;
         }
-        if (const char* se = getenv("TPCTRACK_SWEEPERS")) t->sweepers = atoi(se);
     }
     if (const char* ge = getenv("TPCTRACK_GROUP_EVENTS")) t->group_events = atoi(ge);
     Batch* b0 = get_slot(t, 0);
@@ -890,7 +903,10 @@ int tpc_debug_get(tpc_tracker* tr, int32_t what, int32_t event, void* buf, size_
         case TPC_DBG_TL_ROWS: {
             std::vector<int32_t> l(std::max(s, 1));
             if (s) CK(cudaMemcpy(l.data(), t->v.tl_rows + s0, 4 * (size_t)s, cudaMemcpyDeviceToHost));
-            for (int k = 0; k < s; k++) { ob[3 * k] = l[k] & 0xff; ob[3 * k + 1] = (l[k] >> 8) & 0xff; ob[3 * k + 2] = l[k] >> 16; }
+            for (int k = 0; k < s; k++) {
+                const bool built = (l[k] >> 16) > 0;   // 0 hits: the start hit was skipped by the seed de-duplication
+                ob[3 * k] = built ? (l[k] & 0xff) : -1; ob[3 * k + 1] = built ? ((l[k] >> 8) & 0xff) : -1; ob[3 * k + 2] = l[k] >> 16;
+            }
             return TPC_OK;
         }
         case TPC_DBG_TL_PAR: {
@@ -914,7 +930,8 @@ int tpc_debug_get(tpc_tracker* tr, int32_t what, int32_t event, void* buf, size_
             CK(cudaMemcpy(tab.data(), t->v.tl_tab + (size_t)s0 * stride, 2 * tab.size(), cudaMemcpyDeviceToHost));
             CK(cudaMemcpy(desc.data(), t->v.desc + (size_t)event * bpe, sizeof(BinDesc) * (size_t)bpe, cudaMemcpyDeviceToHost));
             for (int k = 0; k < s; k++) {
-                const int first = rows[k] & 0xff, last = (rows[k] >> 8) & 0xff;
+                const bool built = (rows[k] >> 16) > 0;
+                const int first = built ? (rows[k] & 0xff) : 1, last = built ? ((rows[k] >> 8) & 0xff) : 0;
                 const int tb = sbin[k] - sbin[k] % nr - event * bpe;   // first bin of the tracklet's task, event-local
                 const uint16_t* tp = tab.data() + (size_t)k * stride;
                 for (int r = 0; r < nr; r++)

@@ -34,7 +34,7 @@ class tpc_params(C.Structure):
                 ("win_min", C.c_float), ("win_max", C.c_float), ("max_gap", C.c_int32), ("edge_margin", C.c_float),
                 ("min_tracklet_hits", C.c_int32), ("min_track_hits", C.c_int32), ("refit", C.c_int32),
                 ("merge", C.c_int32), ("merge_dy", C.c_float), ("merge_dz", C.c_float), ("merge_ds", C.c_float),
-                ("merge_dt", C.c_float), ("merge_max_gap", C.c_int32)]
+                ("merge_dt", C.c_float), ("merge_max_gap", C.c_int32), ("seed_dedup", C.c_int32)]
 
     def as_dict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}
@@ -60,7 +60,7 @@ class tpc_event_out(C.Structure):
 class tpc_counters(C.Structure):
     _fields_ = [(n, C.c_int64) for n in ("n_events", "n_clusters", "n_links", "n_seeds", "n_row_visits",
                                          "n_tracklet_hits", "n_tracks", "n_track_hits", "n_kernel_launches",
-                                         "n_retries", "n_updates", "n_refit_visits")]
+                                         "n_retries", "n_updates", "n_refit_visits", "n_tracklets")]
 
     def as_dict(self):
         return {n: int(getattr(self, n)) for n, _ in self._fields_}

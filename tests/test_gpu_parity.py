@@ -66,8 +66,9 @@ def compare_event(trk, out, ev, ref, event=0, check_stages=True):
             assert np.array_equal(rows[same, 0], ref.tl_first_row[same])
             assert np.array_equal(rows[same, 1], ref.tl_last_row[same])
             assert np.array_equal(rows[same, 2], ref.tl_n_hits[same])
-            refp = np.concatenate([ref.tl_par, ref.tl_chi2[:, None]], axis=1)[same]
-            err = np.abs(par[same] - refp) / np.maximum(1.0, np.abs(refp))
+            built = same & (ref.tl_n_hits > 0)     # a start hit skipped by the seed de-duplication (R23) has no fit
+            refp = np.concatenate([ref.tl_par, ref.tl_chi2[:, None]], axis=1)[built]
+            err = np.abs(par[built] - refp) / np.maximum(1.0, np.abs(refp))
             assert err.max(initial=0.0) <= TOL, err.max()
     res = trk.to_numpy(out)
     if flips == 0:
@@ -96,6 +97,24 @@ def test_parity_configs(trk_mod, gen_mod, event_and_oracle, name, device_inputs)
     c = trk.tpc_get_counters()
     assert c["n_clusters"] == ev.n_clusters and c["n_seeds"] == ref.n_seeds and c["n_tracks"] == ref.n_tracks
     assert c["n_links"] == int((ref.clink_up >= 0).sum()) and c["n_kernel_launches"] >= 10
+    assert c["n_tracklets"] == int((ref.tl_n_hits > 0).sum()) < c["n_seeds"]
+    trk.close()
+
+
+@pytest.mark.parametrize("name", ["single_sector", "semicentral"])
+def test_parity_without_seed_dedup(trk_mod, gen_mod, oracle_mod, name):
+    """seed_dedup = 0: every start hit is fitted (three times the tracklets under way: the constructor runs with
+    its large slot count, one CTA per SM)."""
+    ev = gen_mod.generate(name)
+    po = oracle_mod.default_params(); po.seed_dedup = 0
+    ref = oracle_mod.track_event(make_geometry(oracle_mod, gen_mod, ev), ev.sector_offset, ev.y, ev.z, ev.row,
+                                 params=po, precision="float")
+    trk = make_tracker(trk_mod, gen_mod, ev, params=copy_params(po, trk_mod))
+    out = trk.tpc_track_event(ev_dict(ev, True))
+    flips, res = compare_event(trk, out, ev, ref)
+    assert flips == 0
+    c = trk.tpc_get_counters()
+    assert c["n_tracklets"] == c["n_seeds"] == ref.n_seeds
     trk.close()
 
 
