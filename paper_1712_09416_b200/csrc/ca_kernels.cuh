@@ -366,7 +366,7 @@ __global__ void __launch_bounds__(kCleanThreads) k_clean(const View v) {
 // ---------------------------------------------------------------------------------------------------------
 constexpr int kSeedThreads = 128;
 
-__global__ void __launch_bounds__(kSeedThreads) k_seeds(const View v) {
+__global__ void __launch_bounds__(kSeedThreads) k_seeds(const View v, const __grid_constant__ Const c) {
     __shared__ int list_h[TPC_MAX_ROW_HITS];
     __shared__ int list_o[TPC_MAX_ROW_HITS];
     const int bin = blockIdx.x;
@@ -387,9 +387,14 @@ __global__ void __launch_bounds__(kSeedThreads) k_seeds(const View v) {
             const int h0 = list_h[i], h1 = v.clink_up[h0];
             v.seeds[s0 + rank] = h0; v.seed_bin[s0 + rank] = bin;
             const float2 a0 = v.shit[h0], a1 = v.shit[h1];
+            // initial direction of the up pass: s = dy / dl, t = dz / dl along the first link
+            const int r = bin % c.n_rows;
+            const float dx = c.row_x[r + c.p.link_step] - c.row_x[r];
+            const float dy = a1.x - a0.x, dz = a1.y - a0.y;
+            const float dl = sqrtf(dx * dx + dy * dy);
             float4* rec = reinterpret_cast<float4*>(v.seed_rec) + 2 * (size_t)(s0 + rank);
-            rec[0] = make_float4(a0.x, a0.y, a1.x, a1.y);
-            rec[1] = make_float4(__int_as_float(h0), __int_as_float(h1), 0.f, 0.f);
+            rec[0] = make_float4(a0.x, a0.y, dy / dl, dz / dl);
+            rec[1] = make_float4(__int_as_float(h0), __int_as_float(h1), __int_as_float(v.clink_up[h1]), 0.f);
         } else atomicOr((unsigned int*)&v.cnt[CNT_ERR], kErrSeedCapacity);
     }
 }

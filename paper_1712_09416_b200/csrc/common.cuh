@@ -24,7 +24,7 @@ constexpr unsigned kErrBadRow = 1u, kErrRowCapacity = 2u, kErrSeedCapacity = 4u,
 
 // device counters (unsigned long long each)
 constexpr int kNCursors = 4;           // work cursors: [0] K5 sector tasks, [2] refit
-enum { CNT_ERR = 0, CNT_LINKS, CNT_ROW_VISITS, CNT_TL_HITS, CNT_TRACKS, CNT_TRACK_HITS, CNT_UPDATES, CNT_REFIT_VISITS, CNT_TRACKLETS, CNT_N };
+enum { CNT_ERR = 0, CNT_LINKS, CNT_ROW_VISITS, CNT_TL_HITS, CNT_TRACKS, CNT_TRACK_HITS, CNT_UPDATES, CNT_REFIT_VISITS, CNT_TRACKLETS, CNT_PROF, CNT_N = CNT_PROF + 16 };
 
 // One event's input arrays (device pointers) and its place in the batch-global cluster numbering.
 struct EventSrc {
@@ -81,7 +81,8 @@ struct View {
     float* tl_par;           // [6][S_cap] y z s t q chi2
     SeedRec* seed_rec;       // [S_cap] start hit and its up-link: coordinates and sorted indices (K4 -> K5 up sweep)
     UpRec* tl_up;            // [S_cap] what the up pass hands to the down pass, by tracklet
-    UpRec* dn_rec;           // [S_cap] K5 scratch: per task, the list of parked tracklets (id in task | top row << 24)
+    UpRec* dn_rec;           // [S_cap] the same records, per task ordered by top row (written at the turn of the sweeps)
+    uint32_t* kf_park;       // [S_cap] K5 scratch: per task, parked tracklets in order of parking (id in task | top row << 24)
     int32_t *dn_count, *dn_start, *dn_fill;   // [n_bins+1] O9: refitted tracks per (task, first fitted row)
     // K6
     uint32_t* owner;         // [N] best key among tracklets holding the hit

@@ -26,38 +26,53 @@ namespace tpc {
 #ifndef TPC_CT_RING
 #define TPC_CT_RING 3
 #endif
+#ifndef TPC_CT_INL
+#define TPC_CT_INL __forceinline__   // intake / turn inlined: 5.95 ms against 6.42 ms out of line (config 5)
+#endif
 constexpr int kCtWarps = TPC_CT_WARPS;                 // consumer warps of a CTA (one more warp produces)
 constexpr int kCtConsumers = kCtWarps * 32;
 constexpr int kCtThreads = (kCtWarps + 1) * 32;
 constexpr int kCtRing = TPC_CT_RING;                   // rows in flight
-constexpr int kCtWords = 31;                           // 4-byte words of a tracklet's state
+constexpr int kCtWords = 32;                           // 4-byte words of a tracklet's state
+#ifndef TPC_CT_STAGE
+#define TPC_CT_STAGE 48
+#endif
+constexpr int kCtSeedStage = TPC_CT_STAGE;             // start-hit records of a row staged with the row (more: read in place)
 // State slots per sector task = tracklets under way at once, in three tiers (the host moves up one tier when a
 // launch reports kErrSlotCapacity and stays there): shared-memory slots + slots in global memory (L2)
 constexpr int kCtTiers = 3;
-constexpr int kCtCapSmem[kCtTiers] = {512, 1472, 1344};   // tier 0: two CTAs per SM; tiers 1, 2: one
+constexpr int kCtCapSmem[kCtTiers] = {512, 1408, 1280};   // tier 0: two CTAs per SM; tiers 1, 2: one
 constexpr int kCtCapSpill[kCtTiers] = {0, 0, 4096};
-constexpr int kCtCapMax = 1344 + 4096;
+constexpr int kCtCapMax = 1280 + 4096;
 constexpr int kSwCap = 640;                            // hits of a row staged in shared memory; larger rows are read in place
 constexpr int kSwHitBytes = (kSwCap + 2) * 8;          // + alignment slack of the bulk copy (16-byte granules)
 constexpr int kSwCellEntries = kCellsPerHit * kSwCap + kCellPad + 16;
 constexpr int kSwCellBytes = kSwCellEntries * 2;
 static_assert(kSwHitBytes % 16 == 0 && kSwCellBytes % 16 == 0, "bulk copies are 16-byte granular");
 constexpr int kCtDown = 0x100;                         // cmd flag: the row belongs to the down sweep
+constexpr int kCtTurn = 0x200;                         // cmd: between the sweeps (order the parked tracklets by top row)
 
-struct __align__(16) SeedRec { float y0, z0, y1, z1; int32_t h0, h1, pad0, pad1; };   // start hit, its up-link
-struct __align__(16) UpRec { float y, z, s, t, q; int32_t r0, top, id; };             // what the up pass hands down
+// a start hit: its coordinates, the direction (sin phi, tg lambda) of the line to its up-link (DESIGN.md "O5" up pass,
+// initial state), the hit itself, its up-link, and that one's
+struct __align__(16) SeedRec { float y0, z0, s, t; int32_t h0, h1, h2, pad; };
+// what the up pass hands down: its top hit, (sin phi, tg lambda, q/pT) there, start row | top row << 8, the table
+// entry of the row below the top hit, the tracklet
+struct __align__(16) UpRec { float y, z, s, t, q; int32_t rows, below, id; };
 
 struct __align__(128) CtSmem {
     BinDesc desc[TPC_MAX_ROWS + 1];                    // the task's row descriptors
     unsigned char hits[kCtRing][kSwHitBytes];
     unsigned char cells[kCtRing][kSwCellBytes];
-    int32_t lo[TPC_MAX_ROWS + 1];                      // first start hit of each row in the canonical list
-    int32_t cnt[TPC_MAX_ROWS + 1];                     // start hits of the row
+    SeedRec seeds[kCtRing][kCtSeedStage > 0 ? kCtSeedStage : 1];              // the first records of what starts at the row: start hits (up
+                                                       // sweep), parked tracklets with their top hit there (down sweep)
+    int32_t lo[TPC_MAX_ROWS + 1];                      // up sweep: first start hit of each row in the canonical list;
+    int32_t cnt[TPC_MAX_ROWS + 1];                     // start hits of the row.  Down sweep: the same for the parked tracklets
+    int32_t dcnt[TPC_MAX_ROWS + 1];                    // tracklets parked with their top hit in each row
     uint32_t used[2][TPC_MAX_ROW_HITS / 32];           // hits of the row at hand recorded by an up pass (double buffered)
     uint32_t occ[(kCtCapMax + 31) / 32];               // occupied state slots
     unsigned long long full[kCtRing], empty[kCtRing], tbar;
     int32_t cmd[kCtRing];                              // row held by the ring slot (| kCtDown); -1 = no more work
-    int32_t task, abort, n_free, n_hw, n_parked, top_max, i0;
+    int32_t task, abort, n_free, n_hw, n_parked, top_max, i0;   // n_hw: highest slot used so far + 1
 };
 
 // ---- mbarrier / bulk-copy wrappers (PTX ISA: mbarrier, cp.async.bulk) ----
@@ -109,6 +124,7 @@ __device__ __forceinline__ size_t cell_index(int base, int bin) { return (size_t
 __device__ __forceinline__ void ct_producer(const View& v, const Const& c, CtSmem& sm, uint16_t* freel, int cap) {
     const int lane = lane_id();
     const int nr = c.n_rows;
+    const int S = min(v.seed_start[v.n_bins], v.S_cap);
     volatile int32_t* const abort = &sm.abort;
     uint32_t it = 0, tphase = 0;
     bool ok = true;
@@ -118,15 +134,22 @@ __device__ __forceinline__ void ct_producer(const View& v, const Const& c, CtSme
         if (!(ok = mbar_wait(&sm.empty[s], ((it / kCtRing) & 1u) ^ 1u, abort))) return;
         sm.cmd[s] = row | flag;
         const BinDesc& d = sm.desc[row];
-        if (d.n > 0 && d.n <= kSwCap) {
+        const bool rowdata = d.n > 0 && d.n <= kSwCap;
+        // records to stage: start hits of the row (not beyond the pool), or tracklets parked there
+        const int ns = flag ? min(sm.cnt[row], kCtSeedStage) : max(0, min(min(sm.cnt[row], kCtSeedStage), S - sm.lo[row]));
+        const void* const recs = flag ? (const void*)(v.dn_rec + sm.i0 + sm.lo[row]) : (const void*)(v.seed_rec + sm.lo[row]);
+        if (rowdata || ns > 0) {
             const int offh = d.base & 1;
-            const uint32_t hb = (uint32_t)((offh + d.n + 1) & ~1) * 8u;
+            const uint32_t hb = rowdata ? (uint32_t)((offh + d.n + 1) & ~1) * 8u : 0u;
             const size_t g = cell_index(d.base, tb + row);
             const int offc = (int)(g & 7);
-            const uint32_t cb = ((uint32_t)(offc + d.ny * d.nz + 1) * 2u + 15u) & ~15u;
-            mbar_arrive_expect_tx(&sm.full[s], hb + cb);
-            bulk_g2s(sm.hits[s], v.shit + (d.base - offh), hb, &sm.full[s]);
-            bulk_g2s(sm.cells[s], v.cells + (g - offc), cb, &sm.full[s]);
+            const uint32_t cb = rowdata ? (((uint32_t)(offc + d.ny * d.nz + 1) * 2u + 15u) & ~15u) : 0u;
+            mbar_arrive_expect_tx(&sm.full[s], hb + cb + 32u * (uint32_t)ns);
+            if (rowdata) {
+                bulk_g2s(sm.hits[s], v.shit + (d.base - offh), hb, &sm.full[s]);
+                bulk_g2s(sm.cells[s], v.cells + (g - offc), cb, &sm.full[s]);
+            }
+            if (ns > 0) bulk_g2s(sm.seeds[s], recs, 32u * (uint32_t)ns, &sm.full[s]);
         } else {
             mbar_arrive(&sm.full[s]);
         }
@@ -137,7 +160,10 @@ __device__ __forceinline__ void ct_producer(const View& v, const Const& c, CtSme
         for (uint32_t j = it > (uint32_t)kCtRing ? it - kCtRing : 0; ok && j < it; j++)
             ok = mbar_wait(&sm.empty[j % kCtRing], (j / kCtRing) & 1u, abort);
     };
-    auto reset_slots = [&]() {   // the consumers are idle: all state slots are free again, lowest on top
+    auto reset_slots = [&]() {   // the consumers are idle: all state slots are free
+        // the stack of free slots, lowest on top.  (Measured: preferring the slots of the warps' first groups, so that
+        // one round per row serves up to 416 tracklets, is SLOWER, 5.97 against 5.42 ms on config 5 -- a step takes as
+        // long as its slowest lane, and fuller groups have slower slowest lanes.)
         for (int k = lane; k < cap; k += 32) freel[k] = (uint16_t)(cap - 1 - k);
         for (int k = lane; k < (kCtCapMax + 31) / 32; k += 32) sm.occ[k] = 0u;
         if (lane == 0) { sm.n_free = cap; sm.n_hw = 0; }
@@ -161,6 +187,7 @@ __device__ __forceinline__ void ct_producer(const View& v, const Const& c, CtSme
             if (n > 0) f = min(f, r);
         }
         for (int k = lane; k < 2 * (TPC_MAX_ROW_HITS / 32); k += 32) (&sm.used[0][0])[k] = 0u;
+        for (int r = lane; r <= TPC_MAX_ROWS; r += 32) sm.dcnt[r] = 0;
         reset_slots();
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) f = min(f, __shfl_xor_sync(kFull, f, o));
@@ -179,6 +206,19 @@ __device__ __forceinline__ void ct_producer(const View& v, const Const& c, CtSme
         if (!ok) break;
         reset_slots();
         __syncwarp();
+        if (lane == 0) {   // the turn: the consumers order the parked tracklets by top row (lo / cnt become theirs)
+            const int s = (int)(it % kCtRing);
+            if ((ok = mbar_wait(&sm.empty[s], ((it / kCtRing) & 1u) ^ 1u, abort))) {
+                sm.cmd[s] = kCtTurn;
+                mbar_arrive(&sm.full[s]);
+                it++;
+                drain();
+            }
+        }
+        ok = __shfl_sync(kFull, (int)ok, 0) != 0;
+        it = __shfl_sync(kFull, it, 0);
+        __syncwarp();
+        if (!ok) break;
         if (lane == 0) {   // down sweep from the highest top row
             const int tm = *(volatile int32_t*)&sm.top_max;
             for (int row = tm; ok && row >= 0; row--) issue(row, kCtDown, tb);
@@ -230,9 +270,10 @@ __device__ __forceinline__ int sweep_search(const View& v, const Const& c, const
 // ---- a tracklet's state in its shared-memory slot: word k of slot s sits at st[k * cap + s] ----
 struct CtTrk {
     Fit f;
-    float p0, p1, p2, p3, p4, p5;   // state right after the last accepted update
+    float p0, p1, p2, p3, p4, p5;   // state right after the last accepted update (up: p5 = two table entries, see step)
     int i;                          // tracklet = canonical start-hit number (batch-global)
     int cur;                        // up: the linked hit to come; down: table entry of the row below (read one row ahead)
+    int nxt;                        // up: the hit linked above cur (read one link ahead)
     int ph, miss, r0, top, aux;     // ph 1 up/follow, 2 up/extend, 3 down; aux: up = row of cur, down = first row
 };
 __device__ __forceinline__ void ct_load(CtTrk& t, const float* S, int cap) {
@@ -243,7 +284,7 @@ __device__ __forceinline__ void ct_load(CtTrk& t, const float* S, int cap) {
     f.c40 = S[15 * cap]; f.c41 = S[16 * cap]; f.c42 = S[17 * cap]; f.c43 = S[18 * cap]; f.c44 = S[19 * cap];
     f.chi2 = S[20 * cap]; f.n = __float_as_int(S[21 * cap]);
     t.p0 = S[22 * cap]; t.p1 = S[23 * cap]; t.p2 = S[24 * cap]; t.p3 = S[25 * cap]; t.p4 = S[26 * cap]; t.p5 = S[27 * cap];
-    t.i = __float_as_int(S[28 * cap]); t.cur = __float_as_int(S[29 * cap]);
+    t.i = __float_as_int(S[28 * cap]); t.cur = __float_as_int(S[29 * cap]); t.nxt = __float_as_int(S[31 * cap]);
     const uint32_t pk = __float_as_uint(S[30 * cap]);
     t.ph = pk & 3u; t.miss = (pk >> 2) & 63u; t.r0 = (pk >> 8) & 255u; t.top = (pk >> 16) & 255u; t.aux = pk >> 24;
 }
@@ -255,12 +296,24 @@ __device__ __forceinline__ void ct_store(const CtTrk& t, float* S, int cap) {
     S[15 * cap] = f.c40; S[16 * cap] = f.c41; S[17 * cap] = f.c42; S[18 * cap] = f.c43; S[19 * cap] = f.c44;
     S[20 * cap] = f.chi2; S[21 * cap] = __int_as_float(f.n);
     S[22 * cap] = t.p0; S[23 * cap] = t.p1; S[24 * cap] = t.p2; S[25 * cap] = t.p3; S[26 * cap] = t.p4; S[27 * cap] = t.p5;
-    S[28 * cap] = __int_as_float(t.i); S[29 * cap] = __int_as_float(t.cur);
-    S[30 * cap] = __uint_as_float((uint32_t)t.ph | ((uint32_t)t.miss << 2) | ((uint32_t)t.r0 << 8) | ((uint32_t)t.top << 16) |
-                                  ((uint32_t)t.aux << 24));
+    S[28 * cap] = __int_as_float(t.i); S[29 * cap] = __int_as_float(t.cur); S[31 * cap] = __int_as_float(t.nxt);
+    S[30 * cap] = __uint_as_float((uint32_t)t.ph | ((uint32_t)t.miss << 2) | ((uint32_t)t.r0 << 8) |
+                                  ((uint32_t)t.top << 16) | ((uint32_t)t.aux << 24));
 }
 
-// take `need` state slots for the lanes that ask; -1 when the task has more tracklets under way than slots
+// slot -> where its state lives: the first cap_s slots in shared memory, the others in this CTA's stretch of
+// global memory (both multiples of 32, so a warp's 32 slots are all of one kind)
+struct CtSlots {
+    float* st; float* gs; int cap_s, cap_g;
+    __device__ __forceinline__ void load(CtTrk& t, int slot) const {
+        if (slot < cap_s) ct_load(t, st + slot, cap_s); else ct_load(t, gs + (slot - cap_s), cap_g);
+    }
+    __device__ __forceinline__ void store(const CtTrk& t, int slot) const {
+        if (slot < cap_s) ct_store(t, st + slot, cap_s); else ct_store(t, gs + (slot - cap_s), cap_g);
+    }
+};
+
+// take a state slot for every lane that asks; -1 when the task has more tracklets under way than slots
 __device__ __forceinline__ int ct_pop(const View& v, CtSmem& sm, const uint16_t* freel, bool need, int cap) {
     const unsigned m = __ballot_sync(kFull, need);
     if (!m) return -1;
@@ -276,26 +329,117 @@ __device__ __forceinline__ int ct_pop(const View& v, CtSmem& sm, const uint16_t*
     return slot;
 }
 __device__ __forceinline__ void ct_push(CtSmem& sm, uint16_t* freel, int slot, int cap) {
-    atomicAnd(&sm.occ[slot >> 5], ~(1u << (slot & 31)));
     const int idx = atomicAdd(&sm.n_free, 1);
     if (idx >= 0 && idx < cap) freel[idx] = (uint16_t)slot;
 }
-// slot -> where its state lives: the first cap_s slots in shared memory, the others in this CTA's stretch of
-// global memory (both multiples of 32, so a warp's 32 slots are all of one kind)
-struct CtSlots {
-    float* st; float* gs; int cap_s, cap_g;
-    __device__ __forceinline__ void load(CtTrk& t, int slot) const {
-        if (slot < cap_s) ct_load(t, st + slot, cap_s); else ct_load(t, gs + (slot - cap_s), cap_g);
+
+// ---- intake, by all consumer threads between the row steps ----
+// down sweep: the parked tracklets whose top hit is in this row start a fresh fit there (their records come
+// ordered by top row: staged in the ring slot, the ones beyond kCtSeedStage read in place)
+__device__ TPC_CT_INL void ct_intake_down(const View& v, const Const& c, CtSmem& sm, const CtSlots& sl, const uint16_t* freel,
+                                            int cap, int row, int s) {
+    const int n = sm.cnt[row], lo = sm.i0 + sm.lo[row];
+    for (int j0 = 0; j0 < n; j0 += kCtConsumers) {
+        const int j = j0 + (int)threadIdx.x;
+        const int slot = ct_pop(v, sm, freel, j < n, cap);
+        if (slot >= 0) {
+            float4 a4, b4;
+            if (j < kCtSeedStage) {
+                a4 = *reinterpret_cast<const float4*>(&sm.seeds[s][j]);
+                b4 = *(reinterpret_cast<const float4*>(&sm.seeds[s][j]) + 1);
+            } else {
+                a4 = __ldcg(reinterpret_cast<const float4*>(&v.dn_rec[lo + j]));
+                b4 = __ldcg(reinterpret_cast<const float4*>(&v.dn_rec[lo + j]) + 1);
+            }
+            CtTrk t;
+            t.p0 = a4.x; t.p1 = a4.y; t.p2 = a4.z; t.p3 = a4.w; t.p4 = b4.x; t.p5 = 0.f;
+            t.r0 = __float_as_int(b4.y) & 0xff; t.top = row; t.i = __float_as_int(b4.w);
+            t.f.y = t.p0; t.f.z = t.p1; t.f.s = t.p2; t.f.t = t.p3; t.f.q = t.p4;
+            fit_prior(t.f, c); t.f.n = 1;
+            t.aux = row; t.miss = 0; t.ph = 3; t.nxt = -1;
+            t.cur = __float_as_int(b4.z);             // table entry of the row below the top hit
+            sl.store(t, slot);
+        }
     }
-    __device__ __forceinline__ void store(const CtTrk& t, int slot) const {
-        if (slot < cap_s) ct_store(t, st + slot, cap_s); else ct_store(t, gs + (slot - cap_s), cap_g);
+}
+// up sweep: the start hits of this row that no up pass has recorded build a tracklet; returns how many (this thread)
+__device__ TPC_CT_INL unsigned ct_intake_up(const View& v, const Const& c, CtSmem& sm, const CtSlots& sl, const uint16_t* freel,
+                                              int cap, int row, int s, int S) {
+    const int D = c.p.link_step;
+    const bool dedup = c.p.seed_dedup != 0;
+    const int n = sm.cnt[row], lo = sm.lo[row], base = sm.desc[row].base;
+    const uint32_t* const ub = sm.used[row & 1];
+    unsigned built = 0;
+    for (int j0 = 0; j0 < n; j0 += kCtConsumers) {
+        const int j = j0 + (int)threadIdx.x, e = lo + j;
+        bool need = false;
+        int hl = 0;
+        float4 a4 = make_float4(0.f, 0.f, 0.f, 0.f);
+        int4 hh = make_int4(0, 0, 0, 0);
+        if (j < n && e < S) {
+            if (j < kCtSeedStage) {
+                a4 = *reinterpret_cast<const float4*>(&sm.seeds[s][j]);
+                hh = *(reinterpret_cast<const int4*>(&sm.seeds[s][j]) + 1);
+            } else {
+                a4 = __ldg(reinterpret_cast<const float4*>(&v.seed_rec[e]));
+                hh = __ldg(reinterpret_cast<const int4*>(&v.seed_rec[e]) + 1);
+            }
+            hl = hh.x - base;
+            if (dedup && ((ub[hl >> 5] >> (hl & 31)) & 1u)) v.tl_rows[e] = 0;   // skipped: n_hits = 0
+            else need = true;
+        }
+        const int slot = ct_pop(v, sm, freel, need, cap);
+        if (need && slot < 0) v.tl_rows[e] = 0;
+        if (slot >= 0) {
+            built++;
+            CtTrk t;
+            Fit& f = t.f;
+            f.y = a4.x; f.z = a4.y; f.s = a4.z; f.t = a4.w; f.q = 0.f;   // direction of the first link, from K4
+            fit_prior(f, c); f.n = 0;
+            t.p0 = a4.x; t.p1 = a4.y; t.p2 = f.s; t.p3 = f.t; t.p4 = f.q;
+            t.p5 = __uint_as_float(((uint32_t)kNoHit << 16) | (uint32_t)hl);   // table entries: below the top hit | of the row before
+            t.i = e; t.cur = hh.y; t.nxt = hh.z; t.ph = 1; t.miss = 0; t.r0 = row; t.top = row; t.aux = row + D;
+            v.tl_tab[(size_t)e * v.tab_stride + row] = (uint16_t)hl;
+            sl.store(t, slot);
+        }
     }
-};
+    return built;
+}
+// between the sweeps (all consumer warps): the parked tracklets of the task, ordered by top row, into dn_rec
+__device__ TPC_CT_INL void ct_turn(const View& v, CtSmem& sm, int nr) {
+    const int lane = lane_id(), warp = threadIdx.x >> 5;
+    if (warp == 0) {   // lo = exclusive scan of the counts, cnt = the counts, dcnt = 0 (fill counters of the scatter)
+        int carry = 0;
+        for (int r0 = 0; r0 < nr; r0 += 32) {
+            const int r = r0 + lane;
+            const int c = r < nr ? sm.dcnt[r] : 0;
+            int incl = c;
+#pragma unroll
+            for (int o = 1; o < 32; o <<= 1) { const int x = __shfl_up_sync(kFull, incl, o); if (lane >= o) incl += x; }
+            if (r < nr) { sm.lo[r] = carry + incl - c; sm.cnt[r] = c; sm.dcnt[r] = 0; }
+            carry += __shfl_sync(kFull, incl, 31);
+        }
+    }
+    ct_bar();
+    const uint32_t* const plist = v.kf_park + sm.i0;
+    const int np = sm.n_parked;
+    for (int k = threadIdx.x; k < np; k += kCtConsumers) {
+        const uint32_t w = __ldcg(&plist[k]);
+        const int top = (int)(w >> 24), id = sm.i0 + (int)(w & 0xffffffu);
+        const int pos = sm.lo[top] + atomicAdd(&sm.dcnt[top], 1);
+        const float4 a4 = __ldcg(reinterpret_cast<const float4*>(&v.tl_up[id]));
+        const float4 b4 = __ldcg(reinterpret_cast<const float4*>(&v.tl_up[id]) + 1);
+        float4* dst = reinterpret_cast<float4*>(&v.dn_rec[sm.i0 + pos]);
+        dst[0] = a4; dst[1] = b4;
+    }
+    asm volatile("fence.proxy.async;" ::: "memory");   // the producer's bulk copies (async proxy) will read these records
+    ct_bar();
+}
 
 // ---------------------------------------------------------------------------------------------------------
 // K5
 // ---------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kCtThreads, 2) k_construct(const View v, const __grid_constant__ Const c, const int cap_s,
+__global__ void __launch_bounds__(kCtThreads, 2) k_construct(const __grid_constant__ View v, const __grid_constant__ Const c, const int cap_s,
                                                              const int cap_g, float* const spill) {
     extern __shared__ __align__(128) unsigned char ct_raw[];
     CtSmem& sm = *reinterpret_cast<CtSmem*>(ct_raw);
@@ -315,18 +459,31 @@ __global__ void __launch_bounds__(kCtThreads, 2) k_construct(const View v, const
     if (warp == kCtWarps) { ct_producer(v, c, sm, freel, cap); return; }
 
     const int nr = c.n_rows, D = c.p.link_step;
-    const int ctid = threadIdx.x;                       // consumer threads are 0 .. kCtConsumers-1
     const int S = min(v.seed_start[v.n_bins], v.S_cap);
-    const bool dedup = c.p.seed_dedup != 0;
     volatile int32_t* const abort = &sm.abort;
     unsigned visits = 0, updates = 0, built = 0;
     uint32_t it = 0;
+#ifdef TPC_CT_PROF
+    long long pf[16] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0}, tq = clock64();
+#define PF(k) { const long long n_ = clock64(); pf[k] += n_ - tq; tq = n_; }
+#else
+#define PF(k)
+#endif
 
     for (;;) {
         const int s = (int)(it % kCtRing);
+        PF(7)
         if (!mbar_wait(&sm.full[s], (it / kCtRing) & 1u, abort)) break;
+        PF(0)
         const int cmd = sm.cmd[s];
         if (cmd < 0) break;
+        if (cmd == kCtTurn) {
+            ct_turn(v, sm, nr);
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&sm.empty[s]);
+            it++;
+            continue;
+        }
         const int row = cmd & 0xff;
         const bool up = !(cmd & kCtDown);
         const int tb = sm.task * nr;
@@ -336,56 +493,38 @@ __global__ void __launch_bounds__(kCtThreads, 2) k_construct(const View v, const
         const size_t cg = cell_index(dn.x, tb + row);
         const float2* const hits = staged ? reinterpret_cast<const float2*>(sm.hits[s]) + (dn.x & 1) : v.shit + dn.x;
         const uint16_t* const cs = staged ? reinterpret_cast<const uint16_t*>(sm.cells[s]) + (cg & 7) : v.cells + cg;
-        uint32_t* const plist = reinterpret_cast<uint32_t*>(v.dn_rec) + sm.i0;   // parked tracklets of this task
+        uint32_t* const plist = v.kf_park + sm.i0;   // parked tracklets of this task, in order of parking
 
-        if (!up) {
-            // ---- down sweep, intake: the parked tracklets whose top hit is in this row start a fresh fit there ----
-            const int np = sm.n_parked;
-            for (int k0 = 0; k0 < np; k0 += kCtConsumers) {
-                const int k = k0 + ctid;
-                uint32_t w = 0;
-                bool need = false;
-                if (k < np) { w = __ldcg(&plist[k]); need = (int)(w >> 24) == row; }
-                const int slot = ct_pop(v, sm, freel, need, cap);
-                if (slot >= 0) {
-                    const int id = sm.i0 + (int)(w & 0xffffffu);
-                    const float4 a4 = __ldcg(reinterpret_cast<const float4*>(&v.tl_up[id]));
-                    const float4 b4 = __ldcg(reinterpret_cast<const float4*>(&v.tl_up[id]) + 1);
-                    CtTrk t;
-                    t.p0 = a4.x; t.p1 = a4.y; t.p2 = a4.z; t.p3 = a4.w; t.p4 = b4.x; t.p5 = 0.f;
-                    t.r0 = __float_as_int(b4.y); t.top = row; t.i = id;
-                    t.f.y = t.p0; t.f.z = t.p1; t.f.s = t.p2; t.f.t = t.p3; t.f.q = t.p4;
-                    fit_prior(t.f, c); t.f.n = 1;
-                    t.aux = row; t.miss = 0; t.ph = 3;
-                    t.cur = row > t.r0 ? (int)v.tl_tab[(size_t)id * v.tab_stride + row - 1] : (int)kNoHit;
-                    sl.store(t, slot);
-                }
-            }
+        if (!up) {   // down sweep: what starts at this row is taken in BEFORE the row is processed (and starts below it)
+            if (sm.cnt[row] > 0) ct_intake_down(v, c, sm, sl, freel, cap, row, s);
             ct_bar();
         }
-
-        // ---- one pad row for the tracklets under way ----
+        PF(1)
+        // ---- one pad row for the tracklets under way: the warps share the groups of 32 slots ----
         const int n_groups = (*(volatile int32_t*)&sm.n_hw + 31) >> 5;
         for (int g = warp; g < n_groups; g += kCtWarps) {
             const uint32_t occ = *(volatile uint32_t*)&sm.occ[g];
             if (!occ) continue;
             const int slot = (g << 5) + lane;
-            CtTrk t;
             bool on = (occ >> lane) & 1u;
+            CtTrk t;
             if (on) sl.load(t, slot);
             if (on && !up && t.top == row) on = false;          // taken in at this very row: starts below
             Fit& f = t.f;
             uint16_t* const gt = v.tl_tab + (size_t)(on ? t.i : 0) * v.tab_stride;
             bool end = false, search = false, counted = false;
-            int acc = -1;
+            int acc = -1, nn = -1;
             uint16_t eold = kNoHit;
             float ay = 0.f, az = 0.f, iwy = 0.f, iwz = 0.f;
             // part 1: transport and the candidate that is already known
             if (on) {
-                int nxt = -1, known = -1;
+                int known = -1;
                 float ky = 0.f, kz = 0.f;
                 if (up) {
-                    if (t.ph == 1 && row == t.aux) { known = t.cur; nxt = __ldg(&v.clink_up[t.cur]); const float2 hk = hits[t.cur - dn.x]; ky = hk.x; kz = hk.y; }
+                    if (t.ph == 1 && row == t.aux) {
+                        known = t.cur;
+                        const float2 hk = hits[t.cur - dn.x]; ky = hk.x; kz = hk.y;
+                    }
                 } else if (row >= t.r0) {
                     eold = (uint16_t)t.cur;
                     if (row > t.r0) t.cur = gt[row - 1];
@@ -404,7 +543,9 @@ __global__ void __launch_bounds__(kCtThreads, 2) k_construct(const View v, const
                     if (up) {
                         if (t.ph == 1) {
                             if (row == t.aux) {
-                                if (gate_ok) { t.cur = nxt; t.aux += D; if (nxt < 0) t.ph = 2; }
+                                // the link above the next linked hit: needed one link from now, the load has a whole row
+                                if (gate_ok && t.nxt >= 0) nn = __ldg(&v.clink_up[t.nxt]);
+                                if (gate_ok) { t.cur = t.nxt; t.nxt = nn; t.aux += D; if (t.cur < 0) t.ph = 2; }
                                 else { t.ph = 2; search = true; counted = true; }
                             }   // else: in-between row of a step-2 link
                         } else {
@@ -439,6 +580,10 @@ __global__ void __launch_bounds__(kCtThreads, 2) k_construct(const View v, const
                     const uint16_t enew = acc >= 0 ? (uint16_t)(acc - dn.x) : kNoHit;
                     if (up || row < t.r0 || enew != eold) gt[row] = enew;
                     upd = acc >= 0;
+                    if (up) {   // p5 = table entry below the top hit << 16 | entry of the row before this one -> of this one
+                        const uint32_t q = __float_as_uint(t.p5);
+                        t.p5 = __uint_as_float((upd ? q << 16 : q & 0xffff0000u) | enew);
+                    }
                 }
             }
             __syncwarp();
@@ -454,73 +599,49 @@ __global__ void __launch_bounds__(kCtThreads, 2) k_construct(const View v, const
                 }
             }
             __syncwarp();
-            if (on) {
-                if (end || row == (up ? nr - 1 : 0)) {
-                    if (up) {   // park: a fresh fit will start at the top hit in the down sweep
-                        float4* dst = reinterpret_cast<float4*>(&v.tl_up[t.i]);
-                        dst[0] = make_float4(t.p0, t.p1, t.p2, t.p3);
-                        dst[1] = make_float4(t.p4, __int_as_float(t.r0), __int_as_float(t.top), __int_as_float(t.i));
-                        const int k = atomicAdd(&sm.n_parked, 1);
-                        plist[k] = (uint32_t)(t.i - sm.i0) | ((uint32_t)t.top << 24);
-                        atomicMax(&sm.top_max, t.top);
-                    } else {
-                        v.tl_rows[t.i] = t.aux | (t.top << 8) | (f.n << 16);
-                        const int sc = v.S_cap;
-                        v.tl_par[t.i] = t.p0; v.tl_par[sc + t.i] = t.p1; v.tl_par[2 * sc + t.i] = t.p2; v.tl_par[3 * sc + t.i] = t.p3;
-                        v.tl_par[4 * sc + t.i] = t.p4; v.tl_par[5 * sc + t.i] = t.p5;
-                    }
-                    ct_push(sm, freel, slot, cap);
+            const bool fin = on && (end || row == (up ? nr - 1 : 0));
+            if (fin) {
+                if (up) {   // park: a fresh fit will start at the top hit in the down sweep
+                    float4* dst = reinterpret_cast<float4*>(&v.tl_up[t.i]);
+                    const int below = t.top > t.r0 ? (int)(__float_as_uint(t.p5) >> 16) : (int)kNoHit;
+                    dst[0] = make_float4(t.p0, t.p1, t.p2, t.p3);
+                    dst[1] = make_float4(t.p4, __int_as_float(t.r0 | (t.top << 8)), __int_as_float(below), __int_as_float(t.i));
+                    const int k = atomicAdd(&sm.n_parked, 1);
+                    plist[k] = (uint32_t)(t.i - sm.i0) | ((uint32_t)t.top << 24);
+                    atomicAdd(&sm.dcnt[t.top], 1);
+                    atomicMax(&sm.top_max, t.top);
                 } else {
-                    sl.store(t, slot);
+                    v.tl_rows[t.i] = t.aux | (t.top << 8) | (f.n << 16);
+                    const int sc = v.S_cap;
+                    v.tl_par[t.i] = t.p0; v.tl_par[sc + t.i] = t.p1; v.tl_par[2 * sc + t.i] = t.p2; v.tl_par[3 * sc + t.i] = t.p3;
+                    v.tl_par[4 * sc + t.i] = t.p4; v.tl_par[5 * sc + t.i] = t.p5;
                 }
+            } else if (on) {
+                sl.store(t, slot);
             }
+            const unsigned gone = __ballot_sync(kFull, fin);    // this warp alone owns the group's occupancy word now
+            if (gone && lane == 0) sm.occ[g] = occ & ~gone;
+            if (fin) ct_push(sm, freel, slot, cap);
         }
+        PF(3)
         ct_bar();
-
-        if (up) {
-            // ---- up sweep, intake: the start hits of this row that no up pass has recorded build a tracklet ----
-            const int n = sm.cnt[row];
-            const uint32_t* const ub = sm.used[row & 1];
-            for (int j0 = 0; j0 < n; j0 += kCtConsumers) {
-                const int j = j0 + ctid;
-                bool need = false;
-                int e = 0, hl = 0;
-                float4 a4 = make_float4(0.f, 0.f, 0.f, 0.f);
-                int2 h01 = make_int2(0, 0);
-                if (j < n) {
-                    e = sm.lo[row] + j;
-                    if (e < S) {
-                        a4 = __ldg(reinterpret_cast<const float4*>(&v.seed_rec[e]));
-                        h01 = __ldg(reinterpret_cast<const int2*>(&v.seed_rec[e]) + 2);
-                        hl = h01.x - dn.x;
-                        if (dedup && ((ub[hl >> 5] >> (hl & 31)) & 1u)) v.tl_rows[e] = 0;   // skipped: n_hits = 0
-                        else need = true;
-                    }
-                }
-                const int slot = ct_pop(v, sm, freel, need, cap);
-                if (need && slot < 0) v.tl_rows[e] = 0;
-                if (slot >= 0) {
-                    built++;
-                    CtTrk t;
-                    Fit& f = t.f;
-                    const float dx = c.row_x[row + D] - c.row_x[row];
-                    const float dy = a4.z - a4.x, dz = a4.w - a4.y;
-                    const float dl = sqrtf(dx * dx + dy * dy);
-                    f.y = a4.x; f.z = a4.y; f.s = dy / dl; f.t = dz / dl; f.q = 0.f;
-                    fit_prior(f, c); f.n = 0;
-                    t.p0 = a4.x; t.p1 = a4.y; t.p2 = f.s; t.p3 = f.t; t.p4 = f.q; t.p5 = 0.f;
-                    t.i = e; t.cur = h01.y; t.ph = 1; t.miss = 0; t.r0 = row; t.top = row; t.aux = row + D;
-                    v.tl_tab[(size_t)e * v.tab_stride + row] = (uint16_t)hl;
-                    sl.store(t, slot);
-                }
-            }
-            for (int k = ctid; k < TPC_MAX_ROW_HITS / 32; k += kCtConsumers) sm.used[(row + 1) & 1][k] = 0u;
+        PF(4)
+        if (up) {   // up sweep: the start hits of this row are taken in AFTER it is processed (its marks are complete)
+            if (sm.cnt[row] > 0) built += ct_intake_up(v, c, sm, sl, freel, cap, row, s, S);
+            PF(8)
+            for (int k = threadIdx.x; k < TPC_MAX_ROW_HITS / 32; k += kCtConsumers) sm.used[(row + 1) & 1][k] = 0u;
+            PF(9)
             ct_bar();
         }
+        PF(5)
         __syncwarp();
         if (lane == 0) mbar_arrive(&sm.empty[s]);
         it++;
     }
+#ifdef TPC_CT_PROF
+    if (lane == 0 && warp == 0)   // cycles of warp 0 by phase, summed over the CTAs
+        for (int k = 0; k < 16; k++) atomicAdd(&v.cnt[CNT_PROF + k], (unsigned long long)pf[k]);
+#endif
     unsigned long long vs = visits, us = updates, bs = built;
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {

@@ -92,6 +92,7 @@ struct Batch {
     Buf<BinDesc> desc;
     Buf<SeedRec> seed_rec;
     Buf<UpRec> tl_up, dn_rec;
+    Buf<uint32_t> kf_park;
     Buf<int32_t> dn_count, dn_start, dn_fill, tl_cnt;
     int sel_C = 1;                           // selector chunks per sector task
     int ct_tier = 0;                         // K5 slot tier used by this group's last launch
@@ -122,7 +123,7 @@ struct Batch {
         scratch.release(); o_hit.release();
         for (auto& b : o_i) b.release();
         slot.release(); cells.release(); desc.release(); owner.release(); ev_src.release();
-        seed_rec.release(); tl_up.release(); dn_rec.release(); dn_count.release(); dn_start.release(); dn_fill.release(); tl_cnt.release(); o_hit_yz.release(); o_hit_row.release(); trk_hit0.release(); trk_rows.release(); trk_task.release(); mg_next.release(); mg_prev.release(); mg_list.release();
+        seed_rec.release(); tl_up.release(); dn_rec.release(); kf_park.release(); dn_count.release(); dn_start.release(); dn_fill.release(); tl_cnt.release(); o_hit_yz.release(); o_hit_row.release(); trk_hit0.release(); trk_rows.release(); trk_task.release(); mg_next.release(); mg_prev.release(); mg_list.release();
         cnt.release(); kf_cursor.release(); h_ev_src.release(); h_sec_off.release(); h_ev_off.release(); h_cnt.release(); h_nseeds.release();
         for (auto& e : evt) if (e) { cudaEventDestroy(e); e = nullptr; }
         if (kernels_done) { cudaEventDestroy(kernels_done); kernels_done = nullptr; }
@@ -209,7 +210,7 @@ int reserve_batch(const tpc_tracker* tr, Batch* t, int n_events, int64_t N, int6
     RS(link_up, n); RS(link_dn, n); RS(clink_up, n); RS(clink_dn, n); RS(owner, n);
     RS(seeds, S_cap); RS(seed_bin, S_cap); RS(tl_rows, S_cap); RS(tl_par, 6 * (size_t)S_cap);
     RS(tl_tab, (size_t)S_cap * tab_stride(tr->c.n_rows));
-    RS(seed_rec, S_cap); RS(tl_up, S_cap); RS(dn_rec, S_cap); RS(dn_count, nb + 1); RS(dn_start, nb + 1); RS(dn_fill, nb + 1);
+    RS(seed_rec, S_cap); RS(tl_up, S_cap); RS(dn_rec, S_cap); RS(kf_park, S_cap); RS(dn_count, nb + 1); RS(dn_start, nb + 1); RS(dn_fill, nb + 1);
     RS(tl_nown, S_cap + 1); RS(tl_keep, S_cap + 1); RS(tl_cnt, (size_t)t->sel_C * S_cap); RS(trk_scan, S_cap + 2); RS(hit_scan, S_cap + 2);
     RS(ev_off_d, 2 * ((size_t)n_events + 1)); RS(h_ev_off, 2 * ((size_t)n_events + 1));
     RS(scratch, (size_t)std::max<int64_t>(nb, S_cap) / kScanTile + 8);
@@ -283,7 +284,7 @@ int launch_all(const tpc_tracker* tr, Batch* t) {
     mark(2);
     k_clean<<<nb, kCleanThreads, 0, st>>>(v); L++;
     L += scan_exclusive(v.seed_count, v.seed_start, nb, t->scratch.p, st);
-    k_seeds<<<nb, kSeedThreads, 0, st>>>(v); L++;
+    k_seeds<<<nb, kSeedThreads, 0, st>>>(v, c); L++;
     mark(3);
     {   // K5: one CTA per sector task, up sweep then down sweep (kf_construct.cuh)
         const int tier = t->ct_tier;
@@ -390,7 +391,7 @@ int batch_begin(const tpc_tracker* tr, Batch* t, int first_event, int n, const t
     v.o_next = t->o_i[4].p; v.o_prev = t->o_i[5].p; v.o_global = t->o_i[6].p; v.trk_rows = t->trk_rows.p; v.trk_task = t->trk_task.p;
     v.cnt = t->cnt.p; v.kf_cursor = t->kf_cursor.p;
     v.o_hit_yz = t->o_hit_yz.p; v.o_hit_row = t->o_hit_row.p; v.trk_hit0 = t->trk_hit0.p;
-    v.seed_rec = t->seed_rec.p; v.tl_up = t->tl_up.p; v.dn_rec = t->dn_rec.p;
+    v.seed_rec = t->seed_rec.p; v.tl_up = t->tl_up.p; v.dn_rec = t->dn_rec.p; v.kf_park = t->kf_park.p;
     v.dn_count = t->dn_count.p; v.dn_start = t->dn_start.p; v.dn_fill = t->dn_fill.p;
     t->ct_tier = std::max(t->ct_tier, tr->ct_tier);
     if (kCtCapSpill[t->ct_tier] > 0) {   // slots in global memory for every resident CTA (allocated once, on the way up)
@@ -451,6 +452,11 @@ int batch_finish(const tpc_tracker* tr, Batch* t) {
         t->counters.n_updates = (int64_t)t->h_cnt.p[CNT_UPDATES];
         t->counters.n_refit_visits = (int64_t)t->h_cnt.p[CNT_REFIT_VISITS];
         t->counters.n_tracklets = (int64_t)t->h_cnt.p[CNT_TRACKLETS];
+#ifdef TPC_CT_PROF
+        fprintf(stderr, "K5 warp-0 cycles by phase (0 wait-row, 1 intake-dn + barrier, 3 groups, 4 barrier, 5 intake-up + barrier, 7 loop):");
+        for (int k = 0; k < 14; k++) fprintf(stderr, " %.3g", (double)t->h_cnt.p[CNT_PROF + k]);
+        fprintf(stderr, "\n");
+#endif
         return TPC_OK;
     }
 }
