@@ -76,15 +76,21 @@ typedef struct {
     int32_t seed_dedup;         /* 1 (default): a start hit that the up pass of a tracklet built from a lower pad row of
                                  * its sector has already recorded builds no tracklet (R23).
                                  * 0: every start hit is fitted (round-1 behaviour, ~3 tracklets per output track) */
+    int32_t checked;            /* 0 (default) fast mode: cluster coordinates are trusted; a non-finite y or z, or an x
+                                 * that is not row_x[row], gives undefined TRACKS (never a memory fault; a row outside
+                                 * [0, n_rows) is still reported).  1 checked mode: the first
+                                 * kernel also tests every cluster -- y, z finite, and, where x is given (non-NULL),
+                                 * |x - row_x[row]| <= 1e-3 cm -- and the call returns TPC_ERR_ARG otherwise */
 } tpc_params;
 
-/* One event's clusters: SoA, grouped by sector, ANY order inside a sector.
+/* One event's clusters: SoA, grouped by sector, ANY order inside a sector.  Fast mode (tpc_params.checked = 0) trusts
+ * the coordinates: see tpc_params.checked.
  * mem_space 0: x, y, z, row are host pointers; the call copies them to the device (pinned memory makes the
  *              copy asynchronous) and the outputs come back in library-owned pinned host memory.
  * mem_space 1: x, y, z, row are device pointers (must stay valid and unchanged until the call returns); the
  *              outputs are library-owned device memory.
  * sector_offset is ALWAYS a host pointer.  x is redundant with row_x[row]: the library reads row and ignores x
- * (x may be NULL). */
+ * (x may be NULL), except in checked mode, which compares the two. */
 typedef struct {
     int32_t n_clusters;
     const int32_t* sector_offset; /* [n_sectors+1] host, non-decreasing, [0] = 0, [n_sectors] = n_clusters */
@@ -184,7 +190,8 @@ int tpc_track_events(tpc_tracker* t, int32_t n, const tpc_event_in* in, tpc_even
  * with a ticket (0 or 1); at most two batches are in flight (a third submit returns TPC_ERR_ARG).  The `in` array,
  * the sector offsets and the cluster arrays must stay valid and unchanged until the matching wait returns.
  * tpc_wait_events waits for that batch, copies the outputs back (host inputs) and fills out[0..n).  The outputs
- * are library-owned and stay valid until the second submit after this wait, or destroy.  The batch runs as one
+ * are library-owned (each ticket has its own output arrays, host or device) and stay valid until the next wait on
+ * the same ticket number -- so at least until the second submit after this wait -- or destroy.  The batch runs as one
  * group; results are those of tpc_track_events.  Intermediates (tpc_debug_get) are not kept for these batches. */
 int tpc_submit_events(tpc_tracker* t, int32_t n, const tpc_event_in* in, int32_t* ticket);
 int tpc_wait_events(tpc_tracker* t, int32_t ticket, tpc_event_out* out);
@@ -220,6 +227,26 @@ int tpc_get_stage_ms(const tpc_tracker* t, float* ms /* [TPC_N_STAGES] */);
 #define TPC_DBG_SORTED 8     /* int32 [n_clusters(event)]  caller's index of each cluster in (sector,row,cell) order */
 int64_t tpc_debug_size(const tpc_tracker* t, int32_t what, int32_t event); /* bytes, or negative status */
 int tpc_debug_get(tpc_tracker* t, int32_t what, int32_t event, void* buf, size_t bytes);
+
+/* ---- stage-isolated parity ("GPU stage k on the reference's output of stage k-1") ----
+ * tpc_debug_inject overwrites one intermediate of event `event` of the last call with the caller's values (same
+ * layouts, sizes and index convention as tpc_debug_get; buf is a HOST buffer of exactly tpc_debug_size bytes).
+ * Items: TPC_DBG_LINK_UP / LINK_DN (input of K3), TPC_DBG_CLINK_UP / CLINK_DN (input of K4 and K5),
+ * TPC_DBG_TL_ROWS / TL_PAR / TL_TABLE (input of K6; rows with n_hits = 0 mean "no tracklet").  The start-hit list
+ * is not injectable: it is a function of the cleaned links (K4).
+ * tpc_debug_resume then runs the path again FROM a stage on what the work space now holds, for all events of
+ * the last call, and fills out[0 .. n_events) like the call itself did:
+ *   TPC_STAGE_CLEAN (K3, K4, K5, K6): after injecting links;
+ *   TPC_STAGE_SEEDS (K4 from the cleaned links as they stand, K5, K6): after injecting cleaned links;
+ *   TPC_STAGE_CONSTRUCT (K5, K6);  TPC_STAGE_SELECT (K6 only): after injecting tracklets.
+ * Both need a last call with device inputs (mem_space 1) made through tpc_track_event(s) that ran as one group, and
+ * return TPC_ERR_ARG otherwise.  The counters afterwards cover the stages that ran again. */
+#define TPC_STAGE_CLEAN 3
+#define TPC_STAGE_SEEDS 4
+#define TPC_STAGE_CONSTRUCT 5
+#define TPC_STAGE_SELECT 6
+int tpc_debug_inject(tpc_tracker* t, int32_t what, int32_t event, const void* buf, size_t bytes);
+int tpc_debug_resume(tpc_tracker* t, int32_t from_stage, tpc_event_out* out);
 
 #ifdef __cplusplus
 }

@@ -42,7 +42,7 @@ class Params(C.Structure):
         ("refit", C.c_int32),
         ("merge", C.c_int32), ("merge_dy", C.c_float), ("merge_dz", C.c_float), ("merge_ds", C.c_float),
         ("merge_dt", C.c_float), ("merge_max_gap", C.c_int32),
-        ("seed_dedup", C.c_int32),
+        ("seed_dedup", C.c_int32), ("checked", C.c_int32),
     ]
 
     def as_dict(self):

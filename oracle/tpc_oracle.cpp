@@ -64,6 +64,7 @@ typedef struct {
     int32_t merge_max_gap;      /* pad rows that may be missing between the two segments */
     int32_t seed_dedup;         /* O5: 1 = a start hit already recorded by the up pass of an earlier tracklet of its
                                  * sector is skipped (no tracklet is built from it); reading R23 */
+    int32_t checked;            /* 1 = reject non-finite y / z (the oracle is given no x); S23 */
 } oracle_params;
 
 typedef struct {
@@ -696,6 +697,7 @@ void oracle_default_params(oracle_params* p) {
     p->refit = 0;
     p->merge = 0; p->merge_dy = 1.0f; p->merge_dz = 1.0f; p->merge_ds = 0.05f; p->merge_dt = 0.05f; p->merge_max_gap = 6;
     p->seed_dedup = 1;
+    p->checked = 0;
 }
 
 /* precision: 0 = double, 1 = strict float32.  stop_after: 0 = everything, 2 = after O2, 4 = after O4,
@@ -705,8 +707,10 @@ void* oracle_track_event(const oracle_geometry* G, const oracle_params* P, int32
                          int32_t n_threads, int32_t stop_after) {
     if (!G || !P || !sector_offset || G->n_rows <= 0 || G->n_sectors <= 0) return nullptr;
     if (P->link_step < 1 || P->link_step > 2) return nullptr;
-    for (int32_t i = 0; i < n_clusters; i++)
+    for (int32_t i = 0; i < n_clusters; i++) {
         if (row[i] < 0 || row[i] >= G->n_rows) return nullptr;
+        if (P->checked && !(std::isfinite(y[i]) && std::isfinite(z[i]))) return nullptr;
+    }
     if (precision == 1) return run<float>(*G, *P, n_clusters, sector_offset, y, z, row, n_threads, stop_after);
     return run<double>(*G, *P, n_clusters, sector_offset, y, z, row, n_threads, stop_after);
 }

@@ -24,7 +24,7 @@ constexpr int kCountPer = 8;                    // clusters per thread
 constexpr int kCountChunk = 256 * kCountPer;    // clusters per CTA
 constexpr int kCountBins = 2048;                // (sector,row) bins of a chunk counted in shared memory
 
-__global__ void __launch_bounds__(256) k_count(const View v, int ns, int nr) {
+__global__ void __launch_bounds__(256) k_count(const View v, const __grid_constant__ Const c, int ns, int nr) {
     __shared__ int32_t so[64 + 1];
     __shared__ int32_t hist[kCountBins];   // clusters of this chunk per bin, then the chunk's first slot in the bin
     const int e = blockIdx.y;
@@ -50,6 +50,12 @@ __global__ void __launch_bounds__(256) k_count(const View v, int ns, int nr) {
         if (i < i1) {
             const int r = src.row[i];
             if (r < 0 || r >= nr) { atomicOr((unsigned int*)&v.cnt[CNT_ERR], kErrBadRow); continue; }
+            if (c.p.checked) {   // S23: coordinates finite, x on its pad row
+                const float yy = src.y[i], zz = src.z[i];
+                bool bad = !(fabsf(yy) <= 3.0e38f) || !(fabsf(zz) <= 3.0e38f);
+                if (src.x) bad = bad || !(fabsf(src.x[i] - c.row_x[r]) <= 1.0e-3f);
+                if (bad) atomicOr((unsigned int*)&v.cnt[CNT_ERR], kErrBadInput);
+            }
             int s = s_lo;
             while (i >= so[s + 1]) s++;
             const int bl = (s - s_lo) * nr + r;
@@ -219,6 +225,7 @@ __global__ void __launch_bounds__(kNfThreads, TPC_NF_BLOCKS) k_neighbours(const 
     constexpr int kNfCells = kCellsPerHit * kNfCap + kCellPad;   // cell-table entries held in shared memory
     __shared__ uint16_t s_cu[kNfCells], s_cd[kNfCells];
     __shared__ uint16_t s_dl[kNfList][kNfThreads];
+    TPC_RETURN_IF_REJECTED(v);
     const int bin = blockIdx.x;
     const int nr = c.n_rows, D = c.p.link_step;
     const int r = bin % nr;
@@ -322,8 +329,11 @@ __global__ void __launch_bounds__(kNfThreads, TPC_NF_BLOCKS) k_neighbours(const 
 // ---------------------------------------------------------------------------------------------------------
 constexpr int kCleanThreads = 128;
 
+// CLEAN false (stage-isolated runs, tpc_debug_resume): the cleaned links are taken as they stand
+template <bool CLEAN>
 __global__ void __launch_bounds__(kCleanThreads) k_clean(const View v) {
     __shared__ int nstart, nlink;
+    TPC_RETURN_IF_REJECTED(v);
     const int bin = blockIdx.x;
     const int b0 = v.bin_start[bin], n = v.bin_start[bin + 1] - b0;
     if (threadIdx.x == 0) { nstart = 0; nlink = 0; }
@@ -334,11 +344,16 @@ __global__ void __launch_bounds__(kCleanThreads) k_clean(const View v) {
         bool st = false;
         if (k < n) {
             const int h = b0 + k;
-            const int u = v.link_up[h], d = v.link_dn[h];
-            const int cu = (u >= 0 && v.link_dn[u] == h) ? u : -1;
-            const int cd = (d >= 0 && v.link_up[d] == h) ? d : -1;
-            v.clink_up[h] = cu;
-            v.clink_dn[h] = cd;
+            int cu, cd;
+            if (CLEAN) {
+                const int u = v.link_up[h], d = v.link_dn[h];
+                cu = (u >= 0 && v.link_dn[u] == h) ? u : -1;
+                cd = (d >= 0 && v.link_up[d] == h) ? d : -1;
+                v.clink_up[h] = cu;
+                v.clink_dn[h] = cd;
+            } else {
+                cu = v.clink_up[h]; cd = v.clink_dn[h];
+            }
             st = cu >= 0 && cd < 0;
             nl += (cu >= 0);
         }
@@ -369,6 +384,7 @@ constexpr int kSeedThreads = 128;
 __global__ void __launch_bounds__(kSeedThreads) k_seeds(const View v, const __grid_constant__ Const c) {
     __shared__ int list_h[TPC_MAX_ROW_HITS];
     __shared__ int list_o[TPC_MAX_ROW_HITS];
+    TPC_RETURN_IF_REJECTED(v);
     const int bin = blockIdx.x;
     const int s0 = v.seed_start[bin], ns = v.seed_start[bin + 1] - s0;
     if (ns == 0) return;

@@ -20,7 +20,12 @@ constexpr unsigned kFull = 0xffffffffu;
 
 // error bits raised by kernels
 constexpr unsigned kErrBadRow = 1u, kErrRowCapacity = 2u, kErrSeedCapacity = 4u, kErrHang = 8u, kErrSelCapacity = 16u,
-                   kErrSlotCapacity = 32u;   // K5: more tracklets under way in a sector task than state slots
+                   kErrSlotCapacity = 32u,   // K5: more tracklets under way in a sector task than state slots
+                   kErrBadInput = 64u;       // checked mode: non-finite y / z, or x off its pad row
+constexpr unsigned kErrFatal = kErrBadRow | kErrRowCapacity | kErrBadInput;   // the later kernels do nothing after these
+
+// the stages after K1 start with this: a batch that K1 has rejected is not worked on (its arrays may be incomplete)
+#define TPC_RETURN_IF_REJECTED(v) do { if (*(volatile unsigned long long*)&(v).cnt[CNT_ERR] & kErrFatal) return; } while (0)
 
 // device counters (unsigned long long each)
 constexpr int kNCursors = 4;           // work cursors: [0] K5 sector tasks, [2] refit
@@ -28,6 +33,7 @@ enum { CNT_ERR = 0, CNT_LINKS, CNT_ROW_VISITS, CNT_TL_HITS, CNT_TRACKS, CNT_TRAC
 
 // One event's input arrays (device pointers) and its place in the batch-global cluster numbering.
 struct EventSrc {
+    const float* x;          // may be NULL; read in checked mode only
     const float* y;
     const float* z;
     const int32_t* row;

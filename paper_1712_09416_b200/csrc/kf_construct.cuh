@@ -442,6 +442,7 @@ __device__ TPC_CT_INL void ct_turn(const View& v, CtSmem& sm, int nr) {
 __global__ void __launch_bounds__(kCtThreads, 2) k_construct(const __grid_constant__ View v, const __grid_constant__ Const c, const int cap_s,
                                                              const int cap_g, float* const spill) {
     extern __shared__ __align__(128) unsigned char ct_raw[];
+    TPC_RETURN_IF_REJECTED(v);
     CtSmem& sm = *reinterpret_cast<CtSmem*>(ct_raw);
     const int cap = cap_s + cap_g;
     CtSlots sl;

@@ -42,9 +42,10 @@ __global__ void __launch_bounds__(kSelCtaThreads, 2) k_select_claim(const View v
     extern __shared__ uint32_t s_owner[];
     __shared__ int32_t s_base[TPC_MAX_ROWS + 2];
     __shared__ unsigned long long s_claimed;
+    TPC_RETURN_IF_REJECTED(v);
     const int C = v.sel_C, nr = c.n_rows;
     const int task = blockIdx.x / C, ch = blockIdx.x - task * C, tb = task * nr;
-    const int lane = lane_id(), warp = threadIdx.x >> 5, n_warps = kSelCtaThreads / 32;
+    const int lane = lane_id();
     int r_lo, r_hi;
     sel_chunk(v, tb, nr, ch, C, r_lo, r_hi);
     for (int r = r_lo + threadIdx.x; r <= r_hi; r += kSelCtaThreads) s_base[r - r_lo] = v.bin_start[tb + r];
@@ -61,7 +62,7 @@ __global__ void __launch_bounds__(kSelCtaThreads, 2) k_select_claim(const View v
     const int i0 = min(v.seed_start[tb], S), i1 = min(v.seed_start[tb + nr], S);
     // The task's row -> hit tables are one contiguous block; a thread takes 8 consecutive rows of one tracklet
     // (one 16-byte load), so the block streams through with every load independent of the others.
-    const int g_lo = r_lo >> 3, G = ((r_hi - 1) >> 3) - g_lo + 1;
+    const int g_lo = r_lo >> 3, G = max(((r_hi - 1) >> 3) - g_lo + 1, 1);   // (an empty chunk has r_hi == r_lo)
     const int n_units = (i1 - i0) * G;
     unsigned claimed = 0;
     for (int pass = 0; pass < 2; pass++) {
@@ -120,6 +121,7 @@ __global__ void __launch_bounds__(kSelCtaThreads, 2) k_select_write(const View v
     __shared__ int32_t s_base[TPC_MAX_ROWS + 2];
     __shared__ int32_t s_list[kSelTile];
     __shared__ int32_t s_n;
+    TPC_RETURN_IF_REJECTED(v);
     const int C = v.sel_C, nr = c.n_rows;
     const int task = blockIdx.x / C, ch = blockIdx.x - task * C, tb = task * nr;
     const int lane = lane_id(), warp = threadIdx.x >> 5, n_warps = kSelCtaThreads / 32;
@@ -137,7 +139,7 @@ __global__ void __launch_bounds__(kSelCtaThreads, 2) k_select_write(const View v
     // A lane takes 8 consecutive rows of one kept tracklet (one 16-byte load); the G row groups of a tracklet sit
     // in G neighbouring lanes, so a warp works on 32 / G tracklets at once and a segmented scan over the groups'
     // owned-hit counts gives every group its place in the track's hit list.
-    const int g_lo = r_lo >> 3, G = ((r_hi - 1) >> 3) - g_lo + 1;   // G <= 32
+    const int g_lo = r_lo >> 3, G = max(((r_hi - 1) >> 3) - g_lo + 1, 1);   // (an empty chunk has r_hi == r_lo)   // G <= 32
     const int T = 32 / G;
     const int tl = lane / G, gi = lane - tl * G, g = g_lo + gi;
     for (int tile = i0; tile < i1; tile += kSelTile) {

@@ -79,7 +79,7 @@ struct Batch {
     std::vector<int32_t> ev_n, ev_off;       // clusters per event, offset in the group
     tpc_counters counters;                   // of the group's last run
     // device pools
-    Buf<float> in_y, in_z, tl_par, o_f[kOutF];
+    Buf<float> in_x, in_y, in_z, tl_par, o_f[kOutF];
     Buf<float2> thit, shit;
     Buf<int32_t> in_row, sec_off, bin_count, bin_start, tidx, sorig, link_up, link_dn, clink_up, clink_dn, seed_count,
         seed_start, seeds, seed_bin, tl_rows, tl_nown, tl_keep, trk_scan, hit_scan, ev_off_d, scratch,
@@ -114,7 +114,7 @@ struct Batch {
         memset(&counters, 0, sizeof counters);
     }
     void free_all() {
-        in_y.release(); in_z.release(); thit.release(); shit.release(); tl_par.release();
+        in_x.release(); in_y.release(); in_z.release(); thit.release(); shit.release(); tl_par.release();
         for (auto& b : o_f) b.release();
         in_row.release(); sec_off.release(); bin_count.release(); bin_start.release(); tidx.release(); sorig.release();
         link_up.release(); link_dn.release(); clink_up.release(); clink_dn.release(); seed_count.release();
@@ -145,6 +145,8 @@ struct tpc_tracker {
     // the last call
     tpc_counters counters;
     bool have_result = false;
+    bool one_group = false;                  // the last call ran as one group of device-input events (inject / resume)
+    const tpc_event_in* last_in = nullptr;   // its events
     int n_events = 0;
     std::vector<int> ev_slot, ev_local;      // where the intermediates of each event are (-1: overwritten since)
     Buf<int32_t> h_o_i[kOutI], h_o_hit;          // host-input calls: the outputs of all groups, pinned
@@ -155,8 +157,10 @@ struct tpc_tracker {
     struct Async {
         Batch* b = nullptr;
         bool busy = false;
-        Buf<int32_t> h_o_i[kOutI], h_o_hit;
+        Buf<int32_t> h_o_i[kOutI], h_o_hit;      // host inputs: this ticket's outputs, pinned
         Buf<float> h_o_f[kOutF];
+        Buf<int32_t> d_o_i[kOutI], d_o_hit;      // device inputs: this ticket's outputs (swapped with the batch's at wait,
+        Buf<float> d_o_f[kOutF];                 // so that the batch's next run does not write over them)
     } async[2];
 
     tpc_tracker() {
@@ -180,9 +184,11 @@ struct tpc_tracker {
         slots.clear();
         for (auto& a : async) {
             if (a.b) { cudaStreamSynchronize(a.b->stream); a.b->free_all(); cudaStreamDestroy(a.b->stream); delete a.b; a.b = nullptr; }
-            a.h_o_hit.release();
+            a.h_o_hit.release(); a.d_o_hit.release();
             for (auto& b : a.h_o_i) b.release();
             for (auto& b : a.h_o_f) b.release();
+            for (auto& b : a.d_o_i) b.release();
+            for (auto& b : a.d_o_f) b.release();
         }
         for (auto s : own_streams) cudaStreamDestroy(s);
         own_streams.clear();
@@ -255,38 +261,45 @@ int validate(const tpc_tracker* t, int n, const tpc_event_in* in) {
 }
 
 // launch K1..K6 for the staged group; counts launches
-int launch_all(const tpc_tracker* tr, Batch* t) {
+// launch the stages from `from` on (1 = K1 ... 6 = K6; TPC_STAGE_*) for the staged group; counts launches
+int launch_all(const tpc_tracker* tr, Batch* t, int from = 1) {
     const View& v = t->v;
     const Const& c = tr->c;
     cudaStream_t st = t->stream;
     const int ns = c.n_sectors, nr = c.n_rows;
     const int nb = v.n_bins;
     int64_t L = 0;
-    CK(cudaMemsetAsync(v.bin_count, 0, sizeof(int32_t) * (nb + 1), st));
+    if (from <= 1) CK(cudaMemsetAsync(v.bin_count, 0, sizeof(int32_t) * (nb + 1), st));
     CK(cudaMemsetAsync(v.cnt, 0, sizeof(unsigned long long) * CNT_N, st));
     CK(cudaMemsetAsync(v.kf_cursor, 0, sizeof(unsigned long long) * kNCursors, st));
     auto mark = [&](int k) { if (tr->profiling) cudaEventRecord(t->evt[k], st); };
     mark(0);
     int maxn = 0;
     for (int e = 0; e < t->n_events; e++) maxn = std::max(maxn, t->ev_n[e]);
-    if (maxn > 0) {
-        dim3 g((maxn + kCountChunk - 1) / kCountChunk, t->n_events);
-        k_count<<<g, 256, 0, st>>>(v, ns, nr); L++;
+    if (from <= 1) {
+        if (maxn > 0) {
+            dim3 g((maxn + kCountChunk - 1) / kCountChunk, t->n_events);
+            k_count<<<g, 256, 0, st>>>(v, c, ns, nr); L++;
+        }
+        L += scan_exclusive(v.bin_count, v.bin_start, nb, t->scratch.p, st);
+        if (maxn > 0) {
+            dim3 g((maxn + 255) / 256, t->n_events);
+            k_scatter<<<g, 256, 0, st>>>(v, ns, nr); L++;
+        }
+        k_sort_row<<<nb, kSortThreads, 0, st>>>(v); L++;
     }
-    L += scan_exclusive(v.bin_count, v.bin_start, nb, t->scratch.p, st);
-    if (maxn > 0) {
-        dim3 g((maxn + 255) / 256, t->n_events);
-        k_scatter<<<g, 256, 0, st>>>(v, ns, nr); L++;
-    }
-    k_sort_row<<<nb, kSortThreads, 0, st>>>(v); L++;
     mark(1);
-    k_neighbours<<<nb, kNfThreads, 0, st>>>(v, c); L++;
+    if (from <= 2) { k_neighbours<<<nb, kNfThreads, 0, st>>>(v, c); L++; }
     mark(2);
-    k_clean<<<nb, kCleanThreads, 0, st>>>(v); L++;
-    L += scan_exclusive(v.seed_count, v.seed_start, nb, t->scratch.p, st);
-    k_seeds<<<nb, kSeedThreads, 0, st>>>(v, c); L++;
+    if (from <= 4) {
+        if (from <= 3) k_clean<true><<<nb, kCleanThreads, 0, st>>>(v);
+        else k_clean<false><<<nb, kCleanThreads, 0, st>>>(v);   // start hits of the cleaned links as they stand
+        L++;
+        L += scan_exclusive(v.seed_count, v.seed_start, nb, t->scratch.p, st);
+        k_seeds<<<nb, kSeedThreads, 0, st>>>(v, c); L++;
+    }
     mark(3);
-    {   // K5: one CTA per sector task, up sweep then down sweep (kf_construct.cuh)
+    if (from <= 5) {   // K5: one CTA per sector task, up sweep then down sweep (kf_construct.cuh)
         const int tier = t->ct_tier;
         const int grid = std::max(1, std::min(tr->ct_blocks[tier], v.n_tasks));
         k_construct<<<grid, kCtThreads, ct_smem_bytes(tier), st>>>(v, c, kCtCapSmem[tier], kCtCapSpill[tier], tr->ct_spill.p); L++;
@@ -342,29 +355,33 @@ int batch_begin(const tpc_tracker* tr, Batch* t, int first_event, int n, const t
             for (int s = 0; s < ns; s++)
                 max_task = std::max<int64_t>(max_task, in[e].sector_offset[s + 1] - in[e].sector_offset[s]);
         const int64_t room = kSelCap - TPC_MAX_ROW_HITS - 1;
-        const int C = (int)std::max<int64_t>(1, (max_task + room - 1) / room);
-        if (C > t->sel_C) { t->tl_cnt.release(); }
-        t->sel_C = std::max(t->sel_C, C);
+        t->sel_C = (int)std::max<int64_t>(1, (max_task + room - 1) / room);   // of THIS group (tl_cnt only grows)
     }
     if ((rc = reserve_batch(tr, t, n, N, S_cap)) != TPC_OK) return rc;
     if (t->host_in) {
         const size_t nn = (size_t)std::max<int64_t>(N, 1);
         if ((rc = t->in_y.reserve(nn)) != TPC_OK || (rc = t->in_z.reserve(nn)) != TPC_OK || (rc = t->in_row.reserve(nn)) != TPC_OK)
             return rc;
+        if (tr->c.p.checked && (rc = t->in_x.reserve(nn)) != TPC_OK) return rc;
     }
     // the event table and the sector offsets
     for (int e = 0; e < n; e++) {
         EventSrc& s = t->h_ev_src.p[e];
         s.n = in[e].n_clusters; s.off = t->ev_off[e];
+        s.x = nullptr;
         if (t->host_in) {
             s.y = t->in_y.p + s.off; s.z = t->in_z.p + s.off; s.row = t->in_row.p + s.off;
+            if (tr->c.p.checked && in[e].x) {
+                s.x = t->in_x.p + s.off;
+                if (copy_inputs && s.n > 0) CK(cudaMemcpyAsync(t->in_x.p + s.off, in[e].x, sizeof(float) * s.n, cudaMemcpyHostToDevice, st));
+            }
             if (copy_inputs && s.n > 0) {
                 CK(cudaMemcpyAsync(t->in_y.p + s.off, in[e].y, sizeof(float) * s.n, cudaMemcpyHostToDevice, st));
                 CK(cudaMemcpyAsync(t->in_z.p + s.off, in[e].z, sizeof(float) * s.n, cudaMemcpyHostToDevice, st));
                 CK(cudaMemcpyAsync(t->in_row.p + s.off, in[e].row, sizeof(int32_t) * s.n, cudaMemcpyHostToDevice, st));
             }
         } else {
-            s.y = in[e].y; s.z = in[e].z; s.row = in[e].row;
+            s.x = tr->c.p.checked ? in[e].x : nullptr; s.y = in[e].y; s.z = in[e].z; s.row = in[e].row;
         }
         memcpy(t->h_sec_off.p + (size_t)e * (ns + 1), in[e].sector_offset, sizeof(int32_t) * (ns + 1));
     }
@@ -423,6 +440,7 @@ int batch_finish(const tpc_tracker* tr, Batch* t) {
         const unsigned err = (unsigned)(t->h_cnt.p[CNT_ERR] & 0xffffffffu);
         const int32_t n_seeds = t->h_nseeds.p[0];
         if (err & kErrBadRow) { set_err("a cluster has row outside [0,%d)", nr); return TPC_ERR_ARG; }
+        if (err & kErrBadInput) { set_err("checked mode: a cluster has a non-finite y or z, or an x more than 1e-3 cm off row_x[row]"); return TPC_ERR_ARG; }
         if (err & kErrHang) { set_err("the constructor lost a shared-memory pipeline signal"); return TPC_ERR_CUDA; }
         if (err & kErrSelCapacity) { set_err("selector: a chunk of pad rows exceeds the shared-memory owner table"); return TPC_ERR_CAPACITY; }
         if (err & kErrRowCapacity) {
@@ -509,6 +527,7 @@ void tpc_default_params(tpc_params* p) {
     p->refit = 0;
     p->merge = 0; p->merge_dy = 1.0f; p->merge_dz = 1.0f; p->merge_ds = 0.05f; p->merge_dt = 0.05f; p->merge_max_gap = 6;
     p->seed_dedup = 1;
+    p->checked = 0;
 }
 
 const char* tpc_status_string(int s) {
@@ -541,7 +560,7 @@ tpc_tracker* tpc_tracker_create_ex(const tpc_geometry* g, float bz, const tpc_pa
     if (params) p = *params; else tpc_default_params(&p);
     if (p.link_step < 1 || p.link_step > 2 || p.min_tracklet_hits < 1 || p.min_track_hits < 1 || p.max_gap < 0 || p.max_gap > 60 ||
         p.seed_dedup < 0 || p.seed_dedup > 1 || p.refit < 0 || p.refit > 1 || p.merge < 0 || p.merge > 1 ||
-        (p.merge && !p.refit) || p.merge_max_gap < 0 || !(p.merge_dy > 0.f) || !(p.merge_dz > 0.f) || !(p.merge_ds > 0.f) || !(p.merge_dt > 0.f)) {
+        p.checked < 0 || p.checked > 1 || (p.merge && !p.refit) || p.merge_max_gap < 0 || !(p.merge_dy > 0.f) || !(p.merge_dz > 0.f) || !(p.merge_ds > 0.f) || !(p.merge_dt > 0.f)) {
         set_err("params: link_step must be 1 or 2, minimum hit counts >= 1, max_gap in [0,60], seed_dedup 0 or 1, refit 0 or 1, merge 0 or 1 (needs refit) with positive tolerances");
         return nullptr;
     }
@@ -737,6 +756,8 @@ int tpc_track_events(tpc_tracker* t, int32_t n, const tpc_event_in* in, tpc_even
         o.hit_idx = ohit + h;
     }
     t->have_result = true;
+    t->one_group = !host_in && n_groups == 1;
+    t->last_in = in;
     return TPC_OK;
 }
 
@@ -776,6 +797,7 @@ int tpc_wait_events(tpc_tracker* t, int32_t ticket, tpc_event_out* out) {
     t->counters = b->counters;
     if (t->profiling) for (int k = 0; k < TPC_N_STAGES; k++) t->stage_ms[k] = b->stage_ms[k];
     t->have_result = false;   // no intermediates for these batches
+    t->one_group = false;
     const int n = b->n_events;
     const int64_t T = b->counters.n_tracks, H = b->counters.n_track_hits;
     const int nI = t->c.p.merge ? kOutI : 4, nF = t->c.p.refit ? kOutF : 7;
@@ -796,9 +818,12 @@ int tpc_wait_events(tpc_tracker* t, int32_t ticket, tpc_event_out* out) {
         for (int k = 0; k < kOutF; k++) of[k] = a.h_o_f[k].p;
         ohit = a.h_o_hit.p;
     } else {
-        for (int k = 0; k < kOutI; k++) oi[k] = b->o_i[k].p;
-        for (int k = 0; k < kOutF; k++) of[k] = b->o_f[k].p;
-        ohit = b->v.o_hit_idx;
+        // the ticket takes the arrays that hold this run's outputs; the batch goes on with the ticket's previous ones
+        // (whose contents the caller no longer needs: they belong to the wait before last on this ticket)
+        for (int k = 0; k < kOutI; k++) { std::swap(a.d_o_i[k], b->o_i[k]); oi[k] = a.d_o_i[k].p; }
+        for (int k = 0; k < kOutF; k++) { std::swap(a.d_o_f[k], b->o_f[k]); of[k] = a.d_o_f[k].p; }
+        std::swap(a.d_o_hit, b->o_hit);
+        ohit = a.d_o_hit.p;
     }
     const int32_t* toff = b->h_ev_off.p;
     const int32_t* hoff = b->h_ev_off.p + (n + 1);
@@ -947,6 +972,127 @@ int tpc_debug_get(tpc_tracker* tr, int32_t what, int32_t event, void* buf, size_
         }
         default: set_err("unknown debug item"); return TPC_ERR_ARG;
     }
+}
+
+int tpc_debug_inject(tpc_tracker* tr, int32_t what, int32_t event, const void* buf, size_t bytes) {
+    if (!tr || !tr->one_group) { set_err("inject needs a last call with device inputs that ran as one group"); return TPC_ERR_ARG; }
+    const int64_t need = tpc_debug_size(tr, what, event);
+    if (need < 0) return (int)need;
+    int g0, g1, s0, s1;
+    const Batch* tc = nullptr;
+    int rc = dbg_ranges(tr, event, &tc, &g0, &g1, &s0, &s1);
+    if (rc != TPC_OK) return rc;
+    if (!buf || bytes != (size_t)need) { set_err("inject: the buffer must hold exactly %lld bytes", (long long)need); return TPC_ERR_ARG; }
+    Batch* t = const_cast<Batch*>(tc);
+    const int n = g1 - g0, s = s1 - s0, nr = tr->c.n_rows;
+    std::vector<int32_t> sorig(std::max(n, 1)), inv(std::max(n, 1), -1);
+    if (n) CK(cudaMemcpy(sorig.data(), t->v.sorig + g0, 4 * (size_t)n, cudaMemcpyDeviceToHost));
+    for (int k = 0; k < n; k++) {
+        if (sorig[k] < 0 || sorig[k] >= n) { set_err("inject: inconsistent work space"); return TPC_ERR_CUDA; }
+        inv[sorig[k]] = g0 + k;   // caller's index -> sorted (batch-global) index
+    }
+    const int32_t* ib = (const int32_t*)buf;
+    switch (what) {
+        case TPC_DBG_LINK_UP: case TPC_DBG_LINK_DN: case TPC_DBG_CLINK_UP: case TPC_DBG_CLINK_DN: {
+            int32_t* dst = what == TPC_DBG_LINK_UP ? t->v.link_up : what == TPC_DBG_LINK_DN ? t->v.link_dn
+                           : what == TPC_DBG_CLINK_UP ? t->v.clink_up : t->v.clink_dn;
+            std::vector<int32_t> l(std::max(n, 1));
+            for (int i = 0; i < n; i++) {
+                const int32_t h = ib[i];
+                if (h >= n) { set_err("inject: hit index %d outside the event", h); return TPC_ERR_ARG; }
+                l[inv[i] - g0] = h < 0 ? -1 : inv[h];
+            }
+            if (n) CK(cudaMemcpy(dst + g0, l.data(), 4 * (size_t)n, cudaMemcpyHostToDevice));
+            return TPC_OK;
+        }
+        case TPC_DBG_TL_ROWS: {
+            std::vector<int32_t> l(std::max(s, 1));
+            for (int k = 0; k < s; k++) {
+                const int first = ib[3 * k], last = ib[3 * k + 1], nh = ib[3 * k + 2];
+                if (nh < 0 || nh > nr || (nh > 0 && (first < 0 || last >= nr || first > last))) { set_err("inject: bad tracklet rows"); return TPC_ERR_ARG; }
+                l[k] = nh > 0 ? (first | (last << 8) | (nh << 16)) : 0;
+            }
+            if (s) CK(cudaMemcpy(t->v.tl_rows + s0, l.data(), 4 * (size_t)s, cudaMemcpyHostToDevice));
+            return TPC_OK;
+        }
+        case TPC_DBG_TL_PAR: {
+            std::vector<float> l(std::max(s, 1));
+            const float* fb = (const float*)buf;
+            for (int j = 0; j < 6; j++) {
+                for (int k = 0; k < s; k++) l[k] = fb[6 * k + j];
+                if (s) CK(cudaMemcpy(t->v.tl_par + (size_t)j * t->S_cap + s0, l.data(), 4 * (size_t)s, cudaMemcpyHostToDevice));
+            }
+            return TPC_OK;
+        }
+        case TPC_DBG_TL_TABLE: {
+            if (!s) return TPC_OK;
+            const int stride = t->v.tab_stride;
+            const int bpe = tr->c.n_sectors * nr;
+            std::vector<int32_t> sbin(s);
+            std::vector<uint16_t> tab((size_t)s * stride, kNoHit);
+            std::vector<BinDesc> desc(bpe);
+            CK(cudaMemcpy(sbin.data(), t->v.seed_bin + s0, 4 * (size_t)s, cudaMemcpyDeviceToHost));
+            CK(cudaMemcpy(desc.data(), t->v.desc + (size_t)tr->ev_local[event] * bpe, sizeof(BinDesc) * (size_t)bpe, cudaMemcpyDeviceToHost));
+            const int ev_bin0 = tr->ev_local[event] * bpe;
+            for (int k = 0; k < s; k++) {
+                const int tb = sbin[k] - sbin[k] % nr - ev_bin0;   // first bin of the tracklet's task, event-local
+                for (int r = 0; r < nr; r++) {
+                    const int32_t h = ib[(size_t)k * nr + r];
+                    if (h < 0) continue;
+                    if (h >= n) { set_err("inject: hit index %d outside the event", h); return TPC_ERR_ARG; }
+                    const int loc = inv[h] - desc[tb + r].base;
+                    if (loc < 0 || loc >= desc[tb + r].n) { set_err("inject: tracklet %d, row %d: the hit is not of that row", k, r); return TPC_ERR_ARG; }
+                    tab[(size_t)k * stride + r] = (uint16_t)loc;
+                }
+            }
+            CK(cudaMemcpy(t->v.tl_tab + (size_t)s0 * stride, tab.data(), 2 * tab.size(), cudaMemcpyHostToDevice));
+            return TPC_OK;
+        }
+        default: set_err("this intermediate cannot be injected"); return TPC_ERR_ARG;
+    }
+}
+
+int tpc_debug_resume(tpc_tracker* tr, int32_t from_stage, tpc_event_out* out) {
+    if (!tr || !out || !tr->one_group) { set_err("resume needs a last call with device inputs that ran as one group"); return TPC_ERR_ARG; }
+    if (from_stage < TPC_STAGE_CLEAN || from_stage > TPC_STAGE_SELECT) { set_err("resume: stage must be TPC_STAGE_CLEAN .. TPC_STAGE_SELECT"); return TPC_ERR_ARG; }
+    Batch* t = tr->slots[0];
+    const int n = t->n_events;
+    cudaStream_t st = t->stream;
+    CK(cudaStreamSynchronize(st));
+    memset(&t->counters, 0, sizeof(tpc_counters));
+    int rc = launch_all(tr, t, from_stage);
+    if (rc != TPC_OK) return rc;
+    CK(cudaMemcpyAsync(t->h_cnt.p, t->v.cnt, sizeof(unsigned long long) * CNT_N, cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(t->h_ev_off.p, t->v.ev_off, sizeof(int32_t) * 2 * (n + 1), cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(t->h_nseeds.p, t->v.seed_start + t->v.n_bins, sizeof(int32_t), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    const unsigned err = (unsigned)(t->h_cnt.p[CNT_ERR] & 0xffffffffu);
+    if (err) { set_err("resume: the kernels reported error bits 0x%x (pools are not grown here)", err); return TPC_ERR_CAPACITY; }
+    if (t->h_nseeds.p[0] > t->S_cap) { set_err("resume: more start hits than the tracklet pool holds"); return TPC_ERR_CAPACITY; }
+    t->counters.n_events = n; t->counters.n_clusters = t->N;
+    t->counters.n_links = (int64_t)t->h_cnt.p[CNT_LINKS]; t->counters.n_seeds = t->h_nseeds.p[0];
+    t->counters.n_row_visits = (int64_t)t->h_cnt.p[CNT_ROW_VISITS]; t->counters.n_tracklet_hits = (int64_t)t->h_cnt.p[CNT_TL_HITS];
+    t->counters.n_tracks = (int64_t)t->h_cnt.p[CNT_TRACKS]; t->counters.n_track_hits = (int64_t)t->h_cnt.p[CNT_TRACK_HITS];
+    t->counters.n_updates = (int64_t)t->h_cnt.p[CNT_UPDATES]; t->counters.n_refit_visits = (int64_t)t->h_cnt.p[CNT_REFIT_VISITS];
+    t->counters.n_tracklets = (int64_t)t->h_cnt.p[CNT_TRACKLETS];
+    tr->counters = t->counters;
+    const int32_t* toff = t->h_ev_off.p;
+    const int32_t* hoff = t->h_ev_off.p + (n + 1);
+    const bool rf = tr->c.p.refit != 0, mg = tr->c.p.merge != 0;
+    for (int e = 0; e < n; e++) {
+        tpc_event_out& o = out[e];
+        const int64_t a = toff[e], h = hoff[e];
+        o.n_tracks = toff[e + 1] - toff[e]; o.n_track_hits = hoff[e + 1] - hoff[e];
+        o.trk_sector = t->o_i[0].p + a; o.trk_first_hit = t->o_i[1].p + a; o.trk_n_hits = t->o_i[2].p + a; o.trk_ndf = t->o_i[3].p + a;
+        o.trk_x = t->o_f[0].p + a; o.trk_y = t->o_f[1].p + a; o.trk_z = t->o_f[2].p + a; o.trk_sinphi = t->o_f[3].p + a;
+        o.trk_tgl = t->o_f[4].p + a; o.trk_qpt = t->o_f[5].p + a; o.trk_chi2 = t->o_f[6].p + a;
+        o.hit_idx = t->v.o_hit_idx + h;
+        o.trk_out_x = rf ? t->o_f[7].p + a : nullptr; o.trk_out_y = rf ? t->o_f[8].p + a : nullptr; o.trk_out_z = rf ? t->o_f[9].p + a : nullptr;
+        o.trk_out_sinphi = rf ? t->o_f[10].p + a : nullptr; o.trk_out_tgl = rf ? t->o_f[11].p + a : nullptr;
+        o.trk_out_qpt = rf ? t->o_f[12].p + a : nullptr;
+        o.trk_next = mg ? t->o_i[4].p + a : nullptr; o.trk_prev = mg ? t->o_i[5].p + a : nullptr; o.trk_global = mg ? t->o_i[6].p + a : nullptr;
+    }
+    return TPC_OK;
 }
 
 }  // extern "C"

@@ -17,6 +17,7 @@ LIB_PATH = Path(os.environ.get("TPCTRACK_LIB") or Path(__file__).resolve().paren
 
 TPC_OK, TPC_ERR_ARG, TPC_ERR_GEOMETRY, TPC_ERR_CAPACITY, TPC_ERR_CUDA = 0, -1, -2, -3, -4
 N_STAGES = 6   # TPC_N_STAGES
+STAGE = {"clean": 3, "seeds": 4, "construct": 5, "select": 6}   # TPC_STAGE_*
 DBG = {"link_up": 0, "link_dn": 1, "clink_up": 2, "clink_dn": 3, "start_hit": 4, "tl_rows": 5, "tl_par": 6,
        "tl_table": 7, "sorted": 8}
 
@@ -34,7 +35,7 @@ class tpc_params(C.Structure):
                 ("win_min", C.c_float), ("win_max", C.c_float), ("max_gap", C.c_int32), ("edge_margin", C.c_float),
                 ("min_tracklet_hits", C.c_int32), ("min_track_hits", C.c_int32), ("refit", C.c_int32),
                 ("merge", C.c_int32), ("merge_dy", C.c_float), ("merge_dz", C.c_float), ("merge_ds", C.c_float),
-                ("merge_dt", C.c_float), ("merge_max_gap", C.c_int32), ("seed_dedup", C.c_int32)]
+                ("merge_dt", C.c_float), ("merge_max_gap", C.c_int32), ("seed_dedup", C.c_int32), ("checked", C.c_int32)]
 
     def as_dict(self):
         return {n: getattr(self, n) for n, _ in self._fields_}
@@ -99,6 +100,8 @@ def _load():
     lib.tpc_debug_size.restype = C.c_int64
     lib.tpc_debug_size.argtypes = [C.c_void_p, C.c_int32, C.c_int32]
     lib.tpc_debug_get.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_size_t]
+    lib.tpc_debug_inject.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_size_t]
+    lib.tpc_debug_resume.argtypes = [C.c_void_p, C.c_int32, C.POINTER(tpc_event_out)]
     return lib
 
 
@@ -107,7 +110,8 @@ lib = _load()
 EXPORTS = ("tpc_default_params", "tpc_tracker_create", "tpc_tracker_create_ex", "tpc_tracker_set_stream",
            "tpc_tracker_set_group_events",
            "tpc_track_event", "tpc_track_events", "tpc_submit_events", "tpc_wait_events", "tpc_tracker_destroy", "tpc_status_string", "tpc_last_error",
-           "tpc_get_counters", "tpc_tracker_set_profiling", "tpc_get_stage_ms", "tpc_debug_size", "tpc_debug_get")
+           "tpc_get_counters", "tpc_tracker_set_profiling", "tpc_get_stage_ms", "tpc_debug_size", "tpc_debug_get",
+           "tpc_debug_inject", "tpc_debug_resume")
 
 
 def tpc_status_string(status: int) -> str:
@@ -174,8 +178,10 @@ class Tracker:
             so = np.ascontiguousarray(ev["sector_offset"], dtype=np.int32)
             keep.append(so)
             spaces = set()
-            ptrs = {}
-            for k in ("y", "z", "row"):
+            ptrs = {"x": None}
+            for k in ("x", "y", "z", "row"):
+                if k == "x" and ev.get("x") is None:     # optional: only the checked mode reads it
+                    continue
                 a = ev[k]
                 if isinstance(a, np.ndarray):
                     want = np.int32 if k == "row" else np.float32
@@ -190,12 +196,12 @@ class Tracker:
                 spaces.add(sp)
             assert len(spaces) == 1, "y, z, row must live in one memory space"
             ncl = int(so[-1])
-            ins[i] = tpc_event_in(ncl, so.ctypes.data, None, ptrs["y"], ptrs["z"], ptrs["row"], spaces.pop())
+            ins[i] = tpc_event_in(ncl, so.ctypes.data, ptrs["x"], ptrs["y"], ptrs["z"], ptrs["row"], spaces.pop())
         return ins, keep
 
     def tpc_track_events(self, events):
-        """events: list of dicts with sector_offset (host int32), y, z (float32), row (int32): all numpy (host)
-        or all torch CUDA tensors (device).  Returns a list of raw ``tpc_event_out`` structs (pointers are
+        """events: list of dicts with sector_offset (host int32), y, z (float32), row (int32), optionally x: all
+        numpy (host) or all torch CUDA tensors (device).  Returns a list of raw ``tpc_event_out`` structs (pointers are
         library-owned; host or device like the input) -- see ``to_numpy``."""
         n = len(events)
         ins, keep = self._marshal(events)
@@ -258,6 +264,17 @@ class Tracker:
         elif what == "tl_table":
             a = a.reshape(-1, self.n_rows)
         return a
+
+    def tpc_debug_inject(self, what: str, a: np.ndarray, event: int = 0):
+        """Overwrite an intermediate of the last call (layout of ``tpc_debug_get``)."""
+        a = np.ascontiguousarray(a, dtype=np.float32 if what == "tl_par" else np.int32)
+        _check(lib.tpc_debug_inject(self._h, DBG[what], event, a.ctypes.data, a.nbytes))
+
+    def tpc_debug_resume(self, from_stage: str, n_events: int = 1):
+        """Run the path again from ``from_stage`` ("clean", "seeds", "construct", "select") on the work space."""
+        outs = (tpc_event_out * n_events)()
+        _check(lib.tpc_debug_resume(self._h, STAGE[from_stage], outs))
+        return list(outs)
 
     @staticmethod
     def as_tensor(ptr, n, dt):

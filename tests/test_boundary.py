@@ -34,7 +34,7 @@ def test_library_exports_every_declared_symbol(tr):
 
 
 def test_struct_layouts_match_header(tr):
-    assert C.sizeof(tr.tpc_params) == 26 * 4
+    assert C.sizeof(tr.tpc_params) == 27 * 4
     assert C.sizeof(tr.tpc_event_in) == 8 + 8 * 5 + 8          # int32 + pad, 5 pointers, int32 + pad
     assert C.sizeof(tr.tpc_event_out) == 8 + 8 * 21
     assert C.sizeof(tr.tpc_counters) == 13 * 8
