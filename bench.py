@@ -33,12 +33,33 @@ METRIC = "central_pbpb_events_per_s"
 UNIT = "events/s"
 
 
+HBM_NOMINAL_GBS = 8000.0   # BASELINE.json:5 "nominal ~8 TB/s"
+
+
 def measured_peaks():
     p = ROOT / "MEASURED_PEAKS.json"
     if p.exists():
         d = json.loads(p.read_text())
         return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
     return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+def run_config(args, n_events):
+    """What identifies a measured configuration (profiles/traffic.json is valid for exactly one)."""
+    return {"workload": args.workload, "events": n_events, "link_step": args.link_step, "refit": bool(args.refit),
+            "merge": bool(args.merge), "seed_dedup": not args.no_seed_dedup}
+
+
+def committed_traffic(cfg):
+    """DRAM bytes per step of each stage from the committed ncu --set full capture -- only when that capture was
+    taken on this very configuration; tagged with the commit it was taken at."""
+    tf = ROOT / "profiles" / "traffic.json"
+    if not tf.exists():
+        return None
+    d = json.loads(tf.read_text())
+    if d.get("config") != cfg:
+        return None
+    return d
 
 
 class ClockSampler(threading.Thread):
@@ -93,13 +114,13 @@ def make_events(workload, n_events):
 
 def stage_bytes(c):
     """Algorithmic bytes per stage from the run's own counters."""
-    N, S, V, A, T, H = (c[k] for k in ("n_clusters", "n_seeds", "n_row_visits", "n_tracklet_hits", "n_tracks",
-                                       "n_track_hits"))
+    N, S, V, A, T, H, B = (c[k] for k in ("n_clusters", "n_seeds", "n_row_visits", "n_tracklet_hits", "n_tracks",
+                                          "n_track_hits", "n_tracklets"))
     return {
         "K1_sort_grid": 26 * N,
         "K2_neighbours": 18 * N,
-        "K3K4_clean_seeds": 24 * N + 4 * S,
-        "K5_construct": 12 * V + 4 * A + 40 * S,
+        "K3K4_clean_seeds": 24 * N + 36 * S,
+        "K5_construct": 12 * V + 4 * A + 36 * S + 124 * B,
         "K6_select": 16 * A + 4 * H + 44 * T,
         "K7_refit": (12 * H + 44 * T) if c.get("n_refit_visits", 0) else 0,
     }
@@ -110,6 +131,40 @@ def k5_flops(c):
     writes them (no fused multiply-add): 164 per row visit (transport 160, gate weights 4), 107 per accepted
     measurement (gate 7, two scalar updates 100)."""
     return 164 * c["n_row_visits"] + 107 * c["n_updates"]
+
+
+def cpu_baselines(evs, rx, gen):
+    """The oracle as it stands, timed on the host cores on bounded samples of the workload: all
+    hardware threads in strict-float32 mode (the reference of the parity tests) and in double, and one thread."""
+    import oracle
+    geom = oracle.Geometry(evs[0].n_sectors, rx, gen.TAN_HALF_ANGLE, evs[0].sigma, evs[0].sigma, evs[0].bz)
+    cores = oracle.max_threads()
+    out = {}
+    nb = min(2, len(evs))
+    t0 = time.perf_counter()
+    for ev in evs[:nb]:
+        oracle.track_event(geom, ev.sector_offset, ev.y, ev.z, ev.row, precision="float")
+    dt = time.perf_counter() - t0
+    out.update({"value": nb / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+                "sample": "first %d events of the batch (%d clusters), strict-float32 mode, OpenMP over sectors"
+                          % (nb, sum(ev.n_clusters for ev in evs[:nb]))})
+    ev = evs[0]
+    t0 = time.perf_counter()
+    oracle.track_event(geom, ev.sector_offset, ev.y, ev.z, ev.row, precision="double")
+    dt = time.perf_counter() - t0
+    out["double"] = {"value": 1.0 / dt, "unit": UNIT, "cores": cores,
+                     "sample": "first event of the batch (%d clusters), double mode" % ev.n_clusters}
+    # one thread: the first sectors of the first event (about a ninth of it), scaled to whole events
+    ns1 = max(1, min(4, ev.n_sectors))
+    g1 = oracle.Geometry(ns1, rx, gen.TAN_HALF_ANGLE, ev.sigma, ev.sigma, ev.bz)
+    n1 = int(ev.sector_offset[ns1])
+    t0 = time.perf_counter()
+    oracle.track_event(g1, ev.sector_offset[:ns1 + 1], ev.y[:n1], ev.z[:n1], ev.row[:n1], precision="float", n_threads=1)
+    dt = time.perf_counter() - t0
+    out["one_thread"] = {"value": (n1 / max(ev.n_clusters, 1)) / dt, "unit": UNIT, "cores": 1,
+                         "sample": "sectors 0-%d of the first event (%d of its %d clusters) on one thread, strict-float32 "
+                                   "mode, scaled to whole events by the cluster share" % (ns1 - 1, n1, ev.n_clusters)}
+    return out
 
 
 def fp32_peak_tflops(sm_count, sm_max_mhz):
@@ -181,7 +236,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--events", type=int, default=16, help="events per batch (one step)")
-    ap.add_argument("--workload", default="central", choices=["central", "semicentral", "pp", "single_sector"])
+    ap.add_argument("--workload", default="central", choices=["central", "semicentral", "pp", "single_sector", "dense"],
+                    help="dense = 2.5 x the central multiplicity (SURVEY.md 8(f).4; not a BASELINE.json config)")
+    ap.add_argument("--no-seed-dedup", action="store_true", help="fit every start hit (round-1 behaviour)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--link-step", type=int, default=1, choices=[1, 2], help="neighbour rows r +- step (SURVEY.md 8(f).4)")
@@ -212,11 +269,12 @@ def main():
     rx = gen.row_x().astype(np.float32)
     params = None
     args.refit = args.refit or args.merge
-    if args.refit or args.link_step != 1:
+    if args.refit or args.link_step != 1 or args.no_seed_dedup:
         params = tracker.tpc_default_params()
         params.refit = int(args.refit)
         params.merge = int(args.merge)
         params.link_step = args.link_step
+        params.seed_dedup = int(not args.no_seed_dedup)
     trk = tracker.Tracker(evs[0].n_sectors, rx, gen.TAN_HALF_ANGLE, evs[0].sigma, evs[0].sigma, evs[0].bz,
                           params=params, max_events=len(evs), max_clusters=n_total)
     stream = torch.cuda.Stream()
@@ -314,40 +372,40 @@ def main():
         for k, name in enumerate(names):
             gbs = sb[name] / (stage_ms[k] * 1e-3) / 1e9 if stage_ms[k] > 0 else None
             stages[name] = {"ms": round(float(stage_ms[k]), 4), "algorithmic_bytes": int(sb[name]),
-                            "GBps": gbs, "frac_of_hbm_peak": (gbs / peak if gbs else None)}
+                            "GBps": gbs, "frac_of_hbm_peak": (gbs / peak if gbs else None),
+                            "frac_of_nominal_8TBps": (gbs / HBM_NOMINAL_GBS if gbs else None)}
         dom = max(names, key=lambda n: stages[n]["ms"])
-        traffic = None
-        tf = ROOT / "profiles" / "traffic.json"   # DRAM bytes per step from the committed ncu --set full capture
-        if tf.exists():
-            traffic = json.loads(tf.read_text()).get(dom)
+        # DRAM bytes per step from the committed ncu --set full capture: only for the configuration it was taken on
+        cap = committed_traffic(run_config(args, len(evs)))
+        traffic = cap.get(dom) if cap else None
         if dom == "K5_construct":
             # K5 = k_sweep<up> + k_sweep<down> (two launches of one kernel template, timed together with CUDA events
             # on the launching stream inside the timed region).  Arithmetic intensity ~20 flop/B: bound by FP32 issue.
             sm_count = torch.cuda.get_device_properties(local_rank).multi_processor_count
-            alu_peak = fp32_peak_tflops(sm_count, clocks.get("sm_max_mhz"))
+            derived = fp32_peak_tflops(sm_count, clocks.get("sm_max_mhz"))
+            fused, unfused = tracker.tpc_measure_fp32_peak()          # measured here, on this device, after the run
             tfl = k5_flops(counters) / (stage_ms[names.index(dom)] * 1e-3) / 1e12
-            roofline = {"bound": "alu", "kernel": "K5 k_sweep<up> + k_sweep<down> (2 launches per step)",
-                        "achieved": tfl, "peak": alu_peak, "unit": "TFLOP/s", "frac": tfl / alu_peak,
-                        "traffic": traffic,
-                        "peak_source": "derived: %d SMs x 128 FP32 lanes x 2 (FMA) x %.0f MHz; the method's "
-                                       "arithmetic is un-fused, so 0.5 is its ceiling" % (sm_count, clocks.get("sm_max_mhz") or 1965.0),
+            roofline = {"bound": "alu", "kernel": "K5 k_construct (1 launch per step: up and down sweep of every sector task)",
+                        "achieved": tfl, "peak": fused, "unit": "TFLOP/s", "frac": tfl / fused,
+                        "traffic": traffic, "traffic_commit": cap.get("commit") if cap else None,
+                        "peak_source": "measured by tpc_measure_fp32_peak on this device: independent FFMA chains, "
+                                       "multiply and add counted separately",
+                        "peak_unfused_measured": unfused, "frac_of_unfused": tfl / unfused,
+                        "peak_derived": derived,
+                        "note": "the method's arithmetic is defined without contraction (strict float32 parity), so the "
+                                "un-fused multiply + add rate is its ceiling; derived = %d SMs x 128 lanes x 2 x %.0f MHz"
+                                % (sm_count, clocks.get("sm_max_mhz") or 1965.0),
                         "hbm": {"achieved": stages[dom]["GBps"], "peak": peak, "unit": "GB/s",
-                                "frac": stages[dom]["frac_of_hbm_peak"], "peak_source": peak_src}}
+                                "frac": stages[dom]["frac_of_hbm_peak"], "peak_source": peak_src,
+                                "frac_of_nominal_8TBps": stages[dom]["frac_of_nominal_8TBps"]}}
         else:
             roofline = {"bound": "hbm", "kernel": dom, "achieved": stages[dom]["GBps"], "peak": peak, "unit": "GB/s",
-                        "frac": stages[dom]["frac_of_hbm_peak"], "traffic": traffic, "peak_source": peak_src}
+                        "frac": stages[dom]["frac_of_hbm_peak"], "traffic": traffic,
+                        "traffic_commit": cap.get("commit") if cap else None, "peak_source": peak_src,
+                        "frac_of_nominal_8TBps": stages[dom]["frac_of_nominal_8TBps"]}
         cpu = None
         if not args.no_cpu_baseline:
-            import oracle
-            geom = oracle.Geometry(evs[0].n_sectors, rx, gen.TAN_HALF_ANGLE, evs[0].sigma, evs[0].sigma, evs[0].bz)
-            nb = min(2, len(evs))
-            t0 = time.perf_counter()
-            for ev in evs[:nb]:
-                oracle.track_event(geom, ev.sector_offset, ev.y, ev.z, ev.row, precision="float")
-            dt = time.perf_counter() - t0
-            cpu = {"value": nb / dt, "unit": UNIT, "cores": oracle.max_threads(), "kind": "oracle",
-                   "sample": "first %d events of the batch (%d clusters), strict-float32 mode, OpenMP over sectors"
-                             % (nb, sum(ev.n_clusters for ev in evs[:nb]))}
+            cpu = cpu_baselines(evs, rx, gen)
         value = aggregate_value(len(evs), args.steps, ms, world)
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -355,6 +413,8 @@ def main():
             "dtype": "f32", "data": "synthetic",
             "config": {"workload": ("%d x central Pb-Pb-like events per step (BASELINE.json config 5 = 16 x config 4)" % len(evs))
                                    if args.workload == "central" else "%d x %s event(s) per step" % (len(evs), args.workload),
+                       "link_step": args.link_step, "refit": bool(args.refit), "merge": bool(args.merge),
+                       "seed_dedup": not args.no_seed_dedup,
                        "events_per_step": len(evs), "clusters_per_step": int(n_total),
                        "tracks_per_step": int(n_tracks), "parallelism": "replicas only" if world > 1 else "1 GPU",
                        "l2": "inputs (%.0f MB per step) larger than L2 (126 MB); no flush" % (12 * n_total / 1e6)},

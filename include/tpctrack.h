@@ -211,6 +211,12 @@ int tpc_get_counters(const tpc_tracker* t, tpc_counters* c);
 int tpc_tracker_set_profiling(tpc_tracker* t, int32_t on);
 int tpc_get_stage_ms(const tpc_tracker* t, float* ms /* [TPC_N_STAGES] */);
 
+/* Measured FP32 arithmetic peaks of the current device, in TFLOP/s (multiply and add counted separately): independent
+ * chains of fused multiply-adds, and of un-fused multiply + add pairs -- the ceiling of arithmetic that is defined
+ * without contraction, as this tracker's is.  The denominators of the constructor's
+ * roofline in bench.py; takes a few milliseconds; not part of the hot path. */
+int tpc_measure_fp32_peak(float* fused_tflops, float* unfused_tflops);
+
 /* ---- intermediates of the last call, for stage-by-stage parity tests (not part of the hot path) ----
  * All hit indices are the caller's indices within event `event`; -1 = none.  buf is a HOST buffer of `bytes`
  * bytes; the call fails with TPC_ERR_ARG if it is too small.  Sizes: tpc_debug_size().  After a host-input batch

@@ -25,7 +25,8 @@ constexpr unsigned kErrBadRow = 1u, kErrRowCapacity = 2u, kErrSeedCapacity = 4u,
 constexpr unsigned kErrFatal = kErrBadRow | kErrRowCapacity | kErrBadInput;   // the later kernels do nothing after these
 
 // the stages after K1 start with this: a batch that K1 has rejected is not worked on (its arrays may be incomplete)
-#define TPC_RETURN_IF_REJECTED(v) do { if (*(volatile unsigned long long*)&(v).cnt[CNT_ERR] & kErrFatal) return; } while (0)
+// (a cached read: K1's bits were set by earlier kernels; a volatile one makes every warp of the grid queue at one L2 line)
+#define TPC_RETURN_IF_REJECTED(v) do { if (__ldg(&(v).cnt[CNT_ERR]) & kErrFatal) return; } while (0)
 
 // device counters (unsigned long long each)
 constexpr int kNCursors = 4;           // work cursors: [0] K5 sector tasks, [2] refit

@@ -15,6 +15,7 @@
 #include "sel_kernels.cuh"
 #include "kf_refit.cuh"
 #include "merge_kernels.cuh"
+#include "peak_kernels.cuh"
 
 namespace {
 
@@ -82,9 +83,9 @@ struct Batch {
     Buf<float> in_x, in_y, in_z, tl_par, o_f[kOutF];
     Buf<float2> thit, shit;
     Buf<int32_t> in_row, sec_off, bin_count, bin_start, tidx, sorig, link_up, link_dn, clink_up, clink_dn, seed_count,
-        seed_start, seeds, seed_bin, tl_rows, tl_nown, tl_keep, trk_scan, hit_scan, ev_off_d, scratch,
+        seed_start, seeds, seed_bin, tl_rows, tl_nown, tl_keep, trk_scan, hit_scan, ev_off_d,
         o_i[kOutI], o_hit, trk_rows, trk_task, mg_list;
-    Buf<unsigned long long> mg_next, mg_prev;
+    Buf<unsigned long long> mg_next, mg_prev, scratch;
     Buf<uint16_t> slot, cells, tl_tab;
     Buf<float2> o_hit_yz;
     Buf<uint8_t> o_hit_row;
@@ -219,7 +220,7 @@ int reserve_batch(const tpc_tracker* tr, Batch* t, int n_events, int64_t N, int6
     RS(seed_rec, S_cap); RS(tl_up, S_cap); RS(dn_rec, S_cap); RS(kf_park, S_cap); RS(dn_count, nb + 1); RS(dn_start, nb + 1); RS(dn_fill, nb + 1);
     RS(tl_nown, S_cap + 1); RS(tl_keep, S_cap + 1); RS(tl_cnt, (size_t)t->sel_C * S_cap); RS(trk_scan, S_cap + 2); RS(hit_scan, S_cap + 2);
     RS(ev_off_d, 2 * ((size_t)n_events + 1)); RS(h_ev_off, 2 * ((size_t)n_events + 1));
-    RS(scratch, (size_t)std::max<int64_t>(nb, S_cap) / kScanTile + 8);
+    RS(scratch, (size_t)std::max<int64_t>(nb, S_cap) / kScanTile + 8);   // scans: tile counter + status words
     RS(cnt, CNT_N); RS(h_cnt, CNT_N); RS(kf_cursor, kNCursors); RS(h_nseeds, 1);
     for (int k = 0; k < kOutI; k++) RS(o_i[k], S_cap);
     for (int k = 0; k < kOutF; k++) RS(o_f[k], S_cap);
@@ -972,6 +973,34 @@ int tpc_debug_get(tpc_tracker* tr, int32_t what, int32_t event, void* buf, size_
         }
         default: set_err("unknown debug item"); return TPC_ERR_ARG;
     }
+}
+
+int tpc_measure_fp32_peak(float* fused_tflops, float* unfused_tflops) {
+    if (!fused_tflops || !unfused_tflops) { set_err("null result pointers"); return TPC_ERR_ARG; }
+    int dev = 0, sms = 0;
+    CK(cudaGetDevice(&dev));
+    CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+    const int blocks = sms * 8;                      // 2048 threads per SM: every scheduler has 16 warps to pick from
+    float* d = nullptr;
+    CK(cudaMalloc((void**)&d, 4));
+    cudaEvent_t e0, e1;
+    CK(cudaEventCreate(&e0)); CK(cudaEventCreate(&e1));
+    float best[2] = {0.f, 0.f};
+    for (int fused = 0; fused < 2; fused++)
+        for (int rep = 0; rep < 6; rep++) {          // first launches warm up; the best of the rest counts
+            CK(cudaEventRecord(e0, 0));
+            if (fused) k_fp32_peak<true><<<blocks, kPeakThreads>>>(d, 1.0000001f, 1.0e-7f);
+            else k_fp32_peak<false><<<blocks, kPeakThreads>>>(d, 1.0000001f, 1.0e-7f);
+            CK(cudaEventRecord(e1, 0));
+            CK(cudaEventSynchronize(e1));
+            float ms = 0.f;
+            CK(cudaEventElapsedTime(&ms, e0, e1));
+            if (rep >= 2 && ms > 0.f) best[fused] = std::max(best[fused], (float)(fp32_peak_flops_per_launch(blocks) / (ms * 1e-3) / 1e12));
+        }
+    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d);
+    CK(cudaGetLastError());
+    *fused_tflops = best[1]; *unfused_tflops = best[0];
+    return TPC_OK;
 }
 
 int tpc_debug_inject(tpc_tracker* tr, int32_t what, int32_t event, const void* buf, size_t bytes) {

@@ -81,6 +81,9 @@ RECIPES = {
                       loopers=True, config_id=4),
     "central_batch16": Recipe("central_batch16", n_primaries=8000, frac_secondaries=0.20, sigma=0.08,
                               noise_frac=0.10, loopers=True, n_events=16, config_id=5),
+    # not a BASELINE.json config: SURVEY.md 8(f).4 "higher-occupancy events (2-3x cluster density)": 2.5 x central
+    "dense": Recipe("dense", n_primaries=20000, frac_secondaries=0.20, sigma=0.08, noise_frac=0.10, loopers=True,
+                    config_id=6),
 }
 
 TRK_COLS = ("pt", "charge", "eta", "phi", "vx", "vy", "vz", "primary")

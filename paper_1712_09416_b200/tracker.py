@@ -102,6 +102,7 @@ def _load():
     lib.tpc_debug_get.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_size_t]
     lib.tpc_debug_inject.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_size_t]
     lib.tpc_debug_resume.argtypes = [C.c_void_p, C.c_int32, C.POINTER(tpc_event_out)]
+    lib.tpc_measure_fp32_peak.argtypes = [C.POINTER(C.c_float), C.POINTER(C.c_float)]
     return lib
 
 
@@ -111,7 +112,7 @@ EXPORTS = ("tpc_default_params", "tpc_tracker_create", "tpc_tracker_create_ex", 
            "tpc_tracker_set_group_events",
            "tpc_track_event", "tpc_track_events", "tpc_submit_events", "tpc_wait_events", "tpc_tracker_destroy", "tpc_status_string", "tpc_last_error",
            "tpc_get_counters", "tpc_tracker_set_profiling", "tpc_get_stage_ms", "tpc_debug_size", "tpc_debug_get",
-           "tpc_debug_inject", "tpc_debug_resume")
+           "tpc_debug_inject", "tpc_debug_resume", "tpc_measure_fp32_peak")
 
 
 def tpc_status_string(status: int) -> str:
@@ -120,6 +121,13 @@ def tpc_status_string(status: int) -> str:
 
 def tpc_last_error() -> str:
     return lib.tpc_last_error().decode()
+
+
+def tpc_measure_fp32_peak() -> tuple:
+    """(fused multiply-add, un-fused multiply + add) FP32 TFLOP/s measured on the current device."""
+    a, b = C.c_float(0), C.c_float(0)
+    _check(lib.tpc_measure_fp32_peak(C.byref(a), C.byref(b)))
+    return float(a.value), float(b.value)
 
 
 def tpc_default_params() -> tpc_params:

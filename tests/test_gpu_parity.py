@@ -478,3 +478,31 @@ def test_submit_wait_gives_what_the_sync_call_gives(trk_mod, gen_mod, oracle_mod
         lib_out = (trk_mod.tpc_event_out * 1)()
         trk_mod._check(trk_mod.lib.tpc_wait_events(trk._h, 0, lib_out))     # nothing in flight
     trk.close(); ref_trk.close()
+
+
+def test_parity_central_link_step_2_full_size(trk_mod, gen_mod, oracle_mod):
+    """BASELINE.json config 4 with Delta = 2, every stage and every output compared."""
+    ev = gen_mod.generate("central")
+    po = oracle_mod.default_params(); po.link_step = 2
+    ref = oracle_mod.track_event(make_geometry(oracle_mod, gen_mod, ev), ev.sector_offset, ev.y, ev.z, ev.row,
+                                 params=po, precision="float")
+    trk = make_tracker(trk_mod, gen_mod, ev, params=copy_params(po, trk_mod))
+    out = trk.tpc_track_event(ev_dict(ev, True))
+    flips, res = compare_event(trk, out, ev, ref)
+    assert flips == 0 and res["n_tracks"] > 20000
+    trk.close()
+
+
+def test_parity_dense_workload(trk_mod, gen_mod, oracle_mod):
+    """The bench's second workload (2.5 x central multiplicity, 4.6 M clusters, pad rows of up to ~1000 hits: beyond
+    the 640 hits K2 / K5 stage in shared memory, read in place), every stage and every output compared."""
+    ev = gen_mod.generate("dense")
+    ref = oracle_mod.track_event(make_geometry(oracle_mod, gen_mod, ev), ev.sector_offset, ev.y, ev.z, ev.row,
+                                 precision="float")
+    trk = make_tracker(trk_mod, gen_mod, ev)
+    out = trk.tpc_track_event(ev_dict(ev, True))
+    flips, res = compare_event(trk, out, ev, ref)
+    assert flips == 0 and res["n_tracks"] > 50000
+    c = trk.tpc_get_counters()
+    assert c["n_tracklets"] == int((ref.tl_n_hits > 0).sum())
+    trk.close()
