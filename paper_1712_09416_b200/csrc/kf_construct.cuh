@@ -4,7 +4,7 @@
 // A CTA takes a sector task and sweeps its pad rows twice: upwards for the up passes, then downwards for the down
 // passes.  A producer warp streams the rows -- hits and grid cell table of row r, one
 // cp.async.bulk each, completion on an mbarrier -- through a ring of kCtRing shared-memory slots.  The Kalman
-// state of every tracklet under way (31 words) lives in a shared-memory slot; at each row the 13 consumer warps
+// state of every tracklet under way (32 words) lives in a shared-memory slot; at each row the 9 consumer warps
 // take the occupied slots 32 at a time, load the states, advance them by that row (transport, linked / recorded hit
 // or window search in the staged row, update) and store them back.  All tracklets of the task are therefore at the
 // same row at the same time, which is what the seed de-duplication needs (R23): an up pass marks every
@@ -20,8 +20,12 @@
 
 namespace tpc {
 
+// 9 consumer warps: 2 CTAs x 320 threads per SM leave 96 registers per thread and the row step does not spill.
+// Measured on config 5 (K5 alone): 13 warps (72 registers, 180 B of spills per thread, every spill an L2 round trip
+// because the shared-memory carve-out leaves ~10 KB of L1) 5.82 ms; 11 warps (80 registers, 52 B) 5.62 ms; 10 warps
+// 6.10 ms; 9 warps (no spill) 4.61 ms; 8 warps 4.70 ms.
 #ifndef TPC_CT_WARPS
-#define TPC_CT_WARPS 13
+#define TPC_CT_WARPS 9
 #endif
 #ifndef TPC_CT_RING
 #define TPC_CT_RING 3
