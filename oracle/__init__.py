@@ -57,9 +57,10 @@ class _Geometry(C.Structure):
 _FIELDS = ["link_up", "link_dn", "clink_up", "clink_dn", "nf_margin", "seed_offset", "start_hit",
            "tl_first_row", "tl_last_row", "tl_n_hits", "tl_par", "tl_chi2", "tl_margin", "tl_table",
            "trk_sector", "trk_first_hit", "trk_n_hits", "trk_ndf", "trk_seed", "trk_first_row",
-           "trk_x", "trk_y", "trk_z", "trk_sinphi", "trk_tgl", "trk_qpt", "trk_chi2", "trk_margin", "hit_idx", "tl_cov", "trk_row_out", "trk_out", "trk_next", "trk_prev", "trk_global", "trk_merge_margin"]
+           "trk_x", "trk_y", "trk_z", "trk_sinphi", "trk_tgl", "trk_qpt", "trk_chi2", "trk_margin", "hit_idx", "tl_cov", "trk_row_out", "trk_out", "trk_next", "trk_prev", "trk_global", "trk_merge_margin",
+           "trk_g", "trk_g_ndf", "trk_g_n_hits", "trk_g_sector"]
 _F64 = {"nf_margin", "tl_par", "tl_cov", "tl_chi2", "tl_margin", "trk_x", "trk_y", "trk_z", "trk_sinphi", "trk_tgl",
-        "trk_qpt", "trk_chi2", "trk_margin", "trk_out", "trk_merge_margin"}
+        "trk_qpt", "trk_chi2", "trk_margin", "trk_out", "trk_merge_margin", "trk_g"}
 
 _lib = None
 
@@ -82,6 +83,8 @@ def lib():
         l.oracle_update.argtypes = [C.POINTER(_Geometry), C.POINTER(Params), C.c_double, C.c_double, C.c_void_p,
                                     C.c_void_p, C.c_void_p]
         l.oracle_max_threads.restype = C.c_int32
+        l.oracle_rotate.restype = C.c_int32
+        l.oracle_rotate.argtypes = [C.POINTER(_Geometry), C.POINTER(Params), C.c_void_p, C.c_double, C.c_double, C.c_void_p, C.c_void_p]
         l.oracle_merge_tracks.restype = C.c_int32
         l.oracle_merge_tracks.argtypes = [C.POINTER(_Geometry), C.POINTER(Params), C.c_int32, C.c_int32] + [C.c_void_p] * 9
         _lib = l
@@ -143,7 +146,7 @@ def track_event(geom: Geometry, sector_offset, y, z, row, params: Params | None 
         shapes = {"link_up": (N,), "link_dn": (N,), "clink_up": (N,), "clink_dn": (N,), "nf_margin": (N,),
                   "seed_offset": (geom.n_sectors + 1,), "start_hit": (S,), "tl_first_row": (S,), "tl_last_row": (S,),
                   "tl_n_hits": (S,), "tl_par": (S, 5), "tl_cov": (S, 5), "tl_chi2": (S,), "tl_margin": (S,), "tl_table": (S, NR),
-                  "hit_idx": (H,), "trk_out": (T, 6)}
+                  "hit_idx": (H,), "trk_out": (T, 6), "trk_g": (T, 7)}
         out = Result(n_clusters=N, n_seeds=S, n_tracks=T, n_track_hits=H)
         for i, name in enumerate(_FIELDS):
             shape = shapes.get(name, (T,))
@@ -198,3 +201,16 @@ def merge_tracks(geom: Geometry, sector, first_row, par, row_out, out, params: P
     if rc != 0:
         raise ValueError("oracle_merge_tracks: bad arguments")
     return nx, pv, gl, mg
+
+
+def rotate(geom: Geometry, x: float, angle: float, state, cov, params: Params | None = None):
+    """One O10 rotation step in double: the fit given at ``x`` in one sector frame, expressed in a frame whose axis is
+    turned by ``angle`` (rad; negative = the next sector in azimuth).  Returns ok, x', state, cov."""
+    p = params if params is not None else default_params()
+    g, _keep = geom._c()
+    st = np.array(state, np.float64).copy()
+    cv = np.array(cov, np.float64).reshape(5, 5).copy()
+    xx = np.array([x], np.float64)
+    rc = lib().oracle_rotate(C.byref(g), C.byref(p), xx.ctypes.data, float(np.sin(angle)), float(np.cos(angle)),
+                             st.ctypes.data, cv.ctypes.data)
+    return rc == 0, float(xx[0]), st, cv

@@ -123,6 +123,9 @@ struct Result {
     std::vector<int32_t> trk_row_out, trk_next, trk_prev, trk_global; /* global: first segment of the chain */
     std::vector<double> trk_out; /* [T][6] x y z sin phi tg lambda q/pT */
     std::vector<double> trk_merge_margin; /* [T] smallest relative margin of the O9 decisions a segment took part in */
+    /* O10: fit of the global track (chain of linked segments), stored at the chain's first segment; zero elsewhere */
+    std::vector<double> trk_g;            /* [T][7] x y z sin phi tg lambda q/pT chi2, in the frame of trk_g_sector */
+    std::vector<int32_t> trk_g_ndf, trk_g_n_hits, trk_g_sector;
 };
 
 template <class R> struct Sector {
@@ -263,6 +266,124 @@ template <class R> struct Sector {
                 for (int l = 0; l < 5; l++) acc = acc + M[i][l] * F[j][l];
                 f.C[i][j] = acc; f.C[j][i] = acc;
             }
+        return true;
+    }
+
+    /* ---- O10: the fit, given at x in the frame of one sector, expressed in the frame of a neighbouring sector, whose
+       axis is turned by the angle with sine sn and cosine cd (sn < 0: the next sector in azimuth).  The reference
+       point stays the same point of space; its new abscissa x' is returned in x.  Parameters:
+         x' = x cd - y sn, y' = x sn + y cd, s' = s cd + sqrt(1 - s^2) sn; z, t, q unchanged.
+       Covariance C' = J C J^T with the first-order change of the parameters AT THE PLANE x' = const (a shift dy of
+       the point leaves that plane by -sn dy, and is brought back along the track over dl = sn dy / c'):
+         dy'/dy = cd + sn s'/c',  dz'/dy = t sn / c',  ds'/dy = kappa sn,  ds'/ds = cd - (s/c) sn,  identity elsewhere.
+       false (fit untouched) if |sin phi| exceeds s_max before or after. */
+    bool rotate(Fit<R>& f, R& x, R sn, R cd, Margin& mg) const {
+        const R s = f.s;
+        if (gt(std::fabs(s), R(P.sin_max), mg)) return false;
+        const R c = std::sqrt(R(1) - s * s);
+        const R s1 = s * cd + c * sn;
+        if (gt(std::fabs(s1), R(P.sin_max), mg)) return false;
+        const R c1 = std::sqrt(R(1) - s1 * s1);
+        const R ic1 = R(1) / c1;
+        const R kap = kB * f.q;
+        const R Jyy = cd + sn * (s1 * ic1);
+        const R Jzy = (f.t * sn) * ic1;
+        const R Jsy = kap * sn;
+        const R Jss = cd - (s * (R(1) / c)) * sn;
+        const R x1 = x * cd - f.y * sn, y1 = x * sn + f.y * cd;
+        x = x1; f.y = y1; f.s = s1;
+        R J[5][5];
+        for (int i = 0; i < 5; i++) for (int j = 0; j < 5; j++) J[i][j] = (i == j) ? R(1) : R(0);
+        J[0][0] = Jyy; J[1][0] = Jzy; J[2][0] = Jsy; J[2][2] = Jss;
+        R M[5][5];
+        for (int i = 0; i < 5; i++)
+            for (int l = 0; l < 5; l++) {
+                R acc = R(0);
+                for (int k = 0; k < 5; k++) acc = acc + J[i][k] * f.C[k][l];
+                M[i][l] = acc;
+            }
+        for (int i = 0; i < 5; i++)
+            for (int j = 0; j <= i; j++) {
+                R acc = R(0);
+                for (int l = 0; l < 5; l++) acc = acc + M[i][l] * J[j][l];
+                f.C[i][j] = acc; f.C[j][i] = acc;
+            }
+        return true;
+    }
+
+    /* ---- O10 fit of a global track: the chain of linked segments seg[0..m) (hit lists row-ascending, at least 2 hits
+       in seg[0]), each in its own sector sec[k]; sn_up[k], k >= 1: sine of the turn from sector sec[k-1] to sec[k].
+       Up pass as O8 through seg[0]; at the top hit of a segment the fit is turned into the next segment's frame
+       (rotate), moved in ONE step to the row of that segment's first hit, updated with it, and goes on row by row.
+       Down pass: fresh fit at the last hit the up pass used, (s, t, q) from there, prior covariance, the same way
+       back.  A failed transport or rotation ends a pass.  Result: state after the last update of the down pass, in
+       the frame of the sector where it ended. */
+    bool global_fit(const std::vector<const std::vector<int32_t>*>& seg, const std::vector<R>& sn_up, R cd, double g[7],
+                    int& n_fit, int& end_seg) const {
+        const int m = (int)seg.size();
+        Margin mg;
+        Fit<R> f, snap;
+        const std::vector<int32_t>& h0 = *seg[0];
+        if (h0.size() < 2) return false;
+        {
+            const R dx = X[grow[h0[1]]] - X[grow[h0[0]]];
+            const R dy = R(gy[h0[1]]) - R(gy[h0[0]]), dz = R(gz[h0[1]]) - R(gz[h0[0]]);
+            const R dl = std::sqrt(dx * dx + dy * dy);
+            f.y = R(gy[h0[0]]); f.z = R(gz[h0[0]]); f.s = dy / dl; f.t = dz / dl; f.q = R(0);
+            prior(f); f.n = 1;
+        }
+        snap = f;
+        int k_top = 0, j_top = 0;                 /* segment / position of the last hit the up pass used */
+        {
+            R xc = X[grow[h0[0]]];
+            bool alive = true;
+            for (int k = 0; k < m && alive; k++) {
+                const std::vector<int32_t>& hk = *seg[k];
+                int j = 0;
+                if (k == 0) j = 1;
+                else {   /* into the frame of segment k, then to the row of its first hit */
+                    if (!rotate(f, xc, sn_up[k], cd, mg)) break;
+                    const R xb = X[grow[hk[0]]];
+                    if (xb != xc && !transport(f, xc, xb, mg)) break;
+                    xc = xb;
+                    update(f, hk[0]); snap = f; k_top = k; j_top = 0; j = 1;
+                }
+                for (int row = grow[hk[j - 1]] + 1; j < (int)hk.size() && row <= grow[hk.back()]; row++) {
+                    if (!transport(f, xc, X[row], mg)) { alive = false; break; }
+                    xc = X[row];
+                    if (row == grow[hk[j]]) { update(f, hk[j]); snap = f; k_top = k; j_top = j; j++; }
+                }
+            }
+        }
+        {
+            const int32_t ht = (*seg[k_top])[j_top];
+            f.y = R(gy[ht]); f.z = R(gz[ht]); f.s = snap.s; f.t = snap.t; f.q = snap.q;
+            prior(f); f.n = 1;
+            snap = f;
+            int ref_row = grow[ht];
+            end_seg = k_top;
+            R xc = X[grow[ht]];
+            bool alive = true;
+            for (int k = k_top; k >= 0 && alive; k--) {
+                const std::vector<int32_t>& hk = *seg[k];
+                int j = (k == k_top) ? j_top - 1 : (int)hk.size() - 1;
+                if (k < k_top) {   /* back into the frame of segment k, then to the row of its top hit */
+                    if (!rotate(f, xc, R(0) - sn_up[k + 1], cd, mg)) break;
+                    const R xb = X[grow[hk[j]]];
+                    if (xb != xc && !transport(f, xc, xb, mg)) break;
+                    xc = xb;
+                    update(f, hk[j]); snap = f; ref_row = grow[hk[j]]; end_seg = k; j--;
+                }
+                for (int row = grow[hk[j + 1]] - 1; j >= 0 && row >= grow[hk[0]]; row--) {
+                    if (!transport(f, xc, X[row], mg)) { alive = false; break; }
+                    xc = X[row];
+                    if (row == grow[hk[j]]) { update(f, hk[j]); snap = f; ref_row = row; end_seg = k; j--; }
+                }
+            }
+            g[0] = (double)X[ref_row];
+        }
+        g[1] = (double)snap.y; g[2] = (double)snap.z; g[3] = (double)snap.s; g[4] = (double)snap.t; g[5] = (double)snap.q;
+        g[6] = (double)snap.chi2; n_fit = snap.n;
         return true;
     }
 
@@ -666,8 +787,43 @@ Result* run(const oracle_geometry& G, const oracle_params& P, int32_t n, const i
             for (int32_t h : outs[s].hits[k]) res->hit_idx.push_back(h);
         }
     }
-    if (P.merge && P.refit && stop_after == 0) merge_segments<R>(G, P, *res);
-    else {
+    {
+        const size_t T = res->trk_sector.size();
+        res->trk_g.assign(7 * T, 0.0); res->trk_g_ndf.assign(T, 0); res->trk_g_n_hits.assign(T, 0); res->trk_g_sector.assign(T, -1);
+    }
+    if (P.merge && P.refit && stop_after == 0) {
+        merge_segments<R>(G, P, *res);
+        /* ---- O10: one fit per global track ("global reconstruction") ---- */
+        const int T = (int)res->trk_sector.size();
+        const int half = G.n_sectors / 2;
+        const double step = 2.0 * 3.14159265358979323846 / (double)std::max(half, 1);
+        const R cd = R(std::cos(step)), sd = R(std::sin(step));
+        Sector<R> S(P, G, y, z, row);
+        std::vector<std::vector<int32_t>> hl(T);
+        for (int a = 0; a < T; a++)
+            hl[a].assign(res->hit_idx.begin() + res->trk_first_hit[a], res->hit_idx.begin() + res->trk_first_hit[a] + res->trk_n_hits[a]);
+        for (int a = 0; a < T; a++) {
+            if (res->trk_prev[a] >= 0 || res->trk_row_out[a] < 0) continue;   /* not the first segment / no refit */
+            std::vector<const std::vector<int32_t>*> seg;
+            std::vector<R> sn_up;
+            for (int b = a, pb = -1; b >= 0; pb = b, b = res->trk_next[b]) {
+                seg.push_back(&hl[b]);
+                if (pb < 0) sn_up.push_back(R(0));
+                else {
+                    const int dk = ((res->trk_sector[b] % half) - (res->trk_sector[pb] % half) + half) % half;
+                    sn_up.push_back(dk == 1 ? R(0) - sd : sd);
+                }
+            }
+            double g[7];
+            int n_fit = 0, end_seg = 0;
+            if (!S.global_fit(seg, sn_up, cd, g, n_fit, end_seg)) continue;
+            for (int j = 0; j < 7; j++) res->trk_g[7 * (size_t)a + j] = g[j];
+            res->trk_g_ndf[a] = 2 * n_fit - 5; res->trk_g_n_hits[a] = n_fit;
+            int b = a;
+            for (int k = 0; k < end_seg; k++) b = res->trk_next[b];
+            res->trk_g_sector[a] = res->trk_sector[b];
+        }
+    } else {
         const size_t T = res->trk_sector.size();
         res->trk_next.assign(T, -1); res->trk_prev.assign(T, -1); res->trk_global.resize(T);
         res->trk_merge_margin.assign(T, std::numeric_limits<double>::infinity());
@@ -728,7 +884,8 @@ enum {
     F_LINK_UP = 0, F_LINK_DN, F_CLINK_UP, F_CLINK_DN, F_NF_MARGIN, F_SEED_OFFSET, F_START_HIT,
     F_TL_FIRST_ROW, F_TL_LAST_ROW, F_TL_N_HITS, F_TL_PAR, F_TL_CHI2, F_TL_MARGIN, F_TL_TABLE,
     F_TRK_SECTOR, F_TRK_FIRST_HIT, F_TRK_N_HITS, F_TRK_NDF, F_TRK_SEED, F_TRK_FIRST_ROW,
-    F_TRK_X, F_TRK_Y, F_TRK_Z, F_TRK_SINPHI, F_TRK_TGL, F_TRK_QPT, F_TRK_CHI2, F_TRK_MARGIN, F_HIT_IDX, F_TL_COV, F_TRK_ROW_OUT, F_TRK_OUT, F_TRK_NEXT, F_TRK_PREV, F_TRK_GLOBAL, F_TRK_MERGE_MARGIN
+    F_TRK_X, F_TRK_Y, F_TRK_Z, F_TRK_SINPHI, F_TRK_TGL, F_TRK_QPT, F_TRK_CHI2, F_TRK_MARGIN, F_HIT_IDX, F_TL_COV, F_TRK_ROW_OUT, F_TRK_OUT, F_TRK_NEXT, F_TRK_PREV, F_TRK_GLOBAL, F_TRK_MERGE_MARGIN,
+    F_TRK_G, F_TRK_G_NDF, F_TRK_G_N_HITS, F_TRK_G_SECTOR
 };
 
 /* copy one result field into caller memory (int32 or float64, shapes in oracle/__init__.py) */
@@ -776,6 +933,10 @@ int32_t oracle_copy(const void* rv, int32_t field, void* dst) {
         case F_TRK_PREV: copy_out(r->trk_prev, dst); break;
         case F_TRK_GLOBAL: copy_out(r->trk_global, dst); break;
         case F_TRK_MERGE_MARGIN: copy_out(r->trk_merge_margin, dst); break;
+        case F_TRK_G: copy_out(r->trk_g, dst); break;
+        case F_TRK_G_NDF: copy_out(r->trk_g_ndf, dst); break;
+        case F_TRK_G_N_HITS: copy_out(r->trk_g_n_hits, dst); break;
+        case F_TRK_G_SECTOR: copy_out(r->trk_g_sector, dst); break;
         default: return -1;
     }
     return 0;
@@ -823,6 +984,24 @@ void oracle_update(const oracle_geometry* G, const oracle_params* P, double my, 
     S.update1(f, 1, mz, (double)G->sigma_z * (double)G->sigma_z);
     state[0] = f.y; state[1] = f.z; state[2] = f.s; state[3] = f.t; state[4] = f.q; *chi2 = f.chi2;
     for (int i = 0; i < 5; i++) for (int j = 0; j < 5; j++) cov[5 * i + j] = f.C[i][j];
+}
+
+/* one rotation step of O10 in double: state [y z s t q], cov 25 row-major, x in/out; angle given by its sine / cosine.
+ * Returns 0 ok, 1 failed. */
+int32_t oracle_rotate(const oracle_geometry* G, const oracle_params* P, double* x, double sn, double cd, double* state,
+                      double* cov) {
+    oracle_geometry g = *G;
+    float rx[1] = {0.f};
+    g.n_rows = 1; g.row_x = rx;
+    Margin mg;
+    Sector<double> S(*P, g, nullptr, nullptr, nullptr);
+    Fit<double> f;
+    f.y = state[0]; f.z = state[1]; f.s = state[2]; f.t = state[3]; f.q = state[4];
+    for (int i = 0; i < 5; i++) for (int j = 0; j < 5; j++) f.C[i][j] = cov[5 * i + j];
+    if (!S.rotate(f, *x, sn, cd, mg)) return 1;
+    state[0] = f.y; state[1] = f.z; state[2] = f.s; state[3] = f.t; state[4] = f.q;
+    for (int i = 0; i < 5; i++) for (int j = 0; j < 5; j++) cov[5 * i + j] = f.C[i][j];
+    return 0;
 }
 
 /* O9 on caller-given segments (for the pins): T segments with sector, first fitted row, parameters
