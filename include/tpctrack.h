@@ -68,7 +68,8 @@ typedef struct {
                                  * gate; trk_x/y/z/sinphi/tgl/qpt/chi2/ndf are then the refit's (x = row of the
                                  * lowest hit the down pass reached, ndf = 2 * hits in the refit - 5) */
     int32_t merge;              /* 1: link the track segments of one particle across sector borders (O9, SURVEY.md
-                                 * 8(f).2; needs refit = 1): trk_next / trk_prev.  Sectors: n_sectors / 2 per side,
+                                 * 8(f).2; needs refit = 1): trk_next / trk_prev / trk_global, and fit every global
+                                 * track over all its segments (O10): trk_g_*.  Sectors: n_sectors / 2 per side,
                                  * sector s = side * (n_sectors / 2) + k at azimuth (k + 1/2) * 4 pi / n_sectors */
     float merge_dy, merge_dz;   /* cm: tolerated |dy|, |dz| between the extrapolated and the found segment */
     float merge_ds, merge_dt;   /* tolerated |d sin phi|, |d tg lambda| */
@@ -134,6 +135,21 @@ typedef struct {
     const int32_t* trk_prev;      /* [n_tracks] */
     const int32_t* trk_global;    /* [n_tracks] the global track a segment belongs to = the chain of linked segments,
                                    * named by the index of its first (innermost) segment */
+    /* tpc_params.merge = 1: the fit of the global track over the hits of ALL its segments (up and
+     * down pass as the refit, the fit turned into the next sector's frame at each border), stored at the chain's
+     * first segment i = trk_global[...]: parameters at x = trk_g_x[i] in the frame of sector trk_g_sector[i]
+     * (normally the first segment's).  A lone segment's global fit is its refit; entries of segments that are not
+     * the first of their chain are 0 (trk_g_sector -1). */
+    const float* trk_g_x;         /* [n_tracks] cm */
+    const float* trk_g_y;
+    const float* trk_g_z;
+    const float* trk_g_sinphi;
+    const float* trk_g_tgl;
+    const float* trk_g_qpt;
+    const float* trk_g_chi2;
+    const int32_t* trk_g_ndf;     /* [n_tracks] 2 * trk_g_n_hits - 5 */
+    const int32_t* trk_g_n_hits;  /* [n_tracks] hits in the global fit */
+    const int32_t* trk_g_sector;  /* [n_tracks] */
 } tpc_event_out;
 
 /* Counters of the last call (whole batch); used for the algorithmic-byte count of DESIGN.md. */

@@ -111,6 +111,9 @@ struct View {
     float *o_xo, *o_yo, *o_zo, *o_so, *o_to, *o_qo;   // [S_cap] outer state of the refit (up pass at its top hit)
     int32_t *o_next, *o_prev;   // [S_cap] O9 links, event-local track index or -1
     int32_t* o_global;          // [S_cap] first segment of the chain a track belongs to, event-local
+    // O10: fit of the global track, at its first segment
+    float *o_gx, *o_gy, *o_gz, *o_gs, *o_gt, *o_gq, *o_gchi2;
+    int32_t *o_gndf, *o_gnhits, *o_gsector;
     unsigned long long* cnt; // [CNT_N]
     unsigned long long* kf_cursor;  // [kNCursors] units of work handed out: [0] K5 sector tasks, [2] refit
 };

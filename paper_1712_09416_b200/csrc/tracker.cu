@@ -15,11 +15,15 @@
 #include "sel_kernels.cuh"
 #include "kf_refit.cuh"
 #include "merge_kernels.cuh"
+#include "kf_global.cuh"
 #include "peak_kernels.cuh"
 
 namespace {
 
-constexpr int kOutI = 7, kOutF = 13;   // int32 / float arrays per track: 4 + next, prev, global; 7 + the outer state
+// int32 / float arrays per track: 4 + next, prev, global + global fit (ndf, hits, sector); 7 + the outer state (6) + the
+// global fit (7)
+constexpr int kOutI = 10, kOutF = 20;
+constexpr int kOutI_plain = 4, kOutF_plain = 7, kOutF_refit = 13;
 
 thread_local std::string g_err;
 
@@ -222,8 +226,11 @@ int reserve_batch(const tpc_tracker* tr, Batch* t, int n_events, int64_t N, int6
     RS(ev_off_d, 2 * ((size_t)n_events + 1)); RS(h_ev_off, 2 * ((size_t)n_events + 1));
     RS(scratch, (size_t)std::max<int64_t>(nb, S_cap) / kScanTile + 8);   // scans: tile counter + status words
     RS(cnt, CNT_N); RS(h_cnt, CNT_N); RS(kf_cursor, kNCursors); RS(h_nseeds, 1);
-    for (int k = 0; k < kOutI; k++) RS(o_i[k], S_cap);
-    for (int k = 0; k < kOutF; k++) RS(o_f[k], S_cap);
+    {   // output arrays: only those that this tracker's parameters fill
+        const int nI = tr->c.p.merge ? kOutI : kOutI_plain, nF = tr->c.p.merge ? kOutF : tr->c.p.refit ? kOutF_refit : kOutF_plain;
+        for (int k = 0; k < nI; k++) RS(o_i[k], S_cap);
+        for (int k = 0; k < nF; k++) RS(o_f[k], S_cap);
+    }
     if (tr->c.p.refit) { RS(trk_rows, S_cap); RS(trk_task, S_cap); }
     if (tr->c.p.merge) { RS(mg_next, S_cap); RS(mg_prev, S_cap); RS(mg_list, S_cap); }
     RS(o_hit, n);
@@ -328,6 +335,8 @@ int launch_all(const tpc_tracker* tr, Batch* t, int from = 1) {
         k_merge_pairs<<<g, 128, 0, st>>>(v, c, t->mg_list.p, t->mg_next.p, t->mg_prev.p); L++;
         k_merge_mutual<<<g, 128, 0, st>>>(v, c, t->mg_next.p, t->mg_prev.p); L++;
         k_merge_chain<<<g, 128, 0, st>>>(v, ns); L++;
+        k_global_prep<<<g, kGfThreads, 0, st>>>(v, t->mg_list.p); L++;               // O10: the chains' first segments ...
+        k_global_fit<<<tr->rf_blocks, kGfThreads, 0, st>>>(v, c, t->mg_list.p); L++;   // ... and their fits
     }
     mark(6);
     CK(cudaGetLastError());
@@ -406,6 +415,9 @@ int batch_begin(const tpc_tracker* tr, Batch* t, int first_event, int n, const t
     v.o_x = t->o_f[0].p; v.o_y = t->o_f[1].p; v.o_z = t->o_f[2].p; v.o_sinphi = t->o_f[3].p;
     v.o_tgl = t->o_f[4].p; v.o_qpt = t->o_f[5].p; v.o_chi2 = t->o_f[6].p;
     v.o_xo = t->o_f[7].p; v.o_yo = t->o_f[8].p; v.o_zo = t->o_f[9].p; v.o_so = t->o_f[10].p; v.o_to = t->o_f[11].p; v.o_qo = t->o_f[12].p;
+    v.o_gndf = t->o_i[7].p; v.o_gnhits = t->o_i[8].p; v.o_gsector = t->o_i[9].p;
+    v.o_gx = t->o_f[13].p; v.o_gy = t->o_f[14].p; v.o_gz = t->o_f[15].p; v.o_gs = t->o_f[16].p; v.o_gt = t->o_f[17].p;
+    v.o_gq = t->o_f[18].p; v.o_gchi2 = t->o_f[19].p;
     v.o_next = t->o_i[4].p; v.o_prev = t->o_i[5].p; v.o_global = t->o_i[6].p; v.trk_rows = t->trk_rows.p; v.trk_task = t->trk_task.p;
     v.cnt = t->cnt.p; v.kf_cursor = t->kf_cursor.p;
     v.o_hit_yz = t->o_hit_yz.p; v.o_hit_row = t->o_hit_row.p; v.trk_hit0 = t->trk_hit0.p;
@@ -681,7 +693,7 @@ int tpc_track_events(tpc_tracker* t, int32_t n, const tpc_event_in* in, tpc_even
     t->n_events = n;
 
     int64_t T_cum = 0, H_cum = 0;
-    const int nI = t->c.p.merge ? kOutI : 4, nF = t->c.p.refit ? kOutF : 7;   // arrays that hold something
+    const int nI = t->c.p.merge ? kOutI : kOutI_plain, nF = t->c.p.merge ? kOutF : t->c.p.refit ? kOutF_refit : kOutF_plain;   // arrays that hold something
     std::vector<int64_t> trk_off(n + 1, 0), hit_off(n + 1, 0);   // per event, in the call's output arrays
     std::vector<const Batch*> ev_batch(n, nullptr);
     int g_issue = 0, g_done = 0;
@@ -754,6 +766,10 @@ int tpc_track_events(tpc_tracker* t, int32_t n, const tpc_event_in* in, tpc_even
         o.trk_out_sinphi = rf ? of[10] + a : nullptr; o.trk_out_tgl = rf ? of[11] + a : nullptr;
         o.trk_out_qpt = rf ? of[12] + a : nullptr;
         o.trk_next = mg ? oi[4] + a : nullptr; o.trk_prev = mg ? oi[5] + a : nullptr; o.trk_global = mg ? oi[6] + a : nullptr;
+        o.trk_g_ndf = mg ? oi[7] + a : nullptr; o.trk_g_n_hits = mg ? oi[8] + a : nullptr; o.trk_g_sector = mg ? oi[9] + a : nullptr;
+        o.trk_g_x = mg ? of[13] + a : nullptr; o.trk_g_y = mg ? of[14] + a : nullptr; o.trk_g_z = mg ? of[15] + a : nullptr;
+        o.trk_g_sinphi = mg ? of[16] + a : nullptr; o.trk_g_tgl = mg ? of[17] + a : nullptr; o.trk_g_qpt = mg ? of[18] + a : nullptr;
+        o.trk_g_chi2 = mg ? of[19] + a : nullptr;
         o.hit_idx = ohit + h;
     }
     t->have_result = true;
@@ -801,7 +817,7 @@ int tpc_wait_events(tpc_tracker* t, int32_t ticket, tpc_event_out* out) {
     t->one_group = false;
     const int n = b->n_events;
     const int64_t T = b->counters.n_tracks, H = b->counters.n_track_hits;
-    const int nI = t->c.p.merge ? kOutI : 4, nF = t->c.p.refit ? kOutF : 7;
+    const int nI = t->c.p.merge ? kOutI : kOutI_plain, nF = t->c.p.merge ? kOutF : t->c.p.refit ? kOutF_refit : kOutF_plain;
     const int32_t* oi[kOutI]; const float* of[kOutF]; const int32_t* ohit;
     if (b->host_in) {
         for (int k = 0; k < nI; k++) {
@@ -841,6 +857,10 @@ int tpc_wait_events(tpc_tracker* t, int32_t ticket, tpc_event_out* out) {
         o.trk_out_sinphi = rf ? of[10] + at : nullptr; o.trk_out_tgl = rf ? of[11] + at : nullptr;
         o.trk_out_qpt = rf ? of[12] + at : nullptr;
         o.trk_next = mg ? oi[4] + at : nullptr; o.trk_prev = mg ? oi[5] + at : nullptr; o.trk_global = mg ? oi[6] + at : nullptr;
+        o.trk_g_ndf = mg ? oi[7] + at : nullptr; o.trk_g_n_hits = mg ? oi[8] + at : nullptr; o.trk_g_sector = mg ? oi[9] + at : nullptr;
+        o.trk_g_x = mg ? of[13] + at : nullptr; o.trk_g_y = mg ? of[14] + at : nullptr; o.trk_g_z = mg ? of[15] + at : nullptr;
+        o.trk_g_sinphi = mg ? of[16] + at : nullptr; o.trk_g_tgl = mg ? of[17] + at : nullptr; o.trk_g_qpt = mg ? of[18] + at : nullptr;
+        o.trk_g_chi2 = mg ? of[19] + at : nullptr;
     }
     return TPC_OK;
 }
@@ -1120,6 +1140,10 @@ int tpc_debug_resume(tpc_tracker* tr, int32_t from_stage, tpc_event_out* out) {
         o.trk_out_sinphi = rf ? t->o_f[10].p + a : nullptr; o.trk_out_tgl = rf ? t->o_f[11].p + a : nullptr;
         o.trk_out_qpt = rf ? t->o_f[12].p + a : nullptr;
         o.trk_next = mg ? t->o_i[4].p + a : nullptr; o.trk_prev = mg ? t->o_i[5].p + a : nullptr; o.trk_global = mg ? t->o_i[6].p + a : nullptr;
+        o.trk_g_ndf = mg ? t->o_i[7].p + a : nullptr; o.trk_g_n_hits = mg ? t->o_i[8].p + a : nullptr; o.trk_g_sector = mg ? t->o_i[9].p + a : nullptr;
+        o.trk_g_x = mg ? t->o_f[13].p + a : nullptr; o.trk_g_y = mg ? t->o_f[14].p + a : nullptr; o.trk_g_z = mg ? t->o_f[15].p + a : nullptr;
+        o.trk_g_sinphi = mg ? t->o_f[16].p + a : nullptr; o.trk_g_tgl = mg ? t->o_f[17].p + a : nullptr; o.trk_g_qpt = mg ? t->o_f[18].p + a : nullptr;
+        o.trk_g_chi2 = mg ? t->o_f[19].p + a : nullptr;
     }
     return TPC_OK;
 }

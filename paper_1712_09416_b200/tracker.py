@@ -50,12 +50,15 @@ _OUT_I = ("trk_sector", "trk_first_hit", "trk_n_hits", "trk_ndf")
 _OUT_F = ("trk_x", "trk_y", "trk_z", "trk_sinphi", "trk_tgl", "trk_qpt", "trk_chi2")
 _OUT_F2 = ("trk_out_x", "trk_out_y", "trk_out_z", "trk_out_sinphi", "trk_out_tgl", "trk_out_qpt")   # refit = 1
 _OUT_I2 = ("trk_next", "trk_prev", "trk_global")                                                                   # merge = 1
+_OUT_F3 = ("trk_g_x", "trk_g_y", "trk_g_z", "trk_g_sinphi", "trk_g_tgl", "trk_g_qpt", "trk_g_chi2")   # merge = 1 (O10)
+_OUT_I3 = ("trk_g_ndf", "trk_g_n_hits", "trk_g_sector")
 
 
 class tpc_event_out(C.Structure):
     _fields_ = ([("n_tracks", C.c_int32), ("n_track_hits", C.c_int32)] + [(n, C.c_void_p) for n in _OUT_I]
                 + [(n, C.c_void_p) for n in _OUT_F] + [("hit_idx", C.c_void_p)]
-                + [(n, C.c_void_p) for n in _OUT_F2] + [(n, C.c_void_p) for n in _OUT_I2])
+                + [(n, C.c_void_p) for n in _OUT_F2] + [(n, C.c_void_p) for n in _OUT_I2]
+                + [(n, C.c_void_p) for n in _OUT_F3] + [(n, C.c_void_p) for n in _OUT_I3])
 
 
 class tpc_counters(C.Structure):
@@ -317,7 +320,10 @@ class Tracker:
         for k in _OUT_F2:          # present with refit = 1
             if getattr(out, k):
                 res[k] = fetch(getattr(out, k), T, np.float32)
-        for k in _OUT_I2:          # present with merge = 1
+        for k in _OUT_I2 + _OUT_I3:          # present with merge = 1
             if getattr(out, k):
                 res[k] = fetch(getattr(out, k), T, np.int32)
+        for k in _OUT_F3:
+            if getattr(out, k):
+                res[k] = fetch(getattr(out, k), T, np.float32)
         return res

@@ -22,7 +22,7 @@ def tr():
 def declared_functions():
     src = (ROOT / "include" / "tpctrack.h").read_text()
     src = re.sub(r"/\*.*?\*/", "", src, flags=re.S)
-    return sorted(set(re.findall(r"\b(tpc_[a-z_]+)\s*\(", src)))
+    return sorted(set(re.findall(r"\b(tpc_[a-z0-9_]+)\s*\(", src)))
 
 
 def test_library_exports_every_declared_symbol(tr):
@@ -36,7 +36,7 @@ def test_library_exports_every_declared_symbol(tr):
 def test_struct_layouts_match_header(tr):
     assert C.sizeof(tr.tpc_params) == 27 * 4
     assert C.sizeof(tr.tpc_event_in) == 8 + 8 * 5 + 8          # int32 + pad, 5 pointers, int32 + pad
-    assert C.sizeof(tr.tpc_event_out) == 8 + 8 * 21
+    assert C.sizeof(tr.tpc_event_out) == 8 + 8 * 31
     assert C.sizeof(tr.tpc_counters) == 13 * 8
     assert C.sizeof(tr.tpc_geometry) == 8 + 8 + 16 + 8
 

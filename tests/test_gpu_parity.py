@@ -334,6 +334,16 @@ def test_merge_parity(trk_mod, gen_mod, oracle_mod, name, device):
     assert np.array_equal(res["trk_next"], ref.trk_next) and np.array_equal(res["trk_prev"], ref.trk_prev)
     assert np.array_equal(res["trk_global"], ref.trk_global)
     assert (res["trk_next"] >= 0).sum() >= (40 if name == "pp" else 1000)
+    # O10: the fit of every global track over all its segments
+    for k in ("trk_g_ndf", "trk_g_n_hits", "trk_g_sector"):
+        assert np.array_equal(res[k], ref[k]), k
+    gfit = np.stack([res[k] for k in ("trk_g_x", "trk_g_y", "trk_g_z", "trk_g_sinphi", "trk_g_tgl", "trk_g_qpt",
+                                      "trk_g_chi2")], axis=1)
+    err = np.abs(gfit - ref.trk_g) / np.maximum(1.0, np.abs(ref.trk_g))
+    assert err.max(initial=0.0) <= TOL, err.max()
+    chains = (ref.trk_prev < 0) & (ref.trk_next >= 0)
+    more = res["trk_g_n_hits"][chains] > res["trk_n_hits"][chains]      # more hits than the first segment alone
+    assert more.mean() > 0.9                                            # (a failed turn at a border ends a pass early)
     trk.close()
 
 
