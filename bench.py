@@ -9,7 +9,7 @@ K5 Kalman tracklet constructor, K6 selector + output) over one batch of 16 synth
 
 * default arm: ``value`` = events/s with the inputs resident in HBM; ``e2e`` = the same work from pinned HOST
   buffers (H2D of the clusters and D2H of the tracks inside the timed region) through ``tpc_submit_events`` /
-  ``tpc_wait_events`` with two batches in flight (``e2e.single_call``: ``tpc_track_events``, one call at a time); ``roofline`` = the dominant kernel
+  ``tpc_wait_events`` with three batches in flight (``e2e.single_call``: ``tpc_track_events``, one call at a time); ``roofline`` = the dominant kernel
   (K5) against the measured HBM copy bandwidth; ``cpu_baseline`` = the oracle timed on the host cores.
 * ``--impl reference``: the CPU oracle, as it stands, on the host cores (one event per step).
 * N > 1 (torchrun): replicas only -- every rank tracks its own batch on its own GPU; no collective on the data path.
@@ -333,23 +333,25 @@ def main():
         e2e = {"value": aggregate_value(len(evs), args.steps, ms_e, world), "unit": UNIT,
                "h2d_bytes_per_step": int(12 * n_total + sum(4 * (ev.n_sectors + 1) for ev in evs)),
                "d2h_bytes_per_step": int(44 * n_tracks + 4 * n_hits), "ms_per_step": ms_e / args.steps}
-        # Pipelined: tpc_submit_events / tpc_wait_events keep two batches in flight on one tracker, so that the copies
+        # Pipelined: tpc_submit_events / tpc_wait_events keep three batches in flight on one tracker, so that the copies
         # of one batch overlap the kernels of the other.  Same host buffers, same bytes per step; every step's result
         # is waited for and read.  Reported beside the single-call figure, not instead of it.
         trk.tpc_tracker_set_profiling(False)
-        for _ in range(2):                # warm-up with both tickets in flight (each owns its work space and buffers)
-            ta, tb = trk.tpc_submit_events(host_in), trk.tpc_submit_events(host_in)
-            trk.tpc_wait_events(ta); trk.tpc_wait_events(tb)
+        for _ in range(2):                # warm-up with all tickets in flight (each owns its work space and buffers)
+            tk = [trk.tpc_submit_events(host_in) for _ in range(3)]
+            for x in tk:
+                trk.tpc_wait_events(x)
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         barrier()
         e0.record()
-        prev = trk.tpc_submit_events(host_in)
-        for _ in range(args.steps - 1):
-            nxt = trk.tpc_submit_events(host_in)
-            got = sum(o.n_tracks for o in trk.tpc_wait_events(prev))
+        # three batches in flight: the clusters of step k+2 are on their way in while the kernels of step k+1 run and
+        # the tracks of step k go out
+        flight = [trk.tpc_submit_events(host_in) for _ in range(min(2, args.steps))]
+        for k in range(args.steps):
+            if k + 2 < args.steps:
+                flight.append(trk.tpc_submit_events(host_in))
+            got = sum(o.n_tracks for o in trk.tpc_wait_events(flight.pop(0)))
             assert got == n_tracks
-            prev = nxt
-        got = sum(o.n_tracks for o in trk.tpc_wait_events(prev))
         torch.cuda.synchronize()          # every wait has returned: all work is complete
         e1.record()
         barrier()
@@ -359,7 +361,7 @@ def main():
         e2e = {"value": aggregate_value(len(evs), args.steps, ms_p, world), "unit": UNIT,
                "h2d_bytes_per_step": e2e["h2d_bytes_per_step"], "d2h_bytes_per_step": e2e["d2h_bytes_per_step"],
                "ms_per_step": ms_p / args.steps,
-               "api": "tpc_submit_events / tpc_wait_events, two batches in flight on one tracker; every step copies its "
+               "api": "tpc_submit_events / tpc_wait_events, three batches in flight on one tracker; every step copies its "
                       "clusters in from pinned host memory and its tracks out, and every result is waited for",
                "single_call": {"value": e2e["value"], "unit": UNIT, "ms_per_step": e2e["ms_per_step"],
                                "api": "tpc_track_events, one call at a time (copies of its event groups overlap its kernels)"}}

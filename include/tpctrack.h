@@ -199,11 +199,11 @@ int tpc_track_event(tpc_tracker* t, const tpc_event_in* in, tpc_event_out* out);
  * in/out are host arrays of n structs; all inputs must share one mem_space. */
 int tpc_track_events(tpc_tracker* t, int32_t n, const tpc_event_in* in, tpc_event_out* out);
 
-/* The same pass in two halves, so that two batches can be in flight: while the kernels of one batch run, the
+/* The same pass in two halves, so that up to three batches can be in flight: while the kernels of one batch run, the
  * clusters of the next are copied in and the tracks of the one before are copied out ("asynchronous data
  * processing", the paper's title; the sync call above exposes those copies).
  * tpc_submit_events enqueues the input copies and all kernels of a batch on a stream of its own and returns at once
- * with a ticket (0 or 1); at most two batches are in flight (a third submit returns TPC_ERR_ARG).  The `in` array,
+ * with a ticket (0, 1 or 2); at most three batches are in flight (a fourth submit returns TPC_ERR_ARG).  The `in` array,
  * the sector offsets and the cluster arrays must stay valid and unchanged until the matching wait returns.
  * tpc_wait_events waits for that batch, copies the outputs back (host inputs) and fills out[0..n).  The outputs
  * are library-owned (each ticket has its own output arrays, host or device) and stay valid until the next wait on

@@ -33,9 +33,9 @@ namespace tpc {
 #ifndef TPC_CT_INL
 #define TPC_CT_INL __forceinline__   // intake / turn inlined: 5.95 ms against 6.42 ms out of line (config 5)
 #endif
-constexpr int kCtWarps = TPC_CT_WARPS;                 // consumer warps of a CTA (one more warp produces)
-constexpr int kCtConsumers = kCtWarps * 32;
-constexpr int kCtThreads = (kCtWarps + 1) * 32;
+constexpr int kCtWarps = TPC_CT_WARPS;                 // consumer warps of a CTA (one more warp produces), two CTAs per SM
+constexpr int kCtWarpsWide = 19;                       // ... of the one-CTA-per-SM tiers (640 threads x 96 registers, no spills)
+constexpr int ct_threads(int warps) { return (warps + 1) * 32; }
 constexpr int kCtRing = TPC_CT_RING;                   // rows in flight
 constexpr int kCtWords = 32;                           // 4-byte words of a tracklet's state
 #ifndef TPC_CT_STAGE
@@ -45,7 +45,10 @@ constexpr int kCtSeedStage = TPC_CT_STAGE;             // start-hit records of a
 // State slots per sector task = tracklets under way at once, in three tiers (the host moves up one tier when a
 // launch reports kErrSlotCapacity and stays there): shared-memory slots + slots in global memory (L2)
 constexpr int kCtTiers = 3;
-constexpr int kCtCapSmem[kCtTiers] = {512, 1408, 1280};   // tier 0: two CTAs per SM; tiers 1, 2: one
+#ifndef TPC_CT_CAP0
+#define TPC_CT_CAP0 512
+#endif
+constexpr int kCtCapSmem[kCtTiers] = {TPC_CT_CAP0, 1408, 1280};   // tier 0: two CTAs per SM; tiers 1, 2: one
 constexpr int kCtCapSpill[kCtTiers] = {0, 0, 4096};
 constexpr int kCtCapMax = 1280 + 4096;
 constexpr int kSwCap = 640;                            // hits of a row staged in shared memory; larger rows are read in place
@@ -118,7 +121,7 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
                  ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 // barrier of the consumer warps only (the producer never joins)
-__device__ __forceinline__ void ct_bar() { asm volatile("bar.sync 1, %0;" ::"n"(kCtConsumers) : "memory"); }
+template <int W> __device__ __forceinline__ void ct_bar() { asm volatile("bar.sync 1, %0;" ::"n"(W * 32) : "memory"); }
 
 __device__ __forceinline__ size_t cell_index(int base, int bin) { return (size_t)kCellsPerHit * base + (size_t)bin * kCellPad; }
 
@@ -340,10 +343,11 @@ __device__ __forceinline__ void ct_push(CtSmem& sm, uint16_t* freel, int slot, i
 // ---- intake, by all consumer threads between the row steps ----
 // down sweep: the parked tracklets whose top hit is in this row start a fresh fit there (their records come
 // ordered by top row: staged in the ring slot, the ones beyond kCtSeedStage read in place)
+template <int W>
 __device__ TPC_CT_INL void ct_intake_down(const View& v, const Const& c, CtSmem& sm, const CtSlots& sl, const uint16_t* freel,
                                             int cap, int row, int s) {
     const int n = sm.cnt[row], lo = sm.i0 + sm.lo[row];
-    for (int j0 = 0; j0 < n; j0 += kCtConsumers) {
+    for (int j0 = 0; j0 < n; j0 += W * 32) {
         const int j = j0 + (int)threadIdx.x;
         const int slot = ct_pop(v, sm, freel, j < n, cap);
         if (slot >= 0) {
@@ -367,6 +371,7 @@ __device__ TPC_CT_INL void ct_intake_down(const View& v, const Const& c, CtSmem&
     }
 }
 // up sweep: the start hits of this row that no up pass has recorded build a tracklet; returns how many (this thread)
+template <int W>
 __device__ TPC_CT_INL unsigned ct_intake_up(const View& v, const Const& c, CtSmem& sm, const CtSlots& sl, const uint16_t* freel,
                                               int cap, int row, int s, int S) {
     const int D = c.p.link_step;
@@ -374,7 +379,7 @@ __device__ TPC_CT_INL unsigned ct_intake_up(const View& v, const Const& c, CtSme
     const int n = sm.cnt[row], lo = sm.lo[row], base = sm.desc[row].base;
     const uint32_t* const ub = sm.used[row & 1];
     unsigned built = 0;
-    for (int j0 = 0; j0 < n; j0 += kCtConsumers) {
+    for (int j0 = 0; j0 < n; j0 += W * 32) {
         const int j = j0 + (int)threadIdx.x, e = lo + j;
         bool need = false;
         int hl = 0;
@@ -410,6 +415,7 @@ __device__ TPC_CT_INL unsigned ct_intake_up(const View& v, const Const& c, CtSme
     return built;
 }
 // between the sweeps (all consumer warps): the parked tracklets of the task, ordered by top row, into dn_rec
+template <int W>
 __device__ TPC_CT_INL void ct_turn(const View& v, CtSmem& sm, int nr) {
     const int lane = lane_id(), warp = threadIdx.x >> 5;
     if (warp == 0) {   // lo = exclusive scan of the counts, cnt = the counts, dcnt = 0 (fill counters of the scatter)
@@ -424,10 +430,10 @@ __device__ TPC_CT_INL void ct_turn(const View& v, CtSmem& sm, int nr) {
             carry += __shfl_sync(kFull, incl, 31);
         }
     }
-    ct_bar();
+    ct_bar<W>();
     const uint32_t* const plist = v.kf_park + sm.i0;
     const int np = sm.n_parked;
-    for (int k = threadIdx.x; k < np; k += kCtConsumers) {
+    for (int k = threadIdx.x; k < np; k += W * 32) {
         const uint32_t w = __ldcg(&plist[k]);
         const int top = (int)(w >> 24), id = sm.i0 + (int)(w & 0xffffffu);
         const int pos = sm.lo[top] + atomicAdd(&sm.dcnt[top], 1);
@@ -437,13 +443,14 @@ __device__ TPC_CT_INL void ct_turn(const View& v, CtSmem& sm, int nr) {
         dst[0] = a4; dst[1] = b4;
     }
     asm volatile("fence.proxy.async;" ::: "memory");   // the producer's bulk copies (async proxy) will read these records
-    ct_bar();
+    ct_bar<W>();
 }
 
 // ---------------------------------------------------------------------------------------------------------
 // K5
 // ---------------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kCtThreads, 2) k_construct(const __grid_constant__ View v, const __grid_constant__ Const c, const int cap_s,
+template <int W>
+__global__ void __launch_bounds__((W + 1) * 32, W <= 10 ? 2 : 1) k_construct(const __grid_constant__ View v, const __grid_constant__ Const c, const int cap_s,
                                                              const int cap_g, float* const spill) {
     extern __shared__ __align__(128) unsigned char ct_raw[];
     TPC_RETURN_IF_REJECTED(v);
@@ -455,13 +462,13 @@ __global__ void __launch_bounds__(kCtThreads, 2) k_construct(const __grid_consta
     uint16_t* const freel = reinterpret_cast<uint16_t*>(sl.st + (size_t)kCtWords * cap_s);   // stack of free slots
     const int warp = threadIdx.x >> 5, lane = lane_id();
     if (threadIdx.x == 0) {
-        for (int s = 0; s < kCtRing; s++) { mbar_init(&sm.full[s], 1); mbar_init(&sm.empty[s], kCtWarps); }
+        for (int s = 0; s < kCtRing; s++) { mbar_init(&sm.full[s], 1); mbar_init(&sm.empty[s], W); }
         mbar_init(&sm.tbar, 1);
         sm.abort = 0;
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
-    if (warp == kCtWarps) { ct_producer(v, c, sm, freel, cap); return; }
+    if (warp == W) { ct_producer(v, c, sm, freel, cap); return; }
 
     const int nr = c.n_rows, D = c.p.link_step;
     const int S = min(v.seed_start[v.n_bins], v.S_cap);
@@ -483,7 +490,7 @@ __global__ void __launch_bounds__(kCtThreads, 2) k_construct(const __grid_consta
         const int cmd = sm.cmd[s];
         if (cmd < 0) break;
         if (cmd == kCtTurn) {
-            ct_turn(v, sm, nr);
+            ct_turn<W>(v, sm, nr);
             __syncwarp();
             if (lane == 0) mbar_arrive(&sm.empty[s]);
             it++;
@@ -500,14 +507,18 @@ __global__ void __launch_bounds__(kCtThreads, 2) k_construct(const __grid_consta
         const uint16_t* const cs = staged ? reinterpret_cast<const uint16_t*>(sm.cells[s]) + (cg & 7) : v.cells + cg;
         uint32_t* const plist = v.kf_park + sm.i0;   // parked tracklets of this task, in order of parking
 
-        if (!up) {   // down sweep: what starts at this row is taken in BEFORE the row is processed (and starts below it)
-            if (sm.cnt[row] > 0) ct_intake_down(v, c, sm, sl, freel, cap, row, s);
-            ct_bar();
+        // The consumer warps meet at barriers only around an intake: rows where nothing starts (most rows of a sparse
+        // event) are processed by every warp on its own, up to a ring's depth apart.
+        const bool intake = sm.cnt[row] > 0;
+        if (!up && intake) {   // down sweep: what starts at this row is taken in BEFORE the row is processed (and starts
+            ct_bar<W>();          // below it); all slots freed by the rows above are back on the stack
+            ct_intake_down<W>(v, c, sm, sl, freel, cap, row, s);
+            ct_bar<W>();
         }
         PF(1)
         // ---- one pad row for the tracklets under way: the warps share the groups of 32 slots ----
         const int n_groups = (*(volatile int32_t*)&sm.n_hw + 31) >> 5;
-        for (int g = warp; g < n_groups; g += kCtWarps) {
+        for (int g = warp; g < n_groups; g += W) {
             const uint32_t occ = *(volatile uint32_t*)&sm.occ[g];
             if (!occ) continue;
             const int slot = (g << 5) + lane;
@@ -597,8 +608,10 @@ __global__ void __launch_bounds__(kCtThreads, 2) k_construct(const __grid_consta
                 updates++;
                 if (up) {
                     t.p0 = ay; t.p1 = az; t.p2 = f.s; t.p3 = f.t; t.p4 = f.q; t.top = row;
-                    const int hl = acc - dn.x;                  // seed de-duplication: this hit is being followed
-                    atomicOr(&sm.used[row & 1][hl >> 5], 1u << (hl & 31));
+                    if (intake) {                               // seed de-duplication: this hit is being followed
+                        const int hl = acc - dn.x;              // (marks matter only where start hits wait)
+                        atomicOr(&sm.used[row & 1][hl >> 5], 1u << (hl & 31));
+                    }
                 } else {
                     t.p0 = f.y; t.p1 = f.z; t.p2 = f.s; t.p3 = f.t; t.p4 = f.q; t.p5 = f.chi2; t.aux = row;
                 }
@@ -629,14 +642,19 @@ __global__ void __launch_bounds__(kCtThreads, 2) k_construct(const __grid_consta
             if (fin) ct_push(sm, freel, slot, cap);
         }
         PF(3)
-        ct_bar();
-        PF(4)
-        if (up) {   // up sweep: the start hits of this row are taken in AFTER it is processed (its marks are complete)
-            if (sm.cnt[row] > 0) built += ct_intake_up(v, c, sm, sl, freel, cap, row, s, S);
+        // up sweep: the start hits of this row are taken in AFTER it is processed (its marks are complete); the marks'
+        // other buffer is cleared here for the next row if start hits wait there (its last readers, the intake two rows
+        // down, are behind that row's barriers)
+        const bool next_intake = up && row + 1 < nr && sm.cnt[row + 1] > 0;
+        if (up && (intake || next_intake)) {
+            ct_bar<W>();
+            PF(4)
+            if (intake) built += ct_intake_up<W>(v, c, sm, sl, freel, cap, row, s, S);
             PF(8)
-            for (int k = threadIdx.x; k < TPC_MAX_ROW_HITS / 32; k += kCtConsumers) sm.used[(row + 1) & 1][k] = 0u;
+            if (next_intake)
+                for (int k = threadIdx.x; k < TPC_MAX_ROW_HITS / 32; k += W * 32) sm.used[(row + 1) & 1][k] = 0u;
             PF(9)
-            ct_bar();
+            ct_bar<W>();
         }
         PF(5)
         __syncwarp();

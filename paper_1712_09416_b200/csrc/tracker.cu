@@ -24,6 +24,7 @@ namespace {
 // global fit (7)
 constexpr int kOutI = 10, kOutF = 20;
 constexpr int kOutI_plain = 4, kOutF_plain = 7, kOutF_refit = 13;
+constexpr int kAsync = 3;              // batches in flight through tpc_submit_events
 
 thread_local std::string g_err;
 
@@ -158,7 +159,8 @@ struct tpc_tracker {
     Buf<float> h_o_f[kOutF];
     bool profiling = false;
     float stage_ms[TPC_N_STAGES] = {};
-    // tpc_submit_events / tpc_wait_events: two batches in flight, each with its own work space, stream and outputs
+    // tpc_submit_events / tpc_wait_events: up to three batches in flight (copy in | kernels | copy out), each with its
+    // own work space, stream and outputs
     struct Async {
         Batch* b = nullptr;
         bool busy = false;
@@ -166,7 +168,8 @@ struct tpc_tracker {
         Buf<float> h_o_f[kOutF];
         Buf<int32_t> d_o_i[kOutI], d_o_hit;      // device inputs: this ticket's outputs (swapped with the batch's at wait,
         Buf<float> d_o_f[kOutF];                 // so that the batch's next run does not write over them)
-    } async[2];
+    } async[kAsync];
+    int last_ticket = -1;                    // the batch submitted last (the next one's kernels queue behind its kernels)
 
     tpc_tracker() {
         for (auto& a : async) {
@@ -310,7 +313,9 @@ int launch_all(const tpc_tracker* tr, Batch* t, int from = 1) {
     if (from <= 5) {   // K5: one CTA per sector task, up sweep then down sweep (kf_construct.cuh)
         const int tier = t->ct_tier;
         const int grid = std::max(1, std::min(tr->ct_blocks[tier], v.n_tasks));
-        k_construct<<<grid, kCtThreads, ct_smem_bytes(tier), st>>>(v, c, kCtCapSmem[tier], kCtCapSpill[tier], tr->ct_spill.p); L++;
+        if (tier == 0) k_construct<kCtWarps><<<grid, ct_threads(kCtWarps), ct_smem_bytes(tier), st>>>(v, c, kCtCapSmem[tier], kCtCapSpill[tier], tr->ct_spill.p);
+        else k_construct<kCtWarpsWide><<<grid, ct_threads(kCtWarpsWide), ct_smem_bytes(tier), st>>>(v, c, kCtCapSmem[tier], kCtCapSpill[tier], tr->ct_spill.p);
+        L++;
     }
     mark(4);
     // K6: claims + owned counts per (task, chunk) in shared memory, keep flags, scans, output
@@ -602,13 +607,17 @@ tpc_tracker* tpc_tracker_create_ex(const tpc_geometry* g, float bz, const tpc_pa
         int per_sm = 0;
         size_t most = 0;
         for (int k = 0; k < kCtTiers; k++) most = std::max(most, ct_smem_bytes(k));
-        if (cudaFuncSetAttribute(k_construct, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)most) != cudaSuccess) {
+        if (cudaFuncSetAttribute(k_construct<kCtWarps>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ct_smem_bytes(0)) != cudaSuccess ||
+            cudaFuncSetAttribute(k_construct<kCtWarpsWide>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)most) != cudaSuccess) {
             set_err("k_construct: %zu bytes of shared memory cannot be configured: %s", most, cudaGetErrorString(cudaGetLastError()));
             delete t;
             return nullptr;
         }
         for (int k = 0; k < kCtTiers; k++) {
-            if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_construct, kCtThreads, ct_smem_bytes(k)) != cudaSuccess || per_sm < 1) {
+            const cudaError_t e = k == 0
+                ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_construct<kCtWarps>, ct_threads(kCtWarps), ct_smem_bytes(k))
+                : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_construct<kCtWarpsWide>, ct_threads(kCtWarpsWide), ct_smem_bytes(k));
+            if (e != cudaSuccess || per_sm < 1) {
                 set_err("k_construct cannot be configured: %s", cudaGetErrorString(cudaGetLastError()));
                 delete t;
                 return nullptr;
@@ -783,8 +792,8 @@ int tpc_submit_events(tpc_tracker* t, int32_t n, const tpc_event_in* in, int32_t
     if (rc != TPC_OK) return rc;
     if (!ticket) { set_err("null ticket"); return TPC_ERR_ARG; }
     int k = -1;
-    for (int j = 0; j < 2; j++) if (!t->async[j].busy) { k = j; break; }
-    if (k < 0) { set_err("two batches are in flight: wait for one first"); return TPC_ERR_ARG; }
+    for (int j = 0; j < kAsync; j++) if (!t->async[j].busy) { k = j; break; }
+    if (k < 0) { set_err("%d batches are in flight: wait for one first", kAsync); return TPC_ERR_ARG; }
     tpc_tracker::Async& a = t->async[k];
     if (!a.b) {
         cudaStream_t s = nullptr;
@@ -793,19 +802,23 @@ int tpc_submit_events(tpc_tracker* t, int32_t n, const tpc_event_in* in, int32_t
         a.b->stream = s;
         if (cudaEventCreateWithFlags(&a.b->kernels_done, cudaEventDisableTiming) != cudaSuccess) { set_err("cudaEventCreate failed"); return TPC_ERR_CUDA; }
     }
-    // copy-in | kernels | copy-out pipeline: the kernels of this batch queue behind those of the batch in flight, so
-    // that two batches never share the SMs; only the copies run beside the other batch's kernels
-    tpc_tracker::Async& o = t->async[1 - k];
-    a.b->wait_for = (o.busy && o.b) ? o.b->kernels_done : nullptr;
+    // copy-in | kernels | copy-out pipeline: the kernels of this batch queue behind those of the batch submitted before
+    // it, so that two batches never share the SMs; only the copies run beside another batch's kernels
+    a.b->wait_for = nullptr;
+    if (t->last_ticket >= 0 && t->last_ticket != k) {
+        tpc_tracker::Async& o = t->async[t->last_ticket];
+        if (o.busy && o.b) a.b->wait_for = o.b->kernels_done;
+    }
     memset(&a.b->counters, 0, sizeof(tpc_counters));
     if ((rc = batch_begin(t, a.b, 0, n, in, 0, true)) != TPC_OK) { cudaStreamSynchronize(a.b->stream); return rc; }
     a.busy = true;
+    t->last_ticket = k;
     *ticket = k;
     return TPC_OK;
 }
 
 int tpc_wait_events(tpc_tracker* t, int32_t ticket, tpc_event_out* out) {
-    if (!t || !out || ticket < 0 || ticket > 1 || !t->async[ticket].busy) { set_err("no batch in flight under this ticket"); return TPC_ERR_ARG; }
+    if (!t || !out || ticket < 0 || ticket >= kAsync || !t->async[ticket].busy) { set_err("no batch in flight under this ticket"); return TPC_ERR_ARG; }
     tpc_tracker::Async& a = t->async[ticket];
     Batch* b = a.b;
     a.busy = false;

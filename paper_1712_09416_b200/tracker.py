@@ -226,7 +226,7 @@ class Tracker:
         return self.tpc_track_events([event])[0]
 
     def tpc_submit_events(self, events) -> int:
-        """Enqueue a batch (copies in + all kernels) and return its ticket; at most two batches in flight.  The
+        """Enqueue a batch (copies in + all kernels) and return its ticket; at most three batches in flight.  The
         events' arrays must stay unchanged until ``tpc_wait_events(ticket)`` returns."""
         n = len(events)
         ins, keep = self._marshal(events)

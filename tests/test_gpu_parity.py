@@ -454,8 +454,8 @@ def test_parity_other_row_counts(trk_mod, gen_mod, oracle_mod, n_rows):
 
 @pytest.mark.parametrize("device", [True, False])
 def test_submit_wait_gives_what_the_sync_call_gives(trk_mod, gen_mod, oracle_mod, device):
-    """tpc_submit_events / tpc_wait_events: two batches in flight, results those of tpc_track_events (refit and
-    merge on); a third submit and a wait on an idle ticket are refused."""
+    """tpc_submit_events / tpc_wait_events: three batches in flight, results those of tpc_track_events (refit and
+    merge on); a fourth submit and a wait on an idle ticket are refused."""
     p = oracle_mod.default_params()
     p.refit = 1; p.merge = 1
     batches = [[gen_mod.generate("pp", 0), gen_mod.generate("semicentral", 0)],
@@ -466,13 +466,14 @@ def test_submit_wait_gives_what_the_sync_call_gives(trk_mod, gen_mod, oracle_mod
     dicts = [[ev_dict(ev, device) for ev in b] for b in batches]
     t0 = trk.tpc_submit_events(dicts[0])
     t1 = trk.tpc_submit_events(dicts[1])
-    assert {t0, t1} == {0, 1}
+    t2 = trk.tpc_submit_events(dicts[2])
+    assert {t0, t1, t2} == {0, 1, 2}
     with pytest.raises(trk_mod.TpcError):
-        trk.tpc_submit_events(dicts[2])               # two in flight already
+        trk.tpc_submit_events(dicts[3])               # three in flight already
     got = {0: [trk.to_numpy(o) for o in trk.tpc_wait_events(t0)]}
-    t2 = trk.tpc_submit_events(dicts[2])               # the freed ticket is handed out again
+    t3 = trk.tpc_submit_events(dicts[3])               # the freed ticket is handed out again
+    assert t3 == t0
     got[1] = [trk.to_numpy(o) for o in trk.tpc_wait_events(t1)]
-    t3 = trk.tpc_submit_events(dicts[3])
     got[2] = [trk.to_numpy(o) for o in trk.tpc_wait_events(t2)]
     got[3] = [trk.to_numpy(o) for o in trk.tpc_wait_events(t3)]
     for k, b in enumerate(batches):
