@@ -105,11 +105,18 @@ class ClockSampler(threading.Thread):
         return {"sm_mhz": float(np.median(self.samples)), "sm_max_mhz": self.max_mhz, "reasons": sorted(self.reasons)}
 
 
-def make_events(workload, n_events):
+def event_seeds(workload, n_events, rank=0):
+    """Seeds of the events rank `rank` tracks: replicas only -- every rank has its OWN batch
+    of n_events events, disjoint from the other ranks'; rank 0's batch is the single-GPU batch."""
     from paper_1712_09416_b200 import gen
     recipe = gen.RECIPES[workload]
     base = 1000 * gen.RECIPES["central_batch16"].config_id if workload == "central" else 1000 * recipe.config_id
-    return [gen.generate(recipe, seed=base + e) for e in range(n_events)]
+    return [base + rank * n_events + e for e in range(n_events)]
+
+
+def make_events(workload, n_events, rank=0):
+    from paper_1712_09416_b200 import gen
+    return [gen.generate(gen.RECIPES[workload], seed=s) for s in event_seeds(workload, n_events, rank)]
 
 
 def stage_bytes(c):
@@ -264,7 +271,7 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     from paper_1712_09416_b200 import gen, tracker
 
-    evs = make_events(args.workload, args.events)
+    evs = make_events(args.workload, args.events, rank)
     n_total = sum(ev.n_clusters for ev in evs)
     rx = gen.row_x().astype(np.float32)
     params = None
