@@ -84,43 +84,60 @@ __global__ void __launch_bounds__(256) k_count(const View v, const __grid_consta
     }
 }
 
-// K1b: move (y, z, index) into the bin, arrival order.
+// K1b: move (y, z, index) into the bin, arrival order.  kScatterPer clusters per thread, all loads of a thread
+// issued before the first dependent one (the kernel waits on memory latency, not on bandwidth).
+constexpr int kScatterPer = 4;
+constexpr int kScatterChunk = 256 * kScatterPer;
+
 __global__ void __launch_bounds__(256) k_scatter(const View v, int ns, int nr) {
     __shared__ int32_t so[64 + 1];
     const int e = blockIdx.y;
     const EventSrc src = v.ev[e];
-    if (blockIdx.x * 256 >= src.n) return;
+    const int i0 = blockIdx.x * kScatterChunk;
+    if (i0 >= src.n) return;
     for (int k = threadIdx.x; k <= ns; k += 256) so[k] = v.sec_off[e * (ns + 1) + k];
+    int r[kScatterPer], sl[kScatterPer];
+    float2 h[kScatterPer];
+#pragma unroll
+    for (int j = 0; j < kScatterPer; j++) {
+        const int i = i0 + j * 256 + threadIdx.x;
+        r[j] = -1; sl[j] = 0; h[j] = make_float2(0.f, 0.f);
+        if (i < src.n) {
+            r[j] = src.row[i]; sl[j] = v.slot[src.off + i];
+            h[j] = make_float2(src.y[i], src.z[i]);
+        }
+    }
     __syncthreads();
-    const int i = blockIdx.x * 256 + threadIdx.x;
-    if (i >= src.n) return;
-    const int r = src.row[i];
-    if (r < 0 || r >= nr) return;
-    const int s = sector_of(so, ns, i);
-    const int bin = (e * ns + s) * nr + r;
-    const int sl = v.slot[src.off + i];
-    if (sl >= TPC_MAX_ROW_HITS) return;
-    const int pos = v.bin_start[bin] + sl;
-    v.thit[pos] = make_float2(src.y[i], src.z[i]);
-    v.tidx[pos] = i;
+    int pos[kScatterPer];
+#pragma unroll
+    for (int j = 0; j < kScatterPer; j++) {
+        const int i = i0 + j * 256 + threadIdx.x;
+        pos[j] = -1;
+        if (r[j] >= 0 && r[j] < nr && sl[j] < TPC_MAX_ROW_HITS)
+            pos[j] = __ldg(&v.bin_start[(e * ns + sector_of(so, ns, i)) * nr + r[j]]) + sl[j];
+    }
+#pragma unroll
+    for (int j = 0; j < kScatterPer; j++)
+        if (pos[j] >= 0) { v.thit[pos[j]] = h[j]; v.tidx[pos[j]] = i0 + j * 256 + (int)threadIdx.x; }
 }
 
 // ---------------------------------------------------------------------------------------------------------
 // K1c: one CTA per bin: bounding box -> grid dims -> counting sort of the bin by grid cell -> cell table.
 // The grid only accelerates the window searches; windows are defined on coordinates and every tie is broken
 // on the caller's index, so neither the grid's shape nor the order inside a cell changes a result.
+// A bin of up to kSortReg * kSortThreads hits (every pad row of a central event) is read ONCE, into registers.
 // ---------------------------------------------------------------------------------------------------------
 #ifndef TPC_SORT_THREADS
 #define TPC_SORT_THREADS 128
 #endif
 constexpr int kSortThreads = TPC_SORT_THREADS;
+constexpr int kSortReg = 4;
 
 __global__ void __launch_bounds__(kSortThreads) k_sort_row(const View v) {
     __shared__ int cnt[kMaxCells + 1];                    // hits per cell, then first hit of each cell
-    __shared__ uint16_t ck[TPC_MAX_ROW_HITS];             // cell of hit k
+    __shared__ uint16_t ck[TPC_MAX_ROW_HITS];             // cell of hit k       } larger bins only
     __shared__ uint16_t rk[TPC_MAX_ROW_HITS];             // arrival rank of hit k inside its cell
     __shared__ float red[4][kSortThreads / 32];
-    __shared__ float box[4];
     __shared__ int scan_total;
     const int bin = blockIdx.x;
     const int b0 = v.bin_start[bin];
@@ -134,11 +151,27 @@ __global__ void __launch_bounds__(kSortThreads) k_sort_row(const View v) {
         }
         return;
     }
+    const bool small = n <= kSortReg * kSortThreads;
+    float2 hr[kSortReg];
+    int ir[kSortReg];
     // bounding box
     float ymin = 3.0e38f, ymax = -3.0e38f, zmin = 3.0e38f, zmax = -3.0e38f;
-    for (int k = threadIdx.x; k < n; k += kSortThreads) {
-        const float2 h = v.thit[b0 + k];
-        ymin = fminf(ymin, h.x); ymax = fmaxf(ymax, h.x); zmin = fminf(zmin, h.y); zmax = fmaxf(zmax, h.y);
+    if (small) {
+#pragma unroll
+        for (int j = 0; j < kSortReg; j++) {
+            const int k = j * kSortThreads + threadIdx.x;
+            if (k < n) { hr[j] = v.thit[b0 + k]; ir[j] = v.tidx[b0 + k]; }
+        }
+#pragma unroll
+        for (int j = 0; j < kSortReg; j++)
+            if (j * kSortThreads + (int)threadIdx.x < n) {
+                ymin = fminf(ymin, hr[j].x); ymax = fmaxf(ymax, hr[j].x); zmin = fminf(zmin, hr[j].y); zmax = fmaxf(zmax, hr[j].y);
+            }
+    } else {
+        for (int k = threadIdx.x; k < n; k += kSortThreads) {
+            const float2 h = v.thit[b0 + k];
+            ymin = fminf(ymin, h.x); ymax = fmaxf(ymax, h.x); zmin = fminf(zmin, h.y); zmax = fmaxf(zmax, h.y);
+        }
     }
 #pragma unroll
     for (int o = 16; o > 0; o >>= 1) {
@@ -150,15 +183,11 @@ __global__ void __launch_bounds__(kSortThreads) k_sort_row(const View v) {
         red[0][w] = ymin; red[1][w] = ymax; red[2][w] = zmin; red[3][w] = zmax;
     }
     __syncthreads();
-    if (threadIdx.x == 0) {
-        for (int w = 1; w < kSortThreads / 32; w++) {
-            ymin = fminf(ymin, red[0][w]); ymax = fmaxf(ymax, red[1][w]);
-            zmin = fminf(zmin, red[2][w]); zmax = fmaxf(zmax, red[3][w]);
-        }
-        box[0] = ymin; box[1] = ymax; box[2] = zmin; box[3] = zmax;
+#pragma unroll
+    for (int w = 0; w < kSortThreads / 32; w++) {   // min / max: the same value in every thread, whatever the order
+        ymin = fminf(ymin, red[0][w]); ymax = fmaxf(ymax, red[1][w]);
+        zmin = fminf(zmin, red[2][w]); zmax = fmaxf(zmax, red[3][w]);
     }
-    __syncthreads();
-    ymin = box[0]; ymax = box[1]; zmin = box[2]; zmax = box[3];
     // grid dims: cells of about one hit's area, ~0.6 : 1/0.6 in (y : z), then kCellsPerHit times finer in y (the
     // hits of the cells iy0..iy1 of one grid row are contiguous, so fine y cells cost no extra range), never finer
     // than 0.35 x 1.2 cm
@@ -174,11 +203,21 @@ __global__ void __launch_bounds__(kSortThreads) k_sort_row(const View v) {
     const int ncell = ny * nz;
     for (int q = threadIdx.x; q <= ncell; q += kSortThreads) cnt[q] = 0;
     __syncthreads();
-    for (int k = threadIdx.x; k < n; k += kSortThreads) {
-        const float2 h = v.thit[b0 + k];
-        const int cell = grid_cell(h.y, zmin, idz, nz) * ny + grid_cell(h.x, ymin, idy, ny);
-        ck[k] = (uint16_t)cell;
-        rk[k] = (uint16_t)atomicAdd(&cnt[cell], 1);
+    int ckr[kSortReg], rkr[kSortReg];
+    if (small) {
+#pragma unroll
+        for (int j = 0; j < kSortReg; j++)
+            if (j * kSortThreads + (int)threadIdx.x < n) {
+                ckr[j] = grid_cell(hr[j].y, zmin, idz, nz) * ny + grid_cell(hr[j].x, ymin, idy, ny);
+                rkr[j] = atomicAdd(&cnt[ckr[j]], 1);
+            }
+    } else {
+        for (int k = threadIdx.x; k < n; k += kSortThreads) {
+            const float2 h = v.thit[b0 + k];
+            const int cell = grid_cell(h.y, zmin, idz, nz) * ny + grid_cell(h.x, ymin, idy, ny);
+            ck[k] = (uint16_t)cell;
+            rk[k] = (uint16_t)atomicAdd(&cnt[cell], 1);
+        }
     }
     __syncthreads();
     // exclusive scan of cnt[0..ncell): each thread owns a contiguous chunk
@@ -192,10 +231,20 @@ __global__ void __launch_bounds__(kSortThreads) k_sort_row(const View v) {
     }
     __syncthreads();
     for (int q = threadIdx.x; q <= ncell; q += kSortThreads) cs[q] = (uint16_t)(q < ncell ? cnt[q] : n);
-    for (int k = threadIdx.x; k < n; k += kSortThreads) {
-        const int pos = b0 + cnt[ck[k]] + rk[k];
-        v.shit[pos] = v.thit[b0 + k];
-        v.sorig[pos] = v.tidx[b0 + k];
+    if (small) {
+#pragma unroll
+        for (int j = 0; j < kSortReg; j++)
+            if (j * kSortThreads + (int)threadIdx.x < n) {
+                const int pos = b0 + cnt[ckr[j]] + rkr[j];
+                v.shit[pos] = hr[j];
+                v.sorig[pos] = ir[j];
+            }
+    } else {
+        for (int k = threadIdx.x; k < n; k += kSortThreads) {
+            const int pos = b0 + cnt[ck[k]] + rk[k];
+            v.shit[pos] = v.thit[b0 + k];
+            v.sorig[pos] = v.tidx[b0 + k];
+        }
     }
     if (threadIdx.x == 0) {
         BinDesc d; d.y0 = ymin; d.z0 = zmin; d.idy = idy; d.idz = idz; d.base = b0; d.n = n; d.ny = ny; d.nz = nz;
@@ -218,13 +267,12 @@ constexpr int kNfThreads = 128;
 #define TPC_NF_BLOCKS 12
 #endif
 constexpr int kNfCap = TPC_NF_CAP;   // hits of a neighbour row held in shared memory; larger rows are read in place
-constexpr int kNfList = 8;     // down-candidates remembered per hit; more -> nested walk
+constexpr int kNfReg = 4;      // candidates of a window remembered per hit (in a register); more -> nested walk
 
 __global__ void __launch_bounds__(kNfThreads, TPC_NF_BLOCKS) k_neighbours(const View v, const __grid_constant__ Const c) {
     __shared__ float2 s_hu[kNfCap], s_hd[kNfCap];
     constexpr int kNfCells = kCellsPerHit * kNfCap + kCellPad;   // cell-table entries held in shared memory
     __shared__ uint16_t s_cu[kNfCells], s_cd[kNfCells];
-    __shared__ uint16_t s_dl[kNfList][kNfThreads];
     TPC_RETURN_IF_REJECTED(v);
     const int bin = blockIdx.x;
     const int nr = c.n_rows, D = c.p.link_step;
@@ -280,38 +328,59 @@ __global__ void __launch_bounds__(kNfThreads, TPC_NF_BLOCKS) k_neighbours(const 
             }
             if (take) { best = dev; bpair = (u << 16) | d; }
         };
-        // down-candidates inside the window, remembered
+        // The candidates inside the two windows are first collected -- up to kNfReg of each side as 16-bit
+        // row-local indices packed into a 64-bit register -- and the pairs are then evaluated in ONE flat loop: a
+        // warp's trip count is its largest pair count, not the sum over nested loops with diverging trip counts.
         const CellWin wd = cell_window(gfd, nyd, dd.w, y0, z0, wyd, wzd);
-        int nd = 0;
+        unsigned long long ld = 0ull, lu = 0ull;
+        int nd = 0, nu = 0;
         for (int iz = wd.iz0; iz <= wd.iz1; iz++) {
             int p = cd[iz * nyd + wd.iy0];
             const int pe = cd[iz * nyd + wd.iy1 + 1];
             for (; p < pe; p++) {
                 const float2 pd = hd[p];
                 if (fabsf(pd.x - y0) <= wyd && fabsf(pd.y - z0) <= wzd) {
-                    if (nd < kNfList) s_dl[nd][threadIdx.x] = (uint16_t)p;
+                    if (nd < kNfReg) ld |= (unsigned long long)p << (16 * nd);
                     nd++;
                 }
             }
         }
+        CellWin wu = wd;
         if (nd > 0) {
-            const CellWin wu = cell_window(gfu, nyu, du.w, y0, z0, wyu, wzu);
+            wu = cell_window(gfu, nyu, du.w, y0, z0, wyu, wzu);
+            for (int iz = wu.iz0; iz <= wu.iz1; iz++) {
+                int p = cu[iz * nyu + wu.iy0];
+                const int pe = cu[iz * nyu + wu.iy1 + 1];
+                for (; p < pe; p++) {
+                    const float2 pu = hu[p];
+                    if (fabsf(pu.x - y0) <= wyu && fabsf(pu.y - z0) <= wzu) {
+                        if (nu < kNfReg) lu |= (unsigned long long)p << (16 * nu);
+                        nu++;
+                    }
+                }
+            }
+        }
+        if (nd <= kNfReg && nu <= kNfReg) {
+            const int np = nd * nu;
+            int ju = 0, jd = 0;
+            for (int q = 0; q < np; q++) {
+                const int u = (int)(lu >> (16 * ju)) & 0xffff, d = (int)(ld >> (16 * jd)) & 0xffff;
+                eval(u, hu[u], d, hd[d]);
+                if (++jd == nd) { jd = 0; ju++; }
+            }
+        } else if (nu > 0) {   // a crowded window: walk both again, nested
             for (int iz = wu.iz0; iz <= wu.iz1; iz++) {
                 int p = cu[iz * nyu + wu.iy0];
                 const int pe = cu[iz * nyu + wu.iy1 + 1];
                 for (; p < pe; p++) {
                     const float2 pu = hu[p];
                     if (!(fabsf(pu.x - y0) <= wyu && fabsf(pu.y - z0) <= wzu)) continue;
-                    if (nd <= kNfList) {
-                        for (int j = 0; j < nd; j++) { const int d = s_dl[j][threadIdx.x]; eval(p, pu, d, hd[d]); }
-                    } else {
-                        for (int jz = wd.iz0; jz <= wd.iz1; jz++) {
-                            int q = cd[jz * nyd + wd.iy0];
-                            const int qe = cd[jz * nyd + wd.iy1 + 1];
-                            for (; q < qe; q++) {
-                                const float2 pd = hd[q];
-                                if (fabsf(pd.x - y0) <= wyd && fabsf(pd.y - z0) <= wzd) eval(p, pu, q, pd);
-                            }
+                    for (int jz = wd.iz0; jz <= wd.iz1; jz++) {
+                        int q = cd[jz * nyd + wd.iy0];
+                        const int qe = cd[jz * nyd + wd.iy1 + 1];
+                        for (; q < qe; q++) {
+                            const float2 pd = hd[q];
+                            if (fabsf(pd.x - y0) <= wyd && fabsf(pd.y - z0) <= wzd) eval(p, pu, q, pd);
                         }
                     }
                 }

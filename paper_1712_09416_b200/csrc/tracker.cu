@@ -300,7 +300,7 @@ int launch_all(const tpc_tracker* tr, Batch* t, int from = 1) {
         }
         L += scan_exclusive(v.bin_count, v.bin_start, nb, t->scratch.p, st);
         if (maxn > 0) {
-            dim3 g((maxn + 255) / 256, t->n_events);
+            dim3 g((maxn + kScatterChunk - 1) / kScatterChunk, t->n_events);
             k_scatter<<<g, 256, 0, st>>>(v, ns, nr); L++;
         }
         k_sort_row<<<nb, kSortThreads, 0, st>>>(v); L++;
