@@ -27,6 +27,9 @@ namespace tpc {
 #ifndef TPC_CT_WARPS
 #define TPC_CT_WARPS 9
 #endif
+#ifndef TPC_CT_MINB
+#define TPC_CT_MINB 2
+#endif
 #ifndef TPC_CT_RING
 #define TPC_CT_RING 3
 #endif
@@ -48,10 +51,16 @@ constexpr int kCtTiers = 3;
 #ifndef TPC_CT_CAP0
 #define TPC_CT_CAP0 512
 #endif
+#ifndef TPC_CT_SPILL0
+#define TPC_CT_SPILL0 0
+#endif
 constexpr int kCtCapSmem[kCtTiers] = {TPC_CT_CAP0, 1408, 1280};   // tier 0: two CTAs per SM; tiers 1, 2: one
-constexpr int kCtCapSpill[kCtTiers] = {0, 0, 4096};
+constexpr int kCtCapSpill[kCtTiers] = {TPC_CT_SPILL0, 0, 4096};
 constexpr int kCtCapMax = 1280 + 4096;
-constexpr int kSwCap = 640;                            // hits of a row staged in shared memory; larger rows are read in place
+#ifndef TPC_SW_CAP
+#define TPC_SW_CAP 640
+#endif
+constexpr int kSwCap = TPC_SW_CAP;                            // hits of a row staged in shared memory; larger rows are read in place
 constexpr int kSwHitBytes = (kSwCap + 2) * 8;          // + alignment slack of the bulk copy (16-byte granules)
 constexpr int kSwCellEntries = kCellsPerHit * kSwCap + kCellPad + 16;
 constexpr int kSwCellBytes = kSwCellEntries * 2;
@@ -66,20 +75,25 @@ struct __align__(16) SeedRec { float y0, z0, s, t; int32_t h0, h1, h2, pad; };
 // entry of the row below the top hit, the tracklet
 struct __align__(16) UpRec { float y, z, s, t, q; int32_t rows, below, id; };
 
+#ifndef TPC_CT_ROWS
+#define TPC_CT_ROWS (TPC_MAX_ROWS + 1)
+#endif
+constexpr int kCtRows = TPC_CT_ROWS;
 struct __align__(128) CtSmem {
-    BinDesc desc[TPC_MAX_ROWS + 1];                    // the task's row descriptors
+    BinDesc desc[kCtRows];                    // the task's row descriptors
     unsigned char hits[kCtRing][kSwHitBytes];
     unsigned char cells[kCtRing][kSwCellBytes];
     SeedRec seeds[kCtRing][kCtSeedStage > 0 ? kCtSeedStage : 1];              // the first records of what starts at the row: start hits (up
                                                        // sweep), parked tracklets with their top hit there (down sweep)
-    int32_t lo[TPC_MAX_ROWS + 1];                      // up sweep: first start hit of each row in the canonical list;
-    int32_t cnt[TPC_MAX_ROWS + 1];                     // start hits of the row.  Down sweep: the same for the parked tracklets
-    int32_t dcnt[TPC_MAX_ROWS + 1];                    // tracklets parked with their top hit in each row
+    int32_t lo[kCtRows];                      // up sweep: first start hit of each row in the canonical list;
+    int32_t cnt[kCtRows];                     // start hits of the row.  Down sweep: the same for the parked tracklets
+    int32_t dcnt[kCtRows];                    // tracklets parked with their top hit in each row
     uint32_t used[2][TPC_MAX_ROW_HITS / 32];           // hits of the row at hand recorded by an up pass (double buffered)
     uint32_t occ[(kCtCapMax + 31) / 32];               // occupied state slots
     unsigned long long full[kCtRing], empty[kCtRing], tbar;
     int32_t cmd[kCtRing];                              // row held by the ring slot (| kCtDown); -1 = no more work
     int32_t task, abort, n_free, n_hw, n_parked, top_max, i0;   // n_hw: highest slot used so far + 1
+    uint32_t n_visits[20], n_updates[20], n_built, n_done;   // this CTA's share of the run's counters (per consumer warp)
 };
 
 // ---- mbarrier / bulk-copy wrappers (PTX ISA: mbarrier, cp.async.bulk) ----
@@ -194,7 +208,7 @@ __device__ __forceinline__ void ct_producer(const View& v, const Const& c, CtSme
             if (n > 0) f = min(f, r);
         }
         for (int k = lane; k < 2 * (TPC_MAX_ROW_HITS / 32); k += 32) (&sm.used[0][0])[k] = 0u;
-        for (int r = lane; r <= TPC_MAX_ROWS; r += 32) sm.dcnt[r] = 0;
+        for (int r = lane; r < kCtRows; r += 32) sm.dcnt[r] = 0;
         reset_slots();
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) f = min(f, __shfl_xor_sync(kFull, f, o));
@@ -277,7 +291,9 @@ __device__ __forceinline__ int sweep_search(const View& v, const Const& c, const
 // ---- a tracklet's state in its shared-memory slot: word k of slot s sits at st[k * cap + s] ----
 struct CtTrk {
     Fit f;
-    float p0, p1, p2, p3, p4, p5;   // state right after the last accepted update (up: p5 = two table entries, see step)
+    float p5;                       // up: two table entries (see the row step).  The state right after the last accepted
+                                    // update (words 22..27 of the slot) is written there at an update and read at the end
+                                    // of the pass only: it never sits in registers across the Kalman arithmetic
     int i;                          // tracklet = canonical start-hit number (batch-global)
     int cur;                        // up: the linked hit to come; down: table entry of the row below (read one row ahead)
     int nxt;                        // up: the hit linked above cur (read one link ahead)
@@ -290,7 +306,7 @@ __device__ __forceinline__ void ct_load(CtTrk& t, const float* S, int cap) {
     f.c22 = S[10 * cap]; f.c30 = S[11 * cap]; f.c31 = S[12 * cap]; f.c32 = S[13 * cap]; f.c33 = S[14 * cap];
     f.c40 = S[15 * cap]; f.c41 = S[16 * cap]; f.c42 = S[17 * cap]; f.c43 = S[18 * cap]; f.c44 = S[19 * cap];
     f.chi2 = S[20 * cap]; f.n = __float_as_int(S[21 * cap]);
-    t.p0 = S[22 * cap]; t.p1 = S[23 * cap]; t.p2 = S[24 * cap]; t.p3 = S[25 * cap]; t.p4 = S[26 * cap]; t.p5 = S[27 * cap];
+    t.p5 = S[27 * cap];
     t.i = __float_as_int(S[28 * cap]); t.cur = __float_as_int(S[29 * cap]); t.nxt = __float_as_int(S[31 * cap]);
     const uint32_t pk = __float_as_uint(S[30 * cap]);
     t.ph = pk & 3u; t.miss = (pk >> 2) & 63u; t.r0 = (pk >> 8) & 255u; t.top = (pk >> 16) & 255u; t.aux = pk >> 24;
@@ -302,7 +318,7 @@ __device__ __forceinline__ void ct_store(const CtTrk& t, float* S, int cap) {
     S[10 * cap] = f.c22; S[11 * cap] = f.c30; S[12 * cap] = f.c31; S[13 * cap] = f.c32; S[14 * cap] = f.c33;
     S[15 * cap] = f.c40; S[16 * cap] = f.c41; S[17 * cap] = f.c42; S[18 * cap] = f.c43; S[19 * cap] = f.c44;
     S[20 * cap] = f.chi2; S[21 * cap] = __int_as_float(f.n);
-    S[22 * cap] = t.p0; S[23 * cap] = t.p1; S[24 * cap] = t.p2; S[25 * cap] = t.p3; S[26 * cap] = t.p4; S[27 * cap] = t.p5;
+    S[27 * cap] = t.p5;
     S[28 * cap] = __int_as_float(t.i); S[29 * cap] = __int_as_float(t.cur); S[31 * cap] = __int_as_float(t.nxt);
     S[30 * cap] = __uint_as_float((uint32_t)t.ph | ((uint32_t)t.miss << 2) | ((uint32_t)t.r0 << 8) |
                                   ((uint32_t)t.top << 16) | ((uint32_t)t.aux << 24));
@@ -310,13 +326,19 @@ __device__ __forceinline__ void ct_store(const CtTrk& t, float* S, int cap) {
 
 // slot -> where its state lives: the first cap_s slots in shared memory, the others in this CTA's stretch of
 // global memory (both multiples of 32, so a warp's 32 slots are all of one kind)
+template <bool G>   // G: the tier has slots in global memory
 struct CtSlots {
     float* st; float* gs; int cap_s, cap_g;
     __device__ __forceinline__ void load(CtTrk& t, int slot) const {
-        if (slot < cap_s) ct_load(t, st + slot, cap_s); else ct_load(t, gs + (slot - cap_s), cap_g);
+        if (!G || slot < cap_s) ct_load(t, st + slot, cap_s); else ct_load(t, gs + (slot - cap_s), cap_g);
     }
     __device__ __forceinline__ void store(const CtTrk& t, int slot) const {
-        if (slot < cap_s) ct_store(t, st + slot, cap_s); else ct_store(t, gs + (slot - cap_s), cap_g);
+        if (!G || slot < cap_s) ct_store(t, st + slot, cap_s); else ct_store(t, gs + (slot - cap_s), cap_g);
+    }
+    // words 22.. of a slot: the state right after the last accepted update
+    __device__ __forceinline__ float* snap(int slot, int& stride) const {
+        if (!G || slot < cap_s) { stride = cap_s; return st + slot + 22 * cap_s; }
+        stride = cap_g; return gs + (slot - cap_s) + 22 * cap_g;
     }
 };
 
@@ -343,8 +365,8 @@ __device__ __forceinline__ void ct_push(CtSmem& sm, uint16_t* freel, int slot, i
 // ---- intake, by all consumer threads between the row steps ----
 // down sweep: the parked tracklets whose top hit is in this row start a fresh fit there (their records come
 // ordered by top row: staged in the ring slot, the ones beyond kCtSeedStage read in place)
-template <int W>
-__device__ TPC_CT_INL void ct_intake_down(const View& v, const Const& c, CtSmem& sm, const CtSlots& sl, const uint16_t* freel,
+template <int W, bool G>
+__device__ TPC_CT_INL void ct_intake_down(const View& v, const Const& c, CtSmem& sm, const CtSlots<G>& sl, const uint16_t* freel,
                                             int cap, int row, int s) {
     const int n = sm.cnt[row], lo = sm.i0 + sm.lo[row];
     for (int j0 = 0; j0 < n; j0 += W * 32) {
@@ -360,25 +382,26 @@ __device__ TPC_CT_INL void ct_intake_down(const View& v, const Const& c, CtSmem&
                 b4 = __ldcg(reinterpret_cast<const float4*>(&v.dn_rec[lo + j]) + 1);
             }
             CtTrk t;
-            t.p0 = a4.x; t.p1 = a4.y; t.p2 = a4.z; t.p3 = a4.w; t.p4 = b4.x; t.p5 = 0.f;
+            t.p5 = 0.f;
             t.r0 = __float_as_int(b4.y) & 0xff; t.top = row; t.i = __float_as_int(b4.w);
-            t.f.y = t.p0; t.f.z = t.p1; t.f.s = t.p2; t.f.t = t.p3; t.f.q = t.p4;
+            t.f.y = a4.x; t.f.z = a4.y; t.f.s = a4.z; t.f.t = a4.w; t.f.q = b4.x;
             fit_prior(t.f, c); t.f.n = 1;
             t.aux = row; t.miss = 0; t.ph = 3; t.nxt = -1;
             t.cur = __float_as_int(b4.z);             // table entry of the row below the top hit
             sl.store(t, slot);
+            int sn; float* const P = sl.snap(slot, sn);
+            P[0] = a4.x; P[sn] = a4.y; P[2 * sn] = a4.z; P[3 * sn] = a4.w; P[4 * sn] = b4.x;
         }
     }
 }
 // up sweep: the start hits of this row that no up pass has recorded build a tracklet; returns how many (this thread)
-template <int W>
-__device__ TPC_CT_INL unsigned ct_intake_up(const View& v, const Const& c, CtSmem& sm, const CtSlots& sl, const uint16_t* freel,
+template <int W, bool G>
+__device__ TPC_CT_INL void ct_intake_up(const View& v, const Const& c, CtSmem& sm, const CtSlots<G>& sl, const uint16_t* freel,
                                               int cap, int row, int s, int S) {
     const int D = c.p.link_step;
     const bool dedup = c.p.seed_dedup != 0;
     const int n = sm.cnt[row], lo = sm.lo[row], base = sm.desc[row].base;
     const uint32_t* const ub = sm.used[row & 1];
-    unsigned built = 0;
     for (int j0 = 0; j0 < n; j0 += W * 32) {
         const int j = j0 + (int)threadIdx.x, e = lo + j;
         bool need = false;
@@ -400,19 +423,19 @@ __device__ TPC_CT_INL unsigned ct_intake_up(const View& v, const Const& c, CtSme
         const int slot = ct_pop(v, sm, freel, need, cap);
         if (need && slot < 0) v.tl_rows[e] = 0;
         if (slot >= 0) {
-            built++;
+            atomicAdd(&sm.n_built, 1u);
             CtTrk t;
             Fit& f = t.f;
             f.y = a4.x; f.z = a4.y; f.s = a4.z; f.t = a4.w; f.q = 0.f;   // direction of the first link, from K4
             fit_prior(f, c); f.n = 0;
-            t.p0 = a4.x; t.p1 = a4.y; t.p2 = f.s; t.p3 = f.t; t.p4 = f.q;
             t.p5 = __uint_as_float(((uint32_t)kNoHit << 16) | (uint32_t)hl);   // table entries: below the top hit | of the row before
             t.i = e; t.cur = hh.y; t.nxt = hh.z; t.ph = 1; t.miss = 0; t.r0 = row; t.top = row; t.aux = row + D;
             v.tl_tab[(size_t)e * v.tab_stride + row] = (uint16_t)hl;
             sl.store(t, slot);
+            int sn; float* const P = sl.snap(slot, sn);
+            P[0] = a4.x; P[sn] = a4.y; P[2 * sn] = a4.z; P[3 * sn] = a4.w; P[4 * sn] = 0.f;
         }
     }
-    return built;
 }
 // between the sweeps (all consumer warps): the parked tracklets of the task, ordered by top row, into dn_rec
 template <int W>
@@ -449,14 +472,19 @@ __device__ TPC_CT_INL void ct_turn(const View& v, CtSmem& sm, int nr) {
 // ---------------------------------------------------------------------------------------------------------
 // K5
 // ---------------------------------------------------------------------------------------------------------
-template <int W>
-__global__ void __launch_bounds__((W + 1) * 32, W <= 10 ? 2 : 1) k_construct(const __grid_constant__ View v, const __grid_constant__ Const c, const int cap_s,
+template <int W, bool G>
+#ifdef TPC_CT_MAXNREG
+__global__ void __maxnreg__(TPC_CT_MAXNREG) k_construct(
+#else
+__global__ void __launch_bounds__((W + 1) * 32, W <= 15 ? TPC_CT_MINB : 1) k_construct(
+#endif
+const __grid_constant__ View v, const __grid_constant__ Const c, const int cap_s,
                                                              const int cap_g, float* const spill) {
     extern __shared__ __align__(128) unsigned char ct_raw[];
     TPC_RETURN_IF_REJECTED(v);
     CtSmem& sm = *reinterpret_cast<CtSmem*>(ct_raw);
     const int cap = cap_s + cap_g;
-    CtSlots sl;
+    CtSlots<G> sl;
     sl.st = reinterpret_cast<float*>(ct_raw + sizeof(CtSmem)); sl.cap_s = cap_s; sl.cap_g = cap_g;
     sl.gs = spill + (size_t)blockIdx.x * kCtWords * cap_g;
     uint16_t* const freel = reinterpret_cast<uint16_t*>(sl.st + (size_t)kCtWords * cap_s);   // stack of free slots
@@ -464,7 +492,8 @@ __global__ void __launch_bounds__((W + 1) * 32, W <= 10 ? 2 : 1) k_construct(con
     if (threadIdx.x == 0) {
         for (int s = 0; s < kCtRing; s++) { mbar_init(&sm.full[s], 1); mbar_init(&sm.empty[s], W); }
         mbar_init(&sm.tbar, 1);
-        sm.abort = 0;
+        sm.abort = 0; sm.n_built = 0u; sm.n_done = 0u;
+        for (int k = 0; k < 20; k++) { sm.n_visits[k] = 0u; sm.n_updates[k] = 0u; }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
@@ -473,7 +502,6 @@ __global__ void __launch_bounds__((W + 1) * 32, W <= 10 ? 2 : 1) k_construct(con
     const int nr = c.n_rows, D = c.p.link_step;
     const int S = min(v.seed_start[v.n_bins], v.S_cap);
     volatile int32_t* const abort = &sm.abort;
-    unsigned visits = 0, updates = 0, built = 0;
     uint32_t it = 0;
 #ifdef TPC_CT_PROF
     long long pf[16] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0}, tq = clock64();
@@ -505,19 +533,21 @@ __global__ void __launch_bounds__((W + 1) * 32, W <= 10 ? 2 : 1) k_construct(con
         const size_t cg = cell_index(dn.x, tb + row);
         const float2* const hits = staged ? reinterpret_cast<const float2*>(sm.hits[s]) + (dn.x & 1) : v.shit + dn.x;
         const uint16_t* const cs = staged ? reinterpret_cast<const uint16_t*>(sm.cells[s]) + (cg & 7) : v.cells + cg;
-        uint32_t* const plist = v.kf_park + sm.i0;   // parked tracklets of this task, in order of parking
 
         // The consumer warps meet at barriers only around an intake: rows where nothing starts (most rows of a sparse
         // event) are processed by every warp on its own, up to a ring's depth apart.
         const bool intake = sm.cnt[row] > 0;
         if (!up && intake) {   // down sweep: what starts at this row is taken in BEFORE the row is processed (and starts
             ct_bar<W>();          // below it); all slots freed by the rows above are back on the stack
-            ct_intake_down<W>(v, c, sm, sl, freel, cap, row, s);
+            ct_intake_down<W, G>(v, c, sm, sl, freel, cap, row, s);
             ct_bar<W>();
         }
         PF(1)
         // ---- one pad row for the tracklets under way: the warps share the groups of 32 slots ----
         const int n_groups = (*(volatile int32_t*)&sm.n_hw + 31) >> 5;
+#ifdef TPC_CT_HIST
+        if (warp == 0 && lane == 0) atomicAdd(&v.cnt[CNT_PROF + min(n_groups, 15)], 1ull);
+#endif
         for (int g = warp; g < n_groups; g += W) {
             const uint32_t occ = *(volatile uint32_t*)&sm.occ[g];
             if (!occ) continue;
@@ -528,7 +558,7 @@ __global__ void __launch_bounds__((W + 1) * 32, W <= 10 ? 2 : 1) k_construct(con
             if (on && !up && t.top == row) on = false;          // taken in at this very row: starts below
             Fit& f = t.f;
             uint16_t* const gt = v.tl_tab + (size_t)(on ? t.i : 0) * v.tab_stride;
-            bool end = false, search = false, counted = false;
+            bool end = false, search = false, counted = false, vis = false;
             int acc = -1, nn = -1;
             uint16_t eold = kNoHit;
             float ay = 0.f, az = 0.f, iwy = 0.f, iwz = 0.f;
@@ -548,7 +578,7 @@ __global__ void __launch_bounds__((W + 1) * 32, W <= 10 ? 2 : 1) k_construct(con
                 }
                 end = !fit_transport(f, c.row_x[up ? row - 1 : row + 1], c.row_x[row], c);
                 if (!end) {
-                    visits++;
+                    vis = true;
                     iwy = 1.f / (f.c00 + c.sigma_y2); iwz = 1.f / (f.c11 + c.sigma_z2);
                     bool gate_ok = false;
                     if (known >= 0) {   // the gate value of (ky, kz) on the predicted state
@@ -605,40 +635,46 @@ __global__ void __launch_bounds__((W + 1) * 32, W <= 10 ? 2 : 1) k_construct(con
             __syncwarp();
             if (upd) {
                 fit_update(f, ay, az, iwy, c);
-                updates++;
+                int sn; float* const P = sl.snap(slot, sn);
                 if (up) {
-                    t.p0 = ay; t.p1 = az; t.p2 = f.s; t.p3 = f.t; t.p4 = f.q; t.top = row;
+                    P[0] = ay; P[sn] = az; P[2 * sn] = f.s; P[3 * sn] = f.t; P[4 * sn] = f.q; t.top = row;
                     if (intake) {                               // seed de-duplication: this hit is being followed
                         const int hl = acc - dn.x;              // (marks matter only where start hits wait)
                         atomicOr(&sm.used[row & 1][hl >> 5], 1u << (hl & 31));
                     }
                 } else {
-                    t.p0 = f.y; t.p1 = f.z; t.p2 = f.s; t.p3 = f.t; t.p4 = f.q; t.p5 = f.chi2; t.aux = row;
+                    P[0] = f.y; P[sn] = f.z; P[2 * sn] = f.s; P[3 * sn] = f.t; P[4 * sn] = f.q; t.p5 = f.chi2; t.aux = row;
                 }
             }
             __syncwarp();
             const bool fin = on && (end || row == (up ? nr - 1 : 0));
             if (fin) {
+                int sn; const float* const P = sl.snap(slot, sn);
+                const float p0 = P[0], p1 = P[sn], p2 = P[2 * sn], p3 = P[3 * sn], p4 = P[4 * sn];
                 if (up) {   // park: a fresh fit will start at the top hit in the down sweep
                     float4* dst = reinterpret_cast<float4*>(&v.tl_up[t.i]);
                     const int below = t.top > t.r0 ? (int)(__float_as_uint(t.p5) >> 16) : (int)kNoHit;
-                    dst[0] = make_float4(t.p0, t.p1, t.p2, t.p3);
-                    dst[1] = make_float4(t.p4, __int_as_float(t.r0 | (t.top << 8)), __int_as_float(below), __int_as_float(t.i));
+                    dst[0] = make_float4(p0, p1, p2, p3);
+                    dst[1] = make_float4(p4, __int_as_float(t.r0 | (t.top << 8)), __int_as_float(below), __int_as_float(t.i));
                     const int k = atomicAdd(&sm.n_parked, 1);
-                    plist[k] = (uint32_t)(t.i - sm.i0) | ((uint32_t)t.top << 24);
+                    v.kf_park[sm.i0 + k] = (uint32_t)(t.i - sm.i0) | ((uint32_t)t.top << 24);   // in order of parking
                     atomicAdd(&sm.dcnt[t.top], 1);
                     atomicMax(&sm.top_max, t.top);
                 } else {
                     v.tl_rows[t.i] = t.aux | (t.top << 8) | (f.n << 16);
                     const int sc = v.S_cap;
-                    v.tl_par[t.i] = t.p0; v.tl_par[sc + t.i] = t.p1; v.tl_par[2 * sc + t.i] = t.p2; v.tl_par[3 * sc + t.i] = t.p3;
-                    v.tl_par[4 * sc + t.i] = t.p4; v.tl_par[5 * sc + t.i] = t.p5;
+                    v.tl_par[t.i] = p0; v.tl_par[sc + t.i] = p1; v.tl_par[2 * sc + t.i] = p2; v.tl_par[3 * sc + t.i] = p3;
+                    v.tl_par[4 * sc + t.i] = p4; v.tl_par[5 * sc + t.i] = t.p5;
                 }
             } else if (on) {
                 sl.store(t, slot);
             }
             const unsigned gone = __ballot_sync(kFull, fin);    // this warp alone owns the group's occupancy word now
-            if (gone && lane == 0) sm.occ[g] = occ & ~gone;
+            const unsigned nvis = __popc(__ballot_sync(kFull, vis)), nupd = __popc(__ballot_sync(kFull, upd));
+            if (lane == 0) {
+                if (gone) sm.occ[g] = occ & ~gone;
+                sm.n_visits[warp] += nvis; sm.n_updates[warp] += nupd;
+            }
             if (fin) ct_push(sm, freel, slot, cap);
         }
         PF(3)
@@ -649,7 +685,7 @@ __global__ void __launch_bounds__((W + 1) * 32, W <= 10 ? 2 : 1) k_construct(con
         if (up && (intake || next_intake)) {
             ct_bar<W>();
             PF(4)
-            if (intake) built += ct_intake_up<W>(v, c, sm, sl, freel, cap, row, s, S);
+            if (intake) ct_intake_up<W, G>(v, c, sm, sl, freel, cap, row, s, S);
             PF(8)
             if (next_intake)
                 for (int k = threadIdx.x; k < TPC_MAX_ROW_HITS / 32; k += W * 32) sm.used[(row + 1) & 1][k] = 0u;
@@ -665,13 +701,15 @@ __global__ void __launch_bounds__((W + 1) * 32, W <= 10 ? 2 : 1) k_construct(con
     if (lane == 0 && warp == 0)   // cycles of warp 0 by phase, summed over the CTAs
         for (int k = 0; k < 16; k++) atomicAdd(&v.cnt[CNT_PROF + k], (unsigned long long)pf[k]);
 #endif
-    unsigned long long vs = visits, us = updates, bs = built;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-        vs += __shfl_xor_sync(kFull, vs, o); us += __shfl_xor_sync(kFull, us, o); bs += __shfl_xor_sync(kFull, bs, o);
-    }
-    if (lane == 0 && (vs | bs)) {
-        atomicAdd(&v.cnt[CNT_ROW_VISITS], vs); atomicAdd(&v.cnt[CNT_UPDATES], us); atomicAdd(&v.cnt[CNT_TRACKLETS], bs);
+    __syncwarp();
+    if (lane == 0) {
+        const uint32_t vs = sm.n_visits[warp], us = sm.n_updates[warp];
+        if (vs) { atomicAdd(&v.cnt[CNT_ROW_VISITS], (unsigned long long)vs); atomicAdd(&v.cnt[CNT_UPDATES], (unsigned long long)us); }
+        __threadfence_block();
+        if (atomicAdd(&sm.n_done, 1u) == (uint32_t)(W - 1)) {   // the last consumer warp out
+            const uint32_t bs = *(volatile uint32_t*)&sm.n_built;
+            if (bs) atomicAdd(&v.cnt[CNT_TRACKLETS], (unsigned long long)bs);
+        }
     }
 }
 

@@ -319,8 +319,9 @@ int launch_all(const tpc_tracker* tr, Batch* t, int from = 1) {
     if (from <= 5) {   // K5: one CTA per sector task, up sweep then down sweep (kf_construct.cuh)
         const int tier = t->ct_tier;
         const int grid = std::max(1, std::min(tr->ct_blocks[tier], v.n_tasks));
-        if (tier == 0) k_construct<kCtWarps><<<grid, ct_threads(kCtWarps), ct_smem_bytes(tier), st>>>(v, c, kCtCapSmem[tier], kCtCapSpill[tier], tr->ct_spill.p);
-        else k_construct<kCtWarpsWide><<<grid, ct_threads(kCtWarpsWide), ct_smem_bytes(tier), st>>>(v, c, kCtCapSmem[tier], kCtCapSpill[tier], tr->ct_spill.p);
+        if (tier == 0) k_construct<kCtWarps, (kCtCapSpill[0] > 0)><<<grid, ct_threads(kCtWarps), ct_smem_bytes(tier), st>>>(v, c, kCtCapSmem[tier], kCtCapSpill[tier], tr->ct_spill.p);
+        else if (kCtCapSpill[tier] == 0) k_construct<kCtWarpsWide, false><<<grid, ct_threads(kCtWarpsWide), ct_smem_bytes(tier), st>>>(v, c, kCtCapSmem[tier], kCtCapSpill[tier], tr->ct_spill.p);
+        else k_construct<kCtWarpsWide, true><<<grid, ct_threads(kCtWarpsWide), ct_smem_bytes(tier), st>>>(v, c, kCtCapSmem[tier], kCtCapSpill[tier], tr->ct_spill.p);
         L++;
     }
     mark(4);
@@ -525,6 +526,11 @@ int batch_finish(const tpc_tracker* tr, Batch* t) {
         t->counters.n_updates = (int64_t)t->h_cnt.p[CNT_UPDATES];
         t->counters.n_refit_visits = (int64_t)t->h_cnt.p[CNT_REFIT_VISITS];
         t->counters.n_tracklets = (int64_t)t->h_cnt.p[CNT_TRACKLETS];
+#ifdef TPC_CT_HIST
+        fprintf(stderr, "K5 row steps by groups of 32 slots in use (0..15+):");
+        for (int k = 0; k < 16; k++) fprintf(stderr, " %.0f", (double)t->h_cnt.p[CNT_PROF + k]);
+        fprintf(stderr, "\n");
+#endif
 #ifdef TPC_CT_PROF
         fprintf(stderr, "K5 warp-0 cycles by phase (0 wait-row, 1 intake-dn + barrier, 3 groups, 4 barrier, 5 intake-up + barrier, 7 loop):");
         for (int k = 0; k < 14; k++) fprintf(stderr, " %.3g", (double)t->h_cnt.p[CNT_PROF + k]);
@@ -644,22 +650,24 @@ tpc_tracker* tpc_tracker_create_ex(const tpc_geometry* g, float bz, const tpc_pa
         int per_sm = 0;
         size_t most = 0;
         for (int k = 0; k < kCtTiers; k++) most = std::max(most, ct_smem_bytes(k));
-        if (cudaFuncSetAttribute(k_construct<kCtWarps>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ct_smem_bytes(0)) != cudaSuccess ||
-            cudaFuncSetAttribute(k_construct<kCtWarpsWide>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)most) != cudaSuccess) {
+        if (cudaFuncSetAttribute(k_construct<kCtWarps, (kCtCapSpill[0] > 0)>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ct_smem_bytes(0)) != cudaSuccess ||
+            cudaFuncSetAttribute(k_construct<kCtWarpsWide, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)most) != cudaSuccess ||
+            cudaFuncSetAttribute(k_construct<kCtWarpsWide, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)most) != cudaSuccess) {
             set_err("k_construct: %zu bytes of shared memory cannot be configured: %s", most, cudaGetErrorString(cudaGetLastError()));
             delete t;
             return nullptr;
         }
         for (int k = 0; k < kCtTiers; k++) {
             const cudaError_t e = k == 0
-                ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_construct<kCtWarps>, ct_threads(kCtWarps), ct_smem_bytes(k))
-                : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_construct<kCtWarpsWide>, ct_threads(kCtWarpsWide), ct_smem_bytes(k));
+                ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_construct<kCtWarps, (kCtCapSpill[0] > 0)>, ct_threads(kCtWarps), ct_smem_bytes(k))
+                : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_construct<kCtWarpsWide, true>, ct_threads(kCtWarpsWide), ct_smem_bytes(k));
             if (e != cudaSuccess || per_sm < 1) {
                 set_err("k_construct cannot be configured: %s", cudaGetErrorString(cudaGetLastError()));
                 delete t;
                 return nullptr;
             }
             t->ct_blocks[k] = t->sm_count * per_sm;
+            if (getenv("TPCTRACK_VERBOSE")) fprintf(stderr, "[tpctrack] K5 tier %d: %d CTAs per SM, %zu bytes of shared memory\n", k, per_sm, ct_smem_bytes(k));
         }
         if (!p.seed_dedup) t->ct_tier = 1;   // ~3x the tracklets under way
         if (const char* se = getenv("TPCTRACK_CT_TIER")) t->ct_tier = std::max(0, std::min(atoi(se), kCtTiers - 1));
