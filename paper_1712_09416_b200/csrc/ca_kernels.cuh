@@ -261,18 +261,19 @@ __global__ void __launch_bounds__(kSortThreads) k_sort_row(const View v) {
 // ---------------------------------------------------------------------------------------------------------
 constexpr int kNfThreads = 128;
 #ifndef TPC_NF_CAP
-#define TPC_NF_CAP 640
+#define TPC_NF_CAP 448
 #endif
 #ifndef TPC_NF_BLOCKS
 #define TPC_NF_BLOCKS 12
 #endif
 constexpr int kNfCap = TPC_NF_CAP;   // hits of a neighbour row held in shared memory; larger rows are read in place
-constexpr int kNfReg = 4;      // candidates of a window remembered per hit (in a register); more -> nested walk
+constexpr int kNfList = 8;     // candidates of a window remembered per hit; more -> nested walk
 
 __global__ void __launch_bounds__(kNfThreads, TPC_NF_BLOCKS) k_neighbours(const View v, const __grid_constant__ Const c) {
     __shared__ float2 s_hu[kNfCap], s_hd[kNfCap];
     constexpr int kNfCells = kCellsPerHit * kNfCap + kCellPad;   // cell-table entries held in shared memory
     __shared__ uint16_t s_cu[kNfCells], s_cd[kNfCells];
+    __shared__ uint16_t s_dl[kNfList][kNfThreads], s_ul[kNfList][kNfThreads];   // row-local candidates of the thread's hit
     TPC_RETURN_IF_REJECTED(v);
     const int bin = blockIdx.x;
     const int nr = c.n_rows, D = c.p.link_step;
@@ -328,11 +329,10 @@ __global__ void __launch_bounds__(kNfThreads, TPC_NF_BLOCKS) k_neighbours(const 
             }
             if (take) { best = dev; bpair = (u << 16) | d; }
         };
-        // The candidates inside the two windows are first collected -- up to kNfReg of each side as 16-bit
-        // row-local indices packed into a 64-bit register -- and the pairs are then evaluated in ONE flat loop: a
-        // warp's trip count is its largest pair count, not the sum over nested loops with diverging trip counts.
+        // The candidates inside the two windows are first collected -- up to kNfList of each side, row-local indices
+        // in shared memory -- and the pairs are then evaluated in ONE flat loop: a warp's trip count is its largest
+        // pair count, not the sum over nested loops with diverging trip counts.
         const CellWin wd = cell_window(gfd, nyd, dd.w, y0, z0, wyd, wzd);
-        unsigned long long ld = 0ull, lu = 0ull;
         int nd = 0, nu = 0;
         for (int iz = wd.iz0; iz <= wd.iz1; iz++) {
             int p = cd[iz * nyd + wd.iy0];
@@ -340,7 +340,7 @@ __global__ void __launch_bounds__(kNfThreads, TPC_NF_BLOCKS) k_neighbours(const 
             for (; p < pe; p++) {
                 const float2 pd = hd[p];
                 if (fabsf(pd.x - y0) <= wyd && fabsf(pd.y - z0) <= wzd) {
-                    if (nd < kNfReg) ld |= (unsigned long long)p << (16 * nd);
+                    if (nd < kNfList) s_dl[nd][threadIdx.x] = (uint16_t)p;
                     nd++;
                 }
             }
@@ -354,17 +354,17 @@ __global__ void __launch_bounds__(kNfThreads, TPC_NF_BLOCKS) k_neighbours(const 
                 for (; p < pe; p++) {
                     const float2 pu = hu[p];
                     if (fabsf(pu.x - y0) <= wyu && fabsf(pu.y - z0) <= wzu) {
-                        if (nu < kNfReg) lu |= (unsigned long long)p << (16 * nu);
+                        if (nu < kNfList) s_ul[nu][threadIdx.x] = (uint16_t)p;
                         nu++;
                     }
                 }
             }
         }
-        if (nd <= kNfReg && nu <= kNfReg) {
+        if (nd <= kNfList && nu <= kNfList) {
             const int np = nd * nu;
             int ju = 0, jd = 0;
             for (int q = 0; q < np; q++) {
-                const int u = (int)(lu >> (16 * ju)) & 0xffff, d = (int)(ld >> (16 * jd)) & 0xffff;
+                const int u = s_ul[ju][threadIdx.x], d = s_dl[jd][threadIdx.x];
                 eval(u, hu[u], d, hd[d]);
                 if (++jd == nd) { jd = 0; ju++; }
             }

@@ -25,7 +25,7 @@ namespace tpc {
 // because the shared-memory carve-out leaves ~10 KB of L1) 5.82 ms; 11 warps (80 registers, 52 B) 5.62 ms; 10 warps
 // 6.10 ms; 9 warps (no spill) 4.61 ms; 8 warps 4.70 ms.
 #ifndef TPC_CT_WARPS
-#define TPC_CT_WARPS 9
+#define TPC_CT_WARPS 12
 #endif
 #ifndef TPC_CT_MINB
 #define TPC_CT_MINB 2
@@ -36,10 +36,14 @@ namespace tpc {
 #ifndef TPC_CT_INL
 #define TPC_CT_INL __forceinline__   // intake / turn inlined: 5.95 ms against 6.42 ms out of line (config 5)
 #endif
-constexpr int kCtWarps = TPC_CT_WARPS;                 // consumer warps of a CTA (one more warp produces), two CTAs per SM
-constexpr int kCtWarpsWide = 19;                       // ... of the one-CTA-per-SM tiers (640 threads x 96 registers, no spills)
-constexpr int ct_threads(int warps) { return (warps + 1) * 32; }
+constexpr int kCtWarps = TPC_CT_WARPS;                 // warps of a CTA, two CTAs per SM
+constexpr int kCtWarpsWide = 20;                       // ... of the one-CTA-per-SM tiers (640 threads x 96 registers, no spills)
+constexpr int ct_threads(int warps) { return warps * 32; }
 constexpr int kCtRing = TPC_CT_RING;                   // rows in flight
+#ifndef TPC_CT_DNB
+#define TPC_CT_DNB 4
+#endif
+constexpr int kCtDnBatch = TPC_CT_DNB;                 // down sweep: the parked tracklets of this many rows are taken in at once
 constexpr int kCtWords = 32;                           // 4-byte words of a tracklet's state
 #ifndef TPC_CT_STAGE
 #define TPC_CT_STAGE 48
@@ -65,8 +69,6 @@ constexpr int kSwHitBytes = (kSwCap + 2) * 8;          // + alignment slack of t
 constexpr int kSwCellEntries = kCellsPerHit * kSwCap + kCellPad + 16;
 constexpr int kSwCellBytes = kSwCellEntries * 2;
 static_assert(kSwHitBytes % 16 == 0 && kSwCellBytes % 16 == 0, "bulk copies are 16-byte granular");
-constexpr int kCtDown = 0x100;                         // cmd flag: the row belongs to the down sweep
-constexpr int kCtTurn = 0x200;                         // cmd: between the sweeps (order the parked tracklets by top row)
 
 // a start hit: its coordinates, the direction (sin phi, tg lambda) of the line to its up-link (DESIGN.md "O5" up pass,
 // initial state), the hit itself, its up-link, and that one's
@@ -90,9 +92,9 @@ struct __align__(128) CtSmem {
     int32_t dcnt[kCtRows];                    // tracklets parked with their top hit in each row
     uint32_t used[2][TPC_MAX_ROW_HITS / 32];           // hits of the row at hand recorded by an up pass (double buffered)
     uint32_t occ[(kCtCapMax + 31) / 32];               // occupied state slots
-    unsigned long long full[kCtRing], empty[kCtRing], tbar;
-    int32_t cmd[kCtRing];                              // row held by the ring slot (| kCtDown); -1 = no more work
-    int32_t task, abort, n_free, n_hw, n_parked, top_max, i0;   // n_hw: highest slot used so far + 1
+    unsigned long long full[kCtRing], tbar;
+    int32_t rel[kCtRing];                              // warps through with the row in the ring slot
+    int32_t task, first, abort, n_free, n_hw, n_parked, top_max, i0;   // first: lowest row with a start hit; n_hw: highest slot used so far + 1
     uint32_t n_visits[20], n_updates[20], n_built, n_done;   // this CTA's share of the run's counters (per consumer warp)
 };
 
@@ -140,122 +142,87 @@ template <int W> __device__ __forceinline__ void ct_bar() { asm volatile("bar.sy
 __device__ __forceinline__ size_t cell_index(int base, int bin) { return (size_t)kCellsPerHit * base + (size_t)bin * kCellPad; }
 
 // ---------------------------------------------------------------------------------------------------------
-// producer warp: hands the CTA its sector tasks and streams their rows, up then down
+// The rows of a sweep go through the ring without a producer warp: the warp that is LAST to be through with a row
+// refills the ring slot it has just freed with the row kCtRing steps ahead (one lane, three bulk copies).
 // ---------------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void ct_producer(const View& v, const Const& c, CtSmem& sm, uint16_t* freel, int cap) {
+// Down sweep: the parked tracklets are taken in -- at a barrier of the warps -- not row by row but kCtDnBatch rows at a
+// time, at the sweep's first row and at every row r with r % kCtDnBatch == kCtDnBatch - 1, for the rows
+// r - r % kCtDnBatch .. r (their records are contiguous in dn_rec); a tracklet taken in early waits in its slot until
+// the sweep has passed its top row.  Between two such rows the warps run on their own, up to a ring's depth apart.
+__device__ __forceinline__ bool ct_dn_intake_row(const CtSmem& sm, int row, int& rlo, int& n) {
+    if (row % kCtDnBatch != kCtDnBatch - 1 && row != *(volatile const int32_t*)&sm.top_max) return false;
+    rlo = row - row % kCtDnBatch;
+    n = sm.lo[row] + sm.cnt[row] - sm.lo[rlo];
+    return n > 0;
+}
+// one lane: the row (hits, grid cell table, the records of what starts there) into the ring slot of iteration j
+__device__ __forceinline__ void ct_issue(const View& v, CtSmem& sm, int row, bool down, int tb, uint32_t j, int S) {
+    const int s = (int)(j % kCtRing);
+    const BinDesc& d = sm.desc[row];
+    const bool rowdata = d.n > 0 && d.n <= kSwCap;
+    // records to stage: start hits of the row (not beyond the pool), or tracklets parked there
+    int rlo = row, nd = 0;
+    if (down) ct_dn_intake_row(sm, row, rlo, nd);
+    const int ns = down ? min(nd, kCtSeedStage) : max(0, min(min(sm.cnt[row], kCtSeedStage), S - sm.lo[row]));
+    const void* const recs = down ? (const void*)(v.dn_rec + sm.i0 + sm.lo[rlo]) : (const void*)(v.seed_rec + sm.lo[row]);
+    if (rowdata || ns > 0) {
+        const int offh = d.base & 1;
+        const uint32_t hb = rowdata ? (uint32_t)((offh + d.n + 1) & ~1) * 8u : 0u;
+        const size_t g = cell_index(d.base, tb + row);
+        const int offc = (int)(g & 7);
+        const uint32_t cb = rowdata ? (((uint32_t)(offc + d.ny * d.nz + 1) * 2u + 15u) & ~15u) : 0u;
+        mbar_arrive_expect_tx(&sm.full[s], hb + cb + 32u * (uint32_t)ns);
+        if (rowdata) {
+            bulk_g2s(sm.hits[s], v.shit + (d.base - offh), hb, &sm.full[s]);
+            bulk_g2s(sm.cells[s], v.cells + (g - offc), cb, &sm.full[s]);
+        }
+        if (ns > 0) bulk_g2s(sm.seeds[s], recs, 32u * (uint32_t)ns, &sm.full[s]);
+    } else {
+        mbar_arrive(&sm.full[s]);
+    }
+}
+
+// warp 0, the other warps waiting at a barrier: all state slots free (the stack of free slots, lowest on top.
+// Measured: preferring the slots of the warps' first groups is SLOWER -- a step takes as long as its slowest lane,
+// and fuller groups have slower slowest lanes)
+__device__ __forceinline__ void ct_reset_slots(CtSmem& sm, uint16_t* freel, int cap) {
+    const int lane = lane_id();
+    for (int k = lane; k < cap; k += 32) freel[k] = (uint16_t)(cap - 1 - k);
+    for (int k = lane; k < (kCtCapMax + 31) / 32; k += 32) sm.occ[k] = 0u;
+    if (lane == 0) { sm.n_free = cap; sm.n_hw = 0; }
+}
+
+// warp 0, the other warps waiting at a barrier: the next sector task and its tables (sm.task >= n_tasks: none left)
+__device__ __forceinline__ void ct_next_task(const View& v, const Const& c, CtSmem& sm, uint16_t* freel, int cap, uint32_t& tphase) {
     const int lane = lane_id();
     const int nr = c.n_rows;
-    const int S = min(v.seed_start[v.n_bins], v.S_cap);
-    volatile int32_t* const abort = &sm.abort;
-    uint32_t it = 0, tphase = 0;
-    bool ok = true;
-    // lane 0: one row into the ring
-    auto issue = [&](int row, int flag, int tb) {
-        const int s = (int)(it % kCtRing);
-        if (!(ok = mbar_wait(&sm.empty[s], ((it / kCtRing) & 1u) ^ 1u, abort))) return;
-        sm.cmd[s] = row | flag;
-        const BinDesc& d = sm.desc[row];
-        const bool rowdata = d.n > 0 && d.n <= kSwCap;
-        // records to stage: start hits of the row (not beyond the pool), or tracklets parked there
-        const int ns = flag ? min(sm.cnt[row], kCtSeedStage) : max(0, min(min(sm.cnt[row], kCtSeedStage), S - sm.lo[row]));
-        const void* const recs = flag ? (const void*)(v.dn_rec + sm.i0 + sm.lo[row]) : (const void*)(v.seed_rec + sm.lo[row]);
-        if (rowdata || ns > 0) {
-            const int offh = d.base & 1;
-            const uint32_t hb = rowdata ? (uint32_t)((offh + d.n + 1) & ~1) * 8u : 0u;
-            const size_t g = cell_index(d.base, tb + row);
-            const int offc = (int)(g & 7);
-            const uint32_t cb = rowdata ? (((uint32_t)(offc + d.ny * d.nz + 1) * 2u + 15u) & ~15u) : 0u;
-            mbar_arrive_expect_tx(&sm.full[s], hb + cb + 32u * (uint32_t)ns);
-            if (rowdata) {
-                bulk_g2s(sm.hits[s], v.shit + (d.base - offh), hb, &sm.full[s]);
-                bulk_g2s(sm.cells[s], v.cells + (g - offc), cb, &sm.full[s]);
-            }
-            if (ns > 0) bulk_g2s(sm.seeds[s], recs, 32u * (uint32_t)ns, &sm.full[s]);
-        } else {
-            mbar_arrive(&sm.full[s]);
-        }
-        it++;
-    };
-    // lane 0: wait until the consumers are through with everything issued so far
-    auto drain = [&]() {
-        for (uint32_t j = it > (uint32_t)kCtRing ? it - kCtRing : 0; ok && j < it; j++)
-            ok = mbar_wait(&sm.empty[j % kCtRing], (j / kCtRing) & 1u, abort);
-    };
-    auto reset_slots = [&]() {   // the consumers are idle: all state slots are free
-        // the stack of free slots, lowest on top.  (Measured: preferring the slots of the warps' first groups, so that
-        // one round per row serves up to 416 tracklets, is SLOWER, 5.97 against 5.42 ms on config 5 -- a step takes as
-        // long as its slowest lane, and fuller groups have slower slowest lanes.)
-        for (int k = lane; k < cap; k += 32) freel[k] = (uint16_t)(cap - 1 - k);
-        for (int k = lane; k < (kCtCapMax + 31) / 32; k += 32) sm.occ[k] = 0u;
-        if (lane == 0) { sm.n_free = cap; sm.n_hw = 0; }
-    };
-    while (ok) {
-        int task = 0;
-        if (lane == 0) task = (int)atomicAdd(&v.kf_cursor[0], 1ull);
-        task = __shfl_sync(kFull, task, 0);
-        if (task >= v.n_tasks) break;
-        const int tb = task * nr;
-        // the consumers are idle here (start of the kernel, or the ring drained): the task's tables may be replaced
-        if (lane == 0) {
-            mbar_arrive_expect_tx(&sm.tbar, (uint32_t)nr * 32u);
-            bulk_g2s(sm.desc, v.desc + tb, (uint32_t)nr * 32u, &sm.tbar);
-            sm.task = task; sm.n_parked = 0; sm.top_max = -1; sm.i0 = v.seed_start[tb];
-        }
-        int f = nr;
-        for (int r = lane; r < nr; r += 32) {
-            const int lo = v.seed_start[tb + r], n = v.seed_start[tb + r + 1] - lo;
-            sm.lo[r] = lo; sm.cnt[r] = n;
-            if (n > 0) f = min(f, r);
-        }
-        for (int k = lane; k < 2 * (TPC_MAX_ROW_HITS / 32); k += 32) (&sm.used[0][0])[k] = 0u;
-        for (int r = lane; r < kCtRows; r += 32) sm.dcnt[r] = 0;
-        reset_slots();
-#pragma unroll
-        for (int o = 16; o > 0; o >>= 1) f = min(f, __shfl_xor_sync(kFull, f, o));
-        if (lane == 0) ok = mbar_wait(&sm.tbar, tphase, abort);
-        tphase ^= 1u;
-        ok = __shfl_sync(kFull, (int)ok, 0) != 0;
-        __syncwarp();
-        if (!ok || f >= nr) continue;
-        if (lane == 0) {   // up sweep
-            for (int row = f; ok && row < nr; row++) issue(row, 0, tb);
-            drain();
-        }
-        ok = __shfl_sync(kFull, (int)ok, 0) != 0;
-        it = __shfl_sync(kFull, it, 0);
-        __syncwarp();
-        if (!ok) break;
-        reset_slots();
-        __syncwarp();
-        if (lane == 0) {   // the turn: the consumers order the parked tracklets by top row (lo / cnt become theirs)
-            const int s = (int)(it % kCtRing);
-            if ((ok = mbar_wait(&sm.empty[s], ((it / kCtRing) & 1u) ^ 1u, abort))) {
-                sm.cmd[s] = kCtTurn;
-                mbar_arrive(&sm.full[s]);
-                it++;
-                drain();
-            }
-        }
-        ok = __shfl_sync(kFull, (int)ok, 0) != 0;
-        it = __shfl_sync(kFull, it, 0);
-        __syncwarp();
-        if (!ok) break;
-        if (lane == 0) {   // down sweep from the highest top row
-            const int tm = *(volatile int32_t*)&sm.top_max;
-            for (int row = tm; ok && row >= 0; row--) issue(row, kCtDown, tb);
-            drain();
-        }
-        ok = __shfl_sync(kFull, (int)ok, 0) != 0;
-        it = __shfl_sync(kFull, it, 0);
-        __syncwarp();
-    }
+    int task = 0;
+    if (lane == 0) task = (int)atomicAdd(&v.kf_cursor[0], 1ull);
+    task = __shfl_sync(kFull, task, 0);
+    if (task >= v.n_tasks) { if (lane == 0) sm.task = task; return; }
+    const int tb = task * nr;
     if (lane == 0) {
-        const int s = (int)(it % kCtRing);
-        if (ok) ok = mbar_wait(&sm.empty[s], ((it / kCtRing) & 1u) ^ 1u, abort);
-        sm.cmd[s] = -1;
-        mbar_arrive(&sm.full[s]);
-        if (!ok) atomicOr((unsigned int*)&v.cnt[CNT_ERR], kErrHang);
+        mbar_arrive_expect_tx(&sm.tbar, (uint32_t)nr * 32u);
+        bulk_g2s(sm.desc, v.desc + tb, (uint32_t)nr * 32u, &sm.tbar);
+        sm.task = task; sm.n_parked = 0; sm.top_max = -1; sm.i0 = v.seed_start[tb];
     }
+    int f = nr;
+    for (int r = lane; r < nr; r += 32) {
+        const int lo = v.seed_start[tb + r], n = v.seed_start[tb + r + 1] - lo;
+        sm.lo[r] = lo; sm.cnt[r] = n;
+        if (n > 0) f = min(f, r);
+    }
+    for (int k = lane; k < 2 * (TPC_MAX_ROW_HITS / 32); k += 32) (&sm.used[0][0])[k] = 0u;
+    for (int r = lane; r < kCtRows; r += 32) sm.dcnt[r] = 0;
+    ct_reset_slots(sm, freel, cap);
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) f = min(f, __shfl_xor_sync(kFull, f, o));
+    if (lane == 0) {
+        sm.first = f;
+        if (!mbar_wait(&sm.tbar, tphase, &sm.abort)) sm.first = nr;   // (the flag is up: every warp leaves at its next wait)
+    }
+    tphase ^= 1u;
+    __syncwarp();
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -367,8 +334,8 @@ __device__ __forceinline__ void ct_push(CtSmem& sm, uint16_t* freel, int slot, i
 // ordered by top row: staged in the ring slot, the ones beyond kCtSeedStage read in place)
 template <int W, bool G>
 __device__ TPC_CT_INL void ct_intake_down(const View& v, const Const& c, CtSmem& sm, const CtSlots<G>& sl, const uint16_t* freel,
-                                            int cap, int row, int s) {
-    const int n = sm.cnt[row], lo = sm.i0 + sm.lo[row];
+                                            int cap, int rlo, int n, int s) {
+    const int lo = sm.i0 + sm.lo[rlo];
     for (int j0 = 0; j0 < n; j0 += W * 32) {
         const int j = j0 + (int)threadIdx.x;
         const int slot = ct_pop(v, sm, freel, j < n, cap);
@@ -383,10 +350,11 @@ __device__ TPC_CT_INL void ct_intake_down(const View& v, const Const& c, CtSmem&
             }
             CtTrk t;
             t.p5 = 0.f;
-            t.r0 = __float_as_int(b4.y) & 0xff; t.top = row; t.i = __float_as_int(b4.w);
+            const int top = (__float_as_int(b4.y) >> 8) & 0xff;
+            t.r0 = __float_as_int(b4.y) & 0xff; t.top = top; t.i = __float_as_int(b4.w);
             t.f.y = a4.x; t.f.z = a4.y; t.f.s = a4.z; t.f.t = a4.w; t.f.q = b4.x;
             fit_prior(t.f, c); t.f.n = 1;
-            t.aux = row; t.miss = 0; t.ph = 3; t.nxt = -1;
+            t.aux = top; t.miss = 0; t.ph = 3; t.nxt = -1;
             t.cur = __float_as_int(b4.z);             // table entry of the row below the top hit
             sl.store(t, slot);
             int sn; float* const P = sl.snap(slot, sn);
@@ -476,7 +444,7 @@ template <int W, bool G>
 #ifdef TPC_CT_MAXNREG
 __global__ void __maxnreg__(TPC_CT_MAXNREG) k_construct(
 #else
-__global__ void __launch_bounds__((W + 1) * 32, W <= 15 ? TPC_CT_MINB : 1) k_construct(
+__global__ void __launch_bounds__(W * 32, W <= 16 ? TPC_CT_MINB : 1) k_construct(
 #endif
 const __grid_constant__ View v, const __grid_constant__ Const c, const int cap_s,
                                                              const int cap_g, float* const spill) {
@@ -490,43 +458,38 @@ const __grid_constant__ View v, const __grid_constant__ Const c, const int cap_s
     uint16_t* const freel = reinterpret_cast<uint16_t*>(sl.st + (size_t)kCtWords * cap_s);   // stack of free slots
     const int warp = threadIdx.x >> 5, lane = lane_id();
     if (threadIdx.x == 0) {
-        for (int s = 0; s < kCtRing; s++) { mbar_init(&sm.full[s], 1); mbar_init(&sm.empty[s], W); }
+        for (int s = 0; s < kCtRing; s++) { mbar_init(&sm.full[s], 1); sm.rel[s] = 0; }
         mbar_init(&sm.tbar, 1);
         sm.abort = 0; sm.n_built = 0u; sm.n_done = 0u;
         for (int k = 0; k < 20; k++) { sm.n_visits[k] = 0u; sm.n_updates[k] = 0u; }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
-    if (warp == W) { ct_producer(v, c, sm, freel, cap); return; }
 
     const int nr = c.n_rows, D = c.p.link_step;
     const int S = min(v.seed_start[v.n_bins], v.S_cap);
     volatile int32_t* const abort = &sm.abort;
-    uint32_t it = 0;
-#ifdef TPC_CT_PROF
-    long long pf[16] = {0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0, 0}, tq = clock64();
-#define PF(k) { const long long n_ = clock64(); pf[k] += n_ - tq; tq = n_; }
-#else
-#define PF(k)
-#endif
+    uint32_t it = 0, tphase = 0;      // rows through the ring so far (the same count in every warp); phase of tbar (warp 0)
+    int phase = 0;                    // 0: a sector task is due; 1: up sweep; 2: down sweep
+    int row = 0, last = 0, tb = 0;    // the row at hand, the last row of the sweep, the task's first bin
 
     for (;;) {
-        const int s = (int)(it % kCtRing);
-        PF(7)
-        if (!mbar_wait(&sm.full[s], (it / kCtRing) & 1u, abort)) break;
-        PF(0)
-        const int cmd = sm.cmd[s];
-        if (cmd < 0) break;
-        if (cmd == kCtTurn) {
-            ct_turn<W>(v, sm, nr);
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&sm.empty[s]);
-            it++;
-            continue;
+        if (phase == 0) {
+            ct_bar<W>();                                         // every warp is through with the task before
+            if (warp == 0) ct_next_task(v, c, sm, freel, cap, tphase);
+            ct_bar<W>();
+            const int task = *(volatile int32_t*)&sm.task;
+            if (task >= v.n_tasks) break;
+            tb = task * nr;
+            row = *(volatile int32_t*)&sm.first; last = nr - 1;
+            if (row > last) continue;                            // no start hit in this sector
+            phase = 1;
+            if (warp == 0 && lane == 0)                          // the ring is empty: its first rows
+                for (int k = 0; k < kCtRing; k++) if (row + k <= last) ct_issue(v, sm, row + k, false, tb, it + k, S);
         }
-        const int row = cmd & 0xff;
-        const bool up = !(cmd & kCtDown);
-        const int tb = sm.task * nr;
+        const bool up = phase == 1;
+        const int s = (int)(it % kCtRing);
+        if (!mbar_wait(&sm.full[s], (it / kCtRing) & 1u, abort)) break;
         const BinDesc& dsc = sm.desc[row];
         const int4 dn = make_int4(dsc.base, dsc.n, dsc.ny, dsc.nz);
         const bool staged = dn.y <= kSwCap;
@@ -537,12 +500,12 @@ const __grid_constant__ View v, const __grid_constant__ Const c, const int cap_s
         // The consumer warps meet at barriers only around an intake: rows where nothing starts (most rows of a sparse
         // event) are processed by every warp on its own, up to a ring's depth apart.
         const bool intake = sm.cnt[row] > 0;
-        if (!up && intake) {   // down sweep: what starts at this row is taken in BEFORE the row is processed (and starts
-            ct_bar<W>();          // below it); all slots freed by the rows above are back on the stack
-            ct_intake_down<W, G>(v, c, sm, sl, freel, cap, row, s);
+        int dn_lo = 0, dn_n = 0;
+        if (!up && ct_dn_intake_row(sm, row, dn_lo, dn_n)) {   // down sweep: what starts at these rows is taken in BEFORE
+            ct_bar<W>();                                        // this row is processed; all slots freed by the rows above
+            ct_intake_down<W, G>(v, c, sm, sl, freel, cap, dn_lo, dn_n, s);   // are back on the stack
             ct_bar<W>();
         }
-        PF(1)
         // ---- one pad row for the tracklets under way: the warps share the groups of 32 slots ----
         const int n_groups = (*(volatile int32_t*)&sm.n_hw + 31) >> 5;
 #ifdef TPC_CT_HIST
@@ -555,7 +518,7 @@ const __grid_constant__ View v, const __grid_constant__ Const c, const int cap_s
             bool on = (occ >> lane) & 1u;
             CtTrk t;
             if (on) sl.load(t, slot);
-            if (on && !up && t.top == row) on = false;          // taken in at this very row: starts below
+            if (on && !up && t.top <= row) on = false;          // starts below its top row
             Fit& f = t.f;
             uint16_t* const gt = v.tl_tab + (size_t)(on ? t.i : 0) * v.tab_stride;
             bool end = false, search = false, counted = false, vis = false;
@@ -677,30 +640,41 @@ const __grid_constant__ View v, const __grid_constant__ Const c, const int cap_s
             }
             if (fin) ct_push(sm, freel, slot, cap);
         }
-        PF(3)
         // up sweep: the start hits of this row are taken in AFTER it is processed (its marks are complete); the marks'
         // other buffer is cleared here for the next row if start hits wait there (its last readers, the intake two rows
         // down, are behind that row's barriers)
         const bool next_intake = up && row + 1 < nr && sm.cnt[row + 1] > 0;
         if (up && (intake || next_intake)) {
             ct_bar<W>();
-            PF(4)
             if (intake) ct_intake_up<W, G>(v, c, sm, sl, freel, cap, row, s, S);
-            PF(8)
             if (next_intake)
                 for (int k = threadIdx.x; k < TPC_MAX_ROW_HITS / 32; k += W * 32) sm.used[(row + 1) & 1][k] = 0u;
-            PF(9)
             ct_bar<W>();
         }
-        PF(5)
+        // through with the row: the last warp refills the ring slot with the row kCtRing steps ahead
         __syncwarp();
-        if (lane == 0) mbar_arrive(&sm.empty[s]);
+        if (lane == 0) {
+            __threadfence_block();
+            if (atomicAdd(&sm.rel[s], 1) == W - 1) {
+                sm.rel[s] = 0;
+                const int r2 = up ? row + kCtRing : row - kCtRing;
+                if (up ? r2 <= last : r2 >= last) ct_issue(v, sm, r2, !up, tb, it + kCtRing, S);
+            }
+        }
         it++;
+        if (row != last) { row += up ? 1 : -1; continue; }
+        if (!up) { phase = 0; continue; }
+        // the turn: every warp is through with the up sweep; the parked tracklets are ordered by top row (lo / cnt
+        // become theirs), all slots are free again, and the down sweep starts from the highest top row
+        ct_bar<W>();
+        if (warp == 0) ct_reset_slots(sm, freel, cap);
+        ct_turn<W>(v, sm, nr);
+        row = *(volatile int32_t*)&sm.top_max; last = 0;
+        if (row < 0) { phase = 0; continue; }
+        phase = 2;
+        if (warp == 0 && lane == 0)
+            for (int k = 0; k < kCtRing; k++) if (row - k >= 0) ct_issue(v, sm, row - k, true, tb, it + k, S);
     }
-#ifdef TPC_CT_PROF
-    if (lane == 0 && warp == 0)   // cycles of warp 0 by phase, summed over the CTAs
-        for (int k = 0; k < 16; k++) atomicAdd(&v.cnt[CNT_PROF + k], (unsigned long long)pf[k]);
-#endif
     __syncwarp();
     if (lane == 0) {
         const uint32_t vs = sm.n_visits[warp], us = sm.n_updates[warp];
