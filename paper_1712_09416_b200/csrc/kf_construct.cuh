@@ -94,7 +94,7 @@ struct __align__(128) CtSmem {
     uint32_t occ[(kCtCapMax + 31) / 32];               // occupied state slots
     unsigned long long full[kCtRing], tbar;
     int32_t rel[kCtRing];                              // warps through with the row in the ring slot
-    int32_t task, first, abort, n_free, n_hw, n_parked, top_max, i0;   // first: lowest row with a start hit; n_hw: highest slot used so far + 1
+    int32_t S, task, first, abort, n_free, n_hw, n_parked, top_max, i0;   // first: lowest row with a start hit; n_hw: highest slot used so far + 1
     uint32_t n_visits[20], n_updates[20], n_built, n_done;   // this CTA's share of the run's counters (per consumer warp)
 };
 
@@ -156,8 +156,8 @@ __device__ __forceinline__ bool ct_dn_intake_row(const CtSmem& sm, int row, int&
     return n > 0;
 }
 // one lane: the row (hits, grid cell table, the records of what starts there) into the ring slot of iteration j
-__device__ __forceinline__ void ct_issue(const View& v, CtSmem& sm, int row, bool down, int tb, uint32_t j, int S) {
-    const int s = (int)(j % kCtRing);
+__device__ __forceinline__ void ct_issue(const View& v, CtSmem& sm, int row, bool down, int tb, uint32_t j) {
+    const int s = (int)(j % kCtRing), S = sm.S;
     const BinDesc& d = sm.desc[row];
     const bool rowdata = d.n > 0 && d.n <= kSwCap;
     // records to stage: start hits of the row (not beyond the pool), or tracklets parked there
@@ -278,7 +278,7 @@ __device__ __forceinline__ void ct_load(CtTrk& t, const float* S, int cap) {
     const uint32_t pk = __float_as_uint(S[30 * cap]);
     t.ph = pk & 3u; t.miss = (pk >> 2) & 63u; t.r0 = (pk >> 8) & 255u; t.top = (pk >> 16) & 255u; t.aux = pk >> 24;
 }
-__device__ __forceinline__ void ct_store(const CtTrk& t, float* S, int cap) {
+__device__ __forceinline__ void ct_store(const CtTrk& t, float* S, int cap, bool up) {
     const Fit& f = t.f;
     S[0] = f.y; S[cap] = f.z; S[2 * cap] = f.s; S[3 * cap] = f.t; S[4 * cap] = f.q;
     S[5 * cap] = f.c00; S[6 * cap] = f.c10; S[7 * cap] = f.c11; S[8 * cap] = f.c20; S[9 * cap] = f.c21;
@@ -286,7 +286,9 @@ __device__ __forceinline__ void ct_store(const CtTrk& t, float* S, int cap) {
     S[15 * cap] = f.c40; S[16 * cap] = f.c41; S[17 * cap] = f.c42; S[18 * cap] = f.c43; S[19 * cap] = f.c44;
     S[20 * cap] = f.chi2; S[21 * cap] = __int_as_float(f.n);
     S[27 * cap] = t.p5;
-    S[28 * cap] = __int_as_float(t.i); S[29 * cap] = __int_as_float(t.cur); S[31 * cap] = __int_as_float(t.nxt);
+    S[28 * cap] = __int_as_float(t.i);
+    if (up) S[29 * cap] = __int_as_float(t.cur);   // down: written by the asynchronous copy of the table word (see the row step)
+    // word 31 (nxt): written at the intake and by the asynchronous copy of the next link
     S[30 * cap] = __uint_as_float((uint32_t)t.ph | ((uint32_t)t.miss << 2) | ((uint32_t)t.r0 << 8) |
                                   ((uint32_t)t.top << 16) | ((uint32_t)t.aux << 24));
 }
@@ -299,8 +301,22 @@ struct CtSlots {
     __device__ __forceinline__ void load(CtTrk& t, int slot) const {
         if (!G || slot < cap_s) ct_load(t, st + slot, cap_s); else ct_load(t, gs + (slot - cap_s), cap_g);
     }
-    __device__ __forceinline__ void store(const CtTrk& t, int slot) const {
-        if (!G || slot < cap_s) ct_store(t, st + slot, cap_s); else ct_store(t, gs + (slot - cap_s), cap_g);
+    __device__ __forceinline__ void store(const CtTrk& t, int slot, bool up) const {
+        if (!G || slot < cap_s) ct_store(t, st + slot, cap_s, up); else ct_store(t, gs + (slot - cap_s), cap_g, up);
+    }
+    // word k of a slot
+    __device__ __forceinline__ float* word(int slot, int k) const {
+        if (!G || slot < cap_s) return st + slot + k * cap_s;
+        return gs + (slot - cap_s) + k * cap_g;
+    }
+    // word k of a slot := the 4 bytes at src, without waiting for them: an asynchronous copy for a slot in shared memory
+    // (the warp waits for its copies when it is through with the row), a plain load and store for one in global memory
+    __device__ __forceinline__ void fetch(int slot, int k, const void* src) const {
+        if (!G || slot < cap_s) {
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(smem_u32(st + slot + k * cap_s)), "l"(src) : "memory");
+        } else {
+            gs[(slot - cap_s) + k * cap_g] = __ldg(reinterpret_cast<const float*>(src));
+        }
     }
     // words 22.. of a slot: the state right after the last accepted update
     __device__ __forceinline__ float* snap(int slot, int& stride) const {
@@ -355,8 +371,12 @@ __device__ TPC_CT_INL void ct_intake_down(const View& v, const Const& c, CtSmem&
             t.f.y = a4.x; t.f.z = a4.y; t.f.s = a4.z; t.f.t = a4.w; t.f.q = b4.x;
             fit_prior(t.f, c); t.f.n = 1;
             t.aux = top; t.miss = 0; t.ph = 3; t.nxt = -1;
-            t.cur = __float_as_int(b4.z);             // table entry of the row below the top hit
-            sl.store(t, slot);
+            t.cur = 0;
+            sl.store(t, slot, false);
+            {   // table entry of the row below the top hit, in both halves of the word (see the row step)
+                const uint32_t below = (uint32_t)__float_as_int(b4.z) & 0xffffu;
+                *sl.word(slot, 29) = __uint_as_float(below | (below << 16));
+            }
             int sn; float* const P = sl.snap(slot, sn);
             P[0] = a4.x; P[sn] = a4.y; P[2 * sn] = a4.z; P[3 * sn] = a4.w; P[4 * sn] = b4.x;
         }
@@ -399,7 +419,8 @@ __device__ TPC_CT_INL void ct_intake_up(const View& v, const Const& c, CtSmem& s
             t.p5 = __uint_as_float(((uint32_t)kNoHit << 16) | (uint32_t)hl);   // table entries: below the top hit | of the row before
             t.i = e; t.cur = hh.y; t.nxt = hh.z; t.ph = 1; t.miss = 0; t.r0 = row; t.top = row; t.aux = row + D;
             v.tl_tab[(size_t)e * v.tab_stride + row] = (uint16_t)hl;
-            sl.store(t, slot);
+            sl.store(t, slot, true);
+            *sl.word(slot, 31) = __int_as_float(t.nxt);
             int sn; float* const P = sl.snap(slot, sn);
             P[0] = a4.x; P[sn] = a4.y; P[2 * sn] = a4.z; P[3 * sn] = a4.w; P[4 * sn] = 0.f;
         }
@@ -460,14 +481,13 @@ const __grid_constant__ View v, const __grid_constant__ Const c, const int cap_s
     if (threadIdx.x == 0) {
         for (int s = 0; s < kCtRing; s++) { mbar_init(&sm.full[s], 1); sm.rel[s] = 0; }
         mbar_init(&sm.tbar, 1);
-        sm.abort = 0; sm.n_built = 0u; sm.n_done = 0u;
+        sm.abort = 0; sm.n_built = 0u; sm.n_done = 0u; sm.S = min(v.seed_start[v.n_bins], v.S_cap);   // start hits of the batch
         for (int k = 0; k < 20; k++) { sm.n_visits[k] = 0u; sm.n_updates[k] = 0u; }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
 
     const int nr = c.n_rows, D = c.p.link_step;
-    const int S = min(v.seed_start[v.n_bins], v.S_cap);
     volatile int32_t* const abort = &sm.abort;
     uint32_t it = 0, tphase = 0;      // rows through the ring so far (the same count in every warp); phase of tbar (warp 0)
     int phase = 0;                    // 0: a sector task is due; 1: up sweep; 2: down sweep
@@ -485,7 +505,7 @@ const __grid_constant__ View v, const __grid_constant__ Const c, const int cap_s
             if (row > last) continue;                            // no start hit in this sector
             phase = 1;
             if (warp == 0 && lane == 0)                          // the ring is empty: its first rows
-                for (int k = 0; k < kCtRing; k++) if (row + k <= last) ct_issue(v, sm, row + k, false, tb, it + k, S);
+                for (int k = 0; k < kCtRing; k++) if (row + k <= last) ct_issue(v, sm, row + k, false, tb, it + k);
         }
         const bool up = phase == 1;
         const int s = (int)(it % kCtRing);
@@ -522,7 +542,7 @@ const __grid_constant__ View v, const __grid_constant__ Const c, const int cap_s
             Fit& f = t.f;
             uint16_t* const gt = v.tl_tab + (size_t)(on ? t.i : 0) * v.tab_stride;
             bool end = false, search = false, counted = false, vis = false;
-            int acc = -1, nn = -1;
+            int acc = -1;
             uint16_t eold = kNoHit;
             float ay = 0.f, az = 0.f, iwy = 0.f, iwz = 0.f;
             // part 1: transport and the candidate that is already known
@@ -535,8 +555,10 @@ const __grid_constant__ View v, const __grid_constant__ Const c, const int cap_s
                         const float2 hk = hits[t.cur - dn.x]; ky = hk.x; kz = hk.y;
                     }
                 } else if (row >= t.r0) {
-                    eold = (uint16_t)t.cur;
-                    if (row > t.r0) t.cur = gt[row - 1];
+                    // the slot's word 29 holds the 4-byte word of the tracklet's table with this row's entry; the one with
+                    // the entry of the row below is fetched now and read at the next row
+                    eold = (uint16_t)((uint32_t)t.cur >> (16 * (row & 1)));
+                    if (row > t.r0) sl.fetch(slot, 29, gt + ((row - 1) & ~1));
                     if (eold != kNoHit) { known = dn.x + eold; const float2 hk = hits[eold]; ky = hk.x; kz = hk.y; }
                 }
                 end = !fit_transport(f, c.row_x[up ? row - 1 : row + 1], c.row_x[row], c);
@@ -552,9 +574,9 @@ const __grid_constant__ View v, const __grid_constant__ Const c, const int cap_s
                     if (up) {
                         if (t.ph == 1) {
                             if (row == t.aux) {
-                                // the link above the next linked hit: needed one link from now, the load has a whole row
-                                if (gate_ok && t.nxt >= 0) nn = __ldg(&v.clink_up[t.nxt]);
-                                if (gate_ok) { t.cur = t.nxt; t.nxt = nn; t.aux += D; if (t.cur < 0) t.ph = 2; }
+                                // the link above the next linked hit (needed one link from now) is fetched into the slot
+                                if (gate_ok && t.nxt >= 0) sl.fetch(slot, 31, &v.clink_up[t.nxt]);
+                                if (gate_ok) { t.cur = t.nxt; t.aux += D; if (t.cur < 0) t.ph = 2; }
                                 else { t.ph = 2; search = true; counted = true; }
                             }   // else: in-between row of a step-2 link
                         } else {
@@ -630,7 +652,7 @@ const __grid_constant__ View v, const __grid_constant__ Const c, const int cap_s
                     v.tl_par[4 * sc + t.i] = p4; v.tl_par[5 * sc + t.i] = t.p5;
                 }
             } else if (on) {
-                sl.store(t, slot);
+                sl.store(t, slot, up);
             }
             const unsigned gone = __ballot_sync(kFull, fin);    // this warp alone owns the group's occupancy word now
             const unsigned nvis = __popc(__ballot_sync(kFull, vis)), nupd = __popc(__ballot_sync(kFull, upd));
@@ -640,13 +662,14 @@ const __grid_constant__ View v, const __grid_constant__ Const c, const int cap_s
             }
             if (fin) ct_push(sm, freel, slot, cap);
         }
+        asm volatile("cp.async.wait_all;" ::: "memory");   // this warp's fetches into its slots have landed
         // up sweep: the start hits of this row are taken in AFTER it is processed (its marks are complete); the marks'
         // other buffer is cleared here for the next row if start hits wait there (its last readers, the intake two rows
         // down, are behind that row's barriers)
         const bool next_intake = up && row + 1 < nr && sm.cnt[row + 1] > 0;
         if (up && (intake || next_intake)) {
             ct_bar<W>();
-            if (intake) ct_intake_up<W, G>(v, c, sm, sl, freel, cap, row, s, S);
+            if (intake) ct_intake_up<W, G>(v, c, sm, sl, freel, cap, row, s, sm.S);
             if (next_intake)
                 for (int k = threadIdx.x; k < TPC_MAX_ROW_HITS / 32; k += W * 32) sm.used[(row + 1) & 1][k] = 0u;
             ct_bar<W>();
@@ -658,7 +681,7 @@ const __grid_constant__ View v, const __grid_constant__ Const c, const int cap_s
             if (atomicAdd(&sm.rel[s], 1) == W - 1) {
                 sm.rel[s] = 0;
                 const int r2 = up ? row + kCtRing : row - kCtRing;
-                if (up ? r2 <= last : r2 >= last) ct_issue(v, sm, r2, !up, tb, it + kCtRing, S);
+                if (up ? r2 <= last : r2 >= last) ct_issue(v, sm, r2, !up, tb, it + kCtRing);
             }
         }
         it++;
@@ -673,7 +696,7 @@ const __grid_constant__ View v, const __grid_constant__ Const c, const int cap_s
         if (row < 0) { phase = 0; continue; }
         phase = 2;
         if (warp == 0 && lane == 0)
-            for (int k = 0; k < kCtRing; k++) if (row - k >= 0) ct_issue(v, sm, row - k, true, tb, it + k, S);
+            for (int k = 0; k < kCtRing; k++) if (row - k >= 0) ct_issue(v, sm, row - k, true, tb, it + k);
     }
     __syncwarp();
     if (lane == 0) {
