@@ -133,15 +133,30 @@ __global__ void __launch_bounds__(256) k_scatter(const View v, int ns, int nr) {
 constexpr int kSortThreads = TPC_SORT_THREADS;
 constexpr int kSortReg = 4;
 
-__global__ void __launch_bounds__(kSortThreads) k_sort_row(const View v) {
-    __shared__ int cnt[kMaxCells + 1];                    // hits per cell, then first hit of each cell
-    __shared__ uint16_t ck[TPC_MAX_ROW_HITS];             // cell of hit k       } larger bins only
-    __shared__ uint16_t rk[TPC_MAX_ROW_HITS];             // arrival rank of hit k inside its cell
+// SMALL: the bins of up to kSortReg * kSortThreads hits (little shared memory: many CTAs per SM); the other launch
+// takes the larger ones
+#ifndef TPC_SORT_BLOCKS
+#define TPC_SORT_BLOCKS 12
+#endif
+template <bool SMALL>
+__global__ void __launch_bounds__(kSortThreads, SMALL ? TPC_SORT_BLOCKS : 7) k_sort_row(const View v) {
+    constexpr int kCells = SMALL ? kCellsPerHit * kSortReg * kSortThreads + kCellPad : kMaxCells;
+    __shared__ int cnt[kCells + 1];                                   // hits per cell, then first hit of each cell
+    __shared__ uint16_t ck[SMALL ? 1 : TPC_MAX_ROW_HITS];             // cell of hit k
+    __shared__ uint16_t rk[SMALL ? 1 : TPC_MAX_ROW_HITS];             // arrival rank of hit k inside its cell
     __shared__ float red[4][kSortThreads / 32];
     __shared__ int scan_total;
-    const int bin = blockIdx.x;
+    // SMALL: a CTA per bin, the larger bins are listed (in seed_count, free until K3); the other launch is a fixed
+    // grid that takes the listed bins in turn
+    for (int bi = blockIdx.x; SMALL ? bi == (int)blockIdx.x : bi < (int)v.cnt[CNT_LARGE_BINS]; bi += gridDim.x) {
+    const int bin = SMALL ? bi : v.seed_count[bi];
     const int b0 = v.bin_start[bin];
     const int n = min(v.bin_start[bin + 1] - b0, TPC_MAX_ROW_HITS);
+    if (SMALL && n > kSortReg * kSortThreads) {
+        if (threadIdx.x == 0) v.seed_count[(int)atomicAdd(&v.cnt[CNT_LARGE_BINS], 1ull)] = bin;
+        return;
+    }
+    if (!SMALL) __syncthreads();   // the shared arrays are free again
     uint16_t* cs = v.cells + (size_t)kCellsPerHit * b0 + (size_t)bin * kCellPad;
     if (n == 0) {
         if (threadIdx.x == 0) {
@@ -151,7 +166,7 @@ __global__ void __launch_bounds__(kSortThreads) k_sort_row(const View v) {
         }
         return;
     }
-    const bool small = n <= kSortReg * kSortThreads;
+    constexpr bool small = SMALL;
     float2 hr[kSortReg];
     int ir[kSortReg];
     // bounding box
@@ -249,6 +264,7 @@ __global__ void __launch_bounds__(kSortThreads) k_sort_row(const View v) {
     if (threadIdx.x == 0) {
         BinDesc d; d.y0 = ymin; d.z0 = zmin; d.idy = idy; d.idz = idz; d.base = b0; d.n = n; d.ny = ny; d.nz = nz;
         v.desc[bin] = d;
+    }
     }
 }
 

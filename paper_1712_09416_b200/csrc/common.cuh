@@ -30,7 +30,7 @@ constexpr unsigned kErrFatal = kErrBadRow | kErrRowCapacity | kErrBadInput;   //
 
 // device counters (unsigned long long each)
 constexpr int kNCursors = 4;           // work cursors: [0] K5 sector tasks, [2] refit
-enum { CNT_ERR = 0, CNT_LINKS, CNT_ROW_VISITS, CNT_TL_HITS, CNT_TRACKS, CNT_TRACK_HITS, CNT_UPDATES, CNT_REFIT_VISITS, CNT_TRACKLETS, CNT_PROF, CNT_N = CNT_PROF + 16 };
+enum { CNT_ERR = 0, CNT_LINKS, CNT_ROW_VISITS, CNT_TL_HITS, CNT_TRACKS, CNT_TRACK_HITS, CNT_UPDATES, CNT_REFIT_VISITS, CNT_TRACKLETS, CNT_LARGE_BINS, CNT_PROF, CNT_N = CNT_PROF + 16 };
 
 // One event's input arrays (device pointers) and its place in the batch-global cluster numbering.
 struct EventSrc {

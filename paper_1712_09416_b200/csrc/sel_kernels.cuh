@@ -41,6 +41,8 @@ __device__ __forceinline__ void sel_chunk(const View& v, int tb, int nr, int c, 
 __global__ void __launch_bounds__(kSelCtaThreads, 2) k_select_claim(const View v, const __grid_constant__ Const c) {
     extern __shared__ uint32_t s_owner[];
     __shared__ int32_t s_base[TPC_MAX_ROWS + 2];
+    __shared__ uint16_t s_list[kSelTile];   // the tracklets of a tile that take part (offsets into the tile)
+    __shared__ int32_t s_n;
     __shared__ unsigned long long s_claimed;
     TPC_RETURN_IF_REJECTED(v);
     const int C = v.sel_C, nr = c.n_rows;
@@ -63,33 +65,52 @@ __global__ void __launch_bounds__(kSelCtaThreads, 2) k_select_claim(const View v
     // The task's row -> hit tables are one contiguous block; a thread takes 8 consecutive rows of one tracklet
     // (one 16-byte load), so the block streams through with every load independent of the others.
     const int g_lo = r_lo >> 3, G = max(((r_hi - 1) >> 3) - g_lo + 1, 1);   // (an empty chunk has r_hi == r_lo)
-    const int n_units = (i1 - i0) * G;
     unsigned claimed = 0;
+    // The tracklets that take part (with the seed de-duplication two start hits in three build none) are listed
+    // first, kSelTile start hits at a time, so that the lanes of the two passes are all at work.
     for (int pass = 0; pass < 2; pass++) {
-        for (int u = threadIdx.x; u < n_units; u += kSelCtaThreads) {
-            const int j = u / G, g = g_lo + (u - j * G);
-            const int i = i0 + j;
-            const int pk = v.tl_rows[i];
-            const int nh = pk >> 16;
-            if (nh < c.p.min_tracklet_hits) continue;
-            const int a = max(pk & 0xff, r_lo), b = min((pk >> 8) & 0xff, r_hi - 1);
-            const int r8 = g << 3;
-            if (r8 > b || r8 + 7 < a) continue;
-            const uint32_t key = ((uint32_t)nh << 24) | (uint32_t)(0xffffff - j);
-            const uint4 q = *reinterpret_cast<const uint4*>(v.tl_tab + (size_t)i * v.tab_stride + r8);
-            const uint32_t w[4] = {q.x, q.y, q.z, q.w};
-            int own = 0;
-#pragma unroll
-            for (int k = 0; k < 8; k++) {
-                const uint32_t e = (w[k >> 1] >> ((k & 1) * 16)) & 0xffffu;
-                const int r = r8 + k;
-                if (e != kNoHit && r >= a && r <= b) {
-                    uint32_t* o = &s_owner[s_base[r - r_lo] - h_lo + (int)e];
-                    if (pass == 0) { atomicMax(o, key); claimed++; }
-                    else own += (*o == key);
+        for (int tile = i0; tile < i1; tile += kSelTile) {
+            __syncthreads();
+            if (threadIdx.x == 0) s_n = 0;
+            __syncthreads();
+            for (int k = threadIdx.x; k < kSelTile; k += kSelCtaThreads) {
+                const int i = tile + k;
+                bool live = false;
+                if (i < i1) {
+                    const int pk = v.tl_rows[i];
+                    live = (pk >> 16) >= c.p.min_tracklet_hits && max(pk & 0xff, r_lo) <= min((pk >> 8) & 0xff, r_hi - 1);
                 }
+                const unsigned m = __ballot_sync(kFull, live);
+                int base = 0;
+                if (lane == 0 && m) base = atomicAdd(&s_n, __popc(m));
+                base = __shfl_sync(kFull, base, 0);
+                if (live) s_list[base + __popc(m & lanemask_lt())] = (uint16_t)k;
             }
-            if (pass == 1 && own) atomicAdd(&v.tl_cnt[(size_t)ch * v.S_cap + i], own);
+            __syncthreads();
+            const int n_units = s_n * G;
+            for (int u = threadIdx.x; u < n_units; u += kSelCtaThreads) {
+                const int q = u / G, g = g_lo + (u - q * G);
+                const int i = tile + (int)s_list[q], pk = v.tl_rows[i];
+                const int nh = pk >> 16;
+                const int a = max(pk & 0xff, r_lo), b = min((pk >> 8) & 0xff, r_hi - 1);
+                const int r8 = g << 3;
+                if (r8 > b || r8 + 7 < a) continue;
+                const uint32_t key = ((uint32_t)nh << 24) | (uint32_t)(0xffffff - (i - i0));
+                const uint4 qw = *reinterpret_cast<const uint4*>(v.tl_tab + (size_t)i * v.tab_stride + r8);
+                const uint32_t w[4] = {qw.x, qw.y, qw.z, qw.w};
+                int own = 0;
+#pragma unroll
+                for (int k = 0; k < 8; k++) {
+                    const uint32_t e = (w[k >> 1] >> ((k & 1) * 16)) & 0xffffu;
+                    const int r = r8 + k;
+                    if (e != kNoHit && r >= a && r <= b) {
+                        uint32_t* o = &s_owner[s_base[r - r_lo] - h_lo + (int)e];
+                        if (pass == 0) { atomicMax(o, key); claimed++; }
+                        else own += (*o == key);
+                    }
+                }
+                if (pass == 1 && own) atomicAdd(&v.tl_cnt[(size_t)ch * v.S_cap + i], own);
+            }
         }
         __syncthreads();
     }

@@ -303,7 +303,8 @@ int launch_all(const tpc_tracker* tr, Batch* t, int from = 1) {
             dim3 g((maxn + kScatterChunk - 1) / kScatterChunk, t->n_events);
             k_scatter<<<g, 256, 0, st>>>(v, ns, nr); L++;
         }
-        k_sort_row<<<nb, kSortThreads, 0, st>>>(v); L++;
+        k_sort_row<true><<<nb, kSortThreads, 0, st>>>(v); L++;
+        k_sort_row<false><<<std::min(nb, 7 * tr->sm_count), kSortThreads, 0, st>>>(v); L++;
     }
     mark(1);
     if (from <= 2) { k_neighbours<<<nb, kNfThreads, 0, st>>>(v, c); L++; }
