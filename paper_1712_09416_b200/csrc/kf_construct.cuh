@@ -266,31 +266,46 @@ struct CtTrk {
     int nxt;                        // up: the hit linked above cur (read one link ahead)
     int ph, miss, r0, top, aux;     // ph 1 up/follow, 2 up/extend, 3 down; aux: up = row of cur, down = first row
 };
-__device__ __forceinline__ void ct_load(CtTrk& t, const float* S, int cap) {
+// A slot's 32 words sit in eight groups of four: word k of slot s of a pool of `cap` slots is float
+// ((k / 4) * cap + s) * 4 + k % 4, so that the 32 lanes of a warp move four words each with one conflict-free 16-byte
+// access.  Groups: (y z s t) (q c00 c10 c11) (c20 c21 c22 c30) (c31 c32 c33 c40) (c41 c42 c43 c44)
+// (chi2 n | snapshot y z) (snapshot s t q | p5) (i cur packed nxt).
+__device__ __forceinline__ float* ct_word(float* B, int slot, int cap, int k) { return B + ((((k >> 2) * cap) + slot) << 2) + (k & 3); }
+__device__ __forceinline__ void ct_load(CtTrk& t, float* B, int slot, int cap) {
     Fit& f = t.f;
-    f.y = S[0]; f.z = S[cap]; f.s = S[2 * cap]; f.t = S[3 * cap]; f.q = S[4 * cap];
-    f.c00 = S[5 * cap]; f.c10 = S[6 * cap]; f.c11 = S[7 * cap]; f.c20 = S[8 * cap]; f.c21 = S[9 * cap];
-    f.c22 = S[10 * cap]; f.c30 = S[11 * cap]; f.c31 = S[12 * cap]; f.c32 = S[13 * cap]; f.c33 = S[14 * cap];
-    f.c40 = S[15 * cap]; f.c41 = S[16 * cap]; f.c42 = S[17 * cap]; f.c43 = S[18 * cap]; f.c44 = S[19 * cap];
-    f.chi2 = S[20 * cap]; f.n = __float_as_int(S[21 * cap]);
-    t.p5 = S[27 * cap];
-    t.i = __float_as_int(S[28 * cap]); t.cur = __float_as_int(S[29 * cap]); t.nxt = __float_as_int(S[31 * cap]);
-    const uint32_t pk = __float_as_uint(S[30 * cap]);
+    const float4 g0 = *reinterpret_cast<const float4*>(ct_word(B, slot, cap, 0));
+    const float4 g1 = *reinterpret_cast<const float4*>(ct_word(B, slot, cap, 4));
+    const float4 g2 = *reinterpret_cast<const float4*>(ct_word(B, slot, cap, 8));
+    const float4 g3 = *reinterpret_cast<const float4*>(ct_word(B, slot, cap, 12));
+    const float4 g4 = *reinterpret_cast<const float4*>(ct_word(B, slot, cap, 16));
+    const float2 g5 = *reinterpret_cast<const float2*>(ct_word(B, slot, cap, 20));
+    const float4 g7 = *reinterpret_cast<const float4*>(ct_word(B, slot, cap, 28));
+    f.y = g0.x; f.z = g0.y; f.s = g0.z; f.t = g0.w;
+    f.q = g1.x; f.c00 = g1.y; f.c10 = g1.z; f.c11 = g1.w;
+    f.c20 = g2.x; f.c21 = g2.y; f.c22 = g2.z; f.c30 = g2.w;
+    f.c31 = g3.x; f.c32 = g3.y; f.c33 = g3.z; f.c40 = g3.w;
+    f.c41 = g4.x; f.c42 = g4.y; f.c43 = g4.z; f.c44 = g4.w;
+    f.chi2 = g5.x; f.n = __float_as_int(g5.y);
+    t.p5 = *ct_word(B, slot, cap, 27);
+    t.i = __float_as_int(g7.x); t.cur = __float_as_int(g7.y); t.nxt = __float_as_int(g7.w);
+    const uint32_t pk = __float_as_uint(g7.z);
     t.ph = pk & 3u; t.miss = (pk >> 2) & 63u; t.r0 = (pk >> 8) & 255u; t.top = (pk >> 16) & 255u; t.aux = pk >> 24;
 }
-__device__ __forceinline__ void ct_store(const CtTrk& t, float* S, int cap, bool up) {
+// first: the slot is being filled (word 28, the tracklet, never changes afterwards)
+__device__ __forceinline__ void ct_store(const CtTrk& t, float* B, int slot, int cap, bool up, bool first = false) {
     const Fit& f = t.f;
-    S[0] = f.y; S[cap] = f.z; S[2 * cap] = f.s; S[3 * cap] = f.t; S[4 * cap] = f.q;
-    S[5 * cap] = f.c00; S[6 * cap] = f.c10; S[7 * cap] = f.c11; S[8 * cap] = f.c20; S[9 * cap] = f.c21;
-    S[10 * cap] = f.c22; S[11 * cap] = f.c30; S[12 * cap] = f.c31; S[13 * cap] = f.c32; S[14 * cap] = f.c33;
-    S[15 * cap] = f.c40; S[16 * cap] = f.c41; S[17 * cap] = f.c42; S[18 * cap] = f.c43; S[19 * cap] = f.c44;
-    S[20 * cap] = f.chi2; S[21 * cap] = __int_as_float(f.n);
-    S[27 * cap] = t.p5;
-    S[28 * cap] = __int_as_float(t.i);
-    if (up) S[29 * cap] = __int_as_float(t.cur);   // down: written by the asynchronous copy of the table word (see the row step)
+    *reinterpret_cast<float4*>(ct_word(B, slot, cap, 0)) = make_float4(f.y, f.z, f.s, f.t);
+    *reinterpret_cast<float4*>(ct_word(B, slot, cap, 4)) = make_float4(f.q, f.c00, f.c10, f.c11);
+    *reinterpret_cast<float4*>(ct_word(B, slot, cap, 8)) = make_float4(f.c20, f.c21, f.c22, f.c30);
+    *reinterpret_cast<float4*>(ct_word(B, slot, cap, 12)) = make_float4(f.c31, f.c32, f.c33, f.c40);
+    *reinterpret_cast<float4*>(ct_word(B, slot, cap, 16)) = make_float4(f.c41, f.c42, f.c43, f.c44);
+    *reinterpret_cast<float2*>(ct_word(B, slot, cap, 20)) = make_float2(f.chi2, __int_as_float(f.n));
+    *ct_word(B, slot, cap, 27) = t.p5;
+    if (first) *ct_word(B, slot, cap, 28) = __int_as_float(t.i);
+    if (up) *ct_word(B, slot, cap, 29) = __int_as_float(t.cur);   // down: written by the asynchronous copy of the table word (see the row step)
     // word 31 (nxt): written at the intake and by the asynchronous copy of the next link
-    S[30 * cap] = __uint_as_float((uint32_t)t.ph | ((uint32_t)t.miss << 2) | ((uint32_t)t.r0 << 8) |
-                                  ((uint32_t)t.top << 16) | ((uint32_t)t.aux << 24));
+    *ct_word(B, slot, cap, 30) = __uint_as_float((uint32_t)t.ph | ((uint32_t)t.miss << 2) | ((uint32_t)t.r0 << 8) |
+                                                 ((uint32_t)t.top << 16) | ((uint32_t)t.aux << 24));
 }
 
 // slot -> where its state lives: the first cap_s slots in shared memory, the others in this CTA's stretch of
@@ -299,29 +314,34 @@ template <bool G>   // G: the tier has slots in global memory
 struct CtSlots {
     float* st; float* gs; int cap_s, cap_g;
     __device__ __forceinline__ void load(CtTrk& t, int slot) const {
-        if (!G || slot < cap_s) ct_load(t, st + slot, cap_s); else ct_load(t, gs + (slot - cap_s), cap_g);
+        if (!G || slot < cap_s) ct_load(t, st, slot, cap_s); else ct_load(t, gs, slot - cap_s, cap_g);
     }
-    __device__ __forceinline__ void store(const CtTrk& t, int slot, bool up) const {
-        if (!G || slot < cap_s) ct_store(t, st + slot, cap_s, up); else ct_store(t, gs + (slot - cap_s), cap_g, up);
+    __device__ __forceinline__ void store(const CtTrk& t, int slot, bool up, bool first = false) const {
+        if (!G || slot < cap_s) ct_store(t, st, slot, cap_s, up, first); else ct_store(t, gs, slot - cap_s, cap_g, up, first);
     }
     // word k of a slot
     __device__ __forceinline__ float* word(int slot, int k) const {
-        if (!G || slot < cap_s) return st + slot + k * cap_s;
-        return gs + (slot - cap_s) + k * cap_g;
+        if (!G || slot < cap_s) return ct_word(st, slot, cap_s, k);
+        return ct_word(gs, slot - cap_s, cap_g, k);
     }
     // word k of a slot := the 4 bytes at src, without waiting for them: an asynchronous copy for a slot in shared memory
     // (the warp waits for its copies when it is through with the row), a plain load and store for one in global memory
     __device__ __forceinline__ void fetch(int slot, int k, const void* src) const {
         if (!G || slot < cap_s) {
-            asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(smem_u32(st + slot + k * cap_s)), "l"(src) : "memory");
+            asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(smem_u32(ct_word(st, slot, cap_s, k))), "l"(src) : "memory");
         } else {
-            gs[(slot - cap_s) + k * cap_g] = __ldg(reinterpret_cast<const float*>(src));
+            *ct_word(gs, slot - cap_s, cap_g, k) = __ldg(reinterpret_cast<const float*>(src));
         }
     }
-    // words 22.. of a slot: the state right after the last accepted update
-    __device__ __forceinline__ float* snap(int slot, int& stride) const {
-        if (!G || slot < cap_s) { stride = cap_s; return st + slot + 22 * cap_s; }
-        stride = cap_g; return gs + (slot - cap_s) + 22 * cap_g;
+    // the state right after the last accepted update: words 22, 23 (y, z) and 24..27 (sin phi, tg lambda, q/pT, p5)
+    __device__ __forceinline__ void snap_put(int slot, float y, float z, float s, float t, float q, float p5) const {
+        *reinterpret_cast<float2*>(word(slot, 22)) = make_float2(y, z);
+        *reinterpret_cast<float4*>(word(slot, 24)) = make_float4(s, t, q, p5);
+    }
+    __device__ __forceinline__ void snap_get(int slot, float& y, float& z, float& s, float& t, float& q) const {
+        const float2 a = *reinterpret_cast<const float2*>(word(slot, 22));
+        const float4 b = *reinterpret_cast<const float4*>(word(slot, 24));
+        y = a.x; z = a.y; s = b.x; t = b.y; q = b.z;
     }
 };
 
@@ -372,13 +392,12 @@ __device__ TPC_CT_INL void ct_intake_down(const View& v, const Const& c, CtSmem&
             fit_prior(t.f, c); t.f.n = 1;
             t.aux = top; t.miss = 0; t.ph = 3; t.nxt = -1;
             t.cur = 0;
-            sl.store(t, slot, false);
+            sl.store(t, slot, false, true);
             {   // table entry of the row below the top hit, in both halves of the word (see the row step)
                 const uint32_t below = (uint32_t)__float_as_int(b4.z) & 0xffffu;
                 *sl.word(slot, 29) = __uint_as_float(below | (below << 16));
             }
-            int sn; float* const P = sl.snap(slot, sn);
-            P[0] = a4.x; P[sn] = a4.y; P[2 * sn] = a4.z; P[3 * sn] = a4.w; P[4 * sn] = b4.x;
+            sl.snap_put(slot, a4.x, a4.y, a4.z, a4.w, b4.x, t.p5);
         }
     }
 }
@@ -419,10 +438,9 @@ __device__ TPC_CT_INL void ct_intake_up(const View& v, const Const& c, CtSmem& s
             t.p5 = __uint_as_float(((uint32_t)kNoHit << 16) | (uint32_t)hl);   // table entries: below the top hit | of the row before
             t.i = e; t.cur = hh.y; t.nxt = hh.z; t.ph = 1; t.miss = 0; t.r0 = row; t.top = row; t.aux = row + D;
             v.tl_tab[(size_t)e * v.tab_stride + row] = (uint16_t)hl;
-            sl.store(t, slot, true);
+            sl.store(t, slot, true, true);
             *sl.word(slot, 31) = __int_as_float(t.nxt);
-            int sn; float* const P = sl.snap(slot, sn);
-            P[0] = a4.x; P[sn] = a4.y; P[2 * sn] = a4.z; P[3 * sn] = a4.w; P[4 * sn] = 0.f;
+            sl.snap_put(slot, a4.x, a4.y, a4.z, a4.w, 0.f, t.p5);
         }
     }
 }
@@ -620,22 +638,22 @@ const __grid_constant__ View v, const __grid_constant__ Const c, const int cap_s
             __syncwarp();
             if (upd) {
                 fit_update(f, ay, az, iwy, c);
-                int sn; float* const P = sl.snap(slot, sn);
                 if (up) {
-                    P[0] = ay; P[sn] = az; P[2 * sn] = f.s; P[3 * sn] = f.t; P[4 * sn] = f.q; t.top = row;
+                    sl.snap_put(slot, ay, az, f.s, f.t, f.q, t.p5); t.top = row;
                     if (intake) {                               // seed de-duplication: this hit is being followed
                         const int hl = acc - dn.x;              // (marks matter only where start hits wait)
                         atomicOr(&sm.used[row & 1][hl >> 5], 1u << (hl & 31));
                     }
                 } else {
-                    P[0] = f.y; P[sn] = f.z; P[2 * sn] = f.s; P[3 * sn] = f.t; P[4 * sn] = f.q; t.p5 = f.chi2; t.aux = row;
+                    t.p5 = f.chi2; t.aux = row;
+                    sl.snap_put(slot, f.y, f.z, f.s, f.t, f.q, t.p5);
                 }
             }
             __syncwarp();
             const bool fin = on && (end || row == (up ? nr - 1 : 0));
             if (fin) {
-                int sn; const float* const P = sl.snap(slot, sn);
-                const float p0 = P[0], p1 = P[sn], p2 = P[2 * sn], p3 = P[3 * sn], p4 = P[4 * sn];
+                float p0, p1, p2, p3, p4;
+                sl.snap_get(slot, p0, p1, p2, p3, p4);
                 if (up) {   // park: a fresh fit will start at the top hit in the down sweep
                     float4* dst = reinterpret_cast<float4*>(&v.tl_up[t.i]);
                     const int below = t.top > t.r0 ? (int)(__float_as_uint(t.p5) >> 16) : (int)kNoHit;
