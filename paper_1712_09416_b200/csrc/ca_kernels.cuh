@@ -464,28 +464,37 @@ __global__ void __launch_bounds__(kCleanThreads) k_clean(const View v) {
 // K4 start-hit compaction in canonical order (task, row, caller's index): K3 collected the row's start hits with
 // warp ballots + prefix popcounts; here a rank by caller's index orders them.
 // ---------------------------------------------------------------------------------------------------------
-constexpr int kSeedThreads = 128;
+constexpr int kSeedThreads = 256;
+constexpr int kSeedWarps = kSeedThreads / 32;   // a warp per bin: no block barrier, eight bins per CTA
+constexpr int kSeedList = 128;                  // start hits of a bin ranked from shared memory; more: from global memory
 
 __global__ void __launch_bounds__(kSeedThreads) k_seeds(const View v, const __grid_constant__ Const c) {
-    __shared__ int list_h[TPC_MAX_ROW_HITS];
-    __shared__ int list_o[TPC_MAX_ROW_HITS];
+    __shared__ int list_h[kSeedWarps][kSeedList];
+    __shared__ int list_o[kSeedWarps][kSeedList];
     TPC_RETURN_IF_REJECTED(v);
-    const int bin = blockIdx.x;
+    const int warp = threadIdx.x >> 5, lane = lane_id();
+    const int bin = blockIdx.x * kSeedWarps + warp;
+    if (bin >= v.n_bins) return;
     const int s0 = v.seed_start[bin], ns = v.seed_start[bin + 1] - s0;
     if (ns == 0) return;
     const int b0 = v.bin_start[bin];
-    for (int i = threadIdx.x; i < ns; i += kSeedThreads) {   // the list K3 left (any order)
-        const int h = v.tidx[b0 + i];
-        list_h[i] = h;
-        list_o[i] = v.sorig[h];
+    const bool staged = ns <= kSeedList;
+    if (staged) {
+        for (int i = lane; i < ns; i += 32) {   // the list K3 left (any order)
+            const int h = v.tidx[b0 + i];
+            list_h[warp][i] = h;
+            list_o[warp][i] = v.sorig[h];
+        }
+        __syncwarp();
     }
-    __syncthreads();
-    for (int i = threadIdx.x; i < ns; i += kSeedThreads) {
-        const int o = list_o[i];
+    for (int i = lane; i < ns; i += 32) {
+        const int h0 = staged ? list_h[warp][i] : v.tidx[b0 + i];
+        const int o = staged ? list_o[warp][i] : v.sorig[h0];
         int rank = 0;
-        for (int j = 0; j < ns; j++) rank += (list_o[j] < o);
+        if (staged) for (int j = 0; j < ns; j++) rank += (list_o[warp][j] < o);
+        else for (int j = 0; j < ns; j++) rank += (v.sorig[v.tidx[b0 + j]] < o);
         if (s0 + rank < v.S_cap) {
-            const int h0 = list_h[i], h1 = v.clink_up[h0];
+            const int h1 = v.clink_up[h0];
             v.seeds[s0 + rank] = h0; v.seed_bin[s0 + rank] = bin;
             const float2 a0 = v.shit[h0], a1 = v.shit[h1];
             // initial direction of the up pass: s = dy / dl, t = dz / dl along the first link

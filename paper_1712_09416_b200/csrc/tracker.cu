@@ -314,7 +314,7 @@ int launch_all(const tpc_tracker* tr, Batch* t, int from = 1) {
         else k_clean<false><<<nb, kCleanThreads, 0, st>>>(v);   // start hits of the cleaned links as they stand
         L++;
         L += scan_exclusive(v.seed_count, v.seed_start, nb, t->scratch.p, st);
-        k_seeds<<<nb, kSeedThreads, 0, st>>>(v, c); L++;
+        k_seeds<<<(nb + kSeedWarps - 1) / kSeedWarps, kSeedThreads, 0, st>>>(v, c); L++;
     }
     mark(3);
     if (from <= 5) {   // K5: one CTA per sector task, up sweep then down sweep (kf_construct.cuh)
