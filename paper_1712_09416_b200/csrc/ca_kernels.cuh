@@ -466,46 +466,72 @@ __global__ void __launch_bounds__(kCleanThreads) k_clean(const View v) {
 // ---------------------------------------------------------------------------------------------------------
 constexpr int kSeedThreads = 256;
 constexpr int kSeedWarps = kSeedThreads / 32;   // a warp per bin: no block barrier, eight bins per CTA
-constexpr int kSeedList = 128;                  // start hits of a bin ranked from shared memory; more: from global memory
+constexpr int kSeedList = 128;                  // start hits of a bin ranked by its warp; more (the lowest rows of a sector,
+                                                // where every long track starts): by the whole CTA afterwards
+
+// start hit number `rank` of bin `bin`: the canonical list and the record the up pass starts from
+__device__ __forceinline__ void seed_write(const View& v, const Const& c, int bin, int s0, int rank, int h0) {
+    if (s0 + rank >= v.S_cap) { atomicOr((unsigned int*)&v.cnt[CNT_ERR], kErrSeedCapacity); return; }
+    const int h1 = v.clink_up[h0];
+    v.seeds[s0 + rank] = h0; v.seed_bin[s0 + rank] = bin;
+    const float2 a0 = v.shit[h0], a1 = v.shit[h1];
+    // initial direction of the up pass: s = dy / dl, t = dz / dl along the first link
+    const int r = bin % c.n_rows;
+    const float dx = c.row_x[r + c.p.link_step] - c.row_x[r];
+    const float dy = a1.x - a0.x, dz = a1.y - a0.y;
+    const float dl = sqrtf(dx * dx + dy * dy);
+    float4* rec = reinterpret_cast<float4*>(v.seed_rec) + 2 * (size_t)(s0 + rank);
+    rec[0] = make_float4(a0.x, a0.y, dy / dl, dz / dl);
+    rec[1] = make_float4(__int_as_float(h0), __int_as_float(h1), __int_as_float(v.clink_up[h1]), 0.f);
+}
 
 __global__ void __launch_bounds__(kSeedThreads) k_seeds(const View v, const __grid_constant__ Const c) {
     __shared__ int list_h[kSeedWarps][kSeedList];
     __shared__ int list_o[kSeedWarps][kSeedList];
+    __shared__ int big_h[TPC_MAX_ROW_HITS], big_o[TPC_MAX_ROW_HITS];
+    __shared__ int s_big[kSeedWarps];
     TPC_RETURN_IF_REJECTED(v);
     const int warp = threadIdx.x >> 5, lane = lane_id();
-    const int bin = blockIdx.x * kSeedWarps + warp;
-    if (bin >= v.n_bins) return;
-    const int s0 = v.seed_start[bin], ns = v.seed_start[bin + 1] - s0;
-    if (ns == 0) return;
-    const int b0 = v.bin_start[bin];
-    const bool staged = ns <= kSeedList;
-    if (staged) {
-        for (int i = lane; i < ns; i += 32) {   // the list K3 left (any order)
-            const int h = v.tidx[b0 + i];
-            list_h[warp][i] = h;
-            list_o[warp][i] = v.sorig[h];
+    {
+        const int bin = blockIdx.x * kSeedWarps + warp;
+        int ns = 0, s0 = 0;
+        if (bin < v.n_bins) { s0 = v.seed_start[bin]; ns = v.seed_start[bin + 1] - s0; }
+        if (lane == 0) s_big[warp] = ns > kSeedList;
+        if (ns > 0 && ns <= kSeedList) {
+            const int b0 = v.bin_start[bin];
+            for (int i = lane; i < ns; i += 32) {   // the list K3 left (any order)
+                const int h = v.tidx[b0 + i];
+                list_h[warp][i] = h;
+                list_o[warp][i] = v.sorig[h];
+            }
+            __syncwarp();
+            for (int i = lane; i < ns; i += 32) {
+                const int o = list_o[warp][i];
+                int rank = 0;
+                for (int j = 0; j < ns; j++) rank += (list_o[warp][j] < o);
+                seed_write(v, c, bin, s0, rank, list_h[warp][i]);
+            }
         }
-        __syncwarp();
     }
-    for (int i = lane; i < ns; i += 32) {
-        const int h0 = staged ? list_h[warp][i] : v.tidx[b0 + i];
-        const int o = staged ? list_o[warp][i] : v.sorig[h0];
-        int rank = 0;
-        if (staged) for (int j = 0; j < ns; j++) rank += (list_o[warp][j] < o);
-        else for (int j = 0; j < ns; j++) rank += (v.sorig[v.tidx[b0 + j]] < o);
-        if (s0 + rank < v.S_cap) {
-            const int h1 = v.clink_up[h0];
-            v.seeds[s0 + rank] = h0; v.seed_bin[s0 + rank] = bin;
-            const float2 a0 = v.shit[h0], a1 = v.shit[h1];
-            // initial direction of the up pass: s = dy / dl, t = dz / dl along the first link
-            const int r = bin % c.n_rows;
-            const float dx = c.row_x[r + c.p.link_step] - c.row_x[r];
-            const float dy = a1.x - a0.x, dz = a1.y - a0.y;
-            const float dl = sqrtf(dx * dx + dy * dy);
-            float4* rec = reinterpret_cast<float4*>(v.seed_rec) + 2 * (size_t)(s0 + rank);
-            rec[0] = make_float4(a0.x, a0.y, dy / dl, dz / dl);
-            rec[1] = make_float4(__int_as_float(h0), __int_as_float(h1), __int_as_float(v.clink_up[h1]), 0.f);
-        } else atomicOr((unsigned int*)&v.cnt[CNT_ERR], kErrSeedCapacity);
+    __syncthreads();
+    for (int w = 0; w < kSeedWarps; w++) {
+        if (!s_big[w]) continue;   // (uniform)
+        const int bin = blockIdx.x * kSeedWarps + w;
+        const int s0 = v.seed_start[bin], ns = min(v.seed_start[bin + 1] - s0, TPC_MAX_ROW_HITS);
+        const int b0 = v.bin_start[bin];
+        __syncthreads();
+        for (int i = threadIdx.x; i < ns; i += kSeedThreads) {
+            const int h = v.tidx[b0 + i];
+            big_h[i] = h;
+            big_o[i] = v.sorig[h];
+        }
+        __syncthreads();
+        for (int i = threadIdx.x; i < ns; i += kSeedThreads) {
+            const int o = big_o[i];
+            int rank = 0;
+            for (int j = 0; j < ns; j++) rank += (big_o[j] < o);
+            seed_write(v, c, bin, s0, rank, big_h[i]);
+        }
     }
 }
 
