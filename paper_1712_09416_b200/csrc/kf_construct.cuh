@@ -2,15 +2,16 @@
 // shared memory, row data staged by TMA bulk copies.
 //
 // A CTA takes a sector task and sweeps its pad rows twice: upwards for the up passes, then downwards for the down
-// passes.  A producer warp streams the rows -- hits and grid cell table of row r, one
-// cp.async.bulk each, completion on an mbarrier -- through a ring of kCtRing shared-memory slots.  The Kalman
-// state of every tracklet under way (32 words) lives in a shared-memory slot; at each row the 9 consumer warps
-// take the occupied slots 32 at a time, load the states, advance them by that row (transport, linked / recorded hit
+// passes.  The rows -- hits and grid cell table of row r, one cp.async.bulk each, completion on an
+// mbarrier -- go through a ring of kCtRing shared-memory slots, refilled by whichever warp is last through a row
+// (there is no producer warp).  The Kalman state of every tracklet under way (32 words) lives in a shared-memory
+// slot; at each row the CTA's 12 warps take the occupied slots 32 at a time, load the states, advance them by that row (transport, linked / recorded hit
 // or window search in the staged row, update) and store them back.  All tracklets of the task are therefore at the
 // same row at the same time, which is what the seed de-duplication needs (R23): an up pass marks every
 // hit it records in a per-row bitmap; after a barrier the start hits of that row are taken in, and those already
 // marked build no tracklet.  A tracklet whose up pass has ended is parked (its top hit and direction, 32 bytes);
-// the down sweep picks it up at its top row.  Nothing depends on which warp or slot a tracklet lands in.
+// the down sweep takes the parked ones in kCtDnBatch rows at a time and starts each below its top row.  Nothing
+// depends on which warp or slot a tracklet lands in.
 //
 // The arithmetic is that of kf_kernels.cuh (fit_transport / fit_update), so every decision is the one DESIGN.md
 // "O5" describes.
@@ -20,10 +21,11 @@
 
 namespace tpc {
 
-// 9 consumer warps: 2 CTAs x 320 threads per SM leave 96 registers per thread and the row step does not spill.
-// Measured on config 5 (K5 alone): 13 warps (72 registers, 180 B of spills per thread, every spill an L2 round trip
-// because the shared-memory carve-out leaves ~10 KB of L1) 5.82 ms; 11 warps (80 registers, 52 B) 5.62 ms; 10 warps
-// 6.10 ms; 9 warps (no spill) 4.61 ms; 8 warps 4.70 ms.
+// 12 warps: 2 CTAs x 384 threads per SM leave 80 registers per thread (the register file is handed out per four
+// warps of a CTA: a thirteenth warp would cost every warp 16 registers).  Measured on config 5 (K5 alone), with a
+// producer warp: 13 + 1 warps (72 registers, 180 B of spills per thread, every spill an L2 round trip because the
+// shared-memory carve-out leaves ~10 KB of L1) 5.82 ms; 9 + 1 warps at 96 registers 4.50 ms; without one: 8 warps
+// 4.57 ms, 12 warps 4.40 ms.
 #ifndef TPC_CT_WARPS
 #define TPC_CT_WARPS 12
 #endif
@@ -136,7 +138,7 @@ __device__ __forceinline__ void bulk_g2s(void* dst, const void* src, uint32_t by
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                  ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
-// barrier of the consumer warps only (the producer never joins)
+// barrier of the CTA's W warps
 template <int W> __device__ __forceinline__ void ct_bar() { asm volatile("bar.sync 1, %0;" ::"n"(W * 32) : "memory"); }
 
 __device__ __forceinline__ size_t cell_index(int base, int bin) { return (size_t)kCellsPerHit * base + (size_t)bin * kCellPad; }
@@ -444,7 +446,7 @@ __device__ TPC_CT_INL void ct_intake_up(const View& v, const Const& c, CtSmem& s
         }
     }
 }
-// between the sweeps (all consumer warps): the parked tracklets of the task, ordered by top row, into dn_rec
+// between the sweeps (all warps): the parked tracklets of the task, ordered by top row, into dn_rec
 template <int W>
 __device__ TPC_CT_INL void ct_turn(const View& v, CtSmem& sm, int nr) {
     const int lane = lane_id(), warp = threadIdx.x >> 5;
@@ -472,7 +474,7 @@ __device__ TPC_CT_INL void ct_turn(const View& v, CtSmem& sm, int nr) {
         float4* dst = reinterpret_cast<float4*>(&v.dn_rec[sm.i0 + pos]);
         dst[0] = a4; dst[1] = b4;
     }
-    asm volatile("fence.proxy.async;" ::: "memory");   // the producer's bulk copies (async proxy) will read these records
+    asm volatile("fence.proxy.async;" ::: "memory");   // the bulk copies (async proxy) will read these records
     ct_bar<W>();
 }
 
@@ -535,7 +537,7 @@ const __grid_constant__ View v, const __grid_constant__ Const c, const int cap_s
         const float2* const hits = staged ? reinterpret_cast<const float2*>(sm.hits[s]) + (dn.x & 1) : v.shit + dn.x;
         const uint16_t* const cs = staged ? reinterpret_cast<const uint16_t*>(sm.cells[s]) + (cg & 7) : v.cells + cg;
 
-        // The consumer warps meet at barriers only around an intake: rows where nothing starts (most rows of a sparse
+        // The warps meet at barriers only around an intake: rows where nothing starts (most rows of a sparse
         // event) are processed by every warp on its own, up to a ring's depth apart.
         const bool intake = sm.cnt[row] > 0;
         int dn_lo = 0, dn_n = 0;
