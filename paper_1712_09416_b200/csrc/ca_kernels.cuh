@@ -118,7 +118,7 @@ __global__ void __launch_bounds__(256) k_scatter(const View v, int ns, int nr) {
     }
 #pragma unroll
     for (int j = 0; j < kScatterPer; j++)
-        if (pos[j] >= 0) { v.thit[pos[j]] = h[j]; v.tidx[pos[j]] = i0 + j * 256 + (int)threadIdx.x; }
+        if (pos[j] >= 0) v.thit[pos[j]] = make_float4(h[j].x, h[j].y, __int_as_float(i0 + j * 256 + (int)threadIdx.x), 0.f);   // one 16-byte store
 }
 
 // ---------------------------------------------------------------------------------------------------------
@@ -175,7 +175,7 @@ __global__ void __launch_bounds__(kSortThreads, SMALL ? TPC_SORT_BLOCKS : 7) k_s
 #pragma unroll
         for (int j = 0; j < kSortReg; j++) {
             const int k = j * kSortThreads + threadIdx.x;
-            if (k < n) { hr[j] = v.thit[b0 + k]; ir[j] = v.tidx[b0 + k]; }
+            if (k < n) { const float4 q = v.thit[b0 + k]; hr[j] = make_float2(q.x, q.y); ir[j] = __float_as_int(q.z); }
         }
 #pragma unroll
         for (int j = 0; j < kSortReg; j++)
@@ -184,7 +184,7 @@ __global__ void __launch_bounds__(kSortThreads, SMALL ? TPC_SORT_BLOCKS : 7) k_s
             }
     } else {
         for (int k = threadIdx.x; k < n; k += kSortThreads) {
-            const float2 h = v.thit[b0 + k];
+            const float4 h = v.thit[b0 + k];
             ymin = fminf(ymin, h.x); ymax = fmaxf(ymax, h.x); zmin = fminf(zmin, h.y); zmax = fmaxf(zmax, h.y);
         }
     }
@@ -228,7 +228,7 @@ __global__ void __launch_bounds__(kSortThreads, SMALL ? TPC_SORT_BLOCKS : 7) k_s
             }
     } else {
         for (int k = threadIdx.x; k < n; k += kSortThreads) {
-            const float2 h = v.thit[b0 + k];
+            const float4 h = v.thit[b0 + k];
             const int cell = grid_cell(h.y, zmin, idz, nz) * ny + grid_cell(h.x, ymin, idy, ny);
             ck[k] = (uint16_t)cell;
             rk[k] = (uint16_t)atomicAdd(&cnt[cell], 1);
@@ -257,8 +257,9 @@ __global__ void __launch_bounds__(kSortThreads, SMALL ? TPC_SORT_BLOCKS : 7) k_s
     } else {
         for (int k = threadIdx.x; k < n; k += kSortThreads) {
             const int pos = b0 + cnt[ck[k]] + rk[k];
-            v.shit[pos] = v.thit[b0 + k];
-            v.sorig[pos] = v.tidx[b0 + k];
+            const float4 q = v.thit[b0 + k];
+            v.shit[pos] = make_float2(q.x, q.y);
+            v.sorig[pos] = __float_as_int(q.z);
         }
     }
     if (threadIdx.x == 0) {

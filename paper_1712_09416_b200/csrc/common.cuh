@@ -70,7 +70,8 @@ struct View {
     int32_t* bin_count;      // [n_bins+1]
     int32_t* bin_start;      // [n_bins+1] exclusive scan of bin_count
     uint16_t* slot;          // [N] position of a cluster inside its bin, arrival order (batch-global cluster order)
-    float2* thit; int32_t* tidx;   // [N] bucketed, unsorted: (y,z), caller's index
+    float4* thit;            // [N] bucketed, unsorted: (y, z, caller's index, -) -- one 16-byte record per scattered store
+    int32_t* tidx;           // [N] scratch: K3's list of the start hits of each bin
     float2* shit; int32_t* sorig;  // [N] sorted by (task,row,cell): (y,z), caller's index in its event
     BinDesc* desc;           // [n_bins]
     uint16_t* cells;         // [kCellsPerHit*N + n_bins*kCellPad] first hit of each cell, relative to the bin's base

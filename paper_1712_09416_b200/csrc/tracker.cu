@@ -86,7 +86,8 @@ struct Batch {
     tpc_counters counters;                   // of the group's last run
     // device pools
     Buf<float> in_x, in_y, in_z, tl_par, o_f[kOutF];
-    Buf<float2> thit, shit;
+    Buf<float2> shit;
+    Buf<float4> thit;
     Buf<int32_t> in_row, sec_off, bin_count, bin_start, tidx, sorig, link_up, link_dn, clink_up, clink_dn, seed_count,
         seed_start, seeds, seed_bin, tl_rows, tl_nown, tl_keep, trk_scan, hit_scan, ev_off_d,
         o_i[kOutI], o_hit, trk_rows, trk_task, mg_list;
