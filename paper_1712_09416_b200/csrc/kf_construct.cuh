@@ -548,9 +548,6 @@ const __grid_constant__ View v, const __grid_constant__ Const c, const int cap_s
         }
         // ---- one pad row for the tracklets under way: the warps share the groups of 32 slots ----
         const int n_groups = (*(volatile int32_t*)&sm.n_hw + 31) >> 5;
-#ifdef TPC_CT_HIST
-        if (warp == 0 && lane == 0) atomicAdd(&v.cnt[CNT_PROF + min(n_groups, 15)], 1ull);
-#endif
         for (int g = warp; g < n_groups; g += W) {
             const uint32_t occ = *(volatile uint32_t*)&sm.occ[g];
             if (!occ) continue;

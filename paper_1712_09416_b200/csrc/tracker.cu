@@ -528,16 +528,6 @@ int batch_finish(const tpc_tracker* tr, Batch* t) {
         t->counters.n_updates = (int64_t)t->h_cnt.p[CNT_UPDATES];
         t->counters.n_refit_visits = (int64_t)t->h_cnt.p[CNT_REFIT_VISITS];
         t->counters.n_tracklets = (int64_t)t->h_cnt.p[CNT_TRACKLETS];
-#ifdef TPC_CT_HIST
-        fprintf(stderr, "K5 row steps by groups of 32 slots in use (0..15+):");
-        for (int k = 0; k < 16; k++) fprintf(stderr, " %.0f", (double)t->h_cnt.p[CNT_PROF + k]);
-        fprintf(stderr, "\n");
-#endif
-#ifdef TPC_CT_PROF
-        fprintf(stderr, "K5 warp-0 cycles by phase (0 wait-row, 1 intake-dn + barrier, 3 groups, 4 barrier, 5 intake-up + barrier, 7 loop):");
-        for (int k = 0; k < 14; k++) fprintf(stderr, " %.3g", (double)t->h_cnt.p[CNT_PROF + k]);
-        fprintf(stderr, "\n");
-#endif
         return TPC_OK;
     }
 }
