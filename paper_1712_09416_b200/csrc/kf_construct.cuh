@@ -312,9 +312,10 @@ __device__ __forceinline__ void ct_store(const CtTrk& t, float* B, int slot, int
 
 // slot -> where its state lives: the first cap_s slots in shared memory, the others in this CTA's stretch of
 // global memory (both multiples of 32, so a warp's 32 slots are all of one kind)
-template <bool G>   // G: the tier has slots in global memory
-struct CtSlots {
-    float* st; float* gs; int cap_s, cap_g;
+template <bool G, int CAPS>   // G: the tier has slots in global memory; CAPS: its slots in shared memory (a compile-time
+struct CtSlots {              // constant: the words of a slot are then at fixed offsets from one address)
+    static constexpr int cap_s = CAPS;
+    float* st; float* gs; int cap_g;
     __device__ __forceinline__ void load(CtTrk& t, int slot) const {
         if (!G || slot < cap_s) ct_load(t, st, slot, cap_s); else ct_load(t, gs, slot - cap_s, cap_g);
     }
@@ -370,8 +371,8 @@ __device__ __forceinline__ void ct_push(CtSmem& sm, uint16_t* freel, int slot, i
 // ---- intake, by all consumer threads between the row steps ----
 // down sweep: the parked tracklets whose top hit is in this row start a fresh fit there (their records come
 // ordered by top row: staged in the ring slot, the ones beyond kCtSeedStage read in place)
-template <int W, bool G>
-__device__ TPC_CT_INL void ct_intake_down(const View& v, const Const& c, CtSmem& sm, const CtSlots<G>& sl, const uint16_t* freel,
+template <int W, bool G, int CAPS>
+__device__ TPC_CT_INL void ct_intake_down(const View& v, const Const& c, CtSmem& sm, const CtSlots<G, CAPS>& sl, const uint16_t* freel,
                                             int cap, int rlo, int n, int s) {
     const int lo = sm.i0 + sm.lo[rlo];
     for (int j0 = 0; j0 < n; j0 += W * 32) {
@@ -404,8 +405,8 @@ __device__ TPC_CT_INL void ct_intake_down(const View& v, const Const& c, CtSmem&
     }
 }
 // up sweep: the start hits of this row that no up pass has recorded build a tracklet; returns how many (this thread)
-template <int W, bool G>
-__device__ TPC_CT_INL void ct_intake_up(const View& v, const Const& c, CtSmem& sm, const CtSlots<G>& sl, const uint16_t* freel,
+template <int W, bool G, int CAPS>
+__device__ TPC_CT_INL void ct_intake_up(const View& v, const Const& c, CtSmem& sm, const CtSlots<G, CAPS>& sl, const uint16_t* freel,
                                               int cap, int row, int s, int S) {
     const int D = c.p.link_step;
     const bool dedup = c.p.seed_dedup != 0;
@@ -481,20 +482,20 @@ __device__ TPC_CT_INL void ct_turn(const View& v, CtSmem& sm, int nr) {
 // ---------------------------------------------------------------------------------------------------------
 // K5
 // ---------------------------------------------------------------------------------------------------------
-template <int W, bool G>
+template <int W, bool G, int CAPS>
 #ifdef TPC_CT_MAXNREG
 __global__ void __maxnreg__(TPC_CT_MAXNREG) k_construct(
 #else
 __global__ void __launch_bounds__(W * 32, W <= 16 ? TPC_CT_MINB : 1) k_construct(
 #endif
-const __grid_constant__ View v, const __grid_constant__ Const c, const int cap_s,
-                                                             const int cap_g, float* const spill) {
+const __grid_constant__ View v, const __grid_constant__ Const c, const int cap_g, float* const spill) {
+    constexpr int cap_s = CAPS;
     extern __shared__ __align__(128) unsigned char ct_raw[];
     TPC_RETURN_IF_REJECTED(v);
     CtSmem& sm = *reinterpret_cast<CtSmem*>(ct_raw);
     const int cap = cap_s + cap_g;
-    CtSlots<G> sl;
-    sl.st = reinterpret_cast<float*>(ct_raw + sizeof(CtSmem)); sl.cap_s = cap_s; sl.cap_g = cap_g;
+    CtSlots<G, CAPS> sl;
+    sl.st = reinterpret_cast<float*>(ct_raw + sizeof(CtSmem)); sl.cap_g = cap_g;
     sl.gs = spill + (size_t)blockIdx.x * kCtWords * cap_g;
     uint16_t* const freel = reinterpret_cast<uint16_t*>(sl.st + (size_t)kCtWords * cap_s);   // stack of free slots
     const int warp = threadIdx.x >> 5, lane = lane_id();
@@ -543,7 +544,7 @@ const __grid_constant__ View v, const __grid_constant__ Const c, const int cap_s
         int dn_lo = 0, dn_n = 0;
         if (!up && ct_dn_intake_row(sm, row, dn_lo, dn_n)) {   // down sweep: what starts at these rows is taken in BEFORE
             ct_bar<W>();                                        // this row is processed; all slots freed by the rows above
-            ct_intake_down<W, G>(v, c, sm, sl, freel, cap, dn_lo, dn_n, s);   // are back on the stack
+            ct_intake_down<W, G, CAPS>(v, c, sm, sl, freel, cap, dn_lo, dn_n, s);   // are back on the stack
             ct_bar<W>();
         }
         // ---- one pad row for the tracklets under way: the warps share the groups of 32 slots ----
@@ -686,7 +687,7 @@ const __grid_constant__ View v, const __grid_constant__ Const c, const int cap_s
         const bool next_intake = up && row + 1 < nr && sm.cnt[row + 1] > 0;
         if (up && (intake || next_intake)) {
             ct_bar<W>();
-            if (intake) ct_intake_up<W, G>(v, c, sm, sl, freel, cap, row, s, sm.S);
+            if (intake) ct_intake_up<W, G, CAPS>(v, c, sm, sl, freel, cap, row, s, sm.S);
             if (next_intake)
                 for (int k = threadIdx.x; k < TPC_MAX_ROW_HITS / 32; k += W * 32) sm.used[(row + 1) & 1][k] = 0u;
             ct_bar<W>();
@@ -726,5 +727,10 @@ const __grid_constant__ View v, const __grid_constant__ Const c, const int cap_s
         }
     }
 }
+
+// the three tiers
+#define TPC_K5_TIER0 k_construct<kCtWarps, (kCtCapSpill[0] > 0), kCtCapSmem[0]>
+#define TPC_K5_TIER1 k_construct<kCtWarpsWide, false, kCtCapSmem[1]>
+#define TPC_K5_TIER2 k_construct<kCtWarpsWide, true, kCtCapSmem[2]>
 
 }  // namespace tpc

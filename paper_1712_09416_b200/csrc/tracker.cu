@@ -321,9 +321,9 @@ int launch_all(const tpc_tracker* tr, Batch* t, int from = 1) {
     if (from <= 5) {   // K5: one CTA per sector task, up sweep then down sweep (kf_construct.cuh)
         const int tier = t->ct_tier;
         const int grid = std::max(1, std::min(tr->ct_blocks[tier], v.n_tasks));
-        if (tier == 0) k_construct<kCtWarps, (kCtCapSpill[0] > 0)><<<grid, ct_threads(kCtWarps), ct_smem_bytes(tier), st>>>(v, c, kCtCapSmem[tier], kCtCapSpill[tier], tr->ct_spill.p);
-        else if (kCtCapSpill[tier] == 0) k_construct<kCtWarpsWide, false><<<grid, ct_threads(kCtWarpsWide), ct_smem_bytes(tier), st>>>(v, c, kCtCapSmem[tier], kCtCapSpill[tier], tr->ct_spill.p);
-        else k_construct<kCtWarpsWide, true><<<grid, ct_threads(kCtWarpsWide), ct_smem_bytes(tier), st>>>(v, c, kCtCapSmem[tier], kCtCapSpill[tier], tr->ct_spill.p);
+        if (tier == 0) TPC_K5_TIER0<<<grid, ct_threads(kCtWarps), ct_smem_bytes(tier), st>>>(v, c, kCtCapSpill[tier], tr->ct_spill.p);
+        else if (tier == 1) TPC_K5_TIER1<<<grid, ct_threads(kCtWarpsWide), ct_smem_bytes(tier), st>>>(v, c, kCtCapSpill[tier], tr->ct_spill.p);
+        else TPC_K5_TIER2<<<grid, ct_threads(kCtWarpsWide), ct_smem_bytes(tier), st>>>(v, c, kCtCapSpill[tier], tr->ct_spill.p);
         L++;
     }
     mark(4);
@@ -642,17 +642,17 @@ tpc_tracker* tpc_tracker_create_ex(const tpc_geometry* g, float bz, const tpc_pa
         int per_sm = 0;
         size_t most = 0;
         for (int k = 0; k < kCtTiers; k++) most = std::max(most, ct_smem_bytes(k));
-        if (cudaFuncSetAttribute(k_construct<kCtWarps, (kCtCapSpill[0] > 0)>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ct_smem_bytes(0)) != cudaSuccess ||
-            cudaFuncSetAttribute(k_construct<kCtWarpsWide, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)most) != cudaSuccess ||
-            cudaFuncSetAttribute(k_construct<kCtWarpsWide, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)most) != cudaSuccess) {
+        if (cudaFuncSetAttribute(TPC_K5_TIER0, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ct_smem_bytes(0)) != cudaSuccess ||
+            cudaFuncSetAttribute(TPC_K5_TIER1, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)most) != cudaSuccess ||
+            cudaFuncSetAttribute(TPC_K5_TIER2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)most) != cudaSuccess) {
             set_err("k_construct: %zu bytes of shared memory cannot be configured: %s", most, cudaGetErrorString(cudaGetLastError()));
             delete t;
             return nullptr;
         }
         for (int k = 0; k < kCtTiers; k++) {
             const cudaError_t e = k == 0
-                ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_construct<kCtWarps, (kCtCapSpill[0] > 0)>, ct_threads(kCtWarps), ct_smem_bytes(k))
-                : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_construct<kCtWarpsWide, true>, ct_threads(kCtWarpsWide), ct_smem_bytes(k));
+                ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, TPC_K5_TIER0, ct_threads(kCtWarps), ct_smem_bytes(k))
+                : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, TPC_K5_TIER2, ct_threads(kCtWarpsWide), ct_smem_bytes(k));
             if (e != cudaSuccess || per_sm < 1) {
                 set_err("k_construct cannot be configured: %s", cudaGetErrorString(cudaGetLastError()));
                 delete t;
