@@ -322,6 +322,9 @@ __global__ void __launch_bounds__(kNfThreads, TPC_NF_BLOCKS) k_neighbours(const 
         hd = s_hd; cd = s_cd;
     }
     __syncthreads();
+    // The common case -- both neighbour rows staged -- is compiled apart with the shared-memory arrays named directly:
+    // the loads of the hot loops are then LDS with immediate offsets, not generic loads that find their space at run time
+    auto all_hits = [&](const float2* hu, const float2* hd, const uint16_t* cu, const uint16_t* cd) __attribute__((always_inline)) {
     const float x0 = c.row_x[r], x1 = c.row_x[r + D], x2 = c.row_x[r - D];
     const float wyu = c.p.nf_slope_y * fabsf(x1 - x0) + c.p.nf_w0, wzu = c.p.nf_slope_z * fabsf(x1 - x0) + c.p.nf_w0;
     const float wyd = c.p.nf_slope_y * fabsf(x2 - x0) + c.p.nf_w0, wzd = c.p.nf_slope_z * fabsf(x2 - x0) + c.p.nf_w0;
@@ -407,6 +410,9 @@ __global__ void __launch_bounds__(kNfThreads, TPC_NF_BLOCKS) k_neighbours(const 
         v.link_up[h] = ok ? du.x + (bpair >> 16) : -1;
         v.link_dn[h] = ok ? dd.x + (bpair & 0xffff) : -1;
     }
+    };
+    if (hu == s_hu && hd == s_hd) all_hits(s_hu, s_hd, s_cu, s_cd);
+    else all_hits(hu, hd, cu, cd);
 }
 
 // ---------------------------------------------------------------------------------------------------------
