@@ -270,6 +270,41 @@ int tpc_debug_get(tpc_tracker* t, int32_t what, int32_t event, void* buf, size_t
 int tpc_debug_inject(tpc_tracker* t, int32_t what, int32_t event, const void* buf, size_t bytes);
 int tpc_debug_resume(tpc_tracker* t, int32_t from_stage, tpc_event_out* out);
 
+/* ---- a prefix sum for callers that cannot allocate device memory ----
+ * Who this is for.  The tracker sizes its work space with cudaMalloc (at create, and again when a batch outgrows a
+ * pool).  Some users of its kernels have no such freedom: an online reconstruction process in which a framework
+ * reserved the whole GPU memory at start-up and forbids its components to ask the driver for more (a cudaMalloc there
+ * fails, or breaks the framework's accounting); code on a path with a latency bound, where cudaMalloc and cudaFree
+ * are ruled out because they may stall every stream of the device for an unbounded time; a plug-in that is only handed
+ * input and output buffers.  For them the library carries ONE entry point that never allocates: the tracker's
+ * exclusive prefix sum of int32 (the step between "count per (sector, pad row) bin" and "offset of each bin" in K1, K4
+ * and K6; BASELINE.json:5 "per-row cluster sort"), with the few words of scratch memory the kernel needs (a tile
+ * counter and one status word per tile of 2048 elements) taken from an array that is part of the library image.
+ *
+ *   out_dev[i] = in_dev[0] + ... + in_dev[i-1]  for i = 0 .. n   (out_dev[0] = 0, out_dev[n] = the total; int32
+ *   arithmetic, wraps on overflow like the tracker's own).  in_dev [n] and out_dev [n + 1] are DEVICE pointers owned by
+ *   the caller, 4-byte aligned, not overlapping; in_dev may be NULL when n = 0.
+ *
+ * Limit.  n <= TPC_SCAN_STATIC_MAX_N (16 Mi elements; the array is 64 KiB + 256 B, held by every GPU that loads the
+ * library until the process ends).  A larger n returns TPC_ERR_CAPACITY with the reason in tpc_last_error() and
+ * launches nothing; n < 0 or a NULL pointer returns TPC_ERR_ARG.
+ * No allocation.  The call makes no cudaMalloc, cudaFree, cudaMallocHost or any library call that allocates: it
+ * enqueues one memset of the scratch words it is about to use and one kernel on `cuda_stream` (a cudaStream_t; NULL =
+ * the default stream) and returns without waiting; the result is complete when that stream has run them.
+ * First call on a device.  It looks up where the built-in array lives on the current device (cudaGetSymbolAddress,
+ * once per device, kept for later calls; this may make the CUDA runtime load the library's device code).  Make this
+ * first call during set-up, with the device that will be used current, and before any stream capture is begun.
+ * One array for everybody.  All calls on a device -- from any thread, stream or tracker -- share that array, and it
+ * keeps what the previous call left in it.  The call clears the words it needs itself, so calls that follow one
+ * another on one stream (or are ordered by events) are independent; two calls whose kernels can overlap on the GPU
+ * race on the array and give wrong sums -- the caller must keep them apart. */
+#define TPC_SCAN_STATIC_MAX_N (1 << 24)
+int tpc_scan_exclusive_static(const int32_t* in_dev, int64_t n, int32_t* out_dev, void* cuda_stream);
+
+/* The same prefix sum the way the tracker itself runs it, for tests: same kernel, scratch words from cudaMalloc, freed
+ * before the call returns; default stream, synchronous.  n up to 2^31 - 2049.  Not for the hot path. */
+int tpc_debug_scan_exclusive(const int32_t* in_dev, int64_t n, int32_t* out_dev);
+
 #ifdef __cplusplus
 }
 #endif

@@ -6,6 +6,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include <vector>
 
@@ -1196,6 +1197,84 @@ int tpc_debug_resume(tpc_tracker* tr, int32_t from_stage, tpc_event_out* out) {
         o.trk_g_sinphi = mg ? t->o_f[16].p + a : nullptr; o.trk_g_tgl = mg ? t->o_f[17].p + a : nullptr; o.trk_g_qpt = mg ? t->o_f[18].p + a : nullptr;
         o.trk_g_chi2 = mg ? t->o_f[19].p + a : nullptr;
     }
+    return TPC_OK;
+}
+
+// ---- prefix sum without any allocation (include/tpctrack.h "tpc_scan_exclusive_static") ----
+//
+// The tracker's prefix-sum kernel (scan.cuh: one launch, tiles that look back over their predecessors) needs a few
+// words of global memory next to its input and output: a counter that hands out tile numbers and one status word per
+// tile.  The tracker takes them from its cudaMalloc'ed work space.  The variant below takes them from an array that is
+// part of the library image instead, so that a caller who must not (or cannot) allocate can still use the kernel.
+//
+// Size: one 8-byte word per tile of kScanTile = 2048 elements, plus the counter, for up to TPC_SCAN_STATIC_MAX_N
+// elements = 8193 words, rounded up to 8 KiB words = 64 KiB + 256 B.  Every GPU that loads the library holds this much
+// until the process exits.
+namespace {
+constexpr int kScanStaticWords = TPC_SCAN_STATIC_MAX_N / tpc::kScanTile + 1 + 31;
+static_assert(TPC_SCAN_STATIC_MAX_N % tpc::kScanTile == 0, "the limit is a whole number of tiles");
+static __device__ __align__(256) unsigned long long g_scan_static[kScanStaticWords];
+
+// In host code `g_scan_static` is only a handle for the runtime (the host-side shadow of the device variable), NOT a
+// device address: a kernel given `g_scan_static` or `&g_scan_static[0]` from the host would fault, or scribble over
+// host memory on a system where the GPU can reach it.  The device address is asked for once per device, with that
+// device current, and remembered here.
+constexpr int kMaxDevices = 64;
+unsigned long long* g_scan_static_addr[kMaxDevices] = {};
+std::mutex g_scan_static_mutex;
+
+int scan_static_address(unsigned long long** addr) {
+    int dev = -1;
+    CK(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kMaxDevices) { set_err("device ordinal %d is outside [0, %d)", dev, kMaxDevices); return TPC_ERR_ARG; }
+    std::lock_guard<std::mutex> lock(g_scan_static_mutex);
+    if (!g_scan_static_addr[dev]) {
+        void* p = nullptr;
+        CK(cudaGetSymbolAddress(&p, g_scan_static));   // the address on the CURRENT device (= dev)
+        if (!p) { set_err("cudaGetSymbolAddress returned a null address on device %d", dev); return TPC_ERR_CUDA; }
+        g_scan_static_addr[dev] = static_cast<unsigned long long*>(p);
+    }
+    *addr = g_scan_static_addr[dev];
+    return TPC_OK;
+}
+
+int scan_check_args(const int32_t* in_dev, int64_t n, const int32_t* out_dev) {
+    if (n < 0) { set_err("scan: n = %lld is negative", (long long)n); return TPC_ERR_ARG; }
+    if (!out_dev || (n > 0 && !in_dev)) { set_err("scan: null device pointer"); return TPC_ERR_ARG; }
+    return TPC_OK;
+}
+}  // namespace
+
+int tpc_scan_exclusive_static(const int32_t* in_dev, int64_t n, int32_t* out_dev, void* cuda_stream) {
+    int rc = scan_check_args(in_dev, n, out_dev);
+    if (rc != TPC_OK) return rc;
+    if (n > TPC_SCAN_STATIC_MAX_N) {
+        set_err("tpc_scan_exclusive_static: n = %lld is beyond TPC_SCAN_STATIC_MAX_N = %d, the most the built-in scratch "
+                "array serves (nothing was launched; cut the input or use a path that may allocate)",
+                (long long)n, TPC_SCAN_STATIC_MAX_N);
+        return TPC_ERR_CAPACITY;
+    }
+    unsigned long long* scratch = nullptr;
+    rc = scan_static_address(&scratch);   // the first call on a device looks the address up; later calls read it back
+    if (rc != TPC_OK) return rc;
+    // The array still holds the tile counter and the status words of whoever used it last: scan_exclusive clears the
+    // words this call will read (a memset on the same stream, in front of the kernel) -- nothing else must be zero.
+    scan_exclusive(in_dev, out_dev, (int)n, scratch, static_cast<cudaStream_t>(cuda_stream));
+    CK(cudaGetLastError());
+    return TPC_OK;
+}
+
+int tpc_debug_scan_exclusive(const int32_t* in_dev, int64_t n, int32_t* out_dev) {
+    int rc = scan_check_args(in_dev, n, out_dev);
+    if (rc != TPC_OK) return rc;
+    if (n > INT32_MAX - tpc::kScanTile) { set_err("scan: n = %lld is too large", (long long)n); return TPC_ERR_ARG; }
+    unsigned long long* scratch = nullptr;
+    CK(cudaMalloc((void**)&scratch, sizeof(unsigned long long) * ((size_t)n / tpc::kScanTile + 2)));
+    scan_exclusive(in_dev, out_dev, (int)n, scratch, nullptr);
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess) e = cudaStreamSynchronize(nullptr);
+    cudaFree(scratch);
+    if (e != cudaSuccess) { set_err("scan failed: %s", cudaGetErrorString(e)); return TPC_ERR_CUDA; }
     return TPC_OK;
 }
 

@@ -106,6 +106,8 @@ def _load():
     lib.tpc_debug_inject.argtypes = [C.c_void_p, C.c_int32, C.c_int32, C.c_void_p, C.c_size_t]
     lib.tpc_debug_resume.argtypes = [C.c_void_p, C.c_int32, C.POINTER(tpc_event_out)]
     lib.tpc_measure_fp32_peak.argtypes = [C.POINTER(C.c_float), C.POINTER(C.c_float)]
+    lib.tpc_scan_exclusive_static.argtypes = [C.c_void_p, C.c_int64, C.c_void_p, C.c_void_p]
+    lib.tpc_debug_scan_exclusive.argtypes = [C.c_void_p, C.c_int64, C.c_void_p]
     return lib
 
 
@@ -115,7 +117,8 @@ EXPORTS = ("tpc_default_params", "tpc_tracker_create", "tpc_tracker_create_ex", 
            "tpc_tracker_set_group_events",
            "tpc_track_event", "tpc_track_events", "tpc_submit_events", "tpc_wait_events", "tpc_tracker_destroy", "tpc_status_string", "tpc_last_error",
            "tpc_get_counters", "tpc_tracker_set_profiling", "tpc_get_stage_ms", "tpc_debug_size", "tpc_debug_get",
-           "tpc_debug_inject", "tpc_debug_resume", "tpc_measure_fp32_peak")
+           "tpc_debug_inject", "tpc_debug_resume", "tpc_measure_fp32_peak", "tpc_scan_exclusive_static",
+           "tpc_debug_scan_exclusive")
 
 
 def tpc_status_string(status: int) -> str:
@@ -131,6 +134,24 @@ def tpc_measure_fp32_peak() -> tuple:
     a, b = C.c_float(0), C.c_float(0)
     _check(lib.tpc_measure_fp32_peak(C.byref(a), C.byref(b)))
     return float(a.value), float(b.value)
+
+
+SCAN_STATIC_MAX_N = 1 << 24   # TPC_SCAN_STATIC_MAX_N
+
+
+def tpc_scan_exclusive_static(in_dev, n: int, out_dev, cuda_stream=None) -> None:
+    """Exclusive prefix sum of ``n`` int32 values for callers that may not allocate device memory (a framework owns
+    all of it, or cudaMalloc's device-wide stall is not acceptable where they run): the kernel's scratch words live in
+    an array inside the library, so only the caller's ``in_dev`` [n] and ``out_dev`` [n + 1] (device pointers, as
+    integers) are touched.  Enqueued on ``cuda_stream`` (integer handle, None = default stream); not waited for.
+    ``n`` beyond ``SCAN_STATIC_MAX_N`` raises TpcError (TPC_ERR_CAPACITY).  All calls share the one array: do not let
+    two of them overlap on the GPU.  See include/tpctrack.h."""
+    _check(lib.tpc_scan_exclusive_static(in_dev, n, out_dev, cuda_stream))
+
+
+def tpc_debug_scan_exclusive(in_dev, n: int, out_dev) -> None:
+    """The same prefix sum with cudaMalloc'ed scratch, as the tracker runs it (tests only; synchronous)."""
+    _check(lib.tpc_debug_scan_exclusive(in_dev, n, out_dev))
 
 
 def tpc_default_params() -> tpc_params:
