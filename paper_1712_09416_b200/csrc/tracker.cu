@@ -104,10 +104,17 @@ struct Batch {
     Buf<int32_t> dn_count, dn_start, dn_fill, tl_cnt;
     int sel_C = 1;                           // selector chunks per sector task
     int ct_tier = 0;                         // K5 slot tier used by this group's last launch
+    Buf<float> ct_spill;                     // tier 2: state slots in global memory, per CTA of THIS group's launch (groups
+                                             // and tickets run on streams of their own: their K5 launches can be resident together)
     // the launch sequence K1..K6 (+ refit, merge) of this group as a CUDA graph, replayed while nothing it bakes in changes
-    struct GraphKey { View v; int tier, maxn, n_events; int64_t S_cap; const float* spill; } gkey;
-    cudaGraphExec_t gexec = nullptr;
-    int64_t graph_launches = 0;              // kernels in the graph
+    // Two graphs are kept: with device inputs a ticket's output arrays alternate between two sets (tpc_wait_events swaps
+    // them with the ticket's), so consecutive runs of one shape need two graphs, not a new capture each time.
+    struct GraphKey { View v; int tier, maxn, n_events; int64_t S_cap; const float* spill; };
+    static constexpr int kGraphs = 2;
+    GraphKey gkey[kGraphs];
+    cudaGraphExec_t gexec[kGraphs] = {};
+    int64_t graph_launches[kGraphs] = {};    // kernels in each graph
+    int graph_victim = 0;                    // the graph that a new shape replaces
     Buf<uint32_t> owner;
     Buf<EventSrc> ev_src;
     Buf<unsigned long long> cnt, kf_cursor;
@@ -136,10 +143,10 @@ struct Batch {
         for (auto& b : o_i) b.release();
         slot.release(); cells.release(); desc.release(); owner.release(); ev_src.release();
         seed_rec.release(); tl_up.release(); dn_rec.release(); kf_park.release(); dn_count.release(); dn_start.release(); dn_fill.release(); tl_cnt.release(); o_hit_yz.release(); o_hit_row.release(); trk_hit0.release(); trk_rows.release(); trk_task.release(); mg_next.release(); mg_prev.release(); mg_list.release();
-        cnt.release(); kf_cursor.release(); h_ev_src.release(); h_sec_off.release(); h_ev_off.release(); h_cnt.release(); h_nseeds.release();
+        cnt.release(); kf_cursor.release(); ct_spill.release(); h_ev_src.release(); h_sec_off.release(); h_ev_off.release(); h_cnt.release(); h_nseeds.release();
         for (auto& e : evt) if (e) { cudaEventDestroy(e); e = nullptr; }
         if (kernels_done) { cudaEventDestroy(kernels_done); kernels_done = nullptr; }
-        if (gexec) { cudaGraphExecDestroy(gexec); gexec = nullptr; }
+        for (auto& g : gexec) if (g) { cudaGraphExecDestroy(g); g = nullptr; }
     }
 };
 
@@ -151,7 +158,6 @@ struct tpc_tracker {
     int sm_count = 148;
     int ct_tier = 0;                         // K5: state-slot tier (kf_construct.cuh); moves up on kErrSlotCapacity
     int ct_blocks[kCtTiers] = {296, 148, 148};   // resident CTAs of the constructor in each tier
-    Buf<float> ct_spill;                     // tier 2: state slots in global memory, per CTA
     int rf_blocks = 148;                     // resident CTAs of the refit
     int group_events = 0;                    // host-input batches: events per group (0 = automatic)
     std::vector<Batch*> slots;               // groups in flight; slots[0] always exists
@@ -211,7 +217,6 @@ struct tpc_tracker {
         h_o_hit.release();
         for (auto& b : h_o_i) b.release();
         for (auto& b : h_o_f) b.release();
-        ct_spill.release();
     }
 };
 
@@ -322,9 +327,9 @@ int launch_all(const tpc_tracker* tr, Batch* t, int from = 1) {
     if (from <= 5) {   // K5: one CTA per sector task, up sweep then down sweep (kf_construct.cuh)
         const int tier = t->ct_tier;
         const int grid = std::max(1, std::min(tr->ct_blocks[tier], v.n_tasks));
-        if (tier == 0) TPC_K5_TIER0<<<grid, ct_threads(kCtWarps), ct_smem_bytes(tier), st>>>(v, c, kCtCapSpill[tier], tr->ct_spill.p);
-        else if (tier == 1) TPC_K5_TIER1<<<grid, ct_threads(kCtWarpsWide), ct_smem_bytes(tier), st>>>(v, c, kCtCapSpill[tier], tr->ct_spill.p);
-        else TPC_K5_TIER2<<<grid, ct_threads(kCtWarpsWide), ct_smem_bytes(tier), st>>>(v, c, kCtCapSpill[tier], tr->ct_spill.p);
+        if (tier == 0) TPC_K5_TIER0<<<grid, ct_threads(kCtWarps), ct_smem_bytes(tier), st>>>(v, c, kCtCapSpill[tier], t->ct_spill.p);
+        else if (tier == 1) TPC_K5_TIER1<<<grid, ct_threads(kCtWarpsWide), ct_smem_bytes(tier), st>>>(v, c, kCtCapSpill[tier], t->ct_spill.p);
+        else TPC_K5_TIER2<<<grid, ct_threads(kCtWarpsWide), ct_smem_bytes(tier), st>>>(v, c, kCtCapSpill[tier], t->ct_spill.p);
         L++;
     }
     mark(4);
@@ -362,28 +367,36 @@ int launch_all(const tpc_tracker* tr, Batch* t, int from = 1) {
 // The same launches through a CUDA graph: captured once per shape of the group (every pointer, size and grid the
 // launches bake in is part of the key), replayed afterwards -- one submission instead of ~25 (15 kernels, 10 memsets).
 int launch_graphed(const tpc_tracker* tr, Batch* t) {
+    // the key is built and compared as raw bytes: cleared first, members copied with memcpy (padding stays zero; the View
+    // of a Batch was cleared at construction and is only ever assigned member by member)
     Batch::GraphKey key;
     memset(&key, 0, sizeof key);
-    key.v = t->v; key.tier = t->ct_tier; key.n_events = t->n_events; key.S_cap = t->S_cap; key.spill = tr->ct_spill.p;
+    memcpy(&key.v, &t->v, sizeof(View));
+    key.tier = t->ct_tier; key.n_events = t->n_events; key.S_cap = t->S_cap; key.spill = t->ct_spill.p;
     for (int e = 0; e < t->n_events; e++) key.maxn = std::max(key.maxn, t->ev_n[e]);
-    if (!t->gexec || memcmp(&key, &t->gkey, sizeof key) != 0) {
-        if (t->gexec) { cudaGraphExecDestroy(t->gexec); t->gexec = nullptr; }
+    int k = -1;
+    for (int i = 0; i < Batch::kGraphs; i++)
+        if (t->gexec[i] && memcmp(&key, &t->gkey[i], sizeof key) == 0) k = i;
+    if (k < 0) {
+        k = t->graph_victim;
+        t->graph_victim = (k + 1) % Batch::kGraphs;
+        if (t->gexec[k]) { cudaGraphExecDestroy(t->gexec[k]); t->gexec[k] = nullptr; }
         cudaGraph_t g = nullptr;
         CK(cudaStreamBeginCapture(t->stream, cudaStreamCaptureModeThreadLocal));
         const int64_t before = t->counters.n_kernel_launches;
         const int rc = launch_all(tr, t);
         const cudaError_t e = cudaStreamEndCapture(t->stream, &g);
-        t->graph_launches = t->counters.n_kernel_launches - before;
+        t->graph_launches[k] = t->counters.n_kernel_launches - before;
         t->counters.n_kernel_launches = before;
         if (rc != TPC_OK) { if (g) cudaGraphDestroy(g); return rc; }
         if (e != cudaSuccess || !g) { set_err("graph capture failed: %s", cudaGetErrorString(e)); return TPC_ERR_CUDA; }
-        const cudaError_t ei = cudaGraphInstantiate(&t->gexec, g, 0);
+        const cudaError_t ei = cudaGraphInstantiate(&t->gexec[k], g, 0);
         cudaGraphDestroy(g);
-        if (ei != cudaSuccess) { t->gexec = nullptr; set_err("graph instantiation failed: %s", cudaGetErrorString(ei)); return TPC_ERR_CUDA; }
-        t->gkey = key;
+        if (ei != cudaSuccess) { t->gexec[k] = nullptr; set_err("graph instantiation failed: %s", cudaGetErrorString(ei)); return TPC_ERR_CUDA; }
+        memcpy(&t->gkey[k], &key, sizeof key);
     }
-    CK(cudaGraphLaunch(t->gexec, t->stream));
-    t->counters.n_kernel_launches += t->graph_launches;
+    CK(cudaGraphLaunch(t->gexec[k], t->stream));
+    t->counters.n_kernel_launches += t->graph_launches[k];
     return TPC_OK;
 }
 
@@ -471,8 +484,7 @@ int batch_begin(const tpc_tracker* tr, Batch* t, int first_event, int n, const t
     // central event: K5 1.46 ms against 2.06 ms with the two-CTAs-per-SM tier; on 16 events 5.83 against 4.72 ms)
     if (n * ns <= tr->sm_count) t->ct_tier = std::max(t->ct_tier, 1);
     if (kCtCapSpill[t->ct_tier] > 0) {   // slots in global memory for every resident CTA (allocated once, on the way up)
-        tpc_tracker* w = const_cast<tpc_tracker*>(tr);
-        if ((rc = w->ct_spill.reserve((size_t)tr->ct_blocks[t->ct_tier] * kCtWords * kCtCapSpill[t->ct_tier])) != TPC_OK) return rc;
+        if ((rc = t->ct_spill.reserve((size_t)tr->ct_blocks[t->ct_tier] * kCtWords * kCtCapSpill[t->ct_tier])) != TPC_OK) return rc;
     }
     t->n_events = n; t->N = N;
     if (tr->profiling)
@@ -1054,23 +1066,27 @@ int tpc_measure_fp32_peak(float* fused_tflops, float* unfused_tflops) {
     CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
     const int blocks = sms * 8;                      // 2048 threads per SM: every scheduler has 16 warps to pick from
     float* d = nullptr;
-    CK(cudaMalloc((void**)&d, 4));
-    cudaEvent_t e0, e1;
-    CK(cudaEventCreate(&e0)); CK(cudaEventCreate(&e1));
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
     float best[2] = {0.f, 0.f};
-    for (int fused = 0; fused < 2; fused++)
-        for (int rep = 0; rep < 6; rep++) {          // first launches warm up; the best of the rest counts
-            CK(cudaEventRecord(e0, 0));
+    cudaError_t e = cudaMalloc((void**)&d, 4);
+    if (e == cudaSuccess) e = cudaEventCreate(&e0);
+    if (e == cudaSuccess) e = cudaEventCreate(&e1);
+    for (int fused = 0; fused < 2 && e == cudaSuccess; fused++)
+        for (int rep = 0; rep < 6 && e == cudaSuccess; rep++) {   // first launches warm up; the best of the rest counts
+            float ms = 0.f;
+            e = cudaEventRecord(e0, 0);
             if (fused) k_fp32_peak<true><<<blocks, kPeakThreads>>>(d, 1.0000001f, 1.0e-7f);
             else k_fp32_peak<false><<<blocks, kPeakThreads>>>(d, 1.0000001f, 1.0e-7f);
-            CK(cudaEventRecord(e1, 0));
-            CK(cudaEventSynchronize(e1));
-            float ms = 0.f;
-            CK(cudaEventElapsedTime(&ms, e0, e1));
-            if (rep >= 2 && ms > 0.f) best[fused] = std::max(best[fused], (float)(fp32_peak_flops_per_launch(blocks) / (ms * 1e-3) / 1e12));
+            if (e == cudaSuccess) e = cudaEventRecord(e1, 0);
+            if (e == cudaSuccess) e = cudaEventSynchronize(e1);
+            if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, e0, e1);
+            if (e == cudaSuccess && rep >= 2 && ms > 0.f) best[fused] = std::max(best[fused], (float)(fp32_peak_flops_per_launch(blocks) / (ms * 1e-3) / 1e12));
         }
-    cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d);
-    CK(cudaGetLastError());
+    if (e == cudaSuccess) e = cudaGetLastError();
+    if (e0) cudaEventDestroy(e0);      // the buffer and the events go on every path, failed or not
+    if (e1) cudaEventDestroy(e1);
+    if (d) cudaFree(d);
+    if (e != cudaSuccess) { set_err("FP32 peak measurement failed: %s", cudaGetErrorString(e)); return TPC_ERR_CUDA; }
     *fused_tflops = best[1]; *unfused_tflops = best[0];
     return TPC_OK;
 }
@@ -1092,6 +1108,8 @@ int tpc_debug_inject(tpc_tracker* tr, int32_t what, int32_t event, const void* b
         if (sorig[k] < 0 || sorig[k] >= n) { set_err("inject: inconsistent work space"); return TPC_ERR_CUDA; }
         inv[sorig[k]] = g0 + k;   // caller's index -> sorted (batch-global) index
     }
+    for (int i = 0; i < n; i++)   // the sorted order must name every cluster once, or inv[] has holes
+        if (inv[i] < 0) { set_err("inject: the work space's sorted order is not a permutation of the event's clusters"); return TPC_ERR_CUDA; }
     const int32_t* ib = (const int32_t*)buf;
     switch (what) {
         case TPC_DBG_LINK_UP: case TPC_DBG_LINK_DN: case TPC_DBG_CLINK_UP: case TPC_DBG_CLINK_DN: {
