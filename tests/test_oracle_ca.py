@@ -99,6 +99,29 @@ def test_coincident_hits_tie_goes_to_lowest_index(oracle_mod, gen_mod):
     assert res.clink_up[1] == -1 or res.clink_dn[res.clink_up[1]] == 1
 
 
+@pytest.mark.parametrize("precision", ["double", "float"])
+def test_deviation_equal_to_d_max_is_accepted(oracle_mod, gen_mod, precision):
+    """"If D_best <= D_max" -- the bound itself is accepted.  Three hits on rows 10, 11, 12 at
+    z = 50: the outer two at y = 0, the middle one at y0.  The interpolated point is (0, 50) whatever the row pitch, so
+    D = y0^2 exactly: y0 = 0.5 gives D = 0.25 = nf_dmax (exact in float32 and double) -> the link is made; the next
+    float32 above 0.5 gives D > 0.25 -> no link.  Kills the mutant `D_best < D_max` of oracle/tpc_oracle.cpp
+    `neighbours`."""
+    rx = gen_mod.row_x()
+    p = oracle_mod.default_params()
+    assert p.nf_dmax == 0.25 and p.nf_slope_y * (rx[11] - rx[10]) + p.nf_w0 > 0.6     # the windows do not decide here
+    row = np.array([10, 11, 12], np.int32)
+    z = np.full(3, 50.0, np.float32)
+    for y0, linked in ((np.float32(0.5), True), (np.nextafter(np.float32(0.5), np.float32(1)), False),
+                       (np.float32(-0.5), True), (np.nextafter(np.float32(-0.5), np.float32(-1)), False)):
+        y = np.array([0.0, y0, 0.0], np.float32)
+        ev = gen_mod.Event(1, np.array([0, 3], np.int32), rx[row].astype(np.float32), y, z, row, np.zeros(3, np.int32),
+                           np.zeros((1, 8)))
+        res = oracle_mod.track_event(make_geometry(oracle_mod, gen_mod, ev), ev.sector_offset, y, z, row,
+                                     precision=precision, stop_after=4)
+        assert (res.link_up[1], res.link_dn[1]) == ((2, 0) if linked else (-1, -1)), (float(y0), precision)
+        assert res.link_up[0] == res.link_up[2] == -1
+
+
 def test_mirror_symmetry(oracle_mod, gen_mod):
     """D(h; u, d) is invariant under y -> -y, so the links of the mirrored sector are the same."""
     ev = gen_mod.tiny_sector(n_tracks=20, seed=11, noise_frac=0.5)

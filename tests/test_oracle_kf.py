@@ -81,6 +81,26 @@ def test_transport_fails_beyond_sin_max(oracle_mod):
     assert ok
 
 
+@pytest.mark.parametrize("precision", ["double", "float"])
+def test_transport_fails_when_it_starts_beyond_sin_max(oracle_mod, precision):
+    """DESIGN.md reading R9: the step fails when |sin phi| is beyond s_max at EITHER end.  Here only the START is
+    beyond it (|s| = 0.96 > 0.95; an update can leave the fit there) while the step leads back inside
+    (|s1| = 0.940): fit and covariance must stay untouched.  Kills the mutant of oracle/tpc_oracle.cpp `transport` that
+    drops its first guard (`|s| > s_max`), which the case above (only |s1| beyond the limit) cannot see."""
+    g = _geom(oracle_mod)
+    cov = np.diag([0.01, 0.02, 0.003, 0.004, 0.5])
+    for sign in (1.0, -1.0):
+        st = np.array([1.0, -2.0, sign * 0.96, 0.3, sign * 10.0])   # kappa = -+0.015: |sin phi| falls by 0.02 over 4/3 cm
+        dx = 4.0 / 3.0
+        assert 0.93 < abs(st[2] + KB * st[4] * dx) < 0.945          # the far end is inside the limit
+        ok, new, cn = oracle_mod.transport(g, 100.0, 100.0 + dx, st, cov, precision=precision)
+        assert not ok and np.array_equal(new, st) and np.array_equal(cn, cov)
+        # the same step from just inside the limit is taken (the guard is |s| > s_max, not the direction of the step)
+        st[2] = sign * 0.949
+        ok, new, _ = oracle_mod.transport(g, 100.0, 100.0 + dx, st, cov, precision=precision)
+        assert ok and abs(new[2] - (st[2] + KB * st[4] * dx)) < 1e-6 and abs(new[2]) < 0.93
+
+
 def test_jacobian_equals_central_differences_of_exact_helix(oracle_mod):
     """C' = F C F^T with C = e_k e_k^T gives column k of F in column k of C' (F_kk = 1)."""
     g = _geom(oracle_mod)

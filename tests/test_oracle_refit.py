@@ -76,6 +76,9 @@ def test_refit_straight_line_limit_equals_least_squares(oracle_mod, gen_mod):
         assert abs(res.trk_sinphi[0] - s_ls) < 5e-6 and abs(res.trk_tgl[0] - t_ls) < 1e-5
 
 
+outer_of = {}   # filled by _compose_refit: what the up pass of the last composed track handed over
+
+
 def _compose_refit(oracle, g, rx, ev, hits):
     """O8 written out with the pinned primitives: returns (params[5], chi2, n_fit, ref_row)."""
     p = oracle.default_params()
@@ -89,6 +92,7 @@ def _compose_refit(oracle, g, rx, ev, hits):
     dl = math.sqrt(dx * dx + dy * dy)
     st = np.array([y[h0], z[h0], dy / dl, dz / dl, 0.0]); cv = prior.copy(); chi2 = 0.0
     snap = (st.copy(), chi2, 1)
+    outer_of.clear()
     on_row = {r: h for r, h in zip(rows, hits)}
     k_top_row = rows[0]
     xc = float(rx[rows[0]])
@@ -100,6 +104,8 @@ def _compose_refit(oracle, g, rx, ev, hits):
         if r in on_row:
             st, cv, chi2 = oracle.update(g, y[on_row[r]], z[on_row[r]], st, cv, chi2)
             snap = (st.copy(), chi2, 0); k_top_row = r
+    # the refit's OUTER state: the up pass right after its last update, not where the pass ended
+    outer_of.update(state=snap[0].copy(), row=k_top_row, running=st.copy(), ended_early=k_top_row < rows[-1])
     ht = on_row[k_top_row]
     st = np.array([y[ht], z[ht], snap[0][2], snap[0][3], snap[0][4]]); cv = prior.copy(); chi2 = 0.0
     out = (st.copy(), 0.0, 1, k_top_row)
@@ -138,8 +144,42 @@ def test_refit_equals_composition_of_pinned_primitives(oracle_mod, gen_mod):
         assert abs(res.trk_chi2[i] - chi2) <= 1e-12 * max(1.0, chi2)
         assert res.trk_ndf[i] == 2 * n - 5 and res.trk_first_row[i] == ref_row
         assert res.trk_x[i] == rx[ref_row]
+        assert res.trk_row_out[i] == outer_of["row"] == rows[-1] and res.trk_out[i, 0] == rx[outer_of["row"]]
+        assert np.allclose(res.trk_out[i, 1:], outer_of["state"], rtol=1e-12, atol=1e-14)
     assert holes > 20                      # rows without a measurement inside the tracks were exercised
     assert np.any(base.trk_n_hits != (base.trk_ndf + 5) // 2)   # the selection did take hits from some tracklets
+
+
+def test_refit_outer_state_is_the_last_snapshot_when_the_up_pass_ends_early(oracle_mod, gen_mod):
+    """pT 0.08-0.16 GeV curlers: the refit's up pass reaches |sin phi| = s_max before the track's last hit, some rows
+    AFTER its last update (rows without a hit were crossed in between).  The outer state (trk_out, trk_row_out, the
+    input of the cross-sector match O9) is then the snapshot taken at the last update, at that hit's row -- not the
+    running fit at the row where the pass ended.  Composition of the pinned transport / update primitives, as in the
+    test above.  Kills the mutant of oracle/tpc_oracle.cpp `refit` that copies the running fit `f` into `out`."""
+    r = gen_mod.Recipe("curlers", n_sectors=36, n_primaries=1500, pt_mode=0, pt_a=0.08, pt_b=0.16, sigma=0.06,
+                       noise_frac=0.05, config_id=61)
+    full = gen_mod.generate(r)
+    # 30 % of the clusters are dropped at random (seeded): the tracks get holes, so that a pass which ends between two
+    # hits has often crossed rows since its last update
+    keep = np.random.default_rng(5).random(full.row.size) < 0.7
+    so = np.concatenate([[0], np.cumsum([int(keep[a:b].sum()) for a, b in zip(full.sector_offset[:-1],
+                                                                               full.sector_offset[1:])])])
+    ev = gen_mod.Event(36, so.astype(np.int32), full.x[keep], full.y[keep], full.z[keep], full.row[keep],
+                       full.label[keep], full.tracks, sigma=full.sigma)
+    g = _geom(oracle_mod, gen_mod, ev.sigma, ev.bz, n_sectors=36)
+    rx = gen_mod.row_x().astype(np.float32)
+    res = oracle_mod.track_event(g, ev.sector_offset, ev.y, ev.z, ev.row, precision="double",
+                                 params=_params(oracle_mod, 1))
+    early = moved = 0
+    last_row = np.array([ev.row[res.hit_idx[res.trk_first_hit[i] + res.trk_n_hits[i] - 1]] for i in range(res.n_tracks)])
+    for i in sorted(set(range(150)) | set(np.nonzero(res.trk_row_out < last_row)[0].tolist())):
+        hits = [int(h) for h in res.hit_idx[res.trk_first_hit[i]:res.trk_first_hit[i] + res.trk_n_hits[i]]]
+        _compose_refit(oracle_mod, g, rx, ev, hits)
+        assert res.trk_row_out[i] == outer_of["row"] and res.trk_out[i, 0] == rx[outer_of["row"]], i
+        assert np.allclose(res.trk_out[i, 1:], outer_of["state"], rtol=1e-12, atol=1e-14), (i, res.trk_out[i], outer_of)
+        early += outer_of["ended_early"]
+        moved += bool(outer_of["ended_early"] and np.abs(outer_of["running"][:3] - outer_of["state"][:3]).max() > 1e-3)
+    assert early >= 8 and moved >= 3, (res.n_tracks, early, moved)   # the case under test did occur
 
 
 @pytest.mark.parametrize("precision", ["double", "float"])
