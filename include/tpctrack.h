@@ -221,7 +221,7 @@ int tpc_get_counters(const tpc_tracker* t, tpc_counters* c);
 
 /* Per-stage device times of the last call, measured with CUDA events on the tracker's stream (off by default:
  * the events cost a few microseconds).  Stages: 0 = K1 bucket + grid sort, 1 = K2 neighbour finder,
- * 2 = K3 cleaner + K4 start hits, 3 = K5 tracklet constructor (up sweep, bucket pass, down sweep),
+ * 2 = K3 cleaner + K4 start hits, 3 = K5 tracklet constructor (one launch: up and down sweep of every sector task),
  * 4 = K6 selector + output, 5 = refit of the output tracks (0 when tpc_params.refit is 0). */
 #define TPC_N_STAGES 6
 int tpc_tracker_set_profiling(tpc_tracker* t, int32_t on);

@@ -124,7 +124,10 @@ __device__ __forceinline__ bool mbar_try_wait_hint(unsigned long long* b, uint32
                  : "=r"(ok) : "r"(smem_u32(b)), "r"(parity), "r"(ns) : "memory");
     return ok != 0;
 }
-// bounded wait: a lost signal ends the kernel with kErrHang instead of hanging the device
+// bounded wait: a lost signal ends the kernel with kErrHang instead of hanging the device.  Every warp of the CTA waits
+// for the same signals in the same order (one per row step, the barriers of a row step come after its wait), so a
+// signal that never comes is missed by ALL warps at the same step: the first to run out of patience raises the flag,
+// the others see it within 64 polls, and all leave the sweep loop together -- none is left behind at a ct_bar.
 __device__ __forceinline__ bool mbar_wait(unsigned long long* b, uint32_t parity, volatile int32_t* abort) {
     if (mbar_try_wait(b, parity)) return true;
     for (unsigned n = 0; n < (1u << 17); n++) {   // a waiting warp issues nothing until the phase completes or the hint runs out
@@ -221,7 +224,7 @@ __device__ __forceinline__ void ct_next_task(const View& v, const Const& c, CtSm
     for (int o = 16; o > 0; o >>= 1) f = min(f, __shfl_xor_sync(kFull, f, o));
     if (lane == 0) {
         sm.first = f;
-        if (!mbar_wait(&sm.tbar, tphase, &sm.abort)) sm.first = nr;   // (the flag is up: every warp leaves at its next wait)
+        if (!mbar_wait(&sm.tbar, tphase, &sm.abort)) sm.first = nr;   // (the flag is up: every warp leaves behind the next barrier)
     }
     tphase ^= 1u;
     __syncwarp();
@@ -520,7 +523,7 @@ const __grid_constant__ View v, const __grid_constant__ Const c, const int cap_g
             if (warp == 0) ct_next_task(v, c, sm, freel, cap, tphase);
             ct_bar<W>();
             const int task = *(volatile int32_t*)&sm.task;
-            if (task >= v.n_tasks) break;
+            if (task >= v.n_tasks || *abort) break;               // (the flag is read behind a barrier: the same in every warp)
             tb = task * nr;
             row = *(volatile int32_t*)&sm.first; last = nr - 1;
             if (row > last) continue;                            // no start hit in this sector
@@ -718,6 +721,7 @@ const __grid_constant__ View v, const __grid_constant__ Const c, const int cap_g
     }
     __syncwarp();
     if (lane == 0) {
+        if (warp == 0 && *abort) atomicOr((unsigned int*)&v.cnt[CNT_ERR], kErrHang);   // the host reports it (TPC_ERR_CUDA)
         const uint32_t vs = sm.n_visits[warp], us = sm.n_updates[warp];
         if (vs) { atomicAdd(&v.cnt[CNT_ROW_VISITS], (unsigned long long)vs); atomicAdd(&v.cnt[CNT_UPDATES], (unsigned long long)us); }
         __threadfence_block();
