@@ -248,6 +248,9 @@ def main():
     ap.add_argument("--no-seed-dedup", action="store_true", help="fit every start hit (round-1 behaviour)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--group-events", type=int, default=0,
+                    help="measurement of event waves (SURVEY.md 8(f).3): cut the device-resident batch into groups of this "
+                         "many events on separate streams (at most four groups) and print only the step time")
     ap.add_argument("--link-step", type=int, default=1, choices=[1, 2], help="neighbour rows r +- step (SURVEY.md 8(f).4)")
     ap.add_argument("--merge", action="store_true", help="also link segments across sector borders (O9, SURVEY.md 8(f).2; implies --refit)")
     ap.add_argument("--refit", action="store_true", help="also refit the output tracks (O8, SURVEY.md 8(f).1; not part of the headline path)")
@@ -286,7 +289,9 @@ def main():
                           params=params, max_events=len(evs), max_clusters=n_total)
     stream = torch.cuda.Stream()
     trk.set_stream(stream.cuda_stream)
-    trk.tpc_tracker_set_profiling(True)
+    trk.tpc_tracker_set_profiling(not args.group_events)   # (per-stage events are per group: off in the wave measurement)
+    if args.group_events:
+        trk.tpc_tracker_set_group_events(args.group_events)
 
     dev_in = [dict(sector_offset=ev.sector_offset, y=torch.from_numpy(ev.y).cuda(), z=torch.from_numpy(ev.z).cuda(),
                    row=torch.from_numpy(ev.row).cuda()) for ev in evs]
@@ -326,8 +331,43 @@ def main():
     sampler = ClockSampler(local_rank)
     sampler.start()
     ms, stage_ms, outs, launches = timed(dev_in, args.steps, True)
-    clocks = sampler.stop()
     counters = trk.tpc_get_counters()
+    # Second pass, the one `value` comes from when the batch is more than one wave of the constructor's CTAs: the same
+    # batch cut into TWO groups of events on two streams (tpc_tracker_set_group_events, a public knob; results do not
+    # depend on it).  Each group's K5 is then a single wave of sector tasks and the groups' kernels overlap: measured
+    # 6.68 against 7.21 ms per step on 16 central events (profiles/r3_waves.md).  Per-stage CUDA events are per group and
+    # would overlap, so the stage times, the roofline and the counters stay those of the one-group pass above.
+    two_groups = None
+    if not args.group_events and len(evs) >= 2 and len(evs) * evs[0].n_sectors > 2 * 148:
+        trk.tpc_tracker_set_profiling(False)
+        trk.tpc_tracker_set_group_events((len(evs) + 1) // 2)
+        for _ in range(args.warmup):
+            trk.tpc_track_events(dev_in)
+        ms2, _, outs2, launches2 = timed(dev_in, args.steps, False)
+        assert [o.n_tracks for o in outs2] == [o.n_tracks for o in outs]
+        assert sum(o.n_track_hits for o in outs2) == sum(o.n_track_hits for o in outs)
+        two_groups = {"one_group_profiled_ms_per_step": ms / args.steps, "one_group_gpu_launches": int(launches),
+                      "groups": 2, "events_per_group": (len(evs) + 1) // 2,
+                      "note": "value / ms_per_step / gpu_launches: the batch as two groups of events on two streams, "
+                              "CUDA-graph replay, no per-stage events; stages / roofline / counters: a separate pass of the "
+                              "same K steps as one group with per-stage CUDA events (its ms_per_step given here)"}
+        ms, outs, launches = ms2, outs2, launches2
+        trk.tpc_tracker_set_group_events(0)
+        trk.tpc_tracker_set_profiling(True)
+    clocks = sampler.stop()
+    if args.group_events:      # wave measurement: the step time of the same batch run as groups; nothing else is reported
+        if rank == 0:
+            print(json.dumps({"metric": METRIC, "value": aggregate_value(len(evs), args.steps, ms, world), "unit": UNIT,
+                              "ms_per_step": ms / args.steps, "steps": args.steps, "warmup": args.warmup, "n_gpus": world,
+                              "config": {"workload": args.workload, "events_per_step": len(evs),
+                                         "group_events": args.group_events,
+                                         "note": "device-resident batch cut into groups of events on separate streams; "
+                                                 "synchronous tpc_track_events calls, timed around the calls"},
+                              "gpu_launches": int(launches), "clocks": clocks}))
+        trk.close()
+        if world > 1:
+            dist.destroy_process_group()
+        return
     n_tracks = sum(o.n_tracks for o in outs)
     n_hits = sum(o.n_track_hits for o in outs)
 
@@ -447,6 +487,9 @@ def main():
             "roofline": roofline, "stages": stages, "cpu_baseline": cpu, "e2e": e2e,
             "gpu_launches": int(launches), "clocks": clocks, "counters": counters,
         }
+        if two_groups:
+            line["passes"] = two_groups
+            line["config"]["event_groups"] = "2 groups of %d events on two streams (tpc_tracker_set_group_events)" % two_groups["events_per_group"]
         print(json.dumps(line))
     trk.close()
     if world > 1:
