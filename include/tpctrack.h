@@ -33,13 +33,15 @@ extern "C" {
 #define TPC_ERR_CUDA (-4)      /* a CUDA call failed; tpc_last_error() has the text */
 
 #define TPC_MAX_ROWS 255
-#define TPC_MAX_ROW_HITS 2048  /* clusters per (sector, pad row) */
+#define TPC_MAX_ROW_HITS 2048  /* clusters per (sector, pad row); a fuller row makes the call fail with TPC_ERR_CAPACITY
+                                * (row-local hit numbers are 16-bit and the row sort works in shared memory) */
 
 /* Geometry of the detector (copied at create; host pointers).  Units: cm, Tesla, GeV/c.
  * Sector-local frame: x along the sector axis (a cluster of pad row r sits at x = row_x[r] exactly), y across,
  * z along the drift (signed: C-side sectors have z < 0).  BASELINE.json:7: 159 rows, 20 degree wedges. */
 typedef struct {
-    int32_t n_sectors;         /* 36 (or 1): the number of independent sector tasks per event */
+    int32_t n_sectors;         /* 36 (or 1): the number of independent sector tasks per event; 1..64 (more is
+                                * TPC_ERR_GEOMETRY: the first kernels keep an event's sector offsets in shared memory) */
     int32_t n_rows;            /* pad rows per sector, 3..TPC_MAX_ROWS */
     const float* row_x;        /* [n_rows] host, strictly increasing */
     float tan_half_angle;      /* tan(10 deg): the wedge is |y| <= row_x * tan_half_angle */
